@@ -1,0 +1,120 @@
+/*
+ * dwf.h -- C ABI of libdwf: the Domain Wall Fermion hopping term Dhop on one B200.
+ *
+ * The operation (BASELINE.json north_star; the paper names it "the Domain Wall Fermion
+ * operator", section 1, "node local 'Wilson' matrix", L223 section 4, "main kernel
+ * DWF code", L254 Fig.6, and never prints it -- SURVEY.md 8(c) reading #1):
+ *
+ *   Dhop psi(x,s) = sum_{mu=0..3} [ (1 - gamma_mu) U_mu(x)        psi(x+mu,s)
+ *                                 + (1 + gamma_mu) U_mu^dag(x-mu) psi(x-mu,s) ]
+ *
+ * x runs over a 4D lattice L0 x L1 x L2 x L3 (mu = 0,1,2,3 = x,y,z,t; time is the LAST extent),
+ * s = 0..Ls-1 is a spectator index, psi(x,s) has 4 spin x 3 colour complex components, U_mu(x)
+ * is a 3x3 complex matrix acting on colour.  DeGrand-Rossi gamma basis.  Boundaries are
+ * periodic; with DWF_ANTIPERIODIC_T a hop that wraps around the time direction gets a factor -1.
+ * No prefactor, no mass term, no fifth-dimension hopping.  1320 flop per output 5D site.
+ *
+ * Everything is extern "C", plain pointers and sizes.  Every function returns a DWF_* status
+ * (0 = success); on error no output is written; nothing aborts or throws.  dwf_last_error()
+ * returns a thread-local detail string for the last failing call of the calling thread.
+ *
+ * CANONICAL (interchange) layouts, reals of the geometry's precision, C order:
+ *   site     x = x0 + L0*(x1 + L1*(x2 + L2*x3))
+ *   parity   p(x) = (x0+x1+x2+x3) & 1  (s is not included)
+ *   gauge    [x][mu][a][b][reim]            U_mu(x)_{ab}: row a, column b, (U psi)_a = sum_b U_ab psi_b
+ *   spinor   [site][s][spin][colour][reim]  site = x (full field), or x>>1 for a half field that
+ *                                           holds the sites of one parity in increasing x
+ *
+ * DEVICE field layout (what `field`, `in`, `out` pointers below hold; produced only by
+ * dwf_import_spinor, read back only by dwf_export_spinor; size dwf_field_bytes):
+ *   complex[chunk][k][site][j]   s = chunk*Sc + j,  k = spin*3 + colour (12 complex components),
+ *                                site = x (full) or x>>1 (half), complex = (re, im) adjacent.
+ *   "SoA complex components, site-fastest, Ls innermost" (north_star subsystem 1): Sc consecutive
+ *   s of one component of one site are contiguous; Sc = dwf_layout_sc(g) is the number of s-slices
+ *   one thread keeps in registers so that each gauge link is loaded once and reused Sc times.
+ * Device pointers must be 16-byte aligned and live on the geometry's device.
+ * `stream` is a cudaStream_t passed as void* (NULL = the default stream).
+ */
+#ifndef DWF_H
+#define DWF_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dwf_geometry dwf_geometry;   /* opaque, library-owned */
+
+enum { DWF_OK = 0, DWF_ERR_INVALID_ARG = 1, DWF_ERR_BAD_GEOMETRY = 2, DWF_ERR_NO_GAUGE = 3,
+       DWF_ERR_CUDA = 4, DWF_ERR_ALLOC = 5, DWF_ERR_UNSUPPORTED = 6 };
+enum { DWF_F32 = 4, DWF_F64 = 8 };                   /* precision = bytes per real            */
+enum { DWF_PERIODIC = 0, DWF_ANTIPERIODIC_T = 1 };   /* time = dims[3]                        */
+enum { DWF_FULL = -1, DWF_EVEN = 0, DWF_ODD = 1 };   /* parity = (x0+x1+x2+x3) & 1            */
+
+/* Create a geometry: lattice extents dims[4] (each even and >= 2), fifth-dimension extent Ls >= 1,
+ * precision DWF_F32 / DWF_F64 (storage AND arithmetic; no mixed precision), bc_time, CUDA device
+ * ordinal.  Allocates the device gauge storage and reduction scratch (owned by the geometry).
+ * Errors: INVALID_ARG (NULL), BAD_GEOMETRY (odd or < 2 extent, Ls < 1, field too large),
+ * UNSUPPORTED (precision), CUDA / ALLOC. */
+int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, int cuda_device,
+                        dwf_geometry **out);
+
+/* Free everything the geometry owns.  Must not race with any other call on g. */
+int dwf_destroy_geometry(dwf_geometry *g);
+
+/* Load (or replace) the gauge field from the canonical layout; src_is_device says where
+ * U_canonical lives (host memory need not be pinned).  Builds the device copies: for every output
+ * site the 8 links it needs, U_mu(x) and the pre-daggered U_mu^dag(x-mu), with the antiperiodic
+ * sign folded in.  Synchronises `stream` before returning: the caller may free U_canonical. */
+int dwf_load_gauge(dwf_geometry *g, const void *U_canonical, int src_is_device, void *stream);
+
+/* out = Dhop in on full fields (device layout).  Asynchronous on `stream`.
+ * Errors: INVALID_ARG (NULL, in == out, misaligned), NO_GAUGE, CUDA.  Partial overlap of in and
+ * out is undefined. */
+int dwf_dhop(const dwf_geometry *g, const void *in_full, void *out_full, void *stream);
+
+/* Checkerboarded variants, first letter = output parity (SURVEY.md 8(c) reading #6):
+ * DhopOE: even half field in -> odd half field out;  DhopEO: odd in -> even out.
+ * (Dhop psi)_odd = DhopOE psi_even, (Dhop psi)_even = DhopEO psi_odd.  Asynchronous. */
+int dwf_dhop_oe(const dwf_geometry *g, const void *in_even, void *out_odd, void *stream);
+int dwf_dhop_eo(const dwf_geometry *g, const void *in_odd, void *out_even, void *stream);
+
+/* *result_host = sum over all reals of |field|^2, accumulated in fp64 in a fixed order
+ * (deterministic).  parity = DWF_FULL for a full field, DWF_EVEN / DWF_ODD for a half field.
+ * Synchronises `stream`. */
+int dwf_norm2(const dwf_geometry *g, const void *field, int parity, double *result_host,
+              void *stream);
+
+/* result_host[0..1] = (re, im) of sum conj(a) b.  Same rules as dwf_norm2. */
+int dwf_inner_product(const dwf_geometry *g, const void *a, const void *b, int parity,
+                      double result_host[2], void *stream);
+
+/* Bytes of a device field: full (DWF_FULL) or half (DWF_EVEN / DWF_ODD).  0 on bad arguments. */
+size_t dwf_field_bytes(const dwf_geometry *g, int parity);
+
+/* Sc of the device layout (s-slices per register block); 0 on NULL. */
+int dwf_layout_sc(const dwf_geometry *g);
+
+/* canonical -> device layout.  Host sources go through an internal staging copy and synchronise
+ * `stream`; device sources are asynchronous. */
+int dwf_import_spinor(const dwf_geometry *g, const void *canonical, int src_is_device, int parity,
+                      void *field_dev, void *stream);
+
+/* device layout -> canonical.  Host destinations synchronise `stream`. */
+int dwf_export_spinor(const dwf_geometry *g, const void *field_dev, int parity, void *canonical,
+                      int dst_is_device, void *stream);
+
+/* Number of kernel launches this library has issued since it was loaded (all threads). */
+unsigned long long dwf_launch_count(void);
+
+/* Select a kernel variant by name for experiments ("auto" = default); UNSUPPORTED if unknown. */
+int dwf_set_option(dwf_geometry *g, const char *key, long long value);
+
+const char *dwf_error_string(int code);
+const char *dwf_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DWF_H */

@@ -1,0 +1,165 @@
+"""CPU oracle for the DWF hopping term Dhop -- TEST INFRASTRUCTURE, NOT PRODUCT.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  It never imports, links or
+calls anything of ``paper_2203_06777_b200`` (the CUDA path), and that package
+never imports this one.
+
+The arithmetic lives in ``dhop_oracle.c`` (plain C, fp64, OpenMP over sites): the
+definition of the operator written out with full 4x4 gamma matrices, see that
+file's header for the passages it follows (PAPER.md L43/L223/L254 name the
+operator; BASELINE.json north_star states it; SURVEY.md 8(c) fixes conventions).
+This module only marshals numpy arrays (canonical layouts of include/dwf.h).
+
+Pins: tests/test_oracle_pins.py (P1-P9 of SURVEY.md 8(c)); nothing is unpinned.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "dhop_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+PERIODIC, ANTIPERIODIC_T = 0, 1
+EVEN, ODD = 0, 1
+
+
+def build(force: bool = False) -> str:
+    """Compile dhop_oracle.c into liboracle.so (in-tree).  Building is not using."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.check_call(
+            ["gcc", "-O2", "-std=c11", "-fcx-limited-range", "-fopenmp", "-fPIC", "-shared",
+             "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        vp, ci, i64 = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64
+        i4 = ctypes.POINTER(ctypes.c_int)
+        lib.orc_gamma.argtypes = [ci, vp]
+        lib.orc_gamma.restype = None
+        lib.orc_check_gamma.restype = ci
+        lib.orc_dhop.argtypes = [i4, ci, ci, vp, ci, vp, ci, vp]
+        lib.orc_dhop.restype = ci
+        lib.orc_dhop_cb.argtypes = [i4, ci, ci, ci, vp, ci, vp, ci, vp]
+        lib.orc_dhop_cb.restype = ci
+        lib.orc_dhop_sites.argtypes = [i4, ci, ci, vp, ci, vp, ci, ci, vp, i64, vp]
+        lib.orc_dhop_sites.restype = ci
+        lib.orc_norm2.argtypes = [vp, ci, i64]
+        lib.orc_norm2.restype = ctypes.c_double
+        lib.orc_inner.argtypes = [vp, vp, ci, i64, vp]
+        lib.orc_inner.restype = None
+        lib.orc_num_threads.restype = ci
+        if lib.orc_check_gamma() != 0:
+            raise RuntimeError("oracle gamma matrices fail their algebra self-check")
+        _lib = lib
+    return _lib
+
+
+def _prec(a: np.ndarray) -> int:
+    if a.dtype == np.float32:
+        return 4
+    if a.dtype == np.float64:
+        return 8
+    raise TypeError("fields must be float32 or float64 arrays of reals")
+
+
+def _dims(dims):
+    d = (ctypes.c_int * 4)(*[int(v) for v in dims])
+    return d, int(dims[0]) * int(dims[1]) * int(dims[2]) * int(dims[3])
+
+
+def _c(a: np.ndarray) -> np.ndarray:
+    if not a.flags.c_contiguous:
+        raise ValueError("arrays must be C-contiguous")
+    return a
+
+
+def num_threads() -> int:
+    return int(_load().orc_num_threads())
+
+
+def gamma(mu: int) -> np.ndarray:
+    """The oracle's own gamma_mu as a complex (4,4) array (for the pins)."""
+    out = np.zeros((4, 4, 2))
+    _load().orc_gamma(mu, out.ctypes.data)
+    return out[..., 0] + 1j * out[..., 1]
+
+
+def dhop(dims, Ls: int, bc_time: int, U: np.ndarray, psi: np.ndarray) -> np.ndarray:
+    """Full Dhop.  U (V4,4,3,3,2), psi (V4,Ls,4,3,2) -> fp64 (V4,Ls,4,3,2)."""
+    d, v4 = _dims(dims)
+    assert U.size == v4 * 72 and psi.size == v4 * Ls * 24
+    out = np.empty((v4, Ls, 4, 3, 2), dtype=np.float64)
+    rc = _load().orc_dhop(d, Ls, bc_time, _c(U).ctypes.data, _prec(U),
+                          _c(psi).ctypes.data, _prec(psi), out.ctypes.data)
+    if rc:
+        raise ValueError("orc_dhop: bad arguments")
+    return out
+
+
+def dhop_cb(dims, Ls: int, bc_time: int, parity_out: int, U: np.ndarray,
+            psi_half: np.ndarray) -> np.ndarray:
+    """Checkerboarded Dhop onto parity_out (ODD: DhopOE, EVEN: DhopEO).
+    psi_half (V4/2,Ls,4,3,2) lives on the opposite parity -> fp64 (V4/2,Ls,4,3,2)."""
+    d, v4 = _dims(dims)
+    assert U.size == v4 * 72 and psi_half.size == (v4 // 2) * Ls * 24
+    out = np.empty((v4 // 2, Ls, 4, 3, 2), dtype=np.float64)
+    rc = _load().orc_dhop_cb(d, Ls, bc_time, parity_out, _c(U).ctypes.data, _prec(U),
+                             _c(psi_half).ctypes.data, _prec(psi_half), out.ctypes.data)
+    if rc:
+        raise ValueError("orc_dhop_cb: bad arguments (extents must be even)")
+    return out
+
+
+def dhop_oe(dims, Ls, bc_time, U, psi_even):
+    """DhopOE: even in -> odd out (SURVEY.md 8(c) reading #6)."""
+    return dhop_cb(dims, Ls, bc_time, ODD, U, psi_even)
+
+
+def dhop_eo(dims, Ls, bc_time, U, psi_odd):
+    """DhopEO: odd in -> even out."""
+    return dhop_cb(dims, Ls, bc_time, EVEN, U, psi_odd)
+
+
+def dhop_sites(dims, Ls: int, bc_time: int, U: np.ndarray, psi: np.ndarray, psi_is_half: bool,
+               sites) -> np.ndarray:
+    """Dhop at the listed output sites (lexicographic indices) -> fp64 (n,Ls,4,3,2)."""
+    d, v4 = _dims(dims)
+    sites = np.ascontiguousarray(sites, dtype=np.int64)
+    assert U.size == v4 * 72
+    assert psi.size == (v4 // 2 if psi_is_half else v4) * Ls * 24
+    assert sites.size == 0 or (0 <= sites.min() and sites.max() < v4)
+    out = np.empty((sites.size, Ls, 4, 3, 2), dtype=np.float64)
+    rc = _load().orc_dhop_sites(d, Ls, bc_time, _c(U).ctypes.data, _prec(U),
+                                _c(psi).ctypes.data, _prec(psi), int(bool(psi_is_half)),
+                                sites.ctypes.data, sites.size, out.ctypes.data)
+    if rc:
+        raise ValueError("orc_dhop_sites: bad arguments")
+    return out
+
+
+def norm2(x: np.ndarray) -> float:
+    """sum of squares of all reals of x (fp64, compensated)."""
+    return float(_load().orc_norm2(_c(x).ctypes.data, _prec(x), x.size))
+
+
+def inner(a: np.ndarray, b: np.ndarray) -> complex:
+    """sum conj(a) * b over all complex entries (last axis = re, im)."""
+    assert a.shape == b.shape and a.dtype == b.dtype and a.size % 2 == 0
+    out = np.zeros(2)
+    _load().orc_inner(_c(a).ctypes.data, _c(b).ctypes.data, _prec(a), a.size // 2, out.ctypes.data)
+    return complex(out[0], out[1])

@@ -1,0 +1,212 @@
+"""Pins for the CPU oracle.  CPU only.
+
+Each pin checks oracle/ against something other than itself: a dense matrix assembled a
+different way, a closed form, or an invariant of the operator.  A dropped term, a wrong sign
+or index, a transposed link or a wrong parity rule fails at least one of them.
+"""
+import numpy as np
+import pytest
+
+import dwf_inputs as gen
+import oracle
+from _util import (GAMMA5, apply_dense, coords, cplx, dense_dhop_matrix, lex, pauli_gammas, reals,
+                   rel_err, shift_index)
+
+TINY = [((2, 2, 2, 2), 2), ((4, 2, 4, 2), 3), ((2, 4, 2, 6), 1)]
+
+
+def test_gamma_algebra_and_basis():
+    g_or = [oracle.gamma(mu) for mu in range(4)]
+    g_pa = pauli_gammas()
+    for mu in range(4):
+        assert np.array_equal(g_or[mu], g_or[mu].conj().T)
+        assert np.allclose(g_or[mu], g_pa[mu], atol=0)           # same basis, built two ways
+        for nu in range(4):
+            anti = g_or[mu] @ g_or[nu] + g_or[nu] @ g_or[mu]
+            assert np.allclose(anti, 2 * np.eye(4) * (mu == nu), atol=0)
+    assert np.allclose(g_or[0] @ g_or[1] @ g_or[2] @ g_or[3], GAMMA5, atol=0)
+
+
+@pytest.mark.parametrize("dims,Ls", TINY)
+@pytest.mark.parametrize("bc", [oracle.PERIODIC, oracle.ANTIPERIODIC_T])
+def test_p1_dense_matrix(dims, Ls, bc):
+    V = int(np.prod(dims))
+    U = gen.gauge_random(dims, seed=11)
+    psi = gen.spinor_gaussian(V, Ls, seed=11)
+    D = dense_dhop_matrix(dims, U, bc == oracle.ANTIPERIODIC_T)
+    want = apply_dense(D, psi)
+    got = oracle.dhop(dims, Ls, bc, U, psi)
+    assert rel_err(got, want) < 1e-14
+
+
+def test_p1_dense_matrix_4x4x4x4():
+    dims, Ls = (4, 4, 4, 4), 1
+    V = 256
+    U = gen.gauge_random(dims, seed=1001)
+    psi = gen.spinor_gaussian(V, Ls, seed=1001)
+    D = dense_dhop_matrix(dims, U, True)
+    assert rel_err(oracle.dhop(dims, Ls, oracle.ANTIPERIODIC_T, U, psi), apply_dense(D, psi)) < 1e-14
+
+
+def test_p1_dense_matrix_fp32_inputs_promoted_exactly():
+    dims, Ls = (2, 4, 2, 2), 2
+    V = int(np.prod(dims))
+    U = gen.gauge_random(dims, seed=5, prec=4)
+    psi = gen.spinor_gaussian(V, Ls, seed=5, prec=4)
+    D = dense_dhop_matrix(dims, U, False)
+    assert rel_err(oracle.dhop(dims, Ls, 0, U, psi), apply_dense(D, psi)) < 1e-14
+
+
+@pytest.mark.parametrize("dims,n,bc", [
+    ((4, 4, 4, 4), (0, 0, 0, 0), 0),
+    ((4, 6, 2, 8), (1, 2, 1, 3), 0),
+    ((4, 6, 2, 8), (3, 5, 0, 2), 1),
+    ((8, 8, 8, 8), (7, 1, 4, 5), 1),
+])
+def test_p2_free_field_plane_wave(dims, n, bc):
+    Ls = 3
+    V = int(np.prod(dims))
+    U = gen.gauge_unit(dims)
+    p = np.array([2 * np.pi * n[mu] / dims[mu] for mu in range(4)])
+    if bc:
+        p[3] = (2 * n[3] + 1) * np.pi / dims[3]
+    rng = np.random.default_rng(3)
+    chi = rng.normal(size=(Ls, 4, 3)) + 1j * rng.normal(size=(Ls, 4, 3))
+    phase = np.exp(1j * (coords(dims) @ p))
+    psi = phase[:, None, None, None] * chi[None]
+    g = pauli_gammas()
+    M = sum(2 * np.cos(p[mu]) * np.eye(4) - 2j * np.sin(p[mu]) * g[mu] for mu in range(4))
+    want = np.einsum("ab,xsbc->xsac", M, psi)
+    got = oracle.dhop(dims, Ls, bc, U, reals(psi))
+    assert rel_err(got, reals(want)) < 1e-13
+    if not bc and not any(n):
+        assert rel_err(got, 8 * reals(psi)) < 1e-14           # p = 0: Dhop psi = 8 psi
+
+
+@pytest.mark.parametrize("dims,Ls,bc", [((4, 2, 4, 2), 2, 0), ((4, 4, 2, 6), 3, 1)])
+def test_p3_gamma5_hermiticity(dims, Ls, bc):
+    V = int(np.prod(dims))
+    U = gen.gauge_random(dims, seed=21)
+    psi = gen.spinor_gaussian(V, Ls, seed=21, stream=gen.STREAM_SPINOR)
+    phi = gen.spinor_gaussian(V, Ls, seed=21, stream=gen.STREAM_SPINOR2)
+    g5 = np.array([1, 1, -1, -1.0])[None, None, :, None, None]
+    lhs = oracle.inner(phi, oracle.dhop(dims, Ls, bc, U, psi))
+    g5Dg5phi = g5 * oracle.dhop(dims, Ls, bc, U, np.ascontiguousarray(g5 * phi))
+    rhs = oracle.inner(np.ascontiguousarray(g5Dg5phi), psi)
+    assert abs(lhs - rhs) / abs(lhs) < 1e-13
+    # and Dhop is NOT hermitian without the gamma5's (the test has teeth)
+    plain = oracle.inner(oracle.dhop(dims, Ls, bc, U, phi), psi)
+    assert abs(lhs - plain) / abs(lhs) > 1e-3
+
+
+@pytest.mark.parametrize("dims,Ls,bc", [((4, 2, 4, 2), 2, 0), ((2, 4, 4, 4), 2, 1)])
+def test_p4_gauge_covariance(dims, Ls, bc):
+    V = int(np.prod(dims))
+    U = cplx(gen.gauge_random(dims, seed=31))                     # (V,4,3,3)
+    psi = cplx(gen.spinor_gaussian(V, Ls, seed=31))               # (V,Ls,4,3)
+    g = cplx(gen.su3_random(V, seed=31))                          # (V,3,3)
+    Ut = np.empty_like(U)
+    for mu in range(4):
+        gp = g[shift_index(dims, mu, +1)]
+        Ut[:, mu] = np.einsum("xab,xbc,xdc->xad", g, U[:, mu], gp.conj())
+    psit = np.einsum("xab,xsib->xsia", g, psi)
+    lhs = oracle.dhop(dims, Ls, bc, reals(Ut), reals(psit))
+    rhs = np.einsum("xab,xsib->xsia", g, cplx(oracle.dhop(dims, Ls, bc, reals(U), reals(psi))))
+    assert rel_err(lhs, reals(rhs)) < 1e-14
+
+
+@pytest.mark.parametrize("dims,Ls,bc", [((4, 2, 4, 2), 2, 0), ((2, 2, 4, 6), 3, 1), ((4, 4, 4, 4), 2, 1)])
+def test_p5_even_odd_reassembly(dims, Ls, bc):
+    V = int(np.prod(dims))
+    U = gen.gauge_random(dims, seed=41)
+    psi = gen.spinor_gaussian(V, Ls, seed=41)
+    par = gen.site_parity(dims)
+    full = oracle.dhop(dims, Ls, bc, U, psi)
+    out_o = oracle.dhop_oe(dims, Ls, bc, U, gen.split_parity(psi, dims, 0))
+    out_e = oracle.dhop_eo(dims, Ls, bc, U, gen.split_parity(psi, dims, 1))
+    # half-field index must be x>>1 within each parity
+    x = np.arange(V)
+    assert np.array_equal(np.sort(x[par == 0] >> 1), np.arange(V // 2))
+    re = np.empty_like(full)
+    re[x[par == 1]] = out_o[x[par == 1] >> 1]
+    re[x[par == 0]] = out_e[x[par == 0] >> 1]
+    assert rel_err(re, full) < 1e-15
+    # Dhop of an even-only field has exactly zero even components
+    psi_e = psi.copy()
+    psi_e[par == 1] = 0
+    assert np.all(oracle.dhop(dims, Ls, bc, U, psi_e)[par == 0] == 0)
+
+
+def test_p5_cb_rejects_odd_extent():
+    with pytest.raises(ValueError):
+        oracle.dhop_cb((3, 2, 2, 2), 1, 0, 1, gen.gauge_unit((3, 2, 2, 2)),
+                       np.zeros((12, 1, 4, 3, 2)))
+
+
+def test_p6_s_equivariance():
+    dims, Ls = (2, 4, 2, 4), 5
+    V = int(np.prod(dims))
+    U = gen.gauge_random(dims, seed=51)
+    psi = gen.spinor_gaussian(V, Ls, seed=51)
+    perm = np.array([3, 0, 4, 1, 2])
+    a = oracle.dhop(dims, Ls, 1, U, psi)
+    b = oracle.dhop(dims, Ls, 1, U, np.ascontiguousarray(psi[:, perm]))
+    assert np.array_equal(a[:, perm], b)
+    one = oracle.dhop(dims, 1, 1, U, np.ascontiguousarray(psi[:, 2:3]))
+    assert np.array_equal(one[:, 0], a[:, 2])
+
+
+def test_p7_linearity_and_translation():
+    dims, Ls = (4, 2, 2, 4), 2
+    V = int(np.prod(dims))
+    U = gen.gauge_random(dims, seed=61)
+    psi = cplx(gen.spinor_gaussian(V, Ls, seed=61, stream=1))
+    phi = cplx(gen.spinor_gaussian(V, Ls, seed=61, stream=2))
+    a, b = 0.3 - 1.1j, -2.0 + 0.5j
+    D = lambda z: cplx(oracle.dhop(dims, Ls, 0, U, reals(z)))
+    assert rel_err(reals(D(a * psi + b * phi)), reals(a * D(psi) + b * D(phi))) < 1e-14
+    # translation by one site in each direction (periodic): shifting U and psi shifts the output
+    for mu in range(4):
+        nb = shift_index(dims, mu, +1)
+        Us = np.ascontiguousarray(U[nb])
+        shifted = cplx(oracle.dhop(dims, Ls, 0, Us, reals(psi[nb])))
+        assert rel_err(reals(shifted), reals(D(psi)[nb])) < 1e-15
+
+
+def test_p8_norm_bound_and_unitary_links():
+    dims, Ls = (8, 8, 8, 8), 2
+    V = int(np.prod(dims))
+    U = gen.gauge_random(dims, seed=71)
+    psi = gen.spinor_gaussian(V, Ls, seed=71)
+    out = oracle.dhop(dims, Ls, 1, U, psi)
+    ratio = np.sqrt(oracle.norm2(out) / oracle.norm2(psi))
+    assert 1.0 < ratio <= 8.0
+
+
+def test_p9_norm2_and_inner():
+    assert oracle.norm2(np.full(1000, 0.5)) == 250.0
+    rng = np.random.default_rng(0)
+    for dt, tol in ((np.float64, 1e-14), (np.float32, 1e-14)):
+        x = rng.normal(size=(501, 2)).astype(dt)
+        y = rng.normal(size=(501, 2)).astype(dt)
+        ref = np.sum(x.astype(np.float64) ** 2)
+        assert abs(oracle.norm2(x) - ref) / ref < tol
+        want = np.vdot(cplx(x.astype(np.float64)), cplx(y.astype(np.float64)))
+        assert abs(oracle.inner(x, y) - want) / abs(want) < 1e-13
+    # compensated sum survives a cancellation-prone sequence
+    z = np.array([1e8, 1.0, 1e-4] * 1000)
+    assert abs(oracle.norm2(z) - 1000 * (1e16 + 1.0 + 1e-8)) / 1e19 < 1e-15
+
+
+def test_sites_subset_matches_full_and_cb():
+    dims, Ls, bc = (4, 4, 2, 6), 2, 1
+    V = int(np.prod(dims))
+    U = gen.gauge_random(dims, seed=81, prec=4)
+    psi = gen.spinor_gaussian(V, Ls, seed=81, prec=4)
+    full = oracle.dhop(dims, Ls, bc, U, psi)
+    sites = np.array([0, 5, 17, V - 1, V // 2])
+    assert np.array_equal(oracle.dhop_sites(dims, Ls, bc, U, psi, False, sites), full[sites])
+    par = gen.site_parity(dims)
+    odd = np.arange(V)[par == 1][[0, 3, 40, -1]]
+    sub = oracle.dhop_sites(dims, Ls, bc, U, gen.split_parity(psi, dims, 0), True, odd)
+    assert np.array_equal(sub, full[odd])
