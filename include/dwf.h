@@ -44,6 +44,12 @@
 extern "C" {
 #endif
 
+#if defined(__GNUC__)
+#define DWF_API __attribute__((visibility("default")))
+#else
+#define DWF_API
+#endif
+
 typedef struct dwf_geometry dwf_geometry;   /* opaque, library-owned */
 
 enum { DWF_OK = 0, DWF_ERR_INVALID_ARG = 1, DWF_ERR_BAD_GEOMETRY = 2, DWF_ERR_NO_GAUGE = 3,
@@ -57,62 +63,62 @@ enum { DWF_FULL = -1, DWF_EVEN = 0, DWF_ODD = 1 };   /* parity = (x0+x1+x2+x3) &
  * ordinal.  Allocates the device gauge storage and reduction scratch (owned by the geometry).
  * Errors: INVALID_ARG (NULL), BAD_GEOMETRY (odd or < 2 extent, Ls < 1, field too large),
  * UNSUPPORTED (precision), CUDA / ALLOC. */
-int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, int cuda_device,
+DWF_API int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, int cuda_device,
                         dwf_geometry **out);
 
 /* Free everything the geometry owns.  Must not race with any other call on g. */
-int dwf_destroy_geometry(dwf_geometry *g);
+DWF_API int dwf_destroy_geometry(dwf_geometry *g);
 
 /* Load (or replace) the gauge field from the canonical layout; src_is_device says where
  * U_canonical lives (host memory need not be pinned).  Builds the device copies: for every output
  * site the 8 links it needs, U_mu(x) and the pre-daggered U_mu^dag(x-mu), with the antiperiodic
  * sign folded in.  Synchronises `stream` before returning: the caller may free U_canonical. */
-int dwf_load_gauge(dwf_geometry *g, const void *U_canonical, int src_is_device, void *stream);
+DWF_API int dwf_load_gauge(dwf_geometry *g, const void *U_canonical, int src_is_device, void *stream);
 
 /* out = Dhop in on full fields (device layout).  Asynchronous on `stream`.
  * Errors: INVALID_ARG (NULL, in == out, misaligned), NO_GAUGE, CUDA.  Partial overlap of in and
  * out is undefined. */
-int dwf_dhop(const dwf_geometry *g, const void *in_full, void *out_full, void *stream);
+DWF_API int dwf_dhop(const dwf_geometry *g, const void *in_full, void *out_full, void *stream);
 
 /* Checkerboarded variants, first letter = output parity (SURVEY.md 8(c) reading #6):
  * DhopOE: even half field in -> odd half field out;  DhopEO: odd in -> even out.
  * (Dhop psi)_odd = DhopOE psi_even, (Dhop psi)_even = DhopEO psi_odd.  Asynchronous. */
-int dwf_dhop_oe(const dwf_geometry *g, const void *in_even, void *out_odd, void *stream);
-int dwf_dhop_eo(const dwf_geometry *g, const void *in_odd, void *out_even, void *stream);
+DWF_API int dwf_dhop_oe(const dwf_geometry *g, const void *in_even, void *out_odd, void *stream);
+DWF_API int dwf_dhop_eo(const dwf_geometry *g, const void *in_odd, void *out_even, void *stream);
 
 /* *result_host = sum over all reals of |field|^2, accumulated in fp64 in a fixed order
  * (deterministic).  parity = DWF_FULL for a full field, DWF_EVEN / DWF_ODD for a half field.
  * Synchronises `stream`. */
-int dwf_norm2(const dwf_geometry *g, const void *field, int parity, double *result_host,
+DWF_API int dwf_norm2(const dwf_geometry *g, const void *field, int parity, double *result_host,
               void *stream);
 
 /* result_host[0..1] = (re, im) of sum conj(a) b.  Same rules as dwf_norm2. */
-int dwf_inner_product(const dwf_geometry *g, const void *a, const void *b, int parity,
+DWF_API int dwf_inner_product(const dwf_geometry *g, const void *a, const void *b, int parity,
                       double result_host[2], void *stream);
 
 /* Bytes of a device field: full (DWF_FULL) or half (DWF_EVEN / DWF_ODD).  0 on bad arguments. */
-size_t dwf_field_bytes(const dwf_geometry *g, int parity);
+DWF_API size_t dwf_field_bytes(const dwf_geometry *g, int parity);
 
 /* Sc of the device layout (s-slices per register block); 0 on NULL. */
-int dwf_layout_sc(const dwf_geometry *g);
+DWF_API int dwf_layout_sc(const dwf_geometry *g);
 
 /* canonical -> device layout.  Host sources go through an internal staging copy and synchronise
  * `stream`; device sources are asynchronous. */
-int dwf_import_spinor(const dwf_geometry *g, const void *canonical, int src_is_device, int parity,
+DWF_API int dwf_import_spinor(const dwf_geometry *g, const void *canonical, int src_is_device, int parity,
                       void *field_dev, void *stream);
 
 /* device layout -> canonical.  Host destinations synchronise `stream`. */
-int dwf_export_spinor(const dwf_geometry *g, const void *field_dev, int parity, void *canonical,
+DWF_API int dwf_export_spinor(const dwf_geometry *g, const void *field_dev, int parity, void *canonical,
                       int dst_is_device, void *stream);
 
 /* Number of kernel launches this library has issued since it was loaded (all threads). */
-unsigned long long dwf_launch_count(void);
+DWF_API unsigned long long dwf_launch_count(void);
 
 /* Select a kernel variant by name for experiments ("auto" = default); UNSUPPORTED if unknown. */
-int dwf_set_option(dwf_geometry *g, const char *key, long long value);
+DWF_API int dwf_set_option(dwf_geometry *g, const char *key, long long value);
 
-const char *dwf_error_string(int code);
-const char *dwf_last_error(void);
+DWF_API const char *dwf_error_string(int code);
+DWF_API const char *dwf_last_error(void);
 
 #ifdef __cplusplus
 }

@@ -1,0 +1,268 @@
+"""paper_2203_06777_b200 -- thin Python binding of libdwf.so (include/dwf.h).
+
+Argument marshalling only: every step of the Dhop path runs in the CUDA kernels of
+``csrc/``.  The functions carry the names of the C ABI (``dwf_create_geometry``,
+``dwf_load_gauge``, ``dwf_dhop``, ``dwf_dhop_oe``, ``dwf_dhop_eo``, ``dwf_norm2`` ...) and take
+numpy arrays (host, canonical layouts) or torch CUDA tensors (device memory).  PyTorch is used
+for device memory and streams only.  There is no CPU fallback: ``load()`` raises when
+``libdwf.so`` cannot be loaded, and this package never imports ``oracle``.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+OK, ERR_INVALID_ARG, ERR_BAD_GEOMETRY, ERR_NO_GAUGE, ERR_CUDA, ERR_ALLOC, ERR_UNSUPPORTED = range(7)
+F32, F64 = 4, 8
+PERIODIC, ANTIPERIODIC_T = 0, 1
+FULL, EVEN, ODD = -1, 0, 1
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdwf.so")
+
+# every symbol include/dwf.h declares (tests check that the library exports all of them)
+SYMBOLS = (
+    "dwf_create_geometry", "dwf_destroy_geometry", "dwf_load_gauge", "dwf_dhop", "dwf_dhop_oe",
+    "dwf_dhop_eo", "dwf_norm2", "dwf_inner_product", "dwf_field_bytes", "dwf_layout_sc",
+    "dwf_import_spinor", "dwf_export_spinor", "dwf_launch_count", "dwf_set_option",
+    "dwf_error_string", "dwf_last_error",
+)
+
+
+class DwfError(RuntimeError):
+    def __init__(self, code: int, what: str, detail: str):
+        super().__init__(f"{what}: {detail} (code {code})")
+        self.code = code
+
+
+_lib = None
+
+
+def load(build_if_missing: bool = True):
+    """Load libdwf.so (building it in-tree with nvcc if it is absent).  Raises if impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        if not build_if_missing:
+            raise RuntimeError(f"{LIB_PATH} is missing: run python -m paper_2203_06777_b200.build")
+        from . import build as _b
+        _b.build()
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, ci, cs = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
+    lib.dwf_create_geometry.argtypes = [ctypes.POINTER(ci), ci, ci, ci, ci, ctypes.POINTER(vp)]
+    lib.dwf_destroy_geometry.argtypes = [vp]
+    lib.dwf_load_gauge.argtypes = [vp, vp, ci, vp]
+    for f in (lib.dwf_dhop, lib.dwf_dhop_oe, lib.dwf_dhop_eo):
+        f.argtypes = [vp, vp, vp, vp]
+    lib.dwf_norm2.argtypes = [vp, vp, ci, ctypes.POINTER(ctypes.c_double), vp]
+    lib.dwf_inner_product.argtypes = [vp, vp, vp, ci, ctypes.POINTER(ctypes.c_double), vp]
+    lib.dwf_field_bytes.argtypes = [vp, ci]
+    lib.dwf_field_bytes.restype = cs
+    lib.dwf_layout_sc.argtypes = [vp]
+    lib.dwf_import_spinor.argtypes = [vp, vp, ci, ci, vp, vp]
+    lib.dwf_export_spinor.argtypes = [vp, vp, ci, vp, ci, vp]
+    lib.dwf_launch_count.argtypes = []
+    lib.dwf_launch_count.restype = ctypes.c_ulonglong
+    lib.dwf_set_option.argtypes = [vp, ctypes.c_char_p, ctypes.c_longlong]
+    lib.dwf_error_string.argtypes = [ci]
+    lib.dwf_error_string.restype = ctypes.c_char_p
+    lib.dwf_last_error.argtypes = []
+    lib.dwf_last_error.restype = ctypes.c_char_p
+    _lib = lib
+    return lib
+
+
+def _check(rc: int, what: str):
+    if rc != OK:
+        lib = load()
+        raise DwfError(rc, what, (lib.dwf_last_error() or lib.dwf_error_string(rc)).decode())
+
+
+def _stream(stream) -> int:
+    """cudaStream_t as an integer: None = torch's current stream."""
+    if stream is None:
+        import torch
+        return int(torch.cuda.current_stream().cuda_stream)
+    if hasattr(stream, "cuda_stream"):
+        return int(stream.cuda_stream)
+    return int(stream)
+
+
+def _ptr(a):
+    """(address, is_device) of a numpy array or a torch tensor."""
+    if isinstance(a, np.ndarray):
+        if not a.flags.c_contiguous:
+            raise ValueError("host arrays must be C-contiguous")
+        return a.ctypes.data, 0
+    if not a.is_contiguous():
+        raise ValueError("tensors must be contiguous")
+    return a.data_ptr(), 1 if a.is_cuda else 0
+
+
+def _dev_ptr(t) -> int:
+    if not getattr(t, "is_cuda", False) or not t.is_contiguous():
+        raise ValueError("device fields must be contiguous torch CUDA tensors")
+    return t.data_ptr()
+
+
+# ---------------------------------------------------------------------------------------------
+# the C ABI, name for name
+# ---------------------------------------------------------------------------------------------
+def dwf_create_geometry(dims, Ls: int, precision: int, bc_time: int = PERIODIC, cuda_device: int = 0) -> int:
+    lib = load()
+    d = (ctypes.c_int * 4)(*[int(v) for v in dims])
+    h = ctypes.c_void_p()
+    _check(lib.dwf_create_geometry(d, int(Ls), int(precision), int(bc_time), int(cuda_device),
+                                   ctypes.byref(h)), "dwf_create_geometry")
+    return h.value
+
+
+def dwf_destroy_geometry(g: int) -> None:
+    _check(load().dwf_destroy_geometry(g), "dwf_destroy_geometry")
+
+
+def dwf_load_gauge(g: int, U, stream=None) -> None:
+    p, on_dev = _ptr(U)
+    _check(load().dwf_load_gauge(g, p, on_dev, _stream(stream)), "dwf_load_gauge")
+
+
+def dwf_dhop(g: int, in_full, out_full, stream=None) -> None:
+    _check(load().dwf_dhop(g, _dev_ptr(in_full), _dev_ptr(out_full), _stream(stream)), "dwf_dhop")
+
+
+def dwf_dhop_oe(g: int, in_even, out_odd, stream=None) -> None:
+    _check(load().dwf_dhop_oe(g, _dev_ptr(in_even), _dev_ptr(out_odd), _stream(stream)), "dwf_dhop_oe")
+
+
+def dwf_dhop_eo(g: int, in_odd, out_even, stream=None) -> None:
+    _check(load().dwf_dhop_eo(g, _dev_ptr(in_odd), _dev_ptr(out_even), _stream(stream)), "dwf_dhop_eo")
+
+
+def dwf_norm2(g: int, field, parity: int = FULL, stream=None) -> float:
+    r = ctypes.c_double()
+    _check(load().dwf_norm2(g, _dev_ptr(field), int(parity), ctypes.byref(r), _stream(stream)), "dwf_norm2")
+    return r.value
+
+
+def dwf_inner_product(g: int, a, b, parity: int = FULL, stream=None) -> complex:
+    r = (ctypes.c_double * 2)()
+    _check(load().dwf_inner_product(g, _dev_ptr(a), _dev_ptr(b), int(parity), r, _stream(stream)),
+           "dwf_inner_product")
+    return complex(r[0], r[1])
+
+
+def dwf_field_bytes(g: int, parity: int = FULL) -> int:
+    return int(load().dwf_field_bytes(g, int(parity)))
+
+
+def dwf_layout_sc(g: int) -> int:
+    return int(load().dwf_layout_sc(g))
+
+
+def dwf_import_spinor(g: int, canonical, parity: int, field_dev, stream=None) -> None:
+    p, on_dev = _ptr(canonical)
+    _check(load().dwf_import_spinor(g, p, on_dev, int(parity), _dev_ptr(field_dev), _stream(stream)),
+           "dwf_import_spinor")
+
+
+def dwf_export_spinor(g: int, field_dev, parity: int, canonical, stream=None) -> None:
+    p, on_dev = _ptr(canonical)
+    _check(load().dwf_export_spinor(g, _dev_ptr(field_dev), int(parity), p, on_dev, _stream(stream)),
+           "dwf_export_spinor")
+
+
+def dwf_launch_count() -> int:
+    return int(load().dwf_launch_count())
+
+
+def dwf_set_option(g: int, key: str, value: int) -> None:
+    _check(load().dwf_set_option(g, key.encode(), int(value)), f"dwf_set_option({key})")
+
+
+# ---------------------------------------------------------------------------------------------
+# convenience wrapper: owns the handle, allocates device fields with torch
+# ---------------------------------------------------------------------------------------------
+class Geometry:
+    """A dwf_geometry handle plus torch-allocated device fields.  No arithmetic here."""
+
+    def __init__(self, dims, Ls: int, precision: int, bc_time: int = PERIODIC, device: int = 0):
+        import torch
+        self.dims = tuple(int(d) for d in dims)
+        self.Ls, self.precision, self.bc_time, self.device = int(Ls), int(precision), int(bc_time), int(device)
+        self.V4 = self.dims[0] * self.dims[1] * self.dims[2] * self.dims[3]
+        self._torch = torch
+        self.handle = dwf_create_geometry(self.dims, Ls, precision, bc_time, device)
+
+    def close(self):
+        if getattr(self, "handle", None):
+            dwf_destroy_geometry(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    @property
+    def np_dtype(self):
+        return np.float32 if self.precision == F32 else np.float64
+
+    @property
+    def torch_dtype(self):
+        return self._torch.float32 if self.precision == F32 else self._torch.float64
+
+    def nsites(self, parity: int = FULL) -> int:
+        return self.V4 if parity == FULL else self.V4 // 2
+
+    def new_field(self, parity: int = FULL):
+        """Uninitialised device field (device layout), a flat torch tensor of reals."""
+        n = dwf_field_bytes(self.handle, parity) // self.precision
+        return self._torch.empty(n, dtype=self.torch_dtype, device=f"cuda:{self.device}")
+
+    def load_gauge(self, U, stream=None):
+        dwf_load_gauge(self.handle, U, stream)
+
+    def import_spinor(self, canonical, parity: int = FULL, out=None, stream=None):
+        out = self.new_field(parity) if out is None else out
+        dwf_import_spinor(self.handle, canonical, parity, out, stream)
+        return out
+
+    def export_spinor(self, field, parity: int = FULL, out=None, stream=None):
+        if out is None:
+            out = np.empty((self.nsites(parity), self.Ls, 4, 3, 2), dtype=self.np_dtype)
+        dwf_export_spinor(self.handle, field, parity, out, stream)
+        return out
+
+    def dhop(self, inp, out=None, stream=None):
+        out = self.new_field(FULL) if out is None else out
+        dwf_dhop(self.handle, inp, out, stream)
+        return out
+
+    def dhop_oe(self, in_even, out=None, stream=None):
+        out = self.new_field(ODD) if out is None else out
+        dwf_dhop_oe(self.handle, in_even, out, stream)
+        return out
+
+    def dhop_eo(self, in_odd, out=None, stream=None):
+        out = self.new_field(EVEN) if out is None else out
+        dwf_dhop_eo(self.handle, in_odd, out, stream)
+        return out
+
+    def norm2(self, field, parity: int = FULL, stream=None) -> float:
+        return dwf_norm2(self.handle, field, parity, stream)
+
+    def inner_product(self, a, b, parity: int = FULL, stream=None) -> complex:
+        return dwf_inner_product(self.handle, a, b, parity, stream)
+
+    def set_option(self, key: str, value: int):
+        dwf_set_option(self.handle, key, value)

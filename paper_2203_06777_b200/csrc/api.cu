@@ -1,0 +1,378 @@
+// api.cu -- the C ABI of include/dwf.h: argument checking, geometry ownership, launch plumbing.
+#include <stdarg.h>
+#include <string.h>
+
+#include <algorithm>
+#include <vector>
+
+#include "dwf_internal.cuh"
+
+namespace dwf {
+
+static thread_local char t_err[512] = "";
+std::atomic<unsigned long long> g_launches{0};
+
+void set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(t_err, sizeof(t_err), fmt, ap);
+    va_end(ap);
+}
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+
+// largest power-of-two exponent <= want that divides extent
+static int fit_shift(int extent, int want)
+{
+    int s = 0;
+    while (s < want && extent % (1 << (s + 1)) == 0) s++;
+    return s;
+}
+
+// Tile table in launch order.  `raster` picks how the 4D grid of tiles is linearised; concurrently
+// resident CTAs then cover a compact region so that halo re-reads hit in L2:
+//   0: lexicographic, direction 0 fastest, time slowest
+//   1: like 0, but direction 2 is split into two macro blocks swept one after the other
+//   2: like 0, but direction 2 is split into four macro blocks
+//   3: time fastest, then 0, 1, 2
+static void build_tile_table(const Tiling &t, int raster, std::vector<int4> &tab)
+{
+    struct Digit { int dim, count; };
+    std::vector<Digit> digits;   // fastest first
+    auto split2 = [&](int nsplit) {
+        int n2 = t.ntile[2];
+        int outer = (n2 % nsplit == 0) ? nsplit : 1;
+        digits = {{0, t.ntile[0]}, {1, t.ntile[1]}, {2, n2 / outer}, {3, t.ntile[3]}, {2, outer}};
+    };
+    switch (raster) {
+    case 1: split2(2); break;
+    case 2: split2(4); break;
+    case 3: digits = {{3, t.ntile[3]}, {0, t.ntile[0]}, {1, t.ntile[1]}, {2, t.ntile[2]}}; break;
+    default: digits = {{0, t.ntile[0]}, {1, t.ntile[1]}, {2, t.ntile[2]}, {3, t.ntile[3]}}; break;
+    }
+    tab.resize((size_t)t.ntiles);
+    for (int id = 0; id < t.ntiles; id++) {
+        int c[4] = {0, 0, 0, 0}, mult[4] = {1, 1, 1, 1};
+        int r = id;
+        for (const Digit &d : digits) {
+            c[d.dim] += (r % d.count) * mult[d.dim];
+            mult[d.dim] *= d.count;
+            r /= d.count;
+        }
+        tab[(size_t)id] = make_int4(c[0] << t.sh[0], c[1] << t.sh[1], c[2] << t.sh[2], c[3] << t.sh[3]);
+    }
+}
+
+static void make_tiling(const dwf_geometry *g, bool cb, Tiling &t)
+{
+    const Lattice &lat = g->lat;
+    const int ext[4] = {cb ? lat.Lh : lat.L[0], lat.L[1], lat.L[2], lat.L[3]};
+    int sites = 1;
+    for (int d = 0; d < 4; d++) {
+        int want = g->opt_tile[d];
+        if (!cb && d == 0) want += 1;            // same x0 span as the checkerboard tile
+        t.sh[d] = fit_shift(ext[d], want);
+        t.ntile[d] = ext[d] >> t.sh[d];
+        sites <<= t.sh[d];
+    }
+    // keep the CTA within 256 threads: shrink the tile from the slowest direction
+    for (int d = 3; d >= 0 && sites > 256; d--)
+        while (t.sh[d] > 0 && sites > 256) { t.sh[d]--; t.ntile[d] <<= 1; sites >>= 1; }
+    int cpc = std::max(1, std::min(g->opt_cpc, 256 / sites));
+    while (lat.nchunk % cpc) cpc--;
+    t.cpc = cpc;
+    t.ncg = lat.nchunk / cpc;
+    t.threads = sites * cpc;
+    t.ntiles = t.ntile[0] * t.ntile[1] * t.ntile[2] * t.ntile[3];
+}
+
+int rebuild_tilings(dwf_geometry *g)
+{
+    for (int cb = 0; cb < 2; cb++) {
+        Tiling &t = cb ? g->tiling_cb : g->tiling_full;
+        int4 *&dev = cb ? g->tiles_cb : g->tiles_full;
+        make_tiling(g, cb != 0, t);
+        std::vector<int4> tab;
+        build_tile_table(t, g->opt_raster, tab);
+        if (dev) { cudaFree(dev); dev = nullptr; }
+        DWF_CUDA_CHECK(cudaMalloc(&dev, tab.size() * sizeof(int4)));
+        DWF_CUDA_CHECK(cudaMemcpy(dev, tab.data(), tab.size() * sizeof(int4), cudaMemcpyHostToDevice));
+    }
+    return DWF_OK;
+}
+
+static int ensure_staging(dwf_geometry *g, size_t bytes)
+{
+    if (g->staging_bytes >= bytes) return DWF_OK;
+    if (g->staging) { cudaFree(g->staging); g->staging = nullptr; g->staging_bytes = 0; }
+    if (cudaMalloc(&g->staging, bytes) != cudaSuccess) {
+        cudaGetLastError();
+        set_error("cannot allocate %zu bytes of device staging", bytes);
+        return DWF_ERR_ALLOC;
+    }
+    g->staging_bytes = bytes;
+    return DWF_OK;
+}
+
+static bool parity_ok(int p) { return p == DWF_FULL || p == DWF_EVEN || p == DWF_ODD; }
+static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
+}  // namespace dwf
+
+using namespace dwf;
+
+extern "C" {
+
+const char *dwf_error_string(int code)
+{
+    switch (code) {
+    case DWF_OK: return "success";
+    case DWF_ERR_INVALID_ARG: return "invalid argument";
+    case DWF_ERR_BAD_GEOMETRY: return "bad geometry";
+    case DWF_ERR_NO_GAUGE: return "gauge field not loaded";
+    case DWF_ERR_CUDA: return "CUDA error";
+    case DWF_ERR_ALLOC: return "allocation failed";
+    case DWF_ERR_UNSUPPORTED: return "unsupported";
+    }
+    return "unknown error code";
+}
+
+const char *dwf_last_error(void) { return t_err; }
+
+unsigned long long dwf_launch_count(void) { return g_launches.load(); }
+
+int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, int cuda_device, dwf_geometry **out)
+{
+    if (!dims || !out) { set_error("dwf_create_geometry: NULL argument"); return DWF_ERR_INVALID_ARG; }
+    if (precision != DWF_F32 && precision != DWF_F64) { set_error("precision must be 4 or 8"); return DWF_ERR_UNSUPPORTED; }
+    if (bc_time != DWF_PERIODIC && bc_time != DWF_ANTIPERIODIC_T) { set_error("bad bc_time"); return DWF_ERR_INVALID_ARG; }
+    if (Ls < 1) { set_error("Ls must be >= 1"); return DWF_ERR_BAD_GEOMETRY; }
+    long long V4 = 1;
+    for (int d = 0; d < 4; d++) {
+        if (dims[d] < 2 || (dims[d] & 1)) { set_error("extent %d is %d: must be even and >= 2", d, dims[d]); return DWF_ERR_BAD_GEOMETRY; }
+        V4 *= dims[d];
+        if (V4 > (1LL << 30)) { set_error("4D volume too large"); return DWF_ERR_BAD_GEOMETRY; }
+    }
+    if ((double)V4 * Ls * 12 >= 2147483647.0) { set_error("5D field exceeds 2^31 complex elements"); return DWF_ERR_BAD_GEOMETRY; }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || cuda_device < 0 || cuda_device >= ndev) {
+        cudaGetLastError();
+        set_error("CUDA device %d not available (%d devices)", cuda_device, ndev);
+        return DWF_ERR_CUDA;
+    }
+    DeviceGuard guard(cuda_device);
+    if (!guard.ok) { set_error("cannot select CUDA device %d", cuda_device); return DWF_ERR_CUDA; }
+
+    dwf_geometry *g = new (std::nothrow) dwf_geometry();
+    if (!g) return DWF_ERR_ALLOC;
+    memset(g, 0, sizeof(*g));
+    for (int d = 0; d < 4; d++) g->lat.L[d] = dims[d];
+    g->lat.Lh = dims[0] / 2;
+    g->lat.Ls = Ls;
+    g->lat.V4 = V4;
+    g->lat.Vh = V4 / 2;
+    // s-slices per thread: two complex per 128-bit load in fp32, one in fp64
+    int sc = (precision == DWF_F32) ? 2 : 1;
+    while (Ls % sc) sc >>= 1;
+    g->lat.Sc = sc;
+    g->lat.nchunk = Ls / sc;
+    g->prec = precision;
+    g->bc_time = bc_time;
+    g->device = cuda_device;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) { delete g; set_error("cudaGetDeviceProperties failed"); return DWF_ERR_CUDA; }
+    g->sm_count = prop.multiProcessorCount;
+    g->opt_tile[0] = 2; g->opt_tile[1] = 2; g->opt_tile[2] = 1; g->opt_tile[3] = 1;
+    g->opt_cpc = 4;
+    g->opt_raster = 0;
+    g->opt_variant = 0;
+
+    g->gauge_bytes = (size_t)8 * 18 * (size_t)g->lat.Vh * (size_t)precision;
+    g->reduce_blocks = g->sm_count * 8;
+    bool ok = cudaMalloc(&g->gauge[0], g->gauge_bytes) == cudaSuccess &&
+              cudaMalloc(&g->gauge[1], g->gauge_bytes) == cudaSuccess &&
+              cudaMalloc(&g->partials, sizeof(double) * 2 * (size_t)g->reduce_blocks) == cudaSuccess &&
+              cudaMalloc(&g->result_dev, sizeof(double) * 2) == cudaSuccess;
+    if (!ok || rebuild_tilings(g) != DWF_OK) {
+        cudaGetLastError();
+        if (ok == false) set_error("device allocation failed (gauge %zu bytes x 2)", g->gauge_bytes);
+        dwf_destroy_geometry(g);
+        return ok ? DWF_ERR_CUDA : DWF_ERR_ALLOC;
+    }
+    *out = g;
+    return DWF_OK;
+}
+
+int dwf_destroy_geometry(dwf_geometry *g)
+{
+    if (!g) return DWF_OK;
+    DeviceGuard guard(g->device);
+    cudaFree(g->gauge[0]);
+    cudaFree(g->gauge[1]);
+    cudaFree(g->partials);
+    cudaFree(g->result_dev);
+    cudaFree(g->tiles_cb);
+    cudaFree(g->tiles_full);
+    cudaFree(g->staging);
+    cudaGetLastError();
+    delete g;
+    return DWF_OK;
+}
+
+int dwf_set_option(dwf_geometry *g, const char *key, long long value)
+{
+    if (!g || !key) { set_error("dwf_set_option: NULL argument"); return DWF_ERR_INVALID_ARG; }
+    DeviceGuard guard(g->device);
+    int v = (int)value;
+    if (!strcmp(key, "tile0") || !strcmp(key, "tile1") || !strcmp(key, "tile2") || !strcmp(key, "tile3")) {
+        if (v < 0 || v > 8) { set_error("tile exponent out of range"); return DWF_ERR_INVALID_ARG; }
+        g->opt_tile[key[4] - '0'] = v;
+    } else if (!strcmp(key, "cpc")) {
+        if (v < 1) { set_error("cpc must be >= 1"); return DWF_ERR_INVALID_ARG; }
+        g->opt_cpc = v;
+    } else if (!strcmp(key, "raster")) {
+        g->opt_raster = v;
+    } else if (!strcmp(key, "variant")) {
+        g->opt_variant = v;
+        return DWF_OK;
+    } else {
+        set_error("unknown option '%s'", key);
+        return DWF_ERR_UNSUPPORTED;
+    }
+    return rebuild_tilings(g);
+}
+
+size_t dwf_field_bytes(const dwf_geometry *g, int parity)
+{
+    if (!g || !parity_ok(parity)) return 0;
+    const long long nsites = (parity == DWF_FULL) ? g->lat.V4 : g->lat.Vh;
+    return (size_t)nsites * (size_t)g->lat.Ls * 24 * (size_t)g->prec;
+}
+
+int dwf_layout_sc(const dwf_geometry *g) { return g ? g->lat.Sc : 0; }
+
+int dwf_load_gauge(dwf_geometry *g, const void *U, int src_is_device, void *stream)
+{
+    if (!g || !U) { set_error("dwf_load_gauge: NULL argument"); return DWF_ERR_INVALID_ARG; }
+    DeviceGuard guard(g->device);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t bytes = (size_t)g->lat.V4 * 72 * (size_t)g->prec;
+    const void *src = U;
+    if (!src_is_device) {
+        int rc = ensure_staging(g, bytes);
+        if (rc) return rc;
+        DWF_CUDA_CHECK(cudaMemcpyAsync(g->staging, U, bytes, cudaMemcpyHostToDevice, st));
+        src = g->staging;
+    }
+    int rc = launch_pack_gauge(g, src, st);
+    if (rc) return rc;
+    DWF_CUDA_CHECK(cudaStreamSynchronize(st));
+    g->gauge_loaded = true;
+    return DWF_OK;
+}
+
+static int dhop_common(const dwf_geometry *g, const void *in, void *out, int parity_out, void *stream, const char *who)
+{
+    if (!g || !in || !out) { set_error("%s: NULL argument", who); return DWF_ERR_INVALID_ARG; }
+    if (in == out) { set_error("%s: in-place application is not defined (in == out)", who); return DWF_ERR_INVALID_ARG; }
+    if (!aligned16(in) || !aligned16(out)) { set_error("%s: field pointers must be 16-byte aligned", who); return DWF_ERR_INVALID_ARG; }
+    if (!g->gauge_loaded) { set_error("%s: call dwf_load_gauge first", who); return DWF_ERR_NO_GAUGE; }
+    DeviceGuard guard(g->device);
+    return launch_dhop(g, in, out, parity_out, static_cast<cudaStream_t>(stream));
+}
+
+int dwf_dhop(const dwf_geometry *g, const void *in_full, void *out_full, void *stream)
+{
+    return dhop_common(g, in_full, out_full, DWF_FULL, stream, "dwf_dhop");
+}
+int dwf_dhop_oe(const dwf_geometry *g, const void *in_even, void *out_odd, void *stream)
+{
+    return dhop_common(g, in_even, out_odd, DWF_ODD, stream, "dwf_dhop_oe");
+}
+int dwf_dhop_eo(const dwf_geometry *g, const void *in_odd, void *out_even, void *stream)
+{
+    return dhop_common(g, in_odd, out_even, DWF_EVEN, stream, "dwf_dhop_eo");
+}
+
+int dwf_norm2(const dwf_geometry *g, const void *field, int parity, double *result_host, void *stream)
+{
+    if (!g || !field || !result_host || !parity_ok(parity)) { set_error("dwf_norm2: bad argument"); return DWF_ERR_INVALID_ARG; }
+    if (!aligned16(field)) { set_error("dwf_norm2: field must be 16-byte aligned"); return DWF_ERR_INVALID_ARG; }
+    DeviceGuard guard(g->device);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int rc = launch_norm2(g, field, dwf_field_bytes(g, parity) / (size_t)g->prec, st);
+    if (rc) return rc;
+    double r = 0;
+    DWF_CUDA_CHECK(cudaMemcpyAsync(&r, g->result_dev, sizeof(double), cudaMemcpyDeviceToHost, st));
+    DWF_CUDA_CHECK(cudaStreamSynchronize(st));
+    *result_host = r;
+    return DWF_OK;
+}
+
+int dwf_inner_product(const dwf_geometry *g, const void *a, const void *b, int parity, double result_host[2], void *stream)
+{
+    if (!g || !a || !b || !result_host || !parity_ok(parity)) { set_error("dwf_inner_product: bad argument"); return DWF_ERR_INVALID_ARG; }
+    if (!aligned16(a) || !aligned16(b)) { set_error("dwf_inner_product: fields must be 16-byte aligned"); return DWF_ERR_INVALID_ARG; }
+    DeviceGuard guard(g->device);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int rc = launch_inner(g, a, b, dwf_field_bytes(g, parity) / (size_t)g->prec / 2, st);
+    if (rc) return rc;
+    double r[2] = {0, 0};
+    DWF_CUDA_CHECK(cudaMemcpyAsync(r, g->result_dev, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    DWF_CUDA_CHECK(cudaStreamSynchronize(st));
+    result_host[0] = r[0];
+    result_host[1] = r[1];
+    return DWF_OK;
+}
+
+int dwf_import_spinor(const dwf_geometry *g, const void *canonical, int src_is_device, int parity, void *field_dev, void *stream)
+{
+    if (!g || !canonical || !field_dev || !parity_ok(parity)) { set_error("dwf_import_spinor: bad argument"); return DWF_ERR_INVALID_ARG; }
+    if (!aligned16(field_dev) || (src_is_device && !aligned16(canonical))) { set_error("dwf_import_spinor: device pointers must be 16-byte aligned"); return DWF_ERR_INVALID_ARG; }
+    if (canonical == field_dev) { set_error("dwf_import_spinor: in-place conversion not supported"); return DWF_ERR_INVALID_ARG; }
+    DeviceGuard guard(g->device);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t bytes = dwf_field_bytes(g, parity);
+    const void *src = canonical;
+    if (!src_is_device) {
+        int rc = ensure_staging(const_cast<dwf_geometry *>(g), bytes);
+        if (rc) return rc;
+        DWF_CUDA_CHECK(cudaMemcpyAsync(g->staging, canonical, bytes, cudaMemcpyHostToDevice, st));
+        src = g->staging;
+    }
+    int rc = launch_import(g, src, parity, field_dev, st);
+    if (rc) return rc;
+    if (!src_is_device) DWF_CUDA_CHECK(cudaStreamSynchronize(st));
+    return DWF_OK;
+}
+
+int dwf_export_spinor(const dwf_geometry *g, const void *field_dev, int parity, void *canonical, int dst_is_device, void *stream)
+{
+    if (!g || !canonical || !field_dev || !parity_ok(parity)) { set_error("dwf_export_spinor: bad argument"); return DWF_ERR_INVALID_ARG; }
+    if (!aligned16(field_dev) || (dst_is_device && !aligned16(canonical))) { set_error("dwf_export_spinor: device pointers must be 16-byte aligned"); return DWF_ERR_INVALID_ARG; }
+    if (canonical == field_dev) { set_error("dwf_export_spinor: in-place conversion not supported"); return DWF_ERR_INVALID_ARG; }
+    DeviceGuard guard(g->device);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t bytes = dwf_field_bytes(g, parity);
+    if (dst_is_device) return launch_export(g, field_dev, parity, canonical, st);
+    int rc = ensure_staging(const_cast<dwf_geometry *>(g), bytes);
+    if (rc) return rc;
+    rc = launch_export(g, field_dev, parity, g->staging, st);
+    if (rc) return rc;
+    DWF_CUDA_CHECK(cudaMemcpyAsync(canonical, g->staging, bytes, cudaMemcpyDeviceToHost, st));
+    DWF_CUDA_CHECK(cudaStreamSynchronize(st));
+    return DWF_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,253 @@
+// dhop.cu -- the Dhop kernels (hot path rows a2-a6 of SURVEY.md section 8).
+//
+//   Dhop psi(x,s) = sum_mu [ (1-gamma_mu) U_mu(x) psi(x+mu,s) + (1+gamma_mu) U_mu^dag(x-mu) psi(x-mu,s) ]
+//
+// One thread owns one output 4D site and SC consecutive s-slices.  For each of the 8 legs it
+//   (a2) computes the neighbour's site index (periodic wrap; checkerboard x0 rule),
+//   (a3) loads the neighbour spinor (12 complex x SC, 128-bit loads) and projects it with
+//        (1 -/+ gamma_mu) to a half spinor (2 spins x 3 colours),
+//   (a4) loads the link for this leg ONCE and multiplies it into the SC half spinors,
+//   (a5) reconstructs the lower two spin components and accumulates in registers,
+// then writes the 12 x SC complex results with streaming stores.  Backward links are stored
+// pre-daggered and carry the antiperiodic sign, so all 8 legs run the same mat-vec.
+//
+// Projection / reconstruction in the DeGrand-Rossi basis (derived from gamma (1 +/- gamma) =
+// +/-(1 +/- gamma); rows 0,1 of (1 + e gamma_mu) psi are h0,h1, rows 2,3 follow from them):
+//   mu=x: h0 = psi0 + e i psi3, h1 = psi1 + e i psi2, r2 = -e i h1, r3 = -e i h0
+//   mu=y: h0 = psi0 - e   psi3, h1 = psi1 + e   psi2, r2 =  e   h1, r3 = -e   h0
+//   mu=z: h0 = psi0 + e i psi2, h1 = psi1 - e i psi3, r2 = -e i h0, r3 =  e i h1
+//   mu=t: h0 = psi0 + e   psi2, h1 = psi1 + e   psi3, r2 =  e   h0, r3 =  e   h1
+// with e = -1 on the forward leg (x+mu) and e = +1 on the backward leg (x-mu).
+#include "complex_ops.cuh"
+#include "dwf_internal.cuh"
+
+namespace dwf {
+
+// gauge storage: per leg 9 complex planes over the Vh output sites of one parity
+template <typename T> struct LinkIO;
+template <> struct LinkIO<float> {
+    // planes are paired into float4 (complex 2v, 2v+1), the ninth complex is a float2 tail
+    static __device__ __forceinline__ void load(const float *leg, long long Vh, int site, float2 (&U)[9])
+    {
+#pragma unroll
+        for (int v = 0; v < 4; v++) {
+            float4 q = __ldg(reinterpret_cast<const float4 *>(leg + (size_t)v * 4 * Vh) + site);
+            U[2 * v] = make_float2(q.x, q.y);
+            U[2 * v + 1] = make_float2(q.z, q.w);
+        }
+        U[8] = __ldg(reinterpret_cast<const float2 *>(leg + (size_t)16 * Vh) + site);
+    }
+};
+template <> struct LinkIO<double> {
+    static __device__ __forceinline__ void load(const double *leg, long long Vh, int site, double2 (&U)[9])
+    {
+#pragma unroll
+        for (int v = 0; v < 9; v++)
+            U[v] = __ldg(reinterpret_cast<const double2 *>(leg + (size_t)v * 2 * Vh) + site);
+    }
+};
+
+// one leg: acc += reconstruct( U * project(psi_neighbour) )
+template <typename T, int SC, int MU, bool FWD, bool FIRST>
+__device__ __forceinline__ void dhop_leg(typename CxT<T>::type (&acc)[12][SC],
+                                         const typename CxT<T>::type *__restrict__ nb,  // neighbour, component 0
+                                         size_t kstride,                                // complex elements between components
+                                         const T *__restrict__ leg_links, long long Vh, int gsite)
+{
+    using C = typename CxT<T>::type;
+    C psi[12][SC];
+#pragma unroll
+    for (int k = 0; k < 12; k++) load_cx<SC>(nb + (size_t)k * kstride, psi[k]);
+    C U[9];
+    LinkIO<T>::load(leg_links, Vh, gsite, U);
+
+#pragma unroll
+    for (int j = 0; j < SC; j++) {
+        C h0[3], h1[3];
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            const C p0 = psi[0 + c][j], p1 = psi[3 + c][j], p2 = psi[6 + c][j], p3 = psi[9 + c][j];
+            if constexpr (MU == 0) {
+                h0[c] = FWD ? csubi(p0, p3) : caddi(p0, p3);
+                h1[c] = FWD ? csubi(p1, p2) : caddi(p1, p2);
+            } else if constexpr (MU == 1) {
+                h0[c] = FWD ? cadd(p0, p3) : csub(p0, p3);
+                h1[c] = FWD ? csub(p1, p2) : cadd(p1, p2);
+            } else if constexpr (MU == 2) {
+                h0[c] = FWD ? csubi(p0, p2) : caddi(p0, p2);
+                h1[c] = FWD ? caddi(p1, p3) : csubi(p1, p3);
+            } else {
+                h0[c] = FWD ? csub(p0, p2) : cadd(p0, p2);
+                h1[c] = FWD ? csub(p1, p3) : cadd(p1, p3);
+            }
+        }
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            C x0 = cmul(U[3 * a], h0[0]);
+            x0 = cmac(x0, U[3 * a + 1], h0[1]);
+            x0 = cmac(x0, U[3 * a + 2], h0[2]);
+            C x1 = cmul(U[3 * a], h1[0]);
+            x1 = cmac(x1, U[3 * a + 1], h1[1]);
+            x1 = cmac(x1, U[3 * a + 2], h1[2]);
+            // rows 2,3 as multiples of x0/x1: value = sgn * (i?) * x
+            if constexpr (FIRST) {
+                acc[0 + a][j] = x0;
+                acc[3 + a][j] = x1;
+                if constexpr (MU == 0) {
+                    acc[6 + a][j] = FWD ? cmuli(x1) : cmulni(x1);
+                    acc[9 + a][j] = FWD ? cmuli(x0) : cmulni(x0);
+                } else if constexpr (MU == 1) {
+                    acc[6 + a][j] = FWD ? cneg(x1) : x1;
+                    acc[9 + a][j] = FWD ? x0 : cneg(x0);
+                } else if constexpr (MU == 2) {
+                    acc[6 + a][j] = FWD ? cmuli(x0) : cmulni(x0);
+                    acc[9 + a][j] = FWD ? cmulni(x1) : cmuli(x1);
+                } else {
+                    acc[6 + a][j] = FWD ? cneg(x0) : x0;
+                    acc[9 + a][j] = FWD ? cneg(x1) : x1;
+                }
+            } else {
+                acc[0 + a][j] = cadd(acc[0 + a][j], x0);
+                acc[3 + a][j] = cadd(acc[3 + a][j], x1);
+                if constexpr (MU == 0) {
+                    acc[6 + a][j] = FWD ? caddi(acc[6 + a][j], x1) : csubi(acc[6 + a][j], x1);
+                    acc[9 + a][j] = FWD ? caddi(acc[9 + a][j], x0) : csubi(acc[9 + a][j], x0);
+                } else if constexpr (MU == 1) {
+                    acc[6 + a][j] = FWD ? csub(acc[6 + a][j], x1) : cadd(acc[6 + a][j], x1);
+                    acc[9 + a][j] = FWD ? cadd(acc[9 + a][j], x0) : csub(acc[9 + a][j], x0);
+                } else if constexpr (MU == 2) {
+                    acc[6 + a][j] = FWD ? caddi(acc[6 + a][j], x0) : csubi(acc[6 + a][j], x0);
+                    acc[9 + a][j] = FWD ? csubi(acc[9 + a][j], x1) : caddi(acc[9 + a][j], x1);
+                } else {
+                    acc[6 + a][j] = FWD ? csub(acc[6 + a][j], x0) : cadd(acc[6 + a][j], x0);
+                    acc[9 + a][j] = FWD ? csub(acc[9 + a][j], x1) : cadd(acc[9 + a][j], x1);
+                }
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// direct kernel: neighbours are read straight from global memory (L1/L2 catch the reuse).
+// CB = true : in/out are half fields; out has parity `parity_out`, in the opposite parity.
+// CB = false: in/out are full fields (lexicographic sites); the links of site x live in the
+//             gauge set of x's parity at index x>>1.
+// ---------------------------------------------------------------------------------------------
+template <typename T, int SC, bool CB, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB)
+dhop_direct_kernel(const typename CxT<T>::type *__restrict__ in, typename CxT<T>::type *__restrict__ out,
+                   const T *__restrict__ gauge_even, const T *__restrict__ gauge_odd,
+                   const int4 *__restrict__ tiles, const Lattice lat, const Tiling til, const int parity_out)
+{
+    using C = typename CxT<T>::type;
+    const int nsh = til.sh[0] + til.sh[1] + til.sh[2] + til.sh[3];
+    const int tid = threadIdx.x;
+    const int ls = tid & ((1 << nsh) - 1);
+    const int chunk = (blockIdx.x % til.ncg) * til.cpc + (tid >> nsh);
+    const int4 org = tiles[blockIdx.x / til.ncg];
+
+    int l = ls;
+    const int c0 = org.x + (l & ((1 << til.sh[0]) - 1)); l >>= til.sh[0];
+    const int x1 = org.y + (l & ((1 << til.sh[1]) - 1)); l >>= til.sh[1];
+    const int x2 = org.z + (l & ((1 << til.sh[2]) - 1)); l >>= til.sh[2];
+    const int x3 = org.w + l;
+
+    const int L1 = lat.L[1], L2 = lat.L[2], L3 = lat.L[3];
+    const int W0 = CB ? lat.Lh : lat.L[0];           // row length in field sites
+    const long long Vs = CB ? lat.Vh : lat.V4;       // sites per field
+    const size_t kstride = (size_t)Vs * SC;
+
+    const int row = x1 + L1 * (x2 + L2 * x3);
+    const int site = c0 + W0 * row;
+
+    // gauge set and index
+    int par, gsite;
+    if constexpr (CB) { par = parity_out; gsite = site; }
+    else { par = (c0 + x1 + x2 + x3) & 1; gsite = site >> 1; }
+    const T *gset = par ? gauge_odd : gauge_even;
+    const long long Vh = lat.Vh;
+
+    // neighbour site indices
+    int n0p, n0m;
+    if constexpr (CB) {
+        const int r = (x1 + x2 + x3 + parity_out) & 1;      // x0 = 2*c0 + r
+        int hp = c0 + r;       if (hp == W0) hp = 0;
+        int hm = c0 - 1 + r;   if (hm < 0) hm = W0 - 1;
+        n0p = hp + W0 * row;
+        n0m = hm + W0 * row;
+    } else {
+        n0p = (c0 + 1 == W0 ? 0 : c0 + 1) + W0 * row;
+        n0m = (c0 == 0 ? W0 - 1 : c0 - 1) + W0 * row;
+    }
+    const int s1 = W0, s2 = W0 * L1, s3 = W0 * L1 * L2;
+    const int n1p = site + (x1 + 1 == L1 ? -(L1 - 1) * s1 : s1);
+    const int n1m = site + (x1 == 0 ? (L1 - 1) * s1 : -s1);
+    const int n2p = site + (x2 + 1 == L2 ? -(L2 - 1) * s2 : s2);
+    const int n2m = site + (x2 == 0 ? (L2 - 1) * s2 : -s2);
+    const int n3p = site + (x3 + 1 == L3 ? -(L3 - 1) * s3 : s3);
+    const int n3m = site + (x3 == 0 ? (L3 - 1) * s3 : -s3);
+
+    const C *base = in + (size_t)chunk * 12 * kstride;
+    const size_t lstride = (size_t)18 * Vh;          // reals per leg
+
+    C acc[12][SC];
+    dhop_leg<T, SC, 0, true,  true >(acc, base + (size_t)n0p * SC, kstride, gset + 0 * lstride, Vh, gsite);
+    dhop_leg<T, SC, 0, false, false>(acc, base + (size_t)n0m * SC, kstride, gset + 1 * lstride, Vh, gsite);
+    dhop_leg<T, SC, 1, true,  false>(acc, base + (size_t)n1p * SC, kstride, gset + 2 * lstride, Vh, gsite);
+    dhop_leg<T, SC, 1, false, false>(acc, base + (size_t)n1m * SC, kstride, gset + 3 * lstride, Vh, gsite);
+    dhop_leg<T, SC, 2, true,  false>(acc, base + (size_t)n2p * SC, kstride, gset + 4 * lstride, Vh, gsite);
+    dhop_leg<T, SC, 2, false, false>(acc, base + (size_t)n2m * SC, kstride, gset + 5 * lstride, Vh, gsite);
+    dhop_leg<T, SC, 3, true,  false>(acc, base + (size_t)n3p * SC, kstride, gset + 6 * lstride, Vh, gsite);
+    dhop_leg<T, SC, 3, false, false>(acc, base + (size_t)n3m * SC, kstride, gset + 7 * lstride, Vh, gsite);
+
+    C *o = out + (size_t)chunk * 12 * kstride + (size_t)site * SC;
+#pragma unroll
+    for (int k = 0; k < 12; k++) store_cx<SC>(o + (size_t)k * kstride, acc[k]);
+}
+
+template <typename T, int SC, bool CB, int MAXT, int MINB>
+static int launch_direct(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st)
+{
+    using C = typename CxT<T>::type;
+    const Tiling &til = CB ? g->tiling_cb : g->tiling_full;
+    const int4 *tiles = CB ? g->tiles_cb : g->tiles_full;
+    if (til.threads > MAXT) {
+        set_error("tile of %d threads exceeds kernel limit %d", til.threads, MAXT);
+        return DWF_ERR_UNSUPPORTED;
+    }
+    dim3 grid((unsigned)(til.ntiles * til.ncg)), block((unsigned)til.threads);
+    dhop_direct_kernel<T, SC, CB, MAXT, MINB><<<grid, block, 0, st>>>(
+        static_cast<const C *>(in), static_cast<C *>(out), static_cast<const T *>(g->gauge[0]),
+        static_cast<const T *>(g->gauge[1]), tiles, g->lat, til, parity_out);
+    count_launch();
+    DWF_CUDA_CHECK(cudaGetLastError());
+    return DWF_OK;
+}
+
+template <typename T, bool CB>
+static int dispatch_sc(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st)
+{
+    constexpr bool F32 = sizeof(T) == 4;
+    switch (g->lat.Sc) {
+    case 1: return launch_direct<T, 1, CB, 256, F32 ? 3 : 2>(g, in, out, parity_out, st);
+    case 2: return launch_direct<T, 2, CB, 256, F32 ? 2 : 1>(g, in, out, parity_out, st);
+    case 4:
+        if constexpr (F32) return launch_direct<T, 4, CB, 256, 1>(g, in, out, parity_out, st);
+        break;
+    }
+    set_error("unsupported Sc=%d for precision %d", g->lat.Sc, (int)sizeof(T));
+    return DWF_ERR_UNSUPPORTED;
+}
+
+// parity_out: DWF_FULL, DWF_EVEN (DhopEO), DWF_ODD (DhopOE)
+int launch_dhop(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st)
+{
+    if (g->prec == DWF_F32) {
+        if (parity_out == DWF_FULL) return dispatch_sc<float, false>(g, in, out, 0, st);
+        return dispatch_sc<float, true>(g, in, out, parity_out, st);
+    }
+    if (parity_out == DWF_FULL) return dispatch_sc<double, false>(g, in, out, 0, st);
+    return dispatch_sc<double, true>(g, in, out, parity_out, st);
+}
+
+}  // namespace dwf

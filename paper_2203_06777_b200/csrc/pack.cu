@@ -1,0 +1,142 @@
+// pack.cu -- canonical <-> device layout conversion (hot path row a1 of SURVEY.md section 8).
+//
+// Spinor: canonical [site][s][k][reim]  <->  device complex[chunk][k][site][j], s = chunk*Sc + j.
+// Gauge : canonical [x][mu][a][b][reim]  ->  for each output parity p and each output site of that
+//         parity (cb index x>>1) the 8 links that site multiplies with:
+//            leg 2*mu   : U_mu(x)                       (forward hop,  psi(x+mu))
+//            leg 2*mu+1 : U_mu(x-mu)^dagger             (backward hop, psi(x-mu))
+//         each times -1 when the hop wraps around an antiperiodic time direction, stored planar
+//         over sites as [leg][9 complex planes][cb site] (fp32: planes paired into float4 + a
+//         float2 tail; fp64: double2 planes).  Every canonical link appears exactly once in each
+//         parity set, so one half-Dhop still reads the whole gauge field exactly once.
+#include "dwf_internal.cuh"
+
+namespace dwf {
+
+template <typename T, bool IMPORT>
+__global__ void __launch_bounds__(256)
+spinor_reorder_kernel(const T *__restrict__ src, T *__restrict__ dst, long long nsites, int Ls, int Sc)
+{
+    // one thread per complex element of the DEVICE layout (coalesced on the device side)
+    const long long n = nsites * Ls * 12;
+    const int nchunk = Ls / Sc;
+    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n;
+         e += (long long)gridDim.x * blockDim.x) {
+        long long r = e;
+        const int j = (int)(r % Sc); r /= Sc;
+        const long long site = r % nsites; r /= nsites;
+        const int k = (int)(r % 12);
+        const int chunk = (int)(r / 12);
+        (void)nchunk;
+        const int s = chunk * Sc + j;
+        const long long c = ((site * Ls + s) * 12 + k);     // canonical complex index
+        using V = typename std::conditional<sizeof(T) == 4, float2, double2>::type;
+        if (IMPORT) reinterpret_cast<V *>(dst)[e] = reinterpret_cast<const V *>(src)[c];
+        else        reinterpret_cast<V *>(dst)[c] = reinterpret_cast<const V *>(src)[e];
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+gauge_pack_kernel(const T *__restrict__ U, T *__restrict__ set_even, T *__restrict__ set_odd,
+                  const Lattice lat, const int antiperiodic_t)
+{
+    // one thread per (lexicographic site x, leg)
+    const long long n = lat.V4 * 8;
+    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n;
+         e += (long long)gridDim.x * blockDim.x) {
+        const long long x = e % lat.V4;
+        const int leg = (int)(e / lat.V4);
+        const int mu = leg >> 1;
+        const bool bwd = leg & 1;
+        int c[4];
+        long long r = x;
+        c[0] = (int)(r % lat.L[0]); r /= lat.L[0];
+        c[1] = (int)(r % lat.L[1]); r /= lat.L[1];
+        c[2] = (int)(r % lat.L[2]); r /= lat.L[2];
+        c[3] = (int)r;
+        const int par = (c[0] + c[1] + c[2] + c[3]) & 1;
+        T *set = par ? set_odd : set_even;
+        const long long cb = x >> 1;
+
+        T sign = 1;
+        long long src_site = x;
+        if (bwd) {
+            int cm[4] = {c[0], c[1], c[2], c[3]};
+            cm[mu] = (c[mu] == 0) ? lat.L[mu] - 1 : c[mu] - 1;
+            src_site = cm[0] + (long long)lat.L[0] * (cm[1] + (long long)lat.L[1] * (cm[2] + (long long)lat.L[2] * cm[3]));
+            if (antiperiodic_t && mu == 3 && c[3] == 0) sign = -1;
+        } else {
+            if (antiperiodic_t && mu == 3 && c[3] == lat.L[3] - 1) sign = -1;
+        }
+        const T *u = U + (src_site * 4 + mu) * 18;
+        T *legbase = set + (size_t)leg * 18 * lat.Vh;
+#pragma unroll
+        for (int a = 0; a < 3; a++)
+#pragma unroll
+            for (int b = 0; b < 3; b++) {
+                T re, im;
+                if (bwd) { re = u[(b * 3 + a) * 2]; im = -u[(b * 3 + a) * 2 + 1]; }   // dagger
+                else     { re = u[(a * 3 + b) * 2]; im =  u[(a * 3 + b) * 2 + 1]; }
+                const int cidx = a * 3 + b;          // complex plane
+                size_t off;
+                if (sizeof(T) == 4) {
+                    // planes 0..7 paired into float4 vectors, plane 8 a float2 tail
+                    off = (cidx < 8) ? (size_t)(cidx >> 1) * 4 * lat.Vh + (size_t)cb * 4 + (cidx & 1) * 2
+                                     : (size_t)16 * lat.Vh + (size_t)cb * 2;
+                } else {
+                    off = (size_t)cidx * 2 * lat.Vh + (size_t)cb * 2;
+                }
+                legbase[off] = sign * re;
+                legbase[off + 1] = sign * im;
+            }
+    }
+}
+
+static int grid_for(long long n, int sm_count)
+{
+    long long b = (n + 255) / 256;
+    long long cap = (long long)sm_count * 16;
+    return (int)(b < cap ? (b < 1 ? 1 : b) : cap);
+}
+
+int launch_pack_gauge(const dwf_geometry *g, const void *U_dev, cudaStream_t st)
+{
+    const int grid = grid_for(g->lat.V4 * 8, g->sm_count);
+    if (g->prec == DWF_F32)
+        gauge_pack_kernel<float><<<grid, 256, 0, st>>>(static_cast<const float *>(U_dev), static_cast<float *>(g->gauge[0]),
+                                                      static_cast<float *>(g->gauge[1]), g->lat, g->bc_time == DWF_ANTIPERIODIC_T);
+    else
+        gauge_pack_kernel<double><<<grid, 256, 0, st>>>(static_cast<const double *>(U_dev), static_cast<double *>(g->gauge[0]),
+                                                       static_cast<double *>(g->gauge[1]), g->lat, g->bc_time == DWF_ANTIPERIODIC_T);
+    count_launch();
+    DWF_CUDA_CHECK(cudaGetLastError());
+    return DWF_OK;
+}
+
+template <bool IMPORT>
+static int launch_reorder(const dwf_geometry *g, const void *src, void *dst, int parity, cudaStream_t st)
+{
+    const long long nsites = (parity == DWF_FULL) ? g->lat.V4 : g->lat.Vh;
+    const int grid = grid_for(nsites * g->lat.Ls * 12, g->sm_count);
+    if (g->prec == DWF_F32)
+        spinor_reorder_kernel<float, IMPORT><<<grid, 256, 0, st>>>(static_cast<const float *>(src), static_cast<float *>(dst),
+                                                                  nsites, g->lat.Ls, g->lat.Sc);
+    else
+        spinor_reorder_kernel<double, IMPORT><<<grid, 256, 0, st>>>(static_cast<const double *>(src), static_cast<double *>(dst),
+                                                                   nsites, g->lat.Ls, g->lat.Sc);
+    count_launch();
+    DWF_CUDA_CHECK(cudaGetLastError());
+    return DWF_OK;
+}
+
+int launch_import(const dwf_geometry *g, const void *canonical_dev, int parity, void *field, cudaStream_t st)
+{
+    return launch_reorder<true>(g, canonical_dev, field, parity, st);
+}
+int launch_export(const dwf_geometry *g, const void *field, int parity, void *canonical_dev, cudaStream_t st)
+{
+    return launch_reorder<false>(g, field, canonical_dev, parity, st);
+}
+
+}  // namespace dwf

@@ -1,0 +1,140 @@
+// reduce.cu -- norm2 and inner product (hot path row a7 of SURVEY.md section 8; the paper's
+// accelerator_sum primitive, section 2.1).
+//
+// Two passes, both deterministic: (1) a fixed-size grid strides over the field with 128-bit
+// loads, accumulates in fp64 per thread, reduces with warp shuffles and one shared-memory step
+// to one partial per CTA; (2) a single CTA adds the partials in a fixed order.  The device
+// layout is a permutation of the canonical one, so the sum runs over the raw buffer.
+#include "dwf_internal.cuh"
+
+namespace dwf {
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// block-wide sum of NV values per thread; result valid in thread 0
+template <int NV>
+__device__ __forceinline__ void block_sum(double (&v)[NV], double *smem /* [NV][32] */)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+#pragma unroll
+    for (int i = 0; i < NV; i++) {
+        v[i] = warp_sum(v[i]);
+        if (lane == 0) smem[i * 32 + warp] = v[i];
+    }
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll
+        for (int i = 0; i < NV; i++) {
+            double t = (lane < nwarp) ? smem[i * 32 + lane] : 0.0;
+            v[i] = warp_sum(t);
+        }
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+norm2_partial_kernel(const T *__restrict__ x, size_t nreal, double *__restrict__ partials)
+{
+    __shared__ double smem[32];
+    constexpr int W = 16 / sizeof(T);                       // reals per 128-bit vector
+    using V = typename std::conditional<sizeof(T) == 4, float4, double2>::type;
+    const size_t nvec = nreal / W;
+    double acc[1] = {0.0};
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+        V q = __ldcs(reinterpret_cast<const V *>(x) + i);
+        if constexpr (sizeof(T) == 4) {
+            acc[0] += (double)q.x * q.x + (double)q.y * q.y;
+            acc[0] += (double)q.z * q.z + (double)q.w * q.w;
+        } else {
+            acc[0] += q.x * q.x + q.y * q.y;
+        }
+    }
+    // tail (nreal is a multiple of 24, so this never runs for fp32/fp64 fields; kept for safety)
+    if (blockIdx.x == 0 && threadIdx.x == 0)
+        for (size_t i = nvec * W; i < nreal; i++) acc[0] += (double)x[i] * (double)x[i];
+    block_sum<1>(acc, smem);
+    if (threadIdx.x == 0) partials[blockIdx.x] = acc[0];
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+inner_partial_kernel(const T *__restrict__ a, const T *__restrict__ b, size_t ncomplex, double *__restrict__ partials)
+{
+    __shared__ double smem[64];
+    using V = typename std::conditional<sizeof(T) == 4, float4, double2>::type;
+    constexpr int CW = 8 / sizeof(T);                       // complex numbers per 128-bit vector
+    const size_t nvec = ncomplex / CW;
+    double acc[2] = {0.0, 0.0};
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+        V p = __ldcs(reinterpret_cast<const V *>(a) + i);
+        V q = __ldcs(reinterpret_cast<const V *>(b) + i);
+        // conj(a) * b = (ar br + ai bi) + i (ar bi - ai br)
+        acc[0] += (double)p.x * q.x + (double)p.y * q.y;
+        acc[1] += (double)p.x * q.y - (double)p.y * q.x;
+        if constexpr (sizeof(T) == 4) {
+            acc[0] += (double)p.z * q.z + (double)p.w * q.w;
+            acc[1] += (double)p.z * q.w - (double)p.w * q.z;
+        }
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0)
+        for (size_t i = nvec * CW; i < ncomplex; i++) {
+            acc[0] += (double)a[2 * i] * b[2 * i] + (double)a[2 * i + 1] * b[2 * i + 1];
+            acc[1] += (double)a[2 * i] * b[2 * i + 1] - (double)a[2 * i + 1] * b[2 * i];
+        }
+    block_sum<2>(acc, smem);
+    if (threadIdx.x == 0) {
+        partials[2 * blockIdx.x] = acc[0];
+        partials[2 * blockIdx.x + 1] = acc[1];
+    }
+}
+
+// one CTA: result[i] = sum over blocks of partials[NV*block + i], fixed order
+template <int NV>
+__global__ void __launch_bounds__(256)
+final_sum_kernel(const double *__restrict__ partials, int nblocks, double *__restrict__ result)
+{
+    __shared__ double smem[NV * 32];
+    double acc[NV];
+#pragma unroll
+    for (int i = 0; i < NV; i++) acc[i] = 0.0;
+    for (int b = threadIdx.x; b < nblocks; b += blockDim.x)
+#pragma unroll
+        for (int i = 0; i < NV; i++) acc[i] += partials[NV * b + i];
+    block_sum<NV>(acc, smem);
+    if (threadIdx.x == 0)
+#pragma unroll
+        for (int i = 0; i < NV; i++) result[i] = acc[i];
+}
+
+int launch_norm2(const dwf_geometry *g, const void *field, size_t nreal, cudaStream_t st)
+{
+    const int nb = g->reduce_blocks;
+    if (g->prec == DWF_F32)
+        norm2_partial_kernel<float><<<nb, 256, 0, st>>>(static_cast<const float *>(field), nreal, g->partials);
+    else
+        norm2_partial_kernel<double><<<nb, 256, 0, st>>>(static_cast<const double *>(field), nreal, g->partials);
+    final_sum_kernel<1><<<1, 256, 0, st>>>(g->partials, nb, g->result_dev);
+    count_launch(2);
+    DWF_CUDA_CHECK(cudaGetLastError());
+    return DWF_OK;
+}
+
+int launch_inner(const dwf_geometry *g, const void *a, const void *b, size_t ncomplex, cudaStream_t st)
+{
+    const int nb = g->reduce_blocks;
+    if (g->prec == DWF_F32)
+        inner_partial_kernel<float><<<nb, 256, 0, st>>>(static_cast<const float *>(a), static_cast<const float *>(b), ncomplex, g->partials);
+    else
+        inner_partial_kernel<double><<<nb, 256, 0, st>>>(static_cast<const double *>(a), static_cast<const double *>(b), ncomplex, g->partials);
+    final_sum_kernel<2><<<1, 256, 0, st>>>(g->partials, nb, g->result_dev);
+    count_launch(2);
+    DWF_CUDA_CHECK(cudaGetLastError());
+    return DWF_OK;
+}
+
+}  // namespace dwf
