@@ -1,0 +1,390 @@
+#!/usr/bin/env python
+"""bench.py -- Dhop throughput on B200 (BASELINE.json metric: GFlop/s at 1320 flop per output
+5D site, and the fraction of the HBM roofline of the minimal-traffic model).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload c4]
+
+Workload at N=1: BASELINE.json configs[3] ("C4"): 32^4 x Ls=16, complex fp32, near-unit gauge
+(eps=0.2), Gaussian spinor on the even checkerboard.  One STEP = one red-black matvec as the
+config states it, plus the reduction of the hot path's last row:
+    chi_o = DhopOE psi_e ;  phi_e = DhopEO chi_o ;  n = norm2(phi_e) -> host (8 bytes)
+`value` counts 2 x 1320 x (V4/2 x Ls) flop per step (the norm2 flops are not counted).
+Inputs are resident in HBM before the timed region; fields are far larger than L2 (805 MB per
+half field, 604 MB of links), so no L2 flush is needed between iterations.
+
+`e2e` is the same step through the C ABI with HOST buffers: every step imports psi_e from
+pinned host memory (H2D + reorder), runs the three calls, and exports phi_e back to pinned
+host memory (reorder + D2H).
+
+`--impl reference` times the CPU oracle (oracle/, plain fp64 definition, OpenMP) on the host
+cores on the same workload; there is no other reference implementation (the paper ships none).
+
+Multi-GPU: the path does not shard (north_star: one GPU, no halo exchange) -- "replicas only":
+every rank runs the same workload on its own GPU, value = total sites / max time over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+FLOP_PER_SITE = 1320
+
+WORKLOADS = {
+    # name: dims, Ls, precision, bc_time, gauge kind, seed
+    "c3": dict(dims=(16, 16, 16, 16), Ls=16, prec=4, bc=0, gauge="random", seed=1003),
+    "c4": dict(dims=(32, 32, 32, 32), Ls=16, prec=4, bc=0, gauge="near_unit", seed=1004),
+    "c4d": dict(dims=(32, 32, 32, 32), Ls=16, prec=8, bc=0, gauge="near_unit", seed=1004),
+    "c5": dict(dims=(48, 48, 48, 96), Ls=12, prec=4, bc=1, gauge="random", seed=1005),
+    "tiny": dict(dims=(8, 8, 8, 8), Ls=8, prec=4, bc=1, gauge="random", seed=1002),
+}
+
+
+def workload_name(w):
+    d = w["dims"]
+    return (f"DWF even/odd Dhop {d[0]}x{d[1]}x{d[2]}x{d[3]} x Ls={w['Ls']} complex "
+            f"fp{w['prec'] * 8}, {w['gauge']} SU(3) gauge, DhopOE then DhopEO then norm2")
+
+
+def model_bytes_cb(w):
+    """Minimal-traffic model of ONE half-Dhop: one spinor read + one write per
+    output site, the whole gauge field once."""
+    d = w["dims"]
+    V4 = d[0] * d[1] * d[2] * d[3]
+    return (V4 // 2) * w["Ls"] * 48 * w["prec"] + V4 * 72 * w["prec"]
+
+
+def make_inputs(w):
+    import dwf_inputs as gen
+    d = w["dims"]
+    if w["gauge"] == "near_unit":
+        U = gen.gauge_near_unit(d, w["seed"], 0.2, prec=w["prec"])
+    else:
+        U = gen.gauge_random(d, w["seed"], prec=w["prec"])
+    psi_e = gen.spinor_gaussian(gen.volume(d) // 2, w["Ls"], w["seed"], prec=w["prec"])
+    return U, psi_e
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+            nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+            nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+            nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+            nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake",
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(0.005)
+
+    def start(self):
+        if self.nv:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def physical_gpu_index(local_rank):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+# ---------------------------------------------------------------------------------------------
+# the CPU oracle arm (cpu_baseline leg and --impl reference)
+# ---------------------------------------------------------------------------------------------
+def oracle_step(w, U, psi_e):
+    """One whole step of the workload on the host cores with the oracle as it stands."""
+    import oracle
+    d, Ls, bc = w["dims"], w["Ls"], w["bc"]
+    t0 = time.perf_counter()
+    chi_o = oracle.dhop_oe(d, Ls, bc, U, psi_e)
+    phi_e = oracle.dhop_eo(d, Ls, bc, U, chi_o)
+    n = oracle.norm2(phi_e)
+    return time.perf_counter() - t0, n
+
+
+def cpu_baseline(w, U, psi_e, steps=1):
+    import oracle
+    d = w["dims"]
+    sites = (d[0] * d[1] * d[2] * d[3] // 2) * w["Ls"]
+    runs = [oracle_step(w, U, psi_e) for _ in range(steps)]
+    best = min(r[0] for r in runs)
+    cpu_baseline.norm2 = runs[0][1]
+    return {"value": 2 * FLOP_PER_SITE * sites / best / 1e9, "unit": "GFlop/s",
+            "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"one whole step (DhopOE + DhopEO + norm2) of the same workload, {best:.2f} s, fp64"}
+
+
+def run_reference(args, w):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    U, psi_e = make_inputs(w)
+    d = w["dims"]
+    sites = (d[0] * d[1] * d[2] * d[3] // 2) * w["Ls"]
+    # each step is a bounded sample of the workload so that K steps end within minutes:
+    # a whole step when it is cheap, else the OE/EO pair at a seeded sample of output sites
+    probe, _ = oracle_step(w, U, psi_e)
+    budget = 120.0
+    whole = probe * (args.steps + args.warmup) <= budget
+    if whole:
+        for _ in range(max(0, args.warmup - 1)):
+            oracle_step(w, U, psi_e)
+        times = [oracle_step(w, U, psi_e)[0] for _ in range(args.steps)]
+        per_step_sites, sample = 2 * sites, "whole steps"
+    else:
+        import dwf_inputs as gen
+        par = gen.site_parity(d)
+        rng = np.random.default_rng(w["seed"])
+        n = max(1024, int(len(par) / 2 * budget / (probe * (args.steps + args.warmup))))
+        odd = rng.choice(np.nonzero(par == 1)[0], n, replace=False)
+        times = []
+        for i in range(args.warmup + args.steps):
+            t0 = time.perf_counter()
+            oracle.dhop_sites(d, w["Ls"], w["bc"], U, psi_e, True, odd)
+            if i >= args.warmup:
+                times.append(time.perf_counter() - t0)
+        per_step_sites, sample = n * w["Ls"], f"DhopOE at {n} sampled odd sites per step"
+    tot = sum(times)
+    val = FLOP_PER_SITE * per_step_sites * len(times) / tot / 1e9
+    line = {
+        "impl": "reference", "metric": "Dhop GFlop/s (1320 flop/5D site)", "value": val, "unit": "GFlop/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * tot / len(times), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(w), "note": "CPU oracle on host cores: " + sample},
+        "cpu_baseline": {"value": val, "unit": "GFlop/s", "cores": oracle.num_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": val, "unit": "GFlop/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------
+# the CUDA arm
+# ---------------------------------------------------------------------------------------------
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+# `ncu --set full` capture summarised under profiles/ (None until a capture exists).
+NCU_TRAFFIC_BYTES = {}
+
+
+def run_gpu(args, w):
+    import torch
+    import paper_2203_06777_b200 as dwf
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dwf.load()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    d, Ls, prec = w["dims"], w["Ls"], w["prec"]
+    V4 = d[0] * d[1] * d[2] * d[3]
+    sites = (V4 // 2) * Ls                          # output 5D sites of one half-Dhop
+    U, psi_e = make_inputs(w)
+
+    g = dwf.Geometry(d, Ls, prec, w["bc"], device=local_rank)
+    for kv in args.opt or []:
+        k, v = kv.split("=")
+        g.set_option(k, int(v))
+    g.load_gauge(U)
+    f_in = g.import_spinor(psi_e, dwf.EVEN)
+    f_mid, f_out = g.new_field(dwf.ODD), g.new_field(dwf.EVEN)
+
+    def step():
+        g.dhop_oe(f_in, f_mid)
+        g.dhop_eo(f_mid, f_out)
+        return g.norm2(f_out, dwf.EVEN)
+
+    for _ in range(args.warmup):
+        n_gpu = step()
+
+    # ---- timed region: K steps, device time, per-launch events on the launching stream ----
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    barrier()
+    sampler.start()
+    l0 = dwf.dwf_launch_count()
+    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_start.record()
+    for k in range(args.steps):
+        ev[k][0].record()
+        g.dhop_oe(f_in, f_mid)
+        ev[k][1].record()
+        g.dhop_eo(f_mid, f_out)
+        ev[k][2].record()
+        n_gpu = g.norm2(f_out, dwf.EVEN)
+        ev[k][3].record()
+    t_end.record()
+    barrier()
+    launches = dwf.dwf_launch_count() - l0
+    clocks = sampler.stop()
+    ms_total = max_over_ranks(t_start.elapsed_time(t_end))
+    ms_step = ms_total / args.steps
+    t_oe = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
+    t_eo = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
+    t_n2 = float(np.mean([e[2].elapsed_time(e[3]) for e in ev]))
+    value = world * 2 * FLOP_PER_SITE * sites / (ms_step * 1e-3) / 1e9
+
+    # ---- e2e: the same step through the C ABI with HOST buffers ----
+    host_in = torch.empty(psi_e.shape, dtype=torch.from_numpy(psi_e).dtype, pin_memory=True)
+    host_in.copy_(torch.from_numpy(psi_e))
+    host_out = torch.empty_like(host_in, pin_memory=True)
+    hin, hout = host_in.numpy(), host_out.numpy()
+
+    def step_e2e():
+        g.import_spinor(hin, dwf.EVEN, out=f_in)
+        g.dhop_oe(f_in, f_mid)
+        g.dhop_eo(f_mid, f_out)
+        g.export_spinor(f_out, dwf.EVEN, out=hout)
+        return g.norm2(f_out, dwf.EVEN)
+
+    k_e2e = max(1, min(args.steps, 10))
+    for _ in range(2):
+        step_e2e()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(k_e2e):
+        n_e2e = step_e2e()
+    e1.record()
+    barrier()
+    ms_e2e = max_over_ranks(e0.elapsed_time(e1)) / k_e2e
+    e2e_val = world * 2 * FLOP_PER_SITE * sites / (ms_e2e * 1e-3) / 1e9
+    field_bytes = psi_e.nbytes
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    peak, peak_src = peaks()
+    t_dhop = 0.5 * (t_oe + t_eo)
+    mb = model_bytes_cb(w)
+    achieved = mb / (t_dhop * 1e-3) / 1e9
+    line = {
+        "metric": "Dhop GFlop/s (1320 flop/5D site)", "value": value, "unit": "GFlop/s",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if prec == 4 else "f64", "data": "synthetic",
+        "config": {"workload": workload_name(w), "name": args.workload, "dims": list(d), "Ls": Ls,
+                   "l2": "inputs larger than L2 (805 MB half fields, 604 MB links); no flush",
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "layout_sc": dwf.dwf_layout_sc(g.handle)},
+        "clocks": clocks,
+        "e2e": {"value": e2e_val, "unit": "GFlop/s", "ms_per_step": ms_e2e,
+                "h2d_bytes_per_step": field_bytes, "d2h_bytes_per_step": field_bytes + 8},
+        "gpu_launches": int(launches),
+        "kernels_ms": {"dhop_oe": t_oe, "dhop_eo": t_eo, "norm2": t_n2},
+        "dhop_only_gflops": FLOP_PER_SITE * sites / (t_dhop * 1e-3) / 1e9,
+        "roofline": {"bound": "hbm", "kernel": "dhop (even/odd)", "achieved": achieved, "peak": peak,
+                     "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": mb,
+                     "traffic": NCU_TRAFFIC_BYTES.get(args.workload)},
+    }
+    if world == 1 and not args.no_cpu:
+        cb = cpu_baseline(w, U, psi_e)
+        line["cpu_baseline"] = cb
+        # free full-size sanity check: norm2 of the step's result, CUDA path (fp32/fp64) vs oracle (fp64)
+        line["check"] = {"norm2_gpu": n_gpu, "norm2_oracle": cpu_baseline.norm2,
+                         "rel_diff": abs(n_gpu - cpu_baseline.norm2) / cpu_baseline.norm2}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="dwf", choices=["dwf", "reference"])
+    ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--opt", action="append", help="kernel tunable key=value (dwf_set_option)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "dwf" else args.warmup
+    w = WORKLOADS[args.workload]
+    if args.impl == "reference":
+        run_reference(args, w)
+    else:
+        run_gpu(args, w)
+
+
+if __name__ == "__main__":
+    main()
