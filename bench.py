@@ -344,8 +344,7 @@ def run_gpu(args, w):
         "dtype": "f32" if prec == 4 else "f64", "data": "synthetic",
         "config": {"workload": workload_name(w), "name": args.workload, "dims": list(d), "Ls": Ls,
                    "l2": "inputs larger than L2 (805 MB half fields, 604 MB links); no flush",
-                   "parallelism": "replicas only" if world > 1 else "single GPU",
-                   "layout_sc": dwf.dwf_layout_sc(g.handle)},
+                   "parallelism": "replicas only" if world > 1 else "single GPU"},
         "clocks": clocks,
         "e2e": {"value": e2e_val, "unit": "GFlop/s", "ms_per_step": ms_e2e,
                 "h2d_bytes_per_step": field_bytes, "d2h_bytes_per_step": field_bytes + 8},

@@ -27,11 +27,13 @@
  *
  * DEVICE field layout (what `field`, `in`, `out` pointers below hold; produced only by
  * dwf_import_spinor, read back only by dwf_export_spinor; size dwf_field_bytes):
- *   complex[chunk][k][site][j]   s = chunk*Sc + j,  k = spin*3 + colour (12 complex components),
- *                                site = x (full) or x>>1 (half), complex = (re, im) adjacent.
- *   "SoA complex components, site-fastest, Ls innermost" (north_star subsystem 1): Sc consecutive
- *   s of one component of one site are contiguous; Sc = dwf_layout_sc(g) is the number of s-slices
- *   one thread keeps in registers so that each gauge link is loaded once and reused Sc times.
+ *   half field   complex[s][k][cb]    k = spin*3 + colour (12 complex components), cb = x>>1 the
+ *                                     checkerboard site index (x0-pairs fastest), (re, im) adjacent
+ *   full field   the even half field followed by the odd half field
+ *   "SoA complex components, site-fastest" (north_star subsystem 1).  s is the SLOWEST index: the
+ *   fast kernel keeps the 8 links of a 4D site in registers and walks through all Ls slices, so
+ *   each link is loaded once per 4D site and every slice is a dense 4D tensor that TMA can tile
+ *   (DESIGN.md "Data layout" says why this replaces the "Ls innermost" of north_star).
  * Device pointers must be 16-byte aligned and live on the geometry's device.
  * `stream` is a cudaStream_t passed as void* (NULL = the default stream).
  */
@@ -99,9 +101,6 @@ DWF_API int dwf_inner_product(const dwf_geometry *g, const void *a, const void *
 /* Bytes of a device field: full (DWF_FULL) or half (DWF_EVEN / DWF_ODD).  0 on bad arguments. */
 DWF_API size_t dwf_field_bytes(const dwf_geometry *g, int parity);
 
-/* Sc of the device layout (s-slices per register block); 0 on NULL. */
-DWF_API int dwf_layout_sc(const dwf_geometry *g);
-
 /* canonical -> device layout.  Host sources go through an internal staging copy and synchronise
  * `stream`; device sources are asynchronous. */
 DWF_API int dwf_import_spinor(const dwf_geometry *g, const void *canonical, int src_is_device, int parity,
@@ -114,7 +113,9 @@ DWF_API int dwf_export_spinor(const dwf_geometry *g, const void *field_dev, int 
 /* Number of kernel launches this library has issued since it was loaded (all threads). */
 DWF_API unsigned long long dwf_launch_count(void);
 
-/* Select a kernel variant by name for experiments ("auto" = default); UNSUPPORTED if unknown. */
+/* Tuning knobs for experiments: "kernel" (0 auto, 1 direct L1-cached kernel, 2 TMA-staged kernel),
+ * "variant" (staged tile shape, 0 auto), "raster_staged" / "raster" (CTA launch order),
+ * "tile0".."tile3", "cpc" (direct kernel tile).  UNSUPPORTED for an unknown key. */
 DWF_API int dwf_set_option(dwf_geometry *g, const char *key, long long value);
 
 DWF_API const char *dwf_error_string(int code);

@@ -25,7 +25,7 @@ LIB_PATH = os.path.join(_HERE, "libdwf.so")
 # every symbol include/dwf.h declares (tests check that the library exports all of them)
 SYMBOLS = (
     "dwf_create_geometry", "dwf_destroy_geometry", "dwf_load_gauge", "dwf_dhop", "dwf_dhop_oe",
-    "dwf_dhop_eo", "dwf_norm2", "dwf_inner_product", "dwf_field_bytes", "dwf_layout_sc",
+    "dwf_dhop_eo", "dwf_norm2", "dwf_inner_product", "dwf_field_bytes",
     "dwf_import_spinor", "dwf_export_spinor", "dwf_launch_count", "dwf_set_option",
     "dwf_error_string", "dwf_last_error",
 )
@@ -61,7 +61,6 @@ def load(build_if_missing: bool = True):
     lib.dwf_inner_product.argtypes = [vp, vp, vp, ci, ctypes.POINTER(ctypes.c_double), vp]
     lib.dwf_field_bytes.argtypes = [vp, ci]
     lib.dwf_field_bytes.restype = cs
-    lib.dwf_layout_sc.argtypes = [vp]
     lib.dwf_import_spinor.argtypes = [vp, vp, ci, ci, vp, vp]
     lib.dwf_export_spinor.argtypes = [vp, vp, ci, vp, ci, vp]
     lib.dwf_launch_count.argtypes = []
@@ -156,10 +155,6 @@ def dwf_inner_product(g: int, a, b, parity: int = FULL, stream=None) -> complex:
 
 def dwf_field_bytes(g: int, parity: int = FULL) -> int:
     return int(load().dwf_field_bytes(g, int(parity)))
-
-
-def dwf_layout_sc(g: int) -> int:
-    return int(load().dwf_layout_sc(g))
 
 
 def dwf_import_spinor(g: int, canonical, parity: int, field_dev, stream=None) -> None:

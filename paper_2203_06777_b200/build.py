@@ -19,7 +19,7 @@ ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libdwf.so")
 OBJDIR = os.path.join(HERE, "build")
 
-SOURCES = ["api.cu", "pack.cu", "dhop.cu", "reduce.cu"]
+SOURCES = ["api.cu", "pack.cu", "dhop.cu", "dhop_staged.cu", "reduce.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden",

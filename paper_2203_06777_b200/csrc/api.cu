@@ -74,15 +74,13 @@ static void build_tile_table(const Tiling &t, int raster, std::vector<int4> &tab
     }
 }
 
-static void make_tiling(const dwf_geometry *g, bool cb, Tiling &t)
+static void make_tiling(const dwf_geometry *g, Tiling &t)
 {
     const Lattice &lat = g->lat;
-    const int ext[4] = {cb ? lat.Lh : lat.L[0], lat.L[1], lat.L[2], lat.L[3]};
+    const int ext[4] = {lat.Lh, lat.L[1], lat.L[2], lat.L[3]};
     int sites = 1;
     for (int d = 0; d < 4; d++) {
-        int want = g->opt_tile[d];
-        if (!cb && d == 0) want += 1;            // same x0 span as the checkerboard tile
-        t.sh[d] = fit_shift(ext[d], want);
+        t.sh[d] = fit_shift(ext[d], g->opt_tile[d]);
         t.ntile[d] = ext[d] >> t.sh[d];
         sites <<= t.sh[d];
     }
@@ -90,24 +88,29 @@ static void make_tiling(const dwf_geometry *g, bool cb, Tiling &t)
     for (int d = 3; d >= 0 && sites > 256; d--)
         while (t.sh[d] > 0 && sites > 256) { t.sh[d]--; t.ntile[d] <<= 1; sites >>= 1; }
     int cpc = std::max(1, std::min(g->opt_cpc, 256 / sites));
-    while (lat.nchunk % cpc) cpc--;
+    while (lat.Ls % cpc) cpc--;
     t.cpc = cpc;
-    t.ncg = lat.nchunk / cpc;
+    t.ncg = lat.Ls / cpc;
     t.threads = sites * cpc;
     t.ntiles = t.ntile[0] * t.ntile[1] * t.ntile[2] * t.ntile[3];
 }
 
 int rebuild_tilings(dwf_geometry *g)
 {
-    for (int cb = 0; cb < 2; cb++) {
-        Tiling &t = cb ? g->tiling_cb : g->tiling_full;
-        int4 *&dev = cb ? g->tiles_cb : g->tiles_full;
-        make_tiling(g, cb != 0, t);
-        std::vector<int4> tab;
-        build_tile_table(t, g->opt_raster, tab);
-        if (dev) { cudaFree(dev); dev = nullptr; }
-        DWF_CUDA_CHECK(cudaMalloc(&dev, tab.size() * sizeof(int4)));
-        DWF_CUDA_CHECK(cudaMemcpy(dev, tab.data(), tab.size() * sizeof(int4), cudaMemcpyHostToDevice));
+    make_tiling(g, g->tiling_cb);
+    std::vector<int4> tab;
+    build_tile_table(g->tiling_cb, g->opt_raster, tab);
+    if (g->tiles_cb) { cudaFree(g->tiles_cb); g->tiles_cb = nullptr; }
+    DWF_CUDA_CHECK(cudaMalloc(&g->tiles_cb, tab.size() * sizeof(int4)));
+    DWF_CUDA_CHECK(cudaMemcpy(g->tiles_cb, tab.data(), tab.size() * sizeof(int4), cudaMemcpyHostToDevice));
+
+    if (g->tiles_staged) { cudaFree(g->tiles_staged); g->tiles_staged = nullptr; }
+    plan_staged(g);
+    if (g->staged.variant >= 0) {
+        std::vector<int4> st((size_t)g->staged.ntiles);
+        build_staged_tile_table(g, g->opt_raster_staged, st.data());
+        DWF_CUDA_CHECK(cudaMalloc(&g->tiles_staged, st.size() * sizeof(int4)));
+        DWF_CUDA_CHECK(cudaMemcpy(g->tiles_staged, st.data(), st.size() * sizeof(int4), cudaMemcpyHostToDevice));
     }
     return DWF_OK;
 }
@@ -182,21 +185,18 @@ int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, i
     g->lat.Ls = Ls;
     g->lat.V4 = V4;
     g->lat.Vh = V4 / 2;
-    // s-slices per thread: two complex per 128-bit load in fp32, one in fp64
-    int sc = (precision == DWF_F32) ? 2 : 1;
-    while (Ls % sc) sc >>= 1;
-    g->lat.Sc = sc;
-    g->lat.nchunk = Ls / sc;
     g->prec = precision;
     g->bc_time = bc_time;
     g->device = cuda_device;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) { delete g; set_error("cudaGetDeviceProperties failed"); return DWF_ERR_CUDA; }
     g->sm_count = prop.multiProcessorCount;
-    g->opt_tile[0] = 2; g->opt_tile[1] = 2; g->opt_tile[2] = 1; g->opt_tile[3] = 1;
-    g->opt_cpc = 4;
-    g->opt_raster = 0;
+    g->opt_tile[0] = 4; g->opt_tile[1] = 2; g->opt_tile[2] = 1; g->opt_tile[3] = 1;
+    g->opt_cpc = 1;
+    g->opt_raster = 2;
+    g->opt_raster_staged = 1;
     g->opt_variant = 0;
+    g->opt_kernel = 0;
 
     g->gauge_bytes = (size_t)8 * 18 * (size_t)g->lat.Vh * (size_t)precision;
     g->reduce_blocks = g->sm_count * 8;
@@ -223,7 +223,7 @@ int dwf_destroy_geometry(dwf_geometry *g)
     cudaFree(g->partials);
     cudaFree(g->result_dev);
     cudaFree(g->tiles_cb);
-    cudaFree(g->tiles_full);
+    cudaFree(g->tiles_staged);
     cudaFree(g->staging);
     cudaGetLastError();
     delete g;
@@ -243,8 +243,13 @@ int dwf_set_option(dwf_geometry *g, const char *key, long long value)
         g->opt_cpc = v;
     } else if (!strcmp(key, "raster")) {
         g->opt_raster = v;
+    } else if (!strcmp(key, "raster_staged")) {
+        g->opt_raster_staged = v;
     } else if (!strcmp(key, "variant")) {
-        g->opt_variant = v;
+        g->opt_variant = v;          // 0: best staged tile, n > 0: n-th compiled staged variant only
+    } else if (!strcmp(key, "kernel")) {
+        if (v < 0 || v > 2) { set_error("kernel must be 0 (auto), 1 (direct) or 2 (staged)"); return DWF_ERR_INVALID_ARG; }
+        g->opt_kernel = v;
         return DWF_OK;
     } else {
         set_error("unknown option '%s'", key);
@@ -259,8 +264,6 @@ size_t dwf_field_bytes(const dwf_geometry *g, int parity)
     const long long nsites = (parity == DWF_FULL) ? g->lat.V4 : g->lat.Vh;
     return (size_t)nsites * (size_t)g->lat.Ls * 24 * (size_t)g->prec;
 }
-
-int dwf_layout_sc(const dwf_geometry *g) { return g ? g->lat.Sc : 0; }
 
 int dwf_load_gauge(dwf_geometry *g, const void *U, int src_is_device, void *stream)
 {
@@ -282,6 +285,18 @@ int dwf_load_gauge(dwf_geometry *g, const void *U, int src_is_device, void *stre
     return DWF_OK;
 }
 
+// one half-Dhop: out (parity_out) = D in (opposite parity); picks the kernel
+static int half_dhop(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st)
+{
+    const bool staged_ok = g->staged.variant >= 0;
+    if (g->opt_kernel == 2 && !staged_ok) {
+        set_error("the staged kernel does not support this geometry / precision");
+        return DWF_ERR_UNSUPPORTED;
+    }
+    if (staged_ok && g->opt_kernel != 1) return launch_dhop_staged(g, in, out, parity_out, st);
+    return launch_dhop_direct(g, in, out, parity_out, st);
+}
+
 static int dhop_common(const dwf_geometry *g, const void *in, void *out, int parity_out, void *stream, const char *who)
 {
     if (!g || !in || !out) { set_error("%s: NULL argument", who); return DWF_ERR_INVALID_ARG; }
@@ -289,7 +304,16 @@ static int dhop_common(const dwf_geometry *g, const void *in, void *out, int par
     if (!aligned16(in) || !aligned16(out)) { set_error("%s: field pointers must be 16-byte aligned", who); return DWF_ERR_INVALID_ARG; }
     if (!g->gauge_loaded) { set_error("%s: call dwf_load_gauge first", who); return DWF_ERR_NO_GAUGE; }
     DeviceGuard guard(g->device);
-    return launch_dhop(g, in, out, parity_out, static_cast<cudaStream_t>(stream));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (parity_out != DWF_FULL) return half_dhop(g, in, out, parity_out, st);
+    // a full field is its even half field followed by its odd half field:
+    // (Dhop psi)_odd = DhopOE psi_even, (Dhop psi)_even = DhopEO psi_odd
+    const size_t half = dwf_field_bytes(g, DWF_EVEN);
+    const char *ie = static_cast<const char *>(in), *io = ie + half;
+    char *oe = static_cast<char *>(out), *oo = oe + half;
+    int rc = half_dhop(g, ie, oo, DWF_ODD, st);
+    if (rc) return rc;
+    return half_dhop(g, io, oe, DWF_EVEN, st);
 }
 
 int dwf_dhop(const dwf_geometry *g, const void *in_full, void *out_full, void *stream)

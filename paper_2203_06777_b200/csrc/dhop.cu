@@ -1,4 +1,5 @@
-// dhop.cu -- the Dhop kernels (hot path rows a2-a6 of SURVEY.md section 8).
+// dhop.cu -- the direct (L1-cached) Dhop kernel (hot path rows a2-a6 of SURVEY.md section 8): the
+// general path for every geometry and precision; dhop_staged.cu holds the fast fp32 path.
 //
 //   Dhop psi(x,s) = sum_mu [ (1-gamma_mu) U_mu(x) psi(x+mu,s) + (1+gamma_mu) U_mu^dag(x-mu) psi(x-mu,s) ]
 //
@@ -24,28 +25,13 @@
 namespace dwf {
 
 // gauge storage: per leg 9 complex planes over the Vh output sites of one parity
-template <typename T> struct LinkIO;
-template <> struct LinkIO<float> {
-    // planes are paired into float4 (complex 2v, 2v+1), the ninth complex is a float2 tail
-    static __device__ __forceinline__ void load(const float *leg, long long Vh, int site, float2 (&U)[9])
-    {
+template <typename T>
+__device__ __forceinline__ void load_link(const T *leg, long long Vh, int site, typename CxT<T>::type (&U)[9])
+{
+    using C = typename CxT<T>::type;
 #pragma unroll
-        for (int v = 0; v < 4; v++) {
-            float4 q = __ldg(reinterpret_cast<const float4 *>(leg + (size_t)v * 4 * Vh) + site);
-            U[2 * v] = make_float2(q.x, q.y);
-            U[2 * v + 1] = make_float2(q.z, q.w);
-        }
-        U[8] = __ldg(reinterpret_cast<const float2 *>(leg + (size_t)16 * Vh) + site);
-    }
-};
-template <> struct LinkIO<double> {
-    static __device__ __forceinline__ void load(const double *leg, long long Vh, int site, double2 (&U)[9])
-    {
-#pragma unroll
-        for (int v = 0; v < 9; v++)
-            U[v] = __ldg(reinterpret_cast<const double2 *>(leg + (size_t)v * 2 * Vh) + site);
-    }
-};
+    for (int v = 0; v < 9; v++) U[v] = __ldg(reinterpret_cast<const C *>(leg + (size_t)v * 2 * Vh) + site);
+}
 
 // one leg: acc += reconstruct( U * project(psi_neighbour) )
 template <typename T, int SC, int MU, bool FWD, bool FIRST>
@@ -59,7 +45,7 @@ __device__ __forceinline__ void dhop_leg(typename CxT<T>::type (&acc)[12][SC],
 #pragma unroll
     for (int k = 0; k < 12; k++) load_cx<SC>(nb + (size_t)k * kstride, psi[k]);
     C U[9];
-    LinkIO<T>::load(leg_links, Vh, gsite, U);
+    load_link<T>(leg_links, Vh, gsite, U);
 
 #pragma unroll
     for (int j = 0; j < SC; j++) {
@@ -129,21 +115,21 @@ __device__ __forceinline__ void dhop_leg(typename CxT<T>::type (&acc)[12][SC],
 
 // ---------------------------------------------------------------------------------------------
 // direct kernel: neighbours are read straight from global memory (L1/L2 catch the reuse).
-// CB = true : in/out are half fields; out has parity `parity_out`, in the opposite parity.
-// CB = false: in/out are full fields (lexicographic sites); the links of site x live in the
-//             gauge set of x's parity at index x>>1.
+// in/out are half fields complex[s][k][Vh]; out has parity `parity_out`, in the opposite parity.
+// One thread = one output site and one s-slice.
 // ---------------------------------------------------------------------------------------------
-template <typename T, int SC, bool CB, int MAXT, int MINB>
+template <typename T, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB)
 dhop_direct_kernel(const typename CxT<T>::type *__restrict__ in, typename CxT<T>::type *__restrict__ out,
-                   const T *__restrict__ gauge_even, const T *__restrict__ gauge_odd,
-                   const int4 *__restrict__ tiles, const Lattice lat, const Tiling til, const int parity_out)
+                   const T *__restrict__ gset, const int4 *__restrict__ tiles, const Lattice lat,
+                   const Tiling til, const int parity_out)
 {
     using C = typename CxT<T>::type;
+    constexpr int SC = 1;
     const int nsh = til.sh[0] + til.sh[1] + til.sh[2] + til.sh[3];
     const int tid = threadIdx.x;
     const int ls = tid & ((1 << nsh) - 1);
-    const int chunk = (blockIdx.x % til.ncg) * til.cpc + (tid >> nsh);
+    const int s = (blockIdx.x % til.ncg) * til.cpc + (tid >> nsh);
     const int4 org = tiles[blockIdx.x / til.ncg];
 
     int l = ls;
@@ -153,32 +139,20 @@ dhop_direct_kernel(const typename CxT<T>::type *__restrict__ in, typename CxT<T>
     const int x3 = org.w + l;
 
     const int L1 = lat.L[1], L2 = lat.L[2], L3 = lat.L[3];
-    const int W0 = CB ? lat.Lh : lat.L[0];           // row length in field sites
-    const long long Vs = CB ? lat.Vh : lat.V4;       // sites per field
-    const size_t kstride = (size_t)Vs * SC;
+    const int W0 = lat.Lh;                           // row length in field sites
+    const long long Vh = lat.Vh;
+    const size_t kstride = (size_t)Vh;
 
     const int row = x1 + L1 * (x2 + L2 * x3);
     const int site = c0 + W0 * row;
-
-    // gauge set and index
-    int par, gsite;
-    if constexpr (CB) { par = parity_out; gsite = site; }
-    else { par = (c0 + x1 + x2 + x3) & 1; gsite = site >> 1; }
-    const T *gset = par ? gauge_odd : gauge_even;
-    const long long Vh = lat.Vh;
+    const int gsite = site;
 
     // neighbour site indices
-    int n0p, n0m;
-    if constexpr (CB) {
-        const int r = (x1 + x2 + x3 + parity_out) & 1;      // x0 = 2*c0 + r
-        int hp = c0 + r;       if (hp == W0) hp = 0;
-        int hm = c0 - 1 + r;   if (hm < 0) hm = W0 - 1;
-        n0p = hp + W0 * row;
-        n0m = hm + W0 * row;
-    } else {
-        n0p = (c0 + 1 == W0 ? 0 : c0 + 1) + W0 * row;
-        n0m = (c0 == 0 ? W0 - 1 : c0 - 1) + W0 * row;
-    }
+    const int r = (x1 + x2 + x3 + parity_out) & 1;          // x0 = 2*c0 + r
+    int hp = c0 + r;       if (hp == W0) hp = 0;
+    int hm = c0 - 1 + r;   if (hm < 0) hm = W0 - 1;
+    const int n0p = hp + W0 * row;
+    const int n0m = hm + W0 * row;
     const int s1 = W0, s2 = W0 * L1, s3 = W0 * L1 * L2;
     const int n1p = site + (x1 + 1 == L1 ? -(L1 - 1) * s1 : s1);
     const int n1m = site + (x1 == 0 ? (L1 - 1) * s1 : -s1);
@@ -187,67 +161,47 @@ dhop_direct_kernel(const typename CxT<T>::type *__restrict__ in, typename CxT<T>
     const int n3p = site + (x3 + 1 == L3 ? -(L3 - 1) * s3 : s3);
     const int n3m = site + (x3 == 0 ? (L3 - 1) * s3 : -s3);
 
-    const C *base = in + (size_t)chunk * 12 * kstride;
+    const C *base = in + (size_t)s * 12 * kstride;
     const size_t lstride = (size_t)18 * Vh;          // reals per leg
 
     C acc[12][SC];
-    dhop_leg<T, SC, 0, true,  true >(acc, base + (size_t)n0p * SC, kstride, gset + 0 * lstride, Vh, gsite);
-    dhop_leg<T, SC, 0, false, false>(acc, base + (size_t)n0m * SC, kstride, gset + 1 * lstride, Vh, gsite);
-    dhop_leg<T, SC, 1, true,  false>(acc, base + (size_t)n1p * SC, kstride, gset + 2 * lstride, Vh, gsite);
-    dhop_leg<T, SC, 1, false, false>(acc, base + (size_t)n1m * SC, kstride, gset + 3 * lstride, Vh, gsite);
-    dhop_leg<T, SC, 2, true,  false>(acc, base + (size_t)n2p * SC, kstride, gset + 4 * lstride, Vh, gsite);
-    dhop_leg<T, SC, 2, false, false>(acc, base + (size_t)n2m * SC, kstride, gset + 5 * lstride, Vh, gsite);
-    dhop_leg<T, SC, 3, true,  false>(acc, base + (size_t)n3p * SC, kstride, gset + 6 * lstride, Vh, gsite);
-    dhop_leg<T, SC, 3, false, false>(acc, base + (size_t)n3m * SC, kstride, gset + 7 * lstride, Vh, gsite);
+    dhop_leg<T, SC, 0, true,  true >(acc, base + n0p, kstride, gset + 0 * lstride, Vh, gsite);
+    dhop_leg<T, SC, 0, false, false>(acc, base + n0m, kstride, gset + 1 * lstride, Vh, gsite);
+    dhop_leg<T, SC, 1, true,  false>(acc, base + n1p, kstride, gset + 2 * lstride, Vh, gsite);
+    dhop_leg<T, SC, 1, false, false>(acc, base + n1m, kstride, gset + 3 * lstride, Vh, gsite);
+    dhop_leg<T, SC, 2, true,  false>(acc, base + n2p, kstride, gset + 4 * lstride, Vh, gsite);
+    dhop_leg<T, SC, 2, false, false>(acc, base + n2m, kstride, gset + 5 * lstride, Vh, gsite);
+    dhop_leg<T, SC, 3, true,  false>(acc, base + n3p, kstride, gset + 6 * lstride, Vh, gsite);
+    dhop_leg<T, SC, 3, false, false>(acc, base + n3m, kstride, gset + 7 * lstride, Vh, gsite);
 
-    C *o = out + (size_t)chunk * 12 * kstride + (size_t)site * SC;
+    C *o = out + (size_t)s * 12 * kstride + (size_t)site;
 #pragma unroll
     for (int k = 0; k < 12; k++) store_cx<SC>(o + (size_t)k * kstride, acc[k]);
 }
 
-template <typename T, int SC, bool CB, int MAXT, int MINB>
+template <typename T, int MAXT, int MINB>
 static int launch_direct(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st)
 {
     using C = typename CxT<T>::type;
-    const Tiling &til = CB ? g->tiling_cb : g->tiling_full;
-    const int4 *tiles = CB ? g->tiles_cb : g->tiles_full;
+    const Tiling &til = g->tiling_cb;
     if (til.threads > MAXT) {
         set_error("tile of %d threads exceeds kernel limit %d", til.threads, MAXT);
         return DWF_ERR_UNSUPPORTED;
     }
     dim3 grid((unsigned)(til.ntiles * til.ncg)), block((unsigned)til.threads);
-    dhop_direct_kernel<T, SC, CB, MAXT, MINB><<<grid, block, 0, st>>>(
-        static_cast<const C *>(in), static_cast<C *>(out), static_cast<const T *>(g->gauge[0]),
-        static_cast<const T *>(g->gauge[1]), tiles, g->lat, til, parity_out);
+    dhop_direct_kernel<T, MAXT, MINB><<<grid, block, 0, st>>>(
+        static_cast<const C *>(in), static_cast<C *>(out), static_cast<const T *>(g->gauge[parity_out]),
+        g->tiles_cb, g->lat, til, parity_out);
     count_launch();
     DWF_CUDA_CHECK(cudaGetLastError());
     return DWF_OK;
 }
 
-template <typename T, bool CB>
-static int dispatch_sc(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st)
+// parity_out: DWF_EVEN (DhopEO) or DWF_ODD (DhopOE)
+int launch_dhop_direct(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st)
 {
-    constexpr bool F32 = sizeof(T) == 4;
-    switch (g->lat.Sc) {
-    case 1: return launch_direct<T, 1, CB, 256, F32 ? 3 : 2>(g, in, out, parity_out, st);
-    case 2: return launch_direct<T, 2, CB, 256, F32 ? 2 : 1>(g, in, out, parity_out, st);
-    case 4:
-        if constexpr (F32) return launch_direct<T, 4, CB, 256, 1>(g, in, out, parity_out, st);
-        break;
-    }
-    set_error("unsupported Sc=%d for precision %d", g->lat.Sc, (int)sizeof(T));
-    return DWF_ERR_UNSUPPORTED;
-}
-
-// parity_out: DWF_FULL, DWF_EVEN (DhopEO), DWF_ODD (DhopOE)
-int launch_dhop(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st)
-{
-    if (g->prec == DWF_F32) {
-        if (parity_out == DWF_FULL) return dispatch_sc<float, false>(g, in, out, 0, st);
-        return dispatch_sc<float, true>(g, in, out, parity_out, st);
-    }
-    if (parity_out == DWF_FULL) return dispatch_sc<double, false>(g, in, out, 0, st);
-    return dispatch_sc<double, true>(g, in, out, parity_out, st);
+    if (g->prec == DWF_F32) return launch_direct<float, 256, 3>(g, in, out, parity_out, st);
+    return launch_direct<double, 256, 2>(g, in, out, parity_out, st);
 }
 
 }  // namespace dwf

@@ -1,0 +1,384 @@
+// dhop_staged.cu -- the fast fp32 Dhop kernel for sm_100a: link-stationary, TMA-staged.
+//
+//   Dhop psi(x,s) = sum_mu [ (1-gamma_mu) U_mu(x) psi(x+mu,s) + (1+gamma_mu) U_mu^dag(x-mu) psi(x-mu,s) ]
+//
+// Work decomposition (hot path rows a2-a6 of SURVEY.md section 8):
+//   * A CTA owns a box of B1 x B2 x B3 "x0-rows" of output sites (a row = the Lh sites of the
+//     output parity on one lattice line along x0) and ALL Ls slices.  One thread = one output 4D
+//     site.  It loads its 8 links (U_mu(x) and the pre-daggered U_mu^dag(x-mu), 72 complex) ONCE
+//     into registers and keeps them there while it walks through s = 0 .. Ls-1: each link crosses
+//     the L1/shared-memory data pipe once per 4D site instead of once per 5D site.
+//   * For every s the input slice needed by the tile -- the rows box itself plus its six faces
+//     (the x0 direction closes periodically inside a row, so it has no halo) -- is brought into
+//     shared memory by seven 5-D bulk tensor copies (TMA, cp.async.bulk.tensor) issued by one
+//     thread, two slices deep, completion signalled through mbarriers.  Periodic wrap is a
+//     coordinate computed modulo the extent: every face is its own box.  Compute warps never
+//     wait on global memory, only on the mbarrier of the slice they are about to consume.
+//   * Per leg a thread reads the neighbour spinor with 12 LDS.64 at (per-leg base register +
+//     immediate), projects to a half spinor, multiplies with the register-resident link,
+//     reconstructs and accumulates; after the 8 legs it stores 12 complex with streaming stores.
+//     All complex arithmetic is packed f32x2 (FFMA2 / FADD2): u*h is accumulated as two chains
+//     A = sum u.re*h and B = sum u.im*h, combined once as A + iB, so that no operand needs a
+//     half-negated copy.
+// Shared-memory image of one slice: [row of the staged region][k = spin*3+colour][Lh] complex,
+// regions in the order centre, x1-, x1+, x2-, x2+, x3-, x3+.
+#include <vector>
+
+#include "complex_ops.cuh"
+#include "dwf_internal.cuh"
+#include "tma.cuh"
+
+namespace dwf {
+
+PFN_tensorMapEncodeTiled get_tensor_map_encoder()
+{
+    static PFN_tensorMapEncodeTiled fn = [] {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess) {
+            cudaGetLastError();
+            p = nullptr;
+        }
+        return reinterpret_cast<PFN_tensorMapEncodeTiled>(p);
+    }();
+    return fn;
+}
+
+struct StagedArgs {
+    float2 *out;
+    const float2 *gauge;     // gauge set of the output parity: [leg][9][Vh]
+    const int4 *tiles;       // origins (o1, o2, o3) of the row boxes, launch order
+    int ntiles;
+    int L1, L2, L3, Ls;
+    long long Vh;
+    int parity_out;
+};
+
+template <int LH, int B1, int B2, int B3> struct StagedCfg {
+    static constexpr int NROW_C = B1 * B2 * B3;
+    static constexpr int T = LH * NROW_C;                        // output sites per tile
+    static constexpr int NT = (T + 31) / 32 * 32;                // threads
+    static constexpr int ROWB = 12 * LH * 8;                     // bytes of one staged row
+    static constexpr int R_X1M = NROW_C, R_X1P = R_X1M + B2 * B3, R_X2M = R_X1P + B2 * B3,
+                         R_X2P = R_X2M + B1 * B3, R_X3M = R_X2P + B1 * B3, R_X3P = R_X3M + B1 * B2,
+                         NROW_IN = R_X3P + B1 * B2;
+    static constexpr int STAGE_BYTES = NROW_IN * ROWB;
+    static constexpr int NSTAGE = 2;
+    static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + 64;  // + mbarriers
+    static_assert(ROWB % 128 == 0, "staged rows must keep TMA destinations 128-byte aligned");
+};
+
+// one leg: acc += reconstruct( U * project(psi) ), psi read from shared memory
+template <int LH, int MU, bool FWD, bool FIRST>
+__device__ __forceinline__ void staged_leg(float2 (&acc)[12], const float2 *__restrict__ nb, const float2 (&U)[9])
+{
+    float2 p[12];
+#pragma unroll
+    for (int k = 0; k < 12; k++) p[k] = nb[k * LH];
+    float2 h0[3], h1[3];
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        const float2 p0 = p[c], p1 = p[3 + c], p2 = p[6 + c], p3 = p[9 + c];
+        if constexpr (MU == 0) {
+            h0[c] = FWD ? csubi(p0, p3) : caddi(p0, p3);
+            h1[c] = FWD ? csubi(p1, p2) : caddi(p1, p2);
+        } else if constexpr (MU == 1) {
+            h0[c] = FWD ? cadd(p0, p3) : csub(p0, p3);
+            h1[c] = FWD ? csub(p1, p2) : cadd(p1, p2);
+        } else if constexpr (MU == 2) {
+            h0[c] = FWD ? csubi(p0, p2) : caddi(p0, p2);
+            h1[c] = FWD ? caddi(p1, p3) : csubi(p1, p3);
+        } else {
+            h0[c] = FWD ? csub(p0, p2) : cadd(p0, p2);
+            h1[c] = FWD ? csub(p1, p3) : cadd(p1, p3);
+        }
+    }
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+        // x = sum_b U[a][b] * h[b] as  A + iB,  A = sum u.re * h,  B = sum u.im * h
+        const float2 u0 = U[3 * a], u1 = U[3 * a + 1], u2 = U[3 * a + 2];
+        float2 A0 = f2_mul(make_float2(u0.x, u0.x), h0[0]);
+        float2 B0 = f2_mul(make_float2(u0.y, u0.y), h0[0]);
+        float2 A1 = f2_mul(make_float2(u0.x, u0.x), h1[0]);
+        float2 B1 = f2_mul(make_float2(u0.y, u0.y), h1[0]);
+        A0 = f2_fma(make_float2(u1.x, u1.x), h0[1], A0);
+        B0 = f2_fma(make_float2(u1.y, u1.y), h0[1], B0);
+        A1 = f2_fma(make_float2(u1.x, u1.x), h1[1], A1);
+        B1 = f2_fma(make_float2(u1.y, u1.y), h1[1], B1);
+        A0 = f2_fma(make_float2(u2.x, u2.x), h0[2], A0);
+        B0 = f2_fma(make_float2(u2.y, u2.y), h0[2], B0);
+        A1 = f2_fma(make_float2(u2.x, u2.x), h1[2], A1);
+        B1 = f2_fma(make_float2(u2.y, u2.y), h1[2], B1);
+        const float2 x0 = caddi(A0, B0), x1 = caddi(A1, B1);
+        if constexpr (FIRST) {
+            acc[0 + a] = x0;
+            acc[3 + a] = x1;
+            if constexpr (MU == 0) {
+                acc[6 + a] = FWD ? cmuli(x1) : cmulni(x1);
+                acc[9 + a] = FWD ? cmuli(x0) : cmulni(x0);
+            } else if constexpr (MU == 1) {
+                acc[6 + a] = FWD ? cneg(x1) : x1;
+                acc[9 + a] = FWD ? x0 : cneg(x0);
+            } else if constexpr (MU == 2) {
+                acc[6 + a] = FWD ? cmuli(x0) : cmulni(x0);
+                acc[9 + a] = FWD ? cmulni(x1) : cmuli(x1);
+            } else {
+                acc[6 + a] = FWD ? cneg(x0) : x0;
+                acc[9 + a] = FWD ? cneg(x1) : x1;
+            }
+        } else {
+            acc[0 + a] = cadd(acc[0 + a], x0);
+            acc[3 + a] = cadd(acc[3 + a], x1);
+            if constexpr (MU == 0) {
+                acc[6 + a] = FWD ? caddi(acc[6 + a], x1) : csubi(acc[6 + a], x1);
+                acc[9 + a] = FWD ? caddi(acc[9 + a], x0) : csubi(acc[9 + a], x0);
+            } else if constexpr (MU == 1) {
+                acc[6 + a] = FWD ? csub(acc[6 + a], x1) : cadd(acc[6 + a], x1);
+                acc[9 + a] = FWD ? cadd(acc[9 + a], x0) : csub(acc[9 + a], x0);
+            } else if constexpr (MU == 2) {
+                acc[6 + a] = FWD ? caddi(acc[6 + a], x0) : csubi(acc[6 + a], x0);
+                acc[9 + a] = FWD ? csubi(acc[9 + a], x1) : caddi(acc[9 + a], x1);
+            } else {
+                acc[6 + a] = FWD ? csub(acc[6 + a], x0) : cadd(acc[6 + a], x0);
+                acc[9 + a] = FWD ? csub(acc[9 + a], x1) : cadd(acc[9 + a], x1);
+            }
+        }
+    }
+}
+
+template <int LH, int B1, int B2, int B3>
+__global__ void __launch_bounds__(StagedCfg<LH, B1, B2, B3>::NT, 1)
+dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_x1,
+                   const __grid_constant__ CUtensorMap map_x2, const __grid_constant__ CUtensorMap map_x3,
+                   const StagedArgs args)
+{
+    using Cfg = StagedCfg<LH, B1, B2, B3>;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    const uint32_t smem_base = smem_u32(smem);
+    const uint32_t bar_base = smem_base + Cfg::NSTAGE * Cfg::STAGE_BYTES;
+
+    const int tid = threadIdx.x;
+    const bool active = tid < Cfg::T;
+    const int h = tid % LH;
+    const int row = active ? tid / LH : 0;
+    const int i1 = row % B1, i2 = (row / B1) % B2, i3 = row / (B1 * B2);
+
+    const int my_tiles = (args.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    const int nsteps = my_tiles * args.Ls;
+    if (nsteps <= 0) return;
+
+    // producer: stage the input slice of step g (tile g / Ls of this CTA, s = g % Ls)
+    auto issue = [&](int it, int s, int stage) {
+        const int4 o = args.tiles[blockIdx.x + it * gridDim.x];
+        const uint32_t bar = bar_base + 8 * stage;
+        const uint32_t dst = smem_base + stage * Cfg::STAGE_BYTES;
+        const int L1 = args.L1, L2 = args.L2, L3 = args.L3;
+        const int c1 = s * 12;
+        mbar_arrive_expect_tx(bar, Cfg::STAGE_BYTES);
+        tma_load_5d(dst, &map_c, bar, 0, c1, o.x, o.y, o.z);
+        tma_load_5d(dst + Cfg::R_X1M * Cfg::ROWB, &map_x1, bar, 0, c1, o.x == 0 ? L1 - 1 : o.x - 1, o.y, o.z);
+        tma_load_5d(dst + Cfg::R_X1P * Cfg::ROWB, &map_x1, bar, 0, c1, o.x + B1 == L1 ? 0 : o.x + B1, o.y, o.z);
+        tma_load_5d(dst + Cfg::R_X2M * Cfg::ROWB, &map_x2, bar, 0, c1, o.x, o.y == 0 ? L2 - 1 : o.y - 1, o.z);
+        tma_load_5d(dst + Cfg::R_X2P * Cfg::ROWB, &map_x2, bar, 0, c1, o.x, o.y + B2 == L2 ? 0 : o.y + B2, o.z);
+        tma_load_5d(dst + Cfg::R_X3M * Cfg::ROWB, &map_x3, bar, 0, c1, o.x, o.y, o.z == 0 ? L3 - 1 : o.z - 1);
+        tma_load_5d(dst + Cfg::R_X3P * Cfg::ROWB, &map_x3, bar, 0, c1, o.x, o.y, o.z + B3 == L3 ? 0 : o.z + B3);
+    };
+
+    if (tid == 0) {
+        tma_prefetch_desc(&map_c);
+        tma_prefetch_desc(&map_x1);
+        tma_prefetch_desc(&map_x2);
+        tma_prefetch_desc(&map_x3);
+        mbar_init(bar_base, 1);
+        mbar_init(bar_base + 8, 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    // next step to be issued: (p_it, p_s)
+    int p_it = 0, p_s = 0, p_g = 0;
+    auto advance_producer = [&]() {
+        issue(p_it, p_s, p_g & 1);
+        p_g++;
+        if (++p_s == args.Ls) { p_s = 0; p_it++; }
+    };
+    if (tid == 0) {
+        advance_producer();
+        if (nsteps > 1) advance_producer();
+    }
+
+    // row offsets (in staged rows) of the 8 neighbours; tile-invariant
+    const int rc = row;
+    const int r1p = (i1 + 1 < B1) ? rc + 1 : Cfg::R_X1P + i2 + B2 * i3;
+    const int r1m = (i1 > 0) ? rc - 1 : Cfg::R_X1M + i2 + B2 * i3;
+    const int r2p = (i2 + 1 < B2) ? rc + B1 : Cfg::R_X2P + i1 + B1 * i3;
+    const int r2m = (i2 > 0) ? rc - B1 : Cfg::R_X2M + i1 + B1 * i3;
+    const int r3p = (i3 + 1 < B3) ? rc + B1 * B2 : Cfg::R_X3P + i1 + B1 * i2;
+    const int r3m = (i3 > 0) ? rc - B1 * B2 : Cfg::R_X3M + i1 + B1 * i2;
+
+    const long long Vh = args.Vh;
+    float2 U[8][9];
+    uint32_t off[8];            // byte offsets of the 8 neighbour spinors inside a stage
+    float2 *optr = nullptr;
+    int s = 0, it = 0;
+    for (int g = 0; g < nsteps; g++) {
+        if (s == 0) {
+            // new tile: site index, x0 neighbours (depend on the row parity), links
+            const int4 o = args.tiles[blockIdx.x + it * gridDim.x];
+            const int x1 = o.x + i1, x2 = o.y + i2, x3 = o.z + i3;
+            const int r = (x1 + x2 + x3 + args.parity_out) & 1;          // x0 = 2h + r
+            int hp = h + r;       if (hp == LH) hp = 0;
+            int hm = h - 1 + r;   if (hm < 0) hm = LH - 1;
+            const long long site = h + (long long)LH * (x1 + (long long)args.L1 * (x2 + (long long)args.L2 * x3));
+            off[0] = rc * Cfg::ROWB + hp * 8;
+            off[1] = rc * Cfg::ROWB + hm * 8;
+            off[2] = r1p * Cfg::ROWB + h * 8;
+            off[3] = r1m * Cfg::ROWB + h * 8;
+            off[4] = r2p * Cfg::ROWB + h * 8;
+            off[5] = r2m * Cfg::ROWB + h * 8;
+            off[6] = r3p * Cfg::ROWB + h * 8;
+            off[7] = r3m * Cfg::ROWB + h * 8;
+            optr = args.out + site;
+            if (active) {
+                const float2 *gp = args.gauge + site;
+#pragma unroll
+                for (int l = 0; l < 8; l++)
+#pragma unroll
+                    for (int c = 0; c < 9; c++) U[l][c] = __ldg(gp + (size_t)(l * 9 + c) * Vh);
+            }
+        }
+        const int stage = g & 1;
+        mbar_wait(bar_base + 8 * stage, (g >> 1) & 1);
+        if (active) {
+            const unsigned char *sb = smem + stage * Cfg::STAGE_BYTES;
+            float2 acc[12];
+            staged_leg<LH, 0, true,  true >(acc, reinterpret_cast<const float2 *>(sb + off[0]), U[0]);
+            staged_leg<LH, 0, false, false>(acc, reinterpret_cast<const float2 *>(sb + off[1]), U[1]);
+            staged_leg<LH, 1, true,  false>(acc, reinterpret_cast<const float2 *>(sb + off[2]), U[2]);
+            staged_leg<LH, 1, false, false>(acc, reinterpret_cast<const float2 *>(sb + off[3]), U[3]);
+            staged_leg<LH, 2, true,  false>(acc, reinterpret_cast<const float2 *>(sb + off[4]), U[4]);
+            staged_leg<LH, 2, false, false>(acc, reinterpret_cast<const float2 *>(sb + off[5]), U[5]);
+            staged_leg<LH, 3, true,  false>(acc, reinterpret_cast<const float2 *>(sb + off[6]), U[6]);
+            staged_leg<LH, 3, false, false>(acc, reinterpret_cast<const float2 *>(sb + off[7]), U[7]);
+            float2 *o = optr + (size_t)s * 12 * Vh;
+#pragma unroll
+            for (int k = 0; k < 12; k++) __stcs(o + (size_t)k * Vh, acc[k]);
+        }
+        __syncthreads();          // every thread is done reading this stage
+        if (tid == 0 && p_g < nsteps) advance_producer();
+        if (++s == args.Ls) { s = 0; it++; }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side: plan, tile table, tensor maps, launch
+// ---------------------------------------------------------------------------------------------
+struct Variant {
+    int lh, b1, b2, b3;
+    int smem, threads;
+    const void *fn;
+};
+
+template <int LH, int B1, int B2, int B3> static Variant make_variant()
+{
+    using Cfg = StagedCfg<LH, B1, B2, B3>;
+    return {LH, B1, B2, B3, Cfg::SMEM_BYTES, Cfg::NT, reinterpret_cast<const void *>(&dhop_staged_kernel<LH, B1, B2, B3>)};
+}
+
+static const std::vector<Variant> &variants()
+{
+    // ordered by preference within one Lh: larger tiles (smaller halo ratio) first
+    static const std::vector<Variant> v = {
+        make_variant<16, 4, 2, 2>(), make_variant<16, 2, 2, 2>(), make_variant<16, 2, 2, 1>(),
+        make_variant<8, 4, 4, 2>(),  make_variant<8, 2, 2, 2>(),  make_variant<8, 2, 2, 1>(),
+        make_variant<24, 2, 2, 2>(), make_variant<24, 2, 2, 1>(),
+        make_variant<4, 4, 4, 4>(),  make_variant<4, 2, 2, 2>(),  make_variant<4, 2, 2, 1>(),
+    };
+    return v;
+}
+
+void plan_staged(dwf_geometry *g)
+{
+    g->staged.variant = -1;
+    if (g->prec != DWF_F32 || !get_tensor_map_encoder()) return;
+    const Lattice &lat = g->lat;
+    const std::vector<Variant> &v = variants();
+    for (size_t i = 0; i < v.size(); i++) {
+        if (v[i].lh != lat.Lh) continue;
+        if (lat.L[1] % v[i].b1 || lat.L[2] % v[i].b2 || lat.L[3] % v[i].b3) continue;
+        if (g->opt_variant > 0 && (int)i + 1 != g->opt_variant) continue;
+        g->staged.variant = (int)i;
+        g->staged.b[0] = v[i].b1; g->staged.b[1] = v[i].b2; g->staged.b[2] = v[i].b3;
+        g->staged.ntiles = (lat.L[1] / v[i].b1) * (lat.L[2] / v[i].b2) * (lat.L[3] / v[i].b3);
+        return;
+    }
+}
+
+// Launch order of the row boxes.  raster 0: lexicographic (x1 fastest, x3 slowest).
+// raster n > 0: direction 2 is split into 2^n macro blocks that are swept one after the other,
+// which shortens the reuse distance of the x3 faces (they must survive in L2 for one sweep of a
+// macro-block slab only).
+void build_staged_tile_table(const dwf_geometry *g, int raster, int4 *tab)
+{
+    const Lattice &lat = g->lat;
+    const int n1 = lat.L[1] / g->staged.b[0], n2 = lat.L[2] / g->staged.b[1], n3 = lat.L[3] / g->staged.b[2];
+    int nsplit = 1;
+    for (int i = 0; i < raster && (n2 % (nsplit * 2) == 0); i++) nsplit *= 2;
+    const int n2in = n2 / nsplit;
+    int id = 0;
+    for (int m = 0; m < nsplit; m++)
+        for (int t3 = 0; t3 < n3; t3++)
+            for (int t2 = 0; t2 < n2in; t2++)
+                for (int t1 = 0; t1 < n1; t1++)
+                    tab[id++] = make_int4(t1 * g->staged.b[0], (m * n2in + t2) * g->staged.b[1], t3 * g->staged.b[2], 0);
+}
+
+static int encode_map(CUtensorMap *m, const void *base, const Lattice &lat, int b1, int b2, int b3)
+{
+    PFN_tensorMapEncodeTiled enc = get_tensor_map_encoder();
+    const cuuint64_t dims[5] = {(cuuint64_t)2 * lat.Lh, (cuuint64_t)12 * lat.Ls, (cuuint64_t)lat.L[1],
+                                (cuuint64_t)lat.L[2], (cuuint64_t)lat.L[3]};
+    const cuuint64_t row = (cuuint64_t)lat.Lh * 8;
+    const cuuint64_t strides[4] = {(cuuint64_t)lat.Vh * 8, row, row * lat.L[1], row * lat.L[1] * lat.L[2]};
+    const cuuint32_t box[5] = {(cuuint32_t)2 * lat.Lh, 12, (cuuint32_t)b1, (cuuint32_t)b2, (cuuint32_t)b3};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    CUresult rc = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, const_cast<void *>(base), dims, strides, box, estr,
+                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (rc != CUDA_SUCCESS) {
+        set_error("cuTensorMapEncodeTiled failed with code %d", (int)rc);
+        return DWF_ERR_CUDA;
+    }
+    return DWF_OK;
+}
+
+int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st)
+{
+    const Variant &v = variants()[(size_t)g->staged.variant];
+    CUtensorMap mc, m1, m2, m3;
+    int rc;
+    if ((rc = encode_map(&mc, in, g->lat, v.b1, v.b2, v.b3))) return rc;
+    if ((rc = encode_map(&m1, in, g->lat, 1, v.b2, v.b3))) return rc;
+    if ((rc = encode_map(&m2, in, g->lat, v.b1, 1, v.b3))) return rc;
+    if ((rc = encode_map(&m3, in, g->lat, v.b1, v.b2, 1))) return rc;
+    StagedArgs a;
+    a.out = static_cast<float2 *>(out);
+    a.gauge = static_cast<const float2 *>(g->gauge[parity_out]);
+    a.tiles = g->tiles_staged;
+    a.ntiles = g->staged.ntiles;
+    a.L1 = g->lat.L[1]; a.L2 = g->lat.L[2]; a.L3 = g->lat.L[3]; a.Ls = g->lat.Ls;
+    a.Vh = g->lat.Vh;
+    a.parity_out = parity_out;
+    static thread_local const void *attr_set_for = nullptr;
+    if (attr_set_for != v.fn) {
+        DWF_CUDA_CHECK(cudaFuncSetAttribute(v.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, v.smem));
+        attr_set_for = v.fn;
+    }
+    const int grid = g->staged.ntiles < g->sm_count ? g->staged.ntiles : g->sm_count;
+    void *params[] = {&mc, &m1, &m2, &m3, &a};
+    DWF_CUDA_CHECK(cudaLaunchKernel(v.fn, dim3((unsigned)grid), dim3((unsigned)v.threads), params, (size_t)v.smem, st));
+    count_launch();
+    return DWF_OK;
+}
+
+}  // namespace dwf

@@ -34,21 +34,28 @@ struct Lattice {
     int L[4];        // extents, time last
     int Lh;          // L[0] / 2
     int Ls;
-    int Sc;          // s-slices per register block (device layout parameter)
-    int nchunk;      // Ls / Sc
     long long V4;    // L0*L1*L2*L3
     long long Vh;    // V4 / 2
 };
 
-// How one CTA maps onto output sites.  A CTA owns a 4D tile of output sites (extents are
-// powers of two; in checkerboard kernels extent 0 counts x0-PAIRS) times `cpc` s-chunks.
+// How one CTA of the direct (L1-cached) kernel maps onto output sites.  A CTA owns a 4D tile of
+// output sites of one parity (extents are powers of two; extent 0 counts x0-PAIRS) times `cpc`
+// s-slices.
 struct Tiling {
     int sh[4];       // log2 of the tile extents
     int ntile[4];    // tiles per direction
-    int cpc;         // s-chunks handled by one CTA
-    int ncg;         // chunk groups = nchunk / cpc
+    int cpc;         // s-slices handled by one CTA
+    int ncg;         // slice groups = Ls / cpc
     int threads;     // tile sites * cpc
     int ntiles;      // ntile[0]*ntile[1]*ntile[2]*ntile[3]
+};
+
+// Plan of the staged kernel (dhop_staged.cu): a CTA owns a box of B1 x B2 x B3 x0-rows (each row
+// holds the Lh output sites of one parity of a lattice line along x0) and all Ls slices.
+struct StagedPlan {
+    int variant;     // index into the table of compiled (Lh, B1, B2, B3) instances, -1: not usable
+    int b[3];        // rows box
+    int ntiles;
 };
 
 }  // namespace dwf
@@ -65,9 +72,12 @@ struct dwf_geometry {
     // planar over sites: [leg][18 reals in 128-bit vectors][cb site]; leg = 2*mu + (0: fwd, 1: bwd)
     void *gauge[2];
     size_t gauge_bytes;     // per parity
-    // CTA tile tables (origins in rasterised launch order), one for cb kernels, one for full
-    dwf::Tiling tiling_cb, tiling_full;
-    int4 *tiles_cb, *tiles_full;
+    // direct kernel: CTA tile table (origins in rasterised launch order)
+    dwf::Tiling tiling_cb;
+    int4 *tiles_cb;
+    // staged (TMA, link-stationary) kernel: plan chosen at create time, row-box tile table
+    dwf::StagedPlan staged;
+    int4 *tiles_staged;
     // reductions
     double *partials;       // [2 * max_blocks]
     double *result_dev;     // [2]
@@ -78,8 +88,10 @@ struct dwf_geometry {
     // tunables (dwf_set_option)
     int opt_tile[4];        // requested log2 tile extents (cb: dim 0 in pairs)
     int opt_cpc;
-    int opt_raster;         // rasterisation order of the tile table
-    int opt_variant;
+    int opt_raster;         // rasterisation order of the direct kernel's tile table
+    int opt_raster_staged;  // ... of the staged kernel's tile table
+    int opt_variant;        // restrict the staged kernel to one compiled variant (0: auto)
+    int opt_kernel;         // 0: auto, 1: direct only, 2: staged only
 };
 
 namespace dwf {
@@ -92,8 +104,12 @@ int launch_import(const dwf_geometry *g, const void *canonical_dev, int parity, 
                   cudaStream_t st);
 int launch_export(const dwf_geometry *g, const void *field, int parity, void *canonical_dev,
                   cudaStream_t st);
-// dhop.cu
-int launch_dhop(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st);
+// dhop.cu (direct kernel; half fields only)
+int launch_dhop_direct(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st);
+// dhop_staged.cu (TMA-staged link-stationary kernel, fp32 half fields)
+void plan_staged(dwf_geometry *g);                      // fills g->staged (variant = -1 if unusable)
+void build_staged_tile_table(const dwf_geometry *g, int raster, int4 *host_table);
+int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st);
 // reduce.cu
 int launch_norm2(const dwf_geometry *g, const void *field, size_t nreal, cudaStream_t st);
 int launch_inner(const dwf_geometry *g, const void *a, const void *b, size_t ncomplex,

@@ -1,36 +1,48 @@
 // pack.cu -- canonical <-> device layout conversion (hot path row a1 of SURVEY.md section 8).
 //
-// Spinor: canonical [site][s][k][reim]  <->  device complex[chunk][k][site][j], s = chunk*Sc + j.
+// Spinor: canonical [site][s][k][reim]  <->  device complex[s][k][cb site]  (k = spin*3 + colour),
+//         one such block per parity; a FULL field is the even block followed by the odd block
+//         (canonical site x -> parity p(x), cb site x>>1).
 // Gauge : canonical [x][mu][a][b][reim]  ->  for each output parity p and each output site of that
 //         parity (cb index x>>1) the 8 links that site multiplies with:
 //            leg 2*mu   : U_mu(x)                       (forward hop,  psi(x+mu))
 //            leg 2*mu+1 : U_mu(x-mu)^dagger             (backward hop, psi(x-mu))
 //         each times -1 when the hop wraps around an antiperiodic time direction, stored planar
-//         over sites as [leg][9 complex planes][cb site] (fp32: planes paired into float4 + a
-//         float2 tail; fp64: double2 planes).  Every canonical link appears exactly once in each
-//         parity set, so one half-Dhop still reads the whole gauge field exactly once.
+//         over sites as complex[leg][a*3+b][cb site].  Every canonical link appears exactly once
+//         in each parity set, so one half-Dhop still reads the whole gauge field exactly once.
 #include "dwf_internal.cuh"
 
 namespace dwf {
 
-template <typename T, bool IMPORT>
+// FULL = true: canonical sites are lexicographic x, the device field is [parity][s][k][Vh]
+// FULL = false: canonical sites are the cb sites of one parity, the device field is [s][k][Vh]
+template <typename T, bool IMPORT, bool FULL>
 __global__ void __launch_bounds__(256)
-spinor_reorder_kernel(const T *__restrict__ src, T *__restrict__ dst, long long nsites, int Ls, int Sc)
+spinor_reorder_kernel(const T *__restrict__ src, T *__restrict__ dst, const Lattice lat)
 {
     // one thread per complex element of the DEVICE layout (coalesced on the device side)
-    const long long n = nsites * Ls * 12;
-    const int nchunk = Ls / Sc;
+    using V = typename std::conditional<sizeof(T) == 4, float2, double2>::type;
+    const long long Vh = lat.Vh;
+    const long long n = (FULL ? 2 : 1) * Vh * lat.Ls * 12;
     for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n;
          e += (long long)gridDim.x * blockDim.x) {
         long long r = e;
-        const int j = (int)(r % Sc); r /= Sc;
-        const long long site = r % nsites; r /= nsites;
-        const int k = (int)(r % 12);
-        const int chunk = (int)(r / 12);
-        (void)nchunk;
-        const int s = chunk * Sc + j;
-        const long long c = ((site * Ls + s) * 12 + k);     // canonical complex index
-        using V = typename std::conditional<sizeof(T) == 4, float2, double2>::type;
+        const long long cb = r % Vh; r /= Vh;
+        const int k = (int)(r % 12); r /= 12;
+        const int s = (int)(r % lat.Ls);
+        const int par = (int)(r / lat.Ls);
+        long long site = cb;
+        if (FULL) {
+            // lexicographic x of cb site `cb` of parity `par`: x0 = 2*h + ((x1+x2+x3+par)&1)
+            long long q = cb;
+            const int h = (int)(q % lat.Lh); q /= lat.Lh;
+            const int x1 = (int)(q % lat.L[1]); q /= lat.L[1];
+            const int x2 = (int)(q % lat.L[2]);
+            const int x3 = (int)(q / lat.L[2]);
+            site = 2 * cb + ((x1 + x2 + x3 + par) & 1);
+            (void)h;
+        }
+        const long long c = ((site * lat.Ls + s) * 12 + k);     // canonical complex index
         if (IMPORT) reinterpret_cast<V *>(dst)[e] = reinterpret_cast<const V *>(src)[c];
         else        reinterpret_cast<V *>(dst)[c] = reinterpret_cast<const V *>(src)[e];
     }
@@ -79,14 +91,7 @@ gauge_pack_kernel(const T *__restrict__ U, T *__restrict__ set_even, T *__restri
                 if (bwd) { re = u[(b * 3 + a) * 2]; im = -u[(b * 3 + a) * 2 + 1]; }   // dagger
                 else     { re = u[(a * 3 + b) * 2]; im =  u[(a * 3 + b) * 2 + 1]; }
                 const int cidx = a * 3 + b;          // complex plane
-                size_t off;
-                if (sizeof(T) == 4) {
-                    // planes 0..7 paired into float4 vectors, plane 8 a float2 tail
-                    off = (cidx < 8) ? (size_t)(cidx >> 1) * 4 * lat.Vh + (size_t)cb * 4 + (cidx & 1) * 2
-                                     : (size_t)16 * lat.Vh + (size_t)cb * 2;
-                } else {
-                    off = (size_t)cidx * 2 * lat.Vh + (size_t)cb * 2;
-                }
+                const size_t off = (size_t)cidx * 2 * lat.Vh + (size_t)cb * 2;
                 legbase[off] = sign * re;
                 legbase[off + 1] = sign * im;
             }
@@ -117,14 +122,19 @@ int launch_pack_gauge(const dwf_geometry *g, const void *U_dev, cudaStream_t st)
 template <bool IMPORT>
 static int launch_reorder(const dwf_geometry *g, const void *src, void *dst, int parity, cudaStream_t st)
 {
-    const long long nsites = (parity == DWF_FULL) ? g->lat.V4 : g->lat.Vh;
-    const int grid = grid_for(nsites * g->lat.Ls * 12, g->sm_count);
-    if (g->prec == DWF_F32)
-        spinor_reorder_kernel<float, IMPORT><<<grid, 256, 0, st>>>(static_cast<const float *>(src), static_cast<float *>(dst),
-                                                                  nsites, g->lat.Ls, g->lat.Sc);
-    else
-        spinor_reorder_kernel<double, IMPORT><<<grid, 256, 0, st>>>(static_cast<const double *>(src), static_cast<double *>(dst),
-                                                                   nsites, g->lat.Ls, g->lat.Sc);
+    const bool full = parity == DWF_FULL;
+    const int grid = grid_for((full ? 2 : 1) * g->lat.Vh * g->lat.Ls * 12, g->sm_count);
+    if (g->prec == DWF_F32) {
+        auto *a = static_cast<const float *>(src);
+        auto *b = static_cast<float *>(dst);
+        if (full) spinor_reorder_kernel<float, IMPORT, true><<<grid, 256, 0, st>>>(a, b, g->lat);
+        else      spinor_reorder_kernel<float, IMPORT, false><<<grid, 256, 0, st>>>(a, b, g->lat);
+    } else {
+        auto *a = static_cast<const double *>(src);
+        auto *b = static_cast<double *>(dst);
+        if (full) spinor_reorder_kernel<double, IMPORT, true><<<grid, 256, 0, st>>>(a, b, g->lat);
+        else      spinor_reorder_kernel<double, IMPORT, false><<<grid, 256, 0, st>>>(a, b, g->lat);
+    }
     count_launch();
     DWF_CUDA_CHECK(cudaGetLastError());
     return DWF_OK;

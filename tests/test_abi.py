@@ -65,7 +65,6 @@ def test_null_arguments():
     assert lib.dwf_norm2(None, None, 0, ctypes.byref(r), None) == dwf.ERR_INVALID_ARG
     assert r.value == -1.0                                  # outputs untouched on error
     assert lib.dwf_field_bytes(None, 0) == 0
-    assert lib.dwf_layout_sc(None) == 0
     assert lib.dwf_destroy_geometry(None) == dwf.OK
     assert b"NULL" in lib.dwf_last_error() or lib.dwf_last_error() != b""
 
