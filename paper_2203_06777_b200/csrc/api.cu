@@ -197,6 +197,9 @@ int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, i
     g->opt_raster_staged = 1;
     g->opt_variant = 0;
     g->opt_kernel = 0;
+    g->opt_l2pol = 11212020;     // out, links evict_first; x3+ evict_last; x3- evict_first; top layer evict_last
+    g->opt_ssplit = 1;
+    g->opt_prefetch_links = 0;
 
     g->gauge_bytes = (size_t)8 * 18 * (size_t)g->lat.Vh * (size_t)precision;
     g->reduce_blocks = g->sm_count * 8;
@@ -247,6 +250,27 @@ int dwf_set_option(dwf_geometry *g, const char *key, long long value)
         g->opt_raster_staged = v;
     } else if (!strcmp(key, "variant")) {
         g->opt_variant = v;          // 0: best staged tile, n > 0: n-th compiled staged variant only
+    } else if (!strcmp(key, "l2pol")) {
+        g->opt_l2pol = v;
+        return DWF_OK;
+    } else if (!strcmp(key, "ablate")) {
+        g->opt_ablate = v;
+        return DWF_OK;
+    } else if (!strcmp(key, "prefetch_links")) {
+        g->opt_prefetch_links = v != 0;
+        return DWF_OK;
+    } else if (!strcmp(key, "l2persist")) {
+        // MB of L2 set aside for evict_last ("persisting") lines; device-wide CUDA limit
+        int maxb = 0;
+        DWF_CUDA_CHECK(cudaDeviceGetAttribute(&maxb, cudaDevAttrMaxPersistingL2CacheSize, g->device));
+        size_t want = (size_t)(v < 0 ? 0 : v) << 20;
+        if (want > (size_t)maxb) want = (size_t)maxb;
+        DWF_CUDA_CHECK(cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want));
+        return DWF_OK;
+    } else if (!strcmp(key, "ssplit")) {
+        if (v < 1) { set_error("ssplit must be >= 1"); return DWF_ERR_INVALID_ARG; }
+        g->opt_ssplit = v;
+        return DWF_OK;
     } else if (!strcmp(key, "kernel")) {
         if (v < 0 || v > 2) { set_error("kernel must be 0 (auto), 1 (direct) or 2 (staged)"); return DWF_ERR_INVALID_ARG; }
         g->opt_kernel = v;

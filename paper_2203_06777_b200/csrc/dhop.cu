@@ -24,28 +24,27 @@
 
 namespace dwf {
 
-// gauge storage: per leg 9 complex planes over the Vh output sites of one parity
+// gauge storage: complex[row][leg*9 + a*3+b][h]; `leg` points at component 0 of this site's leg
 template <typename T>
-__device__ __forceinline__ void load_link(const T *leg, long long Vh, int site, typename CxT<T>::type (&U)[9])
+__device__ __forceinline__ void load_link(const typename CxT<T>::type *leg, int W0, typename CxT<T>::type (&U)[9])
 {
-    using C = typename CxT<T>::type;
 #pragma unroll
-    for (int v = 0; v < 9; v++) U[v] = __ldg(reinterpret_cast<const C *>(leg + (size_t)v * 2 * Vh) + site);
+    for (int v = 0; v < 9; v++) U[v] = __ldg(leg + v * W0);
 }
 
 // one leg: acc += reconstruct( U * project(psi_neighbour) )
 template <typename T, int SC, int MU, bool FWD, bool FIRST>
 __device__ __forceinline__ void dhop_leg(typename CxT<T>::type (&acc)[12][SC],
                                          const typename CxT<T>::type *__restrict__ nb,  // neighbour, component 0
-                                         size_t kstride,                                // complex elements between components
-                                         const T *__restrict__ leg_links, long long Vh, int gsite)
+                                         int kstride,                                   // complex elements between components (= Lh)
+                                         const typename CxT<T>::type *__restrict__ leg_links)
 {
     using C = typename CxT<T>::type;
     C psi[12][SC];
 #pragma unroll
-    for (int k = 0; k < 12; k++) load_cx<SC>(nb + (size_t)k * kstride, psi[k]);
+    for (int k = 0; k < 12; k++) load_cx<SC>(nb + k * kstride, psi[k]);
     C U[9];
-    load_link<T>(leg_links, Vh, gsite, U);
+    load_link<T>(leg_links, kstride, U);
 
 #pragma unroll
     for (int j = 0; j < SC; j++) {
@@ -115,7 +114,7 @@ __device__ __forceinline__ void dhop_leg(typename CxT<T>::type (&acc)[12][SC],
 
 // ---------------------------------------------------------------------------------------------
 // direct kernel: neighbours are read straight from global memory (L1/L2 catch the reuse).
-// in/out are half fields complex[s][k][Vh]; out has parity `parity_out`, in the opposite parity.
+// in/out are half fields complex[s][row][k][h]; out has parity `parity_out`, in the opposite parity.
 // One thread = one output site and one s-slice.
 // ---------------------------------------------------------------------------------------------
 template <typename T, int MAXT, int MINB>
@@ -141,42 +140,43 @@ dhop_direct_kernel(const typename CxT<T>::type *__restrict__ in, typename CxT<T>
     const int L1 = lat.L[1], L2 = lat.L[2], L3 = lat.L[3];
     const int W0 = lat.Lh;                           // row length in field sites
     const long long Vh = lat.Vh;
-    const size_t kstride = (size_t)Vh;
 
-    const int row = x1 + L1 * (x2 + L2 * x3);
-    const int site = c0 + W0 * row;
-    const int gsite = site;
+    // a row (lattice line along x0) is a block of 12*W0 complex: [k][h]
+    const long long row = x1 + L1 * (x2 + (long long)L2 * x3);
+    const long long rs = 12 * W0;                    // complex elements per row
+    const long long own = row * rs + c0;
 
-    // neighbour site indices
+    // neighbour element offsets (component 0)
     const int r = (x1 + x2 + x3 + parity_out) & 1;          // x0 = 2*c0 + r
     int hp = c0 + r;       if (hp == W0) hp = 0;
     int hm = c0 - 1 + r;   if (hm < 0) hm = W0 - 1;
-    const int n0p = hp + W0 * row;
-    const int n0m = hm + W0 * row;
-    const int s1 = W0, s2 = W0 * L1, s3 = W0 * L1 * L2;
-    const int n1p = site + (x1 + 1 == L1 ? -(L1 - 1) * s1 : s1);
-    const int n1m = site + (x1 == 0 ? (L1 - 1) * s1 : -s1);
-    const int n2p = site + (x2 + 1 == L2 ? -(L2 - 1) * s2 : s2);
-    const int n2m = site + (x2 == 0 ? (L2 - 1) * s2 : -s2);
-    const int n3p = site + (x3 + 1 == L3 ? -(L3 - 1) * s3 : s3);
-    const int n3m = site + (x3 == 0 ? (L3 - 1) * s3 : -s3);
+    const long long n0p = row * rs + hp;
+    const long long n0m = row * rs + hm;
+    const long long s1 = rs, s2 = rs * L1, s3 = rs * L1 * L2;
+    const long long n1p = own + (x1 + 1 == L1 ? -(L1 - 1) * s1 : s1);
+    const long long n1m = own + (x1 == 0 ? (L1 - 1) * s1 : -s1);
+    const long long n2p = own + (x2 + 1 == L2 ? -(L2 - 1) * s2 : s2);
+    const long long n2m = own + (x2 == 0 ? (L2 - 1) * s2 : -s2);
+    const long long n3p = own + (x3 + 1 == L3 ? -(L3 - 1) * s3 : s3);
+    const long long n3m = own + (x3 == 0 ? (L3 - 1) * s3 : -s3);
 
-    const C *base = in + (size_t)s * 12 * kstride;
-    const size_t lstride = (size_t)18 * Vh;          // reals per leg
+    const C *base = in + (size_t)s * 12 * (size_t)Vh;
+    const C *gl = reinterpret_cast<const C *>(gset) + (size_t)row * 72 * W0 + c0;   // this site's links
+    const int ls9 = 9 * W0;                          // complex elements per leg
 
     C acc[12][SC];
-    dhop_leg<T, SC, 0, true,  true >(acc, base + n0p, kstride, gset + 0 * lstride, Vh, gsite);
-    dhop_leg<T, SC, 0, false, false>(acc, base + n0m, kstride, gset + 1 * lstride, Vh, gsite);
-    dhop_leg<T, SC, 1, true,  false>(acc, base + n1p, kstride, gset + 2 * lstride, Vh, gsite);
-    dhop_leg<T, SC, 1, false, false>(acc, base + n1m, kstride, gset + 3 * lstride, Vh, gsite);
-    dhop_leg<T, SC, 2, true,  false>(acc, base + n2p, kstride, gset + 4 * lstride, Vh, gsite);
-    dhop_leg<T, SC, 2, false, false>(acc, base + n2m, kstride, gset + 5 * lstride, Vh, gsite);
-    dhop_leg<T, SC, 3, true,  false>(acc, base + n3p, kstride, gset + 6 * lstride, Vh, gsite);
-    dhop_leg<T, SC, 3, false, false>(acc, base + n3m, kstride, gset + 7 * lstride, Vh, gsite);
+    dhop_leg<T, SC, 0, true,  true >(acc, base + n0p, W0, gl + 0 * ls9);
+    dhop_leg<T, SC, 0, false, false>(acc, base + n0m, W0, gl + 1 * ls9);
+    dhop_leg<T, SC, 1, true,  false>(acc, base + n1p, W0, gl + 2 * ls9);
+    dhop_leg<T, SC, 1, false, false>(acc, base + n1m, W0, gl + 3 * ls9);
+    dhop_leg<T, SC, 2, true,  false>(acc, base + n2p, W0, gl + 4 * ls9);
+    dhop_leg<T, SC, 2, false, false>(acc, base + n2m, W0, gl + 5 * ls9);
+    dhop_leg<T, SC, 3, true,  false>(acc, base + n3p, W0, gl + 6 * ls9);
+    dhop_leg<T, SC, 3, false, false>(acc, base + n3m, W0, gl + 7 * ls9);
 
-    C *o = out + (size_t)s * 12 * kstride + (size_t)site;
+    C *o = out + (size_t)s * 12 * (size_t)Vh + (size_t)own;
 #pragma unroll
-    for (int k = 0; k < 12; k++) store_cx<SC>(o + (size_t)k * kstride, acc[k]);
+    for (int k = 0; k < 12; k++) store_cx<SC>(o + k * W0, acc[k]);
 }
 
 template <typename T, int MAXT, int MINB>

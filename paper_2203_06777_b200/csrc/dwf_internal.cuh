@@ -92,6 +92,10 @@ struct dwf_geometry {
     int opt_raster_staged;  // ... of the staged kernel's tile table
     int opt_variant;        // restrict the staged kernel to one compiled variant (0: auto)
     int opt_kernel;         // 0: auto, 1: direct only, 2: staged only
+    int opt_l2pol;          // staged kernel: L2 eviction-priority digits (dhop_staged.cu PC_*)
+    int opt_ssplit;         // staged kernel: CTAs sharing one tile (each takes Ls / ssplit slices)
+    int opt_ablate;         // staged kernel: timing experiments (dhop_staged.cu StagedArgs::ablate)
+    int opt_prefetch_links; // staged kernel: L2-prefetch the next tile's links one tile ahead
 };
 
 namespace dwf {

@@ -1,21 +1,23 @@
 // pack.cu -- canonical <-> device layout conversion (hot path row a1 of SURVEY.md section 8).
 //
-// Spinor: canonical [site][s][k][reim]  <->  device complex[s][k][cb site]  (k = spin*3 + colour),
-//         one such block per parity; a FULL field is the even block followed by the odd block
-//         (canonical site x -> parity p(x), cb site x>>1).
+// Spinor: canonical [site][s][k][reim]  <->  device complex[s][row][k][h]  (k = spin*3 + colour;
+//         row = x1 + L1*(x2 + L2*x3) is a lattice line along x0, h = x0>>1 the site of the parity
+//         on that line, so the cb site x>>1 is row*Lh + h), one such block per parity; a FULL
+//         field is the even block followed by the odd block (canonical site x -> parity p(x)).
 // Gauge : canonical [x][mu][a][b][reim]  ->  for each output parity p and each output site of that
 //         parity (cb index x>>1) the 8 links that site multiplies with:
 //            leg 2*mu   : U_mu(x)                       (forward hop,  psi(x+mu))
 //            leg 2*mu+1 : U_mu(x-mu)^dagger             (backward hop, psi(x-mu))
 //         each times -1 when the hop wraps around an antiperiodic time direction, stored planar
-//         over sites as complex[leg][a*3+b][cb site].  Every canonical link appears exactly once
-//         in each parity set, so one half-Dhop still reads the whole gauge field exactly once.
+//         row by row as complex[row][leg*9 + a*3+b][h] (the 72 link components of the Lh output
+//         sites of a row are one contiguous 576*Lh-byte block).  Every canonical link appears
+//         exactly once in each parity set, so one half-Dhop reads the whole gauge field once.
 #include "dwf_internal.cuh"
 
 namespace dwf {
 
-// FULL = true: canonical sites are lexicographic x, the device field is [parity][s][k][Vh]
-// FULL = false: canonical sites are the cb sites of one parity, the device field is [s][k][Vh]
+// FULL = true: canonical sites are lexicographic x, the device field is [parity][s][row][k][h]
+// FULL = false: canonical sites are the cb sites of one parity, the device field is [s][row][k][h]
 template <typename T, bool IMPORT, bool FULL>
 __global__ void __launch_bounds__(256)
 spinor_reorder_kernel(const T *__restrict__ src, T *__restrict__ dst, const Lattice lat)
@@ -23,24 +25,25 @@ spinor_reorder_kernel(const T *__restrict__ src, T *__restrict__ dst, const Latt
     // one thread per complex element of the DEVICE layout (coalesced on the device side)
     using V = typename std::conditional<sizeof(T) == 4, float2, double2>::type;
     const long long Vh = lat.Vh;
+    const long long nrow = Vh / lat.Lh;
     const long long n = (FULL ? 2 : 1) * Vh * lat.Ls * 12;
     for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n;
          e += (long long)gridDim.x * blockDim.x) {
         long long r = e;
-        const long long cb = r % Vh; r /= Vh;
+        const int h = (int)(r % lat.Lh); r /= lat.Lh;
         const int k = (int)(r % 12); r /= 12;
+        const long long row = r % nrow; r /= nrow;
         const int s = (int)(r % lat.Ls);
         const int par = (int)(r / lat.Ls);
+        const long long cb = row * lat.Lh + h;
         long long site = cb;
         if (FULL) {
             // lexicographic x of cb site `cb` of parity `par`: x0 = 2*h + ((x1+x2+x3+par)&1)
-            long long q = cb;
-            const int h = (int)(q % lat.Lh); q /= lat.Lh;
+            long long q = row;
             const int x1 = (int)(q % lat.L[1]); q /= lat.L[1];
             const int x2 = (int)(q % lat.L[2]);
             const int x3 = (int)(q / lat.L[2]);
             site = 2 * cb + ((x1 + x2 + x3 + par) & 1);
-            (void)h;
         }
         const long long c = ((site * lat.Ls + s) * 12 + k);     // canonical complex index
         if (IMPORT) reinterpret_cast<V *>(dst)[e] = reinterpret_cast<const V *>(src)[c];
@@ -82,7 +85,9 @@ gauge_pack_kernel(const T *__restrict__ U, T *__restrict__ set_even, T *__restri
             if (antiperiodic_t && mu == 3 && c[3] == lat.L[3] - 1) sign = -1;
         }
         const T *u = U + (src_site * 4 + mu) * 18;
-        T *legbase = set + (size_t)leg * 18 * lat.Vh;
+        const long long row = cb / lat.Lh;
+        const int h = (int)(cb % lat.Lh);
+        T *legbase = set + ((size_t)row * 72 + (size_t)leg * 9) * 2 * lat.Lh + 2 * h;
 #pragma unroll
         for (int a = 0; a < 3; a++)
 #pragma unroll
@@ -91,7 +96,7 @@ gauge_pack_kernel(const T *__restrict__ U, T *__restrict__ set_even, T *__restri
                 if (bwd) { re = u[(b * 3 + a) * 2]; im = -u[(b * 3 + a) * 2 + 1]; }   // dagger
                 else     { re = u[(a * 3 + b) * 2]; im =  u[(a * 3 + b) * 2 + 1]; }
                 const int cidx = a * 3 + b;          // complex plane
-                const size_t off = (size_t)cidx * 2 * lat.Vh + (size_t)cb * 2;
+                const size_t off = (size_t)cidx * 2 * lat.Lh;
                 legbase[off] = sign * re;
                 legbase[off + 1] = sign * im;
             }
