@@ -24,27 +24,31 @@
 
 namespace dwf {
 
-// gauge storage: complex[row][leg*9 + a*3+b][h]; `leg` points at component 0 of this site's leg
-template <typename T>
-__device__ __forceinline__ void load_link(const typename CxT<T>::type *leg, int W0, typename CxT<T>::type (&U)[9])
+// element offset of component c of a site inside a row block stored as [c/2][h][c&1]; `W0` = Lh,
+// the pointer it is added to already points at (component 0, this site) = row base + 2*h
+__device__ __forceinline__ int pair_off(int c, int W0) { return (c >> 1) * 2 * W0 + (c & 1); }
+
+// gauge storage: complex[row][f/2][h][f&1], f = leg*9 + a*3+b; `site_links` points at f = 0 of this site
+template <typename T, int LEG>
+__device__ __forceinline__ void load_link(const typename CxT<T>::type *site_links, int W0, typename CxT<T>::type (&U)[9])
 {
 #pragma unroll
-    for (int v = 0; v < 9; v++) U[v] = __ldg(leg + v * W0);
+    for (int v = 0; v < 9; v++) U[v] = __ldg(site_links + pair_off(LEG * 9 + v, W0));
 }
 
 // one leg: acc += reconstruct( U * project(psi_neighbour) )
-template <typename T, int SC, int MU, bool FWD, bool FIRST>
+template <typename T, int SC, int MU, bool FWD, bool FIRST, int LEG>
 __device__ __forceinline__ void dhop_leg(typename CxT<T>::type (&acc)[12][SC],
                                          const typename CxT<T>::type *__restrict__ nb,  // neighbour, component 0
-                                         int kstride,                                   // complex elements between components (= Lh)
-                                         const typename CxT<T>::type *__restrict__ leg_links)
+                                         int W0,                                        // Lh
+                                         const typename CxT<T>::type *__restrict__ site_links)
 {
     using C = typename CxT<T>::type;
     C psi[12][SC];
 #pragma unroll
-    for (int k = 0; k < 12; k++) load_cx<SC>(nb + k * kstride, psi[k]);
+    for (int k = 0; k < 12; k++) load_cx<SC>(nb + pair_off(k, W0), psi[k]);
     C U[9];
-    load_link<T>(leg_links, kstride, U);
+    load_link<T, LEG>(site_links, W0, U);
 
 #pragma unroll
     for (int j = 0; j < SC; j++) {
@@ -114,7 +118,7 @@ __device__ __forceinline__ void dhop_leg(typename CxT<T>::type (&acc)[12][SC],
 
 // ---------------------------------------------------------------------------------------------
 // direct kernel: neighbours are read straight from global memory (L1/L2 catch the reuse).
-// in/out are half fields complex[s][row][k][h]; out has parity `parity_out`, in the opposite parity.
+// in/out are half fields complex[s][row][k/2][h][k&1]; out has parity `parity_out`, in the opposite parity.
 // One thread = one output site and one s-slice.
 // ---------------------------------------------------------------------------------------------
 template <typename T, int MAXT, int MINB>
@@ -141,17 +145,17 @@ dhop_direct_kernel(const typename CxT<T>::type *__restrict__ in, typename CxT<T>
     const int W0 = lat.Lh;                           // row length in field sites
     const long long Vh = lat.Vh;
 
-    // a row (lattice line along x0) is a block of 12*W0 complex: [k][h]
+    // a row (lattice line along x0) is a block of 12*W0 complex: [k/2][h][k&1]
     const long long row = x1 + L1 * (x2 + (long long)L2 * x3);
     const long long rs = 12 * W0;                    // complex elements per row
-    const long long own = row * rs + c0;
+    const long long own = row * rs + 2 * c0;
 
     // neighbour element offsets (component 0)
     const int r = (x1 + x2 + x3 + parity_out) & 1;          // x0 = 2*c0 + r
     int hp = c0 + r;       if (hp == W0) hp = 0;
     int hm = c0 - 1 + r;   if (hm < 0) hm = W0 - 1;
-    const long long n0p = row * rs + hp;
-    const long long n0m = row * rs + hm;
+    const long long n0p = row * rs + 2 * hp;
+    const long long n0m = row * rs + 2 * hm;
     const long long s1 = rs, s2 = rs * L1, s3 = rs * L1 * L2;
     const long long n1p = own + (x1 + 1 == L1 ? -(L1 - 1) * s1 : s1);
     const long long n1m = own + (x1 == 0 ? (L1 - 1) * s1 : -s1);
@@ -161,22 +165,21 @@ dhop_direct_kernel(const typename CxT<T>::type *__restrict__ in, typename CxT<T>
     const long long n3m = own + (x3 == 0 ? (L3 - 1) * s3 : -s3);
 
     const C *base = in + (size_t)s * 12 * (size_t)Vh;
-    const C *gl = reinterpret_cast<const C *>(gset) + (size_t)row * 72 * W0 + c0;   // this site's links
-    const int ls9 = 9 * W0;                          // complex elements per leg
+    const C *gl = reinterpret_cast<const C *>(gset) + (size_t)row * 72 * W0 + 2 * c0;   // this site's links
 
     C acc[12][SC];
-    dhop_leg<T, SC, 0, true,  true >(acc, base + n0p, W0, gl + 0 * ls9);
-    dhop_leg<T, SC, 0, false, false>(acc, base + n0m, W0, gl + 1 * ls9);
-    dhop_leg<T, SC, 1, true,  false>(acc, base + n1p, W0, gl + 2 * ls9);
-    dhop_leg<T, SC, 1, false, false>(acc, base + n1m, W0, gl + 3 * ls9);
-    dhop_leg<T, SC, 2, true,  false>(acc, base + n2p, W0, gl + 4 * ls9);
-    dhop_leg<T, SC, 2, false, false>(acc, base + n2m, W0, gl + 5 * ls9);
-    dhop_leg<T, SC, 3, true,  false>(acc, base + n3p, W0, gl + 6 * ls9);
-    dhop_leg<T, SC, 3, false, false>(acc, base + n3m, W0, gl + 7 * ls9);
+    dhop_leg<T, SC, 0, true,  true , 0>(acc, base + n0p, W0, gl);
+    dhop_leg<T, SC, 0, false, false, 1>(acc, base + n0m, W0, gl);
+    dhop_leg<T, SC, 1, true,  false, 2>(acc, base + n1p, W0, gl);
+    dhop_leg<T, SC, 1, false, false, 3>(acc, base + n1m, W0, gl);
+    dhop_leg<T, SC, 2, true,  false, 4>(acc, base + n2p, W0, gl);
+    dhop_leg<T, SC, 2, false, false, 5>(acc, base + n2m, W0, gl);
+    dhop_leg<T, SC, 3, true,  false, 6>(acc, base + n3p, W0, gl);
+    dhop_leg<T, SC, 3, false, false, 7>(acc, base + n3m, W0, gl);
 
     C *o = out + (size_t)s * 12 * (size_t)Vh + (size_t)own;
 #pragma unroll
-    for (int k = 0; k < 12; k++) store_cx<SC>(o + k * W0, acc[k]);
+    for (int k = 0; k < 12; k++) store_cx<SC>(o + pair_off(k, W0), acc[k]);
 }
 
 template <typename T, int MAXT, int MINB>

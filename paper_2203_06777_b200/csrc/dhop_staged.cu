@@ -26,9 +26,11 @@
 //     All complex arithmetic is packed f32x2 (FFMA2 / FADD2): u*h is accumulated as two chains
 //     A = sum u.re*h and B = sum u.im*h, combined once as A + iB, so that no operand needs a
 //     half-negated copy.
-// Global layouts: spinor complex[s][row][k][h], links complex[row][leg*9+c][h] (pack.cu).
-// Shared-memory image of one slice: [row of the staged region][k = spin*3+colour][Lh] complex,
+// Global layouts: spinor complex[s][row][k/2][h][k&1], links complex[row][f/2][h][f&1] (pack.cu):
+// two components of a site form one 128-bit vector, so every LDS / LDG / STG is 128 bits wide.
+// Shared-memory image of one slice: [row of the staged region][k/2][Lh][k&1] complex,
 // regions in the order centre, x1-, x1+, x2-, x2+, x3-, x3+; inside a region x3 layer slowest.
+#include <type_traits>
 #include <vector>
 
 #include "complex_ops.cuh"
@@ -65,7 +67,8 @@ struct StagedArgs {
     int ssplit;              // CTAs sharing one tile, each walking Ls / ssplit slices
     int parity_out;
     int l2pol;               // decimal digits, see PC_*
-    int prefetch_links;      // bulk-prefetch the next tile's links into L2 one tile ahead
+    int zigzag;              // walk the slices of every other tile backwards
+    int barrier;             // 1: CTA barrier + thread 0 refills; 0: the last warp to release a buffer refills it
     int ablate;              // timing experiments only (wrong results): 1 no link refill, 2 no stores, 4 no legs, 8 no TMA
 };
 
@@ -86,13 +89,34 @@ template <int LH, int B1, int B2, int B3> struct StagedCfg {
     static_assert(ROWB % 128 == 0, "staged rows must keep TMA destinations 128-byte aligned");
 };
 
+#ifndef DWF_ABL
+#define DWF_ABL 0      // timing experiments: 1 = legs without shared-memory reads, 2 = legs without arithmetic
+#endif
+
 // one leg: acc += reconstruct( U * project(psi) ), psi read from shared memory
-template <int LH, int MU, bool FWD, bool FIRST>
-__device__ __forceinline__ void staged_leg(float2 (&acc)[12], const float2 *__restrict__ nb, const float2 (&U)[9])
+template <int LH, int MU, bool FWD, bool FIRST, int ABL = 0>
+__device__ __forceinline__ void staged_leg(float2 (&acc)[12], const float4 *__restrict__ nb, const float2 *__restrict__ U)
 {
     float2 p[12];
+    if constexpr (ABL == 1) {          // timing experiment: no shared-memory reads
 #pragma unroll
-    for (int k = 0; k < 12; k++) p[k] = nb[k * LH];
+        for (int k = 0; k < 12; k++) p[k] = FIRST ? U[k % 9] : acc[k];
+    } else {
+#pragma unroll
+        for (int j = 0; j < 6; j++) {      // LDS.128: components 2j and 2j+1 of the neighbour site
+            const float4 q = nb[j * LH];
+            p[2 * j] = make_float2(q.x, q.y);
+            p[2 * j + 1] = make_float2(q.z, q.w);
+        }
+    }
+    if constexpr (ABL == 2) {          // timing experiment: no arithmetic
+#pragma unroll
+        for (int k = 0; k < 12; k++) {
+            if (FIRST) acc[k] = p[k];
+            else { acc[k].x = __int_as_float(__float_as_int(acc[k].x) ^ __float_as_int(p[k].x)); acc[k].y = __int_as_float(__float_as_int(acc[k].y) ^ __float_as_int(p[k].y)); }
+        }
+        return;
+    }
     float2 h0[3], h1[3];
 #pragma unroll
     for (int c = 0; c < 3; c++) {
@@ -188,7 +212,6 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     const int my_tiles = (args.ntiles - group + ngroup - 1) / ngroup;
     const int nsteps = my_tiles * nsl;
     if (nsteps <= 0) return;
-
     // L2 policies: the producer thread reads the TMA ones from shared memory (keeps them out of
     // the compute threads' registers); every thread holds the two it uses itself
     uint64_t *pol = reinterpret_cast<uint64_t *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + 16);
@@ -203,7 +226,8 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     // producer: stage the input of step g (slice g % nsl of this CTA's (g / nsl)-th tile) into
     // buffer g & 1; run by one thread (whichever warp freed the buffer last)
     auto issue = [&](int g) {
-        const int it = g / nsl, s = s_first + g % nsl, stage = g & 1;
+        const int it = g / nsl, i = g % nsl, stage = g & 1;
+        const int s = s_first + ((args.zigzag && (it & 1)) ? nsl - 1 - i : i);
         const int4 o = args.tiles[group + it * ngroup];
         const uint32_t bar = bar_base + 8 * stage;
         const uint32_t dst = smem_base + stage * Cfg::STAGE_BYTES;
@@ -227,16 +251,6 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         }
         tma_load_5d_hint(dst + Cfg::R_X3M * Cfg::ROWB, &map_c, bar, 0, 0, o.x, o.y, sb + x3m, pol[PC_X3M]);
         tma_load_5d_hint(dst + Cfg::R_X3P * Cfg::ROWB, &map_c, bar, 0, 0, o.x, o.y, sb + x3p, pol[PC_X3P]);
-        // pull this step's share of the NEXT tile's links into L2 (a row's 72 components are one
-        // contiguous block), so that the register refill during the last slice is not a trip to HBM
-        if (args.prefetch_links && it + 1 < my_tiles) {
-            const int4 on = args.tiles[group + (it + 1) * ngroup];
-            const int per = (Cfg::NROW_C + nsl - 1) / nsl;
-            for (int j = (g % nsl) * per; j < (g % nsl + 1) * per && j < Cfg::NROW_C; j++) {
-                const long long rown = on.x + j % B1 + (long long)L1 * (on.y + (j / B1) % B2 + (long long)L2 * (on.z + j / (B1 * B2)));
-                bulk_prefetch_l2(args.gauge + rown * (72 * LH), 72 * LH * 8);
-            }
-        }
     };
 
     if (tid == 0) {
@@ -264,12 +278,12 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     const int r3p = (i3 + 1 < B3) ? rc + B1 * B2 : Cfg::R_X3P + i1 + B1 * i2;
     const int r3m = (i3 > 0) ? rc - B1 * B2 : Cfg::R_X3M + i1 + B1 * i2;
     uint32_t off[8];            // byte offsets of the 8 neighbour spinors inside a stage
-    off[2] = r1p * Cfg::ROWB + h * 8;
-    off[3] = r1m * Cfg::ROWB + h * 8;
-    off[4] = r2p * Cfg::ROWB + h * 8;
-    off[5] = r2m * Cfg::ROWB + h * 8;
-    off[6] = r3p * Cfg::ROWB + h * 8;
-    off[7] = r3m * Cfg::ROWB + h * 8;
+    off[2] = r1p * Cfg::ROWB + h * 16;
+    off[3] = r1m * Cfg::ROWB + h * 16;
+    off[4] = r2p * Cfg::ROWB + h * 16;
+    off[5] = r2m * Cfg::ROWB + h * 16;
+    off[6] = r3p * Cfg::ROWB + h * 16;
+    off[7] = r3m * Cfg::ROWB + h * 16;
 
     // global row of this thread's site in the it-th tile, and the parity bit r of x0 = 2h + r
     auto tile_row = [&](int it, int &r) -> long long {
@@ -281,23 +295,62 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     auto set_x0_offsets = [&](int r) {
         int hp = h + r;       if (hp == LH) hp = 0;
         int hm = h - 1 + r;   if (hm < 0) hm = LH - 1;
-        off[0] = rc * Cfg::ROWB + hp * 8;
-        off[1] = rc * Cfg::ROWB + hm * 8;
+        off[0] = rc * Cfg::ROWB + hp * 16;
+        off[1] = rc * Cfg::ROWB + hm * 16;
     };
 
-    const long long slice_elems = 12LL * LH * args.L1 * args.L2 * args.L3;   // complex per slice
-    float2 U[8][9];
+    const long long slice_vecs = 6LL * LH * args.L1 * args.L2 * args.L3;   // 128-bit vectors per slice
+    float2 U[72];               // the 8 links of this site, component f = leg*9 + a*3+b
     int r_cur;
     long long grow = tile_row(0, r_cur);
     set_x0_offsets(r_cur);
-    float2 *optr = args.out + grow * (12 * LH) + h + (long long)s_first * slice_elems;
+    float4 *optr = reinterpret_cast<float4 *>(args.out) + grow * (6 * LH) + h + (long long)s_first * slice_vecs;
     if (active) {
-        const float2 *gp = args.gauge + grow * (72 * LH) + h;
+        const float4 *gp = reinterpret_cast<const float4 *>(args.gauge) + grow * (36 * LH) + h;
 #pragma unroll
-        for (int l = 0; l < 8; l++)
-#pragma unroll
-            for (int c = 0; c < 9; c++) U[l][c] = ldg_hint(gp + (l * 9 + c) * LH, pol_g);
+        for (int j = 0; j < 36; j++) {
+            const float4 q = ldg128_hint(gp + j * LH, pol_g);
+            U[2 * j] = make_float2(q.x, q.y);
+            U[2 * j + 1] = make_float2(q.z, q.w);
+        }
     }
+
+    // one slice of the tile: 8 legs out of the staged buffer, then the store.  FETCH = this is the
+    // tile's last slice: the registers of each link are refilled for the next tile right after
+    // the leg that used them last (two code copies, so that the common one carries no loads)
+    auto step = [&](auto fetch_tag, int stage, float4 *o, const float4 *gnext) {
+        constexpr bool FETCH = decltype(fetch_tag)::value;
+        const unsigned char *sb = smem + stage * Cfg::STAGE_BYTES;
+        float2 acc[12];
+#define DWF_LEG(L, MU, FWD, FIRST)                                                                  \
+        staged_leg<LH, MU, FWD, FIRST, DWF_ABL>(acc, reinterpret_cast<const float4 *>(sb + off[L]), U + 9 * (L)); \
+        if constexpr (FETCH) {      /* refill the component pairs whose last use was this leg */      \
+            _Pragma("unroll") for (int j = (9 * (L)) / 2; j < (9 * ((L) + 1)) / 2; j++) {            \
+                const float4 q = ldg128_hint(gnext + j * LH, pol_g);                                \
+                U[2 * j] = make_float2(q.x, q.y);                                                   \
+                U[2 * j + 1] = make_float2(q.z, q.w);                                               \
+            }                                                                                       \
+        }
+        DWF_LEG(0, 0, true,  true)
+        DWF_LEG(1, 0, false, false)
+        DWF_LEG(2, 1, true,  false)
+        DWF_LEG(3, 1, false, false)
+        DWF_LEG(4, 2, true,  false)
+        DWF_LEG(5, 2, false, false)
+        DWF_LEG(6, 3, true,  false)
+        DWF_LEG(7, 3, false, false)
+#undef DWF_LEG
+        if (!(args.ablate & 2)) {
+#pragma unroll
+            for (int j = 0; j < 6; j++)
+                stg128_hint(o + j * LH, make_float4(acc[2 * j].x, acc[2 * j].y, acc[2 * j + 1].x, acc[2 * j + 1].y), pol_o);
+        } else {                                // keep the arithmetic alive
+            float t = 0.f;
+#pragma unroll
+            for (int k = 0; k < 12; k++) t += acc[k].x * acc[k].y;
+            if (t == 1.2345f) stg128_hint(o, make_float4(acc[1].x, acc[1].y, t, t), pol_o);
+        }
+    };
 
     int g = 0;
     for (int it = 0; it < my_tiles; it++) {
@@ -305,43 +358,23 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         int r_next = r_cur;
         long long grow_next = grow;
         if (has_next) grow_next = tile_row(it + 1, r_next);
-        const float2 *gnext = args.gauge + grow_next * (72 * LH) + h;
+        const float4 *gnext = reinterpret_cast<const float4 *>(args.gauge) + grow_next * (36 * LH) + h;
         for (int s = 0; s < nsl; s++, g++) {
             const bool fetch = has_next && s == nsl - 1 && !(args.ablate & 1);     // refill the links during the last slice
             const int stage = g & 1;
             mbar_wait(bar_base + 8 * stage, (g >> 1) & 1);
             if (active && !(args.ablate & 4)) {
-                const unsigned char *sb = smem + stage * Cfg::STAGE_BYTES;
-                float2 acc[12];
-#define DWF_LEG(L, MU, FWD, FIRST)                                                                  \
-                staged_leg<LH, MU, FWD, FIRST>(acc, reinterpret_cast<const float2 *>(sb + off[L]), U[L]); \
-                if (fetch) {                                                                        \
-                    _Pragma("unroll") for (int c = 0; c < 9; c++)                                   \
-                        U[L][c] = ldg_hint(gnext + ((L) * 9 + c) * LH, pol_g);                      \
-                }
-                DWF_LEG(0, 0, true,  true)
-                DWF_LEG(1, 0, false, false)
-                DWF_LEG(2, 1, true,  false)
-                DWF_LEG(3, 1, false, false)
-                DWF_LEG(4, 2, true,  false)
-                DWF_LEG(5, 2, false, false)
-                DWF_LEG(6, 3, true,  false)
-                DWF_LEG(7, 3, false, false)
-#undef DWF_LEG
-                float2 *o = optr + (long long)s * slice_elems;
-                if (!(args.ablate & 2)) {
-#pragma unroll
-                    for (int k = 0; k < 12; k++) stg_hint(o + k * LH, acc[k], pol_o);
-                } else {                                // keep the arithmetic alive
-                    float t = 0.f;
-#pragma unroll
-                    for (int k = 0; k < 12; k++) t += acc[k].x * acc[k].y;
-                    if (t == 1.2345f) stg_hint(o, acc[1], pol_o);
-                }
+                const int sl = (args.zigzag && (it & 1)) ? nsl - 1 - s : s;
+                if (fetch) step(std::true_type{}, stage, optr + (long long)sl * slice_vecs, gnext);
+                else       step(std::false_type{}, stage, optr + (long long)sl * slice_vecs, gnext);
             }
             // This warp is done with the buffer (its results depend on every value it read).  No
             // CTA barrier: the warp that frees a buffer last refills it for step g + 2, everybody
             // else moves on to the next buffer at once.
+            if (args.barrier) {
+                __syncthreads();
+                if (tid == 0 && g + 2 < nsteps) issue(g + 2);
+            } else {
             __syncwarp();
             if ((tid & 31) == 0) {
                 __threadfence_block();
@@ -354,12 +387,13 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
                     }
                 }
             }
+            }
         }
         // tile switch
         grow = grow_next;
         r_cur = r_next;
         set_x0_offsets(r_cur);
-        optr = args.out + grow * (12 * LH) + h + (long long)s_first * slice_elems;
+        optr = reinterpret_cast<float4 *>(args.out) + grow * (6 * LH) + h + (long long)s_first * slice_vecs;
     }
 }
 
@@ -426,16 +460,16 @@ void build_staged_tile_table(const dwf_geometry *g, int raster, int4 *tab)
                     tab[id++] = make_int4(t1 * g->staged.b[0], (m * n2in + t2) * g->staged.b[1], t3 * g->staged.b[2], 0);
 }
 
-// tensor map of a half field complex[s][x3][x2][x1][k][h] seen as 5-D fp32 tensor
-// (2*Lh, 12, L1, L2, L3*Ls): x3 and s share the slowest dimension (the s stride is L3 x3-strides)
+// tensor map of a half field complex[s][x3][x2][x1][k/2][h][k&1] seen as 5-D fp32 tensor
+// (4*Lh, 6, L1, L2, L3*Ls): x3 and s share the slowest dimension (the s stride is L3 x3-strides)
 static int encode_map(CUtensorMap *m, const void *base, const Lattice &lat, int b1, int b2)
 {
     PFN_tensorMapEncodeTiled enc = get_tensor_map_encoder();
-    const cuuint64_t dims[5] = {(cuuint64_t)2 * lat.Lh, 12, (cuuint64_t)lat.L[1], (cuuint64_t)lat.L[2],
+    const cuuint64_t dims[5] = {(cuuint64_t)4 * lat.Lh, 6, (cuuint64_t)lat.L[1], (cuuint64_t)lat.L[2],
                                 (cuuint64_t)lat.L[3] * lat.Ls};
-    const cuuint64_t krow = (cuuint64_t)lat.Lh * 8, row = 12 * krow;
+    const cuuint64_t krow = (cuuint64_t)lat.Lh * 16, row = 6 * krow;
     const cuuint64_t strides[4] = {krow, row, row * lat.L[1], row * lat.L[1] * lat.L[2]};
-    const cuuint32_t box[5] = {(cuuint32_t)2 * lat.Lh, 12, (cuuint32_t)b1, (cuuint32_t)b2, 1};
+    const cuuint32_t box[5] = {(cuuint32_t)4 * lat.Lh, 6, (cuuint32_t)b1, (cuuint32_t)b2, 1};
     const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
     CUresult rc = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, const_cast<void *>(base), dims, strides, box, estr,
                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -463,7 +497,8 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     a.L1 = g->lat.L[1]; a.L2 = g->lat.L[2]; a.L3 = g->lat.L[3]; a.Ls = g->lat.Ls;
     a.parity_out = parity_out;
     a.l2pol = g->opt_l2pol;
-    a.prefetch_links = g->opt_prefetch_links;
+    a.zigzag = g->opt_zigzag;
+    a.barrier = g->opt_barrier;
     a.ablate = g->opt_ablate;
     int ssplit = g->opt_ssplit > 0 ? g->opt_ssplit : 1;
     const int slots = g->sm_count * v.ctas_per_sm;       // co-resident CTAs

@@ -95,7 +95,8 @@ struct dwf_geometry {
     int opt_l2pol;          // staged kernel: L2 eviction-priority digits (dhop_staged.cu PC_*)
     int opt_ssplit;         // staged kernel: CTAs sharing one tile (each takes Ls / ssplit slices)
     int opt_ablate;         // staged kernel: timing experiments (dhop_staged.cu StagedArgs::ablate)
-    int opt_prefetch_links; // staged kernel: L2-prefetch the next tile's links one tile ahead
+    int opt_zigzag;         // staged kernel: walk the slices of every other tile backwards
+    int opt_barrier;        // staged kernel: CTA barrier per step instead of last-warp refill
 };
 
 namespace dwf {

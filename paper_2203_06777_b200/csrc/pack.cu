@@ -1,23 +1,25 @@
 // pack.cu -- canonical <-> device layout conversion (hot path row a1 of SURVEY.md section 8).
 //
-// Spinor: canonical [site][s][k][reim]  <->  device complex[s][row][k][h]  (k = spin*3 + colour;
-//         row = x1 + L1*(x2 + L2*x3) is a lattice line along x0, h = x0>>1 the site of the parity
-//         on that line, so the cb site x>>1 is row*Lh + h), one such block per parity; a FULL
-//         field is the even block followed by the odd block (canonical site x -> parity p(x)).
+// Spinor: canonical [site][s][k][reim]  <->  device complex[s][row][k/2][h][k&1]  (k = spin*3 +
+//         colour; row = x1 + L1*(x2 + L2*x3) is a lattice line along x0, h = x0>>1 the site of the
+//         parity on that line, so the cb site x>>1 is row*Lh + h; two components of a site are
+//         adjacent = one 128-bit vector in fp32), one such block per parity; a FULL field is the
+//         even block followed by the odd block (canonical site x -> parity p(x)).
 // Gauge : canonical [x][mu][a][b][reim]  ->  for each output parity p and each output site of that
 //         parity (cb index x>>1) the 8 links that site multiplies with:
 //            leg 2*mu   : U_mu(x)                       (forward hop,  psi(x+mu))
 //            leg 2*mu+1 : U_mu(x-mu)^dagger             (backward hop, psi(x-mu))
 //         each times -1 when the hop wraps around an antiperiodic time direction, stored planar
-//         row by row as complex[row][leg*9 + a*3+b][h] (the 72 link components of the Lh output
-//         sites of a row are one contiguous 576*Lh-byte block).  Every canonical link appears
-//         exactly once in each parity set, so one half-Dhop reads the whole gauge field once.
+//         row by row as complex[row][f/2][h][f&1], f = leg*9 + a*3+b (the 72 link components of
+//         the Lh output sites of a row are one contiguous 576*Lh-byte block, in 128-bit pairs).
+//         Every canonical link appears exactly once in each parity set, so one half-Dhop reads
+//         the whole gauge field once.
 #include "dwf_internal.cuh"
 
 namespace dwf {
 
-// FULL = true: canonical sites are lexicographic x, the device field is [parity][s][row][k][h]
-// FULL = false: canonical sites are the cb sites of one parity, the device field is [s][row][k][h]
+// FULL = true: canonical sites are lexicographic x, the device field is [parity][s][row][k/2][h][k&1]
+// FULL = false: canonical sites are the cb sites of one parity, the device field is [s][row][k/2][h][k&1]
 template <typename T, bool IMPORT, bool FULL>
 __global__ void __launch_bounds__(256)
 spinor_reorder_kernel(const T *__restrict__ src, T *__restrict__ dst, const Lattice lat)
@@ -29,9 +31,11 @@ spinor_reorder_kernel(const T *__restrict__ src, T *__restrict__ dst, const Latt
     const long long n = (FULL ? 2 : 1) * Vh * lat.Ls * 12;
     for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n;
          e += (long long)gridDim.x * blockDim.x) {
+        // device element e = ((((par*Ls + s)*nrow + row)*6 + k/2)*Lh + h)*2 + (k&1)
         long long r = e;
+        const int klo = (int)(r & 1); r >>= 1;
         const int h = (int)(r % lat.Lh); r /= lat.Lh;
-        const int k = (int)(r % 12); r /= 12;
+        const int k = 2 * (int)(r % 6) + klo; r /= 6;
         const long long row = r % nrow; r /= nrow;
         const int s = (int)(r % lat.Ls);
         const int par = (int)(r / lat.Ls);
@@ -87,7 +91,7 @@ gauge_pack_kernel(const T *__restrict__ U, T *__restrict__ set_even, T *__restri
         const T *u = U + (src_site * 4 + mu) * 18;
         const long long row = cb / lat.Lh;
         const int h = (int)(cb % lat.Lh);
-        T *legbase = set + ((size_t)row * 72 + (size_t)leg * 9) * 2 * lat.Lh + 2 * h;
+        T *rowbase = set + (size_t)row * 72 * 2 * lat.Lh;
 #pragma unroll
         for (int a = 0; a < 3; a++)
 #pragma unroll
@@ -95,10 +99,10 @@ gauge_pack_kernel(const T *__restrict__ U, T *__restrict__ set_even, T *__restri
                 T re, im;
                 if (bwd) { re = u[(b * 3 + a) * 2]; im = -u[(b * 3 + a) * 2 + 1]; }   // dagger
                 else     { re = u[(a * 3 + b) * 2]; im =  u[(a * 3 + b) * 2 + 1]; }
-                const int cidx = a * 3 + b;          // complex plane
-                const size_t off = (size_t)cidx * 2 * lat.Lh;
-                legbase[off] = sign * re;
-                legbase[off + 1] = sign * im;
+                const int f = leg * 9 + a * 3 + b;   // link component 0..71, stored in pairs
+                const size_t off = (((size_t)(f >> 1) * lat.Lh + h) * 2 + (f & 1)) * 2;
+                rowbase[off] = sign * re;
+                rowbase[off + 1] = sign * im;
             }
     }
 }

@@ -77,15 +77,22 @@ __device__ __forceinline__ float2 ldg_hint(const float2 *p, uint64_t policy)
                  : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(policy));
     return v;
 }
+__device__ __forceinline__ float4 ldg128_hint(const float4 *p, uint64_t policy)
+{
+    float4 v;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.f32 {%0, %1, %2, %3}, [%4], %5;"
+                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p), "l"(policy));
+    return v;
+}
+__device__ __forceinline__ void stg128_hint(float4 *p, float4 v, uint64_t policy)
+{
+    asm volatile("st.global.L1::no_allocate.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p), "f"(v.x),
+                 "f"(v.y), "f"(v.z), "f"(v.w), "l"(policy) : "memory");
+}
 __device__ __forceinline__ void stg_hint(float2 *p, float2 v, uint64_t policy)
 {
     asm volatile("st.global.L1::no_allocate.L2::cache_hint.v2.f32 [%0], {%1, %2}, %3;" ::"l"(p), "f"(v.x), "f"(v.y),
                  "l"(policy) : "memory");
-}
-// asynchronous prefetch of `bytes` (multiple of 16) contiguous global bytes into L2
-__device__ __forceinline__ void bulk_prefetch_l2(const void *p, uint32_t bytes)
-{
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 // orders this thread's earlier generic-proxy accesses before later async-proxy (TMA) ones
 __device__ __forceinline__ void fence_proxy_async()
