@@ -199,8 +199,8 @@ int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, i
     g->opt_kernel = 0;
     g->opt_l2pol = 11212020;     // out, links evict_first; x3+ evict_last; x3- evict_first; top layer evict_last
     g->opt_ssplit = 1;
-    g->opt_zigzag = 0;
-    g->opt_barrier = 0;
+    g->opt_zigzag = 1;
+    g->opt_barrier = 1;
 
     g->gauge_bytes = (size_t)8 * 18 * (size_t)g->lat.Vh * (size_t)precision;
     g->reduce_blocks = g->sm_count * 8;

@@ -82,7 +82,8 @@ template <int LH, int B1, int B2, int B3> struct StagedCfg {
                          NROW_IN = R_X3P + B1 * B2;
     static constexpr int STAGE_BYTES = NROW_IN * ROWB;
     static constexpr int NSTAGE = 2;
-    static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + 80;  // + mbarriers (16 B) + 6 L2 policies + 2 counters
+    static constexpr int NORIG = 64;                              // tile origins cached in shared memory
+    static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + 80 + NORIG * 16;  // + mbarriers (16 B) + 6 L2 policies + 2 counters + origins
     // small tiles run two CTAs per SM (registers: 2 x 128 x 256 = 64 K): one CTA computes while
     // the other waits at its barrier or on its TMA
     static constexpr int CTAS_PER_SM = (NT <= 128 && 2 * (SMEM_BYTES + 1024) <= 232448) ? 2 : 1;
@@ -191,7 +192,8 @@ __device__ __forceinline__ void staged_leg(float2 (&acc)[12], const float4 *__re
 template <int LH, int B1, int B2, int B3>
 __global__ void __launch_bounds__(StagedCfg<LH, B1, B2, B3>::NT, StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM)
 dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_x1,
-                   const __grid_constant__ CUtensorMap map_x2, const StagedArgs args)
+                   const __grid_constant__ CUtensorMap map_x2, const __grid_constant__ CUtensorMap map_x3,
+                   const StagedArgs args)
 {
     using Cfg = StagedCfg<LH, B1, B2, B3>;
     extern __shared__ __align__(1024) unsigned char smem[];
@@ -222,13 +224,18 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     // per buffer: how many warps have finished reading it in the current step
     unsigned int *released = reinterpret_cast<unsigned int *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + 64);
     const uint64_t pol_g = l2_policy(args.l2pol / 1000000 % 10), pol_o = l2_policy(args.l2pol / 10000000 % 10);
+    // origins of this CTA's first NORIG tiles: read once, so that neither the producer nor the
+    // tile switch waits on a global load
+    int4 *orig = reinterpret_cast<int4 *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + 80);
+    for (int it = tid; it < my_tiles && it < Cfg::NORIG; it += Cfg::NT) orig[it] = args.tiles[group + it * ngroup];
+    auto tile_origin = [&](int it) -> int4 { return it < Cfg::NORIG ? orig[it] : args.tiles[group + it * ngroup]; };
 
     // producer: stage the input of step g (slice g % nsl of this CTA's (g / nsl)-th tile) into
     // buffer g & 1; run by one thread (whichever warp freed the buffer last)
     auto issue = [&](int g) {
         const int it = g / nsl, i = g % nsl, stage = g & 1;
         const int s = s_first + ((args.zigzag && (it & 1)) ? nsl - 1 - i : i);
-        const int4 o = args.tiles[group + it * ngroup];
+        const int4 o = tile_origin(it);
         const uint32_t bar = bar_base + 8 * stage;
         const uint32_t dst = smem_base + stage * Cfg::STAGE_BYTES;
         const int L1 = args.L1, L2 = args.L2, L3 = args.L3;
@@ -237,26 +244,28 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         const int x1m = o.x == 0 ? L1 - 1 : o.x - 1, x1p = o.x + B1 == L1 ? 0 : o.x + B1;
         const int x2m = o.y == 0 ? L2 - 1 : o.y - 1, x2p = o.y + B2 == L2 ? 0 : o.y + B2;
         const int x3m = o.z == 0 ? L3 - 1 : o.z - 1, x3p = o.z + B3 == L3 ? 0 : o.z + B3;
-        mbar_arrive_expect_tx(bar, Cfg::STAGE_BYTES);
-#pragma unroll
-        for (int j = 0; j < B3; j++) {
-            const bool top = j == B3 - 1;
-            const uint64_t pc = pol[top ? PC_CENTRE_TOP : PC_CENTRE], pf = pol[top ? PC_X12_TOP : PC_X12];
-            const int c4 = sb + o.z + j;
-            tma_load_5d_hint(dst + (j * B1 * B2) * Cfg::ROWB, &map_c, bar, 0, 0, o.x, o.y, c4, pc);
-            tma_load_5d_hint(dst + (Cfg::R_X1M + j * B2) * Cfg::ROWB, &map_x1, bar, 0, 0, x1m, o.y, c4, pf);
-            tma_load_5d_hint(dst + (Cfg::R_X1P + j * B2) * Cfg::ROWB, &map_x1, bar, 0, 0, x1p, o.y, c4, pf);
-            tma_load_5d_hint(dst + (Cfg::R_X2M + j * B1) * Cfg::ROWB, &map_x2, bar, 0, 0, o.x, x2m, c4, pf);
-            tma_load_5d_hint(dst + (Cfg::R_X2P + j * B1) * Cfg::ROWB, &map_x2, bar, 0, 0, o.x, x2p, c4, pf);
+        const bool no12 = args.ablate & 32, no3 = args.ablate & 16;     // timing experiments: skip faces
+        mbar_arrive_expect_tx(bar, (Cfg::NROW_IN - (no12 ? Cfg::R_X3M - Cfg::R_X1M : 0) - (no3 ? Cfg::NROW_IN - Cfg::R_X3M : 0)) * Cfg::ROWB);
+        // seven boxes: the centre and the x1 / x2 faces span the B3 layers of the tile in one copy each
+        const int c4 = sb + o.z;
+        tma_load_5d_hint(dst, &map_c, bar, 0, 0, o.x, o.y, c4, pol[PC_CENTRE]);
+        if (!no12) {
+            tma_load_5d_hint(dst + Cfg::R_X1M * Cfg::ROWB, &map_x1, bar, 0, 0, x1m, o.y, c4, pol[PC_X12]);
+            tma_load_5d_hint(dst + Cfg::R_X1P * Cfg::ROWB, &map_x1, bar, 0, 0, x1p, o.y, c4, pol[PC_X12]);
+            tma_load_5d_hint(dst + Cfg::R_X2M * Cfg::ROWB, &map_x2, bar, 0, 0, o.x, x2m, c4, pol[PC_X12]);
+            tma_load_5d_hint(dst + Cfg::R_X2P * Cfg::ROWB, &map_x2, bar, 0, 0, o.x, x2p, c4, pol[PC_X12]);
         }
-        tma_load_5d_hint(dst + Cfg::R_X3M * Cfg::ROWB, &map_c, bar, 0, 0, o.x, o.y, sb + x3m, pol[PC_X3M]);
-        tma_load_5d_hint(dst + Cfg::R_X3P * Cfg::ROWB, &map_c, bar, 0, 0, o.x, o.y, sb + x3p, pol[PC_X3P]);
+        if (!no3) {
+            tma_load_5d_hint(dst + Cfg::R_X3M * Cfg::ROWB, &map_x3, bar, 0, 0, o.x, o.y, sb + x3m, pol[PC_X3M]);
+            tma_load_5d_hint(dst + Cfg::R_X3P * Cfg::ROWB, &map_x3, bar, 0, 0, o.x, o.y, sb + x3p, pol[PC_X3P]);
+        }
     };
 
     if (tid == 0) {
         tma_prefetch_desc(&map_c);
         tma_prefetch_desc(&map_x1);
         tma_prefetch_desc(&map_x2);
+        tma_prefetch_desc(&map_x3);
         mbar_init(bar_base, 1);
         mbar_init(bar_base + 8, 1);
         mbar_fence_init();
@@ -287,7 +296,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
 
     // global row of this thread's site in the it-th tile, and the parity bit r of x0 = 2h + r
     auto tile_row = [&](int it, int &r) -> long long {
-        const int4 o = args.tiles[group + it * ngroup];
+        const int4 o = tile_origin(it);
         const int x1 = o.x + i1, x2 = o.y + i2, x3 = o.z + i3;
         r = (x1 + x2 + x3 + args.parity_out) & 1;
         return x1 + (long long)args.L1 * (x2 + (long long)args.L2 * x3);
@@ -420,6 +429,7 @@ static const std::vector<Variant> &variants()
         make_variant<8, 4, 4, 2>(),  make_variant<8, 2, 2, 2>(),  make_variant<8, 2, 2, 1>(),
         make_variant<24, 2, 2, 2>(), make_variant<24, 2, 2, 1>(),
         make_variant<4, 4, 4, 4>(),  make_variant<4, 2, 2, 2>(),  make_variant<4, 2, 2, 1>(),
+        make_variant<16, 2, 2, 4>(), make_variant<16, 2, 4, 2>(), make_variant<16, 8, 2, 1>(), make_variant<16, 1, 2, 8>(),
     };
     return v;
 }
@@ -441,35 +451,46 @@ void plan_staged(dwf_geometry *g)
     }
 }
 
-// Launch order of the row boxes.  raster 0: lexicographic (x1 fastest, x3 slowest).
-// raster n > 0: direction 2 is split into 2^n macro blocks that are swept one after the other,
-// which shortens the reuse distance of the x3 faces (they must survive in L2 for one sweep of a
-// macro-block slab only).
+// Launch order of the row boxes.  raster = 10 * order + n.
+// order picks the nesting of the three row directions (fastest, middle, slowest):
+//   0: (x1, x2, x3)   1: (x3, x2, x1)   2: (x2, x3, x1)   3: (x1, x3, x2)
+// n > 0: the middle direction is split into 2^n macro blocks that are swept one after the other,
+// which shortens the reuse distance of the faces in the slowest direction (they must survive in
+// L2 for one sweep step of a macro-block slab only).
 void build_staged_tile_table(const dwf_geometry *g, int raster, int4 *tab)
 {
+    static const int perm[4][3] = {{0, 1, 2}, {2, 1, 0}, {1, 2, 0}, {0, 2, 1}};
     const Lattice &lat = g->lat;
-    const int n1 = lat.L[1] / g->staged.b[0], n2 = lat.L[2] / g->staged.b[1], n3 = lat.L[3] / g->staged.b[2];
+    int order = raster / 10, nlog = raster % 10;
+    if (order < 0 || order > 3) order = 0;
+    const int *pm = perm[order];
+    int n[3];
+    for (int d = 0; d < 3; d++) n[d] = lat.L[d + 1] / g->staged.b[d];
+    const int nf = n[pm[0]], nm = n[pm[1]], nsl = n[pm[2]];
     int nsplit = 1;
-    for (int i = 0; i < raster && (n2 % (nsplit * 2) == 0); i++) nsplit *= 2;
-    const int n2in = n2 / nsplit;
+    for (int i = 0; i < nlog && (nm % (nsplit * 2) == 0); i++) nsplit *= 2;
+    const int nmin = nm / nsplit;
     int id = 0;
     for (int m = 0; m < nsplit; m++)
-        for (int t3 = 0; t3 < n3; t3++)
-            for (int t2 = 0; t2 < n2in; t2++)
-                for (int t1 = 0; t1 < n1; t1++)
-                    tab[id++] = make_int4(t1 * g->staged.b[0], (m * n2in + t2) * g->staged.b[1], t3 * g->staged.b[2], 0);
+        for (int ts = 0; ts < nsl; ts++)
+            for (int tm = 0; tm < nmin; tm++)
+                for (int tf = 0; tf < nf; tf++) {
+                    int t[3];
+                    t[pm[0]] = tf; t[pm[1]] = m * nmin + tm; t[pm[2]] = ts;
+                    tab[id++] = make_int4(t[0] * g->staged.b[0], t[1] * g->staged.b[1], t[2] * g->staged.b[2], 0);
+                }
 }
 
 // tensor map of a half field complex[s][x3][x2][x1][k/2][h][k&1] seen as 5-D fp32 tensor
 // (4*Lh, 6, L1, L2, L3*Ls): x3 and s share the slowest dimension (the s stride is L3 x3-strides)
-static int encode_map(CUtensorMap *m, const void *base, const Lattice &lat, int b1, int b2)
+static int encode_map(CUtensorMap *m, const void *base, const Lattice &lat, int b1, int b2, int b3)
 {
     PFN_tensorMapEncodeTiled enc = get_tensor_map_encoder();
     const cuuint64_t dims[5] = {(cuuint64_t)4 * lat.Lh, 6, (cuuint64_t)lat.L[1], (cuuint64_t)lat.L[2],
                                 (cuuint64_t)lat.L[3] * lat.Ls};
     const cuuint64_t krow = (cuuint64_t)lat.Lh * 16, row = 6 * krow;
     const cuuint64_t strides[4] = {krow, row, row * lat.L[1], row * lat.L[1] * lat.L[2]};
-    const cuuint32_t box[5] = {(cuuint32_t)4 * lat.Lh, 6, (cuuint32_t)b1, (cuuint32_t)b2, 1};
+    const cuuint32_t box[5] = {(cuuint32_t)4 * lat.Lh, 6, (cuuint32_t)b1, (cuuint32_t)b2, (cuuint32_t)b3};
     const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
     CUresult rc = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, const_cast<void *>(base), dims, strides, box, estr,
                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -484,11 +505,12 @@ static int encode_map(CUtensorMap *m, const void *base, const Lattice &lat, int 
 int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st)
 {
     const Variant &v = variants()[(size_t)g->staged.variant];
-    CUtensorMap mc, m1, m2;
+    CUtensorMap mc, m1, m2, m3;
     int rc;
-    if ((rc = encode_map(&mc, in, g->lat, v.b1, v.b2))) return rc;
-    if ((rc = encode_map(&m1, in, g->lat, 1, v.b2))) return rc;
-    if ((rc = encode_map(&m2, in, g->lat, v.b1, 1))) return rc;
+    if ((rc = encode_map(&mc, in, g->lat, v.b1, v.b2, v.b3))) return rc;
+    if ((rc = encode_map(&m1, in, g->lat, 1, v.b2, v.b3))) return rc;
+    if ((rc = encode_map(&m2, in, g->lat, v.b1, 1, v.b3))) return rc;
+    if ((rc = encode_map(&m3, in, g->lat, v.b1, v.b2, 1))) return rc;
     StagedArgs a;
     a.out = static_cast<float2 *>(out);
     a.gauge = static_cast<const float2 *>(g->gauge[parity_out]);
@@ -511,7 +533,7 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     }
     const int ngroup_max = slots / ssplit;
     const int ngroup = g->staged.ntiles < ngroup_max ? g->staged.ntiles : ngroup_max;
-    void *params[] = {&mc, &m1, &m2, &a};
+    void *params[] = {&mc, &m1, &m2, &m3, &a};
     DWF_CUDA_CHECK(cudaLaunchKernel(v.fn, dim3((unsigned)(ngroup * ssplit)), dim3((unsigned)v.threads), params,
                                     (size_t)v.smem, st));
     count_launch();
