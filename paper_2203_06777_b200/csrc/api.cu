@@ -200,7 +200,7 @@ int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, i
     g->opt_l2pol = 11212020;     // out, links evict_first; x3+ evict_last; x3- evict_first; top layer evict_last
     g->opt_ssplit = 1;
     g->opt_zigzag = 1;
-    g->opt_barrier = 1;
+    g->opt_prefetch = 0;
 
     g->gauge_bytes = (size_t)8 * 18 * (size_t)g->lat.Vh * (size_t)precision;
     g->reduce_blocks = g->sm_count * 8;
@@ -260,8 +260,8 @@ int dwf_set_option(dwf_geometry *g, const char *key, long long value)
     } else if (!strcmp(key, "zigzag")) {
         g->opt_zigzag = v != 0;
         return DWF_OK;
-    } else if (!strcmp(key, "barrier")) {
-        g->opt_barrier = v != 0;
+    } else if (!strcmp(key, "prefetch")) {
+        g->opt_prefetch = v;
         return DWF_OK;
     } else if (!strcmp(key, "l2persist")) {
         // MB of L2 set aside for evict_last ("persisting") lines; device-wide CUDA limit

@@ -68,14 +68,16 @@ struct StagedArgs {
     int parity_out;
     int l2pol;               // decimal digits, see PC_*
     int zigzag;              // walk the slices of every other tile backwards
-    int barrier;             // 1: CTA barrier + thread 0 refills; 0: the last warp to release a buffer refills it
+    int prefetch;            // producer prefetches the input of step g + prefetch into L2 (0: off); bit 4..: box mask
     int ablate;              // timing experiments only (wrong results): 1 no link refill, 2 no stores, 4 no legs, 8 no TMA
 };
 
 template <int LH, int B1, int B2, int B3> struct StagedCfg {
     static constexpr int NROW_C = B1 * B2 * B3;
-    static constexpr int T = LH * NROW_C;                        // output sites per tile
-    static constexpr int NT = (T + 31) / 32 * 32;                // threads
+    static constexpr int T = LH * NROW_C;                        // output sites per tile = compute threads
+    static constexpr int NWARP_C = (T + 31) / 32;                // consumer warps with work
+    static constexpr int NTC = (T + 127) / 128 * 128;            // consumer threads (whole warpgroups)
+    static constexpr int NT = 128 + NTC;                         // + one producer warpgroup (one thread issues)
     static constexpr int ROWB = 12 * LH * 8;                     // bytes of one staged row
     static constexpr int R_X1M = NROW_C, R_X1P = R_X1M + B2 * B3, R_X2M = R_X1P + B2 * B3,
                          R_X2P = R_X2M + B1 * B3, R_X3M = R_X2P + B1 * B3, R_X3P = R_X3M + B1 * B2,
@@ -83,10 +85,14 @@ template <int LH, int B1, int B2, int B3> struct StagedCfg {
     static constexpr int STAGE_BYTES = NROW_IN * ROWB;
     static constexpr int NSTAGE = 2;
     static constexpr int NORIG = 64;                              // tile origins cached in shared memory
-    static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + 80 + NORIG * 16;  // + mbarriers (16 B) + 6 L2 policies + 2 counters + origins
-    // small tiles run two CTAs per SM (registers: 2 x 128 x 256 = 64 K): one CTA computes while
-    // the other waits at its barrier or on its TMA
-    static constexpr int CTAS_PER_SM = (NT <= 128 && 2 * (SMEM_BYTES + 1024) <= 232448) ? 2 : 1;
+    // tail: full[2], empty[2] mbarriers (32 B), 6 L2 policies (48 B), origins
+    static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + 80 + NORIG * 16;
+    // small tiles run two CTAs per SM
+    static constexpr int CTAS_PER_SM = (NTC <= 128 && 2 * (SMEM_BYTES + 1024) <= 232448) ? 2 : 1;
+    // register split (setmaxnreg): the producer warpgroup keeps PROD_REGS, the consumers take the rest
+    static constexpr int PROD_REGS = 24;
+    static constexpr int CONS_REGS_RAW = ((65536 / CTAS_PER_SM - 128 * PROD_REGS) / NTC) / 8 * 8;
+    static constexpr int CONS_REGS = CONS_REGS_RAW > 240 ? 240 : CONS_REGS_RAW;
     static_assert(ROWB % 128 == 0, "staged rows must keep TMA destinations 128-byte aligned");
 };
 
@@ -198,14 +204,10 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     using Cfg = StagedCfg<LH, B1, B2, B3>;
     extern __shared__ __align__(1024) unsigned char smem[];
     const uint32_t smem_base = smem_u32(smem);
-    const uint32_t bar_base = smem_base + Cfg::NSTAGE * Cfg::STAGE_BYTES;
+    const uint32_t full_base = smem_base + Cfg::NSTAGE * Cfg::STAGE_BYTES;      // full[2]: TMA data has landed
+    const uint32_t empty_base = full_base + 16;                                 // empty[2]: every consumer warp is done
 
     const int tid = threadIdx.x;
-    const bool active = tid < Cfg::T;
-    const int h = tid % LH;
-    const int row = active ? tid / LH : 0;
-    const int i1 = row % B1, i2 = (row / B1) % B2, i3 = row / (B1 * B2);
-
     // tile group and slice range of this CTA
     const int ngroup = (int)gridDim.x / args.ssplit;
     const int group = (int)blockIdx.x / args.ssplit;
@@ -214,69 +216,97 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     const int my_tiles = (args.ntiles - group + ngroup - 1) / ngroup;
     const int nsteps = my_tiles * nsl;
     if (nsteps <= 0) return;
-    // L2 policies: the producer thread reads the TMA ones from shared memory (keeps them out of
-    // the compute threads' registers); every thread holds the two it uses itself
-    uint64_t *pol = reinterpret_cast<uint64_t *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + 16);
-    if (tid == 0) {
-        int d = args.l2pol;
-        for (int c = 0; c < PC_GAUGE; c++) { pol[c] = l2_policy(d % 10); d /= 10; }
-    }
-    // per buffer: how many warps have finished reading it in the current step
-    unsigned int *released = reinterpret_cast<unsigned int *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + 64);
-    const uint64_t pol_g = l2_policy(args.l2pol / 1000000 % 10), pol_o = l2_policy(args.l2pol / 10000000 % 10);
+    // L2 policies of the TMA copies, read by the producer thread from shared memory
+    uint64_t *pol = reinterpret_cast<uint64_t *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + 32);
     // origins of this CTA's first NORIG tiles: read once, so that neither the producer nor the
     // tile switch waits on a global load
     int4 *orig = reinterpret_cast<int4 *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + 80);
     for (int it = tid; it < my_tiles && it < Cfg::NORIG; it += Cfg::NT) orig[it] = args.tiles[group + it * ngroup];
     auto tile_origin = [&](int it) -> int4 { return it < Cfg::NORIG ? orig[it] : args.tiles[group + it * ngroup]; };
-
-    // producer: stage the input of step g (slice g % nsl of this CTA's (g / nsl)-th tile) into
-    // buffer g & 1; run by one thread (whichever warp freed the buffer last)
-    auto issue = [&](int g) {
-        const int it = g / nsl, i = g % nsl, stage = g & 1;
-        const int s = s_first + ((args.zigzag && (it & 1)) ? nsl - 1 - i : i);
-        const int4 o = tile_origin(it);
-        const uint32_t bar = bar_base + 8 * stage;
-        const uint32_t dst = smem_base + stage * Cfg::STAGE_BYTES;
-        const int L1 = args.L1, L2 = args.L2, L3 = args.L3;
-        if (args.ablate & 8) { mbar_arrive(bar); return; }
-        const int sb = s * L3;                 // x3 and s share tensor dimension 4: coordinate s*L3 + x3
-        const int x1m = o.x == 0 ? L1 - 1 : o.x - 1, x1p = o.x + B1 == L1 ? 0 : o.x + B1;
-        const int x2m = o.y == 0 ? L2 - 1 : o.y - 1, x2p = o.y + B2 == L2 ? 0 : o.y + B2;
-        const int x3m = o.z == 0 ? L3 - 1 : o.z - 1, x3p = o.z + B3 == L3 ? 0 : o.z + B3;
-        const bool no12 = args.ablate & 32, no3 = args.ablate & 16;     // timing experiments: skip faces
-        mbar_arrive_expect_tx(bar, (Cfg::NROW_IN - (no12 ? Cfg::R_X3M - Cfg::R_X1M : 0) - (no3 ? Cfg::NROW_IN - Cfg::R_X3M : 0)) * Cfg::ROWB);
-        // seven boxes: the centre and the x1 / x2 faces span the B3 layers of the tile in one copy each
-        const int c4 = sb + o.z;
-        tma_load_5d_hint(dst, &map_c, bar, 0, 0, o.x, o.y, c4, pol[PC_CENTRE]);
-        if (!no12) {
-            tma_load_5d_hint(dst + Cfg::R_X1M * Cfg::ROWB, &map_x1, bar, 0, 0, x1m, o.y, c4, pol[PC_X12]);
-            tma_load_5d_hint(dst + Cfg::R_X1P * Cfg::ROWB, &map_x1, bar, 0, 0, x1p, o.y, c4, pol[PC_X12]);
-            tma_load_5d_hint(dst + Cfg::R_X2M * Cfg::ROWB, &map_x2, bar, 0, 0, o.x, x2m, c4, pol[PC_X12]);
-            tma_load_5d_hint(dst + Cfg::R_X2P * Cfg::ROWB, &map_x2, bar, 0, 0, o.x, x2p, c4, pol[PC_X12]);
-        }
-        if (!no3) {
-            tma_load_5d_hint(dst + Cfg::R_X3M * Cfg::ROWB, &map_x3, bar, 0, 0, o.x, o.y, sb + x3m, pol[PC_X3M]);
-            tma_load_5d_hint(dst + Cfg::R_X3P * Cfg::ROWB, &map_x3, bar, 0, 0, o.x, o.y, sb + x3p, pol[PC_X3P]);
-        }
-    };
-
     if (tid == 0) {
+        int d = args.l2pol;
+        for (int c = 0; c < PC_GAUGE; c++) { pol[c] = l2_policy(d % 10); d /= 10; }
         tma_prefetch_desc(&map_c);
         tma_prefetch_desc(&map_x1);
         tma_prefetch_desc(&map_x2);
         tma_prefetch_desc(&map_x3);
-        mbar_init(bar_base, 1);
-        mbar_init(bar_base + 8, 1);
+        mbar_init(full_base, 1);
+        mbar_init(full_base + 8, 1);
+        mbar_init(empty_base, Cfg::NWARP_C);
+        mbar_init(empty_base + 8, Cfg::NWARP_C);
         mbar_fence_init();
-        released[0] = 0;
-        released[1] = 0;
     }
     __syncthreads();
-    if (tid == 0) {
-        issue(0);
-        if (nsteps > 1) issue(1);
+
+    // =========================== producer warpgroup ===========================================
+    // One thread stages the input of step g (slice g % nsl of this CTA's (g / nsl)-th tile) into
+    // buffer g & 1 as soon as every consumer warp has released that buffer.  No CTA barrier
+    // anywhere: consumer warps drift apart by up to one stage.
+    if (tid < 128) {
+        reg_dealloc<Cfg::PROD_REGS>();
+        if (tid != 0) return;
+        const int L1 = args.L1, L2 = args.L2, L3 = args.L3;
+        // coordinates of the boxes of step g
+        struct Boxes { int o1, o2, c4, x1m, x1p, x2m, x2p, c3m, c3p; };
+        auto boxes = [&](int g) {
+            const int it = g / nsl, i = g % nsl;
+            const int s = s_first + ((args.zigzag && (it & 1)) ? nsl - 1 - i : i);
+            const int4 o = tile_origin(it);
+            const int sb = s * L3;                 // x3 and s share tensor dimension 4: coordinate s*L3 + x3
+            Boxes b;
+            b.o1 = o.x; b.o2 = o.y; b.c4 = sb + o.z;
+            b.x1m = o.x == 0 ? L1 - 1 : o.x - 1; b.x1p = o.x + B1 == L1 ? 0 : o.x + B1;
+            b.x2m = o.y == 0 ? L2 - 1 : o.y - 1; b.x2p = o.y + B2 == L2 ? 0 : o.y + B2;
+            b.c3m = sb + (o.z == 0 ? L3 - 1 : o.z - 1); b.c3p = sb + (o.z + B3 == L3 ? 0 : o.z + B3);
+            return b;
+        };
+        const int pfd = args.prefetch & 15, pfm = args.prefetch >> 4;
+        for (int g = 0; g < nsteps; g++) {
+            const int stage = g & 1;
+            const uint32_t bar = full_base + 8 * stage;
+            if (pfd && g + pfd < nsteps && !(args.ablate & 8)) {       // DRAM -> L2 runs ahead of the shared-memory ring
+                const Boxes p = boxes(g + pfd);
+                if (pfm & 1) tma_prefetch_5d(&map_c, 0, 0, p.o1, p.o2, p.c4);
+                if (pfm & 2) tma_prefetch_5d(&map_x3, 0, 0, p.o1, p.o2, p.c3p);
+                if (pfm & 4) tma_prefetch_5d(&map_x3, 0, 0, p.o1, p.o2, p.c3m);
+                if (pfm & 8) {
+                    tma_prefetch_5d(&map_x1, 0, 0, p.x1m, p.o2, p.c4);
+                    tma_prefetch_5d(&map_x1, 0, 0, p.x1p, p.o2, p.c4);
+                    tma_prefetch_5d(&map_x2, 0, 0, p.o1, p.x2m, p.c4);
+                    tma_prefetch_5d(&map_x2, 0, 0, p.o1, p.x2p, p.c4);
+                }
+            }
+            if (g >= 2) mbar_wait(empty_base + 8 * stage, ((g >> 1) - 1) & 1);
+            if (args.ablate & 8) { mbar_arrive(bar); continue; }
+            const Boxes b = boxes(g);
+            const uint32_t dst = smem_base + stage * Cfg::STAGE_BYTES;
+            const bool no12 = args.ablate & 32, no3 = args.ablate & 16;     // timing experiments: skip faces
+            mbar_arrive_expect_tx(bar, (Cfg::NROW_IN - (no12 ? Cfg::R_X3M - Cfg::R_X1M : 0) - (no3 ? Cfg::NROW_IN - Cfg::R_X3M : 0)) * Cfg::ROWB);
+            // seven boxes: the centre and the x1 / x2 faces span the B3 layers of the tile in one copy each
+            tma_load_5d_hint(dst, &map_c, bar, 0, 0, b.o1, b.o2, b.c4, pol[PC_CENTRE]);
+            if (!no12) {
+                tma_load_5d_hint(dst + Cfg::R_X1M * Cfg::ROWB, &map_x1, bar, 0, 0, b.x1m, b.o2, b.c4, pol[PC_X12]);
+                tma_load_5d_hint(dst + Cfg::R_X1P * Cfg::ROWB, &map_x1, bar, 0, 0, b.x1p, b.o2, b.c4, pol[PC_X12]);
+                tma_load_5d_hint(dst + Cfg::R_X2M * Cfg::ROWB, &map_x2, bar, 0, 0, b.o1, b.x2m, b.c4, pol[PC_X12]);
+                tma_load_5d_hint(dst + Cfg::R_X2P * Cfg::ROWB, &map_x2, bar, 0, 0, b.o1, b.x2p, b.c4, pol[PC_X12]);
+            }
+            if (!no3) {
+                tma_load_5d_hint(dst + Cfg::R_X3M * Cfg::ROWB, &map_x3, bar, 0, 0, b.o1, b.o2, b.c3m, pol[PC_X3M]);
+                tma_load_5d_hint(dst + Cfg::R_X3P * Cfg::ROWB, &map_x3, bar, 0, 0, b.o1, b.o2, b.c3p, pol[PC_X3P]);
+            }
+        }
+        return;
     }
+
+    // =========================== consumer warpgroups ==========================================
+    reg_alloc<Cfg::CONS_REGS>();
+    const int ctid = tid - 128;
+    if (ctid >= Cfg::NWARP_C * 32) return;                          // warps without sites
+    const bool active = ctid < Cfg::T;
+    const int h = ctid % LH;
+    const int row = active ? ctid / LH : 0;
+    const int i1 = row % B1, i2 = (row / B1) % B2, i3 = row / (B1 * B2);
+    const uint64_t pol_g = l2_policy(args.l2pol / 1000000 % 10), pol_o = l2_policy(args.l2pol / 10000000 % 10);
 
     // row offsets (in staged rows) of the 8 neighbours; tile-invariant
     const int rc = row;
@@ -371,32 +401,15 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         for (int s = 0; s < nsl; s++, g++) {
             const bool fetch = has_next && s == nsl - 1 && !(args.ablate & 1);     // refill the links during the last slice
             const int stage = g & 1;
-            mbar_wait(bar_base + 8 * stage, (g >> 1) & 1);
+            mbar_wait(full_base + 8 * stage, (g >> 1) & 1);
             if (active && !(args.ablate & 4)) {
                 const int sl = (args.zigzag && (it & 1)) ? nsl - 1 - s : s;
                 if (fetch) step(std::true_type{}, stage, optr + (long long)sl * slice_vecs, gnext);
                 else       step(std::false_type{}, stage, optr + (long long)sl * slice_vecs, gnext);
             }
-            // This warp is done with the buffer (its results depend on every value it read).  No
-            // CTA barrier: the warp that frees a buffer last refills it for step g + 2, everybody
-            // else moves on to the next buffer at once.
-            if (args.barrier) {
-                __syncthreads();
-                if (tid == 0 && g + 2 < nsteps) issue(g + 2);
-            } else {
+            // this warp is done with the buffer (its results depend on every value it read)
             __syncwarp();
-            if ((tid & 31) == 0) {
-                __threadfence_block();
-                if (atomicAdd(&released[stage], 1u) == Cfg::NT / 32 - 1) {
-                    released[stage] = 0;
-                    __threadfence_block();
-                    if (g + 2 < nsteps) {
-                        fence_proxy_async();
-                        issue(g + 2);
-                    }
-                }
-            }
-            }
+            if ((ctid & 31) == 0) mbar_arrive(empty_base + 8 * stage);
         }
         // tile switch
         grow = grow_next;
@@ -520,7 +533,7 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     a.parity_out = parity_out;
     a.l2pol = g->opt_l2pol;
     a.zigzag = g->opt_zigzag;
-    a.barrier = g->opt_barrier;
+    a.prefetch = g->opt_prefetch;
     a.ablate = g->opt_ablate;
     int ssplit = g->opt_ssplit > 0 ? g->opt_ssplit : 1;
     const int slots = g->sm_count * v.ctas_per_sm;       // co-resident CTAs

@@ -60,6 +60,12 @@ __device__ __forceinline__ void tma_load_5d_hint(uint32_t dst, const CUtensorMap
         "[%0], [%1, {%3, %4, %5, %6, %7}], [%2], %8;" ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2),
         "r"(c3), "r"(c4), "l"(policy) : "memory");
 }
+// prefetch of the same box into L2 only (no shared-memory destination, no completion signal)
+__device__ __forceinline__ void tma_prefetch_5d(const CUtensorMap *map, int c0, int c1, int c2, int c3, int c4)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.5d.L2.global.tile [%0, {%1, %2, %3, %4, %5}];" ::"l"(map), "r"(c0),
+                 "r"(c1), "r"(c2), "r"(c3), "r"(c4) : "memory");
+}
 // L2 eviction-priority policies: 0 evict_normal, 1 evict_first, 2 evict_last
 __device__ __forceinline__ uint64_t l2_policy(int kind)
 {
@@ -98,6 +104,15 @@ __device__ __forceinline__ void stg_hint(float2 *p, float2 v, uint64_t policy)
 __device__ __forceinline__ void fence_proxy_async()
 {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+// register reallocation between warpgroups (all four warps of a warpgroup must execute it)
+template <int N> __device__ __forceinline__ void reg_alloc()
+{
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N));
+}
+template <int N> __device__ __forceinline__ void reg_dealloc()
+{
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N));
 }
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap *map)
 {
