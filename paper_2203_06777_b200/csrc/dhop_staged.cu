@@ -85,8 +85,12 @@ template <int LH, int B1, int B2, int B3> struct StagedCfg {
     static constexpr int STAGE_BYTES = NROW_IN * ROWB;
     static constexpr int NSTAGE = 2;
     static constexpr int NORIG = 64;                              // tile origins cached in shared memory
-    // tail: full[2], empty[2] mbarriers (32 B), 6 L2 policies (48 B), origins
-    static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + 80 + NORIG * 16;
+    // A stage is four regions with their own full / empty mbarriers, in the order the consumers
+    // finish with them: x3 faces, x2 faces, x1 faces, centre
+    static constexpr int NREG = 4;
+    // tail: full[2][4], empty[2][4] mbarriers (128 B), 6 L2 policies (48 B), origins
+    static constexpr int TAIL_POL = 128, TAIL_ORIG = 176;
+    static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + TAIL_ORIG + NORIG * 16;
     // small tiles run two CTAs per SM
     static constexpr int CTAS_PER_SM = (NTC <= 128 && 2 * (SMEM_BYTES + 1024) <= 232448) ? 2 : 1;
     // register split (setmaxnreg): the producer warpgroup keeps PROD_REGS, the consumers take the rest
@@ -204,8 +208,8 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     using Cfg = StagedCfg<LH, B1, B2, B3>;
     extern __shared__ __align__(1024) unsigned char smem[];
     const uint32_t smem_base = smem_u32(smem);
-    const uint32_t full_base = smem_base + Cfg::NSTAGE * Cfg::STAGE_BYTES;      // full[2]: TMA data has landed
-    const uint32_t empty_base = full_base + 16;                                 // empty[2]: every consumer warp is done
+    const uint32_t full_base = smem_base + Cfg::NSTAGE * Cfg::STAGE_BYTES;      // full[stage][region]: TMA data has landed
+    const uint32_t empty_base = full_base + 64;                                 // empty[stage][region]: every consumer warp is done
 
     const int tid = threadIdx.x;
     // tile group and slice range of this CTA
@@ -217,10 +221,10 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     const int nsteps = my_tiles * nsl;
     if (nsteps <= 0) return;
     // L2 policies of the TMA copies, read by the producer thread from shared memory
-    uint64_t *pol = reinterpret_cast<uint64_t *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + 32);
+    uint64_t *pol = reinterpret_cast<uint64_t *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + Cfg::TAIL_POL);
     // origins of this CTA's first NORIG tiles: read once, so that neither the producer nor the
     // tile switch waits on a global load
-    int4 *orig = reinterpret_cast<int4 *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + 80);
+    int4 *orig = reinterpret_cast<int4 *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + Cfg::TAIL_ORIG);
     for (int it = tid; it < my_tiles && it < Cfg::NORIG; it += Cfg::NT) orig[it] = args.tiles[group + it * ngroup];
     auto tile_origin = [&](int it) -> int4 { return it < Cfg::NORIG ? orig[it] : args.tiles[group + it * ngroup]; };
     if (tid == 0) {
@@ -230,10 +234,10 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         tma_prefetch_desc(&map_x1);
         tma_prefetch_desc(&map_x2);
         tma_prefetch_desc(&map_x3);
-        mbar_init(full_base, 1);
-        mbar_init(full_base + 8, 1);
-        mbar_init(empty_base, Cfg::NWARP_C);
-        mbar_init(empty_base + 8, Cfg::NWARP_C);
+        for (int i = 0; i < 2 * Cfg::NREG; i++) {
+            mbar_init(full_base + 8 * i, 1);
+            mbar_init(empty_base + 8 * i, Cfg::NWARP_C);
+        }
         mbar_fence_init();
     }
     __syncthreads();
@@ -276,23 +280,38 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
                     tma_prefetch_5d(&map_x2, 0, 0, p.o1, p.x2p, p.c4);
                 }
             }
-            if (g >= 2) mbar_wait(empty_base + 8 * stage, ((g >> 1) - 1) & 1);
-            if (args.ablate & 8) { mbar_arrive(bar); continue; }
             const Boxes b = boxes(g);
             const uint32_t dst = smem_base + stage * Cfg::STAGE_BYTES;
-            const bool no12 = args.ablate & 32, no3 = args.ablate & 16;     // timing experiments: skip faces
-            mbar_arrive_expect_tx(bar, (Cfg::NROW_IN - (no12 ? Cfg::R_X3M - Cfg::R_X1M : 0) - (no3 ? Cfg::NROW_IN - Cfg::R_X3M : 0)) * Cfg::ROWB);
-            // seven boxes: the centre and the x1 / x2 faces span the B3 layers of the tile in one copy each
-            tma_load_5d_hint(dst, &map_c, bar, 0, 0, b.o1, b.o2, b.c4, pol[PC_CENTRE]);
-            if (!no12) {
-                tma_load_5d_hint(dst + Cfg::R_X1M * Cfg::ROWB, &map_x1, bar, 0, 0, b.x1m, b.o2, b.c4, pol[PC_X12]);
-                tma_load_5d_hint(dst + Cfg::R_X1P * Cfg::ROWB, &map_x1, bar, 0, 0, b.x1p, b.o2, b.c4, pol[PC_X12]);
-                tma_load_5d_hint(dst + Cfg::R_X2M * Cfg::ROWB, &map_x2, bar, 0, 0, b.o1, b.x2m, b.c4, pol[PC_X12]);
-                tma_load_5d_hint(dst + Cfg::R_X2P * Cfg::ROWB, &map_x2, bar, 0, 0, b.o1, b.x2p, b.c4, pol[PC_X12]);
+            const uint32_t fb = full_base + 32 * stage, eb = empty_base + 32 * stage;
+            const uint32_t epar = ((g >> 1) - 1) & 1;
+            const bool notma = args.ablate & 8, no12 = args.ablate & 32, no3 = args.ablate & 16;   // timing experiments
+            // regions in the order the consumers release them (x3 faces, x2 faces, x1 faces, centre)
+            if (g >= 2) mbar_wait(eb, epar);
+            if (notma || no3) mbar_arrive(fb);
+            else {
+                mbar_arrive_expect_tx(fb, 2 * B1 * B2 * Cfg::ROWB);
+                tma_load_5d_hint(dst + Cfg::R_X3M * Cfg::ROWB, &map_x3, fb, 0, 0, b.o1, b.o2, b.c3m, pol[PC_X3M]);
+                tma_load_5d_hint(dst + Cfg::R_X3P * Cfg::ROWB, &map_x3, fb, 0, 0, b.o1, b.o2, b.c3p, pol[PC_X3P]);
             }
-            if (!no3) {
-                tma_load_5d_hint(dst + Cfg::R_X3M * Cfg::ROWB, &map_x3, bar, 0, 0, b.o1, b.o2, b.c3m, pol[PC_X3M]);
-                tma_load_5d_hint(dst + Cfg::R_X3P * Cfg::ROWB, &map_x3, bar, 0, 0, b.o1, b.o2, b.c3p, pol[PC_X3P]);
+            if (g >= 2) mbar_wait(eb + 8, epar);
+            if (notma || no12) mbar_arrive(fb + 8);
+            else {
+                mbar_arrive_expect_tx(fb + 8, 2 * B1 * B3 * Cfg::ROWB);
+                tma_load_5d_hint(dst + Cfg::R_X2M * Cfg::ROWB, &map_x2, fb + 8, 0, 0, b.o1, b.x2m, b.c4, pol[PC_X12]);
+                tma_load_5d_hint(dst + Cfg::R_X2P * Cfg::ROWB, &map_x2, fb + 8, 0, 0, b.o1, b.x2p, b.c4, pol[PC_X12]);
+            }
+            if (g >= 2) mbar_wait(eb + 16, epar);
+            if (notma || no12) mbar_arrive(fb + 16);
+            else {
+                mbar_arrive_expect_tx(fb + 16, 2 * B2 * B3 * Cfg::ROWB);
+                tma_load_5d_hint(dst + Cfg::R_X1M * Cfg::ROWB, &map_x1, fb + 16, 0, 0, b.x1m, b.o2, b.c4, pol[PC_X12]);
+                tma_load_5d_hint(dst + Cfg::R_X1P * Cfg::ROWB, &map_x1, fb + 16, 0, 0, b.x1p, b.o2, b.c4, pol[PC_X12]);
+            }
+            if (g >= 2) mbar_wait(eb + 24, epar);
+            if (notma) mbar_arrive(fb + 24);
+            else {
+                mbar_arrive_expect_tx(fb + 24, Cfg::NROW_C * Cfg::ROWB);
+                tma_load_5d_hint(dst, &map_c, fb + 24, 0, 0, b.o1, b.o2, b.c4, pol[PC_CENTRE]);
             }
         }
         return;
@@ -357,9 +376,13 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     // one slice of the tile: 8 legs out of the staged buffer, then the store.  FETCH = this is the
     // tile's last slice: the registers of each link are refilled for the next tile right after
     // the leg that used them last (two code copies, so that the common one carries no loads)
-    auto step = [&](auto fetch_tag, int stage, float4 *o, const float4 *gnext) {
+    // Leg order x3, x2, x1, x0: the face regions are handed back to the producer as soon as the
+    // two legs reading them are done, so that their refill has almost two steps to land.
+    auto step = [&](auto fetch_tag, int stage, uint32_t par, float4 *o, const float4 *gnext) {
         constexpr bool FETCH = decltype(fetch_tag)::value;
         const unsigned char *sb = smem + stage * Cfg::STAGE_BYTES;
+        const uint32_t fb = full_base + 32 * stage, eb = empty_base + 32 * stage;
+        const bool legs = !(args.ablate & 4);
         float2 acc[12];
 #define DWF_LEG(L, MU, FWD, FIRST)                                                                  \
         staged_leg<LH, MU, FWD, FIRST, DWF_ABL>(acc, reinterpret_cast<const float4 *>(sb + off[L]), U + 9 * (L)); \
@@ -370,15 +393,36 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
                 U[2 * j + 1] = make_float2(q.z, q.w);                                               \
             }                                                                                       \
         }
-        DWF_LEG(0, 0, true,  true)
-        DWF_LEG(1, 0, false, false)
-        DWF_LEG(2, 1, true,  false)
-        DWF_LEG(3, 1, false, false)
-        DWF_LEG(4, 2, true,  false)
-        DWF_LEG(5, 2, false, false)
-        DWF_LEG(6, 3, true,  false)
-        DWF_LEG(7, 3, false, false)
+#define DWF_RELEASE(R)                                                                              \
+        __syncwarp();                                                                               \
+        if ((ctid & 31) == 0) mbar_arrive(eb + 8 * (R));
+        mbar_wait(fb + 24, par);
+        mbar_wait(fb, par);
+        if (legs) {
+            DWF_LEG(6, 3, true,  true)
+            DWF_LEG(7, 3, false, false)
+        }
+        DWF_RELEASE(0)
+        mbar_wait(fb + 8, par);
+        if (legs) {
+            DWF_LEG(4, 2, true,  false)
+            DWF_LEG(5, 2, false, false)
+        }
+        DWF_RELEASE(1)
+        mbar_wait(fb + 16, par);
+        if (legs) {
+            DWF_LEG(2, 1, true,  false)
+            DWF_LEG(3, 1, false, false)
+        }
+        DWF_RELEASE(2)
+        if (legs) {
+            DWF_LEG(0, 0, true,  false)
+            DWF_LEG(1, 0, false, false)
+        }
+        DWF_RELEASE(3)
 #undef DWF_LEG
+#undef DWF_RELEASE
+        if (!legs || !active) return;
         if (!(args.ablate & 2)) {
 #pragma unroll
             for (int j = 0; j < 6; j++)
@@ -401,15 +445,9 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         for (int s = 0; s < nsl; s++, g++) {
             const bool fetch = has_next && s == nsl - 1 && !(args.ablate & 1);     // refill the links during the last slice
             const int stage = g & 1;
-            mbar_wait(full_base + 8 * stage, (g >> 1) & 1);
-            if (active && !(args.ablate & 4)) {
-                const int sl = (args.zigzag && (it & 1)) ? nsl - 1 - s : s;
-                if (fetch) step(std::true_type{}, stage, optr + (long long)sl * slice_vecs, gnext);
-                else       step(std::false_type{}, stage, optr + (long long)sl * slice_vecs, gnext);
-            }
-            // this warp is done with the buffer (its results depend on every value it read)
-            __syncwarp();
-            if ((ctid & 31) == 0) mbar_arrive(empty_base + 8 * stage);
+            const int sl = (args.zigzag && (it & 1)) ? nsl - 1 - s : s;
+            if (fetch) step(std::true_type{}, stage, (g >> 1) & 1, optr + (long long)sl * slice_vecs, gnext);
+            else       step(std::false_type{}, stage, (g >> 1) & 1, optr + (long long)sl * slice_vecs, gnext);
         }
         // tile switch
         grow = grow_next;

@@ -44,16 +44,25 @@ norm2_partial_kernel(const T *__restrict__ x, size_t nreal, double *__restrict__
     constexpr int W = 16 / sizeof(T);                       // reals per 128-bit vector
     using V = typename std::conditional<sizeof(T) == 4, float4, double2>::type;
     const size_t nvec = nreal / W;
-    double acc[1] = {0.0};
-    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
-        V q = __ldcs(reinterpret_cast<const V *>(x) + i);
-        if constexpr (sizeof(T) == 4) {
-            acc[0] += (double)q.x * q.x + (double)q.y * q.y;
-            acc[0] += (double)q.z * q.z + (double)q.w * q.w;
-        } else {
-            acc[0] += q.x * q.x + q.y * q.y;
-        }
+    // four independent 128-bit loads in flight per thread, one fp64 accumulator each (added in a
+    // fixed order afterwards, so the result does not depend on timing)
+    constexpr int UN = 4;
+    double a4[UN] = {0.0, 0.0, 0.0, 0.0};
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+    auto sq = [](V q) -> double {
+        if constexpr (sizeof(T) == 4) return ((double)q.x * q.x + (double)q.y * q.y) + ((double)q.z * q.z + (double)q.w * q.w);
+        else return q.x * q.x + q.y * q.y;
+    };
+    for (; i + (UN - 1) * stride < nvec; i += UN * stride) {
+        V q[UN];
+#pragma unroll
+        for (int u = 0; u < UN; u++) q[u] = __ldcs(reinterpret_cast<const V *>(x) + i + u * stride);
+#pragma unroll
+        for (int u = 0; u < UN; u++) a4[u] += sq(q[u]);
     }
+    for (; i < nvec; i += stride) a4[0] += sq(__ldcs(reinterpret_cast<const V *>(x) + i));
+    double acc[1] = {(a4[0] + a4[1]) + (a4[2] + a4[3])};
     // tail (nreal is a multiple of 24, so this never runs for fp32/fp64 fields; kept for safety)
     if (blockIdx.x == 0 && threadIdx.x == 0)
         for (size_t i = nvec * W; i < nreal; i++) acc[0] += (double)x[i] * (double)x[i];
