@@ -197,13 +197,14 @@ int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, i
     g->opt_raster_staged = 1;
     g->opt_variant = 0;
     g->opt_kernel = 0;
-    g->opt_l2pol = 11212020;     // out, links evict_first; x3+ evict_last; x3- evict_first; top layer evict_last
+    g->opt_l2pol = 11222222;     // out, links evict_first; every input box evict_last (sweeps: least DRAM re-reads)
     g->opt_ssplit = 1;
     g->opt_zigzag = 1;
     g->opt_prefetch = 0;
+    g->opt_layered = 1;
 
     g->gauge_bytes = (size_t)8 * 18 * (size_t)g->lat.Vh * (size_t)precision;
-    g->reduce_blocks = g->sm_count * 8;
+    g->reduce_blocks = g->sm_count * 32;
     bool ok = cudaMalloc(&g->gauge[0], g->gauge_bytes) == cudaSuccess &&
               cudaMalloc(&g->gauge[1], g->gauge_bytes) == cudaSuccess &&
               cudaMalloc(&g->partials, sizeof(double) * 2 * (size_t)g->reduce_blocks) == cudaSuccess &&
@@ -259,6 +260,9 @@ int dwf_set_option(dwf_geometry *g, const char *key, long long value)
         return DWF_OK;
     } else if (!strcmp(key, "zigzag")) {
         g->opt_zigzag = v != 0;
+        return DWF_OK;
+    } else if (!strcmp(key, "layered")) {
+        g->opt_layered = v != 0;
         return DWF_OK;
     } else if (!strcmp(key, "prefetch")) {
         g->opt_prefetch = v;

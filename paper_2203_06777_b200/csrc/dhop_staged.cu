@@ -68,6 +68,7 @@ struct StagedArgs {
     int parity_out;
     int l2pol;               // decimal digits, see PC_*
     int zigzag;              // walk the slices of every other tile backwards
+    int layered;             // one TMA box per x3 layer (per-layer L2 policies) instead of one per region
     int prefetch;            // producer prefetches the input of step g + prefetch into L2 (0: off); bit 4..: box mask
     int ablate;              // timing experiments only (wrong results): 1 no link refill, 2 no stores, 4 no legs, 8 no TMA
 };
@@ -100,6 +101,10 @@ template <int LH, int B1, int B2, int B3> struct StagedCfg {
     static_assert(ROWB % 128 == 0, "staged rows must keep TMA destinations 128-byte aligned");
 };
 
+#ifndef DWF_REFILL_PER_LEG
+#define DWF_REFILL_PER_LEG 1   // 1: refill a leg's links right after the leg (last slice of a tile); 0: all after the last leg
+#endif
+static constexpr bool REFILL_PER_LEG = DWF_REFILL_PER_LEG;
 #ifndef DWF_ABL
 #define DWF_ABL 0      // timing experiments: 1 = legs without shared-memory reads, 2 = legs without arithmetic
 #endif
@@ -203,6 +208,7 @@ template <int LH, int B1, int B2, int B3>
 __global__ void __launch_bounds__(StagedCfg<LH, B1, B2, B3>::NT, StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM)
 dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_x1,
                    const __grid_constant__ CUtensorMap map_x2, const __grid_constant__ CUtensorMap map_x3,
+                   const __grid_constant__ CUtensorMap map_x1l, const __grid_constant__ CUtensorMap map_x2l,
                    const StagedArgs args)
 {
     using Cfg = StagedCfg<LH, B1, B2, B3>;
@@ -234,6 +240,8 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         tma_prefetch_desc(&map_x1);
         tma_prefetch_desc(&map_x2);
         tma_prefetch_desc(&map_x3);
+        tma_prefetch_desc(&map_x1l);
+        tma_prefetch_desc(&map_x2l);
         for (int i = 0; i < 2 * Cfg::NREG; i++) {
             mbar_init(full_base + 8 * i, 1);
             mbar_init(empty_base + 8 * i, Cfg::NWARP_C);
@@ -297,21 +305,46 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             if (notma || no12) mbar_arrive(fb + 8);
             else {
                 mbar_arrive_expect_tx(fb + 8, 2 * B1 * B3 * Cfg::ROWB);
-                tma_load_5d_hint(dst + Cfg::R_X2M * Cfg::ROWB, &map_x2, fb + 8, 0, 0, b.o1, b.x2m, b.c4, pol[PC_X12]);
-                tma_load_5d_hint(dst + Cfg::R_X2P * Cfg::ROWB, &map_x2, fb + 8, 0, 0, b.o1, b.x2p, b.c4, pol[PC_X12]);
+                if (args.layered) {
+#pragma unroll
+                    for (int j = 0; j < B3; j++) {
+                        const uint64_t pf = pol[j == B3 - 1 ? PC_X12_TOP : PC_X12];
+                        tma_load_5d_hint(dst + (Cfg::R_X2M + j * B1) * Cfg::ROWB, &map_x2l, fb + 8, 0, 0, b.o1, b.x2m, b.c4 + j, pf);
+                        tma_load_5d_hint(dst + (Cfg::R_X2P + j * B1) * Cfg::ROWB, &map_x2l, fb + 8, 0, 0, b.o1, b.x2p, b.c4 + j, pf);
+                    }
+                } else {
+                    tma_load_5d_hint(dst + Cfg::R_X2M * Cfg::ROWB, &map_x2, fb + 8, 0, 0, b.o1, b.x2m, b.c4, pol[PC_X12]);
+                    tma_load_5d_hint(dst + Cfg::R_X2P * Cfg::ROWB, &map_x2, fb + 8, 0, 0, b.o1, b.x2p, b.c4, pol[PC_X12]);
+                }
             }
             if (g >= 2) mbar_wait(eb + 16, epar);
             if (notma || no12) mbar_arrive(fb + 16);
             else {
                 mbar_arrive_expect_tx(fb + 16, 2 * B2 * B3 * Cfg::ROWB);
-                tma_load_5d_hint(dst + Cfg::R_X1M * Cfg::ROWB, &map_x1, fb + 16, 0, 0, b.x1m, b.o2, b.c4, pol[PC_X12]);
-                tma_load_5d_hint(dst + Cfg::R_X1P * Cfg::ROWB, &map_x1, fb + 16, 0, 0, b.x1p, b.o2, b.c4, pol[PC_X12]);
+                if (args.layered) {
+#pragma unroll
+                    for (int j = 0; j < B3; j++) {
+                        const uint64_t pf = pol[j == B3 - 1 ? PC_X12_TOP : PC_X12];
+                        tma_load_5d_hint(dst + (Cfg::R_X1M + j * B2) * Cfg::ROWB, &map_x1l, fb + 16, 0, 0, b.x1m, b.o2, b.c4 + j, pf);
+                        tma_load_5d_hint(dst + (Cfg::R_X1P + j * B2) * Cfg::ROWB, &map_x1l, fb + 16, 0, 0, b.x1p, b.o2, b.c4 + j, pf);
+                    }
+                } else {
+                    tma_load_5d_hint(dst + Cfg::R_X1M * Cfg::ROWB, &map_x1, fb + 16, 0, 0, b.x1m, b.o2, b.c4, pol[PC_X12]);
+                    tma_load_5d_hint(dst + Cfg::R_X1P * Cfg::ROWB, &map_x1, fb + 16, 0, 0, b.x1p, b.o2, b.c4, pol[PC_X12]);
+                }
             }
             if (g >= 2) mbar_wait(eb + 24, epar);
             if (notma) mbar_arrive(fb + 24);
             else {
                 mbar_arrive_expect_tx(fb + 24, Cfg::NROW_C * Cfg::ROWB);
-                tma_load_5d_hint(dst, &map_c, fb + 24, 0, 0, b.o1, b.o2, b.c4, pol[PC_CENTRE]);
+                if (args.layered) {
+#pragma unroll
+                    for (int j = 0; j < B3; j++)
+                        tma_load_5d_hint(dst + (j * B1 * B2) * Cfg::ROWB, &map_x3, fb + 24, 0, 0, b.o1, b.o2, b.c4 + j,
+                                         pol[j == B3 - 1 ? PC_CENTRE_TOP : PC_CENTRE]);
+                } else {
+                    tma_load_5d_hint(dst, &map_c, fb + 24, 0, 0, b.o1, b.o2, b.c4, pol[PC_CENTRE]);
+                }
             }
         }
         return;
@@ -386,7 +419,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         float2 acc[12];
 #define DWF_LEG(L, MU, FWD, FIRST)                                                                  \
         staged_leg<LH, MU, FWD, FIRST, DWF_ABL>(acc, reinterpret_cast<const float4 *>(sb + off[L]), U + 9 * (L)); \
-        if constexpr (FETCH) {      /* refill the component pairs whose last use was this leg */      \
+        if constexpr (FETCH && REFILL_PER_LEG) {   /* refill the component pairs whose last use was this leg */ \
             _Pragma("unroll") for (int j = (9 * (L)) / 2; j < (9 * ((L) + 1)) / 2; j++) {            \
                 const float4 q = ldg128_hint(gnext + j * LH, pol_g);                                \
                 U[2 * j] = make_float2(q.x, q.y);                                                   \
@@ -422,6 +455,21 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         DWF_RELEASE(3)
 #undef DWF_LEG
 #undef DWF_RELEASE
+        // Last slice of the tile: refill the links for the next tile, all at once and in the
+        // order the next step uses them (legs 6, 7, 4, 5, 2, 3, 0, 1).  Spreading the loads over
+        // the legs of this step made later legs wait on the scoreboard the loads share.
+        if constexpr (FETCH && !REFILL_PER_LEG) {
+#pragma unroll
+            for (int q = 0; q < 4; q++) {
+                const int pair = 3 - q;                      // legs 2*pair, 2*pair + 1 = vectors 9*pair .. 9*pair + 8
+#pragma unroll
+                for (int j = 9 * pair; j < 9 * pair + 9; j++) {
+                    const float4 v = ldg128_hint(gnext + j * LH, pol_g);
+                    U[2 * j] = make_float2(v.x, v.y);
+                    U[2 * j + 1] = make_float2(v.z, v.w);
+                }
+            }
+        }
         if (!legs || !active) return;
         if (!(args.ablate & 2)) {
 #pragma unroll
@@ -556,12 +604,14 @@ static int encode_map(CUtensorMap *m, const void *base, const Lattice &lat, int 
 int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st)
 {
     const Variant &v = variants()[(size_t)g->staged.variant];
-    CUtensorMap mc, m1, m2, m3;
+    CUtensorMap mc, m1, m2, m3, m1l, m2l;
     int rc;
     if ((rc = encode_map(&mc, in, g->lat, v.b1, v.b2, v.b3))) return rc;
     if ((rc = encode_map(&m1, in, g->lat, 1, v.b2, v.b3))) return rc;
     if ((rc = encode_map(&m2, in, g->lat, v.b1, 1, v.b3))) return rc;
     if ((rc = encode_map(&m3, in, g->lat, v.b1, v.b2, 1))) return rc;
+    if ((rc = encode_map(&m1l, in, g->lat, 1, v.b2, 1))) return rc;
+    if ((rc = encode_map(&m2l, in, g->lat, v.b1, 1, 1))) return rc;
     StagedArgs a;
     a.out = static_cast<float2 *>(out);
     a.gauge = static_cast<const float2 *>(g->gauge[parity_out]);
@@ -572,6 +622,7 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     a.l2pol = g->opt_l2pol;
     a.zigzag = g->opt_zigzag;
     a.prefetch = g->opt_prefetch;
+    a.layered = g->opt_layered;
     a.ablate = g->opt_ablate;
     int ssplit = g->opt_ssplit > 0 ? g->opt_ssplit : 1;
     const int slots = g->sm_count * v.ctas_per_sm;       // co-resident CTAs
@@ -584,7 +635,7 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     }
     const int ngroup_max = slots / ssplit;
     const int ngroup = g->staged.ntiles < ngroup_max ? g->staged.ntiles : ngroup_max;
-    void *params[] = {&mc, &m1, &m2, &m3, &a};
+    void *params[] = {&mc, &m1, &m2, &m3, &m1l, &m2l, &a};
     DWF_CUDA_CHECK(cudaLaunchKernel(v.fn, dim3((unsigned)(ngroup * ssplit)), dim3((unsigned)v.threads), params,
                                     (size_t)v.smem, st));
     count_launch();
