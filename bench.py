@@ -222,7 +222,7 @@ def run_reference(args, w):
 # ---------------------------------------------------------------------------------------------
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
 # `ncu --set full` capture summarised under profiles/ (None until a capture exists).
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {"c4": 1475511000 + 769920000}   # profiles/r01f_dhop_staged_ws_kernel_ncu.md, launch 1
 
 
 def run_gpu(args, w):
