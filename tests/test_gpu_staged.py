@@ -1,0 +1,173 @@
+"""GPU parity of the TMA-staged, link-stationary fp32 kernel (csrc/dhop_staged.cu) in the launch
+configurations bench.py times: tiles per CTA > 1 (tile switch with link refill), Lh = 16 and
+Lh = 24 rows, every tunable, and BASELINE.json's full-size configs C4 / C5 on sampled output
+sites (oracle.dhop_sites computes them one by one) plus properties that hold at any size.
+Bars: relative L2 error <= 2e-6 (fp32), <= 1e-13 (fp64)."""
+import numpy as np
+import pytest
+
+import dwf_inputs as gen
+import oracle
+from _util import rel_err
+
+pytestmark = pytest.mark.gpu
+
+TOL = {4: 2e-6, 8: 1e-13}
+
+
+def sample_sites(dims, parity, n, seed):
+    """n lexicographic site indices of the given parity: random ones plus the lattice corners and
+    sites on every boundary face (periodic wrap, antiperiodic time hop)."""
+    L = [int(d) for d in dims]
+    rng = np.random.default_rng(seed)
+    coords = rng.integers(0, L, size=(4 * n, 4))
+    edge = []
+    for mask in range(16):
+        edge.append([(L[m] - 1) if (mask >> m) & 1 else 0 for m in range(4)])
+    for m in range(4):
+        for v in (0, 1, L[m] - 2, L[m] - 1):
+            c = rng.integers(0, L, size=(8, 4))
+            c[:, m] = v
+            edge.extend(c.tolist())
+    coords = np.concatenate([np.array(edge, dtype=np.int64), coords])
+    coords = coords[(coords.sum(axis=1) & 1) == parity][:n]
+    x = coords[:, 0] + L[0] * (coords[:, 1] + L[1] * (coords[:, 2] + L[2] * coords[:, 3]))
+    return np.unique(x)
+
+
+def cb_rows(dims, sites):
+    """Row index of lexicographic sites inside the half field of their parity (cb index x >> 1)."""
+    return np.asarray(sites, dtype=np.int64) >> 1
+
+
+def check_cb_against_oracle(lib, dims, Ls, prec, bc, seed, near_unit=False):
+    V = gen.volume(dims)
+    U = gen.gauge_near_unit(dims, seed, 0.2, prec=prec) if near_unit else gen.gauge_random(dims, seed, prec=prec)
+    psi = gen.spinor_gaussian(V, Ls, seed, prec=prec)
+    with lib.Geometry(dims, Ls, prec, bc) as g:
+        g.load_gauge(U)
+        g.set_option("kernel", 2)          # staged kernel or an error: no silent fall back to the direct kernel
+        for p_out in (1, 0):
+            half = gen.split_parity(psi, dims, 1 - p_out)
+            fin = g.import_spinor(half, 1 - p_out)
+            fout = g.dhop_oe(fin) if p_out == 1 else g.dhop_eo(fin)
+            got = g.export_spinor(fout, p_out)
+            want = oracle.dhop_cb(dims, Ls, bc, p_out, U, half)
+            assert rel_err(got, want) <= TOL[prec], (dims, Ls, p_out)
+
+
+def test_staged_lh16_many_tiles_per_cta(lib):
+    # <16,4,2,2> rows boxes: 4 x 8 x 8 = 256 tiles on 148 CTAs -> tile switch and link refill
+    check_cb_against_oracle(lib, (32, 16, 16, 16), 4, 4, lib.ANTIPERIODIC_T, 41)
+
+
+def test_staged_lh16_ragged_tail_of_tiles(lib):
+    # 4 x 5 x 9 = 180 tiles: CTAs with one and with two tiles; Ls = 5 (odd), periodic
+    check_cb_against_oracle(lib, (32, 16, 10, 18), 5, 4, lib.PERIODIC, 42)
+
+
+def test_staged_lh24_many_tiles_per_cta(lib):
+    # <24,2,2,2>: 6 x 6 x 6 = 216 tiles, 192 of 256 consumer threads active, Ls = 3
+    check_cb_against_oracle(lib, (48, 12, 12, 12), 3, 4, lib.ANTIPERIODIC_T, 43)
+
+
+def test_staged_lh8_and_lh4(lib):
+    check_cb_against_oracle(lib, (16, 8, 8, 12), 6, 4, lib.ANTIPERIODIC_T, 44)
+    check_cb_against_oracle(lib, (8, 8, 12, 8), 7, 4, lib.PERIODIC, 45)
+
+
+OPTION_SETS = [
+    {"variant": 2}, {"variant": 3}, {"variant": 12}, {"variant": 13}, {"variant": 14}, {"variant": 15},
+    {"raster_staged": 0}, {"raster_staged": 2}, {"raster_staged": 11}, {"raster_staged": 21}, {"raster_staged": 31},
+    {"zigzag": 0}, {"ssplit": 2}, {"ssplit": 4}, {"layered": 0}, {"prefetch": 17}, {"prefetch": 242},
+    {"l2pol": 0}, {"l2pol": 11212020},
+]
+
+
+def test_staged_tunables_do_not_change_the_result(lib):
+    """Tile shape, launch order, slice split, L2 policies and prefetch only move work around: the
+    arithmetic per output site is the same, so the results must be bit-identical; the direct
+    kernel (kernel=1) sums the legs in another order and is held to the parity bar instead."""
+    import torch
+    dims, Ls, prec, bc = (32, 16, 16, 16), 4, 4, lib.ANTIPERIODIC_T
+    U = gen.gauge_random(dims, 46, prec=prec)
+    half = gen.spinor_gaussian(gen.volume(dims) // 2, Ls, 46, prec=prec)
+    want = oracle.dhop_oe(dims, Ls, bc, U, half)
+    with lib.Geometry(dims, Ls, prec, bc) as g:
+        g.load_gauge(U)
+        fin = g.import_spinor(half, lib.EVEN)
+        ref = g.dhop_oe(fin).clone()
+        assert rel_err(g.export_spinor(ref, lib.ODD), want) <= TOL[prec]
+        defaults = {"variant": 0, "raster_staged": 1, "zigzag": 1, "ssplit": 1, "layered": 1, "prefetch": 0,
+                    "l2pol": 11222222}
+        for opts in OPTION_SETS:
+            for k, v in {**defaults, **opts}.items():
+                g.set_option(k, v)
+            out = g.dhop_oe(fin)
+            assert torch.equal(out, ref), opts
+        for k, v in defaults.items():
+            g.set_option(k, v)
+        g.set_option("kernel", 1)
+        assert rel_err(g.export_spinor(g.dhop_oe(fin), lib.ODD), want) <= TOL[prec]
+        g.set_option("kernel", 2)
+        assert torch.equal(g.dhop_oe(fin), ref)
+
+
+@pytest.mark.parametrize("prec", [4, 8])
+def test_c4_full_size_oe_then_eo_sampled(lib, prec):
+    """BASELINE.json configs[3]: 32^4 x 16, near-unit gauge, Gaussian spinor on the even
+    checkerboard, DhopOE followed by DhopEO -- the launch configuration bench.py times."""
+    dims, Ls, bc, seed = (32, 32, 32, 32), 16, lib.PERIODIC, 1004
+    U = gen.gauge_near_unit(dims, seed, 0.2, prec=prec)
+    psi_e = gen.spinor_gaussian(gen.volume(dims) // 2, Ls, seed, prec=prec)
+    with lib.Geometry(dims, Ls, prec, bc) as g:
+        g.load_gauge(U)
+        f_e = g.import_spinor(psi_e, lib.EVEN)
+        f_o = g.dhop_oe(f_e)
+        f_e2 = g.dhop_eo(f_o)
+        chi_o = g.export_spinor(f_o, lib.ODD)
+        phi_e = g.export_spinor(f_e2, lib.EVEN)
+        n_in, n_mid, n_out = g.norm2(f_e, lib.EVEN), g.norm2(f_o, lib.ODD), g.norm2(f_e2, lib.EVEN)
+    odd = sample_sites(dims, 1, 600, 7)
+    want = oracle.dhop_sites(dims, Ls, bc, U, psi_e, True, odd)
+    assert rel_err(chi_o[cb_rows(dims, odd)], want) <= TOL[prec]
+    even = sample_sites(dims, 0, 600, 8)
+    want = oracle.dhop_sites(dims, Ls, bc, U, chi_o, True, even)      # the GPU's own chi_o is the input here
+    assert rel_err(phi_e[cb_rows(dims, even)], want) <= TOL[prec]
+    # properties at full size: P8 norm bound, and the GPU norm2 against the oracle's on the exported field
+    assert n_mid <= 64.0 * n_in and n_out <= 64.0 * n_mid
+    assert abs(n_mid - oracle.norm2(chi_o)) <= 1e-12 * n_mid
+    assert abs(n_out - oracle.norm2(phi_e)) <= 1e-12 * n_out
+
+
+def test_c5_full_size_sampled(lib):
+    """BASELINE.json configs[4]: 48^3 x 96 x Ls=12 fp32, random SU(3), antiperiodic time: full Dhop,
+    the even/odd pair and norm2 of the result, on sampled sites."""
+    dims, Ls, prec, bc, seed = (48, 48, 48, 96), 12, 4, lib.ANTIPERIODIC_T, 1005
+    V = gen.volume(dims)
+    U = gen.gauge_random(dims, seed, prec=prec)
+    psi = gen.spinor_gaussian(V, Ls, seed, prec=prec)
+    par = gen.site_parity(dims)
+    with lib.Geometry(dims, Ls, prec, bc) as g:
+        g.load_gauge(U)
+        f = g.import_spinor(psi, lib.FULL)
+        out = g.dhop(f)
+        n_in, n_out = g.norm2(f), g.norm2(out)
+        got = g.export_spinor(out, lib.FULL)
+        del f, out
+        assert n_out <= 64.0 * n_in
+        assert abs(n_out - oracle.norm2(got)) <= 1e-12 * n_out
+        sites = np.concatenate([sample_sites(dims, 0, 300, 9), sample_sites(dims, 1, 300, 10)])
+        want = oracle.dhop_sites(dims, Ls, bc, U, psi, False, sites)
+        assert rel_err(got[sites], want) <= TOL[prec]
+        # the even/odd pair must reproduce the two halves of the full result (bitwise: same kernel, same order)
+        for p_out in (1, 0):
+            half = np.ascontiguousarray(psi[par == 1 - p_out])
+            fin = g.import_spinor(half, 1 - p_out)
+            del half
+            fo = g.dhop_oe(fin) if p_out == 1 else g.dhop_eo(fin)
+            got_h = g.export_spinor(fo, p_out)
+            del fin, fo
+            s = sample_sites(dims, p_out, 300, 11 + p_out)
+            assert np.array_equal(got_h[cb_rows(dims, s)], got[s])
+            del got_h
