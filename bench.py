@@ -225,6 +225,22 @@ def run_reference(args, w):
 NCU_TRAFFIC_BYTES = {"c4": 1475511000 + 769920000}   # profiles/r01f_dhop_staged_ws_kernel_ncu.md, launch 1
 
 
+def max_over_ranks(x, dist=None, device="cuda"):
+    """Slowest rank's time (device-timed milliseconds): all-reduce MAX over the process group (N > 1)."""
+    if dist is None:
+        return x
+    import torch
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_gflops(world, sites_per_half_dhop, ms_step):
+    """Replicas only: every rank runs the same two half-Dhops per step, so the
+    whole-job throughput is world x per-rank flop over the slowest rank's step time."""
+    return world * 2 * FLOP_PER_SITE * sites_per_half_dhop / (ms_step * 1e-3) / 1e9
+
+
 def run_gpu(args, w):
     import torch
     import paper_2203_06777_b200 as dwf
@@ -245,13 +261,6 @@ def run_gpu(args, w):
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
-
-    def max_over_ranks(x):
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
 
     d, Ls, prec = w["dims"], w["Ls"], w["prec"]
     V4 = d[0] * d[1] * d[2] * d[3]
@@ -294,12 +303,12 @@ def run_gpu(args, w):
     barrier()
     launches = dwf.dwf_launch_count() - l0
     clocks = sampler.stop()
-    ms_total = max_over_ranks(t_start.elapsed_time(t_end))
+    ms_total = max_over_ranks(t_start.elapsed_time(t_end), dist)
     ms_step = ms_total / args.steps
     t_oe = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
     t_eo = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
     t_n2 = float(np.mean([e[2].elapsed_time(e[3]) for e in ev]))
-    value = world * 2 * FLOP_PER_SITE * sites / (ms_step * 1e-3) / 1e9
+    value = whole_job_gflops(world, sites, ms_step)
 
     # ---- e2e: the same step through the C ABI with HOST buffers ----
     host_in = torch.empty(psi_e.shape, dtype=torch.from_numpy(psi_e).dtype, pin_memory=True)
@@ -324,8 +333,8 @@ def run_gpu(args, w):
         n_e2e = step_e2e()
     e1.record()
     barrier()
-    ms_e2e = max_over_ranks(e0.elapsed_time(e1)) / k_e2e
-    e2e_val = world * 2 * FLOP_PER_SITE * sites / (ms_e2e * 1e-3) / 1e9
+    ms_e2e = max_over_ranks(e0.elapsed_time(e1), dist) / k_e2e
+    e2e_val = whole_job_gflops(world, sites, ms_e2e)
     field_bytes = psi_e.nbytes
 
     if rank != 0:
