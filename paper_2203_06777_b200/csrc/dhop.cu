@@ -45,8 +45,24 @@ __device__ __forceinline__ void dhop_leg(typename CxT<T>::type (&acc)[12][SC],
 {
     using C = typename CxT<T>::type;
     C psi[12][SC];
+    if constexpr (sizeof(T) == 8) {
 #pragma unroll
-    for (int k = 0; k < 12; k++) load_cx<SC>(nb + pair_off(k, W0), psi[k]);
+        for (int k = 0; k < 12; k++) load_cx<SC>(nb + pair_off(k, W0), psi[k]);
+    } else {
+        // fp32 fields store spin pairs (pack.cu): slot 4c + t -> (re|im of spins 0,1 | 2,3)
+        C q[12][SC];
+#pragma unroll
+        for (int k = 0; k < 12; k++) load_cx<SC>(nb + pair_off(k, W0), q[k]);
+#pragma unroll
+        for (int j = 0; j < SC; j++)
+#pragma unroll
+            for (int c = 0; c < 3; c++) {
+                psi[0 + c][j] = C{q[4 * c + 0][j].x, q[4 * c + 1][j].x};
+                psi[3 + c][j] = C{q[4 * c + 0][j].y, q[4 * c + 1][j].y};
+                psi[6 + c][j] = C{q[4 * c + 2][j].x, q[4 * c + 3][j].x};
+                psi[9 + c][j] = C{q[4 * c + 2][j].y, q[4 * c + 3][j].y};
+            }
+    }
     C U[9];
     load_link<T, LEG>(site_links, W0, U);
 
@@ -118,7 +134,7 @@ __device__ __forceinline__ void dhop_leg(typename CxT<T>::type (&acc)[12][SC],
 
 // ---------------------------------------------------------------------------------------------
 // direct kernel: neighbours are read straight from global memory (L1/L2 catch the reuse).
-// in/out are half fields complex[s][row][k/2][h][k&1]; out has parity `parity_out`, in the opposite parity.
+// in/out are half fields pair[s][row][k/2][h][k&1] (slot meaning: pack.cu); out has parity `parity_out`, in the opposite parity.
 // One thread = one output site and one s-slice.
 // ---------------------------------------------------------------------------------------------
 template <typename T, int MAXT, int MINB>
@@ -178,8 +194,24 @@ dhop_direct_kernel(const typename CxT<T>::type *__restrict__ in, typename CxT<T>
     dhop_leg<T, SC, 3, false, false, 7>(acc, base + n3m, W0, gl);
 
     C *o = out + (size_t)s * 12 * (size_t)Vh + (size_t)own;
+    if constexpr (sizeof(T) == 8) {
 #pragma unroll
-    for (int k = 0; k < 12; k++) store_cx<SC>(o + pair_off(k, W0), acc[k]);
+        for (int k = 0; k < 12; k++) store_cx<SC>(o + pair_off(k, W0), acc[k]);
+    } else {
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            C q[4][SC];
+#pragma unroll
+            for (int j = 0; j < SC; j++) {
+                q[0][j] = C{acc[0 + c][j].x, acc[3 + c][j].x};
+                q[1][j] = C{acc[0 + c][j].y, acc[3 + c][j].y};
+                q[2][j] = C{acc[6 + c][j].x, acc[9 + c][j].x};
+                q[3][j] = C{acc[6 + c][j].y, acc[9 + c][j].y};
+            }
+#pragma unroll
+            for (int t = 0; t < 4; t++) store_cx<SC>(o + pair_off(4 * c + t, W0), q[t]);
+        }
+    }
 }
 
 template <typename T, int MAXT, int MINB>

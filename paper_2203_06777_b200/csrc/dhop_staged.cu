@@ -109,97 +109,104 @@ static constexpr bool REFILL_PER_LEG = DWF_REFILL_PER_LEG;
 #define DWF_ABL 0      // timing experiments: 1 = legs without shared-memory reads, 2 = legs without arithmetic
 #endif
 
-// one leg: acc += reconstruct( U * project(psi) ), psi read from shared memory
+// ---- arithmetic on spin pairs ------------------------------------------------------------------
+// A register pair holds one real part of TWO spin components (layout: pack.cu), e.g. for colour c
+//   Are[c] = (re psi_0c, re psi_1c)   Aim[c] = (im psi_0c, im psi_1c)      spins 0,1
+//   Bre[c] = (re psi_2c, re psi_3c)   Bim[c] = (im psi_2c, im psi_3c)      spins 2,3
+// A half spinor h = (h0, h1) is P[c] = (re h0c, re h1c), Q[c] = (im h0c, im h1c), so that
+//   (U h)_a :  Xre[a] = sum_b ( u_ab.re P[b] - u_ab.im Q[b] ),  Xim[a] = sum_b ( u_ab.re Q[b] + u_ab.im P[b] )
+// is 12 packed FMUL2 / FFMA2 per row with the link element as the broadcast scalar and no combine
+// step: 6 + 36 + 12 = 54 packed instructions per leg, the 840 lane-operations of the flop count.
+__device__ __forceinline__ float2 swp(float2 a) { return make_float2(a.y, a.x); }           // (x1, x0)
+__device__ __forceinline__ float2 npm(float2 a) { return make_float2(-a.x, a.y); }          // (-, +)
+__device__ __forceinline__ float2 pnm(float2 a) { return make_float2(a.x, -a.y); }          // (+, -)
+__device__ __forceinline__ float2 neg(float2 a) { return make_float2(-a.x, -a.y); }
+
+// one leg: acc += reconstruct( U * project(psi) ), psi read from shared memory.
+// acc[4a + t]: t = 0 (re of out spins 0,1), 1 (im of 0,1), 2 (re of 2,3), 3 (im of 2,3), colour a:
+// exactly the slot order of the stored field, so the store needs no shuffling.
 template <int LH, int MU, bool FWD, bool FIRST, int ABL = 0>
 __device__ __forceinline__ void staged_leg(float2 (&acc)[12], const float4 *__restrict__ nb, const float2 *__restrict__ U)
 {
-    float2 p[12];
+    float2 q[12];
     if constexpr (ABL == 1) {          // timing experiment: no shared-memory reads
 #pragma unroll
-        for (int k = 0; k < 12; k++) p[k] = FIRST ? U[k % 9] : acc[k];
+        for (int k = 0; k < 12; k++) q[k] = FIRST ? U[k % 9] : acc[k];
     } else {
 #pragma unroll
-        for (int j = 0; j < 6; j++) {      // LDS.128: components 2j and 2j+1 of the neighbour site
-            const float4 q = nb[j * LH];
-            p[2 * j] = make_float2(q.x, q.y);
-            p[2 * j + 1] = make_float2(q.z, q.w);
+        for (int j = 0; j < 6; j++) {      // LDS.128: slots 2j and 2j+1 of the neighbour site
+            const float4 v = nb[j * LH];
+            q[2 * j] = make_float2(v.x, v.y);
+            q[2 * j + 1] = make_float2(v.z, v.w);
         }
     }
     if constexpr (ABL == 2) {          // timing experiment: no arithmetic
 #pragma unroll
         for (int k = 0; k < 12; k++) {
-            if (FIRST) acc[k] = p[k];
-            else { acc[k].x = __int_as_float(__float_as_int(acc[k].x) ^ __float_as_int(p[k].x)); acc[k].y = __int_as_float(__float_as_int(acc[k].y) ^ __float_as_int(p[k].y)); }
+            if (FIRST) acc[k] = q[k];
+            else { acc[k].x = __int_as_float(__float_as_int(acc[k].x) ^ __float_as_int(q[k].x)); acc[k].y = __int_as_float(__float_as_int(acc[k].y) ^ __float_as_int(q[k].y)); }
         }
         return;
     }
-    float2 h0[3], h1[3];
+    // projection (1 -/+ gamma_mu) psi -> upper two spin components, table in SURVEY.md section 8(c)
+    float2 P[3], Q[3];
 #pragma unroll
     for (int c = 0; c < 3; c++) {
-        const float2 p0 = p[c], p1 = p[3 + c], p2 = p[6 + c], p3 = p[9 + c];
-        if constexpr (MU == 0) {
-            h0[c] = FWD ? csubi(p0, p3) : caddi(p0, p3);
-            h1[c] = FWD ? csubi(p1, p2) : caddi(p1, p2);
-        } else if constexpr (MU == 1) {
-            h0[c] = FWD ? cadd(p0, p3) : csub(p0, p3);
-            h1[c] = FWD ? csub(p1, p2) : cadd(p1, p2);
-        } else if constexpr (MU == 2) {
-            h0[c] = FWD ? csubi(p0, p2) : caddi(p0, p2);
-            h1[c] = FWD ? caddi(p1, p3) : csubi(p1, p3);
-        } else {
-            h0[c] = FWD ? csub(p0, p2) : cadd(p0, p2);
-            h1[c] = FWD ? csub(p1, p3) : cadd(p1, p3);
+        const float2 Are = q[4 * c], Aim = q[4 * c + 1], Bre = q[4 * c + 2], Bim = q[4 * c + 3];
+        if constexpr (MU == 0) {            // h0 = psi0 -/+ i psi3, h1 = psi1 -/+ i psi2
+            P[c] = f2_add(Are, FWD ? swp(Bim) : neg(swp(Bim)));
+            Q[c] = f2_add(Aim, FWD ? neg(swp(Bre)) : swp(Bre));
+        } else if constexpr (MU == 1) {     // h0 = psi0 +/- psi3, h1 = psi1 -/+ psi2
+            P[c] = f2_add(Are, FWD ? pnm(swp(Bre)) : npm(swp(Bre)));
+            Q[c] = f2_add(Aim, FWD ? pnm(swp(Bim)) : npm(swp(Bim)));
+        } else if constexpr (MU == 2) {     // h0 = psi0 -/+ i psi2, h1 = psi1 +/- i psi3
+            P[c] = f2_add(Are, FWD ? pnm(Bim) : npm(Bim));
+            Q[c] = f2_add(Aim, FWD ? npm(Bre) : pnm(Bre));
+        } else {                            // h0 = psi0 -/+ psi2, h1 = psi1 -/+ psi3
+            P[c] = f2_add(Are, FWD ? neg(Bre) : Bre);
+            Q[c] = f2_add(Aim, FWD ? neg(Bim) : Bim);
         }
     }
 #pragma unroll
     for (int a = 0; a < 3; a++) {
-        // x = sum_b U[a][b] * h[b] as  A + iB,  A = sum u.re * h,  B = sum u.im * h
         const float2 u0 = U[3 * a], u1 = U[3 * a + 1], u2 = U[3 * a + 2];
-        float2 A0 = f2_mul(make_float2(u0.x, u0.x), h0[0]);
-        float2 B0 = f2_mul(make_float2(u0.y, u0.y), h0[0]);
-        float2 A1 = f2_mul(make_float2(u0.x, u0.x), h1[0]);
-        float2 B1 = f2_mul(make_float2(u0.y, u0.y), h1[0]);
-        A0 = f2_fma(make_float2(u1.x, u1.x), h0[1], A0);
-        B0 = f2_fma(make_float2(u1.y, u1.y), h0[1], B0);
-        A1 = f2_fma(make_float2(u1.x, u1.x), h1[1], A1);
-        B1 = f2_fma(make_float2(u1.y, u1.y), h1[1], B1);
-        A0 = f2_fma(make_float2(u2.x, u2.x), h0[2], A0);
-        B0 = f2_fma(make_float2(u2.y, u2.y), h0[2], B0);
-        A1 = f2_fma(make_float2(u2.x, u2.x), h1[2], A1);
-        B1 = f2_fma(make_float2(u2.y, u2.y), h1[2], B1);
-        const float2 x0 = caddi(A0, B0), x1 = caddi(A1, B1);
+        float2 Xre = f2_mul(make_float2(u0.x, u0.x), P[0]);
+        float2 Xim = f2_mul(make_float2(u0.x, u0.x), Q[0]);
+        Xre = f2_fma(make_float2(-u0.y, -u0.y), Q[0], Xre);
+        Xim = f2_fma(make_float2(u0.y, u0.y), P[0], Xim);
+        Xre = f2_fma(make_float2(u1.x, u1.x), P[1], Xre);
+        Xim = f2_fma(make_float2(u1.x, u1.x), Q[1], Xim);
+        Xre = f2_fma(make_float2(-u1.y, -u1.y), Q[1], Xre);
+        Xim = f2_fma(make_float2(u1.y, u1.y), P[1], Xim);
+        Xre = f2_fma(make_float2(u2.x, u2.x), P[2], Xre);
+        Xim = f2_fma(make_float2(u2.x, u2.x), Q[2], Xim);
+        Xre = f2_fma(make_float2(-u2.y, -u2.y), Q[2], Xre);
+        Xim = f2_fma(make_float2(u2.y, u2.y), P[2], Xim);
+        // lower spin components r2, r3 of the leg as signed / swapped copies of (Xre, Xim)
+        float2 Lre, Lim;
+        if constexpr (MU == 0) {            // r2 = +/- i chi1, r3 = +/- i chi0
+            Lre = FWD ? neg(swp(Xim)) : swp(Xim);
+            Lim = FWD ? swp(Xre) : neg(swp(Xre));
+        } else if constexpr (MU == 1) {     // r2 = -/+ chi1, r3 = +/- chi0
+            Lre = FWD ? npm(swp(Xre)) : pnm(swp(Xre));
+            Lim = FWD ? npm(swp(Xim)) : pnm(swp(Xim));
+        } else if constexpr (MU == 2) {     // r2 = +/- i chi0, r3 = -/+ i chi1
+            Lre = FWD ? npm(Xim) : pnm(Xim);
+            Lim = FWD ? pnm(Xre) : npm(Xre);
+        } else {                            // r2 = -/+ chi0, r3 = -/+ chi1
+            Lre = FWD ? neg(Xre) : Xre;
+            Lim = FWD ? neg(Xim) : Xim;
+        }
         if constexpr (FIRST) {
-            acc[0 + a] = x0;
-            acc[3 + a] = x1;
-            if constexpr (MU == 0) {
-                acc[6 + a] = FWD ? cmuli(x1) : cmulni(x1);
-                acc[9 + a] = FWD ? cmuli(x0) : cmulni(x0);
-            } else if constexpr (MU == 1) {
-                acc[6 + a] = FWD ? cneg(x1) : x1;
-                acc[9 + a] = FWD ? x0 : cneg(x0);
-            } else if constexpr (MU == 2) {
-                acc[6 + a] = FWD ? cmuli(x0) : cmulni(x0);
-                acc[9 + a] = FWD ? cmulni(x1) : cmuli(x1);
-            } else {
-                acc[6 + a] = FWD ? cneg(x0) : x0;
-                acc[9 + a] = FWD ? cneg(x1) : x1;
-            }
+            acc[4 * a] = Xre;
+            acc[4 * a + 1] = Xim;
+            acc[4 * a + 2] = Lre;
+            acc[4 * a + 3] = Lim;
         } else {
-            acc[0 + a] = cadd(acc[0 + a], x0);
-            acc[3 + a] = cadd(acc[3 + a], x1);
-            if constexpr (MU == 0) {
-                acc[6 + a] = FWD ? caddi(acc[6 + a], x1) : csubi(acc[6 + a], x1);
-                acc[9 + a] = FWD ? caddi(acc[9 + a], x0) : csubi(acc[9 + a], x0);
-            } else if constexpr (MU == 1) {
-                acc[6 + a] = FWD ? csub(acc[6 + a], x1) : cadd(acc[6 + a], x1);
-                acc[9 + a] = FWD ? cadd(acc[9 + a], x0) : csub(acc[9 + a], x0);
-            } else if constexpr (MU == 2) {
-                acc[6 + a] = FWD ? caddi(acc[6 + a], x0) : csubi(acc[6 + a], x0);
-                acc[9 + a] = FWD ? csubi(acc[9 + a], x1) : caddi(acc[9 + a], x1);
-            } else {
-                acc[6 + a] = FWD ? csub(acc[6 + a], x0) : cadd(acc[6 + a], x0);
-                acc[9 + a] = FWD ? csub(acc[9 + a], x1) : cadd(acc[9 + a], x1);
-            }
+            acc[4 * a] = f2_add(acc[4 * a], Xre);
+            acc[4 * a + 1] = f2_add(acc[4 * a + 1], Xim);
+            acc[4 * a + 2] = f2_add(acc[4 * a + 2], Lre);
+            acc[4 * a + 3] = f2_add(acc[4 * a + 3], Lim);
         }
     }
 }

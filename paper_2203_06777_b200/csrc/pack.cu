@@ -1,10 +1,16 @@
 // pack.cu -- canonical <-> device layout conversion (hot path row a1 of SURVEY.md section 8).
 //
-// Spinor: canonical [site][s][k][reim]  <->  device complex[s][row][k/2][h][k&1]  (k = spin*3 +
-//         colour; row = x1 + L1*(x2 + L2*x3) is a lattice line along x0, h = x0>>1 the site of the
-//         parity on that line, so the cb site x>>1 is row*Lh + h; two components of a site are
-//         adjacent = one 128-bit vector in fp32), one such block per parity; a FULL field is the
-//         even block followed by the odd block (canonical site x -> parity p(x)).
+// Spinor: canonical [site][s][spin][colour][reim]  <->  device pair[s][row][k/2][h][k&1]: row = x1 +
+//         L1*(x2 + L2*x3) is a lattice line along x0, h = x0>>1 the site of the parity on that line,
+//         so the cb site x>>1 is row*Lh + h; a site has 12 slots k of two reals; slots 2j, 2j+1 of
+//         a site are adjacent (one 128-bit vector in fp32).  One such block per parity; a FULL
+//         field is the even block followed by the odd block (canonical site x -> parity p(x)).
+//         fp64: slot k = spin*3 + colour holds the complex number (re, im).
+//         fp32: slot k = 4*colour + t holds one real part of a PAIR OF SPINS: t = 0: (re psi_0c,
+//         re psi_1c), 1: (im psi_0c, im psi_1c), 2: (re psi_2c, re psi_3c), 3: (im psi_2c,
+//         im psi_3c).  The packed f32x2 arithmetic of dhop_staged.cu then multiplies a link
+//         element (a scalar) into both spin components of a half spinor at once and never needs a
+//         half-negated operand (dhop_staged.cu, "arithmetic").
 // Gauge : canonical [x][mu][a][b][reim]  ->  for each output parity p and each output site of that
 //         parity (cb index x>>1) the 8 links that site multiplies with:
 //            leg 2*mu   : U_mu(x)                       (forward hop,  psi(x+mu))
@@ -49,9 +55,22 @@ spinor_reorder_kernel(const T *__restrict__ src, T *__restrict__ dst, const Latt
             const int x3 = (int)(q / lat.L[2]);
             site = 2 * cb + ((x1 + x2 + x3 + par) & 1);
         }
-        const long long c = ((site * lat.Ls + s) * 12 + k);     // canonical complex index
-        if (IMPORT) reinterpret_cast<V *>(dst)[e] = reinterpret_cast<const V *>(src)[c];
-        else        reinterpret_cast<V *>(dst)[c] = reinterpret_cast<const V *>(src)[e];
+        if constexpr (sizeof(T) == 8) {
+            const long long c = ((site * lat.Ls + s) * 12 + k);     // canonical complex index
+            if (IMPORT) reinterpret_cast<V *>(dst)[e] = reinterpret_cast<const V *>(src)[c];
+            else        reinterpret_cast<V *>(dst)[c] = reinterpret_cast<const V *>(src)[e];
+        } else {
+            // fp32: slot k = 4*colour + t holds the spin pair (2*(t/2), 2*(t/2)+1) of one real part:
+            // t = 0 (re of spins 0,1), 1 (im of 0,1), 2 (re of 2,3), 3 (im of 2,3)
+            const int col = k >> 2, t = k & 3;
+            const long long i0 = (((site * lat.Ls + s) * 12 + ((t >> 1) * 6 + col)) << 1) + (t & 1);   // canonical real
+            if (IMPORT) reinterpret_cast<V *>(dst)[e] = V{src[i0], src[i0 + 6]};
+            else {
+                const V v = reinterpret_cast<const V *>(src)[e];
+                dst[i0] = v.x;
+                dst[i0 + 6] = v.y;
+            }
+        }
     }
 }
 

@@ -83,18 +83,16 @@ inner_partial_kernel(const T *__restrict__ a, const T *__restrict__ b, size_t nc
         V p = __ldcs(reinterpret_cast<const V *>(a) + i);
         V q = __ldcs(reinterpret_cast<const V *>(b) + i);
         // conj(a) * b = (ar br + ai bi) + i (ar bi - ai br)
-        acc[0] += (double)p.x * q.x + (double)p.y * q.y;
-        acc[1] += (double)p.x * q.y - (double)p.y * q.x;
         if constexpr (sizeof(T) == 4) {
-            acc[0] += (double)p.z * q.z + (double)p.w * q.w;
-            acc[1] += (double)p.z * q.w - (double)p.w * q.z;
+            // fp32 vector = (re, re', im, im') of two spin components (pack.cu)
+            acc[0] += ((double)p.x * q.x + (double)p.z * q.z) + ((double)p.y * q.y + (double)p.w * q.w);
+            acc[1] += ((double)p.x * q.z - (double)p.z * q.x) + ((double)p.y * q.w - (double)p.w * q.y);
+        } else {
+            acc[0] += (double)p.x * q.x + (double)p.y * q.y;
+            acc[1] += (double)p.x * q.y - (double)p.y * q.x;
         }
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0)
-        for (size_t i = nvec * CW; i < ncomplex; i++) {
-            acc[0] += (double)a[2 * i] * b[2 * i] + (double)a[2 * i + 1] * b[2 * i + 1];
-            acc[1] += (double)a[2 * i] * b[2 * i + 1] - (double)a[2 * i + 1] * b[2 * i];
-        }
+    // no tail: a field holds 12 complex per site, a multiple of the CW complex of a vector
     block_sum<2>(acc, smem);
     if (threadIdx.x == 0) {
         partials[2 * blockIdx.x] = acc[0];
