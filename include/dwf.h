@@ -27,8 +27,12 @@
  *
  * DEVICE field layout (what `field`, `in`, `out` pointers below hold; produced only by
  * dwf_import_spinor, read back only by dwf_export_spinor; size dwf_field_bytes):
- *   half field   complex[s][k][cb]    k = spin*3 + colour (12 complex components), cb = x>>1 the
- *                                     checkerboard site index (x0-pairs fastest), (re, im) adjacent
+ *   half field   pair[s][row][k/2][h][k&1]: row = x1 + L1*(x2 + L2*x3) (a lattice line along x0),
+ *                h = x0>>1 (cb site x>>1 = row*Lh + h), 12 slots k of two reals per site, slots
+ *                2j and 2j+1 adjacent (one 128-bit vector in fp32).
+ *                fp64: slot k = spin*3 + colour = the complex number (re, im).
+ *                fp32: slot k = 4*colour + t = one real part of a pair of spins, t = 0 (re of
+ *                spins 0,1), 1 (im of 0,1), 2 (re of 2,3), 3 (im of 2,3).
  *   full field   the even half field followed by the odd half field
  *   "SoA complex components, site-fastest" (north_star subsystem 1).  s is the SLOWEST index: the
  *   fast kernel keeps the 8 links of a 4D site in registers and walks through all Ls slices, so

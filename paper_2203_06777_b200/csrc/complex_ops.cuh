@@ -1,12 +1,11 @@
 // complex_ops.cuh -- complex arithmetic on (re, im) register pairs for the Dhop kernels.
 //
-// fp32: every complex add / multiply-accumulate is written with the packed f32x2 PTX
-// instructions of sm_100 (add/mul/fma.rn.f32x2 -> SASS FADD2 / FMUL2 / FFMA2).  A complex number
-// is one 64-bit register pair (re, im); FFMA2 takes a 32-bit register broadcast to both halves,
-// per-half negation and a HI/LO swap as free operand modifiers, so
-//     acc += u * h   =   FFMA2 acc, u.re, (h.re, h.im), acc ;  FFMA2 acc, u.im, (-h.im, h.re), acc
-// is two instructions instead of four scalar FFMAs.  Each lane is an IEEE round-to-nearest fma,
-// so the results are the ones scalar fmaf would give.
+// fp32: the packed f32x2 PTX instructions of sm_100 (add/mul/fma.rn.f32x2 -> SASS FADD2 / FMUL2 /
+// FFMA2) on 64-bit register pairs.  FFMA2 takes a 32-bit register broadcast to both halves and a
+// HI/LO swap as free operand modifiers, FADD2 also a per-half negation.  The direct kernel
+// (dhop.cu) keeps a complex number (re, im) in a pair; the staged kernel (dhop_staged.cu) keeps
+// one real part of two spin components in a pair.  Each lane is an IEEE round-to-nearest
+// operation, so the results are the ones scalar fmaf / + / * would give.
 // fp64: plain DFMA / DADD on double2.
 #pragma once
 #include <cuda_runtime.h>

@@ -1,34 +1,35 @@
-// dhop_staged.cu -- the fast fp32 Dhop kernel for sm_100a: link-stationary, TMA-staged.
+// dhop_staged.cu -- the fast fp32 Dhop kernel for sm_100a: link-stationary, TMA-staged, warp-specialised.
 //
 //   Dhop psi(x,s) = sum_mu [ (1-gamma_mu) U_mu(x) psi(x+mu,s) + (1+gamma_mu) U_mu^dag(x-mu) psi(x-mu,s) ]
 //
 // Work decomposition (hot path rows a2-a6 of SURVEY.md section 8):
 //   * A CTA owns a box of B1 x B2 x B3 "x0-rows" of output sites (a row = the Lh sites of the
 //     output parity on one lattice line along x0) and a contiguous range of s slices (all Ls of
-//     them unless the "ssplit" option shares a tile between CTAs).  One thread = one output 4D
-//     site.  It loads its 8 links (U_mu(x) and the pre-daggered U_mu^dag(x-mu), 72 complex) ONCE
-//     into registers and keeps them there while it walks through its slices: each link crosses
-//     the L1 data pipe once per 4D site instead of once per 5D site.  The links of the NEXT tile
-//     are fetched leg by leg during the last slice of the current tile, each leg's registers
-//     being refilled right after their last use, so the tile switch does not expose the loads.
+//     them unless the "ssplit" option shares a tile between CTAs).  One CONSUMER thread = one
+//     output 4D site.  It loads its 8 links (U_mu(x) and the pre-daggered U_mu^dag(x-mu), 72
+//     complex) ONCE into registers and keeps them there while it walks through its slices: each
+//     link crosses the L1 data pipe once per 4D site instead of once per 5D site.  The links of
+//     the NEXT tile are fetched leg by leg during the last slice of the current tile, each leg's
+//     registers being refilled right after their last use.
 //   * For every s the input slice needed by the tile -- the rows box itself plus its six faces
 //     (the x0 direction closes periodically inside a row, so it has no halo) -- is brought into
-//     shared memory by 5-D bulk tensor copies (TMA, cp.async.bulk.tensor) issued by one thread,
-//     two slices deep, completion signalled through mbarriers.  Periodic wrap is a coordinate
-//     computed modulo the extent: every face is its own box.  The copies are issued per x3 layer
-//     and carry L2 eviction priorities: tiles are swept in ascending x3, so the layers the next
-//     sweep step will need again (top layer of the box, x3+ face) are marked evict_last, the x3-
-//     face (its last use) and the streamed links / output evict_first.  That keeps the
-//     inter-generation halo re-reads of the persistent grid in L2 instead of HBM.
-//   * Per leg a thread reads the neighbour spinor with 12 LDS.64 at (per-leg base register +
-//     immediate), projects to a half spinor, multiplies with the register-resident link,
-//     reconstructs and accumulates; after the 8 legs it stores 12 complex.
-//     All complex arithmetic is packed f32x2 (FFMA2 / FADD2): u*h is accumulated as two chains
-//     A = sum u.re*h and B = sum u.im*h, combined once as A + iB, so that no operand needs a
-//     half-negated copy.
-// Global layouts: spinor complex[s][row][k/2][h][k&1], links complex[row][f/2][h][f&1] (pack.cu):
-// two components of a site form one 128-bit vector, so every LDS / LDG / STG is 128 bits wide.
-// Shared-memory image of one slice: [row of the staged region][k/2][Lh][k&1] complex,
+//     a two-stage shared-memory ring by 5-D bulk tensor copies (TMA, cp.async.bulk.tensor).
+//     Periodic wrap is a coordinate computed modulo the extent: every face is its own box.
+//   * Warp specialisation: the first warpgroup is the PRODUCER.  It gives its registers back
+//     (setmaxnreg.dec), the consumer warpgroups take them (setmaxnreg.inc), and one producer
+//     thread issues all copies.  A stage is four regions -- x3 faces, x2 faces, x1 faces, centre --
+//     each with a "full" mbarrier (TMA transaction count) and an "empty" mbarrier (one arrival
+//     per consumer warp).  Consumers run the legs in the order x3, x2, x1, x0 and release a face
+//     region right after the two legs that read it, so its refill has almost two steps to land.
+//     There is no CTA-wide barrier after the prologue.
+//   * The copies carry L2 eviction priorities (option "l2pol") and are issued per x3 layer
+//     (option "layered") so that layers can differ; links and output are evict_first.
+//   * Arithmetic: see "arithmetic on spin pairs" below -- all packed f32x2 (FFMA2 / FMUL2 / FADD2),
+//     54 instructions per leg, 12 accumulators that are stored as they are.
+// Global layouts (pack.cu): spinor pair[s][row][k/2][h][k&1] with slot k = 4*colour + t holding one
+// real part of a pair of spins; links complex[row][f/2][h][f&1]: two slots of a site form one
+// 128-bit vector, so every LDS / LDG / STG is 128 bits wide.
+// Shared-memory image of one slice: [row of the staged region][k/2][Lh][k&1],
 // regions in the order centre, x1-, x1+, x2-, x2+, x3-, x3+; inside a region x3 layer slowest.
 #include <type_traits>
 #include <vector>
