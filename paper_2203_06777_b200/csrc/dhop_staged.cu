@@ -376,13 +376,16 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     const int r2m = (i2 > 0) ? rc - B1 : Cfg::R_X2M + i1 + B1 * i3;
     const int r3p = (i3 + 1 < B3) ? rc + B1 * B2 : Cfg::R_X3P + i1 + B1 * i2;
     const int r3m = (i3 > 0) ? rc - B1 * B2 : Cfg::R_X3M + i1 + B1 * i2;
-    uint32_t off[8];            // byte offsets of the 8 neighbour spinors inside a stage
-    off[2] = r1p * Cfg::ROWB + h * 16;
-    off[3] = r1m * Cfg::ROWB + h * 16;
-    off[4] = r2p * Cfg::ROWB + h * 16;
-    off[5] = r2m * Cfg::ROWB + h * 16;
-    off[6] = r3p * Cfg::ROWB + h * 16;
-    off[7] = r3m * Cfg::ROWB + h * 16;
+    // Offsets of the 8 neighbour spinors inside a stage, in 16-byte units, two per register.  They
+    // are made opaque to the compiler (empty asm) so that it keeps the four registers instead of
+    // recomputing every offset from the thread index at the head of every leg.
+    constexpr uint32_t ROWV = Cfg::ROWB / 16;
+    uint32_t offp[4];
+    offp[1] = (r1p * ROWV + h) | ((r1m * ROWV + h) << 16);
+    offp[2] = (r2p * ROWV + h) | ((r2m * ROWV + h) << 16);
+    offp[3] = (r3p * ROWV + h) | ((r3m * ROWV + h) << 16);
+    asm volatile("" : "+r"(offp[1]), "+r"(offp[2]), "+r"(offp[3]));
+    static_assert(Cfg::NROW_IN * (Cfg::ROWB / 16) < 65536, "stage offsets must fit 16 bits");
 
     // global row of this thread's site in the it-th tile, and the parity bit r of x0 = 2h + r
     auto tile_row = [&](int it, int &r) -> long long {
@@ -394,8 +397,8 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     auto set_x0_offsets = [&](int r) {
         int hp = h + r;       if (hp == LH) hp = 0;
         int hm = h - 1 + r;   if (hm < 0) hm = LH - 1;
-        off[0] = rc * Cfg::ROWB + hp * 16;
-        off[1] = rc * Cfg::ROWB + hm * 16;
+        offp[0] = (rc * ROWV + hp) | ((rc * ROWV + hm) << 16);
+        asm volatile("" : "+r"(offp[0]));
     };
 
     const long long slice_vecs = 6LL * LH * args.L1 * args.L2 * args.L3;   // 128-bit vectors per slice
@@ -426,7 +429,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         const bool legs = !(args.ablate & 4);
         float2 acc[12];
 #define DWF_LEG(L, MU, FWD, FIRST)                                                                  \
-        staged_leg<LH, MU, FWD, FIRST, DWF_ABL>(acc, reinterpret_cast<const float4 *>(sb + off[L]), U + 9 * (L)); \
+        staged_leg<LH, MU, FWD, FIRST, DWF_ABL>(acc, reinterpret_cast<const float4 *>(sb) + (((L) & 1) ? offp[(L) >> 1] >> 16 : offp[(L) >> 1] & 0xffffu), U + 9 * (L)); \
         if constexpr (FETCH && REFILL_PER_LEG) {   /* refill the component pairs whose last use was this leg */ \
             _Pragma("unroll") for (int j = (9 * (L)) / 2; j < (9 * ((L) + 1)) / 2; j++) {            \
                 const float4 q = ldg128_hint(gnext + j * LH, pol_g);                                \
