@@ -102,6 +102,15 @@ template <int LH, int B1, int B2, int B3> struct StagedCfg {
     static_assert(ROWB % 128 == 0, "staged rows must keep TMA destinations 128-byte aligned");
 };
 
+// Where the consumers synchronise with the producer inside a step:
+//   0: wait for a region right before its two legs, release it right after them
+//   1: wait for the whole stage at the top, release the face regions early (default: the waits are
+//      compiler barriers for memory operations, so mode 0 keeps ptxas from hoisting the LDS of the
+//      next leg pair over them and exposes the LDS latency four times per step)
+//   2: wait at the top, release everything at the end
+#ifndef DWF_SYNC_MODE
+#define DWF_SYNC_MODE 1
+#endif
 #ifndef DWF_REFILL_PER_LEG
 #define DWF_REFILL_PER_LEG 1   // 1: refill a leg's links right after the leg (last slice of a tile); 0: all after the last leg
 #endif
@@ -283,7 +292,6 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         const int pfd = args.prefetch & 15, pfm = args.prefetch >> 4;
         for (int g = 0; g < nsteps; g++) {
             const int stage = g & 1;
-            const uint32_t bar = full_base + 8 * stage;
             if (pfd && g + pfd < nsteps && !(args.ablate & 8)) {       // DRAM -> L2 runs ahead of the shared-memory ring
                 const Boxes p = boxes(g + pfd);
                 if (pfm & 1) tma_prefetch_5d(&map_c, 0, 0, p.o1, p.o2, p.c4);
@@ -440,6 +448,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
 #define DWF_RELEASE(R)                                                                              \
         __syncwarp();                                                                               \
         if ((ctid & 31) == 0) mbar_arrive(eb + 8 * (R));
+#if DWF_SYNC_MODE == 0          /* wait for a region right before its legs, release it right after */
         mbar_wait(fb + 24, par);
         mbar_wait(fb, par);
         if (legs) {
@@ -464,6 +473,37 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             DWF_LEG(1, 0, false, false)
         }
         DWF_RELEASE(3)
+#else                           /* wait for the whole stage first: the legs form one block the compiler may software-pipeline */
+        mbar_wait(fb + 24, par);
+        mbar_wait(fb, par);
+        mbar_wait(fb + 8, par);
+        mbar_wait(fb + 16, par);
+        if (legs) {
+            DWF_LEG(6, 3, true,  true)
+            DWF_LEG(7, 3, false, false)
+#if DWF_SYNC_MODE == 1
+            DWF_RELEASE(0)
+#endif
+            DWF_LEG(4, 2, true,  false)
+            DWF_LEG(5, 2, false, false)
+#if DWF_SYNC_MODE == 1
+            DWF_RELEASE(1)
+#endif
+            DWF_LEG(2, 1, true,  false)
+            DWF_LEG(3, 1, false, false)
+#if DWF_SYNC_MODE == 1
+            DWF_RELEASE(2)
+#endif
+            DWF_LEG(0, 0, true,  false)
+            DWF_LEG(1, 0, false, false)
+        }
+#if DWF_SYNC_MODE == 1
+        if (!legs) { DWF_RELEASE(0) DWF_RELEASE(1) DWF_RELEASE(2) }
+        DWF_RELEASE(3)
+#else
+        DWF_RELEASE(0) DWF_RELEASE(1) DWF_RELEASE(2) DWF_RELEASE(3)
+#endif
+#endif
 #undef DWF_LEG
 #undef DWF_RELEASE
         // Last slice of the tile: refill the links for the next tile, all at once and in the
