@@ -448,6 +448,10 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
 #define DWF_RELEASE(R)                                                                              \
         __syncwarp();                                                                               \
         if ((ctid & 31) == 0) mbar_arrive(eb + 8 * (R));
+        // early release of a face region: ordered after its loads through the accumulators, no
+        // memory clobber (the legs of a step run converged: a lane's loads are part of one warp LDS)
+#define DWF_RELEASE_DEP(R)                                                                          \
+        if ((ctid & 31) == 0) mbar_arrive_after(eb + 8 * (R), acc);
 #if DWF_SYNC_MODE == 0          /* wait for a region right before its legs, release it right after */
         mbar_wait(fb + 24, par);
         mbar_wait(fb, par);
@@ -482,17 +486,17 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             DWF_LEG(6, 3, true,  true)
             DWF_LEG(7, 3, false, false)
 #if DWF_SYNC_MODE == 1
-            DWF_RELEASE(0)
+            DWF_RELEASE_DEP(0)
 #endif
             DWF_LEG(4, 2, true,  false)
             DWF_LEG(5, 2, false, false)
 #if DWF_SYNC_MODE == 1
-            DWF_RELEASE(1)
+            DWF_RELEASE_DEP(1)
 #endif
             DWF_LEG(2, 1, true,  false)
             DWF_LEG(3, 1, false, false)
 #if DWF_SYNC_MODE == 1
-            DWF_RELEASE(2)
+            DWF_RELEASE_DEP(2)
 #endif
             DWF_LEG(0, 0, true,  false)
             DWF_LEG(1, 0, false, false)
@@ -506,6 +510,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
 #endif
 #undef DWF_LEG
 #undef DWF_RELEASE
+#undef DWF_RELEASE_DEP
         // Last slice of the tile: refill the links for the next tile, all at once and in the
         // order the next step uses them (legs 6, 7, 4, 5, 2, 3, 0, 1).  Spreading the loads over
         // the legs of this step made later legs wait on the scoreboard the loads share.
