@@ -260,7 +260,8 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         tma_prefetch_desc(&map_x1l);
         tma_prefetch_desc(&map_x2l);
         for (int i = 0; i < 2 * Cfg::NREG; i++) {
-            mbar_init(full_base + 8 * i, 1);
+            // modes 1, 2: one full barrier per stage collects the four regions (four arrivals)
+            mbar_init(full_base + 8 * i, DWF_SYNC_MODE == 0 ? 1 : Cfg::NREG);
             mbar_init(empty_base + 8 * i, Cfg::NWARP_C);
         }
         mbar_fence_init();
@@ -307,6 +308,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             const Boxes b = boxes(g);
             const uint32_t dst = smem_base + stage * Cfg::STAGE_BYTES;
             const uint32_t fb = full_base + 32 * stage, eb = empty_base + 32 * stage;
+            constexpr uint32_t FS = DWF_SYNC_MODE == 0 ? 8 : 0;      // stride of the per-region full barriers
             const uint32_t epar = ((g >> 1) - 1) & 1;
             const bool notma = args.ablate & 8, no12 = args.ablate & 32, no3 = args.ablate & 16;   // timing experiments
             // regions in the order the consumers release them (x3 faces, x2 faces, x1 faces, centre)
@@ -318,48 +320,48 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
                 tma_load_5d_hint(dst + Cfg::R_X3P * Cfg::ROWB, &map_x3, fb, 0, 0, b.o1, b.o2, b.c3p, pol[PC_X3P]);
             }
             if (g >= 2) mbar_wait(eb + 8, epar);
-            if (notma || no12) mbar_arrive(fb + 8);
+            if (notma || no12) mbar_arrive(fb + 1 * FS);
             else {
-                mbar_arrive_expect_tx(fb + 8, 2 * B1 * B3 * Cfg::ROWB);
+                mbar_arrive_expect_tx(fb + 1 * FS, 2 * B1 * B3 * Cfg::ROWB);
                 if (args.layered) {
 #pragma unroll
                     for (int j = 0; j < B3; j++) {
                         const uint64_t pf = pol[j == B3 - 1 ? PC_X12_TOP : PC_X12];
-                        tma_load_5d_hint(dst + (Cfg::R_X2M + j * B1) * Cfg::ROWB, &map_x2l, fb + 8, 0, 0, b.o1, b.x2m, b.c4 + j, pf);
-                        tma_load_5d_hint(dst + (Cfg::R_X2P + j * B1) * Cfg::ROWB, &map_x2l, fb + 8, 0, 0, b.o1, b.x2p, b.c4 + j, pf);
+                        tma_load_5d_hint(dst + (Cfg::R_X2M + j * B1) * Cfg::ROWB, &map_x2l, fb + 1 * FS, 0, 0, b.o1, b.x2m, b.c4 + j, pf);
+                        tma_load_5d_hint(dst + (Cfg::R_X2P + j * B1) * Cfg::ROWB, &map_x2l, fb + 1 * FS, 0, 0, b.o1, b.x2p, b.c4 + j, pf);
                     }
                 } else {
-                    tma_load_5d_hint(dst + Cfg::R_X2M * Cfg::ROWB, &map_x2, fb + 8, 0, 0, b.o1, b.x2m, b.c4, pol[PC_X12]);
-                    tma_load_5d_hint(dst + Cfg::R_X2P * Cfg::ROWB, &map_x2, fb + 8, 0, 0, b.o1, b.x2p, b.c4, pol[PC_X12]);
+                    tma_load_5d_hint(dst + Cfg::R_X2M * Cfg::ROWB, &map_x2, fb + 1 * FS, 0, 0, b.o1, b.x2m, b.c4, pol[PC_X12]);
+                    tma_load_5d_hint(dst + Cfg::R_X2P * Cfg::ROWB, &map_x2, fb + 1 * FS, 0, 0, b.o1, b.x2p, b.c4, pol[PC_X12]);
                 }
             }
             if (g >= 2) mbar_wait(eb + 16, epar);
-            if (notma || no12) mbar_arrive(fb + 16);
+            if (notma || no12) mbar_arrive(fb + 2 * FS);
             else {
-                mbar_arrive_expect_tx(fb + 16, 2 * B2 * B3 * Cfg::ROWB);
+                mbar_arrive_expect_tx(fb + 2 * FS, 2 * B2 * B3 * Cfg::ROWB);
                 if (args.layered) {
 #pragma unroll
                     for (int j = 0; j < B3; j++) {
                         const uint64_t pf = pol[j == B3 - 1 ? PC_X12_TOP : PC_X12];
-                        tma_load_5d_hint(dst + (Cfg::R_X1M + j * B2) * Cfg::ROWB, &map_x1l, fb + 16, 0, 0, b.x1m, b.o2, b.c4 + j, pf);
-                        tma_load_5d_hint(dst + (Cfg::R_X1P + j * B2) * Cfg::ROWB, &map_x1l, fb + 16, 0, 0, b.x1p, b.o2, b.c4 + j, pf);
+                        tma_load_5d_hint(dst + (Cfg::R_X1M + j * B2) * Cfg::ROWB, &map_x1l, fb + 2 * FS, 0, 0, b.x1m, b.o2, b.c4 + j, pf);
+                        tma_load_5d_hint(dst + (Cfg::R_X1P + j * B2) * Cfg::ROWB, &map_x1l, fb + 2 * FS, 0, 0, b.x1p, b.o2, b.c4 + j, pf);
                     }
                 } else {
-                    tma_load_5d_hint(dst + Cfg::R_X1M * Cfg::ROWB, &map_x1, fb + 16, 0, 0, b.x1m, b.o2, b.c4, pol[PC_X12]);
-                    tma_load_5d_hint(dst + Cfg::R_X1P * Cfg::ROWB, &map_x1, fb + 16, 0, 0, b.x1p, b.o2, b.c4, pol[PC_X12]);
+                    tma_load_5d_hint(dst + Cfg::R_X1M * Cfg::ROWB, &map_x1, fb + 2 * FS, 0, 0, b.x1m, b.o2, b.c4, pol[PC_X12]);
+                    tma_load_5d_hint(dst + Cfg::R_X1P * Cfg::ROWB, &map_x1, fb + 2 * FS, 0, 0, b.x1p, b.o2, b.c4, pol[PC_X12]);
                 }
             }
             if (g >= 2) mbar_wait(eb + 24, epar);
-            if (notma) mbar_arrive(fb + 24);
+            if (notma) mbar_arrive(fb + 3 * FS);
             else {
-                mbar_arrive_expect_tx(fb + 24, Cfg::NROW_C * Cfg::ROWB);
+                mbar_arrive_expect_tx(fb + 3 * FS, Cfg::NROW_C * Cfg::ROWB);
                 if (args.layered) {
 #pragma unroll
                     for (int j = 0; j < B3; j++)
-                        tma_load_5d_hint(dst + (j * B1 * B2) * Cfg::ROWB, &map_x3, fb + 24, 0, 0, b.o1, b.o2, b.c4 + j,
+                        tma_load_5d_hint(dst + (j * B1 * B2) * Cfg::ROWB, &map_x3, fb + 3 * FS, 0, 0, b.o1, b.o2, b.c4 + j,
                                          pol[j == B3 - 1 ? PC_CENTRE_TOP : PC_CENTRE]);
                 } else {
-                    tma_load_5d_hint(dst, &map_c, fb + 24, 0, 0, b.o1, b.o2, b.c4, pol[PC_CENTRE]);
+                    tma_load_5d_hint(dst, &map_c, fb + 3 * FS, 0, 0, b.o1, b.o2, b.c4, pol[PC_CENTRE]);
                 }
             }
         }
@@ -478,10 +480,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         }
         DWF_RELEASE(3)
 #else                           /* wait for the whole stage first: the legs form one block the compiler may software-pipeline */
-        mbar_wait(fb + 24, par);
         mbar_wait(fb, par);
-        mbar_wait(fb + 8, par);
-        mbar_wait(fb + 16, par);
         if (legs) {
             DWF_LEG(6, 3, true,  true)
             DWF_LEG(7, 3, false, false)
