@@ -222,7 +222,7 @@ def run_reference(args, w):
 # ---------------------------------------------------------------------------------------------
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
 # `ncu --set full` capture summarised under profiles/ (None until a capture exists).
-NCU_TRAFFIC_BYTES = {"c4": 1475084000 + 769487000}   # profiles/r01g_dhop_staged_pairs_kernel_ncu.md, launch 1
+NCU_TRAFFIC_BYTES = {"c4": 1471999000 + 769403000}   # profiles/r01h_dhop_staged_kernel_ncu.md, launch 1
 
 
 def max_over_ranks(x, dist=None, device="cuda"):
