@@ -117,9 +117,21 @@ DWF_API int dwf_export_spinor(const dwf_geometry *g, const void *field_dev, int 
 /* Number of kernel launches this library has issued since it was loaded (all threads). */
 DWF_API unsigned long long dwf_launch_count(void);
 
-/* Tuning knobs for experiments: "kernel" (0 auto, 1 direct L1-cached kernel, 2 TMA-staged kernel),
- * "variant" (staged tile shape, 0 auto), "raster_staged" / "raster" (CTA launch order),
- * "tile0".."tile3", "cpc" (direct kernel tile).  UNSUPPORTED for an unknown key. */
+/* Tuning knobs for experiments; none of them changes a result of the staged kernel by a bit
+ * (tests/test_gpu_staged.py).  UNSUPPORTED for an unknown key, INVALID_ARG for a bad value.
+ *   "kernel"         0 auto, 1 direct (L1-cached) kernel, 2 TMA-staged kernel (error if it has no
+ *                    variant for the geometry: fp32, Lh = 4, 8, 16 or 24, box extents dividing L1..L3)
+ *   "variant"        staged tile shape: 0 auto, n > 0 the n-th compiled (Lh, B1, B2, B3) instance
+ *   "raster_staged"  launch order of the staged tiles, 10 * order + log2(macro blocks) (dhop_staged.cu); -1 auto
+ *   "zigzag"         1: every other tile walks its s slices backwards (L2 reuse between tiles)
+ *   "ssplit"         CTAs sharing one tile, each taking Ls / ssplit slices
+ *   "layered"        1: one TMA box per x3 layer, so that L2 policies can differ per layer
+ *   "l2pol"          decimal digits, one L2 eviction class per access type (dhop_staged.cu PC_*):
+ *                    0 evict_normal, 1 evict_first, 2 evict_last
+ *   "prefetch"       low 4 bits: L2 prefetch distance in steps (0 off), higher bits: box mask
+ *   "l2persist"      MB of L2 set aside for evict_last lines (device-wide CUDA limit)
+ *   "ablate"         timing experiments that give WRONG results (skip loads / legs / stores); 0 = off
+ *   "raster", "tile0".."tile3", "cpc"   direct kernel: CTA launch order, log2 tile extents, slices per CTA */
 DWF_API int dwf_set_option(dwf_geometry *g, const char *key, long long value);
 
 DWF_API const char *dwf_error_string(int code);

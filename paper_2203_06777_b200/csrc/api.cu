@@ -108,7 +108,15 @@ int rebuild_tilings(dwf_geometry *g)
     plan_staged(g);
     if (g->staged.variant >= 0) {
         std::vector<int4> st((size_t)g->staged.ntiles);
-        build_staged_tile_table(g, g->opt_raster_staged, st.data());
+        int raster = g->opt_raster_staged;
+        if (raster < 0) {
+            // auto: x1 fastest, x3 slowest, direction 2 split until a macro block has at most 96 tile
+            // columns per x3 layer (C4: 128 -> 64, C5: 576 -> 72; measured optimum on both)
+            const int n1 = g->lat.L[1] / g->staged.b[0], n2 = g->lat.L[2] / g->staged.b[1];
+            raster = 0;
+            while (raster < 9 && n1 * (n2 >> raster) > 96 && (n2 % (2 << raster)) == 0) raster++;
+        }
+        build_staged_tile_table(g, raster, st.data());
         DWF_CUDA_CHECK(cudaMalloc(&g->tiles_staged, st.size() * sizeof(int4)));
         DWF_CUDA_CHECK(cudaMemcpy(g->tiles_staged, st.data(), st.size() * sizeof(int4), cudaMemcpyHostToDevice));
     }
@@ -194,7 +202,7 @@ int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, i
     g->opt_tile[0] = 4; g->opt_tile[1] = 2; g->opt_tile[2] = 1; g->opt_tile[3] = 1;
     g->opt_cpc = 1;
     g->opt_raster = 2;
-    g->opt_raster_staged = 1;
+    g->opt_raster_staged = -1;   // auto
     g->opt_variant = 0;
     g->opt_kernel = 0;
     g->opt_l2pol = 11222222;     // out, links evict_first; every input box evict_last (sweeps: least DRAM re-reads)

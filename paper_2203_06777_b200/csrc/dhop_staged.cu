@@ -584,6 +584,7 @@ static const std::vector<Variant> &variants()
         make_variant<24, 2, 2, 2>(), make_variant<24, 2, 2, 1>(),
         make_variant<4, 4, 4, 4>(),  make_variant<4, 2, 2, 2>(),  make_variant<4, 2, 2, 1>(),
         make_variant<16, 2, 2, 4>(), make_variant<16, 2, 4, 2>(), make_variant<16, 8, 2, 1>(), make_variant<16, 1, 2, 8>(),
+        make_variant<24, 3, 1, 3>(), make_variant<24, 1, 3, 3>(), make_variant<24, 3, 3, 1>(),
     };
     return v;
 }
