@@ -98,6 +98,15 @@ DWF_API int dwf_dhop_eo(const dwf_geometry *g, const void *in_odd, void *out_eve
 DWF_API int dwf_norm2(const dwf_geometry *g, const void *field, int parity, double *result_host,
               void *stream);
 
+/* DhopOE / DhopEO fused with the norm2 of their result (SURVEY.md 8(a) rows a6 + a7 in one pass):
+ * out = D in and *result_host = sum |out|^2, fp64 accumulation in a fixed order (deterministic
+ * for a given geometry and option set; it differs from dwf_norm2(out) only in summation order,
+ * relative difference <= 1e-12).  The fast fp32 kernel accumulates in its epilogue, so the
+ * output field is not read again; other geometries run the two passes.  Arguments and errors
+ * as dwf_dhop_oe / dwf_dhop_eo; synchronises `stream` like dwf_norm2. */
+DWF_API int dwf_dhop_oe_norm2(const dwf_geometry *g, const void *in_even, void *out_odd, double *result_host, void *stream);
+DWF_API int dwf_dhop_eo_norm2(const dwf_geometry *g, const void *in_odd, void *out_even, double *result_host, void *stream);
+
 /* result_host[0..1] = (re, im) of sum conj(a) b.  Same rules as dwf_norm2. */
 DWF_API int dwf_inner_product(const dwf_geometry *g, const void *a, const void *b, int parity,
                       double result_host[2], void *stream);

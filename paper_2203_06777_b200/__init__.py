@@ -25,7 +25,7 @@ LIB_PATH = os.path.join(_HERE, "libdwf.so")
 # every symbol include/dwf.h declares (tests check that the library exports all of them)
 SYMBOLS = (
     "dwf_create_geometry", "dwf_destroy_geometry", "dwf_load_gauge", "dwf_dhop", "dwf_dhop_oe",
-    "dwf_dhop_eo", "dwf_norm2", "dwf_inner_product", "dwf_field_bytes",
+    "dwf_dhop_eo", "dwf_dhop_oe_norm2", "dwf_dhop_eo_norm2", "dwf_norm2", "dwf_inner_product", "dwf_field_bytes",
     "dwf_import_spinor", "dwf_export_spinor", "dwf_launch_count", "dwf_set_option",
     "dwf_error_string", "dwf_last_error",
 )
@@ -58,6 +58,8 @@ def load(build_if_missing: bool = True):
     for f in (lib.dwf_dhop, lib.dwf_dhop_oe, lib.dwf_dhop_eo):
         f.argtypes = [vp, vp, vp, vp]
     lib.dwf_norm2.argtypes = [vp, vp, ci, ctypes.POINTER(ctypes.c_double), vp]
+    for f in (lib.dwf_dhop_oe_norm2, lib.dwf_dhop_eo_norm2):
+        f.argtypes = [vp, vp, vp, ctypes.POINTER(ctypes.c_double), vp]
     lib.dwf_inner_product.argtypes = [vp, vp, vp, ci, ctypes.POINTER(ctypes.c_double), vp]
     lib.dwf_field_bytes.argtypes = [vp, ci]
     lib.dwf_field_bytes.restype = cs
@@ -138,6 +140,20 @@ def dwf_dhop_oe(g: int, in_even, out_odd, stream=None) -> None:
 
 def dwf_dhop_eo(g: int, in_odd, out_even, stream=None) -> None:
     _check(load().dwf_dhop_eo(g, _dev_ptr(in_odd), _dev_ptr(out_even), _stream(stream)), "dwf_dhop_eo")
+
+
+def dwf_dhop_oe_norm2(g: int, in_even, out_odd, stream=None) -> float:
+    r = ctypes.c_double()
+    _check(load().dwf_dhop_oe_norm2(g, _dev_ptr(in_even), _dev_ptr(out_odd), ctypes.byref(r), _stream(stream)),
+           "dwf_dhop_oe_norm2")
+    return r.value
+
+
+def dwf_dhop_eo_norm2(g: int, in_odd, out_even, stream=None) -> float:
+    r = ctypes.c_double()
+    _check(load().dwf_dhop_eo_norm2(g, _dev_ptr(in_odd), _dev_ptr(out_even), ctypes.byref(r), _stream(stream)),
+           "dwf_dhop_eo_norm2")
+    return r.value
 
 
 def dwf_norm2(g: int, field, parity: int = FULL, stream=None) -> float:
@@ -252,6 +268,16 @@ class Geometry:
         out = self.new_field(EVEN) if out is None else out
         dwf_dhop_eo(self.handle, in_odd, out, stream)
         return out
+
+    def dhop_oe_norm2(self, in_even, out=None, stream=None):
+        """DhopOE fused with norm2 of its result: returns (out_odd, norm2)."""
+        out = self.new_field(ODD) if out is None else out
+        return out, dwf_dhop_oe_norm2(self.handle, in_even, out, stream)
+
+    def dhop_eo_norm2(self, in_odd, out=None, stream=None):
+        """DhopEO fused with norm2 of its result: returns (out_even, norm2)."""
+        out = self.new_field(EVEN) if out is None else out
+        return out, dwf_dhop_eo_norm2(self.handle, in_odd, out, stream)
 
     def norm2(self, field, parity: int = FULL, stream=None) -> float:
         return dwf_norm2(self.handle, field, parity, stream)

@@ -369,6 +369,50 @@ int dwf_dhop_eo(const dwf_geometry *g, const void *in_odd, void *out_even, void 
     return dhop_common(g, in_odd, out_even, DWF_EVEN, stream, "dwf_dhop_eo");
 }
 
+// out = D in on half fields and *result_host = norm2(out): the reduction runs in the epilogue of the
+// Dhop kernel (staged path) or as a second pass over `out` (direct path)
+static int dhop_norm2_common(const dwf_geometry *g, const void *in, void *out, int parity_out, double *result_host,
+                             void *stream, const char *who)
+{
+    if (!g || !in || !out || !result_host) { set_error("%s: NULL argument", who); return DWF_ERR_INVALID_ARG; }
+    if (in == out) { set_error("%s: in-place application is not defined (in == out)", who); return DWF_ERR_INVALID_ARG; }
+    if (!aligned16(in) || !aligned16(out)) { set_error("%s: field pointers must be 16-byte aligned", who); return DWF_ERR_INVALID_ARG; }
+    if (!g->gauge_loaded) { set_error("%s: call dwf_load_gauge first", who); return DWF_ERR_NO_GAUGE; }
+    DeviceGuard guard(g->device);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const bool staged_ok = g->staged.variant >= 0;
+    if (g->opt_kernel == 2 && !staged_ok) {
+        set_error("the staged kernel does not support this geometry / precision");
+        return DWF_ERR_UNSUPPORTED;
+    }
+    int rc;
+    if (staged_ok && g->opt_kernel != 1) {
+        int nblocks = 0;
+        rc = launch_dhop_staged(g, in, out, parity_out, st, g->partials, &nblocks);
+        if (rc) return rc;
+        rc = launch_final_sum(g, nblocks, st);
+    } else {
+        rc = launch_dhop_direct(g, in, out, parity_out, st);
+        if (rc) return rc;
+        rc = launch_norm2(g, out, dwf_field_bytes(g, parity_out) / (size_t)g->prec, st);
+    }
+    if (rc) return rc;
+    double r = 0;
+    DWF_CUDA_CHECK(cudaMemcpyAsync(&r, g->result_dev, sizeof(double), cudaMemcpyDeviceToHost, st));
+    DWF_CUDA_CHECK(cudaStreamSynchronize(st));
+    *result_host = r;
+    return DWF_OK;
+}
+
+int dwf_dhop_oe_norm2(const dwf_geometry *g, const void *in_even, void *out_odd, double *result_host, void *stream)
+{
+    return dhop_norm2_common(g, in_even, out_odd, DWF_ODD, result_host, stream, "dwf_dhop_oe_norm2");
+}
+int dwf_dhop_eo_norm2(const dwf_geometry *g, const void *in_odd, void *out_even, double *result_host, void *stream)
+{
+    return dhop_norm2_common(g, in_odd, out_even, DWF_EVEN, result_host, stream, "dwf_dhop_eo_norm2");
+}
+
 int dwf_norm2(const dwf_geometry *g, const void *field, int parity, double *result_host, void *stream)
 {
     if (!g || !field || !result_host || !parity_ok(parity)) { set_error("dwf_norm2: bad argument"); return DWF_ERR_INVALID_ARG; }

@@ -71,6 +71,7 @@ struct StagedArgs {
     int zigzag;              // walk the slices of every other tile backwards
     int layered;             // one TMA box per x3 layer (per-layer L2 policies) instead of one per region
     int prefetch;            // producer prefetches the input of step g + prefetch into L2 (0: off); bit 4..: box mask
+    double *norm_partials;   // NORM kernels: one partial sum of |out|^2 per CTA (fixed order inside the CTA)
     int ablate;              // timing experiments only (wrong results): 1 no link refill, 2 no stores, 4 no legs, 8 no TMA
 };
 
@@ -92,7 +93,8 @@ template <int LH, int B1, int B2, int B3> struct StagedCfg {
     static constexpr int NREG = 4;
     // tail: full[2][4], empty[2][4] mbarriers (128 B), 6 L2 policies (48 B), origins
     static constexpr int TAIL_POL = 128, TAIL_ORIG = 176;
-    static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + TAIL_ORIG + NORIG * 16;
+    static constexpr int TAIL_NORM = TAIL_ORIG + NORIG * 16;    // one fp64 partial per consumer warp (fused norm2)
+    static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + TAIL_NORM + 8 * NWARP_C;
     // small tiles run two CTAs per SM
     static constexpr int CTAS_PER_SM = (NTC <= 128 && 2 * (SMEM_BYTES + 1024) <= 232448) ? 2 : 1;
     // register split (setmaxnreg): the producer warpgroup keeps PROD_REGS, the consumers take the rest
@@ -221,7 +223,9 @@ __device__ __forceinline__ void staged_leg(float2 (&acc)[12], const float4 *__re
     }
 }
 
-template <int LH, int B1, int B2, int B3>
+// NORM: also accumulate |out|^2 (fp64, fixed order) and write one partial per CTA -- norm2 of the
+// result fused into the kernel that produces it (saves re-reading the output field).
+template <int LH, int B1, int B2, int B3, bool NORM>
 __global__ void __launch_bounds__(StagedCfg<LH, B1, B2, B3>::NT, StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM)
 dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_x1,
                    const __grid_constant__ CUtensorMap map_x2, const __grid_constant__ CUtensorMap map_x3,
@@ -242,7 +246,10 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     const int s_first = ((int)blockIdx.x % args.ssplit) * nsl;
     const int my_tiles = (args.ntiles - group + ngroup - 1) / ngroup;
     const int nsteps = my_tiles * nsl;
-    if (nsteps <= 0) return;
+    if (nsteps <= 0) {
+        if (NORM && tid == 0) args.norm_partials[blockIdx.x] = 0.0;
+        return;
+    }
     // L2 policies of the TMA copies, read by the producer thread from shared memory
     uint64_t *pol = reinterpret_cast<uint64_t *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + Cfg::TAIL_POL);
     // origins of this CTA's first NORIG tiles: read once, so that neither the producer nor the
@@ -432,6 +439,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     // the leg that used them last (two code copies, so that the common one carries no loads)
     // Leg order x3, x2, x1, x0: the face regions are handed back to the producer as soon as the
     // two legs reading them are done, so that their refill has almost two steps to land.
+    double nsum = 0.0;          // NORM: this thread's share of |out|^2
     auto step = [&](auto fetch_tag, int stage, uint32_t par, float4 *o, const float4 *gnext) {
         constexpr bool FETCH = decltype(fetch_tag)::value;
         const unsigned char *sb = smem + stage * Cfg::STAGE_BYTES;
@@ -526,6 +534,10 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             }
         }
         if (!legs || !active) return;
+        if constexpr (NORM) {
+#pragma unroll
+            for (int k = 0; k < 12; k++) nsum += (double)acc[k].x * acc[k].x + (double)acc[k].y * acc[k].y;
+        }
         if (!(args.ablate & 2)) {
 #pragma unroll
             for (int j = 0; j < 6; j++)
@@ -558,6 +570,21 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         set_x0_offsets(r_cur);
         optr = reinterpret_cast<float4 *>(args.out) + grow * (6 * LH) + h + (long long)s_first * slice_vecs;
     }
+
+    if constexpr (NORM) {
+        // lanes -> warp (xor butterfly), warps -> CTA in warp order: the same order in every run
+        double v = nsum;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        double *slots = reinterpret_cast<double *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + Cfg::TAIL_NORM);
+        if ((ctid & 31) == 0) slots[ctid >> 5] = v;
+        asm volatile("bar.sync 1, %0;" ::"n"(Cfg::NWARP_C * 32) : "memory");      // consumer warps only
+        if (ctid == 0) {
+            double t = 0.0;
+            for (int w = 0; w < Cfg::NWARP_C; w++) t += slots[w];
+            args.norm_partials[blockIdx.x] = t;
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -566,13 +593,15 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
 struct Variant {
     int lh, b1, b2, b3;
     int smem, threads, ctas_per_sm;
-    const void *fn;
+    const void *fn, *fn_norm;
 };
 
 template <int LH, int B1, int B2, int B3> static Variant make_variant()
 {
     using Cfg = StagedCfg<LH, B1, B2, B3>;
-    return {LH, B1, B2, B3, Cfg::SMEM_BYTES, Cfg::NT, Cfg::CTAS_PER_SM, reinterpret_cast<const void *>(&dhop_staged_kernel<LH, B1, B2, B3>)};
+    return {LH, B1, B2, B3, Cfg::SMEM_BYTES, Cfg::NT, Cfg::CTAS_PER_SM,
+            reinterpret_cast<const void *>(&dhop_staged_kernel<LH, B1, B2, B3, false>),
+            reinterpret_cast<const void *>(&dhop_staged_kernel<LH, B1, B2, B3, true>)};
 }
 
 static const std::vector<Variant> &variants()
@@ -657,7 +686,8 @@ static int encode_map(CUtensorMap *m, const void *base, const Lattice &lat, int 
     return DWF_OK;
 }
 
-int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st)
+int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st,
+                       double *norm_partials, int *norm_blocks)
 {
     const Variant &v = variants()[(size_t)g->staged.variant];
     CUtensorMap mc, m1, m2, m3, m1l, m2l;
@@ -680,20 +710,23 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     a.prefetch = g->opt_prefetch;
     a.layered = g->opt_layered;
     a.ablate = g->opt_ablate;
+    a.norm_partials = norm_partials;
     int ssplit = g->opt_ssplit > 0 ? g->opt_ssplit : 1;
     const int slots = g->sm_count * v.ctas_per_sm;       // co-resident CTAs
     while (ssplit > 1 && (g->lat.Ls % ssplit || slots % ssplit)) ssplit--;
     a.ssplit = ssplit;
-    static thread_local const void *attr_set_for = nullptr;
-    if (attr_set_for != v.fn) {
-        DWF_CUDA_CHECK(cudaFuncSetAttribute(v.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, v.smem));
-        attr_set_for = v.fn;
+    const void *fn = norm_partials ? v.fn_norm : v.fn;
+    static thread_local const void *attr_set_for[2] = {nullptr, nullptr};
+    if (attr_set_for[norm_partials != nullptr] != fn) {
+        DWF_CUDA_CHECK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, v.smem));
+        attr_set_for[norm_partials != nullptr] = fn;
     }
     const int ngroup_max = slots / ssplit;
     const int ngroup = g->staged.ntiles < ngroup_max ? g->staged.ntiles : ngroup_max;
     void *params[] = {&mc, &m1, &m2, &m3, &m1l, &m2l, &a};
-    DWF_CUDA_CHECK(cudaLaunchKernel(v.fn, dim3((unsigned)(ngroup * ssplit)), dim3((unsigned)v.threads), params,
+    DWF_CUDA_CHECK(cudaLaunchKernel(fn, dim3((unsigned)(ngroup * ssplit)), dim3((unsigned)v.threads), params,
                                     (size_t)v.smem, st));
+    if (norm_blocks) *norm_blocks = ngroup * ssplit;
     count_launch();
     return DWF_OK;
 }

@@ -115,9 +115,12 @@ int launch_dhop_direct(const dwf_geometry *g, const void *in, void *out, int par
 // dhop_staged.cu (TMA-staged link-stationary kernel, fp32 half fields)
 void plan_staged(dwf_geometry *g);                      // fills g->staged (variant = -1 if unusable)
 void build_staged_tile_table(const dwf_geometry *g, int raster, int4 *host_table);
-int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st);
+// norm_partials != nullptr: the fused-norm2 kernel writes one partial of |out|^2 per CTA there, *norm_blocks = their number
+int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st,
+                       double *norm_partials = nullptr, int *norm_blocks = nullptr);
 // reduce.cu
 int launch_norm2(const dwf_geometry *g, const void *field, size_t nreal, cudaStream_t st);
+int launch_final_sum(const dwf_geometry *g, int nblocks, cudaStream_t st);   // result_dev[0] = sum of partials[0..nblocks)
 int launch_inner(const dwf_geometry *g, const void *a, const void *b, size_t ncomplex,
                  cudaStream_t st);
 

@@ -131,6 +131,14 @@ int launch_norm2(const dwf_geometry *g, const void *field, size_t nreal, cudaStr
     return DWF_OK;
 }
 
+int launch_final_sum(const dwf_geometry *g, int nblocks, cudaStream_t st)
+{
+    final_sum_kernel<1><<<1, 256, 0, st>>>(g->partials, nblocks, g->result_dev);
+    count_launch();
+    DWF_CUDA_CHECK(cudaGetLastError());
+    return DWF_OK;
+}
+
 int launch_inner(const dwf_geometry *g, const void *a, const void *b, size_t ncomplex, cudaStream_t st)
 {
     const int nb = g->reduce_blocks;

@@ -171,3 +171,29 @@ def test_c5_full_size_sampled(lib):
             s = sample_sites(dims, p_out, 300, 11 + p_out)
             assert np.array_equal(got_h[cb_rows(dims, s)], got[s])
             del got_h
+
+
+@pytest.mark.parametrize("dims,Ls,prec", [((32, 16, 16, 16), 4, 4), ((48, 12, 12, 12), 3, 4), ((8, 8, 8, 8), 8, 8),
+                                          ((12, 6, 2, 4), 5, 4)])
+def test_fused_dhop_norm2(lib, dims, Ls, prec):
+    """dwf_dhop_oe_norm2 / dwf_dhop_eo_norm2: the same output bits as the plain call, and the
+    reduction of the epilogue (staged fp32 kernel) or of the second pass (other geometries) within
+    1e-12 of dwf_norm2 of that output and of the oracle's sum; deterministic."""
+    import torch
+    bc = lib.ANTIPERIODIC_T
+    U = gen.gauge_random(dims, 51, prec=prec)
+    half = gen.spinor_gaussian(gen.volume(dims) // 2, Ls, 51, prec=prec)
+    with lib.Geometry(dims, Ls, prec, bc) as g:
+        g.load_gauge(U)
+        for p_out in (1, 0):
+            fin = g.import_spinor(half, 1 - p_out)
+            plain = g.dhop_oe(fin) if p_out == 1 else g.dhop_eo(fin)
+            fused, n = g.dhop_oe_norm2(fin) if p_out == 1 else g.dhop_eo_norm2(fin)
+            assert torch.equal(fused, plain)
+            n_sep = g.norm2(plain, p_out)
+            assert abs(n - n_sep) <= 1e-12 * n_sep
+            assert abs(n - oracle.norm2(g.export_spinor(fused, p_out))) <= 1e-12 * n_sep
+            _, n2 = g.dhop_oe_norm2(fin) if p_out == 1 else g.dhop_eo_norm2(fin)
+            assert n2 == n
+        with pytest.raises(lib.DwfError):
+            lib.dwf_dhop_eo_norm2(g.handle, fin, fin)
