@@ -223,7 +223,7 @@ def run_reference(args, w):
 # ---------------------------------------------------------------------------------------------
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
 # `ncu --set full` capture summarised under profiles/ (None until a capture exists).
-NCU_TRAFFIC_BYTES = {"c4": 1471999000 + 769403000}   # profiles/r01h_dhop_staged_kernel_ncu.md, launch 1
+NCU_TRAFFIC_BYTES = {"c4": 1474414000 + 769279000}   # profiles/r01i_bench_step_ncu.md, launch 1 (DhopOE)
 
 
 def max_over_ranks(x, dist=None, device="cuda"):
