@@ -56,6 +56,10 @@ def _load():
         lib.orc_dhop.restype = ci
         lib.orc_dhop_cb.argtypes = [i4, ci, ci, ci, vp, ci, vp, ci, vp]
         lib.orc_dhop_cb.restype = ci
+        lib.orc_dhop_dag.argtypes = lib.orc_dhop.argtypes
+        lib.orc_dhop_dag.restype = ci
+        lib.orc_dhop_cb_dag.argtypes = lib.orc_dhop_cb.argtypes
+        lib.orc_dhop_cb_dag.restype = ci
         lib.orc_dhop_sites.argtypes = [i4, ci, ci, vp, ci, vp, ci, ci, vp, i64, vp]
         lib.orc_dhop_sites.restype = ci
         lib.orc_norm2.argtypes = [vp, ci, i64]
@@ -99,12 +103,13 @@ def gamma(mu: int) -> np.ndarray:
     return out[..., 0] + 1j * out[..., 1]
 
 
-def dhop(dims, Ls: int, bc_time: int, U: np.ndarray, psi: np.ndarray) -> np.ndarray:
-    """Full Dhop.  U (V4,4,3,3,2), psi (V4,Ls,4,3,2) -> fp64 (V4,Ls,4,3,2)."""
+def dhop(dims, Ls: int, bc_time: int, U: np.ndarray, psi: np.ndarray, dagger: bool = False) -> np.ndarray:
+    """Full Dhop (dagger: its matrix adjoint).  U (V4,4,3,3,2), psi (V4,Ls,4,3,2) -> fp64 (V4,Ls,4,3,2)."""
     d, v4 = _dims(dims)
     assert U.size == v4 * 72 and psi.size == v4 * Ls * 24
     out = np.empty((v4, Ls, 4, 3, 2), dtype=np.float64)
-    rc = _load().orc_dhop(d, Ls, bc_time, _c(U).ctypes.data, _prec(U),
+    fn = _load().orc_dhop_dag if dagger else _load().orc_dhop
+    rc = fn(d, Ls, bc_time, _c(U).ctypes.data, _prec(U),
                           _c(psi).ctypes.data, _prec(psi), out.ctypes.data)
     if rc:
         raise ValueError("orc_dhop: bad arguments")
@@ -112,13 +117,14 @@ def dhop(dims, Ls: int, bc_time: int, U: np.ndarray, psi: np.ndarray) -> np.ndar
 
 
 def dhop_cb(dims, Ls: int, bc_time: int, parity_out: int, U: np.ndarray,
-            psi_half: np.ndarray) -> np.ndarray:
+            psi_half: np.ndarray, dagger: bool = False) -> np.ndarray:
     """Checkerboarded Dhop onto parity_out (ODD: DhopOE, EVEN: DhopEO).
     psi_half (V4/2,Ls,4,3,2) lives on the opposite parity -> fp64 (V4/2,Ls,4,3,2)."""
     d, v4 = _dims(dims)
     assert U.size == v4 * 72 and psi_half.size == (v4 // 2) * Ls * 24
     out = np.empty((v4 // 2, Ls, 4, 3, 2), dtype=np.float64)
-    rc = _load().orc_dhop_cb(d, Ls, bc_time, parity_out, _c(U).ctypes.data, _prec(U),
+    fn = _load().orc_dhop_cb_dag if dagger else _load().orc_dhop_cb
+    rc = fn(d, Ls, bc_time, parity_out, _c(U).ctypes.data, _prec(U),
                              _c(psi_half).ctypes.data, _prec(psi_half), out.ctypes.data)
     if rc:
         raise ValueError("orc_dhop_cb: bad arguments (extents must be even)")

@@ -134,6 +134,7 @@ typedef struct {
     const void *U;   int u_prec;
     const void *psi; int psi_prec;
     int psi_half;    /* 0: psi is a full field; 1: psi is a half field (index x>>1) */
+    int dagger;      /* 0: Dhop; 1: Dhop^dagger */
 } orc_ctx;
 
 static inline size_t lex(const int L[4], const int x[4])
@@ -149,7 +150,10 @@ static inline void coords(const int L[4], size_t site, int x[4])
     x[3] = (int)site;
 }
 
-/* out[spin][colour] = (Dhop psi)(x, s), the definition written out term by term */
+/* out[spin][colour] = (Dhop psi)(x, s), the definition written out term by term.
+ * Dagger: the matrix adjoint of Dhop.  gamma_mu is Hermitian and the hop matrices W_mu, W_mu^dag
+ * change places under the adjoint, so Dhop^dag has (1 + gamma_mu) on the forward hop and
+ * (1 - gamma_mu) on the backward hop, with the same links. */
 static void dhop_site(const orc_ctx *c, const int x[4], int s, cplx out[4][3])
 {
     for (int al = 0; al < 4; al++)
@@ -194,8 +198,8 @@ static void dhop_site(const orc_ctx *c, const int x[4], int s, cplx out[4][3])
         for (int al = 0; al < 4; al++)
             for (int be = 0; be < 4; be++) {
                 cplx one = (al == be) ? 1.0 : 0.0;
-                cplx pm = one - GAMMA[mu][al][be];
-                cplx pp = one + GAMMA[mu][al][be];
+                cplx pm = c->dagger ? one + GAMMA[mu][al][be] : one - GAMMA[mu][al][be];   /* forward hop  */
+                cplx pp = c->dagger ? one - GAMMA[mu][al][be] : one + GAMMA[mu][al][be];   /* backward hop */
                 for (int a = 0; a < 3; a++)
                     out[al][a] += sp * pm * tf[be][a] + sm * pp * tb[be][a];
             }
@@ -216,6 +220,7 @@ static void make_ctx(orc_ctx *c, const int dims[4], int Ls, int antiperiodic_t,
     for (int m = 0; m < 4; m++) c->L[m] = dims[m];
     c->Ls = Ls; c->antiperiodic_t = antiperiodic_t;
     c->U = U; c->u_prec = u_prec; c->psi = psi; c->psi_prec = psi_prec; c->psi_half = psi_half;
+    c->dagger = 0;
 }
 
 static void store_site(double *out, size_t osite, int Ls, int s, cplx r[4][3])
@@ -229,11 +234,12 @@ static void store_site(double *out, size_t osite, int Ls, int s, cplx r[4][3])
 }
 
 /* Full Dhop: psi, out are full canonical fields (out always fp64). */
-int orc_dhop(const int dims[4], int Ls, int antiperiodic_t,
-             const void *U, int u_prec, const void *psi, int psi_prec, double *out)
+static int dhop_full(const int dims[4], int Ls, int antiperiodic_t, int dagger,
+                     const void *U, int u_prec, const void *psi, int psi_prec, double *out)
 {
     if (bad_args(dims, Ls, u_prec, psi_prec) || orc_check_gamma()) return 1;
     orc_ctx c; make_ctx(&c, dims, Ls, antiperiodic_t, U, u_prec, psi, psi_prec, 0);
+    c.dagger = dagger;
     const int64_t V4 = (int64_t)dims[0] * dims[1] * dims[2] * dims[3];
     #pragma omp parallel for schedule(static)
     for (int64_t site = 0; site < V4; site++) {
@@ -251,13 +257,14 @@ int orc_dhop(const int dims[4], int Ls, int antiperiodic_t,
  * field of the opposite parity, out the half field of parity_out (index x>>1).
  * parity_out = 1: DhopOE (even in -> odd out); parity_out = 0: DhopEO.
  * All extents must be even (x>>1 is a bijection within a parity only if L0 is even). */
-int orc_dhop_cb(const int dims[4], int Ls, int antiperiodic_t, int parity_out,
-                const void *U, int u_prec, const void *psi_half, int psi_prec, double *out_half)
+static int dhop_cb(const int dims[4], int Ls, int antiperiodic_t, int parity_out, int dagger,
+                   const void *U, int u_prec, const void *psi_half, int psi_prec, double *out_half)
 {
     if (bad_args(dims, Ls, u_prec, psi_prec) || orc_check_gamma()) return 1;
     if (parity_out != 0 && parity_out != 1) return 1;
     for (int m = 0; m < 4; m++) if (dims[m] & 1) return 1;
     orc_ctx c; make_ctx(&c, dims, Ls, antiperiodic_t, U, u_prec, psi_half, psi_prec, 1);
+    c.dagger = dagger;
     const int64_t V4 = (int64_t)dims[0] * dims[1] * dims[2] * dims[3];
     #pragma omp parallel for schedule(static)
     for (int64_t site = 0; site < V4; site++) {
@@ -270,6 +277,27 @@ int orc_dhop_cb(const int dims[4], int Ls, int antiperiodic_t, int parity_out,
         }
     }
     return 0;
+}
+
+int orc_dhop(const int dims[4], int Ls, int antiperiodic_t,
+             const void *U, int u_prec, const void *psi, int psi_prec, double *out)
+{
+    return dhop_full(dims, Ls, antiperiodic_t, 0, U, u_prec, psi, psi_prec, out);
+}
+int orc_dhop_dag(const int dims[4], int Ls, int antiperiodic_t,
+                 const void *U, int u_prec, const void *psi, int psi_prec, double *out)
+{
+    return dhop_full(dims, Ls, antiperiodic_t, 1, U, u_prec, psi, psi_prec, out);
+}
+int orc_dhop_cb(const int dims[4], int Ls, int antiperiodic_t, int parity_out,
+                const void *U, int u_prec, const void *psi_half, int psi_prec, double *out_half)
+{
+    return dhop_cb(dims, Ls, antiperiodic_t, parity_out, 0, U, u_prec, psi_half, psi_prec, out_half);
+}
+int orc_dhop_cb_dag(const int dims[4], int Ls, int antiperiodic_t, int parity_out,
+                    const void *U, int u_prec, const void *psi_half, int psi_prec, double *out_half)
+{
+    return dhop_cb(dims, Ls, antiperiodic_t, parity_out, 1, U, u_prec, psi_half, psi_prec, out_half);
 }
 
 /* Dhop at a list of output sites (lexicographic indices), all s: out[n][Ls][4][3][2].

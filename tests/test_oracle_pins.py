@@ -210,3 +210,45 @@ def test_sites_subset_matches_full_and_cb():
     odd = np.arange(V)[par == 1][[0, 3, 40, -1]]
     sub = oracle.dhop_sites(dims, Ls, bc, U, gen.split_parity(psi, dims, 0), True, odd)
     assert np.array_equal(sub, full[odd])
+
+
+# ---- Dhop^dagger: the oracle's projector swap against the matrix adjoint ------------
+
+@pytest.mark.parametrize("dims,Ls", TINY)
+@pytest.mark.parametrize("bc", [oracle.PERIODIC, oracle.ANTIPERIODIC_T])
+def test_dagger_is_the_adjoint_of_the_dense_matrix(dims, Ls, bc):
+    """numpy's conjugate transpose of the brute-force matrix knows nothing about projectors."""
+    V = int(np.prod(dims))
+    U = gen.gauge_random(dims, seed=21)
+    psi = gen.spinor_gaussian(V, Ls, seed=21)
+    D = dense_dhop_matrix(dims, U, bc == oracle.ANTIPERIODIC_T)
+    assert rel_err(oracle.dhop(dims, Ls, bc, U, psi, dagger=True), apply_dense(D.conj().T, psi)) < 1e-14
+    assert rel_err(oracle.dhop(dims, Ls, bc, U, psi, dagger=True), oracle.dhop(dims, Ls, bc, U, psi)) > 0.1
+
+
+@pytest.mark.parametrize("dims,Ls,bc", [((4, 2, 4, 2), 2, 0), ((4, 4, 2, 6), 3, 1)])
+def test_dagger_is_gamma5_dhop_gamma5_and_adjoint_under_the_inner_product(dims, Ls, bc):
+    V = int(np.prod(dims))
+    U = gen.gauge_random(dims, seed=22)
+    psi = gen.spinor_gaussian(V, Ls, seed=22, stream=gen.STREAM_SPINOR)
+    phi = gen.spinor_gaussian(V, Ls, seed=22, stream=gen.STREAM_SPINOR2)
+    g5 = np.array([1.0, 1.0, -1.0, -1.0]).reshape(1, 1, 4, 1, 1)
+    # gamma5-hermiticity, using only the plain (non-dagger) oracle on the right-hand side
+    assert rel_err(oracle.dhop(dims, Ls, bc, U, psi, dagger=True), g5 * oracle.dhop(dims, Ls, bc, U, g5 * psi)) < 1e-14
+    # <phi, D psi> = <D^dag phi, psi>
+    lhs = oracle.inner(phi, oracle.dhop(dims, Ls, bc, U, psi))
+    rhs = oracle.inner(oracle.dhop(dims, Ls, bc, U, phi, dagger=True), psi)
+    assert abs(lhs - rhs) <= 1e-12 * abs(lhs)
+
+
+@pytest.mark.parametrize("dims,Ls,bc", [((4, 2, 4, 2), 2, 0), ((2, 2, 4, 6), 3, 1)])
+def test_dagger_even_odd_reassembly(dims, Ls, bc):
+    V = int(np.prod(dims))
+    U = gen.gauge_random(dims, seed=23)
+    psi = gen.spinor_gaussian(V, Ls, seed=23)
+    full = oracle.dhop(dims, Ls, bc, U, psi, dagger=True)
+    par = gen.site_parity(dims)
+    for p_out in (0, 1):
+        half = gen.split_parity(psi, dims, 1 - p_out)
+        got = oracle.dhop_cb(dims, Ls, bc, p_out, U, half, dagger=True)
+        assert rel_err(got, full[par == p_out]) < 1e-15
