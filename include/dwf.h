@@ -92,6 +92,15 @@ DWF_API int dwf_dhop(const dwf_geometry *g, const void *in_full, void *out_full,
 DWF_API int dwf_dhop_oe(const dwf_geometry *g, const void *in_even, void *out_odd, void *stream);
 DWF_API int dwf_dhop_eo(const dwf_geometry *g, const void *in_odd, void *out_even, void *stream);
 
+/* The adjoint operator (the first NEXT row; needed for CG on the normal equations):
+ *   Dhop^dag psi(x,s) = sum_mu [ (1+gamma_mu) U_mu(x) psi(x+mu,s) + (1-gamma_mu) U_mu^dag(x-mu) psi(x-mu,s) ]
+ * = gamma5 Dhop gamma5 (the hop matrices change places under the adjoint, gamma_mu is Hermitian, so
+ * only the projectors swap; PAPER.md never writes the operator, BASELINE.json north_star does).
+ * Same layouts, parities (first letter = output parity), errors and asynchrony as the calls above. */
+DWF_API int dwf_dhop_dag(const dwf_geometry *g, const void *in_full, void *out_full, void *stream);
+DWF_API int dwf_dhop_oe_dag(const dwf_geometry *g, const void *in_even, void *out_odd, void *stream);
+DWF_API int dwf_dhop_eo_dag(const dwf_geometry *g, const void *in_odd, void *out_even, void *stream);
+
 /* *result_host = sum over all reals of |field|^2, accumulated in fp64 in a fixed order
  * (deterministic).  parity = DWF_FULL for a full field, DWF_EVEN / DWF_ODD for a half field.
  * Synchronises `stream`. */

@@ -25,7 +25,7 @@ LIB_PATH = os.path.join(_HERE, "libdwf.so")
 # every symbol include/dwf.h declares (tests check that the library exports all of them)
 SYMBOLS = (
     "dwf_create_geometry", "dwf_destroy_geometry", "dwf_load_gauge", "dwf_dhop", "dwf_dhop_oe",
-    "dwf_dhop_eo", "dwf_dhop_oe_norm2", "dwf_dhop_eo_norm2", "dwf_norm2", "dwf_inner_product", "dwf_field_bytes",
+    "dwf_dhop_eo", "dwf_dhop_dag", "dwf_dhop_oe_dag", "dwf_dhop_eo_dag", "dwf_dhop_oe_norm2", "dwf_dhop_eo_norm2", "dwf_norm2", "dwf_inner_product", "dwf_field_bytes",
     "dwf_import_spinor", "dwf_export_spinor", "dwf_launch_count", "dwf_set_option",
     "dwf_error_string", "dwf_last_error",
 )
@@ -55,7 +55,7 @@ def load(build_if_missing: bool = True):
     lib.dwf_create_geometry.argtypes = [ctypes.POINTER(ci), ci, ci, ci, ci, ctypes.POINTER(vp)]
     lib.dwf_destroy_geometry.argtypes = [vp]
     lib.dwf_load_gauge.argtypes = [vp, vp, ci, vp]
-    for f in (lib.dwf_dhop, lib.dwf_dhop_oe, lib.dwf_dhop_eo):
+    for f in (lib.dwf_dhop, lib.dwf_dhop_oe, lib.dwf_dhop_eo, lib.dwf_dhop_dag, lib.dwf_dhop_oe_dag, lib.dwf_dhop_eo_dag):
         f.argtypes = [vp, vp, vp, vp]
     lib.dwf_norm2.argtypes = [vp, vp, ci, ctypes.POINTER(ctypes.c_double), vp]
     for f in (lib.dwf_dhop_oe_norm2, lib.dwf_dhop_eo_norm2):
@@ -140,6 +140,18 @@ def dwf_dhop_oe(g: int, in_even, out_odd, stream=None) -> None:
 
 def dwf_dhop_eo(g: int, in_odd, out_even, stream=None) -> None:
     _check(load().dwf_dhop_eo(g, _dev_ptr(in_odd), _dev_ptr(out_even), _stream(stream)), "dwf_dhop_eo")
+
+
+def dwf_dhop_dag(g: int, in_full, out_full, stream=None) -> None:
+    _check(load().dwf_dhop_dag(g, _dev_ptr(in_full), _dev_ptr(out_full), _stream(stream)), "dwf_dhop_dag")
+
+
+def dwf_dhop_oe_dag(g: int, in_even, out_odd, stream=None) -> None:
+    _check(load().dwf_dhop_oe_dag(g, _dev_ptr(in_even), _dev_ptr(out_odd), _stream(stream)), "dwf_dhop_oe_dag")
+
+
+def dwf_dhop_eo_dag(g: int, in_odd, out_even, stream=None) -> None:
+    _check(load().dwf_dhop_eo_dag(g, _dev_ptr(in_odd), _dev_ptr(out_even), _stream(stream)), "dwf_dhop_eo_dag")
 
 
 def dwf_dhop_oe_norm2(g: int, in_even, out_odd, stream=None) -> float:
@@ -257,6 +269,21 @@ class Geometry:
     def dhop(self, inp, out=None, stream=None):
         out = self.new_field(FULL) if out is None else out
         dwf_dhop(self.handle, inp, out, stream)
+        return out
+
+    def dhop_dag(self, inp, out=None, stream=None):
+        out = self.new_field(FULL) if out is None else out
+        dwf_dhop_dag(self.handle, inp, out, stream)
+        return out
+
+    def dhop_oe_dag(self, in_even, out=None, stream=None):
+        out = self.new_field(ODD) if out is None else out
+        dwf_dhop_oe_dag(self.handle, in_even, out, stream)
+        return out
+
+    def dhop_eo_dag(self, in_odd, out=None, stream=None):
+        out = self.new_field(EVEN) if out is None else out
+        dwf_dhop_eo_dag(self.handle, in_odd, out, stream)
         return out
 
     def dhop_oe(self, in_even, out=None, stream=None):

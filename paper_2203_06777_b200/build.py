@@ -19,7 +19,12 @@ ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libdwf.so")
 OBJDIR = os.path.join(HERE, "build")
 
-SOURCES = ["api.cu", "pack.cu", "dhop.cu", "dhop_staged.cu", "reduce.cu"]
+# (source, object name, extra defines): dhop_staged.cu is compiled once per kernel MODE so that the
+# three sets of template instances build in parallel
+SOURCES = [("api.cu", "api.o", []), ("pack.cu", "pack.o", []), ("dhop.cu", "dhop.o", []), ("reduce.cu", "reduce.o", []),
+           ("dhop_staged.cu", "dhop_staged_m0.o", ["-DDWF_STAGED_MODE=0"]),
+           ("dhop_staged.cu", "dhop_staged_m1.o", ["-DDWF_STAGED_MODE=1"]),
+           ("dhop_staged.cu", "dhop_staged_m2.o", ["-DDWF_STAGED_MODE=2"])]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden",
@@ -54,11 +59,12 @@ def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = _nvcc()
     extra = ["-Xptxas", "-v"] if verbose else []
 
-    def compile_one(src):
-        obj = os.path.join(OBJDIR, src.replace(".cu", ".o"))
-        cmd = [nvcc, *NVCC_FLAGS, *extra, "-c", os.path.join(CSRC, src), "-o", obj]
+    def compile_one(item):
+        src, objname, defines = item
+        obj = os.path.join(OBJDIR, objname)
+        cmd = [nvcc, *NVCC_FLAGS, *extra, *defines, "-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
-        return src, obj, r
+        return objname, obj, r
 
     with concurrent.futures.ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
         results = list(ex.map(compile_one, SOURCES))

@@ -326,18 +326,19 @@ int dwf_load_gauge(dwf_geometry *g, const void *U, int src_is_device, void *stre
 }
 
 // one half-Dhop: out (parity_out) = D in (opposite parity); picks the kernel
-static int half_dhop(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st)
+static int half_dhop(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger = false)
 {
     const bool staged_ok = g->staged.variant >= 0;
     if (g->opt_kernel == 2 && !staged_ok) {
         set_error("the staged kernel does not support this geometry / precision");
         return DWF_ERR_UNSUPPORTED;
     }
-    if (staged_ok && g->opt_kernel != 1) return launch_dhop_staged(g, in, out, parity_out, st);
-    return launch_dhop_direct(g, in, out, parity_out, st);
+    if (staged_ok && g->opt_kernel != 1) return launch_dhop_staged(g, in, out, parity_out, st, nullptr, nullptr, dagger);
+    return launch_dhop_direct(g, in, out, parity_out, st, dagger);
 }
 
-static int dhop_common(const dwf_geometry *g, const void *in, void *out, int parity_out, void *stream, const char *who)
+static int dhop_common(const dwf_geometry *g, const void *in, void *out, int parity_out, void *stream, const char *who,
+                       bool dagger = false)
 {
     if (!g || !in || !out) { set_error("%s: NULL argument", who); return DWF_ERR_INVALID_ARG; }
     if (in == out) { set_error("%s: in-place application is not defined (in == out)", who); return DWF_ERR_INVALID_ARG; }
@@ -345,15 +346,15 @@ static int dhop_common(const dwf_geometry *g, const void *in, void *out, int par
     if (!g->gauge_loaded) { set_error("%s: call dwf_load_gauge first", who); return DWF_ERR_NO_GAUGE; }
     DeviceGuard guard(g->device);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (parity_out != DWF_FULL) return half_dhop(g, in, out, parity_out, st);
+    if (parity_out != DWF_FULL) return half_dhop(g, in, out, parity_out, st, dagger);
     // a full field is its even half field followed by its odd half field:
     // (Dhop psi)_odd = DhopOE psi_even, (Dhop psi)_even = DhopEO psi_odd
     const size_t half = dwf_field_bytes(g, DWF_EVEN);
     const char *ie = static_cast<const char *>(in), *io = ie + half;
     char *oe = static_cast<char *>(out), *oo = oe + half;
-    int rc = half_dhop(g, ie, oo, DWF_ODD, st);
+    int rc = half_dhop(g, ie, oo, DWF_ODD, st, dagger);
     if (rc) return rc;
-    return half_dhop(g, io, oe, DWF_EVEN, st);
+    return half_dhop(g, io, oe, DWF_EVEN, st, dagger);
 }
 
 int dwf_dhop(const dwf_geometry *g, const void *in_full, void *out_full, void *stream)
@@ -367,6 +368,18 @@ int dwf_dhop_oe(const dwf_geometry *g, const void *in_even, void *out_odd, void 
 int dwf_dhop_eo(const dwf_geometry *g, const void *in_odd, void *out_even, void *stream)
 {
     return dhop_common(g, in_odd, out_even, DWF_EVEN, stream, "dwf_dhop_eo");
+}
+int dwf_dhop_dag(const dwf_geometry *g, const void *in_full, void *out_full, void *stream)
+{
+    return dhop_common(g, in_full, out_full, DWF_FULL, stream, "dwf_dhop_dag", true);
+}
+int dwf_dhop_oe_dag(const dwf_geometry *g, const void *in_even, void *out_odd, void *stream)
+{
+    return dhop_common(g, in_even, out_odd, DWF_ODD, stream, "dwf_dhop_oe_dag", true);
+}
+int dwf_dhop_eo_dag(const dwf_geometry *g, const void *in_odd, void *out_even, void *stream)
+{
+    return dhop_common(g, in_odd, out_even, DWF_EVEN, stream, "dwf_dhop_eo_dag", true);
 }
 
 // out = D in on half fields and *result_host = norm2(out): the reduction runs in the epilogue of the

@@ -137,7 +137,8 @@ __device__ __forceinline__ void dhop_leg(typename CxT<T>::type (&acc)[12][SC],
 // in/out are half fields pair[s][row][k/2][h][k&1] (slot meaning: pack.cu); out has parity `parity_out`, in the opposite parity.
 // One thread = one output site and one s-slice.
 // ---------------------------------------------------------------------------------------------
-template <typename T, int MAXT, int MINB>
+// DAG: Dhop^dagger -- the projectors (1 - gamma) and (1 + gamma) change places
+template <typename T, int MAXT, int MINB, bool DAG>
 __global__ void __launch_bounds__(MAXT, MINB)
 dhop_direct_kernel(const typename CxT<T>::type *__restrict__ in, typename CxT<T>::type *__restrict__ out,
                    const T *__restrict__ gset, const int4 *__restrict__ tiles, const Lattice lat,
@@ -184,14 +185,14 @@ dhop_direct_kernel(const typename CxT<T>::type *__restrict__ in, typename CxT<T>
     const C *gl = reinterpret_cast<const C *>(gset) + (size_t)row * 72 * W0 + 2 * c0;   // this site's links
 
     C acc[12][SC];
-    dhop_leg<T, SC, 0, true,  true , 0>(acc, base + n0p, W0, gl);
-    dhop_leg<T, SC, 0, false, false, 1>(acc, base + n0m, W0, gl);
-    dhop_leg<T, SC, 1, true,  false, 2>(acc, base + n1p, W0, gl);
-    dhop_leg<T, SC, 1, false, false, 3>(acc, base + n1m, W0, gl);
-    dhop_leg<T, SC, 2, true,  false, 4>(acc, base + n2p, W0, gl);
-    dhop_leg<T, SC, 2, false, false, 5>(acc, base + n2m, W0, gl);
-    dhop_leg<T, SC, 3, true,  false, 6>(acc, base + n3p, W0, gl);
-    dhop_leg<T, SC, 3, false, false, 7>(acc, base + n3m, W0, gl);
+    dhop_leg<T, SC, 0, true != DAG, true, 0>(acc, base + n0p, W0, gl);
+    dhop_leg<T, SC, 0, false != DAG, false, 1>(acc, base + n0m, W0, gl);
+    dhop_leg<T, SC, 1, true != DAG, false, 2>(acc, base + n1p, W0, gl);
+    dhop_leg<T, SC, 1, false != DAG, false, 3>(acc, base + n1m, W0, gl);
+    dhop_leg<T, SC, 2, true != DAG, false, 4>(acc, base + n2p, W0, gl);
+    dhop_leg<T, SC, 2, false != DAG, false, 5>(acc, base + n2m, W0, gl);
+    dhop_leg<T, SC, 3, true != DAG, false, 6>(acc, base + n3p, W0, gl);
+    dhop_leg<T, SC, 3, false != DAG, false, 7>(acc, base + n3m, W0, gl);
 
     C *o = out + (size_t)s * 12 * (size_t)Vh + (size_t)own;
     if constexpr (sizeof(T) == 8) {
@@ -214,7 +215,7 @@ dhop_direct_kernel(const typename CxT<T>::type *__restrict__ in, typename CxT<T>
     }
 }
 
-template <typename T, int MAXT, int MINB>
+template <typename T, int MAXT, int MINB, bool DAG>
 static int launch_direct(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st)
 {
     using C = typename CxT<T>::type;
@@ -224,7 +225,7 @@ static int launch_direct(const dwf_geometry *g, const void *in, void *out, int p
         return DWF_ERR_UNSUPPORTED;
     }
     dim3 grid((unsigned)(til.ntiles * til.ncg)), block((unsigned)til.threads);
-    dhop_direct_kernel<T, MAXT, MINB><<<grid, block, 0, st>>>(
+    dhop_direct_kernel<T, MAXT, MINB, DAG><<<grid, block, 0, st>>>(
         static_cast<const C *>(in), static_cast<C *>(out), static_cast<const T *>(g->gauge[parity_out]),
         g->tiles_cb, g->lat, til, parity_out);
     count_launch();
@@ -233,10 +234,13 @@ static int launch_direct(const dwf_geometry *g, const void *in, void *out, int p
 }
 
 // parity_out: DWF_EVEN (DhopEO) or DWF_ODD (DhopOE)
-int launch_dhop_direct(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st)
+int launch_dhop_direct(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger)
 {
-    if (g->prec == DWF_F32) return launch_direct<float, 256, 3>(g, in, out, parity_out, st);
-    return launch_direct<double, 256, 2>(g, in, out, parity_out, st);
+    if (g->prec == DWF_F32)
+        return dagger ? launch_direct<float, 256, 3, true>(g, in, out, parity_out, st)
+                      : launch_direct<float, 256, 3, false>(g, in, out, parity_out, st);
+    return dagger ? launch_direct<double, 256, 2, true>(g, in, out, parity_out, st)
+                  : launch_direct<double, 256, 2, false>(g, in, out, parity_out, st);
 }
 
 }  // namespace dwf

@@ -40,6 +40,11 @@
 
 namespace dwf {
 
+#ifndef DWF_STAGED_MODE
+#define DWF_STAGED_MODE 0      // which kernel MODE this translation unit instantiates (see "Kernel instances")
+#endif
+
+#if DWF_STAGED_MODE == 0
 PFN_tensorMapEncodeTiled get_tensor_map_encoder()
 {
     static PFN_tensorMapEncodeTiled fn = [] {
@@ -54,6 +59,7 @@ PFN_tensorMapEncodeTiled get_tensor_map_encoder()
     }();
     return fn;
 }
+#endif
 
 // L2 policy classes of the kernel's global accesses (option "l2pol", one decimal digit each,
 // class 0 = least significant; digit 0 evict_normal, 1 evict_first, 2 evict_last)
@@ -223,9 +229,11 @@ __device__ __forceinline__ void staged_leg(float2 (&acc)[12], const float4 *__re
     }
 }
 
-// NORM: also accumulate |out|^2 (fp64, fixed order) and write one partial per CTA -- norm2 of the
-// result fused into the kernel that produces it (saves re-reading the output field).
-template <int LH, int B1, int B2, int B3, bool NORM>
+// MODE 0: Dhop.  MODE 1 (NORM): also accumulate |out|^2 (fp64, fixed order) and write one partial per
+// CTA -- norm2 of the result fused into the kernel that produces it (saves re-reading the output
+// field).  MODE 2 (DAG): Dhop^dagger = the projectors (1 - gamma) and (1 + gamma) change places, same
+// links and neighbours.
+template <int LH, int B1, int B2, int B3, int MODE>
 __global__ void __launch_bounds__(StagedCfg<LH, B1, B2, B3>::NT, StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM)
 dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_x1,
                    const __grid_constant__ CUtensorMap map_x2, const __grid_constant__ CUtensorMap map_x3,
@@ -233,6 +241,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
                    const StagedArgs args)
 {
     using Cfg = StagedCfg<LH, B1, B2, B3>;
+    constexpr bool NORM = MODE == 1, DAG = MODE == 2;
     extern __shared__ __align__(1024) unsigned char smem[];
     const uint32_t smem_base = smem_u32(smem);
     const uint32_t full_base = smem_base + Cfg::NSTAGE * Cfg::STAGE_BYTES;      // full[stage][region]: TMA data has landed
@@ -447,7 +456,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         const bool legs = !(args.ablate & 4);
         float2 acc[12];
 #define DWF_LEG(L, MU, FWD, FIRST)                                                                  \
-        staged_leg<LH, MU, FWD, FIRST, DWF_ABL>(acc, reinterpret_cast<const float4 *>(sb) + (((L) & 1) ? offp[(L) >> 1] >> 16 : offp[(L) >> 1] & 0xffffu), U + 9 * (L)); \
+        staged_leg<LH, MU, (FWD) != DAG, FIRST, DWF_ABL>(acc, reinterpret_cast<const float4 *>(sb) + (((L) & 1) ? offp[(L) >> 1] >> 16 : offp[(L) >> 1] & 0xffffu), U + 9 * (L)); \
         if constexpr (FETCH && REFILL_PER_LEG) {   /* refill the component pairs whose last use was this leg */ \
             _Pragma("unroll") for (int j = (9 * (L)) / 2; j < (9 * ((L) + 1)) / 2; j++) {            \
                 const float4 q = ldg128_hint(gnext + j * LH, pol_g);                                \
@@ -588,33 +597,53 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
 }
 
 // ---------------------------------------------------------------------------------------------
+// Kernel instances.  This file is compiled once per MODE (-DDWF_STAGED_MODE=0|1|2, build.py) so
+// that the three sets of instances build in parallel; each translation unit exports the entry
+// points of its MODE in the order of DWF_STAGED_VARIANTS, the MODE 0 unit also holds the host code.
+// Ordered by preference within one Lh: larger tiles (smaller halo ratio) first; the "variant"
+// option counts from 1 in this order.
+// ---------------------------------------------------------------------------------------------
+#define DWF_STAGED_VARIANTS(X)                                                                       \
+    X(16, 4, 2, 2) X(16, 2, 2, 2) X(16, 2, 2, 1) X(8, 4, 4, 2) X(8, 2, 2, 2) X(8, 2, 2, 1)           \
+    X(24, 2, 2, 2) X(24, 2, 2, 1) X(4, 4, 4, 4) X(4, 2, 2, 2) X(4, 2, 2, 1)                           \
+    X(16, 2, 2, 4) X(16, 2, 4, 2) X(16, 8, 2, 1) X(16, 1, 2, 8) X(24, 3, 1, 3) X(24, 1, 3, 3) X(24, 3, 3, 1)
+
+const void *const *staged_kernels_mode0();
+const void *const *staged_kernels_mode1();
+const void *const *staged_kernels_mode2();
+
+#define DWF_CAT2(a, b) a##b
+#define DWF_CAT(a, b) DWF_CAT2(a, b)
+const void *const *DWF_CAT(staged_kernels_mode, DWF_STAGED_MODE)()
+{
+#define X(LH, B1, B2, B3) reinterpret_cast<const void *>(&dhop_staged_kernel<LH, B1, B2, B3, DWF_STAGED_MODE>),
+    static const void *const tab[] = {DWF_STAGED_VARIANTS(X)};
+#undef X
+    return tab;
+}
+
+#if DWF_STAGED_MODE == 0
+// ---------------------------------------------------------------------------------------------
 // host side: plan, tile table, tensor maps, launch
 // ---------------------------------------------------------------------------------------------
 struct Variant {
     int lh, b1, b2, b3;
     int smem, threads, ctas_per_sm;
-    const void *fn, *fn_norm;
+    const void *fn[3];       // MODE 0 (Dhop), 1 (Dhop + norm2), 2 (Dhop^dagger)
 };
-
-template <int LH, int B1, int B2, int B3> static Variant make_variant()
-{
-    using Cfg = StagedCfg<LH, B1, B2, B3>;
-    return {LH, B1, B2, B3, Cfg::SMEM_BYTES, Cfg::NT, Cfg::CTAS_PER_SM,
-            reinterpret_cast<const void *>(&dhop_staged_kernel<LH, B1, B2, B3, false>),
-            reinterpret_cast<const void *>(&dhop_staged_kernel<LH, B1, B2, B3, true>)};
-}
 
 static const std::vector<Variant> &variants()
 {
-    // ordered by preference within one Lh: larger tiles (smaller halo ratio) first
-    static const std::vector<Variant> v = {
-        make_variant<16, 4, 2, 2>(), make_variant<16, 2, 2, 2>(), make_variant<16, 2, 2, 1>(),
-        make_variant<8, 4, 4, 2>(),  make_variant<8, 2, 2, 2>(),  make_variant<8, 2, 2, 1>(),
-        make_variant<24, 2, 2, 2>(), make_variant<24, 2, 2, 1>(),
-        make_variant<4, 4, 4, 4>(),  make_variant<4, 2, 2, 2>(),  make_variant<4, 2, 2, 1>(),
-        make_variant<16, 2, 2, 4>(), make_variant<16, 2, 4, 2>(), make_variant<16, 8, 2, 1>(), make_variant<16, 1, 2, 8>(),
-        make_variant<24, 3, 1, 3>(), make_variant<24, 1, 3, 3>(), make_variant<24, 3, 3, 1>(),
-    };
+    static const std::vector<Variant> v = [] {
+        std::vector<Variant> t;
+        const void *const *k0 = staged_kernels_mode0(), *const *k1 = staged_kernels_mode1(), *const *k2 = staged_kernels_mode2();
+#define X(LH, B1, B2, B3)                                                                            \
+        t.push_back({LH, B1, B2, B3, StagedCfg<LH, B1, B2, B3>::SMEM_BYTES, StagedCfg<LH, B1, B2, B3>::NT,  \
+                     StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM, {k0[t.size()], k1[t.size()], k2[t.size()]}});
+        DWF_STAGED_VARIANTS(X)
+#undef X
+        return t;
+    }();
     return v;
 }
 
@@ -687,8 +716,9 @@ static int encode_map(CUtensorMap *m, const void *base, const Lattice &lat, int 
 }
 
 int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st,
-                       double *norm_partials, int *norm_blocks)
+                       double *norm_partials, int *norm_blocks, bool dagger)
 {
+    if (dagger && norm_partials) { set_error("no fused norm2 for the dagger kernel"); return DWF_ERR_UNSUPPORTED; }
     const Variant &v = variants()[(size_t)g->staged.variant];
     CUtensorMap mc, m1, m2, m3, m1l, m2l;
     int rc;
@@ -715,11 +745,12 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     const int slots = g->sm_count * v.ctas_per_sm;       // co-resident CTAs
     while (ssplit > 1 && (g->lat.Ls % ssplit || slots % ssplit)) ssplit--;
     a.ssplit = ssplit;
-    const void *fn = norm_partials ? v.fn_norm : v.fn;
-    static thread_local const void *attr_set_for[2] = {nullptr, nullptr};
-    if (attr_set_for[norm_partials != nullptr] != fn) {
+    const int mode = norm_partials ? 1 : (dagger ? 2 : 0);
+    const void *fn = v.fn[mode];
+    static thread_local const void *attr_set_for[3] = {nullptr, nullptr, nullptr};
+    if (attr_set_for[mode] != fn) {
         DWF_CUDA_CHECK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, v.smem));
-        attr_set_for[norm_partials != nullptr] = fn;
+        attr_set_for[mode] = fn;
     }
     const int ngroup_max = slots / ssplit;
     const int ngroup = g->staged.ntiles < ngroup_max ? g->staged.ntiles : ngroup_max;
@@ -730,5 +761,6 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     count_launch();
     return DWF_OK;
 }
+#endif  // DWF_STAGED_MODE == 0
 
 }  // namespace dwf

@@ -111,13 +111,14 @@ int launch_import(const dwf_geometry *g, const void *canonical_dev, int parity, 
 int launch_export(const dwf_geometry *g, const void *field, int parity, void *canonical_dev,
                   cudaStream_t st);
 // dhop.cu (direct kernel; half fields only)
-int launch_dhop_direct(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st);
+int launch_dhop_direct(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st,
+                       bool dagger = false);
 // dhop_staged.cu (TMA-staged link-stationary kernel, fp32 half fields)
 void plan_staged(dwf_geometry *g);                      // fills g->staged (variant = -1 if unusable)
 void build_staged_tile_table(const dwf_geometry *g, int raster, int4 *host_table);
 // norm_partials != nullptr: the fused-norm2 kernel writes one partial of |out|^2 per CTA there, *norm_blocks = their number
 int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st,
-                       double *norm_partials = nullptr, int *norm_blocks = nullptr);
+                       double *norm_partials = nullptr, int *norm_blocks = nullptr, bool dagger = false);
 // reduce.cu
 int launch_norm2(const dwf_geometry *g, const void *field, size_t nreal, cudaStream_t st);
 int launch_final_sum(const dwf_geometry *g, int nblocks, cudaStream_t st);   // result_dev[0] = sum of partials[0..nblocks)
