@@ -188,6 +188,8 @@ int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, i
     dwf_geometry *g = new (std::nothrow) dwf_geometry();
     if (!g) return DWF_ERR_ALLOC;
     memset(g, 0, sizeof(*g));
+    static std::atomic<unsigned long long> next_uid{1};
+    g->uid = next_uid.fetch_add(1);
     for (int d = 0; d < 4; d++) g->lat.L[d] = dims[d];
     g->lat.Lh = dims[0] / 2;
     g->lat.Ls = Ls;

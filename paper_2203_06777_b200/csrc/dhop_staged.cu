@@ -720,14 +720,29 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
 {
     if (dagger && norm_partials) { set_error("no fused norm2 for the dagger kernel"); return DWF_ERR_UNSUPPORTED; }
     const Variant &v = variants()[(size_t)g->staged.variant];
-    CUtensorMap mc, m1, m2, m3, m1l, m2l;
-    int rc;
-    if ((rc = encode_map(&mc, in, g->lat, v.b1, v.b2, v.b3))) return rc;
-    if ((rc = encode_map(&m1, in, g->lat, 1, v.b2, v.b3))) return rc;
-    if ((rc = encode_map(&m2, in, g->lat, v.b1, 1, v.b3))) return rc;
-    if ((rc = encode_map(&m3, in, g->lat, v.b1, v.b2, 1))) return rc;
-    if ((rc = encode_map(&m1l, in, g->lat, 1, v.b2, 1))) return rc;
-    if ((rc = encode_map(&m2l, in, g->lat, v.b1, 1, 1))) return rc;
+    // The six tensor maps depend on the input pointer and the tile shape only.  A solver applies the
+    // operator to the same few buffers over and over, so the encoded maps are kept in a small
+    // per-thread cache (keyed by geometry id, variant and pointer): no driver calls on a hit.
+    struct MapSet { unsigned long long gid; int variant; const void *in; CUtensorMap m[6]; };
+    static thread_local MapSet cache[8];
+    static thread_local unsigned next_slot = 0;
+    MapSet *ms = nullptr;
+    for (MapSet &c : cache)
+        if (c.in == in && c.gid == g->uid && c.variant == g->staged.variant) { ms = &c; break; }
+    if (!ms) {
+        MapSet t;
+        t.gid = g->uid; t.variant = g->staged.variant; t.in = in;
+        int rc;
+        if ((rc = encode_map(&t.m[0], in, g->lat, v.b1, v.b2, v.b3))) return rc;
+        if ((rc = encode_map(&t.m[1], in, g->lat, 1, v.b2, v.b3))) return rc;
+        if ((rc = encode_map(&t.m[2], in, g->lat, v.b1, 1, v.b3))) return rc;
+        if ((rc = encode_map(&t.m[3], in, g->lat, v.b1, v.b2, 1))) return rc;
+        if ((rc = encode_map(&t.m[4], in, g->lat, 1, v.b2, 1))) return rc;
+        if ((rc = encode_map(&t.m[5], in, g->lat, v.b1, 1, 1))) return rc;
+        ms = &cache[next_slot++ % 8];
+        *ms = t;
+    }
+    CUtensorMap &mc = ms->m[0], &m1 = ms->m[1], &m2 = ms->m[2], &m3 = ms->m[3], &m1l = ms->m[4], &m2l = ms->m[5];
     StagedArgs a;
     a.out = static_cast<float2 *>(out);
     a.gauge = static_cast<const float2 *>(g->gauge[parity_out]);

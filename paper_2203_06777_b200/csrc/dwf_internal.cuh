@@ -62,6 +62,7 @@ struct StagedPlan {
 
 // the opaque handle of dwf.h
 struct dwf_geometry {
+    unsigned long long uid;  // unique per created geometry (never reused; keys the tensor-map cache)
     dwf::Lattice lat;
     int prec;               // DWF_F32 / DWF_F64
     int bc_time;
