@@ -101,6 +101,18 @@ DWF_API int dwf_dhop_dag(const dwf_geometry *g, const void *in_full, void *out_f
 DWF_API int dwf_dhop_oe_dag(const dwf_geometry *g, const void *in_even, void *out_odd, void *stream);
 DWF_API int dwf_dhop_eo_dag(const dwf_geometry *g, const void *in_odd, void *out_even, void *stream);
 
+/* The Wilson-matrix fusion of SURVEY.md 8(f1):  out = a x + b (DhopOE in)   resp.   a x + b (DhopEO in),
+ * x and out half fields of the OUTPUT parity.  With a = 4 + m, b = -1/2 this is one half of the
+ * even/odd Wilson matrix M = (4 + m) - Dhop/2, with a = 1 one half of its Schur complement.  The fast
+ * fp32 kernel stages x by TMA next to the input slice and combines in its store epilogue (one
+ * pass; x == out allowed); other geometries / fp64 run Dhop followed by an elementwise pass
+ * (x == out is then UNSUPPORTED).  a, b are rounded to the geometry's precision.  `in` must differ
+ * from x and out.  Asynchronous on `stream`.  Errors as dwf_dhop_oe. */
+DWF_API int dwf_dhop_oe_axpy(const dwf_geometry *g, const void *in_even, const void *x_odd, double a, double b,
+                     void *out_odd, void *stream);
+DWF_API int dwf_dhop_eo_axpy(const dwf_geometry *g, const void *in_odd, const void *x_even, double a, double b,
+                     void *out_even, void *stream);
+
 /* *result_host = sum over all reals of |field|^2, accumulated in fp64 in a fixed order
  * (deterministic).  parity = DWF_FULL for a full field, DWF_EVEN / DWF_ODD for a half field.
  * Synchronises `stream`. */

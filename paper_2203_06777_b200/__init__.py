@@ -25,7 +25,7 @@ LIB_PATH = os.path.join(_HERE, "libdwf.so")
 # every symbol include/dwf.h declares (tests check that the library exports all of them)
 SYMBOLS = (
     "dwf_create_geometry", "dwf_destroy_geometry", "dwf_load_gauge", "dwf_dhop", "dwf_dhop_oe",
-    "dwf_dhop_eo", "dwf_dhop_dag", "dwf_dhop_oe_dag", "dwf_dhop_eo_dag", "dwf_dhop_oe_norm2", "dwf_dhop_eo_norm2", "dwf_norm2", "dwf_inner_product", "dwf_field_bytes",
+    "dwf_dhop_eo", "dwf_dhop_dag", "dwf_dhop_oe_dag", "dwf_dhop_eo_dag", "dwf_dhop_oe_axpy", "dwf_dhop_eo_axpy", "dwf_dhop_oe_norm2", "dwf_dhop_eo_norm2", "dwf_norm2", "dwf_inner_product", "dwf_field_bytes",
     "dwf_import_spinor", "dwf_export_spinor", "dwf_launch_count", "dwf_set_option",
     "dwf_error_string", "dwf_last_error",
 )
@@ -58,6 +58,8 @@ def load(build_if_missing: bool = True):
     for f in (lib.dwf_dhop, lib.dwf_dhop_oe, lib.dwf_dhop_eo, lib.dwf_dhop_dag, lib.dwf_dhop_oe_dag, lib.dwf_dhop_eo_dag):
         f.argtypes = [vp, vp, vp, vp]
     lib.dwf_norm2.argtypes = [vp, vp, ci, ctypes.POINTER(ctypes.c_double), vp]
+    for f in (lib.dwf_dhop_oe_axpy, lib.dwf_dhop_eo_axpy):
+        f.argtypes = [vp, vp, vp, ctypes.c_double, ctypes.c_double, vp, vp]
     for f in (lib.dwf_dhop_oe_norm2, lib.dwf_dhop_eo_norm2):
         f.argtypes = [vp, vp, vp, ctypes.POINTER(ctypes.c_double), vp]
     lib.dwf_inner_product.argtypes = [vp, vp, vp, ci, ctypes.POINTER(ctypes.c_double), vp]
@@ -152,6 +154,16 @@ def dwf_dhop_oe_dag(g: int, in_even, out_odd, stream=None) -> None:
 
 def dwf_dhop_eo_dag(g: int, in_odd, out_even, stream=None) -> None:
     _check(load().dwf_dhop_eo_dag(g, _dev_ptr(in_odd), _dev_ptr(out_even), _stream(stream)), "dwf_dhop_eo_dag")
+
+
+def dwf_dhop_oe_axpy(g: int, in_even, x_odd, a: float, b: float, out_odd, stream=None) -> None:
+    _check(load().dwf_dhop_oe_axpy(g, _dev_ptr(in_even), _dev_ptr(x_odd), float(a), float(b), _dev_ptr(out_odd),
+                                   _stream(stream)), "dwf_dhop_oe_axpy")
+
+
+def dwf_dhop_eo_axpy(g: int, in_odd, x_even, a: float, b: float, out_even, stream=None) -> None:
+    _check(load().dwf_dhop_eo_axpy(g, _dev_ptr(in_odd), _dev_ptr(x_even), float(a), float(b), _dev_ptr(out_even),
+                                   _stream(stream)), "dwf_dhop_eo_axpy")
 
 
 def dwf_dhop_oe_norm2(g: int, in_even, out_odd, stream=None) -> float:
@@ -294,6 +306,18 @@ class Geometry:
     def dhop_eo(self, in_odd, out=None, stream=None):
         out = self.new_field(EVEN) if out is None else out
         dwf_dhop_eo(self.handle, in_odd, out, stream)
+        return out
+
+    def dhop_oe_axpy(self, in_even, x_odd, a, b, out=None, stream=None):
+        """out = a x + b DhopOE in (x, out odd half fields; x may be out on the fused path)."""
+        out = self.new_field(ODD) if out is None else out
+        dwf_dhop_oe_axpy(self.handle, in_even, x_odd, a, b, out, stream)
+        return out
+
+    def dhop_eo_axpy(self, in_odd, x_even, a, b, out=None, stream=None):
+        """out = a x + b DhopEO in (x, out even half fields)."""
+        out = self.new_field(EVEN) if out is None else out
+        dwf_dhop_eo_axpy(self.handle, in_odd, x_even, a, b, out, stream)
         return out
 
     def dhop_oe_norm2(self, in_even, out=None, stream=None):

@@ -428,6 +428,39 @@ int dwf_dhop_eo_norm2(const dwf_geometry *g, const void *in_odd, void *out_even,
     return dhop_norm2_common(g, in_odd, out_even, DWF_EVEN, result_host, stream, "dwf_dhop_eo_norm2");
 }
 
+// out = a x + b (D in) on half fields: one pass in the staged kernel, Dhop then axpby otherwise
+static int dhop_axpy_common(const dwf_geometry *g, const void *in, const void *x, double a, double b, void *out,
+                            int parity_out, void *stream, const char *who)
+{
+    if (!g || !in || !x || !out) { set_error("%s: NULL argument", who); return DWF_ERR_INVALID_ARG; }
+    if (in == out || in == x) { set_error("%s: `in` must differ from `x` and `out` (x == out is allowed)", who); return DWF_ERR_INVALID_ARG; }
+    if (!aligned16(in) || !aligned16(out) || !aligned16(x)) { set_error("%s: field pointers must be 16-byte aligned", who); return DWF_ERR_INVALID_ARG; }
+    if (!g->gauge_loaded) { set_error("%s: call dwf_load_gauge first", who); return DWF_ERR_NO_GAUGE; }
+    DeviceGuard guard(g->device);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const bool staged_ok = g->staged.variant >= 0;
+    if (g->opt_kernel == 2 && !(staged_ok && staged_supports_axpy(g))) {
+        set_error("the staged kernel does not support the fused axpy for this geometry / precision");
+        return DWF_ERR_UNSUPPORTED;
+    }
+    if (staged_ok && g->opt_kernel != 1 && staged_supports_axpy(g))
+        return launch_dhop_staged(g, in, out, parity_out, st, nullptr, nullptr, false, x, (float)a, (float)b);
+    // two passes: out = D in, then out = a x + b out (x == out would be overwritten by the first pass)
+    if (x == out) { set_error("%s: x == out needs the fused kernel, which this geometry / precision does not have", who); return DWF_ERR_UNSUPPORTED; }
+    int rc = half_dhop(g, in, out, parity_out, st);
+    if (rc) return rc;
+    return launch_axpby(g, x, out, a, b, dwf_field_bytes(g, parity_out) / (size_t)g->prec, st);
+}
+
+int dwf_dhop_oe_axpy(const dwf_geometry *g, const void *in_even, const void *x_odd, double a, double b, void *out_odd, void *stream)
+{
+    return dhop_axpy_common(g, in_even, x_odd, a, b, out_odd, DWF_ODD, stream, "dwf_dhop_oe_axpy");
+}
+int dwf_dhop_eo_axpy(const dwf_geometry *g, const void *in_odd, const void *x_even, double a, double b, void *out_even, void *stream)
+{
+    return dhop_axpy_common(g, in_odd, x_even, a, b, out_even, DWF_EVEN, stream, "dwf_dhop_eo_axpy");
+}
+
 int dwf_norm2(const dwf_geometry *g, const void *field, int parity, double *result_host, void *stream)
 {
     if (!g || !field || !result_host || !parity_ok(parity)) { set_error("dwf_norm2: bad argument"); return DWF_ERR_INVALID_ARG; }

@@ -77,6 +77,7 @@ struct StagedArgs {
     int zigzag;              // walk the slices of every other tile backwards
     int layered;             // one TMA box per x3 layer (per-layer L2 policies) instead of one per region
     int prefetch;            // producer prefetches the input of step g + prefetch into L2 (0: off); bit 4..: box mask
+    float axpy_a, axpy_b;    // AXPY kernels: out = a x + b Dhop in
     double *norm_partials;   // NORM kernels: one partial sum of |out|^2 per CTA (fixed order inside the CTA)
     int ablate;              // timing experiments only (wrong results): 1 no link refill, 2 no stores, 4 no legs, 8 no TMA
 };
@@ -232,19 +233,23 @@ __device__ __forceinline__ void staged_leg(float2 (&acc)[12], const float4 *__re
 // MODE 0: Dhop.  MODE 1 (NORM): also accumulate |out|^2 (fp64, fixed order) and write one partial per
 // CTA -- norm2 of the result fused into the kernel that produces it (saves re-reading the output
 // field).  MODE 2 (DAG): Dhop^dagger = the projectors (1 - gamma) and (1 + gamma) change places, same
-// links and neighbours.
+// links and neighbours.  MODE 3 (AXPY): out = a x + b Dhop in, with x a field of the
+// output parity staged by TMA next to the input slice and combined in the store epilogue (the
+// Wilson-matrix fusion of SURVEY.md 8(f1): one pass instead of Dhop followed by an axpy).
 template <int LH, int B1, int B2, int B3, int MODE>
 __global__ void __launch_bounds__(StagedCfg<LH, B1, B2, B3>::NT, StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM)
 dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_x1,
                    const __grid_constant__ CUtensorMap map_x2, const __grid_constant__ CUtensorMap map_x3,
                    const __grid_constant__ CUtensorMap map_x1l, const __grid_constant__ CUtensorMap map_x2l,
-                   const StagedArgs args)
+                   const __grid_constant__ CUtensorMap map_xc, const StagedArgs args)
 {
     using Cfg = StagedCfg<LH, B1, B2, B3>;
-    constexpr bool NORM = MODE == 1, DAG = MODE == 2;
+    constexpr bool NORM = MODE == 1, DAG = MODE == 2, AXPY = MODE == 3;
+    // MODE 3 stages the rows box of the field x as well (read in the epilogue): NROW_C more rows per stage
+    constexpr int STAGE = Cfg::STAGE_BYTES + (AXPY ? Cfg::NROW_C * Cfg::ROWB : 0);
     extern __shared__ __align__(1024) unsigned char smem[];
     const uint32_t smem_base = smem_u32(smem);
-    const uint32_t full_base = smem_base + Cfg::NSTAGE * Cfg::STAGE_BYTES;      // full[stage][region]: TMA data has landed
+    const uint32_t full_base = smem_base + Cfg::NSTAGE * STAGE;      // full[stage][region]: TMA data has landed
     const uint32_t empty_base = full_base + 64;                                 // empty[stage][region]: every consumer warp is done
 
     const int tid = threadIdx.x;
@@ -260,10 +265,10 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         return;
     }
     // L2 policies of the TMA copies, read by the producer thread from shared memory
-    uint64_t *pol = reinterpret_cast<uint64_t *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + Cfg::TAIL_POL);
+    uint64_t *pol = reinterpret_cast<uint64_t *>(smem + Cfg::NSTAGE * STAGE + Cfg::TAIL_POL);
     // origins of this CTA's first NORIG tiles: read once, so that neither the producer nor the
     // tile switch waits on a global load
-    int4 *orig = reinterpret_cast<int4 *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + Cfg::TAIL_ORIG);
+    int4 *orig = reinterpret_cast<int4 *>(smem + Cfg::NSTAGE * STAGE + Cfg::TAIL_ORIG);
     for (int it = tid; it < my_tiles && it < Cfg::NORIG; it += Cfg::NT) orig[it] = args.tiles[group + it * ngroup];
     auto tile_origin = [&](int it) -> int4 { return it < Cfg::NORIG ? orig[it] : args.tiles[group + it * ngroup]; };
     if (tid == 0) {
@@ -322,7 +327,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
                 }
             }
             const Boxes b = boxes(g);
-            const uint32_t dst = smem_base + stage * Cfg::STAGE_BYTES;
+            const uint32_t dst = smem_base + stage * STAGE;
             const uint32_t fb = full_base + 32 * stage, eb = empty_base + 32 * stage;
             constexpr uint32_t FS = DWF_SYNC_MODE == 0 ? 8 : 0;      // stride of the per-region full barriers
             const uint32_t epar = ((g >> 1) - 1) & 1;
@@ -370,7 +375,9 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             if (g >= 2) mbar_wait(eb + 24, epar);
             if (notma) mbar_arrive(fb + 3 * FS);
             else {
-                mbar_arrive_expect_tx(fb + 3 * FS, Cfg::NROW_C * Cfg::ROWB);
+                mbar_arrive_expect_tx(fb + 3 * FS, (AXPY ? 2 : 1) * Cfg::NROW_C * Cfg::ROWB);
+                if constexpr (AXPY)         // rows box of x for this slice, behind the input rows of the stage
+                    tma_load_5d_hint(dst + Cfg::STAGE_BYTES, &map_xc, fb + 3 * FS, 0, 0, b.o1, b.o2, b.c4, pol[PC_X3M]);
                 if (args.layered) {
 #pragma unroll
                     for (int j = 0; j < B3; j++)
@@ -451,7 +458,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     double nsum = 0.0;          // NORM: this thread's share of |out|^2
     auto step = [&](auto fetch_tag, int stage, uint32_t par, float4 *o, const float4 *gnext) {
         constexpr bool FETCH = decltype(fetch_tag)::value;
-        const unsigned char *sb = smem + stage * Cfg::STAGE_BYTES;
+        const unsigned char *sb = smem + stage * STAGE;
         const uint32_t fb = full_base + 32 * stage, eb = empty_base + 32 * stage;
         const bool legs = !(args.ablate & 4);
         float2 acc[12];
@@ -462,6 +469,19 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
                 const float4 q = ldg128_hint(gnext + j * LH, pol_g);                                \
                 U[2 * j] = make_float2(q.x, q.y);                                                   \
                 U[2 * j + 1] = make_float2(q.z, q.w);                                               \
+            }                                                                                       \
+        }
+        // AXPY: acc <- a x + b acc with x out of the stage (before the centre region is released)
+#define DWF_AXPY_EPILOGUE                                                                           \
+        if constexpr (AXPY) {                                                                       \
+            if (legs) {                                                                             \
+                const float4 *xr = reinterpret_cast<const float4 *>(sb + Cfg::STAGE_BYTES) + row * (Cfg::ROWB / 16) + h; \
+                const float2 ca = make_float2(args.axpy_a, args.axpy_a), cb = make_float2(args.axpy_b, args.axpy_b); \
+                _Pragma("unroll") for (int j = 0; j < 6; j++) {                                      \
+                    const float4 xv = xr[j * LH];                                                   \
+                    acc[2 * j] = f2_fma(cb, acc[2 * j], f2_mul(ca, make_float2(xv.x, xv.y)));        \
+                    acc[2 * j + 1] = f2_fma(cb, acc[2 * j + 1], f2_mul(ca, make_float2(xv.z, xv.w))); \
+                }                                                                                   \
             }                                                                                       \
         }
 #define DWF_RELEASE(R)                                                                              \
@@ -495,6 +515,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             DWF_LEG(0, 0, true,  false)
             DWF_LEG(1, 0, false, false)
         }
+        DWF_AXPY_EPILOGUE
         DWF_RELEASE(3)
 #else                           /* wait for the whole stage first: the legs form one block the compiler may software-pipeline */
         mbar_wait(fb, par);
@@ -517,6 +538,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             DWF_LEG(0, 0, true,  false)
             DWF_LEG(1, 0, false, false)
         }
+        DWF_AXPY_EPILOGUE
 #if DWF_SYNC_MODE == 1
         if (!legs) { DWF_RELEASE(0) DWF_RELEASE(1) DWF_RELEASE(2) }
         DWF_RELEASE(3)
@@ -527,6 +549,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
 #undef DWF_LEG
 #undef DWF_RELEASE
 #undef DWF_RELEASE_DEP
+#undef DWF_AXPY_EPILOGUE
         // Last slice of the tile: refill the links for the next tile, all at once and in the
         // order the next step uses them (legs 6, 7, 4, 5, 2, 3, 0, 1).  Spreading the loads over
         // the legs of this step made later legs wait on the scoreboard the loads share.
@@ -585,7 +608,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         double v = nsum;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        double *slots = reinterpret_cast<double *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + Cfg::TAIL_NORM);
+        double *slots = reinterpret_cast<double *>(smem + Cfg::NSTAGE * STAGE + Cfg::TAIL_NORM);
         if ((ctid & 31) == 0) slots[ctid >> 5] = v;
         asm volatile("bar.sync 1, %0;" ::"n"(Cfg::NWARP_C * 32) : "memory");      // consumer warps only
         if (ctid == 0) {
@@ -611,6 +634,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
 const void *const *staged_kernels_mode0();
 const void *const *staged_kernels_mode1();
 const void *const *staged_kernels_mode2();
+const void *const *staged_kernels_mode3();
 
 #define DWF_CAT2(a, b) a##b
 #define DWF_CAT(a, b) DWF_CAT2(a, b)
@@ -629,17 +653,20 @@ const void *const *DWF_CAT(staged_kernels_mode, DWF_STAGED_MODE)()
 struct Variant {
     int lh, b1, b2, b3;
     int smem, threads, ctas_per_sm;
-    const void *fn[3];       // MODE 0 (Dhop), 1 (Dhop + norm2), 2 (Dhop^dagger)
+    const void *fn[4];       // MODE 0 (Dhop), 1 (Dhop + norm2), 2 (Dhop^dagger), 3 (a x + b Dhop)
+    int smem_axpy;           // MODE 3 stages the rows box of x as well
 };
 
 static const std::vector<Variant> &variants()
 {
     static const std::vector<Variant> v = [] {
         std::vector<Variant> t;
-        const void *const *k0 = staged_kernels_mode0(), *const *k1 = staged_kernels_mode1(), *const *k2 = staged_kernels_mode2();
+        const void *const *k0 = staged_kernels_mode0(), *const *k1 = staged_kernels_mode1(), *const *k2 = staged_kernels_mode2(),
+                          *const *k3 = staged_kernels_mode3();
 #define X(LH, B1, B2, B3)                                                                            \
         t.push_back({LH, B1, B2, B3, StagedCfg<LH, B1, B2, B3>::SMEM_BYTES, StagedCfg<LH, B1, B2, B3>::NT,  \
-                     StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM, {k0[t.size()], k1[t.size()], k2[t.size()]}});
+                     StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM, {k0[t.size()], k1[t.size()], k2[t.size()], k3[t.size()]},    \
+                     StagedCfg<LH, B1, B2, B3>::SMEM_BYTES + 2 * StagedCfg<LH, B1, B2, B3>::NROW_C * StagedCfg<LH, B1, B2, B3>::ROWB});
         DWF_STAGED_VARIANTS(X)
 #undef X
         return t;
@@ -715,34 +742,57 @@ static int encode_map(CUtensorMap *m, const void *base, const Lattice &lat, int 
     return DWF_OK;
 }
 
-int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st,
-                       double *norm_partials, int *norm_blocks, bool dagger)
+// The six tensor maps of a field depend on its pointer and the tile shape only.  A solver applies the
+// operator to the same few buffers over and over, so the encoded maps are kept in a small
+// per-thread cache (keyed by geometry id, variant and pointer): no driver calls on a hit.
+struct MapSet { unsigned long long gid; int variant; const void *ptr; CUtensorMap m[6]; };
+
+static int get_maps(const dwf_geometry *g, const Variant &v, const void *ptr, MapSet **out)
 {
-    if (dagger && norm_partials) { set_error("no fused norm2 for the dagger kernel"); return DWF_ERR_UNSUPPORTED; }
-    const Variant &v = variants()[(size_t)g->staged.variant];
-    // The six tensor maps depend on the input pointer and the tile shape only.  A solver applies the
-    // operator to the same few buffers over and over, so the encoded maps are kept in a small
-    // per-thread cache (keyed by geometry id, variant and pointer): no driver calls on a hit.
-    struct MapSet { unsigned long long gid; int variant; const void *in; CUtensorMap m[6]; };
     static thread_local MapSet cache[8];
     static thread_local unsigned next_slot = 0;
-    MapSet *ms = nullptr;
     for (MapSet &c : cache)
-        if (c.in == in && c.gid == g->uid && c.variant == g->staged.variant) { ms = &c; break; }
-    if (!ms) {
-        MapSet t;
-        t.gid = g->uid; t.variant = g->staged.variant; t.in = in;
-        int rc;
-        if ((rc = encode_map(&t.m[0], in, g->lat, v.b1, v.b2, v.b3))) return rc;
-        if ((rc = encode_map(&t.m[1], in, g->lat, 1, v.b2, v.b3))) return rc;
-        if ((rc = encode_map(&t.m[2], in, g->lat, v.b1, 1, v.b3))) return rc;
-        if ((rc = encode_map(&t.m[3], in, g->lat, v.b1, v.b2, 1))) return rc;
-        if ((rc = encode_map(&t.m[4], in, g->lat, 1, v.b2, 1))) return rc;
-        if ((rc = encode_map(&t.m[5], in, g->lat, v.b1, 1, 1))) return rc;
-        ms = &cache[next_slot++ % 8];
-        *ms = t;
+        if (c.ptr == ptr && c.gid == g->uid && c.variant == g->staged.variant) { *out = &c; return DWF_OK; }
+    MapSet t;
+    t.gid = g->uid; t.variant = g->staged.variant; t.ptr = ptr;
+    int rc;
+    if ((rc = encode_map(&t.m[0], ptr, g->lat, v.b1, v.b2, v.b3))) return rc;
+    if ((rc = encode_map(&t.m[1], ptr, g->lat, 1, v.b2, v.b3))) return rc;
+    if ((rc = encode_map(&t.m[2], ptr, g->lat, v.b1, 1, v.b3))) return rc;
+    if ((rc = encode_map(&t.m[3], ptr, g->lat, v.b1, v.b2, 1))) return rc;
+    if ((rc = encode_map(&t.m[4], ptr, g->lat, 1, v.b2, 1))) return rc;
+    if ((rc = encode_map(&t.m[5], ptr, g->lat, v.b1, 1, 1))) return rc;
+    MapSet *ms = &cache[next_slot++ % 8];
+    *ms = t;
+    *out = ms;
+    return DWF_OK;
+}
+
+static const int SMEM_LIMIT = 232448;       // 227 KB of dynamic shared memory per CTA on sm_100
+
+bool staged_supports_axpy(const dwf_geometry *g)
+{
+    return g->staged.variant >= 0 && variants()[(size_t)g->staged.variant].smem_axpy <= SMEM_LIMIT;
+}
+
+int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st,
+                       double *norm_partials, int *norm_blocks, bool dagger, const void *axpy_x, float axpy_a,
+                       float axpy_b)
+{
+    if ((dagger && norm_partials) || (axpy_x && (dagger || norm_partials))) {
+        set_error("the staged kernel has no instance for this combination of modes");
+        return DWF_ERR_UNSUPPORTED;
     }
+    const Variant &v = variants()[(size_t)g->staged.variant];
+    const int mode = norm_partials ? 1 : (dagger ? 2 : (axpy_x ? 3 : 0));
+    const int smem = mode == 3 ? v.smem_axpy : v.smem;
+    if (smem > SMEM_LIMIT) { set_error("tile too large for the fused axpy"); return DWF_ERR_UNSUPPORTED; }
+    MapSet *ms = nullptr, *mx = nullptr;
+    int rc;
+    if ((rc = get_maps(g, v, in, &ms))) return rc;
+    if ((rc = get_maps(g, v, axpy_x ? axpy_x : in, &mx))) return rc;
     CUtensorMap &mc = ms->m[0], &m1 = ms->m[1], &m2 = ms->m[2], &m3 = ms->m[3], &m1l = ms->m[4], &m2l = ms->m[5];
+    CUtensorMap &mxc = mx->m[0];
     StagedArgs a;
     a.out = static_cast<float2 *>(out);
     a.gauge = static_cast<const float2 *>(g->gauge[parity_out]);
@@ -756,22 +806,24 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     a.layered = g->opt_layered;
     a.ablate = g->opt_ablate;
     a.norm_partials = norm_partials;
+    a.axpy_a = axpy_a;
+    a.axpy_b = axpy_b;
     int ssplit = g->opt_ssplit > 0 ? g->opt_ssplit : 1;
-    const int slots = g->sm_count * v.ctas_per_sm;       // co-resident CTAs
+    const int ctas = (v.ctas_per_sm == 2 && 2 * (smem + 1024) > SMEM_LIMIT) ? 1 : v.ctas_per_sm;
+    const int slots = g->sm_count * ctas;       // co-resident CTAs
     while (ssplit > 1 && (g->lat.Ls % ssplit || slots % ssplit)) ssplit--;
     a.ssplit = ssplit;
-    const int mode = norm_partials ? 1 : (dagger ? 2 : 0);
     const void *fn = v.fn[mode];
-    static thread_local const void *attr_set_for[3] = {nullptr, nullptr, nullptr};
+    static thread_local const void *attr_set_for[4] = {nullptr, nullptr, nullptr, nullptr};
     if (attr_set_for[mode] != fn) {
-        DWF_CUDA_CHECK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, v.smem));
+        DWF_CUDA_CHECK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         attr_set_for[mode] = fn;
     }
     const int ngroup_max = slots / ssplit;
     const int ngroup = g->staged.ntiles < ngroup_max ? g->staged.ntiles : ngroup_max;
-    void *params[] = {&mc, &m1, &m2, &m3, &m1l, &m2l, &a};
+    void *params[] = {&mc, &m1, &m2, &m3, &m1l, &m2l, &mxc, &a};
     DWF_CUDA_CHECK(cudaLaunchKernel(fn, dim3((unsigned)(ngroup * ssplit)), dim3((unsigned)v.threads), params,
-                                    (size_t)v.smem, st));
+                                    (size_t)smem, st));
     if (norm_blocks) *norm_blocks = ngroup * ssplit;
     count_launch();
     return DWF_OK;

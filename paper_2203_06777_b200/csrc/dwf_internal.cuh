@@ -119,7 +119,11 @@ void plan_staged(dwf_geometry *g);                      // fills g->staged (vari
 void build_staged_tile_table(const dwf_geometry *g, int raster, int4 *host_table);
 // norm_partials != nullptr: the fused-norm2 kernel writes one partial of |out|^2 per CTA there, *norm_blocks = their number
 int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st,
-                       double *norm_partials = nullptr, int *norm_blocks = nullptr, bool dagger = false);
+                       double *norm_partials = nullptr, int *norm_blocks = nullptr, bool dagger = false,
+                       const void *axpy_x = nullptr, float axpy_a = 0.f, float axpy_b = 0.f);   // axpy_x: out = a x + b Dhop in
+bool staged_supports_axpy(const dwf_geometry *g);
+// pack.cu: out = a x + b out, elementwise over nreal reals (the unfused path of dwf_dhop_*_axpy)
+int launch_axpby(const dwf_geometry *g, const void *x, void *out, double a, double b, size_t nreal, cudaStream_t st);
 // reduce.cu
 int launch_norm2(const dwf_geometry *g, const void *field, size_t nreal, cudaStream_t st);
 int launch_final_sum(const dwf_geometry *g, int nblocks, cudaStream_t st);   // result_dev[0] = sum of partials[0..nblocks)

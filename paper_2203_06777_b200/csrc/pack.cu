@@ -177,4 +177,36 @@ int launch_export(const dwf_geometry *g, const void *field, int parity, void *ca
     return launch_reorder<false>(g, field, canonical_dev, parity, st);
 }
 
+// out = a x + b out over nreal reals (128-bit vectors; nreal is a multiple of 24).  The unfused path of
+// dwf_dhop_oe_axpy / dwf_dhop_eo_axpy (fp64, shapes without a staged variant); x may be out.
+template <typename T>
+__global__ void __launch_bounds__(256)
+axpby_kernel(const T *__restrict__ x, T *__restrict__ out, const T a, const T b, const size_t nvec)
+{
+    using V = typename std::conditional<sizeof(T) == 4, float4, double2>::type;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+        const V p = reinterpret_cast<const V *>(x)[i];
+        V q = reinterpret_cast<V *>(out)[i];
+        q.x = fma(b, q.x, a * p.x);
+        q.y = fma(b, q.y, a * p.y);
+        if constexpr (sizeof(T) == 4) {
+            q.z = fma(b, q.z, a * p.z);
+            q.w = fma(b, q.w, a * p.w);
+        }
+        reinterpret_cast<V *>(out)[i] = q;
+    }
+}
+
+int launch_axpby(const dwf_geometry *g, const void *x, void *out, double a, double b, size_t nreal, cudaStream_t st)
+{
+    const int nb = g->sm_count * 8;
+    if (g->prec == DWF_F32)
+        axpby_kernel<float><<<nb, 256, 0, st>>>(static_cast<const float *>(x), static_cast<float *>(out), (float)a, (float)b, nreal / 4);
+    else
+        axpby_kernel<double><<<nb, 256, 0, st>>>(static_cast<const double *>(x), static_cast<double *>(out), a, b, nreal / 2);
+    count_launch();
+    DWF_CUDA_CHECK(cudaGetLastError());
+    return DWF_OK;
+}
+
 }  // namespace dwf

@@ -252,3 +252,15 @@ def test_dagger_even_odd_reassembly(dims, Ls, bc):
         half = gen.split_parity(psi, dims, 1 - p_out)
         got = oracle.dhop_cb(dims, Ls, bc, p_out, U, half, dagger=True)
         assert rel_err(got, full[par == p_out]) < 1e-15
+
+
+def test_wilson_combination_is_the_dense_matrix_a_plus_b_dhop():
+    """a x + b Dhop x, as the GPU's fused axpy tests form it from the oracle, against (a 1 + b D) x."""
+    dims, Ls, bc = (4, 2, 4, 2), 2, oracle.ANTIPERIODIC_T
+    V = int(np.prod(dims))
+    U = gen.gauge_random(dims, seed=31)
+    psi = gen.spinor_gaussian(V, Ls, seed=31)
+    a, b = 4.3, -0.5
+    D = dense_dhop_matrix(dims, U, True)
+    M = a * np.eye(D.shape[0]) + b * D
+    assert rel_err(a * psi + b * oracle.dhop(dims, Ls, bc, U, psi), apply_dense(M, psi)) < 1e-14
