@@ -218,7 +218,8 @@ int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, i
     bool ok = cudaMalloc(&g->gauge[0], g->gauge_bytes) == cudaSuccess &&
               cudaMalloc(&g->gauge[1], g->gauge_bytes) == cudaSuccess &&
               cudaMalloc(&g->partials, sizeof(double) * 2 * (size_t)g->reduce_blocks) == cudaSuccess &&
-              cudaMalloc(&g->result_dev, sizeof(double) * 2) == cudaSuccess;
+              cudaMalloc(&g->result_dev, sizeof(double) * 2) == cudaSuccess &&
+              cudaHostAlloc(&g->result_pinned, sizeof(double) * 2, cudaHostAllocDefault) == cudaSuccess;
     if (!ok || rebuild_tilings(g) != DWF_OK) {
         cudaGetLastError();
         if (ok == false) set_error("device allocation failed (gauge %zu bytes x 2)", g->gauge_bytes);
@@ -237,6 +238,7 @@ int dwf_destroy_geometry(dwf_geometry *g)
     cudaFree(g->gauge[1]);
     cudaFree(g->partials);
     cudaFree(g->result_dev);
+    cudaFreeHost(g->result_pinned);
     cudaFree(g->tiles_cb);
     cudaFree(g->tiles_staged);
     cudaFree(g->staging);
@@ -412,10 +414,10 @@ static int dhop_norm2_common(const dwf_geometry *g, const void *in, void *out, i
         rc = launch_norm2(g, out, dwf_field_bytes(g, parity_out) / (size_t)g->prec, st);
     }
     if (rc) return rc;
-    double r = 0;
-    DWF_CUDA_CHECK(cudaMemcpyAsync(&r, g->result_dev, sizeof(double), cudaMemcpyDeviceToHost, st));
+    // through the geometry's pinned word: a pageable destination would make the copy a staged, blocking one
+    DWF_CUDA_CHECK(cudaMemcpyAsync(g->result_pinned, g->result_dev, sizeof(double), cudaMemcpyDeviceToHost, st));
     DWF_CUDA_CHECK(cudaStreamSynchronize(st));
-    *result_host = r;
+    *result_host = g->result_pinned[0];
     return DWF_OK;
 }
 
@@ -469,10 +471,10 @@ int dwf_norm2(const dwf_geometry *g, const void *field, int parity, double *resu
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int rc = launch_norm2(g, field, dwf_field_bytes(g, parity) / (size_t)g->prec, st);
     if (rc) return rc;
-    double r = 0;
-    DWF_CUDA_CHECK(cudaMemcpyAsync(&r, g->result_dev, sizeof(double), cudaMemcpyDeviceToHost, st));
+    // through the geometry's pinned word: a pageable destination would make the copy a staged, blocking one
+    DWF_CUDA_CHECK(cudaMemcpyAsync(g->result_pinned, g->result_dev, sizeof(double), cudaMemcpyDeviceToHost, st));
     DWF_CUDA_CHECK(cudaStreamSynchronize(st));
-    *result_host = r;
+    *result_host = g->result_pinned[0];
     return DWF_OK;
 }
 
@@ -484,11 +486,10 @@ int dwf_inner_product(const dwf_geometry *g, const void *a, const void *b, int p
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int rc = launch_inner(g, a, b, dwf_field_bytes(g, parity) / (size_t)g->prec / 2, st);
     if (rc) return rc;
-    double r[2] = {0, 0};
-    DWF_CUDA_CHECK(cudaMemcpyAsync(r, g->result_dev, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    DWF_CUDA_CHECK(cudaMemcpyAsync(g->result_pinned, g->result_dev, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
     DWF_CUDA_CHECK(cudaStreamSynchronize(st));
-    result_host[0] = r[0];
-    result_host[1] = r[1];
+    result_host[0] = g->result_pinned[0];
+    result_host[1] = g->result_pinned[1];
     return DWF_OK;
 }
 

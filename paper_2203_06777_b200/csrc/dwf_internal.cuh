@@ -82,6 +82,7 @@ struct dwf_geometry {
     // reductions
     double *partials;       // [2 * max_blocks]
     double *result_dev;     // [2]
+    double *result_pinned;  // [2] pinned host words the reductions are copied into
     int reduce_blocks;
     // host-side staging for canonical <-> device conversions (lazily grown)
     void *staging;
