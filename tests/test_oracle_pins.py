@@ -264,3 +264,21 @@ def test_wilson_combination_is_the_dense_matrix_a_plus_b_dhop():
     D = dense_dhop_matrix(dims, U, True)
     M = a * np.eye(D.shape[0]) + b * D
     assert rel_err(a * psi + b * oracle.dhop(dims, Ls, bc, U, psi), apply_dense(M, psi)) < 1e-14
+
+
+def test_golden_fixture():
+    """tests/golden/dhop_2x2x2x2.txt (written by tests/golden/make_golden.py from the oracle alone):
+    the oracle still produces it, and the stored numbers satisfy the dense-matrix pin themselves."""
+    import os
+    here = os.path.dirname(os.path.abspath(__file__))
+    stored = np.loadtxt(os.path.join(here, "golden", "dhop_2x2x2x2.txt"))
+    dims, Ls, seed = (2, 2, 2, 2), 1, 2203
+    U = gen.gauge_random(dims, seed)
+    psi = gen.spinor_gaussian(16, Ls, seed)
+    d = oracle.dhop(dims, Ls, oracle.ANTIPERIODIC_T, U, psi)
+    dd = oracle.dhop(dims, Ls, oracle.ANTIPERIODIC_T, U, psi, dagger=True)
+    assert np.allclose(stored[:, 0], d.ravel(), rtol=0, atol=1e-14)
+    assert np.allclose(stored[:, 1], dd.ravel(), rtol=0, atol=1e-14)
+    D = dense_dhop_matrix(dims, U, True)
+    assert rel_err(stored[:, 0].reshape(d.shape), apply_dense(D, psi)) < 1e-14
+    assert rel_err(stored[:, 1].reshape(d.shape), apply_dense(D.conj().T, psi)) < 1e-14
