@@ -334,6 +334,25 @@ def run_gpu(args, w):
     e2e_val = whole_job_gflops(world, sites, ms_e2e)
     field_bytes = psi_e.nbytes
 
+    # ---- optional: the NEXT-row kernels of SURVEY.md 8(f1), each event-timed on its own ----
+    extra = None
+    if args.extra_ops:
+        def timed(fn, n=20):
+            fn()
+            e_a, e_b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e_a.record()
+            for _ in range(n):
+                fn()
+            e_b.record()
+            torch.cuda.synchronize()
+            return e_a.elapsed_time(e_b) / n
+        t_dag = timed(lambda: g.dhop_eo_dag(f_mid, f_out))
+        t_axpy = timed(lambda: g.dhop_eo_axpy(f_mid, f_in, 1.0, -0.25 / (4.3 * 4.3), f_out))
+        mb_axpy = model_bytes_cb(w) + sites * 24 * prec          # + one read of x
+        extra = {"dhop_eo_dag_ms": t_dag, "dhop_eo_axpy_ms": t_axpy,
+                 "axpy_algorithmic_bytes_per_launch": mb_axpy,
+                 "note": "a x + b DhopEO in one pass; model = half-Dhop model + one read of x"}
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -364,6 +383,10 @@ def run_gpu(args, w):
                      "algorithmic_bytes_per_launch": mb,
                      "traffic": NCU_TRAFFIC_BYTES.get(args.workload)},
     }
+    if extra is not None:
+        extra["dag_roofline_frac"] = mb / (extra["dhop_eo_dag_ms"] * 1e-3) / 1e9 / peak
+        extra["axpy_roofline_frac"] = extra["axpy_algorithmic_bytes_per_launch"] / (extra["dhop_eo_axpy_ms"] * 1e-3) / 1e9 / peak
+        line["next_rows"] = extra
     if world == 1 and not args.no_cpu:
         cb = cpu_baseline(w, U, psi_e)
         line["cpu_baseline"] = cb
@@ -383,6 +406,8 @@ def main():
     ap.add_argument("--impl", default="dwf", choices=["dwf", "reference"])
     ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--extra-ops", action="store_true",
+                    help="also time Dhop^dagger and the fused a x + b Dhop (SURVEY.md 8(f1)); adds `next_rows` to the line")
     ap.add_argument("--opt", action="append", help="kernel tunable key=value (dwf_set_option)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "dwf" else args.warmup
