@@ -219,7 +219,9 @@ int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, i
               cudaMalloc(&g->gauge[1], g->gauge_bytes) == cudaSuccess &&
               cudaMalloc(&g->partials, sizeof(double) * 2 * (size_t)g->reduce_blocks) == cudaSuccess &&
               cudaMalloc(&g->result_dev, sizeof(double) * 2) == cudaSuccess &&
-              cudaHostAlloc(&g->result_pinned, sizeof(double) * 2, cudaHostAllocDefault) == cudaSuccess;
+              cudaHostAlloc(&g->mailbox_host, sizeof(double) * 4, cudaHostAllocMapped) == cudaSuccess &&
+              cudaHostGetDevicePointer(&g->mailbox_dev, g->mailbox_host, 0) == cudaSuccess;
+    if (ok) memset(g->mailbox_host, 0, sizeof(double) * 4);
     if (!ok || rebuild_tilings(g) != DWF_OK) {
         cudaGetLastError();
         if (ok == false) set_error("device allocation failed (gauge %zu bytes x 2)", g->gauge_bytes);
@@ -238,7 +240,7 @@ int dwf_destroy_geometry(dwf_geometry *g)
     cudaFree(g->gauge[1]);
     cudaFree(g->partials);
     cudaFree(g->result_dev);
-    cudaFreeHost(g->result_pinned);
+    cudaFreeHost(g->mailbox_host);
     cudaFree(g->tiles_cb);
     cudaFree(g->tiles_staged);
     cudaFree(g->staging);
@@ -386,6 +388,28 @@ int dwf_dhop_eo_dag(const dwf_geometry *g, const void *in_odd, void *out_even, v
     return dhop_common(g, in_odd, out_even, DWF_EVEN, stream, "dwf_dhop_eo_dag", true);
 }
 
+// Waits for the reduction last enqueued on `st` and returns its n values.  The final-sum kernel
+// writes them into mapped host memory followed by its sequence number, so the host polls that
+// word instead of paying a device-to-host copy plus a stream synchronise; cudaStreamQuery is
+// consulted now and then so that a failed launch surfaces as an error instead of a hang.  When the
+// sequence number is visible every earlier operation of the stream has completed (in-order stream).
+static int fetch_reduction(const dwf_geometry *g, cudaStream_t st, int n, double *out)
+{
+    const unsigned long long want = g->mailbox_seq;
+    volatile unsigned long long *seq = reinterpret_cast<volatile unsigned long long *>(g->mailbox_host + 2);
+    for (unsigned long long spins = 1; *seq != want; spins++) {
+        if ((spins & 0x3fff) == 0) {
+            cudaError_t e = cudaStreamQuery(st);
+            if (e == cudaSuccess) break;               // stream drained: the values are there
+            if (e != cudaErrorNotReady) { set_error("reduction failed: %s", cudaGetErrorString(e)); return DWF_ERR_CUDA; }
+        }
+    }
+    std::atomic_thread_fence(std::memory_order_acquire);
+    if (*seq != want) DWF_CUDA_CHECK(cudaStreamSynchronize(st));
+    for (int i = 0; i < n; i++) out[i] = const_cast<const volatile double *>(g->mailbox_host)[i];
+    return DWF_OK;
+}
+
 // out = D in on half fields and *result_host = norm2(out): the reduction runs in the epilogue of the
 // Dhop kernel (staged path) or as a second pass over `out` (direct path)
 static int dhop_norm2_common(const dwf_geometry *g, const void *in, void *out, int parity_out, double *result_host,
@@ -414,11 +438,7 @@ static int dhop_norm2_common(const dwf_geometry *g, const void *in, void *out, i
         rc = launch_norm2(g, out, dwf_field_bytes(g, parity_out) / (size_t)g->prec, st);
     }
     if (rc) return rc;
-    // through the geometry's pinned word: a pageable destination would make the copy a staged, blocking one
-    DWF_CUDA_CHECK(cudaMemcpyAsync(g->result_pinned, g->result_dev, sizeof(double), cudaMemcpyDeviceToHost, st));
-    DWF_CUDA_CHECK(cudaStreamSynchronize(st));
-    *result_host = g->result_pinned[0];
-    return DWF_OK;
+    return fetch_reduction(g, st, 1, result_host);
 }
 
 int dwf_dhop_oe_norm2(const dwf_geometry *g, const void *in_even, void *out_odd, double *result_host, void *stream)
@@ -471,11 +491,7 @@ int dwf_norm2(const dwf_geometry *g, const void *field, int parity, double *resu
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int rc = launch_norm2(g, field, dwf_field_bytes(g, parity) / (size_t)g->prec, st);
     if (rc) return rc;
-    // through the geometry's pinned word: a pageable destination would make the copy a staged, blocking one
-    DWF_CUDA_CHECK(cudaMemcpyAsync(g->result_pinned, g->result_dev, sizeof(double), cudaMemcpyDeviceToHost, st));
-    DWF_CUDA_CHECK(cudaStreamSynchronize(st));
-    *result_host = g->result_pinned[0];
-    return DWF_OK;
+    return fetch_reduction(g, st, 1, result_host);
 }
 
 int dwf_inner_product(const dwf_geometry *g, const void *a, const void *b, int parity, double result_host[2], void *stream)
@@ -486,11 +502,7 @@ int dwf_inner_product(const dwf_geometry *g, const void *a, const void *b, int p
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int rc = launch_inner(g, a, b, dwf_field_bytes(g, parity) / (size_t)g->prec / 2, st);
     if (rc) return rc;
-    DWF_CUDA_CHECK(cudaMemcpyAsync(g->result_pinned, g->result_dev, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-    DWF_CUDA_CHECK(cudaStreamSynchronize(st));
-    result_host[0] = g->result_pinned[0];
-    result_host[1] = g->result_pinned[1];
-    return DWF_OK;
+    return fetch_reduction(g, st, 2, result_host);
 }
 
 int dwf_import_spinor(const dwf_geometry *g, const void *canonical, int src_is_device, int parity, void *field_dev, void *stream)

@@ -82,7 +82,9 @@ struct dwf_geometry {
     // reductions
     double *partials;       // [2 * max_blocks]
     double *result_dev;     // [2]
-    double *result_pinned;  // [2] pinned host words the reductions are copied into
+    double *mailbox_host;   // mapped pinned host memory: [0..1] values, [2] sequence number of the reduction that wrote them
+    double *mailbox_dev;    // the same words as the device sees them
+    unsigned long long mailbox_seq;   // last sequence number handed to a reduction
     int reduce_blocks;
     // host-side staging for canonical <-> device conversions (lazily grown)
     void *staging;

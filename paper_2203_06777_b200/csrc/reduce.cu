@@ -100,10 +100,13 @@ inner_partial_kernel(const T *__restrict__ a, const T *__restrict__ b, size_t nc
     }
 }
 
-// one CTA: result[i] = sum over blocks of partials[NV*block + i], fixed order
+// one CTA: result[i] = sum over blocks of partials[NV*block + i], fixed order.  The result also goes
+// straight into the geometry's mapped host mailbox (values, then a sequence number behind a
+// system-scope fence), so that the host can pick it up without a copy and a stream synchronise.
 template <int NV>
 __global__ void __launch_bounds__(256)
-final_sum_kernel(const double *__restrict__ partials, int nblocks, double *__restrict__ result)
+final_sum_kernel(const double *__restrict__ partials, int nblocks, double *__restrict__ result,
+                 double *mailbox, unsigned long long seq)
 {
     __shared__ double smem[NV * 32];
     double acc[NV];
@@ -113,9 +116,19 @@ final_sum_kernel(const double *__restrict__ partials, int nblocks, double *__res
 #pragma unroll
         for (int i = 0; i < NV; i++) acc[i] += partials[NV * b + i];
     block_sum<NV>(acc, smem);
-    if (threadIdx.x == 0)
+    if (threadIdx.x == 0) {
 #pragma unroll
-        for (int i = 0; i < NV; i++) result[i] = acc[i];
+        for (int i = 0; i < NV; i++) { result[i] = acc[i]; mailbox[i] = acc[i]; }
+        __threadfence_system();
+        *reinterpret_cast<volatile unsigned long long *>(mailbox + 2) = seq;
+    }
+}
+
+// sequence number of the next reduction of this geometry (reductions of one geometry are serialised
+// by contract: they share the partials and the mailbox)
+static unsigned long long next_seq(const dwf_geometry *g)
+{
+    return ++const_cast<dwf_geometry *>(g)->mailbox_seq;
 }
 
 int launch_norm2(const dwf_geometry *g, const void *field, size_t nreal, cudaStream_t st)
@@ -125,7 +138,7 @@ int launch_norm2(const dwf_geometry *g, const void *field, size_t nreal, cudaStr
         norm2_partial_kernel<float><<<nb, 256, 0, st>>>(static_cast<const float *>(field), nreal, g->partials);
     else
         norm2_partial_kernel<double><<<nb, 256, 0, st>>>(static_cast<const double *>(field), nreal, g->partials);
-    final_sum_kernel<1><<<1, 256, 0, st>>>(g->partials, nb, g->result_dev);
+    final_sum_kernel<1><<<1, 256, 0, st>>>(g->partials, nb, g->result_dev, g->mailbox_dev, next_seq(g));
     count_launch(2);
     DWF_CUDA_CHECK(cudaGetLastError());
     return DWF_OK;
@@ -133,7 +146,7 @@ int launch_norm2(const dwf_geometry *g, const void *field, size_t nreal, cudaStr
 
 int launch_final_sum(const dwf_geometry *g, int nblocks, cudaStream_t st)
 {
-    final_sum_kernel<1><<<1, 256, 0, st>>>(g->partials, nblocks, g->result_dev);
+    final_sum_kernel<1><<<1, 256, 0, st>>>(g->partials, nblocks, g->result_dev, g->mailbox_dev, next_seq(g));
     count_launch();
     DWF_CUDA_CHECK(cudaGetLastError());
     return DWF_OK;
@@ -146,7 +159,7 @@ int launch_inner(const dwf_geometry *g, const void *a, const void *b, size_t nco
         inner_partial_kernel<float><<<nb, 256, 0, st>>>(static_cast<const float *>(a), static_cast<const float *>(b), ncomplex, g->partials);
     else
         inner_partial_kernel<double><<<nb, 256, 0, st>>>(static_cast<const double *>(a), static_cast<const double *>(b), ncomplex, g->partials);
-    final_sum_kernel<2><<<1, 256, 0, st>>>(g->partials, nb, g->result_dev);
+    final_sum_kernel<2><<<1, 256, 0, st>>>(g->partials, nb, g->result_dev, g->mailbox_dev, next_seq(g));
     count_launch(2);
     DWF_CUDA_CHECK(cudaGetLastError());
     return DWF_OK;
