@@ -197,3 +197,28 @@ def test_fused_dhop_norm2(lib, dims, Ls, prec):
             assert n2 == n
         with pytest.raises(lib.DwfError):
             lib.dwf_dhop_eo_norm2(g.handle, fin, fin)
+
+
+@pytest.mark.parametrize("opts", [{"ssplit": 2}, {"variant": 2}, {"variant": 12, "raster_staged": 2}, {"zigzag": 0, "layered": 0}])
+def test_other_modes_under_tunables(lib, opts):
+    """The norm2-fused, dagger and axpy instances of the staged kernel under a few tunables: outputs
+    bit-identical to the default configuration, the fused norm within its summation-order tolerance."""
+    import torch
+    dims, Ls, prec, bc = (32, 16, 16, 16), 4, 4, lib.ANTIPERIODIC_T
+    U = gen.gauge_random(dims, 47, prec=prec)
+    half = gen.spinor_gaussian(gen.volume(dims) // 2, Ls, 47, prec=prec)
+    xh = gen.spinor_gaussian(gen.volume(dims) // 2, Ls, 47, gen.STREAM_SPINOR2, prec)
+    with lib.Geometry(dims, Ls, prec, bc) as g:
+        g.load_gauge(U)
+        g.set_option("kernel", 2)
+        fin, fx = g.import_spinor(half, lib.EVEN), g.import_spinor(xh, lib.ODD)
+        ref_n_out, ref_n = g.dhop_oe_norm2(fin)
+        ref_n_out = ref_n_out.clone()
+        ref_d = g.dhop_oe_dag(fin).clone()
+        ref_a = g.dhop_oe_axpy(fin, fx, 4.3, -0.5).clone()
+        for k, v in opts.items():
+            g.set_option(k, v)
+        out, n = g.dhop_oe_norm2(fin)
+        assert torch.equal(out, ref_n_out) and abs(n - ref_n) <= 1e-12 * ref_n
+        assert torch.equal(g.dhop_oe_dag(fin), ref_d)
+        assert torch.equal(g.dhop_oe_axpy(fin, fx, 4.3, -0.5), ref_a)
