@@ -160,7 +160,8 @@ DWF_API unsigned long long dwf_launch_count(void);
  *                    0 evict_normal, 1 evict_first, 2 evict_last
  *   "prefetch"       low 4 bits: L2 prefetch distance in steps (0 off), higher bits: box mask
  *   "l2persist"      MB of L2 set aside for evict_last lines (device-wide CUDA limit)
- *   "ablate"         timing experiments that give WRONG results (skip loads / legs / stores); 0 = off
+ *   "ablate"         timing experiments that give WRONG results (skip loads / legs / stores); only in builds
+ *                    compiled with -DDWF_ABLATE=1, otherwise any value but 0 is UNSUPPORTED
  *   "raster", "tile0".."tile3", "cpc"   direct kernel: CTA launch order, log2 tile extents, slices per CTA */
 DWF_API int dwf_set_option(dwf_geometry *g, const char *key, long long value);
 

@@ -270,6 +270,9 @@ int dwf_set_option(dwf_geometry *g, const char *key, long long value)
         g->opt_l2pol = v;
         return DWF_OK;
     } else if (!strcmp(key, "ablate")) {
+#if !defined(DWF_ABLATE) || !DWF_ABLATE
+        if (v != 0) { set_error("this build has no timing experiments (compile with -DDWF_ABLATE=1)"); return DWF_ERR_UNSUPPORTED; }
+#endif
         g->opt_ablate = v;
         return DWF_OK;
     } else if (!strcmp(key, "zigzag")) {

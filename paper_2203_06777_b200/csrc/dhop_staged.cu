@@ -120,6 +120,9 @@ template <int LH, int B1, int B2, int B3> struct StagedCfg {
 #ifndef DWF_SYNC_MODE
 #define DWF_SYNC_MODE 1
 #endif
+#ifndef DWF_ABLATE
+#define DWF_ABLATE 0          // 1: compile the "ablate" timing experiments into the kernels
+#endif
 #ifndef DWF_REFILL_PER_LEG
 #define DWF_REFILL_PER_LEG 1   // 1: refill a leg's links right after the leg (last slice of a tile); 0: all after the last leg
 #endif
@@ -245,6 +248,8 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
 {
     using Cfg = StagedCfg<LH, B1, B2, B3>;
     constexpr bool NORM = MODE == 1, DAG = MODE == 2, AXPY = MODE == 3;
+    // timing experiments (wrong results) exist only in builds with -DDWF_ABLATE=1; otherwise the tests fold away
+    const int ablate_bits = DWF_ABLATE ? args.ablate : 0;
     // MODE 3 stages the rows box of the field x as well (read in the epilogue): NROW_C more rows per stage
     constexpr int STAGE = Cfg::STAGE_BYTES + (AXPY ? Cfg::NROW_C * Cfg::ROWB : 0);
     extern __shared__ __align__(1024) unsigned char smem[];
@@ -314,7 +319,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         const int pfd = args.prefetch & 15, pfm = args.prefetch >> 4;
         for (int g = 0; g < nsteps; g++) {
             const int stage = g & 1;
-            if (pfd && g + pfd < nsteps && !(args.ablate & 8)) {       // DRAM -> L2 runs ahead of the shared-memory ring
+            if (pfd && g + pfd < nsteps && !(ablate_bits & 8)) {       // DRAM -> L2 runs ahead of the shared-memory ring
                 const Boxes p = boxes(g + pfd);
                 if (pfm & 1) tma_prefetch_5d(&map_c, 0, 0, p.o1, p.o2, p.c4);
                 if (pfm & 2) tma_prefetch_5d(&map_x3, 0, 0, p.o1, p.o2, p.c3p);
@@ -331,7 +336,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             const uint32_t fb = full_base + 32 * stage, eb = empty_base + 32 * stage;
             constexpr uint32_t FS = DWF_SYNC_MODE == 0 ? 8 : 0;      // stride of the per-region full barriers
             const uint32_t epar = ((g >> 1) - 1) & 1;
-            const bool notma = args.ablate & 8, no12 = args.ablate & 32, no3 = args.ablate & 16;   // timing experiments
+            const bool notma = ablate_bits & 8, no12 = ablate_bits & 32, no3 = ablate_bits & 16;   // timing experiments
             // regions in the order the consumers release them (x3 faces, x2 faces, x1 faces, centre)
             if (g >= 2) mbar_wait(eb, epar);
             if (notma || no3) mbar_arrive(fb);
@@ -460,7 +465,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         constexpr bool FETCH = decltype(fetch_tag)::value;
         const unsigned char *sb = smem + stage * STAGE;
         const uint32_t fb = full_base + 32 * stage, eb = empty_base + 32 * stage;
-        const bool legs = !(args.ablate & 4);
+        const bool legs = !(ablate_bits & 4);
         float2 acc[12];
 #define DWF_LEG(L, MU, FWD, FIRST)                                                                  \
         staged_leg<LH, MU, (FWD) != DAG, FIRST, DWF_ABL>(acc, reinterpret_cast<const float4 *>(sb) + (((L) & 1) ? offp[(L) >> 1] >> 16 : offp[(L) >> 1] & 0xffffu), U + 9 * (L)); \
@@ -570,7 +575,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
 #pragma unroll
             for (int k = 0; k < 12; k++) nsum += (double)acc[k].x * acc[k].x + (double)acc[k].y * acc[k].y;
         }
-        if (!(args.ablate & 2)) {
+        if (!(ablate_bits & 2)) {
 #pragma unroll
             for (int j = 0; j < 6; j++)
                 stg128_hint(o + j * LH, make_float4(acc[2 * j].x, acc[2 * j].y, acc[2 * j + 1].x, acc[2 * j + 1].y), pol_o);
@@ -590,7 +595,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         if (has_next) grow_next = tile_row(it + 1, r_next);
         const float4 *gnext = reinterpret_cast<const float4 *>(args.gauge) + grow_next * (36 * LH) + h;
         for (int s = 0; s < nsl; s++, g++) {
-            const bool fetch = has_next && s == nsl - 1 && !(args.ablate & 1);     // refill the links during the last slice
+            const bool fetch = has_next && s == nsl - 1 && !(ablate_bits & 1);     // refill the links during the last slice
             const int stage = g & 1;
             const int sl = (args.zigzag && (it & 1)) ? nsl - 1 - s : s;
             if (fetch) step(std::true_type{}, stage, (g >> 1) & 1, optr + (long long)sl * slice_vecs, gnext);
