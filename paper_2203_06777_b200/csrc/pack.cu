@@ -74,6 +74,73 @@ spinor_reorder_kernel(const T *__restrict__ src, T *__restrict__ dst, const Latt
     }
 }
 
+// fp32: one thread per device site (parity, s, row, h): the 24 reals of a site are one 96-byte record
+// on the canonical side (six 128-bit accesses per thread, whole sectors) and six 128-bit vectors on
+// the device side (consecutive threads = consecutive h: coalesced).
+template <bool IMPORT, bool FULL>
+__global__ void __launch_bounds__(256)
+spinor_reorder_sites_kernel(const float *__restrict__ src, float *__restrict__ dst, const Lattice lat)
+{
+    const long long Vh = lat.Vh;
+    const long long nrow = Vh / lat.Lh;
+    const long long n = (FULL ? 2 : 1) * Vh * lat.Ls;
+    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n;
+         e += (long long)gridDim.x * blockDim.x) {
+        long long r = e;
+        const int h = (int)(r % lat.Lh); r /= lat.Lh;
+        const long long row = r % nrow; r /= nrow;
+        const int s = (int)(r % lat.Ls);
+        const int par = (int)(r / lat.Ls);
+        const long long cb = row * lat.Lh + h;
+        long long site = cb;
+        if (FULL) {
+            long long q = row;
+            const int x1 = (int)(q % lat.L[1]); q /= lat.L[1];
+            const int x2 = (int)(q % lat.L[2]);
+            const int x3 = (int)(q / lat.L[2]);
+            site = 2 * cb + ((x1 + x2 + x3 + par) & 1);
+        }
+        const long long canon = (site * lat.Ls + s) * 6;                                   // in float4
+        const long long dev = (((long long)par * lat.Ls + s) * nrow + row) * 6 * lat.Lh + h;   // in float4: + j * Lh
+        float c[24];
+        if (IMPORT) {
+#pragma unroll
+            for (int j = 0; j < 6; j++) {
+                const float4 q = reinterpret_cast<const float4 *>(src)[canon + j];
+                c[4 * j] = q.x; c[4 * j + 1] = q.y; c[4 * j + 2] = q.z; c[4 * j + 3] = q.w;
+            }
+#pragma unroll
+            for (int j = 0; j < 6; j++) {       // vector j = slots 2j, 2j+1; slot k = 4*col + t
+                float v[4];
+#pragma unroll
+                for (int u = 0; u < 2; u++) {
+                    const int k = 2 * j + u, col = k >> 2, t = k & 3;
+                    const int i0 = ((t >> 1) * 6 + col) * 2 + (t & 1);
+                    v[2 * u] = c[i0];
+                    v[2 * u + 1] = c[i0 + 6];
+                }
+                reinterpret_cast<float4 *>(dst)[dev + (long long)j * lat.Lh] = make_float4(v[0], v[1], v[2], v[3]);
+            }
+        } else {
+#pragma unroll
+            for (int j = 0; j < 6; j++) {
+                const float4 q = reinterpret_cast<const float4 *>(src)[dev + (long long)j * lat.Lh];
+                const float v[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+                for (int u = 0; u < 2; u++) {
+                    const int k = 2 * j + u, col = k >> 2, t = k & 3;
+                    const int i0 = ((t >> 1) * 6 + col) * 2 + (t & 1);
+                    c[i0] = v[2 * u];
+                    c[i0 + 6] = v[2 * u + 1];
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < 6; j++)
+                reinterpret_cast<float4 *>(dst)[canon + j] = make_float4(c[4 * j], c[4 * j + 1], c[4 * j + 2], c[4 * j + 3]);
+        }
+    }
+}
+
 template <typename T>
 __global__ void __launch_bounds__(256)
 gauge_pack_kernel(const T *__restrict__ U, T *__restrict__ set_even, T *__restrict__ set_odd,
@@ -155,8 +222,9 @@ static int launch_reorder(const dwf_geometry *g, const void *src, void *dst, int
     if (g->prec == DWF_F32) {
         auto *a = static_cast<const float *>(src);
         auto *b = static_cast<float *>(dst);
-        if (full) spinor_reorder_kernel<float, IMPORT, true><<<grid, 256, 0, st>>>(a, b, g->lat);
-        else      spinor_reorder_kernel<float, IMPORT, false><<<grid, 256, 0, st>>>(a, b, g->lat);
+        const int gs = grid_for((full ? 2 : 1) * g->lat.Vh * g->lat.Ls, g->sm_count);
+        if (full) spinor_reorder_sites_kernel<IMPORT, true><<<gs, 256, 0, st>>>(a, b, g->lat);
+        else      spinor_reorder_sites_kernel<IMPORT, false><<<gs, 256, 0, st>>>(a, b, g->lat);
     } else {
         auto *a = static_cast<const double *>(src);
         auto *b = static_cast<double *>(dst);
