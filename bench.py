@@ -223,7 +223,7 @@ def run_reference(args, w):
 # ---------------------------------------------------------------------------------------------
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
 # `ncu --set full` capture summarised under profiles/ (None until a capture exists).
-NCU_TRAFFIC_BYTES = {"c4": 1474414000 + 769279000}   # profiles/r01i_bench_step_ncu.md, launch 1 (DhopOE)
+NCU_TRAFFIC_BYTES = {"c4": 1472801000 + 770327000}   # profiles/r01k_bench_step_ncu.md, launch 1 (DhopOE)
 
 
 def max_over_ranks(x, dist=None, device="cuda"):
