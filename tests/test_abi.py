@@ -64,6 +64,14 @@ def test_null_arguments():
     r = ctypes.c_double(-1.0)
     assert lib.dwf_norm2(None, None, 0, ctypes.byref(r), None) == dwf.ERR_INVALID_ARG
     assert r.value == -1.0                                  # outputs untouched on error
+    for f in (lib.dwf_dhop_dag, lib.dwf_dhop_oe_dag, lib.dwf_dhop_eo_dag, lib.dwf_dhop_oe, lib.dwf_dhop_eo):
+        assert f(None, None, None, None) == dwf.ERR_INVALID_ARG
+    for f in (lib.dwf_dhop_oe_norm2, lib.dwf_dhop_eo_norm2):
+        assert f(None, None, None, ctypes.byref(r), None) == dwf.ERR_INVALID_ARG
+        assert r.value == -1.0
+    for f in (lib.dwf_dhop_oe_axpy, lib.dwf_dhop_eo_axpy):
+        assert f(None, None, None, 1.0, 1.0, None, None) == dwf.ERR_INVALID_ARG
+    assert lib.dwf_set_option(None, b"kernel", 1) == dwf.ERR_INVALID_ARG
     assert lib.dwf_field_bytes(None, 0) == 0
     assert lib.dwf_destroy_geometry(None) == dwf.OK
     assert b"NULL" in lib.dwf_last_error() or lib.dwf_last_error() != b""
