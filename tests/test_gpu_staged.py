@@ -222,3 +222,31 @@ def test_other_modes_under_tunables(lib, opts):
         assert torch.equal(out, ref_n_out) and abs(n - ref_n) <= 1e-12 * ref_n
         assert torch.equal(g.dhop_oe_dag(fin), ref_d)
         assert torch.equal(g.dhop_oe_axpy(fin, fx, 4.3, -0.5), ref_a)
+
+
+def test_dhop_calls_can_be_captured_in_a_cuda_graph(lib):
+    """dwf_dhop_oe / dwf_dhop_eo enqueue one kernel each and never synchronise, so a solver may
+    capture them in a CUDA graph (removes the launch gaps that dominate small lattices)."""
+    import torch
+    dims, Ls, prec = (16, 16, 16, 16), 16, 4                     # BASELINE.json configs[2] shape
+    U = gen.gauge_random(dims, 1003, prec=prec)
+    half = gen.spinor_gaussian(gen.volume(dims) // 2, Ls, 1003, prec=prec)
+    with lib.Geometry(dims, Ls, prec, lib.PERIODIC) as g:
+        g.load_gauge(U)
+        f_e = g.import_spinor(half, lib.EVEN)
+        f_o, f_x = g.new_field(lib.ODD), g.new_field(lib.EVEN)
+        g.dhop_oe(f_e, f_o)
+        g.dhop_eo(f_o, f_x)
+        torch.cuda.synchronize()
+        ref = f_x.clone()
+        graph, side = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+        with torch.cuda.stream(side):
+            g.dhop_oe(f_e, f_o)                                  # warm the per-thread tensor-map cache outside the capture
+            torch.cuda.synchronize()
+            with torch.cuda.graph(graph, stream=side):
+                g.dhop_oe(f_e, f_o)
+                g.dhop_eo(f_o, f_x)
+        f_x.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(f_x, ref)
