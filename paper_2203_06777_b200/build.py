@@ -21,7 +21,7 @@ OBJDIR = os.path.join(HERE, "build")
 
 # (source, object name, extra defines): dhop_staged.cu is compiled once per kernel MODE so that the
 # four sets of template instances build in parallel
-SOURCES = [("api.cu", "api.o", []), ("pack.cu", "pack.o", []), ("dhop.cu", "dhop.o", []), ("reduce.cu", "reduce.o", []),
+SOURCES = [("dhop_staged64.cu", "dhop_staged64.o", []), ("api.cu", "api.o", []), ("pack.cu", "pack.o", []), ("dhop.cu", "dhop.o", []), ("reduce.cu", "reduce.o", []),
            ("dhop_staged.cu", "dhop_staged_m0.o", ["-DDWF_STAGED_MODE=0"]),
            ("dhop_staged.cu", "dhop_staged_m1.o", ["-DDWF_STAGED_MODE=1"]),
            ("dhop_staged.cu", "dhop_staged_m2.o", ["-DDWF_STAGED_MODE=2"]),

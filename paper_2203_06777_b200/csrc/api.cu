@@ -120,6 +120,14 @@ int rebuild_tilings(dwf_geometry *g)
         DWF_CUDA_CHECK(cudaMalloc(&g->tiles_staged, st.size() * sizeof(int4)));
         DWF_CUDA_CHECK(cudaMemcpy(g->tiles_staged, st.data(), st.size() * sizeof(int4), cudaMemcpyHostToDevice));
     }
+    if (g->tiles_staged64) { cudaFree(g->tiles_staged64); g->tiles_staged64 = nullptr; }
+    plan_staged64(g);
+    if (g->staged64.variant >= 0) {
+        std::vector<int4> st((size_t)g->staged64.ntiles);
+        build_staged64_tile_table(g, st.data());
+        DWF_CUDA_CHECK(cudaMalloc(&g->tiles_staged64, st.size() * sizeof(int4)));
+        DWF_CUDA_CHECK(cudaMemcpy(g->tiles_staged64, st.data(), st.size() * sizeof(int4), cudaMemcpyHostToDevice));
+    }
     return DWF_OK;
 }
 
@@ -243,6 +251,7 @@ int dwf_destroy_geometry(dwf_geometry *g)
     cudaFreeHost(g->mailbox_host);
     cudaFree(g->tiles_cb);
     cudaFree(g->tiles_staged);
+    cudaFree(g->tiles_staged64);
     cudaFree(g->staging);
     cudaGetLastError();
     delete g;
@@ -337,12 +346,13 @@ int dwf_load_gauge(dwf_geometry *g, const void *U, int src_is_device, void *stre
 // one half-Dhop: out (parity_out) = D in (opposite parity); picks the kernel
 static int half_dhop(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger = false)
 {
-    const bool staged_ok = g->staged.variant >= 0;
-    if (g->opt_kernel == 2 && !staged_ok) {
-        set_error("the staged kernel does not support this geometry / precision");
+    const bool staged_ok = g->staged.variant >= 0, staged64_ok = g->staged64.variant >= 0;
+    if (g->opt_kernel == 2 && !staged_ok && !staged64_ok) {
+        set_error("the staged kernels do not support this geometry / precision");
         return DWF_ERR_UNSUPPORTED;
     }
     if (staged_ok && g->opt_kernel != 1) return launch_dhop_staged(g, in, out, parity_out, st, nullptr, nullptr, dagger);
+    if (staged64_ok && g->opt_kernel != 1) return launch_dhop_staged64(g, in, out, parity_out, st, dagger);
     return launch_dhop_direct(g, in, out, parity_out, st, dagger);
 }
 
@@ -425,7 +435,7 @@ static int dhop_norm2_common(const dwf_geometry *g, const void *in, void *out, i
     DeviceGuard guard(g->device);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const bool staged_ok = g->staged.variant >= 0;
-    if (g->opt_kernel == 2 && !staged_ok) {
+    if (g->opt_kernel == 2 && !staged_ok && g->staged64.variant < 0) {
         set_error("the staged kernel does not support this geometry / precision");
         return DWF_ERR_UNSUPPORTED;
     }
@@ -436,7 +446,7 @@ static int dhop_norm2_common(const dwf_geometry *g, const void *in, void *out, i
         if (rc) return rc;
         rc = launch_final_sum(g, nblocks, st);
     } else {
-        rc = launch_dhop_direct(g, in, out, parity_out, st);
+        rc = half_dhop(g, in, out, parity_out, st);
         if (rc) return rc;
         rc = launch_norm2(g, out, dwf_field_bytes(g, parity_out) / (size_t)g->prec, st);
     }

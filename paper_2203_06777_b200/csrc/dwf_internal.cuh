@@ -79,6 +79,9 @@ struct dwf_geometry {
     // staged (TMA, link-stationary) kernel: plan chosen at create time, row-box tile table
     dwf::StagedPlan staged;
     int4 *tiles_staged;
+    // fp64 staged kernel (dhop_staged64.cu): its own tile shape and table
+    dwf::StagedPlan staged64;
+    int4 *tiles_staged64;
     // reductions
     double *partials;       // [2 * max_blocks]
     double *result_dev;     // [2]
@@ -127,6 +130,10 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
 bool staged_supports_axpy(const dwf_geometry *g);
 // pack.cu: out = a x + b out, elementwise over nreal reals (the unfused path of dwf_dhop_*_axpy)
 int launch_axpby(const dwf_geometry *g, const void *x, void *out, double a, double b, size_t nreal, cudaStream_t st);
+// dhop_staged64.cu (TMA-staged fp64 kernel, links split by colour column over three threads)
+void plan_staged64(dwf_geometry *g);
+void build_staged64_tile_table(const dwf_geometry *g, int4 *host_table);
+int launch_dhop_staged64(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger);
 // reduce.cu
 int launch_norm2(const dwf_geometry *g, const void *field, size_t nreal, cudaStream_t st);
 int launch_final_sum(const dwf_geometry *g, int nblocks, cudaStream_t st);   // result_dev[0] = sum of partials[0..nblocks)
