@@ -30,7 +30,8 @@
  *   half field   pair[s][row][k/2][h][k&1]: row = x1 + L1*(x2 + L2*x3) (a lattice line along x0),
  *                h = x0>>1 (cb site x>>1 = row*Lh + h), 12 slots k of two reals per site, slots
  *                2j and 2j+1 adjacent (one 128-bit vector in fp32).
- *                fp64: slot k = spin*3 + colour = the complex number (re, im).
+ *                fp64: complex[s][row][k][h] instead, k = spin*3 + colour: one plane per component,
+ *                a site's complex number (re, im) is one 128-bit word.
  *                fp32: slot k = 4*colour + t = one real part of a pair of spins, t = 0 (re of
  *                spins 0,1), 1 (im of 0,1), 2 (re of 2,3), 3 (im of 2,3).
  *   full field   the even half field followed by the odd half field

@@ -47,7 +47,7 @@ __device__ __forceinline__ void dhop_leg(typename CxT<T>::type (&acc)[12][SC],
     C psi[12][SC];
     if constexpr (sizeof(T) == 8) {
 #pragma unroll
-        for (int k = 0; k < 12; k++) load_cx<SC>(nb + pair_off(k, W0), psi[k]);
+        for (int k = 0; k < 12; k++) load_cx<SC>(nb + k * W0, psi[k]);      // fp64 fields: complex[..][k][h]
     } else {
         // fp32 fields store spin pairs (pack.cu): slot 4c + t -> (re|im of spins 0,1 | 2,3)
         C q[12][SC];
@@ -165,14 +165,15 @@ dhop_direct_kernel(const typename CxT<T>::type *__restrict__ in, typename CxT<T>
     // a row (lattice line along x0) is a block of 12*W0 complex: [k/2][h][k&1]
     const long long row = x1 + L1 * (x2 + (long long)L2 * x3);
     const long long rs = 12 * W0;                    // complex elements per row
-    const long long own = row * rs + 2 * c0;
+    constexpr int SS = sizeof(T) == 4 ? 2 : 1;       // complex elements between consecutive sites of a component plane
+    const long long own = row * rs + SS * c0;
 
     // neighbour element offsets (component 0)
     const int r = (x1 + x2 + x3 + parity_out) & 1;          // x0 = 2*c0 + r
     int hp = c0 + r;       if (hp == W0) hp = 0;
     int hm = c0 - 1 + r;   if (hm < 0) hm = W0 - 1;
-    const long long n0p = row * rs + 2 * hp;
-    const long long n0m = row * rs + 2 * hm;
+    const long long n0p = row * rs + SS * hp;
+    const long long n0m = row * rs + SS * hm;
     const long long s1 = rs, s2 = rs * L1, s3 = rs * L1 * L2;
     const long long n1p = own + (x1 + 1 == L1 ? -(L1 - 1) * s1 : s1);
     const long long n1m = own + (x1 == 0 ? (L1 - 1) * s1 : -s1);
@@ -197,7 +198,7 @@ dhop_direct_kernel(const typename CxT<T>::type *__restrict__ in, typename CxT<T>
     C *o = out + (size_t)s * 12 * (size_t)Vh + (size_t)own;
     if constexpr (sizeof(T) == 8) {
 #pragma unroll
-        for (int k = 0; k < 12; k++) store_cx<SC>(o + pair_off(k, W0), acc[k]);
+        for (int k = 0; k < 12; k++) store_cx<SC>(o + k * W0, acc[k]);
     } else {
 #pragma unroll
         for (int c = 0; c < 3; c++) {

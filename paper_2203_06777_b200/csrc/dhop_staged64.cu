@@ -16,7 +16,8 @@
 // Everything else follows dhop_staged.cu: a producer warpgroup (setmaxnreg) issues 5-D bulk tensor
 // copies (TMA) of the input slice -- rows box + 6 faces -- into a two-stage shared-memory ring with
 // full / empty mbarriers; consumers walk all Ls slices of a tile with their link columns in registers.
-// Layouts (pack.cu): spinor complex[s][row][k/2][h][k&1], k = spin*3 + colour; links
+// Layouts (pack.cu): spinor complex[s][row][k][h], k = spin*3 + colour (one plane per component:
+// consecutive sites are consecutive 128-bit words); links
 // complex[row][f/2][h][f&1], f = leg*9 + a*3 + b.
 #include <vector>
 
@@ -124,17 +125,15 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
     const int r3p = (i3 + 1 < B3) ? rc + B1 * B2 : Cfg::R_X3P + i1 + B1 * i2;
     const int r3m = (i3 > 0) ? rc - B1 * B2 : Cfg::R_X3M + i1 + B1 * i2;
     uint32_t off[8];            // byte offsets of (neighbour site, component 0) inside a stage
-    off[2] = r1p * Cfg::ROWB + h * 32;
-    off[3] = r1m * Cfg::ROWB + h * 32;
-    off[4] = r2p * Cfg::ROWB + h * 32;
-    off[5] = r2m * Cfg::ROWB + h * 32;
-    off[6] = r3p * Cfg::ROWB + h * 32;
-    off[7] = r3m * Cfg::ROWB + h * 32;
-    // byte offset of component k = spin*3 + C inside a row block [k/2][h][k&1] of 16-byte complex
-    constexpr uint32_t KOFF0 = ((0 * 3 + C) >> 1) * LH * 32 + ((0 * 3 + C) & 1) * 16;
-    constexpr uint32_t KOFF1 = ((1 * 3 + C) >> 1) * LH * 32 + ((1 * 3 + C) & 1) * 16;
-    constexpr uint32_t KOFF2 = ((2 * 3 + C) >> 1) * LH * 32 + ((2 * 3 + C) & 1) * 16;
-    constexpr uint32_t KOFF3 = ((3 * 3 + C) >> 1) * LH * 32 + ((3 * 3 + C) & 1) * 16;
+    off[2] = r1p * Cfg::ROWB + h * 16;
+    off[3] = r1m * Cfg::ROWB + h * 16;
+    off[4] = r2p * Cfg::ROWB + h * 16;
+    off[5] = r2m * Cfg::ROWB + h * 16;
+    off[6] = r3p * Cfg::ROWB + h * 16;
+    off[7] = r3m * Cfg::ROWB + h * 16;
+    // byte offset of component k = spin*3 + C inside a row block [k][h] of 16-byte complex
+    constexpr uint32_t KOFF0 = (0 * 3 + C) * LH * 16, KOFF1 = (1 * 3 + C) * LH * 16;
+    constexpr uint32_t KOFF2 = (2 * 3 + C) * LH * 16, KOFF3 = (3 * 3 + C) * LH * 16;
 
     const long long nrow = (long long)args.L1 * args.L2 * args.L3;
     double2 *red = reinterpret_cast<double2 *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES);
@@ -148,8 +147,8 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
         const long long grow = x1 + (long long)args.L1 * (x2 + (long long)args.L2 * x3);
         int hp = h + r;       if (hp == LH) hp = 0;
         int hm = h - 1 + r;   if (hm < 0) hm = LH - 1;
-        off[0] = rc * Cfg::ROWB + hp * 32;
-        off[1] = rc * Cfg::ROWB + hm * 32;
+        off[0] = rc * Cfg::ROWB + hp * 16;
+        off[1] = rc * Cfg::ROWB + hm * 16;
         {
             const double2 *gp = args.gauge + grow * (72 * LH) + 2 * h;
 #pragma unroll
@@ -160,7 +159,7 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
                     U[leg * 3 + a] = __ldg(gp + (f >> 1) * 2 * LH + (f & 1));
                 }
         }
-        double2 *orow = args.out + grow * (12 * LH) + 2 * h;            // + s * nrow * 12 * LH
+        double2 *orow = args.out + grow * (12 * LH) + h;                // + s * nrow * 12 * LH + k * LH
         for (int s = 0; s < args.Ls; s++, g++) {
             const int stage = g & 1;
             mbar_wait(full_base + 8 * stage, (g >> 1) & 1);
@@ -208,7 +207,7 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
                     const double2 a1 = red[((((buf * 3 + C) * 2 + 1) * 4 + j) * Cfg::TP) + site];
                     const double2 v = cadd(cadd(acc[4 * C + j], a0), a1);
                     const int k = 4 * C + j;
-                    __stcs(o2 + (k >> 1) * 2 * LH + (k & 1), v);
+                    __stcs(o2 + k * LH, v);
                 }
             }
         }
@@ -287,7 +286,7 @@ struct Variant64 {
     const void *fn[2];       // plain, dagger
 };
 
-#define DWF_STAGED64_VARIANTS(X) X(16, 2, 2, 1) X(8, 4, 2, 1) X(8, 2, 2, 2) X(4, 4, 4, 1) X(4, 4, 2, 2) X(4, 2, 2, 2) X(4, 2, 2, 1) X(8, 2, 2, 1) X(16, 2, 1, 1)
+#define DWF_STAGED64_VARIANTS(X) X(16, 2, 1, 2) X(16, 1, 1, 4) X(16, 1, 2, 2) X(16, 2, 2, 1) X(8, 4, 2, 1) X(8, 2, 2, 2) X(4, 4, 4, 1) X(4, 4, 2, 2) X(4, 2, 2, 2) X(4, 2, 2, 1) X(8, 2, 2, 1) X(16, 2, 1, 1)
 
 static const std::vector<Variant64> &variants64()
 {
@@ -313,6 +312,7 @@ void plan_staged64(dwf_geometry *g)
     for (size_t i = 0; i < v.size(); i++) {
         if (v[i].lh != lat.Lh) continue;
         if (lat.L[1] % v[i].b1 || lat.L[2] % v[i].b2 || lat.L[3] % v[i].b3) continue;
+        if (g->opt_variant > 0 && (int)i + 1 != g->opt_variant) continue;
         g->staged64.variant = (int)i;
         g->staged64.b[0] = v[i].b1; g->staged64.b[1] = v[i].b2; g->staged64.b[2] = v[i].b3;
         g->staged64.ntiles = (lat.L[1] / v[i].b1) * (lat.L[2] / v[i].b2) * (lat.L[3] / v[i].b3);
@@ -320,27 +320,39 @@ void plan_staged64(dwf_geometry *g)
     }
 }
 
-// launch order of the row boxes: x1 fastest, x3 slowest (the concurrently resident CTAs share faces in L2)
+// launch order of the row boxes: x1 fastest, x3 slowest, direction 2 split into macro blocks of at most
+// 96 tile columns per x3 layer that are swept one after the other (as in dhop_staged.cu: the CTAs
+// resident at one time then cover several x3 layers of a macro block and share their faces in L2)
 void build_staged64_tile_table(const dwf_geometry *g, int4 *tab)
 {
     const Lattice &lat = g->lat;
     const int *b = g->staged64.b;
+    const int n1 = lat.L[1] / b[0], n2 = lat.L[2] / b[1], n3 = lat.L[3] / b[2];
+    int nsplit = 1;
+    if (g->opt_raster_staged < 0) {
+        while (n1 * (n2 / nsplit) > 96 && n2 % (nsplit * 2) == 0) nsplit *= 2;
+    } else {
+        for (int i = 0; i < g->opt_raster_staged % 10 && n2 % (nsplit * 2) == 0; i++) nsplit *= 2;
+    }
+    const int n2in = n2 / nsplit;
     int id = 0;
-    for (int t3 = 0; t3 < lat.L[3] / b[2]; t3++)
-        for (int t2 = 0; t2 < lat.L[2] / b[1]; t2++)
-            for (int t1 = 0; t1 < lat.L[1] / b[0]; t1++) tab[id++] = make_int4(t1 * b[0], t2 * b[1], t3 * b[2], 0);
+    for (int m = 0; m < nsplit; m++)
+        for (int t3 = 0; t3 < n3; t3++)
+            for (int t2 = 0; t2 < n2in; t2++)
+                for (int t1 = 0; t1 < n1; t1++)
+                    tab[id++] = make_int4(t1 * b[0], (m * n2in + t2) * b[1], t3 * b[2], 0);
 }
 
-// tensor map of an fp64 half field complex[s][x3][x2][x1][k/2][h][k&1] seen as 5-D fp64 tensor
-// (4*Lh, 6, L1, L2, L3*Ls)
+// tensor map of an fp64 half field complex[s][x3][x2][x1][k][h] seen as 5-D fp64 tensor
+// (2*Lh, 12, L1, L2, L3*Ls)
 static int encode_map64(CUtensorMap *m, const void *base, const Lattice &lat, int b1, int b2, int b3)
 {
     PFN_tensorMapEncodeTiled enc = get_tensor_map_encoder();
-    const cuuint64_t dims[5] = {(cuuint64_t)4 * lat.Lh, 6, (cuuint64_t)lat.L[1], (cuuint64_t)lat.L[2],
+    const cuuint64_t dims[5] = {(cuuint64_t)2 * lat.Lh, 12, (cuuint64_t)lat.L[1], (cuuint64_t)lat.L[2],
                                 (cuuint64_t)lat.L[3] * lat.Ls};
-    const cuuint64_t krow = (cuuint64_t)lat.Lh * 32, row = 6 * krow;
+    const cuuint64_t krow = (cuuint64_t)lat.Lh * 16, row = 12 * krow;
     const cuuint64_t strides[4] = {krow, row, row * lat.L[1], row * lat.L[1] * lat.L[2]};
-    const cuuint32_t box[5] = {(cuuint32_t)4 * lat.Lh, 6, (cuuint32_t)b1, (cuuint32_t)b2, (cuuint32_t)b3};
+    const cuuint32_t box[5] = {(cuuint32_t)2 * lat.Lh, 12, (cuuint32_t)b1, (cuuint32_t)b2, (cuuint32_t)b3};
     const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
     CUresult rc = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, const_cast<void *>(base), dims, strides, box, estr,
                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,

@@ -5,7 +5,8 @@
 //         so the cb site x>>1 is row*Lh + h; a site has 12 slots k of two reals; slots 2j, 2j+1 of
 //         a site are adjacent (one 128-bit vector in fp32).  One such block per parity; a FULL
 //         field is the even block followed by the odd block (canonical site x -> parity p(x)).
-//         fp64: slot k = spin*3 + colour holds the complex number (re, im).
+//         fp64: complex[s][row][k][h], k = spin*3 + colour: one plane per component, a site's complex
+//         number (re, im) is one 128-bit vector.
 //         fp32: slot k = 4*colour + t holds one real part of a PAIR OF SPINS: t = 0: (re psi_0c,
 //         re psi_1c), 1: (im psi_0c, im psi_1c), 2: (re psi_2c, re psi_3c), 3: (im psi_2c,
 //         im psi_3c).  The packed f32x2 arithmetic of dhop_staged.cu then multiplies a link
@@ -37,11 +38,18 @@ spinor_reorder_kernel(const T *__restrict__ src, T *__restrict__ dst, const Latt
     const long long n = (FULL ? 2 : 1) * Vh * lat.Ls * 12;
     for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n;
          e += (long long)gridDim.x * blockDim.x) {
-        // device element e = ((((par*Ls + s)*nrow + row)*6 + k/2)*Lh + h)*2 + (k&1)
+        // fp32 device element e = ((((par*Ls + s)*nrow + row)*6 + k/2)*Lh + h)*2 + (k&1)
+        // fp64 device element e =  (((par*Ls + s)*nrow + row)*12 + k)*Lh + h
         long long r = e;
-        const int klo = (int)(r & 1); r >>= 1;
-        const int h = (int)(r % lat.Lh); r /= lat.Lh;
-        const int k = 2 * (int)(r % 6) + klo; r /= 6;
+        int h, k;
+        if constexpr (sizeof(T) == 4) {
+            const int klo = (int)(r & 1); r >>= 1;
+            h = (int)(r % lat.Lh); r /= lat.Lh;
+            k = 2 * (int)(r % 6) + klo; r /= 6;
+        } else {
+            h = (int)(r % lat.Lh); r /= lat.Lh;
+            k = (int)(r % 12); r /= 12;
+        }
         const long long row = r % nrow; r /= nrow;
         const int s = (int)(r % lat.Ls);
         const int par = (int)(r / lat.Ls);
