@@ -20,8 +20,13 @@ host memory (reorder + D2H).
 `--impl reference` times the CPU oracle (oracle/, plain fp64 definition, OpenMP) on the host
 cores on the same workload; there is no other reference implementation (the paper ships none).
 
+`roofline.frac` is the event-timed DhopOE launch of the K timed steps; `roofline.frac_sustained` is the
+same kernel in a >= 2 s loop of back-to-back half-Dhops with no host synchronisation inside
+(the regime in which the board sits at its power limit), with its own clock record.
+
 Multi-GPU: the path does not shard (north_star: one GPU, no halo exchange) -- "replicas only":
 every rank runs the same workload on its own GPU, value = total sites / max time over ranks.
+`--gpus N` without a launcher (no WORLD_SIZE in the environment) starts the N ranks itself.
 """
 from __future__ import annotations
 
@@ -221,9 +226,18 @@ def run_reference(args, w):
 # ---------------------------------------------------------------------------------------------
 # the CUDA arm
 # ---------------------------------------------------------------------------------------------
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
-# `ncu --set full` capture summarised under profiles/ (None until a capture exists).
-NCU_TRAFFIC_BYTES = {"c4": 1472801000 + 770327000}   # profiles/r01k_bench_step_ncu.md, launch 1 (DhopOE)
+def ncu_traffic(workload: str, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+    `ncu --set full` capture summarised under profiles/ (profiles/traffic.json is written beside each
+    summary: {workload: {"kernel": ..., "bytes": ..., "source": ...}}).  None when there is no capture of
+    this workload with the kernel that actually ran."""
+    try:
+        rec = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))[workload]
+    except Exception:
+        return None, None
+    if rec.get("kernel") and rec["kernel"] != kernel:
+        return None, f"capture is of {rec['kernel']}, not of {kernel}"
+    return rec.get("bytes"), rec.get("source")
 
 
 def max_over_ranks(x, dist=None, device="cuda"):
@@ -307,6 +321,26 @@ def run_gpu(args, w):
     t_eo = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
     value = whole_job_gflops(world, sites, ms_step)
 
+    # ---- sustained regime: >= 2 s of half-Dhops back to back, no host synchronisation inside ----
+    # (north_star says "sustains": after ~60 ms the board reaches its power limit and the SM clock sags)
+    sustained = None
+    if args.sustain > 0:
+        n_pairs = max(10, int(args.sustain / (2 * t_oe * 1e-3)) + 1)
+        s_sampler = ClockSampler(physical_gpu_index(local_rank))
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        s_sampler.start()
+        s0.record()
+        for _ in range(n_pairs):
+            g.dhop_oe(f_in, f_mid)
+            g.dhop_eo(f_mid, f_out)
+        s1.record()
+        barrier()
+        s_clocks = s_sampler.stop()
+        ms_sus = max_over_ranks(s0.elapsed_time(s1), dist)
+        sustained = {"seconds": ms_sus * 1e-3, "launches": 2 * n_pairs, "us_per_launch": 1e3 * ms_sus / (2 * n_pairs),
+                     "clocks": s_clocks}
+
     # ---- e2e: the same step through the C ABI with HOST buffers ----
     host_in = torch.empty(psi_e.shape, dtype=torch.from_numpy(psi_e).dtype, pin_memory=True)
     host_in.copy_(torch.from_numpy(psi_e))
@@ -364,13 +398,19 @@ def run_gpu(args, w):
     t_dhop = t_oe
     mb = model_bytes_cb(w)
     achieved = mb / (t_dhop * 1e-3) / 1e9
+    kernel = g.kernel_info()
+    traffic, traffic_src = ncu_traffic(args.workload, kernel)
+    fld_mb, gauge_mb = psi_e.nbytes / 1e6, 2 * U.nbytes / 1e6
+    l2_note = (f"inputs larger than L2 ({fld_mb:.0f} MB half fields, {gauge_mb:.0f} MB links); no flush" if fld_mb > 200 else
+               f"working set ({3 * fld_mb:.0f} MB of fields + {gauge_mb:.0f} MB links) is partly L2-resident across steps: "
+               "model GB/s may exceed the HBM peak; no flush (SURVEY.md 8(d) caveat)")
     line = {
         "metric": "Dhop GFlop/s (1320 flop/5D site)", "value": value, "unit": "GFlop/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if prec == 4 else "f64", "data": "synthetic",
         "config": {"workload": workload_name(w), "name": args.workload, "dims": list(d), "Ls": Ls,
-                   "l2": "inputs larger than L2 (805 MB half fields, 604 MB links); no flush",
+                   "l2": l2_note,
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "clocks": clocks,
         "e2e": {"value": e2e_val, "unit": "GFlop/s", "ms_per_step": ms_e2e,
@@ -378,11 +418,16 @@ def run_gpu(args, w):
         "gpu_launches": int(launches),
         "kernels_ms": {"dhop_oe": t_oe, "dhop_eo_norm2_incl_host_sync": t_eo},
         "dhop_only_gflops": FLOP_PER_SITE * sites / (t_dhop * 1e-3) / 1e9,
-        "roofline": {"bound": "hbm", "kernel": "dhop_staged_kernel (DhopOE launches)", "achieved": achieved, "peak": peak,
+        "roofline": {"bound": "hbm", "kernel": kernel + " (DhopOE launches)", "achieved": achieved, "peak": peak,
                      "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": mb,
-                     "traffic": NCU_TRAFFIC_BYTES.get(args.workload)},
+                     "traffic": traffic, "traffic_source": traffic_src},
     }
+    if sustained is not None:
+        ach_s = mb / (sustained["us_per_launch"] * 1e-6) / 1e9
+        line["roofline"]["frac_sustained"] = ach_s / peak
+        line["roofline"]["achieved_sustained"] = ach_s
+        line["roofline"]["sustained"] = sustained
     if extra is not None:
         extra["dag_roofline_frac"] = mb / (extra["dhop_eo_dag_ms"] * 1e-3) / 1e9 / peak
         extra["axpy_roofline_frac"] = extra["axpy_algorithmic_bytes_per_launch"] / (extra["dhop_eo_axpy_ms"] * 1e-3) / 1e9 / peak
@@ -398,6 +443,27 @@ def run_gpu(args, w):
         dist.destroy_process_group()
 
 
+def spawn_ranks(n: int, argv, check_devices: bool = True) -> int:
+    """`python bench.py --gpus N` without a launcher: start N ranks of this script under
+    torch.distributed.run on this node (one per GPU, rendezvous on 127.0.0.1) and return its exit
+    code.  "Replicas only": the ranks share nothing but the timing all-reduce."""
+    import socket
+    import subprocess
+    if check_devices:
+        import torch
+        have = torch.cuda.device_count()
+        if have < n:
+            print(f"bench.py: --gpus {n} but only {have} CUDA device(s) are visible", file=sys.stderr)
+            return 2
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *argv]
+    return subprocess.call(cmd)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -409,9 +475,13 @@ def main():
     ap.add_argument("--extra-ops", action="store_true",
                     help="also time Dhop^dagger and the fused a x + b Dhop (SURVEY.md 8(f1)); adds `next_rows` to the line")
     ap.add_argument("--opt", action="append", help="kernel tunable key=value (dwf_set_option)")
+    ap.add_argument("--sustain", type=float, default=2.2,
+                    help="seconds of back-to-back half-Dhops for roofline.frac_sustained (0: skip)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "dwf" else args.warmup
     w = WORKLOADS[args.workload]
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "dwf":
+        sys.exit(spawn_ranks(args.gpus, sys.argv[1:]))
     if args.impl == "reference":
         run_reference(args, w)
     else:

@@ -148,6 +148,11 @@ DWF_API int dwf_export_spinor(const dwf_geometry *g, const void *field_dev, int 
 /* Number of kernel launches this library has issued since it was loaded (all threads). */
 DWF_API unsigned long long dwf_launch_count(void);
 
+/* Name of the kernel a half-Dhop on this geometry runs with the current options, e.g.
+ * "dhop_staged_kernel<16,4,2,2>" (Lh and the rows box of the tile), written NUL-terminated into
+ * buf[0..n).  For reports; no effect on results.  Errors: INVALID_ARG. */
+DWF_API int dwf_kernel_info(const dwf_geometry *g, char *buf, size_t n);
+
 /* Tuning knobs for experiments; none of them changes a result of the staged kernel by a bit
  * (tests/test_gpu_staged.py).  UNSUPPORTED for an unknown key, INVALID_ARG for a bad value.
  *   "kernel"         0 auto, 1 direct (L1-cached) kernel, 2 TMA-staged kernel (error if it has no
@@ -161,8 +166,6 @@ DWF_API unsigned long long dwf_launch_count(void);
  *                    0 evict_normal, 1 evict_first, 2 evict_last
  *   "prefetch"       low 4 bits: L2 prefetch distance in steps (0 off), higher bits: box mask
  *   "l2persist"      MB of L2 set aside for evict_last lines (device-wide CUDA limit)
- *   "ablate"         timing experiments that give WRONG results (skip loads / legs / stores); only in builds
- *                    compiled with -DDWF_ABLATE=1, otherwise any value but 0 is UNSUPPORTED
  *   "raster", "tile0".."tile3", "cpc"   direct kernel: CTA launch order, log2 tile extents, slices per CTA */
 DWF_API int dwf_set_option(dwf_geometry *g, const char *key, long long value);
 

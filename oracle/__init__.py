@@ -8,10 +8,14 @@ never imports this one.
 The arithmetic lives in ``dhop_oracle.c`` (plain C, fp64, OpenMP over sites): the
 definition of the operator written out with full 4x4 gamma matrices, see that
 file's header for the passages it follows (PAPER.md L43/L223/L254 name the
-operator; BASELINE.json north_star states it; SURVEY.md 8(c) fixes conventions).
-This module only marshals numpy arrays (canonical layouts of include/dwf.h).
+operator; BASELINE.json north_star states it; SURVEY.md 8(c) fixes conventions),
+and in ``dwf5d_oracle.c``: the rest of the red-black Shamir domain-wall operator
+ as dense linear algebra on the (4 Ls) x (4 Ls) matrix of its
+4D-site-diagonal part.  This module only marshals numpy arrays (canonical layouts
+of include/dwf.h).
 
-Pins: tests/test_oracle_pins.py (P1-P9 of SURVEY.md 8(c)); nothing is unpinned.
+Pins: tests/test_oracle_pins.py (P1-P9 of SURVEY.md 8(c)) and
+tests/test_oracle_pins_dwf.py (the 8(f2) functions); nothing is unpinned.
 """
 from __future__ import annotations
 
@@ -22,7 +26,7 @@ import subprocess
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SRC = os.path.join(_HERE, "dhop_oracle.c")
+_SRCS = [os.path.join(_HERE, "dhop_oracle.c"), os.path.join(_HERE, "dwf5d_oracle.c")]
 _LIB = os.path.join(_HERE, "liboracle.so")
 
 PERIODIC, ANTIPERIODIC_T = 0, 1
@@ -31,11 +35,11 @@ EVEN, ODD = 0, 1
 
 def build(force: bool = False) -> str:
     """Compile dhop_oracle.c into liboracle.so (in-tree).  Building is not using."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(f) for f in _SRCS):
         tmp = _LIB + f".tmp{os.getpid()}"
         subprocess.check_call(
             ["gcc", "-O2", "-std=c11", "-fcx-limited-range", "-fopenmp", "-fPIC", "-shared",
-             "-o", tmp, _SRC, "-lm"])
+             "-o", tmp, *_SRCS, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -67,6 +71,15 @@ def _load():
         lib.orc_inner.argtypes = [vp, vp, ci, i64, vp]
         lib.orc_inner.restype = None
         lib.orc_num_threads.restype = ci
+        dbl = ctypes.c_double
+        lib.orc_mooee_matrix.argtypes = [ci, dbl, dbl, ci, vp]
+        lib.orc_mooee_matrix.restype = ci
+        lib.orc_mooee.argtypes = [i64, ci, dbl, dbl, ci, vp, ci, vp]
+        lib.orc_mooee.restype = ci
+        lib.orc_ddwf.argtypes = [i4, ci, ci, dbl, dbl, ci, vp, ci, vp, ci, vp]
+        lib.orc_ddwf.restype = ci
+        lib.orc_schur.argtypes = [i4, ci, ci, dbl, dbl, ci, ci, vp, ci, vp, ci, vp]
+        lib.orc_schur.restype = ci
         if lib.orc_check_gamma() != 0:
             raise RuntimeError("oracle gamma matrices fail their algebra self-check")
         _lib = lib
@@ -169,3 +182,53 @@ def inner(a: np.ndarray, b: np.ndarray) -> complex:
     out = np.zeros(2)
     _load().orc_inner(_c(a).ctypes.data, _c(b).ctypes.data, _prec(a), a.size // 2, out.ctypes.data)
     return complex(out[0], out[1])
+
+
+# ---------------------------------------------------------------------------------------------
+# the rest of the red-black Shamir domain-wall operator (dwf5d_oracle.c)
+# ---------------------------------------------------------------------------------------------
+M5_APPLY, M5_DAG, M5_INV, M5_INV_DAG = 0, 1, 2, 3
+
+
+def mooee_matrix(Ls: int, M5: float, mass: float, op: int = M5_APPLY) -> np.ndarray:
+    """The oracle's dense (4 Ls, 4 Ls) real matrix of Mooee (index s*4 + spin), its transpose, inverse
+    or inverse transpose (for the pins)."""
+    out = np.empty((4 * Ls, 4 * Ls), dtype=np.float64)
+    if _load().orc_mooee_matrix(int(Ls), float(M5), float(mass), int(op), out.ctypes.data):
+        raise ValueError("orc_mooee_matrix: bad arguments or singular matrix")
+    return out
+
+
+def mooee(Ls: int, M5: float, mass: float, psi: np.ndarray, op: int = M5_APPLY) -> np.ndarray:
+    """The 4D-site-diagonal part of the Shamir DWF matrix applied to a field (nsites, Ls, 4, 3, 2):
+    op = M5_APPLY (Mooee), M5_DAG (its adjoint), M5_INV (inverse), M5_INV_DAG.  fp64 out."""
+    assert psi.ndim == 5 and psi.shape[1:] == (Ls, 4, 3, 2)
+    out = np.empty(psi.shape, dtype=np.float64)
+    if _load().orc_mooee(psi.shape[0], int(Ls), float(M5), float(mass), int(op), _c(psi).ctypes.data, _prec(psi),
+                         out.ctypes.data):
+        raise ValueError("orc_mooee: bad arguments")
+    return out
+
+
+def ddwf(dims, Ls: int, bc_time: int, M5: float, mass: float, U: np.ndarray, psi: np.ndarray,
+         dagger: bool = False) -> np.ndarray:
+    """Full Shamir DWF matrix M = Mooee - Dhop/2 on a full field (V4, Ls, 4, 3, 2) -> fp64."""
+    d, v4 = _dims(dims)
+    assert U.size == v4 * 72 and psi.size == v4 * Ls * 24
+    out = np.empty((v4, Ls, 4, 3, 2), dtype=np.float64)
+    if _load().orc_ddwf(d, Ls, bc_time, float(M5), float(mass), int(bool(dagger)), _c(U).ctypes.data, _prec(U),
+                        _c(psi).ctypes.data, _prec(psi), out.ctypes.data):
+        raise ValueError("orc_ddwf: bad arguments")
+    return out
+
+
+def schur(dims, Ls: int, bc_time: int, M5: float, mass: float, parity: int, U: np.ndarray,
+          psi_half: np.ndarray, dagger: bool = False) -> np.ndarray:
+    """Schur complement S = Mooee - M_pq Mooee^-1 M_qp on parity p (half field in, half field out)."""
+    d, v4 = _dims(dims)
+    assert U.size == v4 * 72 and psi_half.size == (v4 // 2) * Ls * 24
+    out = np.empty((v4 // 2, Ls, 4, 3, 2), dtype=np.float64)
+    if _load().orc_schur(d, Ls, bc_time, float(M5), float(mass), int(bool(dagger)), int(parity),
+                         _c(U).ctypes.data, _prec(U), _c(psi_half).ctypes.data, _prec(psi_half), out.ctypes.data):
+        raise ValueError("orc_schur: bad arguments")
+    return out

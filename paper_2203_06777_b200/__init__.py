@@ -26,7 +26,7 @@ LIB_PATH = os.path.join(_HERE, "libdwf.so")
 SYMBOLS = (
     "dwf_create_geometry", "dwf_destroy_geometry", "dwf_load_gauge", "dwf_dhop", "dwf_dhop_oe",
     "dwf_dhop_eo", "dwf_dhop_dag", "dwf_dhop_oe_dag", "dwf_dhop_eo_dag", "dwf_dhop_oe_axpy", "dwf_dhop_eo_axpy", "dwf_dhop_oe_norm2", "dwf_dhop_eo_norm2", "dwf_norm2", "dwf_inner_product", "dwf_field_bytes",
-    "dwf_import_spinor", "dwf_export_spinor", "dwf_launch_count", "dwf_set_option",
+    "dwf_import_spinor", "dwf_export_spinor", "dwf_launch_count", "dwf_kernel_info", "dwf_set_option",
     "dwf_error_string", "dwf_last_error",
 )
 
@@ -69,6 +69,7 @@ def load(build_if_missing: bool = True):
     lib.dwf_export_spinor.argtypes = [vp, vp, ci, vp, ci, vp]
     lib.dwf_launch_count.argtypes = []
     lib.dwf_launch_count.restype = ctypes.c_ulonglong
+    lib.dwf_kernel_info.argtypes = [vp, ctypes.c_char_p, cs]
     lib.dwf_set_option.argtypes = [vp, ctypes.c_char_p, ctypes.c_longlong]
     lib.dwf_error_string.argtypes = [ci]
     lib.dwf_error_string.restype = ctypes.c_char_p
@@ -84,11 +85,15 @@ def _check(rc: int, what: str):
         raise DwfError(rc, what, (lib.dwf_last_error() or lib.dwf_error_string(rc)).decode())
 
 
-def _stream(stream) -> int:
-    """cudaStream_t as an integer: None = torch's current stream."""
+_geom_info = {}     # handle -> (precision, cuda device, Ls): what the argument checks below need
+
+
+def _stream(stream, g=None) -> int:
+    """cudaStream_t as an integer: None = torch's current stream on the geometry's device."""
     if stream is None:
         import torch
-        return int(torch.cuda.current_stream().cuda_stream)
+        dev = _geom_info[g][1] if g in _geom_info else None
+        return int(torch.cuda.current_stream(dev).cuda_stream)
     if hasattr(stream, "cuda_stream"):
         return int(stream.cuda_stream)
     return int(stream)
@@ -105,10 +110,33 @@ def _ptr(a):
     return a.data_ptr(), 1 if a.is_cuda else 0
 
 
-def _dev_ptr(t) -> int:
+def _dev_ptr(t, g=None, parity=None) -> int:
+    """Address of a device field.  With g and parity: also checks the element type against the
+    geometry's precision and the size against dwf_field_bytes (the C ABI carries no sizes)."""
     if not getattr(t, "is_cuda", False) or not t.is_contiguous():
         raise ValueError("device fields must be contiguous torch CUDA tensors")
+    if g in _geom_info and parity is not None:
+        prec, dev, _ = _geom_info[g]
+        if t.element_size() != prec or not t.dtype.is_floating_point:
+            raise DwfError(ERR_INVALID_ARG, "binding", f"field dtype {t.dtype} does not match the geometry's precision ({prec} bytes per real)")
+        want = dwf_field_bytes(g, parity)
+        if t.numel() * t.element_size() != want:
+            raise DwfError(ERR_INVALID_ARG, "binding", f"field holds {t.numel() * t.element_size()} bytes, the geometry needs {want} (parity {parity})")
+        if t.device.index != dev:
+            raise DwfError(ERR_INVALID_ARG, "binding", f"field lives on cuda:{t.device.index}, the geometry on cuda:{dev}")
     return t.data_ptr()
+
+
+def _canon(a, g, parity):
+    """(address, is_device) of a canonical array, size- and dtype-checked against the geometry."""
+    p, on_dev = _ptr(a)
+    if g in _geom_info:
+        prec = _geom_info[g][0]
+        nbytes = a.nbytes if isinstance(a, np.ndarray) else a.numel() * a.element_size()
+        item = a.itemsize if isinstance(a, np.ndarray) else a.element_size()
+        if item != prec or nbytes != dwf_field_bytes(g, parity):
+            raise DwfError(ERR_INVALID_ARG, "binding", "canonical array does not match the geometry (dtype or size)")
+    return p, on_dev
 
 
 # ---------------------------------------------------------------------------------------------
@@ -120,75 +148,82 @@ def dwf_create_geometry(dims, Ls: int, precision: int, bc_time: int = PERIODIC, 
     h = ctypes.c_void_p()
     _check(lib.dwf_create_geometry(d, int(Ls), int(precision), int(bc_time), int(cuda_device),
                                    ctypes.byref(h)), "dwf_create_geometry")
+    _geom_info[h.value] = (int(precision), int(cuda_device), int(Ls))
     return h.value
 
 
 def dwf_destroy_geometry(g: int) -> None:
+    _geom_info.pop(g, None)
     _check(load().dwf_destroy_geometry(g), "dwf_destroy_geometry")
 
 
 def dwf_load_gauge(g: int, U, stream=None) -> None:
     p, on_dev = _ptr(U)
-    _check(load().dwf_load_gauge(g, p, on_dev, _stream(stream)), "dwf_load_gauge")
+    if g in _geom_info:
+        item = U.itemsize if isinstance(U, np.ndarray) else U.element_size()
+        nbytes = U.nbytes if isinstance(U, np.ndarray) else U.numel() * U.element_size()
+        if item != _geom_info[g][0] or nbytes != dwf_field_bytes(g, FULL) // _geom_info[g][2] * 3:
+            raise DwfError(ERR_INVALID_ARG, "binding", "gauge array does not match the geometry (dtype or size: V4*72 reals)")
+    _check(load().dwf_load_gauge(g, p, on_dev, _stream(stream, g)), "dwf_load_gauge")
 
 
 def dwf_dhop(g: int, in_full, out_full, stream=None) -> None:
-    _check(load().dwf_dhop(g, _dev_ptr(in_full), _dev_ptr(out_full), _stream(stream)), "dwf_dhop")
+    _check(load().dwf_dhop(g, _dev_ptr(in_full, g, FULL), _dev_ptr(out_full, g, FULL), _stream(stream, g)), "dwf_dhop")
 
 
 def dwf_dhop_oe(g: int, in_even, out_odd, stream=None) -> None:
-    _check(load().dwf_dhop_oe(g, _dev_ptr(in_even), _dev_ptr(out_odd), _stream(stream)), "dwf_dhop_oe")
+    _check(load().dwf_dhop_oe(g, _dev_ptr(in_even, g, EVEN), _dev_ptr(out_odd, g, ODD), _stream(stream, g)), "dwf_dhop_oe")
 
 
 def dwf_dhop_eo(g: int, in_odd, out_even, stream=None) -> None:
-    _check(load().dwf_dhop_eo(g, _dev_ptr(in_odd), _dev_ptr(out_even), _stream(stream)), "dwf_dhop_eo")
+    _check(load().dwf_dhop_eo(g, _dev_ptr(in_odd, g, ODD), _dev_ptr(out_even, g, EVEN), _stream(stream, g)), "dwf_dhop_eo")
 
 
 def dwf_dhop_dag(g: int, in_full, out_full, stream=None) -> None:
-    _check(load().dwf_dhop_dag(g, _dev_ptr(in_full), _dev_ptr(out_full), _stream(stream)), "dwf_dhop_dag")
+    _check(load().dwf_dhop_dag(g, _dev_ptr(in_full, g, FULL), _dev_ptr(out_full, g, FULL), _stream(stream, g)), "dwf_dhop_dag")
 
 
 def dwf_dhop_oe_dag(g: int, in_even, out_odd, stream=None) -> None:
-    _check(load().dwf_dhop_oe_dag(g, _dev_ptr(in_even), _dev_ptr(out_odd), _stream(stream)), "dwf_dhop_oe_dag")
+    _check(load().dwf_dhop_oe_dag(g, _dev_ptr(in_even, g, EVEN), _dev_ptr(out_odd, g, ODD), _stream(stream, g)), "dwf_dhop_oe_dag")
 
 
 def dwf_dhop_eo_dag(g: int, in_odd, out_even, stream=None) -> None:
-    _check(load().dwf_dhop_eo_dag(g, _dev_ptr(in_odd), _dev_ptr(out_even), _stream(stream)), "dwf_dhop_eo_dag")
+    _check(load().dwf_dhop_eo_dag(g, _dev_ptr(in_odd, g, ODD), _dev_ptr(out_even, g, EVEN), _stream(stream, g)), "dwf_dhop_eo_dag")
 
 
 def dwf_dhop_oe_axpy(g: int, in_even, x_odd, a: float, b: float, out_odd, stream=None) -> None:
-    _check(load().dwf_dhop_oe_axpy(g, _dev_ptr(in_even), _dev_ptr(x_odd), float(a), float(b), _dev_ptr(out_odd),
-                                   _stream(stream)), "dwf_dhop_oe_axpy")
+    _check(load().dwf_dhop_oe_axpy(g, _dev_ptr(in_even, g, EVEN), _dev_ptr(x_odd, g, ODD), float(a), float(b),
+                                   _dev_ptr(out_odd, g, ODD), _stream(stream, g)), "dwf_dhop_oe_axpy")
 
 
 def dwf_dhop_eo_axpy(g: int, in_odd, x_even, a: float, b: float, out_even, stream=None) -> None:
-    _check(load().dwf_dhop_eo_axpy(g, _dev_ptr(in_odd), _dev_ptr(x_even), float(a), float(b), _dev_ptr(out_even),
-                                   _stream(stream)), "dwf_dhop_eo_axpy")
+    _check(load().dwf_dhop_eo_axpy(g, _dev_ptr(in_odd, g, ODD), _dev_ptr(x_even, g, EVEN), float(a), float(b),
+                                   _dev_ptr(out_even, g, EVEN), _stream(stream, g)), "dwf_dhop_eo_axpy")
 
 
 def dwf_dhop_oe_norm2(g: int, in_even, out_odd, stream=None) -> float:
     r = ctypes.c_double()
-    _check(load().dwf_dhop_oe_norm2(g, _dev_ptr(in_even), _dev_ptr(out_odd), ctypes.byref(r), _stream(stream)),
+    _check(load().dwf_dhop_oe_norm2(g, _dev_ptr(in_even, g, EVEN), _dev_ptr(out_odd, g, ODD), ctypes.byref(r), _stream(stream, g)),
            "dwf_dhop_oe_norm2")
     return r.value
 
 
 def dwf_dhop_eo_norm2(g: int, in_odd, out_even, stream=None) -> float:
     r = ctypes.c_double()
-    _check(load().dwf_dhop_eo_norm2(g, _dev_ptr(in_odd), _dev_ptr(out_even), ctypes.byref(r), _stream(stream)),
+    _check(load().dwf_dhop_eo_norm2(g, _dev_ptr(in_odd, g, ODD), _dev_ptr(out_even, g, EVEN), ctypes.byref(r), _stream(stream, g)),
            "dwf_dhop_eo_norm2")
     return r.value
 
 
 def dwf_norm2(g: int, field, parity: int = FULL, stream=None) -> float:
     r = ctypes.c_double()
-    _check(load().dwf_norm2(g, _dev_ptr(field), int(parity), ctypes.byref(r), _stream(stream)), "dwf_norm2")
+    _check(load().dwf_norm2(g, _dev_ptr(field, g, parity), int(parity), ctypes.byref(r), _stream(stream, g)), "dwf_norm2")
     return r.value
 
 
 def dwf_inner_product(g: int, a, b, parity: int = FULL, stream=None) -> complex:
     r = (ctypes.c_double * 2)()
-    _check(load().dwf_inner_product(g, _dev_ptr(a), _dev_ptr(b), int(parity), r, _stream(stream)),
+    _check(load().dwf_inner_product(g, _dev_ptr(a, g, parity), _dev_ptr(b, g, parity), int(parity), r, _stream(stream, g)),
            "dwf_inner_product")
     return complex(r[0], r[1])
 
@@ -198,19 +233,25 @@ def dwf_field_bytes(g: int, parity: int = FULL) -> int:
 
 
 def dwf_import_spinor(g: int, canonical, parity: int, field_dev, stream=None) -> None:
-    p, on_dev = _ptr(canonical)
-    _check(load().dwf_import_spinor(g, p, on_dev, int(parity), _dev_ptr(field_dev), _stream(stream)),
+    p, on_dev = _canon(canonical, g, parity)
+    _check(load().dwf_import_spinor(g, p, on_dev, int(parity), _dev_ptr(field_dev, g, parity), _stream(stream, g)),
            "dwf_import_spinor")
 
 
 def dwf_export_spinor(g: int, field_dev, parity: int, canonical, stream=None) -> None:
-    p, on_dev = _ptr(canonical)
-    _check(load().dwf_export_spinor(g, _dev_ptr(field_dev), int(parity), p, on_dev, _stream(stream)),
+    p, on_dev = _canon(canonical, g, parity)
+    _check(load().dwf_export_spinor(g, _dev_ptr(field_dev, g, parity), int(parity), p, on_dev, _stream(stream, g)),
            "dwf_export_spinor")
 
 
 def dwf_launch_count() -> int:
     return int(load().dwf_launch_count())
+
+
+def dwf_kernel_info(g: int) -> str:
+    buf = ctypes.create_string_buffer(128)
+    _check(load().dwf_kernel_info(g, buf, 128), "dwf_kernel_info")
+    return buf.value.decode()
 
 
 def dwf_set_option(g: int, key: str, value: int) -> None:
@@ -338,3 +379,6 @@ class Geometry:
 
     def set_option(self, key: str, value: int):
         dwf_set_option(self.handle, key, value)
+
+    def kernel_info(self) -> str:
+        return dwf_kernel_info(self.handle)

@@ -171,6 +171,16 @@ const char *dwf_last_error(void) { return t_err; }
 
 unsigned long long dwf_launch_count(void) { return g_launches.load(); }
 
+int dwf_kernel_info(const dwf_geometry *g, char *buf, size_t n)
+{
+    if (!g || !buf || n == 0) { set_error("dwf_kernel_info: bad argument"); return DWF_ERR_INVALID_ARG; }
+    const bool s32 = g->staged.variant >= 0 && g->opt_kernel != 1, s64 = g->staged64.variant >= 0 && g->opt_kernel != 1;
+    if (s32)      snprintf(buf, n, "dhop_staged_kernel<%d,%d,%d,%d>", g->lat.Lh, g->staged.b[0], g->staged.b[1], g->staged.b[2]);
+    else if (s64) snprintf(buf, n, "dhop_staged64_kernel<%d,%d,%d,%d>", g->lat.Lh, g->staged64.b[0], g->staged64.b[1], g->staged64.b[2]);
+    else          snprintf(buf, n, "dhop_direct_kernel<%s>", g->prec == DWF_F32 ? "float" : "double");
+    return DWF_OK;
+}
+
 int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, int cuda_device, dwf_geometry **out)
 {
     if (!dims || !out) { set_error("dwf_create_geometry: NULL argument"); return DWF_ERR_INVALID_ARG; }
@@ -277,12 +287,6 @@ int dwf_set_option(dwf_geometry *g, const char *key, long long value)
         g->opt_variant = v;          // 0: best staged tile, n > 0: n-th compiled staged variant only
     } else if (!strcmp(key, "l2pol")) {
         g->opt_l2pol = v;
-        return DWF_OK;
-    } else if (!strcmp(key, "ablate")) {
-#if !defined(DWF_ABLATE) || !DWF_ABLATE
-        if (v != 0) { set_error("this build has no timing experiments (compile with -DDWF_ABLATE=1)"); return DWF_ERR_UNSUPPORTED; }
-#endif
-        g->opt_ablate = v;
         return DWF_OK;
     } else if (!strcmp(key, "zigzag")) {
         g->opt_zigzag = v != 0;
@@ -418,7 +422,13 @@ static int fetch_reduction(const dwf_geometry *g, cudaStream_t st, int n, double
         }
     }
     std::atomic_thread_fence(std::memory_order_acquire);
-    if (*seq != want) DWF_CUDA_CHECK(cudaStreamSynchronize(st));
+    if (*seq != want) {
+        DWF_CUDA_CHECK(cudaStreamSynchronize(st));
+        if (*seq != want) {        // the stream drained without the final-sum kernel of this call having run
+            set_error("reduction result never arrived (sequence %llu, expected %llu)", *seq, want);
+            return DWF_ERR_CUDA;
+        }
+    }
     for (int i = 0; i < n; i++) out[i] = const_cast<const volatile double *>(g->mailbox_host)[i];
     return DWF_OK;
 }

@@ -17,11 +17,6 @@ template <> struct CxT<float>  { using type = float2;  };
 template <> struct CxT<double> { using type = double2; };
 
 // ---- packed fp32 primitives -------------------------------------------------------------------
-#ifdef DWF_SCALAR_FP32     // experiment: scalar FFMA / FMUL / FADD instead of the packed forms
-__device__ __forceinline__ float2 f2_fma(float2 a, float2 b, float2 c) { return make_float2(fmaf(a.x, b.x, c.x), fmaf(a.y, b.y, c.y)); }
-__device__ __forceinline__ float2 f2_mul(float2 a, float2 b) { return make_float2(a.x * b.x, a.y * b.y); }
-__device__ __forceinline__ float2 f2_add(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-#else
 __device__ __forceinline__ float2 f2_fma(float2 a, float2 b, float2 c)
 {
     float2 d;
@@ -55,7 +50,6 @@ __device__ __forceinline__ float2 f2_add(float2 a, float2 b)
         : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
     return d;
 }
-#endif
 
 // ---- complex ops, fp32 ------------------------------------------------------------------------
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return f2_add(a, b); }

@@ -316,6 +316,12 @@ void plan_staged64(dwf_geometry *g)
         g->staged64.variant = (int)i;
         g->staged64.b[0] = v[i].b1; g->staged64.b[1] = v[i].b2; g->staged64.b[2] = v[i].b3;
         g->staged64.ntiles = (lat.L[1] / v[i].b1) * (lat.L[2] / v[i].b2) * (lat.L[3] / v[i].b3);
+        // per-device opt-in to the large dynamic shared memory (the caller holds a DeviceGuard)
+        for (int d = 0; d < 2; d++)
+            if (cudaFuncSetAttribute(v[i].fn[d], cudaFuncAttributeMaxDynamicSharedMemorySize, v[i].smem) != cudaSuccess) {
+                cudaGetLastError();
+                g->staged64.variant = -1;
+            }
         return;
     }
 }
@@ -381,11 +387,6 @@ int launch_dhop_staged64(const dwf_geometry *g, const void *in, void *out, int p
     a.L1 = g->lat.L[1]; a.L2 = g->lat.L[2]; a.L3 = g->lat.L[3]; a.Ls = g->lat.Ls;
     a.parity_out = parity_out;
     const void *fn = v.fn[dagger ? 1 : 0];
-    static thread_local const void *attr_set_for[2] = {nullptr, nullptr};
-    if (attr_set_for[dagger ? 1 : 0] != fn) {
-        DWF_CUDA_CHECK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, v.smem));
-        attr_set_for[dagger ? 1 : 0] = fn;
-    }
     const int grid = g->staged64.ntiles < g->sm_count ? g->staged64.ntiles : g->sm_count;
     void *params[] = {&mc, &m1, &m2, &m3, &a};
     DWF_CUDA_CHECK(cudaLaunchKernel(fn, dim3((unsigned)grid), dim3((unsigned)v.threads), params, (size_t)v.smem, st));

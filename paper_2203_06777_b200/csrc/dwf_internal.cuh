@@ -89,7 +89,7 @@ struct dwf_geometry {
     double *mailbox_dev;    // the same words as the device sees them
     unsigned long long mailbox_seq;   // last sequence number handed to a reduction
     int reduce_blocks;
-    // host-side staging for canonical <-> device conversions (lazily grown)
+    // device staging for canonical <-> device conversions of host arrays (lazily grown)
     void *staging;
     size_t staging_bytes;
     // tunables (dwf_set_option)
@@ -101,7 +101,6 @@ struct dwf_geometry {
     int opt_kernel;         // 0: auto, 1: direct only, 2: staged only
     int opt_l2pol;          // staged kernel: L2 eviction-priority digits (dhop_staged.cu PC_*)
     int opt_ssplit;         // staged kernel: CTAs sharing one tile (each takes Ls / ssplit slices)
-    int opt_ablate;         // staged kernel: timing experiments (dhop_staged.cu StagedArgs::ablate)
     int opt_zigzag;         // staged kernel: walk the slices of every other tile backwards
     int opt_layered;        // staged kernel: one TMA box per x3 layer, so that L2 policies can differ per layer
     int opt_prefetch;       // staged kernel: L2 prefetch distance (low 4 bits, steps) and box mask (bits 4..)

@@ -31,15 +31,6 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-// Arrive that is ordered after the COMPLETION of earlier shared-memory loads by data dependence
-// (the twelve values must depend on every loaded word) instead of by a memory clobber, so that
-// the compiler may still move later, unrelated loads above it.
-__device__ __forceinline__ void mbar_arrive_after(uint32_t bar, const float2 (&a)[12])
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar), "f"(a[0].x), "f"(a[1].x), "f"(a[2].x),
-                 "f"(a[3].x), "f"(a[4].x), "f"(a[5].x), "f"(a[6].x), "f"(a[7].x), "f"(a[8].x), "f"(a[9].x),
-                 "f"(a[10].x), "f"(a[11].x));
-}
 // blocks until the phase with the given parity has completed
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
