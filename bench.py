@@ -52,6 +52,9 @@ WORKLOADS = {
     "c4d": dict(dims=(32, 32, 32, 32), Ls=16, prec=8, bc=0, gauge="near_unit", seed=1004),
     "c5": dict(dims=(48, 48, 48, 96), Ls=12, prec=4, bc=1, gauge="random", seed=1005),
     "tiny": dict(dims=(8, 8, 8, 8), Ls=8, prec=4, bc=1, gauge="random", seed=1002),
+    # the Schur complement of the red-black Shamir DWF operator on the C4 shape
+    "schur": dict(dims=(32, 32, 32, 32), Ls=16, prec=4, bc=0, gauge="near_unit", seed=1004, kind="schur"),
+    "schurd": dict(dims=(32, 32, 32, 32), Ls=16, prec=8, bc=0, gauge="near_unit", seed=1004, kind="schur"),
 }
 
 
@@ -443,6 +446,111 @@ def run_gpu(args, w):
         dist.destroy_process_group()
 
 
+def run_gpu_schur(args, w):
+    """--workload schur: SURVEY.md 8(f2) on the C4 shape: one application of the even-site Schur complement
+    S = Mooee - 1/4 DhopEO Mooee^-1 DhopOE (four kernels) per step, plus every kernel of the sequence timed
+    on its own against its own minimal-traffic model (one read + one write of the field for the
+    fifth-dimension passes; + one read of x and the links for a x + b Dhop)."""
+    import torch
+    import paper_2203_06777_b200 as dwf
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dwf.load()
+    d, Ls, prec = w["dims"], w["Ls"], w["prec"]
+    V4 = d[0] * d[1] * d[2] * d[3]
+    sites = (V4 // 2) * Ls
+    M5, mass = 1.8, 0.01
+    U, psi_e = make_inputs(w)
+    g = dwf.Geometry(d, Ls, prec, w["bc"], device=local_rank)
+    for kv in args.opt or []:
+        k, v = kv.split("=")
+        g.set_option(k, int(v))
+    g.load_gauge(U)
+    f_in = g.import_spinor(psi_e, dwf.EVEN)
+    f_out, f_t, f_u = g.new_field(dwf.EVEN), g.new_field(dwf.ODD), g.new_field(dwf.ODD)
+    work = g.new_work(dwf.dwf_schur_work_bytes(g.handle))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step():
+        g.schur(f_in, dwf.EVEN, M5, mass, out=f_out, work=work)
+
+    for _ in range(args.warmup):
+        step()
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    barrier()
+    sampler.start()
+    l0 = dwf.dwf_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    launches = dwf.dwf_launch_count() - l0
+    clocks = sampler.stop()
+    ms_step = max_over_ranks(e0.elapsed_time(e1), dist) / args.steps
+
+    def timed(fn, n=max(10, args.steps // 2)):
+        for _ in range(3):
+            fn()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record()
+        for _ in range(n):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / n
+
+    fb = psi_e.nbytes                                   # bytes of one half field
+    gb = model_bytes_cb(w) - 2 * fb                      # the whole gauge field once
+    peak, peak_src = peaks()
+    parts = {
+        "dhop_oe": (timed(lambda: g.dhop_oe(f_in, f_t)), 2 * fb + gb),
+        "mooee_inv": (timed(lambda: g.mooee_inv(f_t, dwf.ODD, M5, mass, out=f_u)), 2 * fb),
+        "mooee": (timed(lambda: g.mooee(f_in, dwf.EVEN, M5, mass, out=f_out)), 2 * fb),
+        "dhop_eo_axpy": (timed(lambda: g.dhop_eo_axpy(f_u, f_out, 1.0, -0.25, out=f_out)), 3 * fb + gb),
+    }
+    kernels = {k: {"ms": t, "algorithmic_bytes": b, "achieved_gbs": b / (t * 1e-3) / 1e9, "frac": b / (t * 1e-3) / 1e9 / peak}
+               for k, (t, b) in parts.items()}
+    total_model = sum(b for _, b in parts.values())
+    if rank == 0:
+        t_inv, b_inv = parts["mooee_inv"]
+        line = {
+            "metric": "Dhop GFlop/s (1320 flop/5D site)", "value": whole_job_gflops(world, sites, ms_step), "unit": "GFlop/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32" if prec == 4 else "f64", "data": "synthetic",
+            "config": {"workload": f"red-black Shamir DWF Schur complement S = Mooee - 1/4 DhopEO Mooee^-1 DhopOE on the even sites of "
+                                   f"{d[0]}x{d[1]}x{d[2]}x{d[3]} x Ls={Ls} fp{8 * prec}, M5={M5}, m={mass} (SURVEY.md 8(f2)); value counts "
+                                   "the two Dhops' 1320 flop/site only",
+                       "name": args.workload, "dims": list(d), "Ls": Ls, "l2": "fields larger than L2; no flush",
+                       "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "clocks": clocks, "gpu_launches": int(launches),
+            "roofline": {"bound": "hbm", "kernel": "s_op_kernel (Mooee^-1, one read + one write of a half field)",
+                         "achieved": b_inv / (t_inv * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                         "frac": b_inv / (t_inv * 1e-3) / 1e9 / peak, "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": b_inv, "traffic": ncu_traffic("schur", "s_op_kernel")[0]},
+            "schur_step": {"algorithmic_bytes": total_model, "achieved_gbs": total_model / (ms_step * 1e-3) / 1e9,
+                           "frac": total_model / (ms_step * 1e-3) / 1e9 / peak},
+            "kernels": kernels,
+        }
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def spawn_ranks(n: int, argv, check_devices: bool = True) -> int:
     """`python bench.py --gpus N` without a launcher: start N ranks of this script under
     torch.distributed.run on this node (one per GPU, rendezvous on 127.0.0.1) and return its exit
@@ -484,6 +592,8 @@ def main():
         sys.exit(spawn_ranks(args.gpus, sys.argv[1:]))
     if args.impl == "reference":
         run_reference(args, w)
+    elif w.get("kind") == "schur":
+        run_gpu_schur(args, w)
     else:
         run_gpu(args, w)
 

@@ -104,10 +104,9 @@ DWF_API int dwf_dhop_eo_dag(const dwf_geometry *g, const void *in_odd, void *out
 
 /* The Wilson-matrix fusion of SURVEY.md 8(f1):  out = a x + b (DhopOE in)   resp.   a x + b (DhopEO in),
  * x and out half fields of the OUTPUT parity.  With a = 4 + m, b = -1/2 this is one half of the
- * even/odd Wilson matrix M = (4 + m) - Dhop/2, with a = 1 one half of its Schur complement.  The fast
- * fp32 kernel stages x by TMA next to the input slice and combines in its store epilogue (one
- * pass; x == out allowed); other geometries / fp64 run Dhop followed by an elementwise pass
- * (x == out is then UNSUPPORTED).  a, b are rounded to the geometry's precision.  `in` must differ
+ * even/odd Wilson matrix M = (4 + m) - Dhop/2, with a = 1 one half of its Schur complement.  Every
+ * kernel combines in its store epilogue (one pass; the fast fp32 kernel stages x by TMA next to the input
+ * slice); x == out is allowed.  a, b are rounded to the geometry's precision.  `in` must differ
  * from x and out.  Asynchronous on `stream`.  Errors as dwf_dhop_oe. */
 DWF_API int dwf_dhop_oe_axpy(const dwf_geometry *g, const void *in_even, const void *x_odd, double a, double b,
                      void *out_odd, void *stream);
@@ -132,6 +131,55 @@ DWF_API int dwf_dhop_eo_norm2(const dwf_geometry *g, const void *in_odd, void *o
 /* result_host[0..1] = (re, im) of sum conj(a) b.  Same rules as dwf_norm2. */
 DWF_API int dwf_inner_product(const dwf_geometry *g, const void *a, const void *b, int parity,
                       double result_host[2], void *stream);
+
+/* ---- The rest of the red-black domain-wall operator (section 4: "all
+ * kernels involved in the DWF Dirac operator", L250 Fig.5, L254 Fig.6 -- named, never printed).  The
+ * definition is the standard Shamir domain-wall matrix (reading #22), with domain-wall
+ * height M5 and fermion mass `mass`:
+ *
+ *   (M psi)(x,s) = (5 - M5) psi(x,s) - 1/2 (Dhop psi)(x,s) - P_- psi(x,s+1) - P_+ psi(x,s-1),
+ *   P_+- = (1 +- gamma5)/2, gamma5 = diag(+1,+1,-1,-1),  psi(x,Ls) = -mass psi(x,0),  psi(x,-1) = -mass psi(x,Ls-1).
+ *
+ * "Mooee" is M without the Dhop term: diagonal in the 4D site, it couples the slices s of one site.
+ * With the 4D checkerboard, M = [Mee Meo; Moe Moo] with Mee = Moo = Mooee, Meo = -1/2 DhopEO,
+ * Moe = -1/2 DhopOE.  `dagger` != 0 selects the adjoint of the operator everywhere below.
+ * All fields are in the device layout; all calls but dwf_cg_schur are asynchronous on `stream`. */
+
+/* out = Mooee in  /  out = Mooee^{-1} in  on a full (DWF_FULL) or half field of `parity`.  One read and
+ * one write of the field (a thread walks the Ls slices of one 128-bit vector; Ls <= 32; larger Ls
+ * re-reads).  in == out is allowed for Ls <= 32.  Errors: INVALID_ARG (NULL, misaligned, bad parity,
+ * singular Mooee: M5 = 5 or 1 + mass (5-M5)^-Ls = 0), UNSUPPORTED (in == out with Ls > 32), CUDA. */
+DWF_API int dwf_mooee(const dwf_geometry *g, const void *in, void *out, int parity, double M5, double mass,
+                      int dagger, void *stream);
+DWF_API int dwf_mooee_inv(const dwf_geometry *g, const void *in, void *out, int parity, double M5, double mass,
+                          int dagger, void *stream);
+
+/* out = M in on full fields (the unpreconditioned matrix): Mooee, then a x + b Dhop fused into the two
+ * half-Dhop launches.  in != out.  Errors as dwf_dhop. */
+DWF_API int dwf_ddwf(const dwf_geometry *g, const void *in_full, void *out_full, double M5, double mass, int dagger,
+                     void *stream);
+
+/* Schur complement of M on the sites of `parity` p (DWF_EVEN / DWF_ODD), q = 1 - p:
+ *   S = Mooee - M_pq Mooee^{-1} M_qp = Mooee - 1/4 D_pq Mooee^{-1} D_qp        (in, out: half fields of parity p)
+ * Four kernels: Dhop, Mooee^{-1}, Mooee, a x + b Dhop.  `work`: dwf_schur_work_bytes(g) bytes of device
+ * memory owned by the caller (two half fields), 16-byte aligned.  in != out.  Errors as dwf_dhop_oe. */
+DWF_API size_t dwf_schur_work_bytes(const dwf_geometry *g);
+DWF_API int dwf_schur(const dwf_geometry *g, const void *in, void *out, int parity, double M5, double mass, int dagger,
+                      void *work, void *stream);
+
+/* out = a x + b y elementwise on fields of `parity` (any of x, y may be out). */
+DWF_API int dwf_axpby(const dwf_geometry *g, double a, const void *x, double b, const void *y, void *out, int parity,
+                      void *stream);
+
+/* Solve S x = b on parity p by conjugate gradients on the normal equations S^dag S x = S^dag b, start
+ * vector 0, in the geometry's precision (reductions in fp64).  Stops when |S^dag (b - S x)| <= tol |S^dag b|
+ * (recursive residual) or after max_iter iterations; *iters_out = iterations done, *resid_out = the TRUE
+ * relative residual |b - S x| / |b| recomputed at the end (either may be NULL).  `work`:
+ * dwf_cg_work_bytes(g) bytes of device memory (six half fields).  Synchronises `stream` (two host
+ * round trips per iteration for the step lengths).  Not reaching tol is not an error: check *resid_out. */
+DWF_API size_t dwf_cg_work_bytes(const dwf_geometry *g);
+DWF_API int dwf_cg_schur(const dwf_geometry *g, const void *b, void *x, int parity, double M5, double mass, double tol,
+                         int max_iter, void *work, int *iters_out, double *resid_out, void *stream);
 
 /* Bytes of a device field: full (DWF_FULL) or half (DWF_EVEN / DWF_ODD).  0 on bad arguments. */
 DWF_API size_t dwf_field_bytes(const dwf_geometry *g, int parity);

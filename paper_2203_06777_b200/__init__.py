@@ -28,6 +28,7 @@ SYMBOLS = (
     "dwf_dhop_eo", "dwf_dhop_dag", "dwf_dhop_oe_dag", "dwf_dhop_eo_dag", "dwf_dhop_oe_axpy", "dwf_dhop_eo_axpy", "dwf_dhop_oe_norm2", "dwf_dhop_eo_norm2", "dwf_norm2", "dwf_inner_product", "dwf_field_bytes",
     "dwf_import_spinor", "dwf_export_spinor", "dwf_launch_count", "dwf_kernel_info", "dwf_set_option",
     "dwf_error_string", "dwf_last_error",
+    "dwf_mooee", "dwf_mooee_inv", "dwf_ddwf", "dwf_schur_work_bytes", "dwf_schur", "dwf_axpby", "dwf_cg_work_bytes", "dwf_cg_schur",
 )
 
 
@@ -70,6 +71,16 @@ def load(build_if_missing: bool = True):
     lib.dwf_launch_count.argtypes = []
     lib.dwf_launch_count.restype = ctypes.c_ulonglong
     lib.dwf_kernel_info.argtypes = [vp, ctypes.c_char_p, cs]
+    dbl = ctypes.c_double
+    for f in (lib.dwf_mooee, lib.dwf_mooee_inv):
+        f.argtypes = [vp, vp, vp, ci, dbl, dbl, ci, vp]
+    lib.dwf_ddwf.argtypes = [vp, vp, vp, dbl, dbl, ci, vp]
+    lib.dwf_schur.argtypes = [vp, vp, vp, ci, dbl, dbl, ci, vp, vp]
+    lib.dwf_axpby.argtypes = [vp, dbl, vp, dbl, vp, vp, ci, vp]
+    lib.dwf_cg_schur.argtypes = [vp, vp, vp, ci, dbl, dbl, dbl, ci, vp, ctypes.POINTER(ci), ctypes.POINTER(dbl), vp]
+    for f in (lib.dwf_schur_work_bytes, lib.dwf_cg_work_bytes):
+        f.argtypes = [vp]
+        f.restype = cs
     lib.dwf_set_option.argtypes = [vp, ctypes.c_char_p, ctypes.c_longlong]
     lib.dwf_error_string.argtypes = [ci]
     lib.dwf_error_string.restype = ctypes.c_char_p
@@ -244,6 +255,54 @@ def dwf_export_spinor(g: int, field_dev, parity: int, canonical, stream=None) ->
            "dwf_export_spinor")
 
 
+def dwf_mooee(g: int, inp, out, parity: int, M5: float, mass: float, dagger: bool = False, stream=None) -> None:
+    _check(load().dwf_mooee(g, _dev_ptr(inp, g, parity), _dev_ptr(out, g, parity), int(parity), float(M5), float(mass),
+                            int(bool(dagger)), _stream(stream, g)), "dwf_mooee")
+
+
+def dwf_mooee_inv(g: int, inp, out, parity: int, M5: float, mass: float, dagger: bool = False, stream=None) -> None:
+    _check(load().dwf_mooee_inv(g, _dev_ptr(inp, g, parity), _dev_ptr(out, g, parity), int(parity), float(M5), float(mass),
+                                int(bool(dagger)), _stream(stream, g)), "dwf_mooee_inv")
+
+
+def dwf_ddwf(g: int, in_full, out_full, M5: float, mass: float, dagger: bool = False, stream=None) -> None:
+    _check(load().dwf_ddwf(g, _dev_ptr(in_full, g, FULL), _dev_ptr(out_full, g, FULL), float(M5), float(mass),
+                           int(bool(dagger)), _stream(stream, g)), "dwf_ddwf")
+
+
+def dwf_schur_work_bytes(g: int) -> int:
+    return int(load().dwf_schur_work_bytes(g))
+
+
+def dwf_cg_work_bytes(g: int) -> int:
+    return int(load().dwf_cg_work_bytes(g))
+
+
+def _work_ptr(t, need: int) -> int:
+    if not getattr(t, "is_cuda", False) or not t.is_contiguous() or t.numel() * t.element_size() < need:
+        raise DwfError(ERR_INVALID_ARG, "binding", f"workspace must be a contiguous CUDA tensor of at least {need} bytes")
+    return t.data_ptr()
+
+
+def dwf_schur(g: int, inp, out, parity: int, M5: float, mass: float, work, dagger: bool = False, stream=None) -> None:
+    _check(load().dwf_schur(g, _dev_ptr(inp, g, parity), _dev_ptr(out, g, parity), int(parity), float(M5), float(mass),
+                            int(bool(dagger)), _work_ptr(work, dwf_schur_work_bytes(g)), _stream(stream, g)), "dwf_schur")
+
+
+def dwf_axpby(g: int, a: float, x, b: float, y, out, parity: int, stream=None) -> None:
+    _check(load().dwf_axpby(g, float(a), _dev_ptr(x, g, parity), float(b), _dev_ptr(y, g, parity), _dev_ptr(out, g, parity),
+                            int(parity), _stream(stream, g)), "dwf_axpby")
+
+
+def dwf_cg_schur(g: int, b, x, parity: int, M5: float, mass: float, tol: float, max_iter: int, work, stream=None):
+    """Returns (iterations, true relative residual)."""
+    it, res = ctypes.c_int(), ctypes.c_double()
+    _check(load().dwf_cg_schur(g, _dev_ptr(b, g, parity), _dev_ptr(x, g, parity), int(parity), float(M5), float(mass),
+                               float(tol), int(max_iter), _work_ptr(work, dwf_cg_work_bytes(g)), ctypes.byref(it),
+                               ctypes.byref(res), _stream(stream, g)), "dwf_cg_schur")
+    return it.value, res.value
+
+
 def dwf_launch_count() -> int:
     return int(load().dwf_launch_count())
 
@@ -376,6 +435,43 @@ class Geometry:
 
     def inner_product(self, a, b, parity: int = FULL, stream=None) -> complex:
         return dwf_inner_product(self.handle, a, b, parity, stream)
+
+    # ---- the rest of the red-black domain-wall operator ----
+    def new_work(self, nbytes: int):
+        return self._torch.empty(nbytes, dtype=self._torch.uint8, device=f"cuda:{self.device}")
+
+    def mooee(self, inp, parity, M5, mass, dagger=False, out=None, stream=None):
+        out = self.new_field(parity) if out is None else out
+        dwf_mooee(self.handle, inp, out, parity, M5, mass, dagger, stream)
+        return out
+
+    def mooee_inv(self, inp, parity, M5, mass, dagger=False, out=None, stream=None):
+        out = self.new_field(parity) if out is None else out
+        dwf_mooee_inv(self.handle, inp, out, parity, M5, mass, dagger, stream)
+        return out
+
+    def ddwf(self, inp, M5, mass, dagger=False, out=None, stream=None):
+        out = self.new_field(FULL) if out is None else out
+        dwf_ddwf(self.handle, inp, out, M5, mass, dagger, stream)
+        return out
+
+    def schur(self, inp, parity, M5, mass, dagger=False, out=None, work=None, stream=None):
+        out = self.new_field(parity) if out is None else out
+        work = self.new_work(dwf_schur_work_bytes(self.handle)) if work is None else work
+        dwf_schur(self.handle, inp, out, parity, M5, mass, work, dagger, stream)
+        return out
+
+    def axpby(self, a, x, b, y, parity, out=None, stream=None):
+        out = self.new_field(parity) if out is None else out
+        dwf_axpby(self.handle, a, x, b, y, out, parity, stream)
+        return out
+
+    def cg_schur(self, b, parity, M5, mass, tol, max_iter, x=None, work=None, stream=None):
+        """Solve S x = b: returns (x, iterations, true relative residual)."""
+        x = self.new_field(parity) if x is None else x
+        work = self.new_work(dwf_cg_work_bytes(self.handle)) if work is None else work
+        it, res = dwf_cg_schur(self.handle, b, x, parity, M5, mass, tol, max_iter, work, stream)
+        return x, it, res
 
     def set_option(self, key: str, value: int):
         dwf_set_option(self.handle, key, value)

@@ -20,12 +20,14 @@ LIB = os.path.join(HERE, "libdwf.so")
 OBJDIR = os.path.join(HERE, "build")
 
 # (source, object name, extra defines): dhop_staged.cu is compiled once per kernel MODE so that the
-# four sets of template instances build in parallel
+# five sets of template instances build in parallel
 SOURCES = [("dhop_staged64.cu", "dhop_staged64.o", []), ("api.cu", "api.o", []), ("pack.cu", "pack.o", []), ("dhop.cu", "dhop.o", []), ("reduce.cu", "reduce.o", []),
            ("dhop_staged.cu", "dhop_staged_m0.o", ["-DDWF_STAGED_MODE=0"]),
            ("dhop_staged.cu", "dhop_staged_m1.o", ["-DDWF_STAGED_MODE=1"]),
            ("dhop_staged.cu", "dhop_staged_m2.o", ["-DDWF_STAGED_MODE=2"]),
-           ("dhop_staged.cu", "dhop_staged_m3.o", ["-DDWF_STAGED_MODE=3"])]
+           ("dhop_staged.cu", "dhop_staged_m3.o", ["-DDWF_STAGED_MODE=3"]),
+           ("dhop_staged.cu", "dhop_staged_m4.o", ["-DDWF_STAGED_MODE=4"]),
+           ("dwf5d.cu", "dwf5d.o", [])]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden",

@@ -20,18 +20,6 @@ void set_error(const char *fmt, ...)
     va_end(ap);
 }
 
-struct DeviceGuard {
-    int prev = -1;
-    bool ok = true;
-    explicit DeviceGuard(int dev)
-    {
-        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
-        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
-    }
-    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
-};
-
-
 // largest power-of-two exponent <= want that divides extent
 static int fit_shift(int extent, int want)
 {
@@ -144,8 +132,8 @@ static int ensure_staging(dwf_geometry *g, size_t bytes)
     return DWF_OK;
 }
 
-static bool parity_ok(int p) { return p == DWF_FULL || p == DWF_EVEN || p == DWF_ODD; }
-static bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+bool parity_ok(int p) { return p == DWF_FULL || p == DWF_EVEN || p == DWF_ODD; }
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
 
 }  // namespace dwf
 
@@ -347,18 +335,25 @@ int dwf_load_gauge(dwf_geometry *g, const void *U, int src_is_device, void *stre
     return DWF_OK;
 }
 
-// one half-Dhop: out (parity_out) = D in (opposite parity); picks the kernel
-static int half_dhop(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger = false)
+}  // extern "C"
+
+// one half-Dhop: out (parity_out) = D in (opposite parity), or a x + b D in when axpy_x is given; picks
+// the kernel.  Every kernel has the fused a x + b Dhop epilogue, x == out is allowed on all of them.
+int dwf::half_dhop(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger,
+                   const void *axpy_x, double a, double b)
 {
-    const bool staged_ok = g->staged.variant >= 0, staged64_ok = g->staged64.variant >= 0;
+    const bool staged_ok = g->staged.variant >= 0 && (!axpy_x || staged_supports_axpy(g)), staged64_ok = g->staged64.variant >= 0;
     if (g->opt_kernel == 2 && !staged_ok && !staged64_ok) {
         set_error("the staged kernels do not support this geometry / precision");
         return DWF_ERR_UNSUPPORTED;
     }
-    if (staged_ok && g->opt_kernel != 1) return launch_dhop_staged(g, in, out, parity_out, st, nullptr, nullptr, dagger);
-    if (staged64_ok && g->opt_kernel != 1) return launch_dhop_staged64(g, in, out, parity_out, st, dagger);
-    return launch_dhop_direct(g, in, out, parity_out, st, dagger);
+    if (staged_ok && g->opt_kernel != 1)
+        return launch_dhop_staged(g, in, out, parity_out, st, nullptr, nullptr, dagger, axpy_x, (float)a, (float)b);
+    if (staged64_ok && g->opt_kernel != 1) return launch_dhop_staged64(g, in, out, parity_out, st, dagger, axpy_x, a, b);
+    return launch_dhop_direct(g, in, out, parity_out, st, dagger, axpy_x, a, b);
 }
+
+extern "C" {
 
 static int dhop_common(const dwf_geometry *g, const void *in, void *out, int parity_out, void *stream, const char *who,
                        bool dagger = false)
@@ -405,12 +400,14 @@ int dwf_dhop_eo_dag(const dwf_geometry *g, const void *in_odd, void *out_even, v
     return dhop_common(g, in_odd, out_even, DWF_EVEN, stream, "dwf_dhop_eo_dag", true);
 }
 
+}  // extern "C"
+
 // Waits for the reduction last enqueued on `st` and returns its n values.  The final-sum kernel
 // writes them into mapped host memory followed by its sequence number, so the host polls that
 // word instead of paying a device-to-host copy plus a stream synchronise; cudaStreamQuery is
 // consulted now and then so that a failed launch surfaces as an error instead of a hang.  When the
 // sequence number is visible every earlier operation of the stream has completed (in-order stream).
-static int fetch_reduction(const dwf_geometry *g, cudaStream_t st, int n, double *out)
+int dwf::fetch_reduction(const dwf_geometry *g, cudaStream_t st, int n, double *out)
 {
     const unsigned long long want = g->mailbox_seq;
     volatile unsigned long long *seq = reinterpret_cast<volatile unsigned long long *>(g->mailbox_host + 2);
@@ -432,6 +429,8 @@ static int fetch_reduction(const dwf_geometry *g, cudaStream_t st, int n, double
     for (int i = 0; i < n; i++) out[i] = const_cast<const volatile double *>(g->mailbox_host)[i];
     return DWF_OK;
 }
+
+extern "C" {
 
 // out = D in on half fields and *result_host = norm2(out): the reduction runs in the epilogue of the
 // Dhop kernel (staged path) or as a second pass over `out` (direct path)
@@ -483,18 +482,7 @@ static int dhop_axpy_common(const dwf_geometry *g, const void *in, const void *x
     if (!g->gauge_loaded) { set_error("%s: call dwf_load_gauge first", who); return DWF_ERR_NO_GAUGE; }
     DeviceGuard guard(g->device);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const bool staged_ok = g->staged.variant >= 0;
-    if (g->opt_kernel == 2 && !(staged_ok && staged_supports_axpy(g))) {
-        set_error("the staged kernel does not support the fused axpy for this geometry / precision");
-        return DWF_ERR_UNSUPPORTED;
-    }
-    if (staged_ok && g->opt_kernel != 1 && staged_supports_axpy(g))
-        return launch_dhop_staged(g, in, out, parity_out, st, nullptr, nullptr, false, x, (float)a, (float)b);
-    // two passes: out = D in, then out = a x + b out (x == out would be overwritten by the first pass)
-    if (x == out) { set_error("%s: x == out needs the fused kernel, which this geometry / precision does not have", who); return DWF_ERR_UNSUPPORTED; }
-    int rc = half_dhop(g, in, out, parity_out, st);
-    if (rc) return rc;
-    return launch_axpby(g, x, out, a, b, dwf_field_bytes(g, parity_out) / (size_t)g->prec, st);
+    return half_dhop(g, in, out, parity_out, st, false, x, a, b);
 }
 
 int dwf_dhop_oe_axpy(const dwf_geometry *g, const void *in_even, const void *x_odd, double a, double b, void *out_odd, void *stream)

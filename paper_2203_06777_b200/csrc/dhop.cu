@@ -138,11 +138,13 @@ __device__ __forceinline__ void dhop_leg(typename CxT<T>::type (&acc)[12][SC],
 // One thread = one output site and one s-slice.
 // ---------------------------------------------------------------------------------------------
 // DAG: Dhop^dagger -- the projectors (1 - gamma) and (1 + gamma) change places
-template <typename T, int MAXT, int MINB, bool DAG>
+// AXPY: out = a x + b Dhop in, x a half field of the output parity read at the thread's own site (x may
+// be out: every thread reads its x before it writes)
+template <typename T, int MAXT, int MINB, bool DAG, bool AXPY>
 __global__ void __launch_bounds__(MAXT, MINB)
-dhop_direct_kernel(const typename CxT<T>::type *__restrict__ in, typename CxT<T>::type *__restrict__ out,
+dhop_direct_kernel(const typename CxT<T>::type *__restrict__ in, typename CxT<T>::type *out,
                    const T *__restrict__ gset, const int4 *__restrict__ tiles, const Lattice lat,
-                   const Tiling til, const int parity_out)
+                   const Tiling til, const int parity_out, const typename CxT<T>::type *xf, const T ca, const T cb)
 {
     using C = typename CxT<T>::type;
     constexpr int SC = 1;
@@ -196,7 +198,16 @@ dhop_direct_kernel(const typename CxT<T>::type *__restrict__ in, typename CxT<T>
     dhop_leg<T, SC, 3, false != DAG, false, 7>(acc, base + n3m, W0, gl);
 
     C *o = out + (size_t)s * 12 * (size_t)Vh + (size_t)own;
+    const C *xo = AXPY ? xf + (size_t)s * 12 * (size_t)Vh + (size_t)own : nullptr;
     if constexpr (sizeof(T) == 8) {
+        if constexpr (AXPY) {
+#pragma unroll
+            for (int k = 0; k < 12; k++) {
+                const C xv = xo[k * W0];
+                acc[k][0].x = fma(cb, acc[k][0].x, ca * xv.x);
+                acc[k][0].y = fma(cb, acc[k][0].y, ca * xv.y);
+            }
+        }
 #pragma unroll
         for (int k = 0; k < 12; k++) store_cx<SC>(o + k * W0, acc[k]);
     } else {
@@ -210,14 +221,23 @@ dhop_direct_kernel(const typename CxT<T>::type *__restrict__ in, typename CxT<T>
                 q[2][j] = C{acc[6 + c][j].x, acc[9 + c][j].x};
                 q[3][j] = C{acc[6 + c][j].y, acc[9 + c][j].y};
             }
+            if constexpr (AXPY) {
+#pragma unroll
+                for (int t = 0; t < 4; t++) {
+                    const C xv = xo[pair_off(4 * c + t, W0)];
+                    q[t][0].x = fmaf(cb, q[t][0].x, ca * xv.x);
+                    q[t][0].y = fmaf(cb, q[t][0].y, ca * xv.y);
+                }
+            }
 #pragma unroll
             for (int t = 0; t < 4; t++) store_cx<SC>(o + pair_off(4 * c + t, W0), q[t]);
         }
     }
 }
 
-template <typename T, int MAXT, int MINB, bool DAG>
-static int launch_direct(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st)
+template <typename T, int MAXT, int MINB, bool DAG, bool AXPY>
+static int launch_direct(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st,
+                         const void *x, double a, double b)
 {
     using C = typename CxT<T>::type;
     const Tiling &til = g->tiling_cb;
@@ -226,22 +246,30 @@ static int launch_direct(const dwf_geometry *g, const void *in, void *out, int p
         return DWF_ERR_UNSUPPORTED;
     }
     dim3 grid((unsigned)(til.ntiles * til.ncg)), block((unsigned)til.threads);
-    dhop_direct_kernel<T, MAXT, MINB, DAG><<<grid, block, 0, st>>>(
+    dhop_direct_kernel<T, MAXT, MINB, DAG, AXPY><<<grid, block, 0, st>>>(
         static_cast<const C *>(in), static_cast<C *>(out), static_cast<const T *>(g->gauge[parity_out]),
-        g->tiles_cb, g->lat, til, parity_out);
+        g->tiles_cb, g->lat, til, parity_out, static_cast<const C *>(x), (T)a, (T)b);
     count_launch();
     DWF_CUDA_CHECK(cudaGetLastError());
     return DWF_OK;
 }
 
-// parity_out: DWF_EVEN (DhopEO) or DWF_ODD (DhopOE)
-int launch_dhop_direct(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger)
+// parity_out: DWF_EVEN (DhopEO) or DWF_ODD (DhopOE); axpy_x != nullptr: out = a x + b Dhop in
+int launch_dhop_direct(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger,
+                       const void *axpy_x, double a, double b)
 {
-    if (g->prec == DWF_F32)
-        return dagger ? launch_direct<float, 256, 3, true>(g, in, out, parity_out, st)
-                      : launch_direct<float, 256, 3, false>(g, in, out, parity_out, st);
-    return dagger ? launch_direct<double, 256, 2, true>(g, in, out, parity_out, st)
-                  : launch_direct<double, 256, 2, false>(g, in, out, parity_out, st);
+    if (g->prec == DWF_F32) {
+        if (axpy_x)
+            return dagger ? launch_direct<float, 256, 3, true, true>(g, in, out, parity_out, st, axpy_x, a, b)
+                          : launch_direct<float, 256, 3, false, true>(g, in, out, parity_out, st, axpy_x, a, b);
+        return dagger ? launch_direct<float, 256, 3, true, false>(g, in, out, parity_out, st, nullptr, 0, 0)
+                      : launch_direct<float, 256, 3, false, false>(g, in, out, parity_out, st, nullptr, 0, 0);
+    }
+    if (axpy_x)
+        return dagger ? launch_direct<double, 256, 2, true, true>(g, in, out, parity_out, st, axpy_x, a, b)
+                      : launch_direct<double, 256, 2, false, true>(g, in, out, parity_out, st, axpy_x, a, b);
+    return dagger ? launch_direct<double, 256, 2, true, false>(g, in, out, parity_out, st, nullptr, 0, 0)
+                  : launch_direct<double, 256, 2, false, false>(g, in, out, parity_out, st, nullptr, 0, 0);
 }
 
 }  // namespace dwf

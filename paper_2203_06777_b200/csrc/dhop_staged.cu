@@ -205,7 +205,8 @@ __device__ __forceinline__ void staged_leg(float2 (&acc)[12], const float4 *__re
 // field).  MODE 2 (DAG): Dhop^dagger = the projectors (1 - gamma) and (1 + gamma) change places, same
 // links and neighbours.  MODE 3 (AXPY): out = a x + b Dhop in, with x a field of the
 // output parity staged by TMA next to the input slice and combined in the store epilogue (the
-// Wilson-matrix fusion of SURVEY.md 8(f1): one pass instead of Dhop followed by an axpy).
+// Wilson-matrix fusion of SURVEY.md 8(f1): one pass instead of Dhop followed by an axpy).  MODE 4: the
+// same with Dhop^dagger (the last kernel of the adjoint Schur complement).
 template <int LH, int B1, int B2, int B3, int MODE>
 __global__ void __launch_bounds__(StagedCfg<LH, B1, B2, B3>::NT, StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM)
 dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_x1,
@@ -214,7 +215,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
                    const __grid_constant__ CUtensorMap map_xc, const StagedArgs args)
 {
     using Cfg = StagedCfg<LH, B1, B2, B3>;
-    constexpr bool NORM = MODE == 1, DAG = MODE == 2, AXPY = MODE == 3;
+    constexpr bool NORM = MODE == 1, DAG = MODE == 2 || MODE == 4, AXPY = MODE == 3 || MODE == 4;
     // MODE 3 stages the rows box of the field x as well (read in the epilogue): NROW_C more rows per stage
     constexpr int STAGE = Cfg::STAGE_BYTES + (AXPY ? Cfg::NROW_C * Cfg::ROWB : 0);
     extern __shared__ __align__(1024) unsigned char smem[];
@@ -510,8 +511,8 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
 }
 
 // ---------------------------------------------------------------------------------------------
-// Kernel instances.  This file is compiled once per MODE (-DDWF_STAGED_MODE=0|1|2, build.py) so
-// that the three sets of instances build in parallel; each translation unit exports the entry
+// Kernel instances.  This file is compiled once per MODE (-DDWF_STAGED_MODE=0..4, build.py) so
+// that the five sets of instances build in parallel; each translation unit exports the entry
 // points of its MODE in the order of DWF_STAGED_VARIANTS, the MODE 0 unit also holds the host code.
 // Ordered by preference within one Lh: larger tiles (smaller halo ratio) first; the "variant"
 // option counts from 1 in this order.
@@ -525,6 +526,7 @@ const void *const *staged_kernels_mode0();
 const void *const *staged_kernels_mode1();
 const void *const *staged_kernels_mode2();
 const void *const *staged_kernels_mode3();
+const void *const *staged_kernels_mode4();
 
 #define DWF_CAT2(a, b) a##b
 #define DWF_CAT(a, b) DWF_CAT2(a, b)
@@ -543,8 +545,8 @@ const void *const *DWF_CAT(staged_kernels_mode, DWF_STAGED_MODE)()
 struct Variant {
     int lh, b1, b2, b3;
     int smem, threads, ctas_per_sm;
-    const void *fn[4];       // MODE 0 (Dhop), 1 (Dhop + norm2), 2 (Dhop^dagger), 3 (a x + b Dhop)
-    int smem_axpy;           // MODE 3 stages the rows box of x as well
+    const void *fn[5];       // MODE 0 (Dhop), 1 (Dhop + norm2), 2 (Dhop^dagger), 3 (a x + b Dhop), 4 (a x + b Dhop^dagger)
+    int smem_axpy;           // MODEs 3, 4 stage the rows box of x as well
 };
 
 static const std::vector<Variant> &variants()
@@ -552,10 +554,10 @@ static const std::vector<Variant> &variants()
     static const std::vector<Variant> v = [] {
         std::vector<Variant> t;
         const void *const *k0 = staged_kernels_mode0(), *const *k1 = staged_kernels_mode1(), *const *k2 = staged_kernels_mode2(),
-                          *const *k3 = staged_kernels_mode3();
+                          *const *k3 = staged_kernels_mode3(), *const *k4 = staged_kernels_mode4();
 #define X(LH, B1, B2, B3)                                                                            \
         t.push_back({LH, B1, B2, B3, StagedCfg<LH, B1, B2, B3>::SMEM_BYTES, StagedCfg<LH, B1, B2, B3>::NT,  \
-                     StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM, {k0[t.size()], k1[t.size()], k2[t.size()], k3[t.size()]},    \
+                     StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM, {k0[t.size()], k1[t.size()], k2[t.size()], k3[t.size()], k4[t.size()]},    \
                      StagedCfg<LH, B1, B2, B3>::SMEM_BYTES + 2 * StagedCfg<LH, B1, B2, B3>::NROW_C * StagedCfg<LH, B1, B2, B3>::ROWB});
         DWF_STAGED_VARIANTS(X)
 #undef X
@@ -581,8 +583,8 @@ void plan_staged(dwf_geometry *g)
         g->staged.ntiles = (lat.L[1] / v[i].b1) * (lat.L[2] / v[i].b2) * (lat.L[3] / v[i].b3);
         // Opt in to the large dynamic shared memory here, on the geometry's device (the attribute is per
         // device; the caller holds a DeviceGuard), for every kernel MODE of the chosen tile shape.
-        for (int mode = 0; mode < 4; mode++) {
-            const int smem = mode == 3 ? v[i].smem_axpy : v[i].smem;
+        for (int mode = 0; mode < 5; mode++) {
+            const int smem = mode >= 3 ? v[i].smem_axpy : v[i].smem;
             if (smem > SMEM_LIMIT) continue;
             if (cudaFuncSetAttribute(v[i].fn[mode], cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) {
                 cudaGetLastError();
@@ -679,13 +681,13 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
                        double *norm_partials, int *norm_blocks, bool dagger, const void *axpy_x, float axpy_a,
                        float axpy_b)
 {
-    if ((dagger && norm_partials) || (axpy_x && (dagger || norm_partials))) {
+    if (norm_partials && (dagger || axpy_x)) {
         set_error("the staged kernel has no instance for this combination of modes");
         return DWF_ERR_UNSUPPORTED;
     }
     const Variant &v = variants()[(size_t)g->staged.variant];
-    const int mode = norm_partials ? 1 : (dagger ? 2 : (axpy_x ? 3 : 0));
-    const int smem = mode == 3 ? v.smem_axpy : v.smem;
+    const int mode = norm_partials ? 1 : (axpy_x ? (dagger ? 4 : 3) : (dagger ? 2 : 0));
+    const int smem = mode >= 3 ? v.smem_axpy : v.smem;
     if (smem > SMEM_LIMIT) { set_error("tile too large for the fused axpy"); return DWF_ERR_UNSUPPORTED; }
     // The cache hands out pointers into its slots and the second lookup may evict the slot of the
     // first, so the maps are copied before it (they are passed to the kernel by value anyway).

@@ -36,6 +36,8 @@ struct Staged64Args {
     int ntiles;
     int L1, L2, L3, Ls;
     int parity_out;
+    const double2 *axpy_x;   // AXPY kernels: out = a x + b Dhop in (x on the output parity; may be out)
+    double axpy_a, axpy_b;
 };
 
 template <int LH, int B1, int B2, int B3> struct Staged64Cfg {
@@ -105,7 +107,7 @@ __device__ __forceinline__ void leg64(double2 (&acc)[12], const double2 p0, cons
 }
 
 // consumer body for colour column C (compile-time: the colour of a warp is uniform)
-template <int LH, int B1, int B2, int B3, bool DAG, int C>
+template <int LH, int B1, int B2, int B3, bool DAG, bool AXPY, int C>
 __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned char *smem, const uint32_t full_base,
                                           const uint32_t empty_base, const int site, const int my_tiles)
 {
@@ -162,6 +164,16 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
         double2 *orow = args.out + grow * (12 * LH) + h;                // + s * nrow * 12 * LH + k * LH
         for (int s = 0; s < args.Ls; s++, g++) {
             const int stage = g & 1;
+            // AXPY: this thread's four components of x, requested before the wait so that the global-memory
+            // latency hides behind the legs
+            double2 xv[4];
+            if constexpr (AXPY) {
+                if (active) {
+                    const double2 *xp = args.axpy_x + (orow - args.out) + (long long)s * nrow * (12 * LH);
+#pragma unroll
+                    for (int j = 0; j < 4; j++) xv[j] = __ldcs(xp + (4 * C + j) * LH);
+                }
+            }
             mbar_wait(full_base + 8 * stage, (g >> 1) & 1);
             const unsigned char *sb = smem + stage * Cfg::STAGE_BYTES;
             double2 acc[12];
@@ -205,8 +217,12 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
                 for (int j = 0; j < 4; j++) {
                     const double2 a0 = red[((((buf * 3 + C) * 2 + 0) * 4 + j) * Cfg::TP) + site];
                     const double2 a1 = red[((((buf * 3 + C) * 2 + 1) * 4 + j) * Cfg::TP) + site];
-                    const double2 v = cadd(cadd(acc[4 * C + j], a0), a1);
+                    double2 v = cadd(cadd(acc[4 * C + j], a0), a1);
                     const int k = 4 * C + j;
+                    if constexpr (AXPY) {
+                        v.x = fma(args.axpy_b, v.x, args.axpy_a * xv[j].x);
+                        v.y = fma(args.axpy_b, v.y, args.axpy_a * xv[j].y);
+                    }
                     __stcs(o2 + k * LH, v);
                 }
             }
@@ -214,7 +230,7 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
     }
 }
 
-template <int LH, int B1, int B2, int B3, bool DAG>
+template <int LH, int B1, int B2, int B3, bool DAG, bool AXPY>
 __global__ void __launch_bounds__(Staged64Cfg<LH, B1, B2, B3>::NT, 1)
 dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_x1,
                      const __grid_constant__ CUtensorMap map_x2, const __grid_constant__ CUtensorMap map_x3,
@@ -273,9 +289,9 @@ dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_con
     const int ctid = tid - 128;
     if (ctid >= 3 * Cfg::TP) return;
     const int c = ctid / Cfg::TP, site = ctid % Cfg::TP;         // colour-major: uniform per warp
-    if (c == 0)      consume64<LH, B1, B2, B3, DAG, 0>(args, smem, full_base, empty_base, site, my_tiles);
-    else if (c == 1) consume64<LH, B1, B2, B3, DAG, 1>(args, smem, full_base, empty_base, site, my_tiles);
-    else             consume64<LH, B1, B2, B3, DAG, 2>(args, smem, full_base, empty_base, site, my_tiles);
+    if (c == 0)      consume64<LH, B1, B2, B3, DAG, AXPY, 0>(args, smem, full_base, empty_base, site, my_tiles);
+    else if (c == 1) consume64<LH, B1, B2, B3, DAG, AXPY, 1>(args, smem, full_base, empty_base, site, my_tiles);
+    else             consume64<LH, B1, B2, B3, DAG, AXPY, 2>(args, smem, full_base, empty_base, site, my_tiles);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -283,7 +299,7 @@ dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_con
 // ---------------------------------------------------------------------------------------------
 struct Variant64 {
     int lh, b1, b2, b3, smem, threads;
-    const void *fn[2];       // plain, dagger
+    const void *fn[4];       // plain, dagger, a x + b Dhop, a x + b Dhop^dagger
 };
 
 #define DWF_STAGED64_VARIANTS(X) X(16, 2, 1, 2) X(16, 1, 1, 4) X(16, 1, 2, 2) X(16, 2, 2, 1) X(8, 4, 2, 1) X(8, 2, 2, 2) X(4, 4, 4, 1) X(4, 4, 2, 2) X(4, 2, 2, 2) X(4, 2, 2, 1) X(8, 2, 2, 1) X(16, 2, 1, 1)
@@ -294,8 +310,10 @@ static const std::vector<Variant64> &variants64()
         std::vector<Variant64> t;
 #define X(LH, B1, B2, B3)                                                                             \
         t.push_back({LH, B1, B2, B3, Staged64Cfg<LH, B1, B2, B3>::SMEM_BYTES, Staged64Cfg<LH, B1, B2, B3>::NT, \
-                     {reinterpret_cast<const void *>(&dhop_staged64_kernel<LH, B1, B2, B3, false>),    \
-                      reinterpret_cast<const void *>(&dhop_staged64_kernel<LH, B1, B2, B3, true>)}});
+                     {reinterpret_cast<const void *>(&dhop_staged64_kernel<LH, B1, B2, B3, false, false>),    \
+                      reinterpret_cast<const void *>(&dhop_staged64_kernel<LH, B1, B2, B3, true, false>),     \
+                      reinterpret_cast<const void *>(&dhop_staged64_kernel<LH, B1, B2, B3, false, true>),     \
+                      reinterpret_cast<const void *>(&dhop_staged64_kernel<LH, B1, B2, B3, true, true>)}});
         DWF_STAGED64_VARIANTS(X)
 #undef X
         return t;
@@ -317,7 +335,7 @@ void plan_staged64(dwf_geometry *g)
         g->staged64.b[0] = v[i].b1; g->staged64.b[1] = v[i].b2; g->staged64.b[2] = v[i].b3;
         g->staged64.ntiles = (lat.L[1] / v[i].b1) * (lat.L[2] / v[i].b2) * (lat.L[3] / v[i].b3);
         // per-device opt-in to the large dynamic shared memory (the caller holds a DeviceGuard)
-        for (int d = 0; d < 2; d++)
+        for (int d = 0; d < 4; d++)
             if (cudaFuncSetAttribute(v[i].fn[d], cudaFuncAttributeMaxDynamicSharedMemorySize, v[i].smem) != cudaSuccess) {
                 cudaGetLastError();
                 g->staged64.variant = -1;
@@ -370,7 +388,8 @@ static int encode_map64(CUtensorMap *m, const void *base, const Lattice &lat, in
     return DWF_OK;
 }
 
-int launch_dhop_staged64(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger)
+int launch_dhop_staged64(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger,
+                         const void *axpy_x, double axpy_a, double axpy_b)
 {
     const Variant64 &v = variants64()[(size_t)g->staged64.variant];
     CUtensorMap mc, m1, m2, m3;
@@ -386,7 +405,10 @@ int launch_dhop_staged64(const dwf_geometry *g, const void *in, void *out, int p
     a.ntiles = g->staged64.ntiles;
     a.L1 = g->lat.L[1]; a.L2 = g->lat.L[2]; a.L3 = g->lat.L[3]; a.Ls = g->lat.Ls;
     a.parity_out = parity_out;
-    const void *fn = v.fn[dagger ? 1 : 0];
+    a.axpy_x = static_cast<const double2 *>(axpy_x);
+    a.axpy_a = axpy_a;
+    a.axpy_b = axpy_b;
+    const void *fn = v.fn[(dagger ? 1 : 0) + (axpy_x ? 2 : 0)];
     const int grid = g->staged64.ntiles < g->sm_count ? g->staged64.ntiles : g->sm_count;
     void *params[] = {&mc, &m1, &m2, &m3, &a};
     DWF_CUDA_CHECK(cudaLaunchKernel(fn, dim3((unsigned)grid), dim3((unsigned)v.threads), params, (size_t)v.smem, st));

@@ -110,6 +110,25 @@ namespace dwf {
 
 int rebuild_tilings(dwf_geometry *g);
 
+// api.cu helpers used by the other translation units
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+bool parity_ok(int p);
+bool aligned16(const void *p);
+// one half-Dhop (or a x + b Dhop) on the best kernel for the geometry
+int half_dhop(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger = false,
+              const void *axpy_x = nullptr, double a = 0.0, double b = 0.0);
+// waits for the reduction last enqueued on st and returns its n values (through the mapped mailbox)
+int fetch_reduction(const dwf_geometry *g, cudaStream_t st, int n, double *out);
+
 // pack.cu
 int launch_pack_gauge(const dwf_geometry *g, const void *U_canonical_dev, cudaStream_t st);
 int launch_import(const dwf_geometry *g, const void *canonical_dev, int parity, void *field,
@@ -118,7 +137,7 @@ int launch_export(const dwf_geometry *g, const void *field, int parity, void *ca
                   cudaStream_t st);
 // dhop.cu (direct kernel; half fields only)
 int launch_dhop_direct(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st,
-                       bool dagger = false);
+                       bool dagger = false, const void *axpy_x = nullptr, double axpy_a = 0.0, double axpy_b = 0.0);
 // dhop_staged.cu (TMA-staged link-stationary kernel, fp32 half fields)
 void plan_staged(dwf_geometry *g);                      // fills g->staged (variant = -1 if unusable)
 void build_staged_tile_table(const dwf_geometry *g, int raster, int4 *host_table);
@@ -132,7 +151,8 @@ int launch_axpby(const dwf_geometry *g, const void *x, void *out, double a, doub
 // dhop_staged64.cu (TMA-staged fp64 kernel, links split by colour column over three threads)
 void plan_staged64(dwf_geometry *g);
 void build_staged64_tile_table(const dwf_geometry *g, int4 *host_table);
-int launch_dhop_staged64(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger);
+int launch_dhop_staged64(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger,
+                         const void *axpy_x = nullptr, double axpy_a = 0.0, double axpy_b = 0.0);
 // reduce.cu
 int launch_norm2(const dwf_geometry *g, const void *field, size_t nreal, cudaStream_t st);
 int launch_final_sum(const dwf_geometry *g, int nblocks, cudaStream_t st);   // result_dev[0] = sum of partials[0..nblocks)

@@ -71,6 +71,14 @@ def test_null_arguments():
         assert r.value == -1.0
     for f in (lib.dwf_dhop_oe_axpy, lib.dwf_dhop_eo_axpy):
         assert f(None, None, None, 1.0, 1.0, None, None) == dwf.ERR_INVALID_ARG
+    for f in (lib.dwf_mooee, lib.dwf_mooee_inv):
+        assert f(None, None, None, 0, 1.8, 0.1, 0, None) == dwf.ERR_INVALID_ARG
+    assert lib.dwf_ddwf(None, None, None, 1.8, 0.1, 0, None) == dwf.ERR_INVALID_ARG
+    assert lib.dwf_schur(None, None, None, 0, 1.8, 0.1, 0, None, None) == dwf.ERR_INVALID_ARG
+    assert lib.dwf_axpby(None, 1.0, None, 1.0, None, None, 0, None) == dwf.ERR_INVALID_ARG
+    assert lib.dwf_cg_schur(None, None, None, 0, 1.8, 0.1, 1e-8, 10, None, None, None, None) == dwf.ERR_INVALID_ARG
+    assert lib.dwf_schur_work_bytes(None) == 0 and lib.dwf_cg_work_bytes(None) == 0
+    assert lib.dwf_kernel_info(None, None, 0) == dwf.ERR_INVALID_ARG
     assert lib.dwf_set_option(None, b"kernel", 1) == dwf.ERR_INVALID_ARG
     assert lib.dwf_field_bytes(None, 0) == 0
     assert lib.dwf_destroy_geometry(None) == dwf.OK

@@ -1,7 +1,7 @@
 """GPU parity of the Wilson-matrix fusion: dwf_dhop_oe_axpy / dwf_dhop_eo_axpy,
 out = a x + b Dhop in, against a x + b (oracle Dhop) evaluated in fp64 -- on the staged fp32 kernel
-(x staged by TMA, combined in the store epilogue; several tiles per CTA) and on the two-pass path
-(fp64, shapes without a staged variant).  Bars: relative L2 error <= 2e-6 (fp32), <= 1e-13 (fp64)."""
+(x staged by TMA, combined in the store epilogue; several tiles per CTA) and on the fp64 staged and the
+direct kernels (x read at the thread's own site in the epilogue).  Bars: relative L2 error <= 2e-6 (fp32), <= 1e-13 (fp64)."""
 import numpy as np
 import pytest
 
@@ -14,7 +14,7 @@ pytestmark = pytest.mark.gpu
 TOL = {4: 2e-6, 8: 1e-13}
 
 CASES = [
-    # dims, Ls, prec, bc, fused (staged) path expected
+    # dims, Ls, prec, bc, staged fp32 kernel expected (forced with kernel = 2)
     ((32, 16, 16, 16), 4, 4, 1, True), ((48, 12, 12, 12), 3, 4, 0, True), ((16, 8, 8, 12), 6, 4, 1, True),
     ((8, 8, 12, 8), 5, 4, 0, True), ((8, 8, 8, 8), 8, 8, 1, False), ((24, 4, 4, 4), 5, 4, 1, False),
     ((4, 4, 4, 4), 4, 8, 0, False),
@@ -41,17 +41,12 @@ def test_dhop_axpy_matches_oracle(lib, dims, Ls, prec, bc, fused):
             out = call(fin, fx, a, b)
             want = a * x.astype(np.float64) + b * oracle.dhop_cb(dims, Ls, bc, p_out, U, half)
             assert rel_err(g.export_spinor(out, p_out), want) <= TOL[prec]
-            # a = 0, b = 1 is the plain operator, bit for bit on the fused path
+            # a = 0, b = 1 is the plain operator, bit for bit (every kernel combines in its store epilogue)
             plain = g.dhop_oe(fin) if p_out == 1 else g.dhop_eo(fin)
-            assert rel_err(g.export_spinor(call(fin, fx, 0.0, 1.0), p_out), g.export_spinor(plain, p_out)) <= (0 if fused else TOL[prec])
-            if fused:                            # x may be the output buffer
-                inplace = fx.clone()
-                call(fin, inplace, a, b, out=inplace)
-                assert torch.equal(inplace, out)
-            else:
-                with pytest.raises(lib.DwfError) as e:
-                    call(fin, fx, a, b, out=fx)
-                assert e.value.code == lib.ERR_UNSUPPORTED
+            assert torch.equal(call(fin, fx, 0.0, 1.0), plain)
+            inplace = fx.clone()                 # x may be the output buffer
+            call(fin, inplace, a, b, out=inplace)
+            assert torch.equal(inplace, out)
             with pytest.raises(lib.DwfError) as e:
                 call(fin, fin, a, b)
             assert e.value.code == lib.ERR_INVALID_ARG
