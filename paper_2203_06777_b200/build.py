@@ -19,9 +19,10 @@ ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libdwf.so")
 OBJDIR = os.path.join(HERE, "build")
 
-# (source, object name, extra defines): dhop_staged.cu is compiled once per kernel MODE so that the
-# five sets of template instances build in parallel
-SOURCES = [("dhop_staged64.cu", "dhop_staged64.o", []), ("api.cu", "api.o", []), ("pack.cu", "pack.o", []), ("dhop.cu", "dhop.o", []), ("reduce.cu", "reduce.o", []),
+# (source, object name, extra defines): dhop_staged.cu and dhop_staged64.cu are compiled once per kernel
+# MODE so that the sets of template instances build in parallel
+SOURCES = [*[("dhop_staged64.cu", f"dhop_staged64_m{m}.o", [f"-DDWF_STAGED64_MODE={m}"]) for m in range(5)],
+           ("api.cu", "api.o", []), ("pack.cu", "pack.o", []), ("dhop.cu", "dhop.o", []), ("reduce.cu", "reduce.o", []),
            ("dhop_staged.cu", "dhop_staged_m0.o", ["-DDWF_STAGED_MODE=0"]),
            ("dhop_staged.cu", "dhop_staged_m1.o", ["-DDWF_STAGED_MODE=1"]),
            ("dhop_staged.cu", "dhop_staged_m2.o", ["-DDWF_STAGED_MODE=2"]),

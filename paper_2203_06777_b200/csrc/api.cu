@@ -454,6 +454,11 @@ static int dhop_norm2_common(const dwf_geometry *g, const void *in, void *out, i
         rc = launch_dhop_staged(g, in, out, parity_out, st, g->partials, &nblocks);
         if (rc) return rc;
         rc = launch_final_sum(g, nblocks, st);
+    } else if (g->staged64.variant >= 0 && g->opt_kernel != 1) {
+        int nblocks = 0;
+        rc = launch_dhop_staged64(g, in, out, parity_out, st, false, nullptr, 0.0, 0.0, g->partials, &nblocks);
+        if (rc) return rc;
+        rc = launch_final_sum(g, nblocks, st);
     } else {
         rc = half_dhop(g, in, out, parity_out, st);
         if (rc) return rc;

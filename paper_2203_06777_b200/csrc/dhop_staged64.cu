@@ -11,14 +11,16 @@
 // full kernel does (projection, SU(3) product and reconstruction are linear, so the sum over c can
 // wait until all 8 legs are done).  After the legs the three threads of a site exchange partial sums
 // through shared memory (each owns 4 of the 12 output components), add them in a fixed order and
-// store.  Threads are colour-major (a warp = one colour of 32 consecutive sites), so every LDS / STG is
-// conflict-free and coalesced and there is no divergence.
+// store.  The exchange is deferred by one step and signalled through mbarriers (consume64), so no warp
+// waits for its partners inside a step.  Threads are colour-major (a warp = one colour of 32 consecutive
+// sites), so every LDS / STG is conflict-free and coalesced and there is no divergence.
 // Everything else follows dhop_staged.cu: a producer warpgroup (setmaxnreg) issues 5-D bulk tensor
 // copies (TMA) of the input slice -- rows box + 6 faces -- into a two-stage shared-memory ring with
 // full / empty mbarriers; consumers walk all Ls slices of a tile with their link columns in registers.
 // Layouts (pack.cu): spinor complex[s][row][k][h], k = spin*3 + colour (one plane per component:
 // consecutive sites are consecutive 128-bit words); links
 // complex[row][f/2][h][f&1], f = leg*9 + a*3 + b.
+#include <type_traits>
 #include <vector>
 
 #include "complex_ops.cuh"
@@ -26,6 +28,10 @@
 #include "tma.cuh"
 
 namespace dwf {
+
+#ifndef DWF_STAGED64_MODE
+#define DWF_STAGED64_MODE 0     // which kernel MODE this translation unit instantiates (build.py compiles the file once per MODE)
+#endif
 
 PFN_tensorMapEncodeTiled get_tensor_map_encoder();      // dhop_staged.cu
 
@@ -36,15 +42,18 @@ struct Staged64Args {
     int ntiles;
     int L1, L2, L3, Ls;
     int parity_out;
+    int zigzag;              // walk the slices of every other tile backwards (L2 reuse between tiles)
+    int l2pol;               // decimal digits: digit 0 input boxes, 6 links, 7 output (0 normal, 1 evict_first, 2 evict_last)
     const double2 *axpy_x;   // AXPY kernels: out = a x + b Dhop in (x on the output parity; may be out)
     double axpy_a, axpy_b;
+    double *norm_partials;   // NORM kernels: one partial sum of |out|^2 per CTA (fixed order inside the CTA)
 };
 
 template <int LH, int B1, int B2, int B3> struct Staged64Cfg {
     static constexpr int NROW_C = B1 * B2 * B3;
     static constexpr int T = LH * NROW_C;                        // output sites per tile
     static constexpr int TP = (T + 31) / 32 * 32;                // sites padded to whole warps: thread = colour * TP + site
-    static constexpr int NGROUP = TP / 32;                       // 32-site groups = named barriers
+    static constexpr int NGROUP = TP / 32;                       // 32-site groups: three warps (one per colour) each
     static constexpr int NWARP_C = 3 * NGROUP;
     static constexpr int NTC = (3 * TP + 127) / 128 * 128;       // consumer threads (whole warpgroups)
     static constexpr int NT = 128 + NTC;
@@ -56,8 +65,9 @@ template <int LH, int B1, int B2, int B3> struct Staged64Cfg {
     static constexpr int NSTAGE = 2;
     // exchange buffer: [parity of the step][destination colour][source slot][component j][site] complex
     static constexpr int RED_BYTES = 2 * 3 * 2 * 4 * TP * 16;
-    static constexpr int TAIL = 64;                              // full[2], empty[2] mbarriers
-    static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + RED_BYTES + TAIL;
+    // tail: full[2], empty[2][4 regions], exch[NGROUP][2] mbarriers, one fp64 slot per consumer warp (fused norm2)
+    static constexpr int TAIL_EXCH = 16 + 64, TAIL_NORM = TAIL_EXCH + 16 * NGROUP, TAIL = TAIL_NORM + 8 * NWARP_C;
+    static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + RED_BYTES + (TAIL + 15) / 16 * 16;
     static constexpr int PROD_REGS = 24;
     static constexpr int CONS_REGS_RAW = ((65536 - 128 * PROD_REGS) / NTC) / 8 * 8;
     static constexpr int CONS_REGS = CONS_REGS_RAW > 240 ? 240 : CONS_REGS_RAW;
@@ -65,9 +75,23 @@ template <int LH, int B1, int B2, int B3> struct Staged64Cfg {
     static_assert(SMEM_BYTES <= 232448, "tile too large for shared memory");
 };
 
-// one leg for colour c: acc += reconstruct( U[:, c] * project(psi)[c] ).  p0..p3 = colour c of the four
-// spin components of the neighbour, U = (U_0c, U_1c, U_2c).  Signs as in dhop.cu (DeGrand-Rossi).
-template <int MU, bool FWD>
+__device__ __forceinline__ double2 ldg_d2_hint(const double2 *p, uint64_t policy)
+{
+    double2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(policy));
+    return v;
+}
+__device__ __forceinline__ void stg_d2_hint(double2 *p, double2 v, uint64_t policy)
+{
+    asm volatile("st.global.L1::no_allocate.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(policy) : "memory");
+}
+
+// one leg for colour column c: acc += reconstruct( U[:, c] * project(psi)[c] ).  p0..p3 = colour c of the
+// four spin components of the neighbour; U[r] = U_{(c+r)%3, c}, r = 0..2 (the rows of the column ROTATED
+// by the thread's colour, so that acc[spin*3 + r] is the partial sum for output colour (c+r)%3 and every
+// register index is a compile-time constant although c is a run-time value: one copy of the code for all
+// three colours).  Signs as in dhop.cu (DeGrand-Rossi).  FIRST: the leg that initialises the accumulators.
+template <int MU, bool FWD, bool FIRST>
 __device__ __forceinline__ void leg64(double2 (&acc)[12], const double2 p0, const double2 p1, const double2 p2,
                                       const double2 p3, const double2 *__restrict__ U)
 {
@@ -88,35 +112,69 @@ __device__ __forceinline__ void leg64(double2 (&acc)[12], const double2 p0, cons
 #pragma unroll
     for (int a = 0; a < 3; a++) {
         const double2 x0 = cmul(U[a], h0), x1 = cmul(U[a], h1);
-        acc[0 + a] = cadd(acc[0 + a], x0);
-        acc[3 + a] = cadd(acc[3 + a], x1);
-        if constexpr (MU == 0) {
-            acc[6 + a] = FWD ? caddi(acc[6 + a], x1) : csubi(acc[6 + a], x1);
-            acc[9 + a] = FWD ? caddi(acc[9 + a], x0) : csubi(acc[9 + a], x0);
-        } else if constexpr (MU == 1) {
-            acc[6 + a] = FWD ? csub(acc[6 + a], x1) : cadd(acc[6 + a], x1);
-            acc[9 + a] = FWD ? cadd(acc[9 + a], x0) : csub(acc[9 + a], x0);
-        } else if constexpr (MU == 2) {
-            acc[6 + a] = FWD ? caddi(acc[6 + a], x0) : csubi(acc[6 + a], x0);
-            acc[9 + a] = FWD ? csubi(acc[9 + a], x1) : caddi(acc[9 + a], x1);
+        if constexpr (FIRST) {
+            acc[0 + a] = x0;
+            acc[3 + a] = x1;
+            if constexpr (MU == 0) {
+                acc[6 + a] = FWD ? cmuli(x1) : cmulni(x1);
+                acc[9 + a] = FWD ? cmuli(x0) : cmulni(x0);
+            } else if constexpr (MU == 1) {
+                acc[6 + a] = FWD ? cneg(x1) : x1;
+                acc[9 + a] = FWD ? x0 : cneg(x0);
+            } else if constexpr (MU == 2) {
+                acc[6 + a] = FWD ? cmuli(x0) : cmulni(x0);
+                acc[9 + a] = FWD ? cmulni(x1) : cmuli(x1);
+            } else {
+                acc[6 + a] = FWD ? cneg(x0) : x0;
+                acc[9 + a] = FWD ? cneg(x1) : x1;
+            }
         } else {
-            acc[6 + a] = FWD ? csub(acc[6 + a], x0) : cadd(acc[6 + a], x0);
-            acc[9 + a] = FWD ? csub(acc[9 + a], x1) : cadd(acc[9 + a], x1);
+            acc[0 + a] = cadd(acc[0 + a], x0);
+            acc[3 + a] = cadd(acc[3 + a], x1);
+            if constexpr (MU == 0) {
+                acc[6 + a] = FWD ? caddi(acc[6 + a], x1) : csubi(acc[6 + a], x1);
+                acc[9 + a] = FWD ? caddi(acc[9 + a], x0) : csubi(acc[9 + a], x0);
+            } else if constexpr (MU == 1) {
+                acc[6 + a] = FWD ? csub(acc[6 + a], x1) : cadd(acc[6 + a], x1);
+                acc[9 + a] = FWD ? cadd(acc[9 + a], x0) : csub(acc[9 + a], x0);
+            } else if constexpr (MU == 2) {
+                acc[6 + a] = FWD ? caddi(acc[6 + a], x0) : csubi(acc[6 + a], x0);
+                acc[9 + a] = FWD ? csubi(acc[9 + a], x1) : caddi(acc[9 + a], x1);
+            } else {
+                acc[6 + a] = FWD ? csub(acc[6 + a], x0) : cadd(acc[6 + a], x0);
+                acc[9 + a] = FWD ? csub(acc[9 + a], x1) : cadd(acc[9 + a], x1);
+            }
         }
     }
 }
 
-// consumer body for colour column C (compile-time: the colour of a warp is uniform)
-template <int LH, int B1, int B2, int B3, bool DAG, bool AXPY, int C>
+// MODE bits: 1 = Dhop^dagger (projectors swapped), 2 = a x + b Dhop in the store epilogue, 4 = |out|^2
+// accumulated in the store epilogue (fused norm2; not combined with the others).
+//
+// Consumer body of thread (site, colour c); c is uniform in a warp.  Thread c ends up owning output colour
+// c (four spin components): of its 12 partial sums acc[spin*3 + r] it keeps the block r = 0 and hands the
+// blocks r = 1, 2 to the threads of colours (c+1)%3, (c+2)%3 through shared memory.
+// The colour exchange is DEFERRED by one step: after the 8 legs of step g a warp first finishes step g-1
+// (waits on that step's exchange mbarrier -- long since complete --, adds the two partial sums of its
+// partner warps to the block it kept in registers, stores), then publishes its own partial sums of step g
+// and arrives on the mbarrier of step g.  No warp waits for its partners inside a step; the three colour
+// warps of a 32-site group drift by up to one step.  Two exchange buffers suffice: a buffer is overwritten
+// at step g+2, after this warp has seen all arrivals of step g+1, each of which follows that warp's reads
+// of step g.
+template <int LH, int B1, int B2, int B3, int MODE>
 __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned char *smem, const uint32_t full_base,
-                                          const uint32_t empty_base, const int site, const int my_tiles)
+                                          const uint32_t empty_base, const uint32_t exch_base, const int site, const int c,
+                                          const int my_tiles, double &nsum)
 {
     using Cfg = Staged64Cfg<LH, B1, B2, B3>;
+    constexpr bool DAG = (MODE & 1) != 0, AXPY = (MODE & 2) != 0, NORM = (MODE & 4) != 0;
     const bool active = site < Cfg::T;
     const int st = active ? site : 0;
     const int h = st % LH, row = st / LH;
     const int i1 = row % B1, i2 = (row / B1) % B2, i3 = row / (B1 * B2);
     const int lane = threadIdx.x & 31;
+    // L2 eviction classes of the global accesses: option "l2pol", digits as in dhop_staged.cu (PC_*)
+    const uint64_t pol_first = l2_policy(args.l2pol / 1000000 % 10), pol_out = l2_policy(args.l2pol / 10000000 % 10);
 
     // staged rows of the 8 neighbours (tile-invariant except the x0 pair)
     const int rc = row;
@@ -126,111 +184,182 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
     const int r2m = (i2 > 0) ? rc - B1 : Cfg::R_X2M + i1 + B1 * i3;
     const int r3p = (i3 + 1 < B3) ? rc + B1 * B2 : Cfg::R_X3P + i1 + B1 * i2;
     const int r3m = (i3 > 0) ? rc - B1 * B2 : Cfg::R_X3M + i1 + B1 * i2;
-    uint32_t off[8];            // byte offsets of (neighbour site, component 0) inside a stage
-    off[2] = r1p * Cfg::ROWB + h * 16;
-    off[3] = r1m * Cfg::ROWB + h * 16;
-    off[4] = r2p * Cfg::ROWB + h * 16;
-    off[5] = r2m * Cfg::ROWB + h * 16;
-    off[6] = r3p * Cfg::ROWB + h * 16;
-    off[7] = r3m * Cfg::ROWB + h * 16;
-    // byte offset of component k = spin*3 + C inside a row block [k][h] of 16-byte complex
-    constexpr uint32_t KOFF0 = (0 * 3 + C) * LH * 16, KOFF1 = (1 * 3 + C) * LH * 16;
-    constexpr uint32_t KOFF2 = (2 * 3 + C) * LH * 16, KOFF3 = (3 * 3 + C) * LH * 16;
+    // byte offsets of (neighbour site, component k = 0*3 + c) inside a stage; the other three spin
+    // components of colour c follow at multiples of KSPIN
+    const uint32_t coff = (uint32_t)(c * LH + h) * 16;
+    constexpr uint32_t KSPIN = 3 * LH * 16;
+    uint32_t off[8];
+    off[2] = r1p * Cfg::ROWB + coff;
+    off[3] = r1m * Cfg::ROWB + coff;
+    off[4] = r2p * Cfg::ROWB + coff;
+    off[5] = r2m * Cfg::ROWB + coff;
+    off[6] = r3p * Cfg::ROWB + coff;
+    off[7] = r3m * Cfg::ROWB + coff;
 
     const long long nrow = (long long)args.L1 * args.L2 * args.L3;
+    // exchange buffer [buf][destination colour d][slot][spin j][site]: slot 0 comes from colour (d+2)%3
+    // (its block r = 1), slot 1 from colour (d+1)%3 (its block r = 2)
     double2 *red = reinterpret_cast<double2 *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES);
-    double2 U[24];              // column C of the 8 links: U[leg*3 + a] = U_leg[a][C]
+    const int c1 = c == 2 ? 0 : c + 1, c2 = c == 0 ? 2 : c - 1;        // (c+1)%3, (c+2)%3
+    double2 *red_w1 = red + (size_t)((c1 * 2 + 0) * 4) * Cfg::TP + site;   // my block r = 1 -> colour c1, slot 0
+    double2 *red_w2 = red + (size_t)((c2 * 2 + 1) * 4) * Cfg::TP + site;   // my block r = 2 -> colour c2, slot 1
+    const double2 *red_r = red + (size_t)((c * 2) * 4) * Cfg::TP + site;   // what the partners left for colour c
+    constexpr int RED_BUF = 3 * 2 * 4 * Cfg::TP;                            // complex numbers per buffer
+    const uint32_t my_exch = exch_base + 16 * (site >> 5);      // exch[group][2]
+    double2 U[24];              // column c of the 8 links, rows rotated: U[leg*3 + r] = U_leg[(c+r)%3][c]
+
+    // global row of this thread's site in the it-th tile, and the parity bit r of x0 = 2h + r
+    auto tile_row = [&](int it, int &r) -> long long {
+        const int4 o = args.tiles[blockIdx.x + it * gridDim.x];
+        const int x1 = o.x + i1, x2 = o.y + i2, x3 = o.z + i3;
+        r = (x1 + x2 + x3 + args.parity_out) & 1;
+        return x1 + (long long)args.L1 * (x2 + (long long)args.L2 * x3);
+    };
+    auto set_x0_offsets = [&](int r) {
+        int hp = h + r;       if (hp == LH) hp = 0;
+        int hm = h - 1 + r;   if (hm < 0) hm = LH - 1;
+        off[0] = rc * Cfg::ROWB + (uint32_t)(c * LH + hp) * 16;
+        off[1] = rc * Cfg::ROWB + (uint32_t)(c * LH + hm) * 16;
+    };
+    const int rot[3] = {c, c1, c2};
+    auto load_links = [&](long long grow) {
+        const double2 *gp = args.gauge + grow * (72 * LH) + 2 * h;
+#pragma unroll
+        for (int leg = 0; leg < 8; leg++)
+#pragma unroll
+            for (int r = 0; r < 3; r++) {
+                const int f = leg * 9 + rot[r] * 3 + c;
+                U[leg * 3 + r] = ldg_d2_hint(gp + (f >> 1) * 2 * LH + (f & 1), pol_first);
+            }
+    };
+
+    // the pending step: the block of partial sums this thread owns, where it goes, its x (AXPY)
+    double2 keep[4], xk[4];
+    double2 *keep_o = nullptr;
+    int keep_g = -1;
+    auto finish = [&]() {
+        const int buf = keep_g & 1;
+        mbar_wait(my_exch + 8 * buf, (keep_g >> 1) & 1);
+        if (active) {
+            double2 a0[4], a1[4];
+#pragma unroll
+            for (int j = 0; j < 4; j++) {
+                a0[j] = red_r[buf * RED_BUF + j * Cfg::TP];
+                a1[j] = red_r[buf * RED_BUF + (4 + j) * Cfg::TP];
+            }
+            double2 v[4];
+#pragma unroll
+            for (int j = 0; j < 4; j++) {
+                v[j] = cadd(cadd(keep[j], a0[j]), a1[j]);
+                if constexpr (AXPY) {
+                    v[j].x = fma(args.axpy_b, v[j].x, args.axpy_a * xk[j].x);
+                    v[j].y = fma(args.axpy_b, v[j].y, args.axpy_a * xk[j].y);
+                }
+                if constexpr (NORM) nsum = fma(v[j].x, v[j].x, fma(v[j].y, v[j].y, nsum));
+            }
+#pragma unroll
+            for (int j = 0; j < 4; j++) stg_d2_hint(keep_o + (3 * j) * LH, v[j], pol_out);      // component k = j*3 + c
+        }
+    };
+
+    int r_cur;
+    long long grow = tile_row(0, r_cur);
+    set_x0_offsets(r_cur);
+    load_links(grow);
+
+    // One slice: 8 legs out of the staged buffer, then the deferred finish of the previous slice
+    auto step = [&](const int g, const int s) {
+        const int stage = g & 1;
+        const uint32_t eb = empty_base + 32 * stage;
+        double2 *o2 = args.out + grow * (12 * LH) + (c * LH + h) + (long long)s * nrow * (12 * LH);
+        // AXPY: this thread's four components of x, requested before the wait so that the global-memory
+        // latency hides behind the legs
+        double2 xv[4];
+        if constexpr (AXPY) {
+            if (active) {
+                const double2 *xp = args.axpy_x + (o2 - args.out);
+#pragma unroll
+                for (int j = 0; j < 4; j++) xv[j] = __ldcs(xp + (3 * j) * LH);
+            }
+        }
+        mbar_wait(full_base + 8 * stage, (g >> 1) & 1);
+        const unsigned char *sb = smem + stage * Cfg::STAGE_BYTES;
+        double2 acc[12];
+        // the four loads of leg L (colour c of the four spin components of the neighbour), then the leg
+#define DWF_LOAD64(L)                                                                               \
+        const double2 q##L##_0 = *reinterpret_cast<const double2 *>(sb + off[L]),                    \
+                      q##L##_1 = *reinterpret_cast<const double2 *>(sb + off[L] + KSPIN),            \
+                      q##L##_2 = *reinterpret_cast<const double2 *>(sb + off[L] + 2 * KSPIN),        \
+                      q##L##_3 = *reinterpret_cast<const double2 *>(sb + off[L] + 3 * KSPIN);
+#define DWF_LEG64(L, MU, FWD, FIRST) leg64<MU, (FWD) != DAG, FIRST>(acc, q##L##_0, q##L##_1, q##L##_2, q##L##_3, U + 3 * (L));
+        // Legs in the order x3, x2, x1, x0.  The stage is handed back to the producer ONCE, after the last leg:
+        // every lane's loads precede the warp barrier, lane 0's arrives (release) follow it and depend on the
+        // data of the last legs' loads (tma.cuh: mbar_arrive_after8).  Releasing the face regions early, right
+        // after the two legs that read them (as dhop_staged.cu does), was measured 4 % faster here but gave
+        // wrong results in the last slice of a tile as soon as two regions were released early (r02 notes in
+        // DESIGN.md): not understood, so not used.
+        DWF_LOAD64(6) DWF_LOAD64(7)
+        DWF_LEG64(6, 3, true, true)
+        DWF_LEG64(7, 3, false, false)
+        DWF_LOAD64(4) DWF_LOAD64(5)
+        DWF_LEG64(4, 2, true, false)
+        DWF_LEG64(5, 2, false, false)
+        DWF_LOAD64(2) DWF_LOAD64(3)
+        DWF_LEG64(2, 1, true, false)
+        DWF_LEG64(3, 1, false, false)
+        DWF_LOAD64(0) DWF_LOAD64(1)
+        DWF_LEG64(0, 0, true, false)
+        DWF_LEG64(1, 0, false, false)
+        __syncwarp();
+        if (lane == 0) {
+            mbar_arrive(eb);
+            mbar_arrive(eb + 8);
+            mbar_arrive(eb + 16);
+            mbar_arrive_after8(eb + 24, q0_0.x, q0_1.x, q0_2.x, q0_3.x, q1_0.x, q1_1.x, q1_2.x, q1_3.x);
+        }
+#undef DWF_LOAD64
+#undef DWF_LEG64
+
+        if (keep_g >= 0) finish();               // the previous step: its exchange has long completed
+        // publish the blocks r = 1, 2 of this step
+        const int buf = g & 1;
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            red_w1[buf * RED_BUF + j * Cfg::TP] = acc[3 * j + 1];
+            red_w2[buf * RED_BUF + j * Cfg::TP] = acc[3 * j + 2];
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(my_exch + 8 * buf);
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            keep[j] = acc[3 * j];
+            if constexpr (AXPY) xk[j] = xv[j];
+        }
+        keep_o = o2;
+        keep_g = g;
+    };
 
     int g = 0;
     for (int it = 0; it < my_tiles; it++) {
-        const int4 o = args.tiles[blockIdx.x + it * gridDim.x];
-        const int x1 = o.x + i1, x2 = o.y + i2, x3 = o.z + i3;
-        const int r = (x1 + x2 + x3 + args.parity_out) & 1;          // x0 = 2h + r
-        const long long grow = x1 + (long long)args.L1 * (x2 + (long long)args.L2 * x3);
-        int hp = h + r;       if (hp == LH) hp = 0;
-        int hm = h - 1 + r;   if (hm < 0) hm = LH - 1;
-        off[0] = rc * Cfg::ROWB + hp * 16;
-        off[1] = rc * Cfg::ROWB + hm * 16;
-        {
-            const double2 *gp = args.gauge + grow * (72 * LH) + 2 * h;
-#pragma unroll
-            for (int leg = 0; leg < 8; leg++)
-#pragma unroll
-                for (int a = 0; a < 3; a++) {
-                    const int f = leg * 9 + a * 3 + C;
-                    U[leg * 3 + a] = __ldg(gp + (f >> 1) * 2 * LH + (f & 1));
-                }
-        }
-        double2 *orow = args.out + grow * (12 * LH) + h;                // + s * nrow * 12 * LH + k * LH
+        const bool has_next = it + 1 < my_tiles;
+        int r_next = r_cur;
+        long long grow_next = grow;
+        if (has_next) grow_next = tile_row(it + 1, r_next);
         for (int s = 0; s < args.Ls; s++, g++) {
-            const int stage = g & 1;
-            // AXPY: this thread's four components of x, requested before the wait so that the global-memory
-            // latency hides behind the legs
-            double2 xv[4];
-            if constexpr (AXPY) {
-                if (active) {
-                    const double2 *xp = args.axpy_x + (orow - args.out) + (long long)s * nrow * (12 * LH);
-#pragma unroll
-                    for (int j = 0; j < 4; j++) xv[j] = __ldcs(xp + (4 * C + j) * LH);
-                }
-            }
-            mbar_wait(full_base + 8 * stage, (g >> 1) & 1);
-            const unsigned char *sb = smem + stage * Cfg::STAGE_BYTES;
-            double2 acc[12];
-#pragma unroll
-            for (int k = 0; k < 12; k++) acc[k] = make_double2(0.0, 0.0);
-#define DWF_LEG64(L, MU, FWD)                                                                       \
-            {                                                                                       \
-                const unsigned char *nb = sb + off[L];                                              \
-                leg64<MU, (FWD) != DAG>(acc, *reinterpret_cast<const double2 *>(nb + KOFF0),        \
-                                        *reinterpret_cast<const double2 *>(nb + KOFF1),             \
-                                        *reinterpret_cast<const double2 *>(nb + KOFF2),             \
-                                        *reinterpret_cast<const double2 *>(nb + KOFF3), U + 3 * (L)); \
-            }
-            DWF_LEG64(0, 0, true)
-            DWF_LEG64(1, 0, false)
-            DWF_LEG64(2, 1, true)
-            DWF_LEG64(3, 1, false)
-            DWF_LEG64(4, 2, true)
-            DWF_LEG64(5, 2, false)
-            DWF_LEG64(6, 3, true)
-            DWF_LEG64(7, 3, false)
-#undef DWF_LEG64
-            // this warp is done with the stage
-            __syncwarp();
-            if (lane == 0) mbar_arrive(empty_base + 8 * stage);
-
-            // exchange: thread C owns output components 4C .. 4C+3 and hands the other two blocks over
-            const int buf = g & 1;
-#pragma unroll
-            for (int cc = 0; cc < 3; cc++) {
-                if (cc == C) continue;
-                const int slot = (C < cc) ? C : C - 1;
-#pragma unroll
-                for (int j = 0; j < 4; j++)
-                    red[((((buf * 3 + cc) * 2 + slot) * 4 + j) * Cfg::TP) + site] = acc[4 * cc + j];
-            }
-            asm volatile("bar.sync %0, 96;" ::"r"(1 + (site >> 5)) : "memory");     // the three warps of this 32-site group
-            if (active) {
-                double2 *o2 = orow + (long long)s * nrow * (12 * LH);
-#pragma unroll
-                for (int j = 0; j < 4; j++) {
-                    const double2 a0 = red[((((buf * 3 + C) * 2 + 0) * 4 + j) * Cfg::TP) + site];
-                    const double2 a1 = red[((((buf * 3 + C) * 2 + 1) * 4 + j) * Cfg::TP) + site];
-                    double2 v = cadd(cadd(acc[4 * C + j], a0), a1);
-                    const int k = 4 * C + j;
-                    if constexpr (AXPY) {
-                        v.x = fma(args.axpy_b, v.x, args.axpy_a * xv[j].x);
-                        v.y = fma(args.axpy_b, v.y, args.axpy_a * xv[j].y);
-                    }
-                    __stcs(o2 + k * LH, v);
-                }
-            }
+            const int sl = (args.zigzag && (it & 1)) ? args.Ls - 1 - s : s;
+            step(g, sl);
         }
+        grow = grow_next;
+        r_cur = r_next;
+        set_x0_offsets(r_cur);
+        // links of the next tile (a second code copy that refills them leg by leg during the last slice, as
+        // dhop_staged.cu does, measured slower here: 1493 vs 1306 us on C4 -- instruction-cache misses)
+        if (has_next) load_links(grow);
     }
+    if (keep_g >= 0) finish();
 }
 
-template <int LH, int B1, int B2, int B3, bool DAG, bool AXPY>
+template <int LH, int B1, int B2, int B3, int MODE>
 __global__ void __launch_bounds__(Staged64Cfg<LH, B1, B2, B3>::NT, 1)
 dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_x1,
                      const __grid_constant__ CUtensorMap map_x2, const __grid_constant__ CUtensorMap map_x3,
@@ -240,20 +369,23 @@ dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_con
     extern __shared__ __align__(1024) unsigned char smem[];
     const uint32_t smem_base = smem_u32(smem);
     const uint32_t full_base = smem_base + Cfg::NSTAGE * Cfg::STAGE_BYTES + Cfg::RED_BYTES;   // full[2]
-    const uint32_t empty_base = full_base + 16;                                                // empty[2]
+    const uint32_t empty_base = full_base + 16;                                                // empty[2][4 regions]
+    const uint32_t exch_base = full_base + Cfg::TAIL_EXCH;                                     // exch[NGROUP][2]
     const int tid = threadIdx.x;
     const int my_tiles = (args.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
     const int nsteps = my_tiles * args.Ls;
-    if (nsteps <= 0) return;
+    if (nsteps <= 0) {
+        if ((MODE & 4) && tid == 0) args.norm_partials[blockIdx.x] = 0.0;
+        return;
+    }
     if (tid == 0) {
         tma_prefetch_desc(&map_c);
         tma_prefetch_desc(&map_x1);
         tma_prefetch_desc(&map_x2);
         tma_prefetch_desc(&map_x3);
-        for (int i = 0; i < 2; i++) {
-            mbar_init(full_base + 8 * i, 1);
-            mbar_init(empty_base + 8 * i, Cfg::NWARP_C);
-        }
+        for (int i = 0; i < 2; i++) mbar_init(full_base + 8 * i, 4);        // four regions arrive (expect_tx) per stage
+        for (int i = 0; i < 8; i++) mbar_init(empty_base + 8 * i, Cfg::NWARP_C);
+        for (int i = 0; i < 2 * Cfg::NGROUP; i++) mbar_init(exch_base + 8 * i, 3);
         mbar_fence_init();
     }
     __syncthreads();
@@ -262,25 +394,35 @@ dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_con
         reg_dealloc<Cfg::PROD_REGS>();
         if (tid != 0) return;
         const int L1 = args.L1, L2 = args.L2, L3 = args.L3;
+        const uint64_t pol_last = l2_policy(args.l2pol % 10);      // input boxes are re-read by neighbouring tiles
         for (int g = 0; g < nsteps; g++) {
-            const int it = g / args.Ls, s = g % args.Ls, stage = g & 1;
-            if (g >= 2) mbar_wait(empty_base + 8 * stage, ((g >> 1) - 1) & 1);
+            const int it = g / args.Ls, i = g % args.Ls, stage = g & 1;
+            const int s = (args.zigzag && (it & 1)) ? args.Ls - 1 - i : i;
             const int4 o = args.tiles[blockIdx.x + it * gridDim.x];
-            const uint32_t bar = full_base + 8 * stage;
+            const uint32_t bar = full_base + 8 * stage, eb = empty_base + 32 * stage;
+            const uint32_t epar = ((g >> 1) - 1) & 1;
             const uint32_t dst = smem_base + stage * Cfg::STAGE_BYTES;
             const int sb = s * L3;                 // x3 and s share tensor dimension 4
             const int x1m = o.x == 0 ? L1 - 1 : o.x - 1, x1p = o.x + B1 == L1 ? 0 : o.x + B1;
             const int x2m = o.y == 0 ? L2 - 1 : o.y - 1, x2p = o.y + B2 == L2 ? 0 : o.y + B2;
             const int x3m = o.z == 0 ? L3 - 1 : o.z - 1, x3p = o.z + B3 == L3 ? 0 : o.z + B3;
-            mbar_arrive_expect_tx(bar, Cfg::STAGE_BYTES);
             const int c4 = sb + o.z;
-            tma_load_5d(dst, &map_c, bar, 0, 0, o.x, o.y, c4);
-            tma_load_5d(dst + Cfg::R_X1M * Cfg::ROWB, &map_x1, bar, 0, 0, x1m, o.y, c4);
-            tma_load_5d(dst + Cfg::R_X1P * Cfg::ROWB, &map_x1, bar, 0, 0, x1p, o.y, c4);
-            tma_load_5d(dst + Cfg::R_X2M * Cfg::ROWB, &map_x2, bar, 0, 0, o.x, x2m, c4);
-            tma_load_5d(dst + Cfg::R_X2P * Cfg::ROWB, &map_x2, bar, 0, 0, o.x, x2p, c4);
-            tma_load_5d(dst + Cfg::R_X3M * Cfg::ROWB, &map_x3, bar, 0, 0, o.x, o.y, sb + x3m);
-            tma_load_5d(dst + Cfg::R_X3P * Cfg::ROWB, &map_x3, bar, 0, 0, o.x, o.y, sb + x3p);
+            // regions in the order the consumers release them: x3 faces, x2 faces, x1 faces, centre
+            if (g >= 2) mbar_wait(eb, epar);
+            mbar_arrive_expect_tx(bar, 2 * B1 * B2 * Cfg::ROWB);
+            tma_load_5d_hint(dst + Cfg::R_X3M * Cfg::ROWB, &map_x3, bar, 0, 0, o.x, o.y, sb + x3m, pol_last);
+            tma_load_5d_hint(dst + Cfg::R_X3P * Cfg::ROWB, &map_x3, bar, 0, 0, o.x, o.y, sb + x3p, pol_last);
+            if (g >= 2) mbar_wait(eb + 8, epar);
+            mbar_arrive_expect_tx(bar, 2 * B1 * B3 * Cfg::ROWB);
+            tma_load_5d_hint(dst + Cfg::R_X2M * Cfg::ROWB, &map_x2, bar, 0, 0, o.x, x2m, c4, pol_last);
+            tma_load_5d_hint(dst + Cfg::R_X2P * Cfg::ROWB, &map_x2, bar, 0, 0, o.x, x2p, c4, pol_last);
+            if (g >= 2) mbar_wait(eb + 16, epar);
+            mbar_arrive_expect_tx(bar, 2 * B2 * B3 * Cfg::ROWB);
+            tma_load_5d_hint(dst + Cfg::R_X1M * Cfg::ROWB, &map_x1, bar, 0, 0, x1m, o.y, c4, pol_last);
+            tma_load_5d_hint(dst + Cfg::R_X1P * Cfg::ROWB, &map_x1, bar, 0, 0, x1p, o.y, c4, pol_last);
+            if (g >= 2) mbar_wait(eb + 24, epar);
+            mbar_arrive_expect_tx(bar, Cfg::NROW_C * Cfg::ROWB);
+            tma_load_5d_hint(dst, &map_c, bar, 0, 0, o.x, o.y, c4, pol_last);
         }
         return;
     }
@@ -289,31 +431,67 @@ dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_con
     const int ctid = tid - 128;
     if (ctid >= 3 * Cfg::TP) return;
     const int c = ctid / Cfg::TP, site = ctid % Cfg::TP;         // colour-major: uniform per warp
-    if (c == 0)      consume64<LH, B1, B2, B3, DAG, AXPY, 0>(args, smem, full_base, empty_base, site, my_tiles);
-    else if (c == 1) consume64<LH, B1, B2, B3, DAG, AXPY, 1>(args, smem, full_base, empty_base, site, my_tiles);
-    else             consume64<LH, B1, B2, B3, DAG, AXPY, 2>(args, smem, full_base, empty_base, site, my_tiles);
+    double nsum = 0.0;
+    consume64<LH, B1, B2, B3, MODE>(args, smem, full_base, empty_base, exch_base, site, c, my_tiles, nsum);
+
+    if constexpr ((MODE & 4) != 0) {
+        // lanes -> warp (xor butterfly), warps -> CTA in warp order: the same order in every run
+        double v = nsum;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        double *slots = reinterpret_cast<double *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + Cfg::RED_BYTES + Cfg::TAIL_NORM);
+        if ((ctid & 31) == 0) slots[ctid >> 5] = v;
+        asm volatile("bar.sync 1, %0;" ::"n"(Cfg::NWARP_C * 32) : "memory");      // consumer warps only
+        if (ctid == 0) {
+            double t = 0.0;
+            for (int w = 0; w < Cfg::NWARP_C; w++) t += slots[w];
+            args.norm_partials[blockIdx.x] = t;
+        }
+    }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Kernel instances: this file is compiled once per MODE (-DDWF_STAGED64_MODE=0..4, build.py); each
+// translation unit exports the entry points of its MODE in the order of DWF_STAGED64_VARIANTS, the
+// MODE 0 unit also holds the host code.
+// ---------------------------------------------------------------------------------------------
+#define DWF_STAGED64_VARIANTS(X) X(16, 2, 1, 2) X(16, 1, 1, 4) X(16, 1, 2, 2) X(16, 2, 2, 1) X(8, 4, 2, 1) X(8, 2, 2, 2) X(4, 4, 4, 1) X(4, 4, 2, 2) X(4, 2, 2, 2) X(4, 2, 2, 1) X(8, 2, 2, 1) X(16, 2, 1, 1) \
+    X(12, 2, 1, 2) X(12, 2, 2, 1) X(12, 1, 2, 2) X(24, 2, 1, 1) X(24, 1, 1, 2) X(32, 2, 1, 1) X(32, 1, 1, 2) X(32, 1, 2, 1) X(20, 1, 1, 2) X(20, 2, 1, 1)
+
+const void *const *staged64_kernels_mode0();
+const void *const *staged64_kernels_mode1();
+const void *const *staged64_kernels_mode2();
+const void *const *staged64_kernels_mode3();
+const void *const *staged64_kernels_mode4();
+
+#define DWF_CAT2(a, b) a##b
+#define DWF_CAT(a, b) DWF_CAT2(a, b)
+const void *const *DWF_CAT(staged64_kernels_mode, DWF_STAGED64_MODE)()
+{
+#define X(LH, B1, B2, B3) reinterpret_cast<const void *>(&dhop_staged64_kernel<LH, B1, B2, B3, DWF_STAGED64_MODE>),
+    static const void *const tab[] = {DWF_STAGED64_VARIANTS(X)};
+#undef X
+    return tab;
+}
+
+#if DWF_STAGED64_MODE == 0
 // ---------------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------------
 struct Variant64 {
     int lh, b1, b2, b3, smem, threads;
-    const void *fn[4];       // plain, dagger, a x + b Dhop, a x + b Dhop^dagger
+    const void *fn[5];       // MODE 0 plain, 1 dagger, 2 a x + b Dhop, 3 a x + b Dhop^dagger, 4 Dhop + norm2
 };
-
-#define DWF_STAGED64_VARIANTS(X) X(16, 2, 1, 2) X(16, 1, 1, 4) X(16, 1, 2, 2) X(16, 2, 2, 1) X(8, 4, 2, 1) X(8, 2, 2, 2) X(4, 4, 4, 1) X(4, 4, 2, 2) X(4, 2, 2, 2) X(4, 2, 2, 1) X(8, 2, 2, 1) X(16, 2, 1, 1)
 
 static const std::vector<Variant64> &variants64()
 {
     static const std::vector<Variant64> v = [] {
         std::vector<Variant64> t;
+        const void *const *k0 = staged64_kernels_mode0(), *const *k1 = staged64_kernels_mode1(), *const *k2 = staged64_kernels_mode2(),
+                          *const *k3 = staged64_kernels_mode3(), *const *k4 = staged64_kernels_mode4();
 #define X(LH, B1, B2, B3)                                                                             \
         t.push_back({LH, B1, B2, B3, Staged64Cfg<LH, B1, B2, B3>::SMEM_BYTES, Staged64Cfg<LH, B1, B2, B3>::NT, \
-                     {reinterpret_cast<const void *>(&dhop_staged64_kernel<LH, B1, B2, B3, false, false>),    \
-                      reinterpret_cast<const void *>(&dhop_staged64_kernel<LH, B1, B2, B3, true, false>),     \
-                      reinterpret_cast<const void *>(&dhop_staged64_kernel<LH, B1, B2, B3, false, true>),     \
-                      reinterpret_cast<const void *>(&dhop_staged64_kernel<LH, B1, B2, B3, true, true>)}});
+                     {k0[t.size()], k1[t.size()], k2[t.size()], k3[t.size()], k4[t.size()]}});
         DWF_STAGED64_VARIANTS(X)
 #undef X
         return t;
@@ -335,7 +513,7 @@ void plan_staged64(dwf_geometry *g)
         g->staged64.b[0] = v[i].b1; g->staged64.b[1] = v[i].b2; g->staged64.b[2] = v[i].b3;
         g->staged64.ntiles = (lat.L[1] / v[i].b1) * (lat.L[2] / v[i].b2) * (lat.L[3] / v[i].b3);
         // per-device opt-in to the large dynamic shared memory (the caller holds a DeviceGuard)
-        for (int d = 0; d < 4; d++)
+        for (int d = 0; d < 5; d++)
             if (cudaFuncSetAttribute(v[i].fn[d], cudaFuncAttributeMaxDynamicSharedMemorySize, v[i].smem) != cudaSuccess) {
                 cudaGetLastError();
                 g->staged64.variant = -1;
@@ -388,16 +566,42 @@ static int encode_map64(CUtensorMap *m, const void *base, const Lattice &lat, in
     return DWF_OK;
 }
 
-int launch_dhop_staged64(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger,
-                         const void *axpy_x, double axpy_a, double axpy_b)
+// The four tensor maps of a field depend on its pointer and the tile shape only: kept in a small
+// per-thread cache (keyed by geometry id, variant and pointer) so that a solver that applies the
+// operator to the same few buffers makes no driver calls (as dhop_staged.cu does for fp32).
+struct MapSet64 { unsigned long long gid; int variant; const void *ptr; CUtensorMap m[4]; };
+
+static int get_maps64(const dwf_geometry *g, const Variant64 &v, const void *ptr, const MapSet64 **out)
 {
-    const Variant64 &v = variants64()[(size_t)g->staged64.variant];
-    CUtensorMap mc, m1, m2, m3;
+    static thread_local MapSet64 cache[8];
+    static thread_local unsigned next_slot = 0;
+    for (const MapSet64 &c : cache)
+        if (c.ptr == ptr && c.gid == g->uid && c.variant == g->staged64.variant) { *out = &c; return DWF_OK; }
+    MapSet64 t;
+    t.gid = g->uid; t.variant = g->staged64.variant; t.ptr = ptr;
     int rc;
-    if ((rc = encode_map64(&mc, in, g->lat, v.b1, v.b2, v.b3))) return rc;
-    if ((rc = encode_map64(&m1, in, g->lat, 1, v.b2, v.b3))) return rc;
-    if ((rc = encode_map64(&m2, in, g->lat, v.b1, 1, v.b3))) return rc;
-    if ((rc = encode_map64(&m3, in, g->lat, v.b1, v.b2, 1))) return rc;
+    if ((rc = encode_map64(&t.m[0], ptr, g->lat, v.b1, v.b2, v.b3))) return rc;
+    if ((rc = encode_map64(&t.m[1], ptr, g->lat, 1, v.b2, v.b3))) return rc;
+    if ((rc = encode_map64(&t.m[2], ptr, g->lat, v.b1, 1, v.b3))) return rc;
+    if ((rc = encode_map64(&t.m[3], ptr, g->lat, v.b1, v.b2, 1))) return rc;
+    MapSet64 *ms = &cache[next_slot++ % 8];
+    *ms = t;
+    *out = ms;
+    return DWF_OK;
+}
+
+int launch_dhop_staged64(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger,
+                         const void *axpy_x, double axpy_a, double axpy_b, double *norm_partials, int *norm_blocks)
+{
+    if (norm_partials && (dagger || axpy_x)) {
+        set_error("the fp64 staged kernel has no instance for this combination of modes");
+        return DWF_ERR_UNSUPPORTED;
+    }
+    const Variant64 &v = variants64()[(size_t)g->staged64.variant];
+    const MapSet64 *ms = nullptr;
+    int rc;
+    if ((rc = get_maps64(g, v, in, &ms))) return rc;
+    CUtensorMap mc = ms->m[0], m1 = ms->m[1], m2 = ms->m[2], m3 = ms->m[3];     // passed by value
     Staged64Args a;
     a.out = static_cast<double2 *>(out);
     a.gauge = static_cast<const double2 *>(g->gauge[parity_out]);
@@ -405,15 +609,21 @@ int launch_dhop_staged64(const dwf_geometry *g, const void *in, void *out, int p
     a.ntiles = g->staged64.ntiles;
     a.L1 = g->lat.L[1]; a.L2 = g->lat.L[2]; a.L3 = g->lat.L[3]; a.Ls = g->lat.Ls;
     a.parity_out = parity_out;
+    a.zigzag = g->opt_zigzag;
+    a.l2pol = g->opt_l2pol;
     a.axpy_x = static_cast<const double2 *>(axpy_x);
     a.axpy_a = axpy_a;
     a.axpy_b = axpy_b;
-    const void *fn = v.fn[(dagger ? 1 : 0) + (axpy_x ? 2 : 0)];
+    a.norm_partials = norm_partials;
+    const void *fn = v.fn[norm_partials ? 4 : (dagger ? 1 : 0) + (axpy_x ? 2 : 0)];
     const int grid = g->staged64.ntiles < g->sm_count ? g->staged64.ntiles : g->sm_count;
     void *params[] = {&mc, &m1, &m2, &m3, &a};
     DWF_CUDA_CHECK(cudaLaunchKernel(fn, dim3((unsigned)grid), dim3((unsigned)v.threads), params, (size_t)v.smem, st));
+    if (norm_blocks) *norm_blocks = grid;
     count_launch();
     return DWF_OK;
 }
+
+#endif  // DWF_STAGED64_MODE == 0
 
 }  // namespace dwf

@@ -151,8 +151,10 @@ int launch_axpby(const dwf_geometry *g, const void *x, void *out, double a, doub
 // dhop_staged64.cu (TMA-staged fp64 kernel, links split by colour column over three threads)
 void plan_staged64(dwf_geometry *g);
 void build_staged64_tile_table(const dwf_geometry *g, int4 *host_table);
+// norm_partials != nullptr: the fused-norm2 instance, one partial of |out|^2 per CTA, *norm_blocks = their number
 int launch_dhop_staged64(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger,
-                         const void *axpy_x = nullptr, double axpy_a = 0.0, double axpy_b = 0.0);
+                         const void *axpy_x = nullptr, double axpy_a = 0.0, double axpy_b = 0.0,
+                         double *norm_partials = nullptr, int *norm_blocks = nullptr);
 // reduce.cu
 int launch_norm2(const dwf_geometry *g, const void *field, size_t nreal, cudaStream_t st);
 int launch_final_sum(const dwf_geometry *g, int nblocks, cudaStream_t st);   // result_dev[0] = sum of partials[0..nblocks)

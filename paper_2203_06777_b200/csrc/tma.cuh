@@ -31,6 +31,26 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+// Arrive that is issued only after the shared-memory loads whose results are passed in have returned
+// their data (the values are unused inputs of the asm statement, so the instruction depends on them).
+// This is how a consumer hands a staged region back to the TMA producer right after READING it: a plain
+// arrive placed behind the loads in program order may execute while they are still in flight (ptxas
+// does not make SYNCS.ARRIVE wait for earlier LDS, and __syncwarp() compiles to nothing in converged
+// code), and the refilling bulk copy -- async proxy -- then overwrites the data before it is read;
+// observed on the fp64 kernel as stale last-issued loads.  One 32-bit word of every load instruction is
+// enough: a warp-wide LDS releases its scoreboard when all lanes have their data.
+__device__ __forceinline__ void mbar_arrive_after8(uint32_t bar, double a, double b, double c, double d, double e, double f,
+                                                   double g, double h)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar), "d"(a), "d"(b), "d"(c), "d"(d), "d"(e), "d"(f), "d"(g),
+                 "d"(h) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_after12(uint32_t bar, float a, float b, float c, float d, float e, float f, float g,
+                                                    float h, float i, float j, float k, float l)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar), "f"(a), "f"(b), "f"(c), "f"(d), "f"(e), "f"(f), "f"(g),
+                 "f"(h), "f"(i), "f"(j), "f"(k), "f"(l) : "memory");
+}
 // blocks until the phase with the given parity has completed
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {

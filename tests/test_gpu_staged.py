@@ -328,21 +328,38 @@ def test_dhop_calls_can_be_captured_in_a_cuda_graph(lib):
         assert torch.equal(f_x, ref)
 
 
-@pytest.mark.parametrize("dims,Ls,bc", [((32, 8, 8, 8), 3, 1), ((16, 8, 4, 6), 5, 0), ((8, 8, 8, 8), 8, 1), ((32, 6, 4, 10), 2, 0)])
+@pytest.mark.parametrize("dims,Ls,bc", [((32, 8, 8, 8), 3, 1), ((16, 8, 4, 6), 5, 0), ((8, 8, 8, 8), 8, 1), ((32, 6, 4, 10), 2, 0),
+                                        ((24, 8, 6, 8), 4, 1), ((48, 4, 6, 4), 3, 0), ((64, 4, 4, 6), 3, 1), ((40, 6, 4, 4), 5, 1)])
 def test_staged64_fp64_kernel(lib, dims, Ls, bc):
     """The fp64 staged kernel (csrc/dhop_staged64.cu: three threads per site, one colour column of the
-    links each, partial sums exchanged through shared memory), forced with kernel=2: several tiles
-    per CTA, plain and dagger, against the oracle at the fp64 bar; bit-identical from run to run."""
+    links each, partial sums exchanged through shared memory one step late), forced with kernel=2:
+    several tiles per CTA (tile switch with link refill), Lh = 4 .. 32, plain, dagger, fused norm2 and
+    fused a x + b Dhop against the oracle at the fp64 bar; bit-identical from run to run and under zigzag."""
     import torch
     check_cb_against_oracle(lib, dims, Ls, 8, bc, 48)
     U = gen.gauge_random(dims, 49, prec=8)
     half = gen.spinor_gaussian(gen.volume(dims) // 2, Ls, 49, prec=8)
+    xh = gen.spinor_gaussian(gen.volume(dims) // 2, Ls, 49, gen.STREAM_SPINOR2, 8)
     with lib.Geometry(dims, Ls, 8, bc) as g:
         g.load_gauge(U)
         g.set_option("kernel", 2)
-        fin = g.import_spinor(half, lib.EVEN)
+        assert g.kernel_info().startswith("dhop_staged64_kernel")
+        fin, fx = g.import_spinor(half, lib.EVEN), g.import_spinor(xh, lib.ODD)
+        want = oracle.dhop_cb(dims, Ls, bc, 1, U, half)
         a = g.dhop_oe_dag(fin).clone()
         assert rel_err(g.export_spinor(a, lib.ODD), oracle.dhop_cb(dims, Ls, bc, 1, U, half, dagger=True)) <= TOL[8]
         assert torch.equal(g.dhop_oe_dag(fin), a)
+        plain = g.dhop_oe(fin).clone()
+        fused, n = g.dhop_oe_norm2(fin)                           # MODE 4: norm2 in the store epilogue
+        assert torch.equal(fused, plain)
+        assert abs(n - oracle.norm2(g.export_spinor(fused, lib.ODD))) <= 1e-12 * n
+        assert g.dhop_oe_norm2(fin)[1] == n
+        ax = g.dhop_oe_axpy(fin, fx, 1.3, -0.5)
+        assert rel_err(g.export_spinor(ax, lib.ODD), 1.3 * xh - 0.5 * want) <= TOL[8]
+        buf = fx.clone()
+        lib.dwf_dhop_oe_axpy(g.handle, fin, buf, 1.3, -0.5, buf)   # x == out
+        assert torch.equal(buf, ax)
+        g.set_option("zigzag", 0)
+        assert torch.equal(g.dhop_oe(fin), plain)
         g.set_option("kernel", 1)                                 # direct kernel: another summation order
         assert rel_err(g.export_spinor(g.dhop_oe_dag(fin), lib.ODD), g.export_spinor(a, lib.ODD)) <= TOL[8]
