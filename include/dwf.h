@@ -204,7 +204,8 @@ DWF_API int dwf_kernel_info(const dwf_geometry *g, char *buf, size_t n);
 /* Tuning knobs for experiments; none of them changes a result of the staged kernel by a bit
  * (tests/test_gpu_staged.py).  UNSUPPORTED for an unknown key, INVALID_ARG for a bad value.
  *   "kernel"         0 auto, 1 direct (L1-cached) kernel, 2 TMA-staged kernel (error if it has no
- *                    variant for the geometry: fp32, Lh = 4, 8, 16 or 24, box extents dividing L1..L3)
+ *                    variant for the geometry: Lh = L0/2 in {4, 8, 12, 16, 20, 24, 28, 32} (fp64: not 28), box extents
+ *                    dividing L1..L3; other shapes run the direct kernel)
  *   "variant"        staged tile shape: 0 auto, n > 0 the n-th compiled (Lh, B1, B2, B3) instance
  *   "raster_staged"  launch order of the staged tiles, 10 * order + log2(macro blocks) (dhop_staged.cu); -1 auto
  *   "zigzag"         1: every other tile walks its s slices backwards (L2 reuse between tiles)

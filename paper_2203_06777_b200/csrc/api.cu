@@ -342,13 +342,22 @@ int dwf_load_gauge(dwf_geometry *g, const void *U, int src_is_device, void *stre
 int dwf::half_dhop(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger,
                    const void *axpy_x, double a, double b)
 {
-    const bool staged_ok = g->staged.variant >= 0 && (!axpy_x || staged_supports_axpy(g)), staged64_ok = g->staged64.variant >= 0;
-    if (g->opt_kernel == 2 && !staged_ok && !staged64_ok) {
+    const bool staged_any = g->staged.variant >= 0, staged64_ok = g->staged64.variant >= 0;
+    const bool staged_ok = staged_any && (!axpy_x || staged_supports_axpy(g));
+    // tiles whose x rows do not fit into shared memory next to the input slice (Lh = 32): staged Dhop, then
+    // the elementwise pass -- possible whenever x is not the output buffer
+    const bool staged_two_pass = staged_any && !staged_ok && axpy_x != out;
+    if (g->opt_kernel == 2 && !staged_ok && !staged_two_pass && !staged64_ok) {
         set_error("the staged kernels do not support this geometry / precision");
         return DWF_ERR_UNSUPPORTED;
     }
     if (staged_ok && g->opt_kernel != 1)
         return launch_dhop_staged(g, in, out, parity_out, st, nullptr, nullptr, dagger, axpy_x, (float)a, (float)b);
+    if (staged_two_pass && g->opt_kernel != 1) {
+        int rc = launch_dhop_staged(g, in, out, parity_out, st, nullptr, nullptr, dagger);
+        if (rc) return rc;
+        return launch_axpby(g, axpy_x, out, a, b, dwf_field_bytes(g, parity_out) / (size_t)g->prec, st);
+    }
     if (staged64_ok && g->opt_kernel != 1) return launch_dhop_staged64(g, in, out, parity_out, st, dagger, axpy_x, a, b);
     return launch_dhop_direct(g, in, out, parity_out, st, dagger, axpy_x, a, b);
 }

@@ -520,7 +520,9 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
 #define DWF_STAGED_VARIANTS(X)                                                                       \
     X(16, 4, 2, 2) X(16, 2, 2, 2) X(16, 2, 2, 1) X(8, 4, 4, 2) X(8, 2, 2, 2) X(8, 2, 2, 1)           \
     X(24, 2, 2, 2) X(24, 2, 2, 1) X(4, 4, 4, 4) X(4, 2, 2, 2) X(4, 2, 2, 1)                           \
-    X(16, 2, 2, 4) X(16, 2, 4, 2) X(16, 8, 2, 1) X(16, 1, 2, 8) X(24, 3, 1, 3) X(24, 1, 3, 3) X(24, 3, 3, 1)
+    X(16, 2, 2, 4) X(16, 2, 4, 2) X(16, 8, 2, 1) X(16, 1, 2, 8) X(24, 3, 1, 3) X(24, 1, 3, 3) X(24, 3, 3, 1)   \
+    X(12, 4, 2, 2) X(12, 3, 2, 3) X(12, 2, 2, 2) X(12, 2, 2, 1) X(32, 2, 2, 2) X(32, 2, 2, 1)                \
+    X(20, 3, 2, 2) X(20, 2, 2, 2) X(20, 2, 2, 1) X(28, 2, 2, 2) X(28, 2, 2, 1)
 
 const void *const *staged_kernels_mode0();
 const void *const *staged_kernels_mode1();

@@ -1,4 +1,4 @@
-"""Seeded sweep over random geometries (L0 in {8,16,32,48} so that most hit the staged fp32 kernel,
+"""Seeded sweep over random geometries (L0 in {8,16,24,32,40,48,56,64} so that most hit the staged fp32 kernel,
 the other extents even and ragged, Ls 1..12, both boundary conditions): every half-Dhop entry point
 -- plain, dagger, fused norm2, fused axpy -- against the oracle.  Bar: relative L2 error <= 2e-6."""
 import numpy as np
@@ -11,11 +11,11 @@ from _util import rel_err
 pytestmark = pytest.mark.gpu
 
 
-def _cases(n=16, seed=12345):
+def _cases(n=24, seed=12345):
     rng = np.random.default_rng(seed)
     out = []
     while len(out) < n:
-        L0 = int(rng.choice([8, 16, 32, 48]))
+        L0 = int(rng.choice([8, 16, 32, 48, 24, 40, 56, 64]))
         dims = (L0,) + tuple(int(2 * rng.integers(1, 9)) for _ in range(3))
         Ls, bc = int(rng.integers(1, 13)), int(rng.integers(0, 2))
         if gen.volume(dims) * Ls <= 1_500_000:

@@ -76,6 +76,34 @@ def test_staged_lh8_and_lh4(lib):
     check_cb_against_oracle(lib, (8, 8, 12, 8), 7, 4, lib.PERIODIC, 45)
 
 
+@pytest.mark.parametrize("dims,Ls,bc", [((24, 24, 12, 12), 3, 1),    # <12,4,2,2>: the paper's 24^4 volume class
+                                        ((24, 6, 10, 6), 4, 0),      # <12,3,2,3>: L1 not a multiple of 4
+                                        ((24, 6, 2, 6), 5, 1),       # <12,3,2,3> with L2 = 2: both x2 faces are the same row
+                                        ((64, 8, 8, 6), 3, 1),       # <32,2,2,2>: 256-site tiles, 196 KB of staging
+                                        ((64, 4, 6, 2), 2, 0),
+                                        ((40, 12, 8, 4), 3, 1),      # <20,3,2,2>
+                                        ((40, 8, 8, 6), 2, 0),       # <20,2,2,2>
+                                        ((56, 8, 4, 6), 3, 1)])      # <28,2,2,2>
+def test_staged_other_row_lengths(lib, dims, Ls, bc):
+    """Lh = 12, 20, 28, 32 (L0 = 24, 40, 56, 64): the staged fp32 kernel, several tiles per CTA, every MODE."""
+    import torch
+    check_cb_against_oracle(lib, dims, Ls, 4, bc, 61)
+    U = gen.gauge_random(dims, 62, prec=4)
+    half = gen.spinor_gaussian(gen.volume(dims) // 2, Ls, 62, prec=4)
+    xh = gen.spinor_gaussian(gen.volume(dims) // 2, Ls, 62, gen.STREAM_SPINOR2, 4)
+    with lib.Geometry(dims, Ls, 4, bc) as g:
+        g.load_gauge(U)
+        g.set_option("kernel", 2)
+        assert g.kernel_info().startswith("dhop_staged_kernel<%d," % (dims[0] // 2))
+        fin, fx = g.import_spinor(half, lib.EVEN), g.import_spinor(xh, lib.ODD)
+        want = oracle.dhop_cb(dims, Ls, bc, 1, U, half)
+        plain = g.dhop_oe(fin).clone()
+        fused, n = g.dhop_oe_norm2(fin)
+        assert torch.equal(fused, plain) and abs(n - oracle.norm2(g.export_spinor(fused, lib.ODD))) <= 1e-12 * n
+        assert rel_err(g.export_spinor(g.dhop_oe_dag(fin), lib.ODD), oracle.dhop_cb(dims, Ls, bc, 1, U, half, dagger=True)) <= TOL[4]
+        assert rel_err(g.export_spinor(g.dhop_oe_axpy(fin, fx, 1.3, -0.5), lib.ODD), 1.3 * xh.astype(np.float64) - 0.5 * want) <= TOL[4]
+
+
 OPTION_SETS = [
     {"variant": 2}, {"variant": 3}, {"variant": 12}, {"variant": 13}, {"variant": 14}, {"variant": 15},
     {"raster_staged": 0}, {"raster_staged": 1}, {"raster_staged": 3}, {"raster_staged": 11}, {"raster_staged": 21}, {"raster_staged": 31},
