@@ -57,6 +57,8 @@ WORKLOADS = {
     "tiny": dict(dims=(8, 8, 8, 8), Ls=8, prec=4, bc=1, gauge="random", seed=1002),
     # the Schur complement of the red-black Shamir DWF operator on the C4 shape
     "schur": dict(dims=(32, 32, 32, 32), Ls=16, prec=4, bc=0, gauge="near_unit", seed=1004, kind="schur"),
+    # four right-hand sides sharing one gauge load, C4 shape
+    "c4m4": dict(dims=(32, 32, 32, 32), Ls=16, prec=4, bc=0, gauge="near_unit", seed=1004, kind="mrhs", nrhs=4),
     "schurd": dict(dims=(32, 32, 32, 32), Ls=16, prec=8, bc=0, gauge="near_unit", seed=1004, kind="schur"),
 }
 
@@ -554,6 +556,90 @@ def run_gpu_schur(args, w):
         dist.destroy_process_group()
 
 
+def run_gpu_mrhs(args, w):
+    """--workload c4m4: SURVEY.md 8(f4), nrhs right-hand sides per launch.  One step = DhopOE then DhopEO on
+    all of them (2 launches); minimal-traffic model per launch: one read + one write of nrhs half fields and
+    the whole gauge field ONCE: w (48 + 144 / (Ls nrhs)) bytes per output 5D site."""
+    import torch
+    import paper_2203_06777_b200 as dwf
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dwf.load()
+    d, Ls, prec, nrhs = w["dims"], w["Ls"], w["prec"], w["nrhs"]
+    V4 = d[0] * d[1] * d[2] * d[3]
+    sites = (V4 // 2) * Ls * nrhs                      # output 5D sites of one launch
+    U, psi_e = make_inputs(w)
+    g = dwf.Geometry(d, Ls, prec, w["bc"], device=local_rank)
+    for kv in args.opt or []:
+        k, v = kv.split("=")
+        g.set_option(k, int(v))
+    g.load_gauge(U)
+    one = g.import_spinor(psi_e, dwf.EVEN)
+    f_in = torch.cat([one * (1.0 + 0.25 * r) for r in range(nrhs)])      # nrhs different right-hand sides
+    f_mid, f_out = torch.empty_like(f_in), torch.empty_like(f_in)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step():
+        g.dhop_oe_mrhs(f_in, nrhs, out=f_mid)
+        g.dhop_eo_mrhs(f_mid, nrhs, out=f_out)
+
+    for _ in range(args.warmup):
+        step()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(args.steps)]
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    barrier()
+    sampler.start()
+    l0 = dwf.dwf_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for k in range(args.steps):
+        ev[k][0].record()
+        g.dhop_oe_mrhs(f_in, nrhs, out=f_mid)
+        ev[k][1].record()
+        g.dhop_eo_mrhs(f_mid, nrhs, out=f_out)
+    e1.record()
+    barrier()
+    launches = dwf.dwf_launch_count() - l0
+    clocks = sampler.stop()
+    ms_step = max_over_ranks(e0.elapsed_time(e1), dist) / args.steps
+    t_oe = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
+    if rank == 0:
+        peak, peak_src = peaks()
+        mb = sites * 48 * prec + V4 * 72 * prec
+        achieved = mb / (t_oe * 1e-3) / 1e9
+        # the result of the last right-hand side equals the single-RHS call on the same input (bitwise)
+        chk = bool(torch.equal(g.dhop_oe(f_in.view(nrhs, -1)[nrhs - 1].contiguous()), f_mid.view(nrhs, -1)[nrhs - 1]))
+        line = {
+            "metric": "Dhop GFlop/s (1320 flop/5D site)", "value": world * 2 * FLOP_PER_SITE * sites / (ms_step * 1e-3) / 1e9, "unit": "GFlop/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32" if prec == 4 else "f64", "data": "synthetic",
+            "config": {"workload": f"DWF even/odd Dhop {d[0]}x{d[1]}x{d[2]}x{d[3]} x Ls={Ls} fp{8 * prec}, {nrhs} right-hand sides per launch "
+                                   "sharing one gauge load (SURVEY.md 8(f4)), DhopOE then DhopEO",
+                       "name": args.workload, "dims": list(d), "Ls": Ls, "nrhs": nrhs, "l2": "fields larger than L2; no flush",
+                       "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "clocks": clocks, "gpu_launches": int(launches), "kernels_ms": {"dhop_oe_mrhs": t_oe},
+            "roofline": {"bound": "hbm", "kernel": g.kernel_info() + f" ({nrhs} RHS, DhopOE launches)", "achieved": achieved, "peak": peak,
+                         "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src, "algorithmic_bytes_per_launch": mb,
+                         "traffic": ncu_traffic(args.workload, g.kernel_info())[0]},
+            "check": {"last_rhs_equals_single_call_bitwise": chk},
+        }
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def spawn_ranks(n: int, argv, check_devices: bool = True) -> int:
     """`python bench.py --gpus N` without a launcher: start N ranks of this script under
     torch.distributed.run on this node (one per GPU, rendezvous on 127.0.0.1) and return its exit
@@ -597,6 +683,8 @@ def main():
         run_reference(args, w)
     elif w.get("kind") == "schur":
         run_gpu_schur(args, w)
+    elif w.get("kind") == "mrhs":
+        run_gpu_mrhs(args, w)
     else:
         run_gpu(args, w)
 

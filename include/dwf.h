@@ -113,6 +113,16 @@ DWF_API int dwf_dhop_oe_axpy(const dwf_geometry *g, const void *in_even, const v
 DWF_API int dwf_dhop_eo_axpy(const dwf_geometry *g, const void *in_odd, const void *x_even, double a, double b,
                      void *out_even, void *stream);
 
+/* Multiple right-hand sides sharing one gauge load (not in PAPER.md).  `in` and `out` hold
+ * nrhs half fields of the device layout one after the other (nrhs * dwf_field_bytes(g, parity) bytes each);
+ * out_r = DhopOE in_r (dagger != 0: the adjoint) for every r, identical bit for bit to nrhs separate calls.
+ * Dhop does not couple the slices s, so to the staged kernels the nrhs fields are ONE field of nrhs * Ls
+ * slices: a thread loads its 8 links once and walks all of them.  Minimal-traffic model: w (48 + 144 / (Ls
+ * nrhs)) bytes per output 5D site instead of w (48 + 144 / Ls).  The general (direct) kernel runs one launch
+ * per right-hand side.  Asynchronous.  Errors as dwf_dhop_oe; INVALID_ARG for nrhs < 1 or L3 Ls nrhs >= 2^31. */
+DWF_API int dwf_dhop_oe_mrhs(const dwf_geometry *g, const void *in_even, void *out_odd, int nrhs, int dagger, void *stream);
+DWF_API int dwf_dhop_eo_mrhs(const dwf_geometry *g, const void *in_odd, void *out_even, int nrhs, int dagger, void *stream);
+
 /* *result_host = sum over all reals of |field|^2, accumulated in fp64 in a fixed order
  * (deterministic).  parity = DWF_FULL for a full field, DWF_EVEN / DWF_ODD for a half field.
  * Synchronises `stream`. */

@@ -28,6 +28,7 @@ SYMBOLS = (
     "dwf_dhop_eo", "dwf_dhop_dag", "dwf_dhop_oe_dag", "dwf_dhop_eo_dag", "dwf_dhop_oe_axpy", "dwf_dhop_eo_axpy", "dwf_dhop_oe_norm2", "dwf_dhop_eo_norm2", "dwf_norm2", "dwf_inner_product", "dwf_field_bytes",
     "dwf_import_spinor", "dwf_export_spinor", "dwf_launch_count", "dwf_kernel_info", "dwf_set_option",
     "dwf_error_string", "dwf_last_error",
+    "dwf_dhop_oe_mrhs", "dwf_dhop_eo_mrhs",
     "dwf_mooee", "dwf_mooee_inv", "dwf_ddwf", "dwf_schur_work_bytes", "dwf_schur", "dwf_axpby", "dwf_cg_work_bytes", "dwf_cg_schur",
 )
 
@@ -58,6 +59,8 @@ def load(build_if_missing: bool = True):
     lib.dwf_load_gauge.argtypes = [vp, vp, ci, vp]
     for f in (lib.dwf_dhop, lib.dwf_dhop_oe, lib.dwf_dhop_eo, lib.dwf_dhop_dag, lib.dwf_dhop_oe_dag, lib.dwf_dhop_eo_dag):
         f.argtypes = [vp, vp, vp, vp]
+    for f in (lib.dwf_dhop_oe_mrhs, lib.dwf_dhop_eo_mrhs):
+        f.argtypes = [vp, vp, vp, ci, ci, vp]
     lib.dwf_norm2.argtypes = [vp, vp, ci, ctypes.POINTER(ctypes.c_double), vp]
     for f in (lib.dwf_dhop_oe_axpy, lib.dwf_dhop_eo_axpy):
         f.argtypes = [vp, vp, vp, ctypes.c_double, ctypes.c_double, vp, vp]
@@ -200,6 +203,27 @@ def dwf_dhop_oe_dag(g: int, in_even, out_odd, stream=None) -> None:
 
 def dwf_dhop_eo_dag(g: int, in_odd, out_even, stream=None) -> None:
     _check(load().dwf_dhop_eo_dag(g, _dev_ptr(in_odd, g, ODD), _dev_ptr(out_even, g, EVEN), _stream(stream, g)), "dwf_dhop_eo_dag")
+
+
+def _mrhs_ptr(t, g, parity, nrhs):
+    """Address of nrhs device fields stored one after the other (size- and dtype-checked)."""
+    if not getattr(t, "is_cuda", False) or not t.is_contiguous():
+        raise ValueError("device fields must be contiguous torch CUDA tensors")
+    if g in _geom_info:
+        prec = _geom_info[g][0]
+        if t.element_size() != prec or t.numel() * prec != int(nrhs) * dwf_field_bytes(g, parity):
+            raise DwfError(ERR_INVALID_ARG, "binding", "multi-RHS buffer does not match nrhs fields of the geometry (dtype or size)")
+    return t.data_ptr()
+
+
+def dwf_dhop_oe_mrhs(g: int, in_even, out_odd, nrhs: int, dagger: bool = False, stream=None) -> None:
+    _check(load().dwf_dhop_oe_mrhs(g, _mrhs_ptr(in_even, g, EVEN, nrhs), _mrhs_ptr(out_odd, g, ODD, nrhs), int(nrhs),
+                                   int(bool(dagger)), _stream(stream, g)), "dwf_dhop_oe_mrhs")
+
+
+def dwf_dhop_eo_mrhs(g: int, in_odd, out_even, nrhs: int, dagger: bool = False, stream=None) -> None:
+    _check(load().dwf_dhop_eo_mrhs(g, _mrhs_ptr(in_odd, g, ODD, nrhs), _mrhs_ptr(out_even, g, EVEN, nrhs), int(nrhs),
+                                   int(bool(dagger)), _stream(stream, g)), "dwf_dhop_eo_mrhs")
 
 
 def dwf_dhop_oe_axpy(g: int, in_even, x_odd, a: float, b: float, out_odd, stream=None) -> None:
@@ -406,6 +430,17 @@ class Geometry:
     def dhop_eo(self, in_odd, out=None, stream=None):
         out = self.new_field(EVEN) if out is None else out
         dwf_dhop_eo(self.handle, in_odd, out, stream)
+        return out
+
+    def dhop_oe_mrhs(self, in_even, nrhs, dagger=False, out=None, stream=None):
+        """nrhs right-hand sides (fields stored one after the other) in one launch, one gauge load."""
+        out = self._torch.empty_like(in_even) if out is None else out
+        dwf_dhop_oe_mrhs(self.handle, in_even, out, nrhs, dagger, stream)
+        return out
+
+    def dhop_eo_mrhs(self, in_odd, nrhs, dagger=False, out=None, stream=None):
+        out = self._torch.empty_like(in_odd) if out is None else out
+        dwf_dhop_eo_mrhs(self.handle, in_odd, out, nrhs, dagger, stream)
         return out
 
     def dhop_oe_axpy(self, in_even, x_odd, a, b, out=None, stream=None):

@@ -340,7 +340,7 @@ int dwf_load_gauge(dwf_geometry *g, const void *U, int src_is_device, void *stre
 // one half-Dhop: out (parity_out) = D in (opposite parity), or a x + b D in when axpy_x is given; picks
 // the kernel.  Every kernel has the fused a x + b Dhop epilogue, x == out is allowed on all of them.
 int dwf::half_dhop(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger,
-                   const void *axpy_x, double a, double b)
+                   const void *axpy_x, double a, double b, int nrhs)
 {
     const bool staged_any = g->staged.variant >= 0, staged64_ok = g->staged64.variant >= 0;
     const bool staged_ok = staged_any && (!axpy_x || staged_supports_axpy(g));
@@ -352,14 +352,23 @@ int dwf::half_dhop(const dwf_geometry *g, const void *in, void *out, int parity_
         return DWF_ERR_UNSUPPORTED;
     }
     if (staged_ok && g->opt_kernel != 1)
-        return launch_dhop_staged(g, in, out, parity_out, st, nullptr, nullptr, dagger, axpy_x, (float)a, (float)b);
+        return launch_dhop_staged(g, in, out, parity_out, st, nullptr, nullptr, dagger, axpy_x, (float)a, (float)b, nrhs);
     if (staged_two_pass && g->opt_kernel != 1) {
-        int rc = launch_dhop_staged(g, in, out, parity_out, st, nullptr, nullptr, dagger);
+        int rc = launch_dhop_staged(g, in, out, parity_out, st, nullptr, nullptr, dagger, nullptr, 0.f, 0.f, nrhs);
         if (rc) return rc;
-        return launch_axpby(g, axpy_x, out, a, b, dwf_field_bytes(g, parity_out) / (size_t)g->prec, st);
+        return launch_axpby(g, axpy_x, out, a, b, (size_t)nrhs * dwf_field_bytes(g, parity_out) / (size_t)g->prec, st);
     }
-    if (staged64_ok && g->opt_kernel != 1) return launch_dhop_staged64(g, in, out, parity_out, st, dagger, axpy_x, a, b);
-    return launch_dhop_direct(g, in, out, parity_out, st, dagger, axpy_x, a, b);
+    if (staged64_ok && g->opt_kernel != 1)
+        return launch_dhop_staged64(g, in, out, parity_out, st, dagger, axpy_x, a, b, nullptr, nullptr, nrhs);
+    // the direct kernel knows one field: one launch per right-hand side (the links are re-read)
+    const size_t fb = dwf_field_bytes(g, parity_out);
+    for (int r = 0; r < nrhs; r++) {
+        const char *xi = axpy_x ? static_cast<const char *>(axpy_x) + r * fb : nullptr;
+        int rc = launch_dhop_direct(g, static_cast<const char *>(in) + r * fb, static_cast<char *>(out) + r * fb, parity_out, st, dagger,
+                                    xi, a, b);
+        if (rc) return rc;
+    }
+    return DWF_OK;
 }
 
 extern "C" {
@@ -407,6 +416,27 @@ int dwf_dhop_oe_dag(const dwf_geometry *g, const void *in_even, void *out_odd, v
 int dwf_dhop_eo_dag(const dwf_geometry *g, const void *in_odd, void *out_even, void *stream)
 {
     return dhop_common(g, in_odd, out_even, DWF_EVEN, stream, "dwf_dhop_eo_dag", true);
+}
+
+// nrhs right-hand sides in one launch, one gauge load for all of them
+static int dhop_mrhs_common(const dwf_geometry *g, const void *in, void *out, int parity_out, int nrhs, int dagger, void *stream,
+                            const char *who)
+{
+    if (!g || !in || !out || nrhs < 1) { set_error("%s: NULL argument or nrhs < 1", who); return DWF_ERR_INVALID_ARG; }
+    if (in == out) { set_error("%s: in-place application is not defined (in == out)", who); return DWF_ERR_INVALID_ARG; }
+    if (!aligned16(in) || !aligned16(out)) { set_error("%s: field pointers must be 16-byte aligned", who); return DWF_ERR_INVALID_ARG; }
+    if ((double)g->lat.L[3] * g->lat.Ls * nrhs >= 2147483647.0) { set_error("%s: L3 * Ls * nrhs exceeds 2^31", who); return DWF_ERR_INVALID_ARG; }
+    if (!g->gauge_loaded) { set_error("%s: call dwf_load_gauge first", who); return DWF_ERR_NO_GAUGE; }
+    DeviceGuard guard(g->device);
+    return half_dhop(g, in, out, parity_out, static_cast<cudaStream_t>(stream), dagger != 0, nullptr, 0.0, 0.0, nrhs);
+}
+int dwf_dhop_oe_mrhs(const dwf_geometry *g, const void *in_even, void *out_odd, int nrhs, int dagger, void *stream)
+{
+    return dhop_mrhs_common(g, in_even, out_odd, DWF_ODD, nrhs, dagger, stream, "dwf_dhop_oe_mrhs");
+}
+int dwf_dhop_eo_mrhs(const dwf_geometry *g, const void *in_odd, void *out_even, int nrhs, int dagger, void *stream)
+{
+    return dhop_mrhs_common(g, in_odd, out_even, DWF_EVEN, nrhs, dagger, stream, "dwf_dhop_eo_mrhs");
 }
 
 }  // extern "C"

@@ -629,11 +629,11 @@ void build_staged_tile_table(const dwf_geometry *g, int raster, int4 *tab)
 
 // tensor map of a half field complex[s][x3][x2][x1][k/2][h][k&1] seen as 5-D fp32 tensor
 // (4*Lh, 6, L1, L2, L3*Ls): x3 and s share the slowest dimension (the s stride is L3 x3-strides)
-static int encode_map(CUtensorMap *m, const void *base, const Lattice &lat, int b1, int b2, int b3)
+static int encode_map(CUtensorMap *m, const void *base, const Lattice &lat, int Ls, int b1, int b2, int b3)
 {
     PFN_tensorMapEncodeTiled enc = get_tensor_map_encoder();
     const cuuint64_t dims[5] = {(cuuint64_t)4 * lat.Lh, 6, (cuuint64_t)lat.L[1], (cuuint64_t)lat.L[2],
-                                (cuuint64_t)lat.L[3] * lat.Ls};
+                                (cuuint64_t)lat.L[3] * Ls};
     const cuuint64_t krow = (cuuint64_t)lat.Lh * 16, row = 6 * krow;
     const cuuint64_t strides[4] = {krow, row, row * lat.L[1], row * lat.L[1] * lat.L[2]};
     const cuuint32_t box[5] = {(cuuint32_t)4 * lat.Lh, 6, (cuuint32_t)b1, (cuuint32_t)b2, (cuuint32_t)b3};
@@ -650,24 +650,24 @@ static int encode_map(CUtensorMap *m, const void *base, const Lattice &lat, int 
 
 // The six tensor maps of a field depend on its pointer and the tile shape only.  A solver applies the
 // operator to the same few buffers over and over, so the encoded maps are kept in a small
-// per-thread cache (keyed by geometry id, variant and pointer): no driver calls on a hit.
-struct MapSet { unsigned long long gid; int variant; const void *ptr; CUtensorMap m[6]; };
+// per-thread cache (keyed by geometry id, variant, pointer and slice count): no driver calls on a hit.
+struct MapSet { unsigned long long gid; int variant, ls; const void *ptr; CUtensorMap m[6]; };
 
-static int get_maps(const dwf_geometry *g, const Variant &v, const void *ptr, MapSet **out)
+static int get_maps(const dwf_geometry *g, const Variant &v, const void *ptr, int ls, MapSet **out)
 {
     static thread_local MapSet cache[8];
     static thread_local unsigned next_slot = 0;
     for (MapSet &c : cache)
-        if (c.ptr == ptr && c.gid == g->uid && c.variant == g->staged.variant) { *out = &c; return DWF_OK; }
+        if (c.ptr == ptr && c.gid == g->uid && c.variant == g->staged.variant && c.ls == ls) { *out = &c; return DWF_OK; }
     MapSet t;
-    t.gid = g->uid; t.variant = g->staged.variant; t.ptr = ptr;
+    t.gid = g->uid; t.variant = g->staged.variant; t.ptr = ptr; t.ls = ls;
     int rc;
-    if ((rc = encode_map(&t.m[0], ptr, g->lat, v.b1, v.b2, v.b3))) return rc;
-    if ((rc = encode_map(&t.m[1], ptr, g->lat, 1, v.b2, v.b3))) return rc;
-    if ((rc = encode_map(&t.m[2], ptr, g->lat, v.b1, 1, v.b3))) return rc;
-    if ((rc = encode_map(&t.m[3], ptr, g->lat, v.b1, v.b2, 1))) return rc;
-    if ((rc = encode_map(&t.m[4], ptr, g->lat, 1, v.b2, 1))) return rc;
-    if ((rc = encode_map(&t.m[5], ptr, g->lat, v.b1, 1, 1))) return rc;
+    if ((rc = encode_map(&t.m[0], ptr, g->lat, ls, v.b1, v.b2, v.b3))) return rc;
+    if ((rc = encode_map(&t.m[1], ptr, g->lat, ls, 1, v.b2, v.b3))) return rc;
+    if ((rc = encode_map(&t.m[2], ptr, g->lat, ls, v.b1, 1, v.b3))) return rc;
+    if ((rc = encode_map(&t.m[3], ptr, g->lat, ls, v.b1, v.b2, 1))) return rc;
+    if ((rc = encode_map(&t.m[4], ptr, g->lat, ls, 1, v.b2, 1))) return rc;
+    if ((rc = encode_map(&t.m[5], ptr, g->lat, ls, v.b1, 1, 1))) return rc;
     MapSet *ms = &cache[next_slot++ % 8];
     *ms = t;
     *out = ms;
@@ -681,8 +681,12 @@ bool staged_supports_axpy(const dwf_geometry *g)
 
 int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st,
                        double *norm_partials, int *norm_blocks, bool dagger, const void *axpy_x, float axpy_a,
-                       float axpy_b)
+                       float axpy_b, int nrhs)
 {
+    // nrhs > 1: `in`, `out` (and x) hold nrhs fields one after the other.  Dhop is diagonal
+    // in s, so they are ONE field of nrhs * Ls slices to this kernel: the links of a tile stay in registers
+    // for all of them.
+    const int ls = g->lat.Ls * nrhs;
     if (norm_partials && (dagger || axpy_x)) {
         set_error("the staged kernel has no instance for this combination of modes");
         return DWF_ERR_UNSUPPORTED;
@@ -695,11 +699,11 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     // first, so the maps are copied before it (they are passed to the kernel by value anyway).
     MapSet *ms = nullptr;
     int rc;
-    if ((rc = get_maps(g, v, in, &ms))) return rc;
+    if ((rc = get_maps(g, v, in, ls, &ms))) return rc;
     CUtensorMap mc = ms->m[0], m1 = ms->m[1], m2 = ms->m[2], m3 = ms->m[3], m1l = ms->m[4], m2l = ms->m[5];
     CUtensorMap mxc = mc;
     if (axpy_x) {
-        if ((rc = get_maps(g, v, axpy_x, &ms))) return rc;
+        if ((rc = get_maps(g, v, axpy_x, ls, &ms))) return rc;
         mxc = ms->m[0];
     }
     StagedArgs a;
@@ -707,7 +711,7 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     a.gauge = static_cast<const float2 *>(g->gauge[parity_out]);
     a.tiles = g->tiles_staged;
     a.ntiles = g->staged.ntiles;
-    a.L1 = g->lat.L[1]; a.L2 = g->lat.L[2]; a.L3 = g->lat.L[3]; a.Ls = g->lat.Ls;
+    a.L1 = g->lat.L[1]; a.L2 = g->lat.L[2]; a.L3 = g->lat.L[3]; a.Ls = ls;
     a.parity_out = parity_out;
     a.l2pol = g->opt_l2pol;
     a.zigzag = g->opt_zigzag;
@@ -719,7 +723,7 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     int ssplit = g->opt_ssplit > 0 ? g->opt_ssplit : 1;
     const int ctas = (v.ctas_per_sm == 2 && 2 * (smem + 1024) > SMEM_LIMIT) ? 1 : v.ctas_per_sm;
     const int slots = g->sm_count * ctas;       // co-resident CTAs
-    while (ssplit > 1 && (g->lat.Ls % ssplit || slots % ssplit)) ssplit--;
+    while (ssplit > 1 && (ls % ssplit || slots % ssplit)) ssplit--;
     a.ssplit = ssplit;
     const void *fn = v.fn[mode];
     const int ngroup_max = slots / ssplit;

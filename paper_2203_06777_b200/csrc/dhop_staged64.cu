@@ -547,11 +547,11 @@ void build_staged64_tile_table(const dwf_geometry *g, int4 *tab)
 
 // tensor map of an fp64 half field complex[s][x3][x2][x1][k][h] seen as 5-D fp64 tensor
 // (2*Lh, 12, L1, L2, L3*Ls)
-static int encode_map64(CUtensorMap *m, const void *base, const Lattice &lat, int b1, int b2, int b3)
+static int encode_map64(CUtensorMap *m, const void *base, const Lattice &lat, int Ls, int b1, int b2, int b3)
 {
     PFN_tensorMapEncodeTiled enc = get_tensor_map_encoder();
     const cuuint64_t dims[5] = {(cuuint64_t)2 * lat.Lh, 12, (cuuint64_t)lat.L[1], (cuuint64_t)lat.L[2],
-                                (cuuint64_t)lat.L[3] * lat.Ls};
+                                (cuuint64_t)lat.L[3] * Ls};
     const cuuint64_t krow = (cuuint64_t)lat.Lh * 16, row = 12 * krow;
     const cuuint64_t strides[4] = {krow, row, row * lat.L[1], row * lat.L[1] * lat.L[2]};
     const cuuint32_t box[5] = {(cuuint32_t)2 * lat.Lh, 12, (cuuint32_t)b1, (cuuint32_t)b2, (cuuint32_t)b3};
@@ -569,21 +569,21 @@ static int encode_map64(CUtensorMap *m, const void *base, const Lattice &lat, in
 // The four tensor maps of a field depend on its pointer and the tile shape only: kept in a small
 // per-thread cache (keyed by geometry id, variant and pointer) so that a solver that applies the
 // operator to the same few buffers makes no driver calls (as dhop_staged.cu does for fp32).
-struct MapSet64 { unsigned long long gid; int variant; const void *ptr; CUtensorMap m[4]; };
+struct MapSet64 { unsigned long long gid; int variant, ls; const void *ptr; CUtensorMap m[4]; };
 
-static int get_maps64(const dwf_geometry *g, const Variant64 &v, const void *ptr, const MapSet64 **out)
+static int get_maps64(const dwf_geometry *g, const Variant64 &v, const void *ptr, int ls, const MapSet64 **out)
 {
     static thread_local MapSet64 cache[8];
     static thread_local unsigned next_slot = 0;
     for (const MapSet64 &c : cache)
-        if (c.ptr == ptr && c.gid == g->uid && c.variant == g->staged64.variant) { *out = &c; return DWF_OK; }
+        if (c.ptr == ptr && c.gid == g->uid && c.variant == g->staged64.variant && c.ls == ls) { *out = &c; return DWF_OK; }
     MapSet64 t;
-    t.gid = g->uid; t.variant = g->staged64.variant; t.ptr = ptr;
+    t.gid = g->uid; t.variant = g->staged64.variant; t.ptr = ptr; t.ls = ls;
     int rc;
-    if ((rc = encode_map64(&t.m[0], ptr, g->lat, v.b1, v.b2, v.b3))) return rc;
-    if ((rc = encode_map64(&t.m[1], ptr, g->lat, 1, v.b2, v.b3))) return rc;
-    if ((rc = encode_map64(&t.m[2], ptr, g->lat, v.b1, 1, v.b3))) return rc;
-    if ((rc = encode_map64(&t.m[3], ptr, g->lat, v.b1, v.b2, 1))) return rc;
+    if ((rc = encode_map64(&t.m[0], ptr, g->lat, ls, v.b1, v.b2, v.b3))) return rc;
+    if ((rc = encode_map64(&t.m[1], ptr, g->lat, ls, 1, v.b2, v.b3))) return rc;
+    if ((rc = encode_map64(&t.m[2], ptr, g->lat, ls, v.b1, 1, v.b3))) return rc;
+    if ((rc = encode_map64(&t.m[3], ptr, g->lat, ls, v.b1, v.b2, 1))) return rc;
     MapSet64 *ms = &cache[next_slot++ % 8];
     *ms = t;
     *out = ms;
@@ -591,8 +591,9 @@ static int get_maps64(const dwf_geometry *g, const Variant64 &v, const void *ptr
 }
 
 int launch_dhop_staged64(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger,
-                         const void *axpy_x, double axpy_a, double axpy_b, double *norm_partials, int *norm_blocks)
+                         const void *axpy_x, double axpy_a, double axpy_b, double *norm_partials, int *norm_blocks, int nrhs)
 {
+    const int ls = g->lat.Ls * nrhs;       // nrhs fields one after the other = one field of nrhs * Ls slices (dhop_staged.cu)
     if (norm_partials && (dagger || axpy_x)) {
         set_error("the fp64 staged kernel has no instance for this combination of modes");
         return DWF_ERR_UNSUPPORTED;
@@ -600,14 +601,14 @@ int launch_dhop_staged64(const dwf_geometry *g, const void *in, void *out, int p
     const Variant64 &v = variants64()[(size_t)g->staged64.variant];
     const MapSet64 *ms = nullptr;
     int rc;
-    if ((rc = get_maps64(g, v, in, &ms))) return rc;
+    if ((rc = get_maps64(g, v, in, ls, &ms))) return rc;
     CUtensorMap mc = ms->m[0], m1 = ms->m[1], m2 = ms->m[2], m3 = ms->m[3];     // passed by value
     Staged64Args a;
     a.out = static_cast<double2 *>(out);
     a.gauge = static_cast<const double2 *>(g->gauge[parity_out]);
     a.tiles = g->tiles_staged64;
     a.ntiles = g->staged64.ntiles;
-    a.L1 = g->lat.L[1]; a.L2 = g->lat.L[2]; a.L3 = g->lat.L[3]; a.Ls = g->lat.Ls;
+    a.L1 = g->lat.L[1]; a.L2 = g->lat.L[2]; a.L3 = g->lat.L[3]; a.Ls = ls;
     a.parity_out = parity_out;
     a.zigzag = g->opt_zigzag;
     a.l2pol = g->opt_l2pol;

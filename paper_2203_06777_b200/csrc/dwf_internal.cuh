@@ -125,7 +125,7 @@ bool parity_ok(int p);
 bool aligned16(const void *p);
 // one half-Dhop (or a x + b Dhop) on the best kernel for the geometry
 int half_dhop(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger = false,
-              const void *axpy_x = nullptr, double a = 0.0, double b = 0.0);
+              const void *axpy_x = nullptr, double a = 0.0, double b = 0.0, int nrhs = 1);
 // waits for the reduction last enqueued on st and returns its n values (through the mapped mailbox)
 int fetch_reduction(const dwf_geometry *g, cudaStream_t st, int n, double *out);
 
@@ -144,7 +144,8 @@ void build_staged_tile_table(const dwf_geometry *g, int raster, int4 *host_table
 // norm_partials != nullptr: the fused-norm2 kernel writes one partial of |out|^2 per CTA there, *norm_blocks = their number
 int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st,
                        double *norm_partials = nullptr, int *norm_blocks = nullptr, bool dagger = false,
-                       const void *axpy_x = nullptr, float axpy_a = 0.f, float axpy_b = 0.f);   // axpy_x: out = a x + b Dhop in
+                       const void *axpy_x = nullptr, float axpy_a = 0.f, float axpy_b = 0.f,     // axpy_x: out = a x + b Dhop in
+                       int nrhs = 1);                                                           // nrhs fields one after the other
 bool staged_supports_axpy(const dwf_geometry *g);
 // pack.cu: out = a x + b out, elementwise over nreal reals (the unfused path of dwf_dhop_*_axpy)
 int launch_axpby(const dwf_geometry *g, const void *x, void *out, double a, double b, size_t nreal, cudaStream_t st);
@@ -154,7 +155,7 @@ void build_staged64_tile_table(const dwf_geometry *g, int4 *host_table);
 // norm_partials != nullptr: the fused-norm2 instance, one partial of |out|^2 per CTA, *norm_blocks = their number
 int launch_dhop_staged64(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger,
                          const void *axpy_x = nullptr, double axpy_a = 0.0, double axpy_b = 0.0,
-                         double *norm_partials = nullptr, int *norm_blocks = nullptr);
+                         double *norm_partials = nullptr, int *norm_blocks = nullptr, int nrhs = 1);
 // reduce.cu
 int launch_norm2(const dwf_geometry *g, const void *field, size_t nreal, cudaStream_t st);
 int launch_final_sum(const dwf_geometry *g, int nblocks, cudaStream_t st);   // result_dev[0] = sum of partials[0..nblocks)
