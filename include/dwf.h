@@ -194,14 +194,23 @@ DWF_API int dwf_cg_schur(const dwf_geometry *g, const void *b, void *x, int pari
 /* Bytes of a device field: full (DWF_FULL) or half (DWF_EVEN / DWF_ODD).  0 on bad arguments. */
 DWF_API size_t dwf_field_bytes(const dwf_geometry *g, int parity);
 
-/* canonical -> device layout.  Host sources go through an internal staging copy and synchronise
- * `stream`; device sources are asynchronous. */
+/* canonical -> device layout.  Device sources are asynchronous on `stream`.  Host sources (pinned memory
+ * for full PCIe speed) are moved in chunks of whole lattice lines through a ring of two 32 MB device
+ * buffers: the H2D copy of chunk k+1 runs on an internal copy stream under the reorder kernel of chunk k;
+ * the call synchronises `stream` before it returns unless the option "async_host" is set (then the host
+ * array must stay untouched until dwf_host_wait). */
 DWF_API int dwf_import_spinor(const dwf_geometry *g, const void *canonical, int src_is_device, int parity,
                       void *field_dev, void *stream);
 
-/* device layout -> canonical.  Host destinations synchronise `stream`. */
+/* device layout -> canonical.  Host destinations: the same ring in the other direction on a second copy
+ * stream (an export's D2H copies overlap a following import's H2D copies: PCIe is full duplex); the call
+ * waits for the last copy unless "async_host" is set (then the host array is complete after dwf_host_wait). */
 DWF_API int dwf_export_spinor(const dwf_geometry *g, const void *field_dev, int parity, void *canonical,
                       int dst_is_device, void *stream);
+
+/* Blocks until every host transfer (import / export with host arrays) issued on g has completed.  Only needed
+ * with the option "async_host".  Errors: INVALID_ARG, CUDA. */
+DWF_API int dwf_host_wait(const dwf_geometry *g);
 
 /* Number of kernel launches this library has issued since it was loaded (all threads). */
 DWF_API unsigned long long dwf_launch_count(void);
@@ -224,6 +233,8 @@ DWF_API int dwf_kernel_info(const dwf_geometry *g, char *buf, size_t n);
  *   "l2pol"          decimal digits, one L2 eviction class per access type (dhop_staged.cu PC_*):
  *                    0 evict_normal, 1 evict_first, 2 evict_last
  *   "prefetch"       low 4 bits: L2 prefetch distance in steps (0 off), higher bits: box mask
+ *   "async_host"     1: dwf_import_spinor / dwf_export_spinor with host arrays return without synchronising
+ *                    (pipelined steps; dwf_host_wait before touching the host arrays)
  *   "l2persist"      MB of L2 set aside for evict_last lines (device-wide CUDA limit)
  *   "raster", "tile0".."tile3", "cpc"   direct kernel: CTA launch order, log2 tile extents, slices per CTA */
 DWF_API int dwf_set_option(dwf_geometry *g, const char *key, long long value);

@@ -28,7 +28,7 @@ SYMBOLS = (
     "dwf_dhop_eo", "dwf_dhop_dag", "dwf_dhop_oe_dag", "dwf_dhop_eo_dag", "dwf_dhop_oe_axpy", "dwf_dhop_eo_axpy", "dwf_dhop_oe_norm2", "dwf_dhop_eo_norm2", "dwf_norm2", "dwf_inner_product", "dwf_field_bytes",
     "dwf_import_spinor", "dwf_export_spinor", "dwf_launch_count", "dwf_kernel_info", "dwf_set_option",
     "dwf_error_string", "dwf_last_error",
-    "dwf_dhop_oe_mrhs", "dwf_dhop_eo_mrhs",
+    "dwf_dhop_oe_mrhs", "dwf_dhop_eo_mrhs", "dwf_host_wait",
     "dwf_mooee", "dwf_mooee_inv", "dwf_ddwf", "dwf_schur_work_bytes", "dwf_schur", "dwf_axpby", "dwf_cg_work_bytes", "dwf_cg_schur",
 )
 
@@ -71,6 +71,7 @@ def load(build_if_missing: bool = True):
     lib.dwf_field_bytes.restype = cs
     lib.dwf_import_spinor.argtypes = [vp, vp, ci, ci, vp, vp]
     lib.dwf_export_spinor.argtypes = [vp, vp, ci, vp, ci, vp]
+    lib.dwf_host_wait.argtypes = [vp]
     lib.dwf_launch_count.argtypes = []
     lib.dwf_launch_count.restype = ctypes.c_ulonglong
     lib.dwf_kernel_info.argtypes = [vp, ctypes.c_char_p, cs]
@@ -327,6 +328,10 @@ def dwf_cg_schur(g: int, b, x, parity: int, M5: float, mass: float, tol: float, 
     return it.value, res.value
 
 
+def dwf_host_wait(g: int) -> None:
+    _check(load().dwf_host_wait(g), "dwf_host_wait")
+
+
 def dwf_launch_count() -> int:
     return int(load().dwf_launch_count())
 
@@ -507,6 +512,9 @@ class Geometry:
         work = self.new_work(dwf_cg_work_bytes(self.handle)) if work is None else work
         it, res = dwf_cg_schur(self.handle, b, x, parity, M5, mass, tol, max_iter, work, stream)
         return x, it, res
+
+    def host_wait(self):
+        dwf_host_wait(self.handle)
 
     def set_option(self, key: str, value: int):
         dwf_set_option(self.handle, key, value)

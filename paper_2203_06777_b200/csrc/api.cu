@@ -119,16 +119,125 @@ int rebuild_tilings(dwf_geometry *g)
     return DWF_OK;
 }
 
-static int ensure_staging(dwf_geometry *g, size_t bytes)
+// ring of device buffers and copy streams for host transfers (dwf_internal.cuh: HostXfer)
+static const size_t XFER_CHUNK = (size_t)32 << 20;
+
+static int ensure_xfer(dwf_geometry *g)
 {
-    if (g->staging_bytes >= bytes) return DWF_OK;
-    if (g->staging) { cudaFree(g->staging); g->staging = nullptr; g->staging_bytes = 0; }
-    if (cudaMalloc(&g->staging, bytes) != cudaSuccess) {
-        cudaGetLastError();
-        set_error("cannot allocate %zu bytes of device staging", bytes);
-        return DWF_ERR_ALLOC;
+    dwf_geometry::HostXfer &x = g->xfer;
+    if (x.ready) return DWF_OK;
+    x.chunk = XFER_CHUNK;
+    for (int d = 0; d < 2; d++) {
+        DWF_CUDA_CHECK(cudaStreamCreateWithFlags(&x.copy_stream[d], cudaStreamNonBlocking));
+        for (int b = 0; b < 2; b++) {
+            if (cudaMalloc(&x.buf[d][b], x.chunk) != cudaSuccess) {
+                cudaGetLastError();
+                set_error("cannot allocate %zu bytes of device staging", x.chunk);
+                return DWF_ERR_ALLOC;
+            }
+            DWF_CUDA_CHECK(cudaEventCreateWithFlags(&x.filled[d][b], cudaEventDisableTiming));
+            DWF_CUDA_CHECK(cudaEventCreateWithFlags(&x.drained[d][b], cudaEventDisableTiming));
+        }
     }
-    g->staging_bytes = bytes;
+    DWF_CUDA_CHECK(cudaStreamCreateWithFlags(&x.export_stream, cudaStreamNonBlocking));
+    DWF_CUDA_CHECK(cudaEventCreateWithFlags(&x.export_begin, cudaEventDisableTiming));
+    DWF_CUDA_CHECK(cudaEventCreateWithFlags(&x.export_done, cudaEventDisableTiming));
+    x.ready = true;
+    return DWF_OK;
+}
+
+static void destroy_xfer(dwf_geometry *g)
+{
+    dwf_geometry::HostXfer &x = g->xfer;
+    for (int d = 0; d < 2; d++) {
+        if (x.copy_stream[d]) { cudaStreamSynchronize(x.copy_stream[d]); cudaStreamDestroy(x.copy_stream[d]); }
+        for (int b = 0; b < 2; b++) {
+            cudaFree(x.buf[d][b]);
+            if (x.filled[d][b]) cudaEventDestroy(x.filled[d][b]);
+            if (x.drained[d][b]) cudaEventDestroy(x.drained[d][b]);
+        }
+    }
+    if (x.export_stream) { cudaStreamSynchronize(x.export_stream); cudaStreamDestroy(x.export_stream); }
+    if (x.export_begin) cudaEventDestroy(x.export_begin);
+    if (x.export_done) cudaEventDestroy(x.export_done);
+    memset(&x, 0, sizeof(x));
+}
+
+void wait_for_exports(const dwf_geometry *g, cudaStream_t st, const void *written, size_t bytes)
+{
+    const dwf_geometry::HostXfer &x = g->xfer;
+    if (!x.ready || !x.export_pending) return;
+    const char *w = static_cast<const char *>(written);
+    if (w && (w + bytes <= x.export_ptr || x.export_ptr + x.export_bytes <= w)) return;      // disjoint
+    cudaStreamWaitEvent(st, x.export_done, 0);
+}
+
+// canonical host array <-> device field in chunks of whole lattice lines (rows): a chunk of rows is a
+// contiguous range of canonical sites.  IMPORT: H2D of chunk k+1 (copy stream) under the reorder of chunk k
+// (caller's stream); export: reorder of chunk k+1 under the D2H of chunk k.
+template <bool IMPORT>
+static int host_transfer(dwf_geometry *g, const void *field_dev, void *field_dev_w, const void *host_src, void *host_dst, int parity,
+                         cudaStream_t st)
+{
+    int rc = ensure_xfer(g);
+    if (rc) return rc;
+    dwf_geometry::HostXfer &x = g->xfer;
+    const int d = IMPORT ? 0 : 1;
+    const Lattice &lat = g->lat;
+    const long long nrow = lat.Vh / lat.Lh;
+    const size_t row_bytes = (size_t)(parity == DWF_FULL ? 2 : 1) * lat.Lh * lat.Ls * 24 * (size_t)g->prec;
+    long long rows_per_chunk = (long long)(x.chunk / row_bytes);
+    if (rows_per_chunk < 1) {          // a single lattice line larger than a ring buffer: grow the ring (rare: L0 * Ls * 96 B > 32 MB)
+        destroy_xfer(g);
+        rc = ensure_xfer(g);
+        if (rc) return rc;
+        for (int dd = 0; dd < 2; dd++)
+            for (int b = 0; b < 2; b++) {
+                cudaFree(x.buf[dd][b]);
+                if (cudaMalloc(&x.buf[dd][b], row_bytes) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate %zu bytes of device staging", row_bytes); return DWF_ERR_ALLOC; }
+            }
+        x.chunk = row_bytes;
+        rows_per_chunk = 1;
+    }
+    cudaStream_t ks = st;           // stream of the reorder kernels
+    if (IMPORT) {
+        wait_for_exports(g, st, field_dev_w, dwf_field_bytes(g, parity));    // the import may overwrite a field that is still being exported
+    } else {
+        ks = x.export_stream;
+        if (x.export_pending && x.export_ptr != field_dev) DWF_CUDA_CHECK(cudaStreamSynchronize(x.export_stream));   // one export tracked at a time
+        x.export_ptr = static_cast<const char *>(field_dev);
+        x.export_bytes = dwf_field_bytes(g, parity);
+        DWF_CUDA_CHECK(cudaEventRecord(x.export_begin, st));
+        DWF_CUDA_CHECK(cudaStreamWaitEvent(ks, x.export_begin, 0));
+    }
+    for (long long row0 = 0; row0 < nrow; row0 += rows_per_chunk) {
+        const long long nr = (nrow - row0 < rows_per_chunk) ? nrow - row0 : rows_per_chunk;
+        const int b = (int)(x.count[d]++ & 1);
+        const size_t off = (size_t)row0 * row_bytes, bytes = (size_t)nr * row_bytes;
+        if (IMPORT) {
+            DWF_CUDA_CHECK(cudaStreamWaitEvent(x.copy_stream[0], x.drained[0][b], 0));
+            DWF_CUDA_CHECK(cudaMemcpyAsync(x.buf[0][b], static_cast<const char *>(host_src) + off, bytes, cudaMemcpyHostToDevice, x.copy_stream[0]));
+            DWF_CUDA_CHECK(cudaEventRecord(x.filled[0][b], x.copy_stream[0]));
+            DWF_CUDA_CHECK(cudaStreamWaitEvent(st, x.filled[0][b], 0));
+            if ((rc = launch_import(g, x.buf[0][b], parity, field_dev_w, st, row0, nr))) return rc;
+            DWF_CUDA_CHECK(cudaEventRecord(x.drained[0][b], st));
+        } else {
+            DWF_CUDA_CHECK(cudaStreamWaitEvent(ks, x.drained[1][b], 0));
+            if ((rc = launch_export(g, field_dev, parity, x.buf[1][b], ks, row0, nr))) return rc;
+            DWF_CUDA_CHECK(cudaEventRecord(x.filled[1][b], ks));
+            DWF_CUDA_CHECK(cudaStreamWaitEvent(x.copy_stream[1], x.filled[1][b], 0));
+            DWF_CUDA_CHECK(cudaMemcpyAsync(static_cast<char *>(host_dst) + off, x.buf[1][b], bytes, cudaMemcpyDeviceToHost, x.copy_stream[1]));
+            DWF_CUDA_CHECK(cudaEventRecord(x.drained[1][b], x.copy_stream[1]));
+        }
+    }
+    if (!IMPORT) {
+        DWF_CUDA_CHECK(cudaEventRecord(x.export_done, ks));
+        x.export_pending = true;
+    }
+    if (!g->opt_async_host) {
+        DWF_CUDA_CHECK(cudaStreamSynchronize(IMPORT ? st : x.copy_stream[1]));
+        if (!IMPORT) x.export_pending = false;
+    }
     return DWF_OK;
 }
 
@@ -250,7 +359,7 @@ int dwf_destroy_geometry(dwf_geometry *g)
     cudaFree(g->tiles_cb);
     cudaFree(g->tiles_staged);
     cudaFree(g->tiles_staged64);
-    cudaFree(g->staging);
+    destroy_xfer(g);
     cudaGetLastError();
     delete g;
     return DWF_OK;
@@ -297,6 +406,9 @@ int dwf_set_option(dwf_geometry *g, const char *key, long long value)
         if (v < 1) { set_error("ssplit must be >= 1"); return DWF_ERR_INVALID_ARG; }
         g->opt_ssplit = v;
         return DWF_OK;
+    } else if (!strcmp(key, "async_host")) {
+        g->opt_async_host = v != 0;
+        return DWF_OK;
     } else if (!strcmp(key, "kernel")) {
         if (v < 0 || v > 2) { set_error("kernel must be 0 (auto), 1 (direct) or 2 (staged)"); return DWF_ERR_INVALID_ARG; }
         g->opt_kernel = v;
@@ -322,15 +434,18 @@ int dwf_load_gauge(dwf_geometry *g, const void *U, int src_is_device, void *stre
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const size_t bytes = (size_t)g->lat.V4 * 72 * (size_t)g->prec;
     const void *src = U;
-    if (!src_is_device) {
-        int rc = ensure_staging(g, bytes);
-        if (rc) return rc;
-        DWF_CUDA_CHECK(cudaMemcpyAsync(g->staging, U, bytes, cudaMemcpyHostToDevice, st));
-        src = g->staging;
+    void *tmp = nullptr;
+    if (!src_is_device) {           // setup path: a temporary device copy of the canonical links, freed before returning
+        if (cudaMalloc(&tmp, bytes) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate %zu bytes for the gauge upload", bytes); return DWF_ERR_ALLOC; }
+        cudaError_t e = cudaMemcpyAsync(tmp, U, bytes, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) { cudaFree(tmp); set_error("gauge upload failed: %s", cudaGetErrorString(e)); return DWF_ERR_CUDA; }
+        src = tmp;
     }
     int rc = launch_pack_gauge(g, src, st);
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (tmp) cudaFree(tmp);
     if (rc) return rc;
-    DWF_CUDA_CHECK(cudaStreamSynchronize(st));
+    if (e != cudaSuccess) { set_error("dwf_load_gauge failed: %s", cudaGetErrorString(e)); return DWF_ERR_CUDA; }
     g->gauge_loaded = true;
     return DWF_OK;
 }
@@ -342,6 +457,7 @@ int dwf_load_gauge(dwf_geometry *g, const void *U, int src_is_device, void *stre
 int dwf::half_dhop(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger,
                    const void *axpy_x, double a, double b, int nrhs)
 {
+    wait_for_exports(g, st, out, (size_t)nrhs * dwf_field_bytes(g, parity_out));
     const bool staged_any = g->staged.variant >= 0, staged64_ok = g->staged64.variant >= 0;
     const bool staged_ok = staged_any && (!axpy_x || staged_supports_axpy(g));
     // tiles whose x rows do not fit into shared memory next to the input slice (Lh = 32): staged Dhop, then
@@ -482,6 +598,7 @@ static int dhop_norm2_common(const dwf_geometry *g, const void *in, void *out, i
     if (!g->gauge_loaded) { set_error("%s: call dwf_load_gauge first", who); return DWF_ERR_NO_GAUGE; }
     DeviceGuard guard(g->device);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    wait_for_exports(g, st, out, dwf_field_bytes(g, parity_out));
     const bool staged_ok = g->staged.variant >= 0;
     if (g->opt_kernel == 2 && !staged_ok && g->staged64.variant < 0) {
         set_error("the staged kernel does not support this geometry / precision");
@@ -567,18 +684,8 @@ int dwf_import_spinor(const dwf_geometry *g, const void *canonical, int src_is_d
     if (canonical == field_dev) { set_error("dwf_import_spinor: in-place conversion not supported"); return DWF_ERR_INVALID_ARG; }
     DeviceGuard guard(g->device);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const size_t bytes = dwf_field_bytes(g, parity);
-    const void *src = canonical;
-    if (!src_is_device) {
-        int rc = ensure_staging(const_cast<dwf_geometry *>(g), bytes);
-        if (rc) return rc;
-        DWF_CUDA_CHECK(cudaMemcpyAsync(g->staging, canonical, bytes, cudaMemcpyHostToDevice, st));
-        src = g->staging;
-    }
-    int rc = launch_import(g, src, parity, field_dev, st);
-    if (rc) return rc;
-    if (!src_is_device) DWF_CUDA_CHECK(cudaStreamSynchronize(st));
-    return DWF_OK;
+    if (!src_is_device) return host_transfer<true>(const_cast<dwf_geometry *>(g), nullptr, field_dev, canonical, nullptr, parity, st);
+    return launch_import(g, canonical, parity, field_dev, st);
 }
 
 int dwf_export_spinor(const dwf_geometry *g, const void *field_dev, int parity, void *canonical, int dst_is_device, void *stream)
@@ -588,14 +695,18 @@ int dwf_export_spinor(const dwf_geometry *g, const void *field_dev, int parity, 
     if (canonical == field_dev) { set_error("dwf_export_spinor: in-place conversion not supported"); return DWF_ERR_INVALID_ARG; }
     DeviceGuard guard(g->device);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const size_t bytes = dwf_field_bytes(g, parity);
     if (dst_is_device) return launch_export(g, field_dev, parity, canonical, st);
-    int rc = ensure_staging(const_cast<dwf_geometry *>(g), bytes);
-    if (rc) return rc;
-    rc = launch_export(g, field_dev, parity, g->staging, st);
-    if (rc) return rc;
-    DWF_CUDA_CHECK(cudaMemcpyAsync(canonical, g->staging, bytes, cudaMemcpyDeviceToHost, st));
-    DWF_CUDA_CHECK(cudaStreamSynchronize(st));
+    return host_transfer<false>(const_cast<dwf_geometry *>(g), field_dev, nullptr, nullptr, canonical, parity, st);
+}
+
+int dwf_host_wait(const dwf_geometry *g)
+{
+    if (!g) { set_error("dwf_host_wait: NULL argument"); return DWF_ERR_INVALID_ARG; }
+    if (!g->xfer.ready) return DWF_OK;
+    DeviceGuard guard(g->device);
+    DWF_CUDA_CHECK(cudaStreamSynchronize(g->xfer.copy_stream[0]));
+    DWF_CUDA_CHECK(cudaStreamSynchronize(g->xfer.copy_stream[1]));
+    const_cast<dwf_geometry *>(g)->xfer.export_pending = false;
     return DWF_OK;
 }
 

@@ -149,6 +149,7 @@ template <typename V, typename T, int OP>
 static int launch_s_op_t(const dwf_geometry *g, const void *in, void *out, int parity, double M5, double mass, bool dagger,
                          cudaStream_t st)
 {
+    wait_for_exports(g, st, out, dwf_field_bytes(g, parity));
     const Lattice &lat = g->lat;
     const size_t vec_per_site = 96 * (size_t)g->prec / 4 / 16;                 // 6 (fp32) or 12 (fp64) vectors per site
     const size_t slice_vecs = (size_t)lat.Vh * vec_per_site;
@@ -234,6 +235,7 @@ static int blas_blocks(const dwf_geometry *g, size_t nvec)
 static int launch_axpby2(const dwf_geometry *g, double a, const void *x, double b, const void *y, void *out, size_t nreal,
                          cudaStream_t st)
 {
+    wait_for_exports(g, st, out, nreal * (size_t)g->prec);
     if (g->prec == DWF_F32) {
         const size_t nv = nreal / 4;
         axpby_kernel2<float4, float><<<blas_blocks(g, nv), 256, 0, st>>>((float)a, static_cast<const float4 *>(x), (float)b,
@@ -252,6 +254,7 @@ static int launch_axpby2(const dwf_geometry *g, double a, const void *x, double 
 static int cg_update(const dwf_geometry *g, double alpha, const void *p, const void *w, void *x, void *r, size_t nreal,
                      double *rr, cudaStream_t st)
 {
+    wait_for_exports(g, st);
     int nb;
     if (g->prec == DWF_F32) {
         const size_t nv = nreal / 4;

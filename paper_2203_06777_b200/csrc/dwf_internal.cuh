@@ -89,9 +89,28 @@ struct dwf_geometry {
     double *mailbox_dev;    // the same words as the device sees them
     unsigned long long mailbox_seq;   // last sequence number handed to a reduction
     int reduce_blocks;
-    // device staging for canonical <-> device conversions of host arrays (lazily grown)
-    void *staging;
-    size_t staging_bytes;
+    // Host <-> device transfers of canonical arrays (dwf_import_spinor / dwf_export_spinor with host
+    // buffers) go through a bounded ring: per direction (0: import, 1: export) one copy stream and two
+    // device buffers of xfer_chunk bytes; the copy of chunk k+1 overlaps the reorder kernel of chunk k,
+    // and the two directions use different streams (PCIe is full duplex).  Created on first use.
+    struct HostXfer {
+        bool ready;
+        size_t chunk;                       // bytes per ring buffer
+        cudaStream_t copy_stream[2];
+        void *buf[2][2];
+        cudaEvent_t filled[2][2];           // buffer holds a chunk (import: H2D done; export: reorder done)
+        cudaEvent_t drained[2][2];          // buffer may be overwritten (import: reorder done; export: D2H done)
+        unsigned long long count[2];        // chunks issued so far (ring position)
+        // export reorder kernels run on their own stream behind an event of the caller's stream, so that the
+        // caller's stream is not held up for the duration of the D2H copies; library calls that launch work
+        // on a caller's stream first wait for export_done (they might overwrite the field being exported)
+        cudaStream_t export_stream;
+        cudaEvent_t export_begin, export_done;
+        bool export_pending;
+        const char *export_ptr;             // device field (and its size) an asynchronous export is still reading
+        size_t export_bytes;
+    } xfer;
+    int opt_async_host;     // 1: host imports / exports return without synchronising (dwf_host_wait)
     // tunables (dwf_set_option)
     int opt_tile[4];        // requested log2 tile extents (cb: dim 0 in pairs)
     int opt_cpc;
@@ -122,6 +141,9 @@ struct DeviceGuard {
     ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 bool parity_ok(int p);
+// orders later work on st that WRITES [written, written + bytes) behind the reorder kernels of an asynchronous
+// host export still reading that memory (written == nullptr: any memory)
+void wait_for_exports(const dwf_geometry *g, cudaStream_t st, const void *written = nullptr, size_t bytes = 0);
 bool aligned16(const void *p);
 // one half-Dhop (or a x + b Dhop) on the best kernel for the geometry
 int half_dhop(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger = false,
@@ -131,10 +153,11 @@ int fetch_reduction(const dwf_geometry *g, cudaStream_t st, int n, double *out);
 
 // pack.cu
 int launch_pack_gauge(const dwf_geometry *g, const void *U_canonical_dev, cudaStream_t st);
+// row0, nrow_c: lattice lines (rows) covered, nrow_c < 0 = the whole field; canonical_dev points at the first site of the range
 int launch_import(const dwf_geometry *g, const void *canonical_dev, int parity, void *field,
-                  cudaStream_t st);
+                  cudaStream_t st, long long row0 = 0, long long nrow_c = -1);
 int launch_export(const dwf_geometry *g, const void *field, int parity, void *canonical_dev,
-                  cudaStream_t st);
+                  cudaStream_t st, long long row0 = 0, long long nrow_c = -1);
 // dhop.cu (direct kernel; half fields only)
 int launch_dhop_direct(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st,
                        bool dagger = false, const void *axpy_x = nullptr, double axpy_a = 0.0, double axpy_b = 0.0);

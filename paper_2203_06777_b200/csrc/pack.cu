@@ -29,13 +29,15 @@ namespace dwf {
 // FULL = false: canonical sites are the cb sites of one parity, the device field is [s][row][k/2][h][k&1]
 template <typename T, bool IMPORT, bool FULL>
 __global__ void __launch_bounds__(256)
-spinor_reorder_kernel(const T *__restrict__ src, T *__restrict__ dst, const Lattice lat)
+spinor_reorder_kernel(const T *__restrict__ src, T *__restrict__ dst, const Lattice lat, const long long row0, const long long nrow_c)
 {
-    // one thread per complex element of the DEVICE layout (coalesced on the device side)
+    // one thread per complex element of the DEVICE layout (coalesced on the device side).  The call covers
+    // the lattice lines row0 .. row0 + nrow_c - 1; the canonical pointer (src on import, dst on export) is
+    // RELATIVE to the first site of that range (chunked host transfers, api.cu)
     using V = typename std::conditional<sizeof(T) == 4, float2, double2>::type;
     const long long Vh = lat.Vh;
     const long long nrow = Vh / lat.Lh;
-    const long long n = (FULL ? 2 : 1) * Vh * lat.Ls * 12;
+    const long long n = (FULL ? 2 : 1) * nrow_c * lat.Lh * lat.Ls * 12;
     for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n;
          e += (long long)gridDim.x * blockDim.x) {
         // fp32 device element e = ((((par*Ls + s)*nrow + row)*6 + k/2)*Lh + h)*2 + (k&1)
@@ -50,10 +52,11 @@ spinor_reorder_kernel(const T *__restrict__ src, T *__restrict__ dst, const Latt
             h = (int)(r % lat.Lh); r /= lat.Lh;
             k = (int)(r % 12); r /= 12;
         }
-        const long long row = r % nrow; r /= nrow;
+        const long long rowc = r % nrow_c; r /= nrow_c;
+        const long long row = row0 + rowc;
         const int s = (int)(r % lat.Ls);
         const int par = (int)(r / lat.Ls);
-        const long long cb = row * lat.Lh + h;
+        const long long cb = rowc * lat.Lh + h;          // canonical site, relative to the chunk
         long long site = cb;
         if (FULL) {
             // lexicographic x of cb site `cb` of parity `par`: x0 = 2*h + ((x1+x2+x3+par)&1)
@@ -65,16 +68,18 @@ spinor_reorder_kernel(const T *__restrict__ src, T *__restrict__ dst, const Latt
         }
         if constexpr (sizeof(T) == 8) {
             const long long c = ((site * lat.Ls + s) * 12 + k);     // canonical complex index
-            if (IMPORT) reinterpret_cast<V *>(dst)[e] = reinterpret_cast<const V *>(src)[c];
-            else        reinterpret_cast<V *>(dst)[c] = reinterpret_cast<const V *>(src)[e];
+            const long long d = ((((long long)par * lat.Ls + s) * nrow + row) * 12 + k) * lat.Lh + h;   // device complex index
+            if (IMPORT) reinterpret_cast<V *>(dst)[d] = reinterpret_cast<const V *>(src)[c];
+            else        reinterpret_cast<V *>(dst)[c] = reinterpret_cast<const V *>(src)[d];
         } else {
             // fp32: slot k = 4*colour + t holds the spin pair (2*(t/2), 2*(t/2)+1) of one real part:
             // t = 0 (re of spins 0,1), 1 (im of 0,1), 2 (re of 2,3), 3 (im of 2,3)
             const int col = k >> 2, t = k & 3;
             const long long i0 = (((site * lat.Ls + s) * 12 + ((t >> 1) * 6 + col)) << 1) + (t & 1);   // canonical real
-            if (IMPORT) reinterpret_cast<V *>(dst)[e] = V{src[i0], src[i0 + 6]};
+            const long long d = (((((long long)par * lat.Ls + s) * nrow + row) * 6 + (k >> 1)) * lat.Lh + h) * 2 + (k & 1);
+            if (IMPORT) reinterpret_cast<V *>(dst)[d] = V{src[i0], src[i0 + 6]};
             else {
-                const V v = reinterpret_cast<const V *>(src)[e];
+                const V v = reinterpret_cast<const V *>(src)[d];
                 dst[i0] = v.x;
                 dst[i0 + 6] = v.y;
             }
@@ -87,19 +92,21 @@ spinor_reorder_kernel(const T *__restrict__ src, T *__restrict__ dst, const Latt
 // the device side (consecutive threads = consecutive h: coalesced).
 template <bool IMPORT, bool FULL>
 __global__ void __launch_bounds__(256)
-spinor_reorder_sites_kernel(const float *__restrict__ src, float *__restrict__ dst, const Lattice lat)
+spinor_reorder_sites_kernel(const float *__restrict__ src, float *__restrict__ dst, const Lattice lat, const long long row0,
+                            const long long nrow_c)
 {
     const long long Vh = lat.Vh;
     const long long nrow = Vh / lat.Lh;
-    const long long n = (FULL ? 2 : 1) * Vh * lat.Ls;
+    const long long n = (FULL ? 2 : 1) * nrow_c * lat.Lh * lat.Ls;
     for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n;
          e += (long long)gridDim.x * blockDim.x) {
         long long r = e;
         const int h = (int)(r % lat.Lh); r /= lat.Lh;
-        const long long row = r % nrow; r /= nrow;
+        const long long rowc = r % nrow_c; r /= nrow_c;
+        const long long row = row0 + rowc;
         const int s = (int)(r % lat.Ls);
         const int par = (int)(r / lat.Ls);
-        const long long cb = row * lat.Lh + h;
+        const long long cb = rowc * lat.Lh + h;          // canonical site, relative to the chunk
         long long site = cb;
         if (FULL) {
             long long q = row;
@@ -223,34 +230,40 @@ int launch_pack_gauge(const dwf_geometry *g, const void *U_dev, cudaStream_t st)
 }
 
 template <bool IMPORT>
-static int launch_reorder(const dwf_geometry *g, const void *src, void *dst, int parity, cudaStream_t st)
+static int launch_reorder(const dwf_geometry *g, const void *src, void *dst, int parity, cudaStream_t st, long long row0,
+                          long long nrow_c)
 {
     const bool full = parity == DWF_FULL;
-    const int grid = grid_for((full ? 2 : 1) * g->lat.Vh * g->lat.Ls * 12, g->sm_count);
+    if (nrow_c < 0) { row0 = 0; nrow_c = g->lat.Vh / g->lat.Lh; }
+    const long long nsite = (full ? 2 : 1) * nrow_c * g->lat.Lh * g->lat.Ls;
+    const int grid = grid_for(nsite * 12, g->sm_count);
     if (g->prec == DWF_F32) {
         auto *a = static_cast<const float *>(src);
         auto *b = static_cast<float *>(dst);
-        const int gs = grid_for((full ? 2 : 1) * g->lat.Vh * g->lat.Ls, g->sm_count);
-        if (full) spinor_reorder_sites_kernel<IMPORT, true><<<gs, 256, 0, st>>>(a, b, g->lat);
-        else      spinor_reorder_sites_kernel<IMPORT, false><<<gs, 256, 0, st>>>(a, b, g->lat);
+        const int gs = grid_for(nsite, g->sm_count);
+        if (full) spinor_reorder_sites_kernel<IMPORT, true><<<gs, 256, 0, st>>>(a, b, g->lat, row0, nrow_c);
+        else      spinor_reorder_sites_kernel<IMPORT, false><<<gs, 256, 0, st>>>(a, b, g->lat, row0, nrow_c);
     } else {
         auto *a = static_cast<const double *>(src);
         auto *b = static_cast<double *>(dst);
-        if (full) spinor_reorder_kernel<double, IMPORT, true><<<grid, 256, 0, st>>>(a, b, g->lat);
-        else      spinor_reorder_kernel<double, IMPORT, false><<<grid, 256, 0, st>>>(a, b, g->lat);
+        if (full) spinor_reorder_kernel<double, IMPORT, true><<<grid, 256, 0, st>>>(a, b, g->lat, row0, nrow_c);
+        else      spinor_reorder_kernel<double, IMPORT, false><<<grid, 256, 0, st>>>(a, b, g->lat, row0, nrow_c);
     }
     count_launch();
     DWF_CUDA_CHECK(cudaGetLastError());
     return DWF_OK;
 }
 
-int launch_import(const dwf_geometry *g, const void *canonical_dev, int parity, void *field, cudaStream_t st)
+// row0, nrow_c: the lattice lines covered (nrow_c < 0: all); the canonical pointer is relative to the first site of the range
+int launch_import(const dwf_geometry *g, const void *canonical_dev, int parity, void *field, cudaStream_t st, long long row0,
+                  long long nrow_c)
 {
-    return launch_reorder<true>(g, canonical_dev, field, parity, st);
+    return launch_reorder<true>(g, canonical_dev, field, parity, st, row0, nrow_c);
 }
-int launch_export(const dwf_geometry *g, const void *field, int parity, void *canonical_dev, cudaStream_t st)
+int launch_export(const dwf_geometry *g, const void *field, int parity, void *canonical_dev, cudaStream_t st, long long row0,
+                  long long nrow_c)
 {
-    return launch_reorder<false>(g, field, canonical_dev, parity, st);
+    return launch_reorder<false>(g, field, canonical_dev, parity, st, row0, nrow_c);
 }
 
 // out = a x + b out over nreal reals (128-bit vectors; nreal is a multiple of 24).  The unfused path of
