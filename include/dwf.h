@@ -68,8 +68,17 @@ enum { DWF_FULL = -1, DWF_EVEN = 0, DWF_ODD = 1 };   /* parity = (x0+x1+x2+x3) &
 /* Create a geometry: lattice extents dims[4] (each even and >= 2), fifth-dimension extent Ls >= 1,
  * precision DWF_F32 / DWF_F64 (storage AND arithmetic; no mixed precision), bc_time, CUDA device
  * ordinal.  Allocates the device gauge storage and reduction scratch (owned by the geometry).
- * Errors: INVALID_ARG (NULL), BAD_GEOMETRY (odd or < 2 extent, Ls < 1, field too large),
- * UNSUPPORTED (precision), CUDA / ALLOC. */
+ * Errors: INVALID_ARG (NULL), BAD_GEOMETRY (odd or < 2 extent, Ls < 1, field too large: a full 5D field is
+ * limited to 2^31 - 1 complex numbers, i.e. V4 * Ls * 12 < 2^31 -- C5 has 1.5e9 -- and V4 to 2^30 sites),
+ * UNSUPPORTED (precision), CUDA / ALLOC.
+ *
+ * CONCURRENCY.  dwf_dhop, dwf_dhop_oe/eo, their _dag, _axpy and _mrhs forms, dwf_mooee, dwf_mooee_inv, dwf_ddwf,
+ * dwf_schur and dwf_axpby only read the geometry: they may be called concurrently on different streams.
+ * Calls that use the geometry's scratch -- dwf_norm2, dwf_inner_product, dwf_dhop_oe_norm2 / _eo_norm2,
+ * dwf_cg_schur (reduction partials and the result mailbox), dwf_import_spinor / dwf_export_spinor with HOST
+ * arrays and dwf_host_wait (the transfer ring) -- must be serialised by the caller per geometry (one at a
+ * time; they may overlap with the read-only calls).  dwf_load_gauge, dwf_set_option and dwf_destroy_geometry
+ * must not race with anything on the same geometry. */
 DWF_API int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, int cuda_device,
                         dwf_geometry **out);
 
@@ -232,10 +241,8 @@ DWF_API int dwf_kernel_info(const dwf_geometry *g, char *buf, size_t n);
  *   "layered"        1: one TMA box per x3 layer, so that L2 policies can differ per layer
  *   "l2pol"          decimal digits, one L2 eviction class per access type (dhop_staged.cu PC_*):
  *                    0 evict_normal, 1 evict_first, 2 evict_last
- *   "prefetch"       low 4 bits: L2 prefetch distance in steps (0 off), higher bits: box mask
  *   "async_host"     1: dwf_import_spinor / dwf_export_spinor with host arrays return without synchronising
  *                    (pipelined steps; dwf_host_wait before touching the host arrays)
- *   "l2persist"      MB of L2 set aside for evict_last lines (device-wide CUDA limit)
  *   "raster", "tile0".."tile3", "cpc"   direct kernel: CTA launch order, log2 tile extents, slices per CTA */
 DWF_API int dwf_set_option(dwf_geometry *g, const char *key, long long value);
 

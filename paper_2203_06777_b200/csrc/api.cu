@@ -325,7 +325,6 @@ int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, i
     g->opt_l2pol = 11222222;     // out, links evict_first; every input box evict_last (sweeps: least DRAM re-reads)
     g->opt_ssplit = 1;
     g->opt_zigzag = 1;
-    g->opt_prefetch = 0;
     g->opt_layered = 1;
 
     g->gauge_bytes = (size_t)8 * 18 * (size_t)g->lat.Vh * (size_t)precision;
@@ -390,17 +389,6 @@ int dwf_set_option(dwf_geometry *g, const char *key, long long value)
         return DWF_OK;
     } else if (!strcmp(key, "layered")) {
         g->opt_layered = v != 0;
-        return DWF_OK;
-    } else if (!strcmp(key, "prefetch")) {
-        g->opt_prefetch = v;
-        return DWF_OK;
-    } else if (!strcmp(key, "l2persist")) {
-        // MB of L2 set aside for evict_last ("persisting") lines; device-wide CUDA limit
-        int maxb = 0;
-        DWF_CUDA_CHECK(cudaDeviceGetAttribute(&maxb, cudaDevAttrMaxPersistingL2CacheSize, g->device));
-        size_t want = (size_t)(v < 0 ? 0 : v) << 20;
-        if (want > (size_t)maxb) want = (size_t)maxb;
-        DWF_CUDA_CHECK(cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want));
         return DWF_OK;
     } else if (!strcmp(key, "ssplit")) {
         if (v < 1) { set_error("ssplit must be >= 1"); return DWF_ERR_INVALID_ARG; }

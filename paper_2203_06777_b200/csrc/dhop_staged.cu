@@ -77,7 +77,6 @@ struct StagedArgs {
     int l2pol;               // decimal digits, see PC_*
     int zigzag;              // walk the slices of every other tile backwards
     int layered;             // one TMA box per x3 layer (per-layer L2 policies) instead of one per region
-    int prefetch;            // producer prefetches the input of step g + prefetch into L2 (0: off); bit 4..: box mask
     float axpy_a, axpy_b;    // AXPY kernels: out = a x + b Dhop in
     double *norm_partials;   // NORM kernels: one partial sum of |out|^2 per CTA (fixed order inside the CTA)
 };
@@ -282,21 +281,8 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             b.c3m = sb + (o.z == 0 ? L3 - 1 : o.z - 1); b.c3p = sb + (o.z + B3 == L3 ? 0 : o.z + B3);
             return b;
         };
-        const int pfd = args.prefetch & 15, pfm = args.prefetch >> 4;
         for (int g = 0; g < nsteps; g++) {
             const int stage = g & 1;
-            if (pfd && g + pfd < nsteps) {       // DRAM -> L2 runs ahead of the shared-memory ring
-                const Boxes p = boxes(g + pfd);
-                if (pfm & 1) tma_prefetch_5d(&map_c, 0, 0, p.o1, p.o2, p.c4);
-                if (pfm & 2) tma_prefetch_5d(&map_x3, 0, 0, p.o1, p.o2, p.c3p);
-                if (pfm & 4) tma_prefetch_5d(&map_x3, 0, 0, p.o1, p.o2, p.c3m);
-                if (pfm & 8) {
-                    tma_prefetch_5d(&map_x1, 0, 0, p.x1m, p.o2, p.c4);
-                    tma_prefetch_5d(&map_x1, 0, 0, p.x1p, p.o2, p.c4);
-                    tma_prefetch_5d(&map_x2, 0, 0, p.o1, p.x2m, p.c4);
-                    tma_prefetch_5d(&map_x2, 0, 0, p.o1, p.x2p, p.c4);
-                }
-            }
             const Boxes b = boxes(g);
             const uint32_t dst = smem_base + stage * STAGE;
             const uint32_t fb = full_base + 32 * stage, eb = empty_base + 32 * stage;
@@ -715,7 +701,6 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     a.parity_out = parity_out;
     a.l2pol = g->opt_l2pol;
     a.zigzag = g->opt_zigzag;
-    a.prefetch = g->opt_prefetch;
     a.layered = g->opt_layered;
     a.norm_partials = norm_partials;
     a.axpy_a = axpy_a;

@@ -122,7 +122,6 @@ struct dwf_geometry {
     int opt_ssplit;         // staged kernel: CTAs sharing one tile (each takes Ls / ssplit slices)
     int opt_zigzag;         // staged kernel: walk the slices of every other tile backwards
     int opt_layered;        // staged kernel: one TMA box per x3 layer, so that L2 policies can differ per layer
-    int opt_prefetch;       // staged kernel: L2 prefetch distance (low 4 bits, steps) and box mask (bits 4..)
 };
 
 namespace dwf {

@@ -80,17 +80,6 @@ __device__ __forceinline__ void tma_load_5d_hint(uint32_t dst, const CUtensorMap
         "[%0], [%1, {%3, %4, %5, %6, %7}], [%2], %8;" ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2),
         "r"(c3), "r"(c4), "l"(policy) : "memory");
 }
-// prefetch of the same box into L2 only (no shared-memory destination, no completion signal)
-__device__ __forceinline__ void tma_prefetch_5d(const CUtensorMap *map, int c0, int c1, int c2, int c3, int c4)
-{
-    asm volatile("cp.async.bulk.prefetch.tensor.5d.L2.global.tile [%0, {%1, %2, %3, %4, %5}];" ::"l"(map), "r"(c0),
-                 "r"(c1), "r"(c2), "r"(c3), "r"(c4) : "memory");
-}
-// prefetch of a contiguous global range into L2 (size: multiple of 16 bytes)
-__device__ __forceinline__ void bulk_prefetch_l2(const void *p, uint32_t bytes)
-{
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
-}
 // L2 eviction-priority policies: 0 evict_normal, 1 evict_first, 2 evict_last
 __device__ __forceinline__ uint64_t l2_policy(int kind)
 {

@@ -107,13 +107,13 @@ def test_staged_other_row_lengths(lib, dims, Ls, bc):
 OPTION_SETS = [
     {"variant": 2}, {"variant": 3}, {"variant": 12}, {"variant": 13}, {"variant": 14}, {"variant": 15},
     {"raster_staged": 0}, {"raster_staged": 1}, {"raster_staged": 3}, {"raster_staged": 11}, {"raster_staged": 21}, {"raster_staged": 31},
-    {"zigzag": 0}, {"ssplit": 2}, {"ssplit": 4}, {"layered": 0}, {"prefetch": 17}, {"prefetch": 242},
+    {"zigzag": 0}, {"ssplit": 2}, {"ssplit": 4}, {"layered": 0},
     {"l2pol": 0}, {"l2pol": 11212020},
 ]
 
 
 def test_staged_tunables_do_not_change_the_result(lib):
-    """Tile shape, launch order, slice split, L2 policies and prefetch only move work around: the
+    """Tile shape, launch order, slice split, L2 policies only move work around: the
     arithmetic per output site is the same, so the results must be bit-identical; the direct
     kernel (kernel=1) sums the legs in another order and is held to the parity bar instead."""
     import torch
@@ -126,7 +126,7 @@ def test_staged_tunables_do_not_change_the_result(lib):
         fin = g.import_spinor(half, lib.EVEN)
         ref = g.dhop_oe(fin).clone()
         assert rel_err(g.export_spinor(ref, lib.ODD), want) <= TOL[prec]
-        defaults = {"variant": 0, "raster_staged": -1, "zigzag": 1, "ssplit": 1, "layered": 1, "prefetch": 0,
+        defaults = {"variant": 0, "raster_staged": -1, "zigzag": 1, "ssplit": 1, "layered": 1,
                     "l2pol": 11222222}
         for opts in OPTION_SETS:
             for k, v in {**defaults, **opts}.items():
