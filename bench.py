@@ -57,6 +57,8 @@ WORKLOADS = {
     "tiny": dict(dims=(8, 8, 8, 8), Ls=8, prec=4, bc=1, gauge="random", seed=1002),
     # the Schur complement of the red-black Shamir DWF operator on the C4 shape
     "schur": dict(dims=(32, 32, 32, 32), Ls=16, prec=4, bc=0, gauge="near_unit", seed=1004, kind="schur"),
+    # 12-real link storage (third row rebuilt in the kernel), C4 shape
+    "c4g12": dict(dims=(32, 32, 32, 32), Ls=16, prec=4, bc=0, gauge="near_unit", seed=1004, gauge12=1),
     # four right-hand sides sharing one gauge load, C4 shape
     "c4m4": dict(dims=(32, 32, 32, 32), Ls=16, prec=4, bc=0, gauge="near_unit", seed=1004, kind="mrhs", nrhs=4),
     "schurd": dict(dims=(32, 32, 32, 32), Ls=16, prec=8, bc=0, gauge="near_unit", seed=1004, kind="schur"),
@@ -66,7 +68,8 @@ WORKLOADS = {
 def workload_name(w):
     d = w["dims"]
     return (f"DWF even/odd Dhop {d[0]}x{d[1]}x{d[2]}x{d[3]} x Ls={w['Ls']} complex "
-            f"fp{w['prec'] * 8}, {w['gauge']} SU(3) gauge, DhopOE then DhopEO then norm2")
+            f"fp{w['prec'] * 8}, {w['gauge']} SU(3) gauge" + (", 12-real link storage for the plain DhopOE" if w.get("gauge12") else "") +
+            ", DhopOE then DhopEO then norm2")
 
 
 def model_bytes_cb(w):
@@ -74,7 +77,8 @@ def model_bytes_cb(w):
     output site, the whole gauge field once."""
     d = w["dims"]
     V4 = d[0] * d[1] * d[2] * d[3]
-    return (V4 // 2) * w["Ls"] * 48 * w["prec"] + V4 * 72 * w["prec"]
+    link_reals = 48 if w.get("gauge12") else 72            # 12-real storage: two rows of every link
+    return (V4 // 2) * w["Ls"] * 48 * w["prec"] + V4 * link_reals * w["prec"]
 
 
 def make_inputs(w):
@@ -294,6 +298,8 @@ def run_gpu(args, w):
     for kv in args.opt or []:
         k, v = kv.split("=")
         g.set_option(k, int(v))
+    if w.get("gauge12"):
+        g.set_option("gauge12", 1)
     g.load_gauge(U)
     f_in = g.import_spinor(psi_e, dwf.EVEN)
     f_mid, f_out = g.new_field(dwf.ODD), g.new_field(dwf.EVEN)

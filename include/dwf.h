@@ -241,6 +241,13 @@ DWF_API int dwf_kernel_info(const dwf_geometry *g, char *buf, size_t n);
  *   "layered"        1: one TMA box per x3 layer, so that L2 policies can differ per layer
  *   "l2pol"          decimal digits, one L2 eviction class per access type (dhop_staged.cu PC_*):
  *                    0 evict_normal, 1 evict_first, 2 evict_last
+ *   "gauge12"        1: 12-real link storage (fp32 only): the NEXT dwf_load_gauge also keeps a copy
+ *                    with rows 0, 1 of every link only, and dwf_dhop / dwf_dhop_oe / dwf_dhop_eo (the plain calls, on
+ *                    geometries with a staged variant) read that copy and rebuild row 2 = conj(row0 x row1) once
+ *                    per tile: 96 instead of 144 link bytes per 4D site and parity, model w (48 + 96/Ls) B per output
+ *                    site.  The links must be SU(3) matrices; the result is the Dhop of the links with the rebuilt
+ *                    third row (differs from the 18-real result by fp32 roundings of that row).  Until the reload
+ *                    Dhop calls return NO_GAUGE.  UNSUPPORTED on fp64 geometries.
  *   "async_host"     1: dwf_import_spinor / dwf_export_spinor with host arrays return without synchronising
  *                    (pipelined steps; dwf_host_wait before touching the host arrays)
  *   "raster", "tile0".."tile3", "cpc"   direct kernel: CTA launch order, log2 tile extents, slices per CTA */

@@ -184,6 +184,19 @@ def inner(a: np.ndarray, b: np.ndarray) -> complex:
     return complex(out[0], out[1])
 
 
+def reconstruct12(U: np.ndarray) -> np.ndarray:
+    """SURVEY.md 8(f4), 12-real link storage: the links an SU(3)-compressed path works with.  Rows 0 and 1 of
+    every U_mu(x) are kept (promoted exactly to fp64), row 2 is REPLACED by conj(row0 x row1) -- for a matrix of
+    SU(3) that is its own third row (unitarity + det = 1), for the fp32-rounded links of the inputs it differs
+    from the stored third row at the 1e-7 level.  Plain numpy, fp64 out, shape of U."""
+    Uc = U.astype(np.float64)
+    z = Uc[..., 0] + 1j * Uc[..., 1]                     # (..., 3, 3) complex, row a, column b
+    r0, r1 = z[..., 0, :], z[..., 1, :]
+    r2 = np.conj(np.cross(r0, r1))
+    out = np.stack([r0, r1, r2], axis=-2)
+    return np.ascontiguousarray(np.stack([out.real, out.imag], axis=-1))
+
+
 # ---------------------------------------------------------------------------------------------
 # SURVEY.md 8(f2): the rest of the red-black Shamir domain-wall operator (dwf5d_oracle.c)
 # ---------------------------------------------------------------------------------------------

@@ -352,6 +352,8 @@ int dwf_destroy_geometry(dwf_geometry *g)
     DeviceGuard guard(g->device);
     cudaFree(g->gauge[0]);
     cudaFree(g->gauge[1]);
+    cudaFree(g->gauge12[0]);
+    cudaFree(g->gauge12[1]);
     cudaFree(g->partials);
     cudaFree(g->result_dev);
     cudaFreeHost(g->mailbox_host);
@@ -394,6 +396,11 @@ int dwf_set_option(dwf_geometry *g, const char *key, long long value)
         if (v < 1) { set_error("ssplit must be >= 1"); return DWF_ERR_INVALID_ARG; }
         g->opt_ssplit = v;
         return DWF_OK;
+    } else if (!strcmp(key, "gauge12")) {
+        if (v && g->prec != DWF_F32) { set_error("gauge12 needs an fp32 geometry"); return DWF_ERR_UNSUPPORTED; }
+        g->opt_gauge12 = v != 0;
+        if (g->opt_gauge12 && !g->gauge12[0]) g->gauge_loaded = false;        // takes effect at the next dwf_load_gauge
+        return DWF_OK;
     } else if (!strcmp(key, "async_host")) {
         g->opt_async_host = v != 0;
         return DWF_OK;
@@ -430,6 +437,13 @@ int dwf_load_gauge(dwf_geometry *g, const void *U, int src_is_device, void *stre
         src = tmp;
     }
     int rc = launch_pack_gauge(g, src, st);
+    if (!rc && g->opt_gauge12) {
+        // the compressed copy (two thirds of the bytes) next to the full one: only the plain staged fp32 Dhop reads it
+        const size_t b12 = g->gauge_bytes / 3 * 2;
+        for (int p = 0; p < 2 && !rc; p++)
+            if (!g->gauge12[p] && cudaMalloc(&g->gauge12[p], b12) != cudaSuccess) { cudaGetLastError(); set_error("cannot allocate the 12-real gauge copy"); rc = DWF_ERR_ALLOC; }
+        if (!rc) rc = launch_compress_gauge12(g, st);
+    }
     cudaError_t e = cudaStreamSynchronize(st);
     if (tmp) cudaFree(tmp);
     if (rc) return rc;
@@ -456,7 +470,8 @@ int dwf::half_dhop(const dwf_geometry *g, const void *in, void *out, int parity_
         return DWF_ERR_UNSUPPORTED;
     }
     if (staged_ok && g->opt_kernel != 1)
-        return launch_dhop_staged(g, in, out, parity_out, st, nullptr, nullptr, dagger, axpy_x, (float)a, (float)b, nrhs);
+        return launch_dhop_staged(g, in, out, parity_out, st, nullptr, nullptr, dagger, axpy_x, (float)a, (float)b, nrhs,
+                                  g->opt_gauge12 && g->gauge12[0] && !dagger && !axpy_x);
     if (staged_two_pass && g->opt_kernel != 1) {
         int rc = launch_dhop_staged(g, in, out, parity_out, st, nullptr, nullptr, dagger, nullptr, 0.f, 0.f, nrhs);
         if (rc) return rc;

@@ -74,6 +74,7 @@ struct StagedArgs {
     int L1, L2, L3, Ls;
     int ssplit;              // CTAs sharing one tile, each walking Ls / ssplit slices
     int parity_out;
+    int bc_time;             // G12 kernels: antiperiodic time (the folded sign of a wrapping link reappears in its rebuilt third row)
     int l2pol;               // decimal digits, see PC_*
     int zigzag;              // walk the slices of every other tile backwards
     int layered;             // one TMA box per x3 layer (per-layer L2 policies) instead of one per region
@@ -205,7 +206,9 @@ __device__ __forceinline__ void staged_leg(float2 (&acc)[12], const float4 *__re
 // links and neighbours.  MODE 3 (AXPY): out = a x + b Dhop in, with x a field of the
 // output parity staged by TMA next to the input slice and combined in the store epilogue (the
 // Wilson-matrix fusion of SURVEY.md 8(f1): one pass instead of Dhop followed by an axpy).  MODE 4: the
-// same with Dhop^dagger (the last kernel of the adjoint Schur complement).
+// same with Dhop^dagger (the last kernel of the adjoint Schur complement).  MODE 5 (G12): Dhop
+// with 12-real links: only rows 0, 1 of every link are read (24 instead of 36 vectors per
+// site); row 2 = conj(row0 x row1) is rebuilt in registers once per tile, so the arithmetic of a step is unchanged.
 template <int LH, int B1, int B2, int B3, int MODE>
 __global__ void __launch_bounds__(StagedCfg<LH, B1, B2, B3>::NT, StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM)
 dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_x1,
@@ -214,7 +217,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
                    const __grid_constant__ CUtensorMap map_xc, const StagedArgs args)
 {
     using Cfg = StagedCfg<LH, B1, B2, B3>;
-    constexpr bool NORM = MODE == 1, DAG = MODE == 2 || MODE == 4, AXPY = MODE == 3 || MODE == 4;
+    constexpr bool NORM = MODE == 1, DAG = MODE == 2 || MODE == 4, AXPY = MODE == 3 || MODE == 4, G12 = MODE == 5;
     // MODE 3 stages the rows box of the field x as well (read in the epilogue): NROW_C more rows per stage
     constexpr int STAGE = Cfg::STAGE_BYTES + (AXPY ? Cfg::NROW_C * Cfg::ROWB : 0);
     extern __shared__ __align__(1024) unsigned char smem[];
@@ -383,13 +386,42 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     long long grow = tile_row(0, r_cur);
     set_x0_offsets(r_cur);
     float4 *optr = reinterpret_cast<float4 *>(args.out) + grow * (6 * LH) + h + (long long)s_first * slice_vecs;
-    if (active) {
-        const float4 *gp = reinterpret_cast<const float4 *>(args.gauge) + grow * (36 * LH) + h;
+    // G12: vector 3L + v of a site holds the complex numbers 2v, 2v+1 of rows 0, 1 of leg L (row-major), i.e. U[9L + 2v], U[9L + 2v + 1]
+    constexpr int GV = G12 ? 24 : 36;                // 128-bit link vectors per site
+    // row 2 of every link from rows 0, 1: r2 = sgn conj(r0 x r1); sgn = -1 for a time link whose hop wraps around an
+    // antiperiodic lattice (its stored rows carry the folded -1, and (-r0) x (-r1) = r0 x r1)
+    auto rebuild_rows = [&](int x3) {
 #pragma unroll
-        for (int j = 0; j < 36; j++) {
-            const float4 q = ldg128_hint(gp + j * LH, pol_g);
-            U[2 * j] = make_float2(q.x, q.y);
-            U[2 * j + 1] = make_float2(q.z, q.w);
+        for (int L = 0; L < 8; L++) {
+            const float2 *r0 = U + 9 * L, *r1 = U + 9 * L + 3;
+            const bool flip = args.bc_time && ((L == 6 && x3 == args.L3 - 1) || (L == 7 && x3 == 0));
+            const float sg = flip ? -1.f : 1.f;
+#pragma unroll
+            for (int k = 0; k < 3; k++) {
+                const int i = (k + 1) % 3, j = (k + 2) % 3;
+                const float re = (r0[i].x * r1[j].x - r0[i].y * r1[j].y) - (r0[j].x * r1[i].x - r0[j].y * r1[i].y);
+                const float im = (r0[i].x * r1[j].y + r0[i].y * r1[j].x) - (r0[j].x * r1[i].y + r0[j].y * r1[i].x);
+                U[9 * L + 6 + k] = make_float2(sg * re, -sg * im);
+            }
+        }
+    };
+    if (active) {
+        const float4 *gp = reinterpret_cast<const float4 *>(args.gauge) + grow * (GV * LH) + h;
+        if constexpr (G12) {
+#pragma unroll
+            for (int j = 0; j < 24; j++) {
+                const float4 q = ldg128_hint(gp + j * LH, pol_g);
+                U[9 * (j / 3) + 2 * (j % 3)] = make_float2(q.x, q.y);
+                U[9 * (j / 3) + 2 * (j % 3) + 1] = make_float2(q.z, q.w);
+            }
+            rebuild_rows(tile_origin(0).z + i3);
+        } else {
+#pragma unroll
+            for (int j = 0; j < 36; j++) {
+                const float4 q = ldg128_hint(gp + j * LH, pol_g);
+                U[2 * j] = make_float2(q.x, q.y);
+                U[2 * j + 1] = make_float2(q.z, q.w);
+            }
         }
     }
 
@@ -406,7 +438,13 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         float2 acc[12];
 #define DWF_LEG(L, MU, FWD, FIRST)                                                                  \
         staged_leg<LH, MU, (FWD) != DAG, FIRST>(acc, reinterpret_cast<const float4 *>(sb) + (((L) & 1) ? offp[(L) >> 1] >> 16 : offp[(L) >> 1] & 0xffffu), U + 9 * (L)); \
-        if constexpr (FETCH) {     /* refill the component pairs whose last use was this leg */     \
+        if constexpr (FETCH && G12) {   /* rows 0, 1 of this leg; row 2 is rebuilt at the tile switch */ \
+            _Pragma("unroll") for (int v = 0; v < 3; v++) {                                         \
+                const float4 q = ldg128_hint(gnext + (3 * (L) + v) * LH, pol_g);                    \
+                U[9 * (L) + 2 * v] = make_float2(q.x, q.y);                                         \
+                U[9 * (L) + 2 * v + 1] = make_float2(q.z, q.w);                                     \
+            }                                                                                       \
+        } else if constexpr (FETCH) {     /* refill the component pairs whose last use was this leg */ \
             _Pragma("unroll") for (int j = (9 * (L)) / 2; j < (9 * ((L) + 1)) / 2; j++) {            \
                 const float4 q = ldg128_hint(gnext + j * LH, pol_g);                                \
                 U[2 * j] = make_float2(q.x, q.y);                                                   \
@@ -465,7 +503,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         int r_next = r_cur;
         long long grow_next = grow;
         if (has_next) grow_next = tile_row(it + 1, r_next);
-        const float4 *gnext = reinterpret_cast<const float4 *>(args.gauge) + grow_next * (36 * LH) + h;
+        const float4 *gnext = reinterpret_cast<const float4 *>(args.gauge) + grow_next * (GV * LH) + h;
         for (int s = 0; s < nsl; s++, g++) {
             const bool fetch = has_next && s == nsl - 1;     // refill the links during the last slice
             const int stage = g & 1;
@@ -474,6 +512,9 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             else       step(std::false_type{}, stage, (g >> 1) & 1, optr + (long long)sl * slice_vecs, gnext);
         }
         // tile switch
+        if constexpr (G12) {
+            if (has_next) rebuild_rows(tile_origin(it + 1).z + i3);
+        }
         grow = grow_next;
         r_cur = r_next;
         set_x0_offsets(r_cur);
@@ -515,6 +556,7 @@ const void *const *staged_kernels_mode1();
 const void *const *staged_kernels_mode2();
 const void *const *staged_kernels_mode3();
 const void *const *staged_kernels_mode4();
+const void *const *staged_kernels_mode5();
 
 #define DWF_CAT2(a, b) a##b
 #define DWF_CAT(a, b) DWF_CAT2(a, b)
@@ -533,7 +575,7 @@ const void *const *DWF_CAT(staged_kernels_mode, DWF_STAGED_MODE)()
 struct Variant {
     int lh, b1, b2, b3;
     int smem, threads, ctas_per_sm;
-    const void *fn[5];       // MODE 0 (Dhop), 1 (Dhop + norm2), 2 (Dhop^dagger), 3 (a x + b Dhop), 4 (a x + b Dhop^dagger)
+    const void *fn[6];       // MODE 0 (Dhop), 1 (Dhop + norm2), 2 (Dhop^dagger), 3 (a x + b Dhop), 4 (a x + b Dhop^dagger), 5 (Dhop, 12-real links)
     int smem_axpy;           // MODEs 3, 4 stage the rows box of x as well
 };
 
@@ -542,10 +584,10 @@ static const std::vector<Variant> &variants()
     static const std::vector<Variant> v = [] {
         std::vector<Variant> t;
         const void *const *k0 = staged_kernels_mode0(), *const *k1 = staged_kernels_mode1(), *const *k2 = staged_kernels_mode2(),
-                          *const *k3 = staged_kernels_mode3(), *const *k4 = staged_kernels_mode4();
+                          *const *k3 = staged_kernels_mode3(), *const *k4 = staged_kernels_mode4(), *const *k5 = staged_kernels_mode5();
 #define X(LH, B1, B2, B3)                                                                            \
         t.push_back({LH, B1, B2, B3, StagedCfg<LH, B1, B2, B3>::SMEM_BYTES, StagedCfg<LH, B1, B2, B3>::NT,  \
-                     StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM, {k0[t.size()], k1[t.size()], k2[t.size()], k3[t.size()], k4[t.size()]},    \
+                     StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM, {k0[t.size()], k1[t.size()], k2[t.size()], k3[t.size()], k4[t.size()], k5[t.size()]},    \
                      StagedCfg<LH, B1, B2, B3>::SMEM_BYTES + 2 * StagedCfg<LH, B1, B2, B3>::NROW_C * StagedCfg<LH, B1, B2, B3>::ROWB});
         DWF_STAGED_VARIANTS(X)
 #undef X
@@ -571,8 +613,8 @@ void plan_staged(dwf_geometry *g)
         g->staged.ntiles = (lat.L[1] / v[i].b1) * (lat.L[2] / v[i].b2) * (lat.L[3] / v[i].b3);
         // Opt in to the large dynamic shared memory here, on the geometry's device (the attribute is per
         // device; the caller holds a DeviceGuard), for every kernel MODE of the chosen tile shape.
-        for (int mode = 0; mode < 5; mode++) {
-            const int smem = mode >= 3 ? v[i].smem_axpy : v[i].smem;
+        for (int mode = 0; mode < 6; mode++) {
+            const int smem = (mode == 3 || mode == 4) ? v[i].smem_axpy : v[i].smem;
             if (smem > SMEM_LIMIT) continue;
             if (cudaFuncSetAttribute(v[i].fn[mode], cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) {
                 cudaGetLastError();
@@ -667,7 +709,7 @@ bool staged_supports_axpy(const dwf_geometry *g)
 
 int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st,
                        double *norm_partials, int *norm_blocks, bool dagger, const void *axpy_x, float axpy_a,
-                       float axpy_b, int nrhs)
+                       float axpy_b, int nrhs, bool gauge12)
 {
     // nrhs > 1: `in`, `out` (and x) hold nrhs fields one after the other.  Dhop is diagonal
     // in s, so they are ONE field of nrhs * Ls slices to this kernel: the links of a tile stay in registers
@@ -678,8 +720,9 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
         return DWF_ERR_UNSUPPORTED;
     }
     const Variant &v = variants()[(size_t)g->staged.variant];
-    const int mode = norm_partials ? 1 : (axpy_x ? (dagger ? 4 : 3) : (dagger ? 2 : 0));
-    const int smem = mode >= 3 ? v.smem_axpy : v.smem;
+    if (gauge12 && (norm_partials || dagger || axpy_x)) { set_error("12-real links: plain Dhop only"); return DWF_ERR_UNSUPPORTED; }
+    const int mode = gauge12 ? 5 : norm_partials ? 1 : (axpy_x ? (dagger ? 4 : 3) : (dagger ? 2 : 0));
+    const int smem = (mode == 3 || mode == 4) ? v.smem_axpy : v.smem;
     if (smem > SMEM_LIMIT) { set_error("tile too large for the fused axpy"); return DWF_ERR_UNSUPPORTED; }
     // The cache hands out pointers into its slots and the second lookup may evict the slot of the
     // first, so the maps are copied before it (they are passed to the kernel by value anyway).
@@ -694,7 +737,8 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     }
     StagedArgs a;
     a.out = static_cast<float2 *>(out);
-    a.gauge = static_cast<const float2 *>(g->gauge[parity_out]);
+    a.gauge = static_cast<const float2 *>(gauge12 ? g->gauge12[parity_out] : g->gauge[parity_out]);
+    a.bc_time = g->bc_time == DWF_ANTIPERIODIC_T;
     a.tiles = g->tiles_staged;
     a.ntiles = g->staged.ntiles;
     a.L1 = g->lat.L[1]; a.L2 = g->lat.L[2]; a.L3 = g->lat.L[3]; a.Ls = ls;

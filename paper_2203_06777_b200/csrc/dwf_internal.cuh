@@ -73,6 +73,9 @@ struct dwf_geometry {
     // planar over sites: [leg][18 reals in 128-bit vectors][cb site]; leg = 2*mu + (0: fwd, 1: bwd)
     void *gauge[2];
     size_t gauge_bytes;     // per parity
+    // option "gauge12": rows 0, 1 of every link only (12 reals), [row][24 vectors][Lh]; fp32, used by the plain staged Dhop
+    void *gauge12[2];
+    int opt_gauge12;
     // direct kernel: CTA tile table (origins in rasterised launch order)
     dwf::Tiling tiling_cb;
     int4 *tiles_cb;
@@ -152,6 +155,7 @@ int fetch_reduction(const dwf_geometry *g, cudaStream_t st, int n, double *out);
 
 // pack.cu
 int launch_pack_gauge(const dwf_geometry *g, const void *U_canonical_dev, cudaStream_t st);
+int launch_compress_gauge12(const dwf_geometry *g, cudaStream_t st);      // gauge[p] -> gauge12[p]
 // row0, nrow_c: lattice lines (rows) covered, nrow_c < 0 = the whole field; canonical_dev points at the first site of the range
 int launch_import(const dwf_geometry *g, const void *canonical_dev, int parity, void *field,
                   cudaStream_t st, long long row0 = 0, long long nrow_c = -1);
@@ -167,7 +171,8 @@ void build_staged_tile_table(const dwf_geometry *g, int raster, int4 *host_table
 int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st,
                        double *norm_partials = nullptr, int *norm_blocks = nullptr, bool dagger = false,
                        const void *axpy_x = nullptr, float axpy_a = 0.f, float axpy_b = 0.f,     // axpy_x: out = a x + b Dhop in
-                       int nrhs = 1);                                                           // nrhs fields one after the other
+                       int nrhs = 1,                                                            // nrhs fields one after the other
+                       bool gauge12 = false);                                                   // 12-real links (plain Dhop only)
 bool staged_supports_axpy(const dwf_geometry *g);
 // pack.cu: out = a x + b out, elementwise over nreal reals (the unfused path of dwf_dhop_*_axpy)
 int launch_axpby(const dwf_geometry *g, const void *x, void *out, double a, double b, size_t nreal, cudaStream_t st);

@@ -215,6 +215,38 @@ static int grid_for(long long n, int sm_count)
     return (int)(b < cap ? (b < 1 ? 1 : b) : cap);
 }
 
+// 12-real link storage: rows 0 and 1 of each of the 8 links of a site, taken from the packed
+// 18-real set: complex[row][f'/2][h][f'&1], f' = leg*6 + a*3 + b (a < 2).  The staged kernel rebuilds row 2 =
+// conj(row0 x row1) (times the folded boundary sign) when it loads the links of a tile.
+__global__ void __launch_bounds__(256)
+gauge_compress12_kernel(const float2 *__restrict__ full, float2 *__restrict__ c12, const long long nrow, const int Lh)
+{
+    const long long n = nrow * Lh * 48;
+    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x) {
+        // destination element e = ((row*24 + f'/2)*Lh + h)*2 + (f'&1)
+        long long r = e;
+        const int lo = (int)(r & 1); r >>= 1;
+        const int h = (int)(r % Lh); r /= Lh;
+        const int fp = 2 * (int)(r % 24) + lo;
+        const long long row = r / 24;
+        const int leg = fp / 6, ab = fp % 6;
+        const int f = leg * 9 + ab;
+        c12[e] = full[((row * 36 + (f >> 1)) * Lh + h) * 2 + (f & 1)];
+    }
+}
+
+int launch_compress_gauge12(const dwf_geometry *g, cudaStream_t st)
+{
+    const long long nrow = g->lat.Vh / g->lat.Lh;
+    for (int p = 0; p < 2; p++) {
+        gauge_compress12_kernel<<<grid_for(nrow * g->lat.Lh * 48, g->sm_count), 256, 0, st>>>(
+            static_cast<const float2 *>(g->gauge[p]), static_cast<float2 *>(g->gauge12[p]), nrow, g->lat.Lh);
+        count_launch();
+    }
+    DWF_CUDA_CHECK(cudaGetLastError());
+    return DWF_OK;
+}
+
 int launch_pack_gauge(const dwf_geometry *g, const void *U_dev, cudaStream_t st)
 {
     const int grid = grid_for(g->lat.V4 * 8, g->sm_count);

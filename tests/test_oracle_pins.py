@@ -282,3 +282,26 @@ def test_golden_fixture():
     D = dense_dhop_matrix(dims, U, True)
     assert rel_err(stored[:, 0].reshape(d.shape), apply_dense(D, psi)) < 1e-14
     assert rel_err(stored[:, 1].reshape(d.shape), apply_dense(D.conj().T, psi)) < 1e-14
+
+
+def test_reconstruct12_is_the_identity_on_su3_and_pins_the_third_row():
+    """SURVEY.md 8(f4) oracle helper: for exact SU(3) links (fp64 generator) the rebuilt third row IS the third row
+    (unitarity and det = 1 fix it); independent statement: the rebuilt matrix is unitary with determinant 1
+    (numpy.linalg), whatever the third row of the input was; rows 0, 1 are untouched bit for bit."""
+    dims = (4, 2, 4, 2)
+    U = gen.gauge_random(dims, 31, prec=8)
+    R = oracle.reconstruct12(U)
+    assert np.abs(R - U).max() <= 1e-13
+    junk = U.copy()
+    junk[..., 2, :, :] = 7.0                                  # a wrong third row is ignored and replaced
+    R2 = oracle.reconstruct12(junk)
+    assert np.array_equal(R2[..., :2, :, :], U[..., :2, :, :])
+    z = R2[..., 0] + 1j * R2[..., 1]
+    eye = np.einsum("...ab,...cb->...ac", z, z.conj())
+    assert np.abs(eye - np.eye(3)).max() <= 1e-13
+    assert np.abs(np.linalg.det(z) - 1.0).max() <= 1e-13
+    # fp32-rounded links: rows 0, 1 are the fp32 values exactly, row 2 moves by a few fp32 ulps only
+    U32 = gen.gauge_random(dims, 31, prec=4)
+    R32 = oracle.reconstruct12(U32)
+    assert R32.dtype == np.float64 and np.array_equal(R32[..., :2, :, :], U32[..., :2, :, :].astype(np.float64))
+    assert 0 < np.abs(R32 - U32).max() <= 5e-7
