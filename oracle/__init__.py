@@ -29,7 +29,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRCS = [os.path.join(_HERE, "dhop_oracle.c"), os.path.join(_HERE, "dwf5d_oracle.c")]
 _LIB = os.path.join(_HERE, "liboracle.so")
 
-PERIODIC, ANTIPERIODIC_T = 0, 1
+PERIODIC, ANTIPERIODIC_T, OPEN_T = 0, 1, 2     # OPEN_T: hops that would wrap in time contribute nothing
 EVEN, ODD = 0, 1
 
 

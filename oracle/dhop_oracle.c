@@ -168,8 +168,12 @@ static void dhop_site(const orc_ctx *c, const int x[4], int s, cplx out[4][3])
         xm[mu] = (x[mu] - 1 + c->L[mu]) % c->L[mu];
         double sp = 1.0, sm = 1.0;
         if (c->antiperiodic_t && mu == 3) {
-            if (x[3] == c->L[3] - 1) sp = -1.0;   /* forward hop wraps  */
-            if (x[3] == 0)           sm = -1.0;   /* backward hop wraps */
+            /* bc code 1: antiperiodic time, a wrapping hop gets -1.  bc code 2: OPEN time boundary (DESIGN.md
+             * reading #26): a hop that would wrap contributes nothing -- the operator of one
+             * time slab of a domain-decomposed lattice before the neighbours' faces are added. */
+            const double w = (c->antiperiodic_t == 2) ? 0.0 : -1.0;
+            if (x[3] == c->L[3] - 1) sp = w;   /* forward hop wraps  */
+            if (x[3] == 0)           sm = w;   /* backward hop wraps */
         }
         const size_t xps = lex(c->L, xp), xms = lex(c->L, xm);
         const size_t ip = c->psi_half ? (xps >> 1) : xps;

@@ -74,7 +74,8 @@ def dense_dhop_matrix(dims, U, antiperiodic_t):
         W = np.zeros((3 * V, 3 * V), dtype=complex)
         nb = shift_index(dims, mu, +1)
         for x in range(V):
-            sign = -1.0 if (antiperiodic_t and mu == 3 and c[x, 3] == dims[3] - 1) else 1.0
+            wrap = mu == 3 and c[x, 3] == dims[3] - 1
+            sign = (-1.0 if antiperiodic_t == 1 else 0.0 if antiperiodic_t == 2 else 1.0) if wrap else 1.0      # 2: open time boundary
             W[3 * x:3 * x + 3, 3 * nb[x]:3 * nb[x] + 3] += sign * Uc[x, mu]
         D += np.kron(one - g[mu], W) + np.kron(one + g[mu], W.conj().T)
     return D

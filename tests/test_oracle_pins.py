@@ -305,3 +305,43 @@ def test_reconstruct12_is_the_identity_on_su3_and_pins_the_third_row():
     R32 = oracle.reconstruct12(U32)
     assert R32.dtype == np.float64 and np.array_equal(R32[..., :2, :, :], U32[..., :2, :, :].astype(np.float64))
     assert 0 < np.abs(R32 - U32).max() <= 5e-7
+
+
+@pytest.mark.parametrize("dims", [(2, 2, 2, 2), (4, 2, 4, 2), (2, 4, 2, 6)])
+def test_open_time_boundary_against_dense_matrix_and_slab_identity(dims):
+    """SURVEY.md 8(f3) / DESIGN.md reading #26: bc code 2 drops the hops that wrap in time.  Pins: the dense
+    Kronecker matrix with the wrapping blocks of W_3 left out (full, checkerboarded, dagger); and the slab identity
+    the domain decomposition rests on: the periodic (antiperiodic) Dhop on the whole lattice, restricted to a
+    time slab, equals the open-boundary Dhop of the slab plus terms that involve ONLY the neighbouring slabs'
+    boundary layers (changing the other slab's interior does not change the difference)."""
+    Ls = 2
+    U = gen.gauge_random(dims, 17, prec=8)
+    psi = gen.spinor_gaussian(gen.volume(dims), Ls, 17, prec=8)
+    D = dense_dhop_matrix(dims, U, 2)
+    assert rel_err(oracle.dhop(dims, Ls, oracle.OPEN_T, U, psi), apply_dense(D, psi)) <= 1e-14
+    assert rel_err(oracle.dhop(dims, Ls, oracle.OPEN_T, U, psi, dagger=True), apply_dense(D.conj().T, psi)) <= 1e-14
+    par = gen.site_parity(dims)
+    full = oracle.dhop(dims, Ls, oracle.OPEN_T, U, psi)
+    for p_out in (0, 1):
+        got = oracle.dhop_cb(dims, Ls, oracle.OPEN_T, p_out, U, gen.split_parity(psi, dims, 1 - p_out))
+        assert rel_err(got, full[par == p_out]) <= 1e-14
+    if dims[3] >= 4:
+        # two slabs along time: lower = x3 < L3/2.  V4 is lexicographic with x3 slowest, so a slab is a contiguous block
+        L3h = dims[3] // 2
+        ld = dims[:3] + (L3h,)
+        nl = gen.volume(ld)
+        Ul = U.reshape(gen.volume(dims), 4, 3, 3, 2)[:nl]
+        for bc in (oracle.PERIODIC, oracle.ANTIPERIODIC_T):
+            glob = oracle.dhop(dims, Ls, bc, U, psi)[:nl]
+            loc = oracle.dhop(ld, Ls, oracle.OPEN_T, Ul, psi[:nl])
+            diff = glob - loc
+            # the difference lives on the slab's two boundary layers only ...
+            layer = gen.volume(ld[:3] + (1,))
+            assert np.abs(diff[layer:nl - layer]).max() == 0.0 if L3h > 2 else True
+            assert np.abs(diff).max() > 0.1
+            # ... and does not see the interior of the other slab
+            psi2 = psi.copy()
+            if dims[3] - L3h > 2:
+                psi2[nl + layer:-layer] = 0.0
+                glob2 = oracle.dhop(dims, Ls, bc, U, psi2)[:nl]
+                assert np.array_equal(glob2 - loc, diff)
