@@ -57,6 +57,8 @@ WORKLOADS = {
     "tiny": dict(dims=(8, 8, 8, 8), Ls=8, prec=4, bc=1, gauge="random", seed=1002),
     # the Schur complement of the red-black Shamir DWF operator on the C4 shape
     "schur": dict(dims=(32, 32, 32, 32), Ls=16, prec=4, bc=0, gauge="near_unit", seed=1004, kind="schur"),
+    # time-decomposed Dhop, every rank owns a C4-sized slab (weak scaling: global lattice 32^3 x 32 N)
+    "c4slab": dict(dims=(32, 32, 32, 32), Ls=16, prec=4, bc=1, gauge="near_unit", seed=1004, kind="slab"),
     # 12-real link storage (third row rebuilt in the kernel), C4 shape
     "c4g12": dict(dims=(32, 32, 32, 32), Ls=16, prec=4, bc=0, gauge="near_unit", seed=1004, gauge12=1),
     # four right-hand sides sharing one gauge load, C4 shape
@@ -681,6 +683,105 @@ def run_gpu_mrhs(args, w):
         dist.destroy_process_group()
 
 
+def run_gpu_slab(args, w):
+    """--workload c4slab: SURVEY.md 8(f3).  Every rank owns one time slab of `dims` (the global lattice is `world`
+    slabs long in time, antiperiodic), one step = DhopOE then DhopEO of the decomposed operator: face pack, face
+    exchange (NCCL point-to-point between neighbouring ranks; a copy when world = 1) on a side stream under the
+    open-boundary bulk kernel, face terms.  Weak scaling: `value` = all ranks' sites over the slowest rank's time."""
+    import torch
+    import paper_2203_06777_b200 as dwf
+    from paper_2203_06777_b200.dist import SlabDhop
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dwf.load()
+    d, Ls, prec = w["dims"], w["Ls"], w["prec"]
+    V4 = d[0] * d[1] * d[2] * d[3]
+    sites = (V4 // 2) * Ls
+    U, psi_e = make_inputs(w)                        # every rank uses the same slab data: timing does not depend on it
+    gdims = d[:3] + (d[3] * world,)
+    op = SlabDhop(gdims, Ls, prec, w["bc"], rank, world, device=local_rank)
+    op.load_gauge(U)
+    g = op.geometry
+    f_in = g.import_spinor(psi_e, dwf.EVEN)
+    f_mid, f_out = g.new_field(dwf.ODD), g.new_field(dwf.EVEN)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step():
+        op.dhop_oe(f_in, f_mid)
+        op.dhop_eo(f_mid, f_out)
+
+    for _ in range(args.warmup):
+        step()
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(args.steps)]
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    barrier()
+    sampler.start()
+    l0 = dwf.dwf_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for k in range(args.steps):
+        ev[k][0].record()
+        op.dhop_oe(f_in, f_mid)
+        ev[k][1].record()
+        op.dhop_eo(f_mid, f_out)
+    e1.record()
+    barrier()
+    launches = dwf.dwf_launch_count() - l0
+    clocks = sampler.stop()
+    ms_step = max_over_ranks(e0.elapsed_time(e1), dist) / args.steps
+    t_oe = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
+    # the same half-Dhop without decomposition (periodic slab): what the face traffic and kernels cost
+    gp = dwf.Geometry(d, Ls, prec, dwf.PERIODIC, device=local_rank)
+    gp.load_gauge(U)
+    for _ in range(3):
+        gp.dhop_oe(f_in, f_mid)
+    pa, pb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    pa.record()
+    for _ in range(args.steps):
+        gp.dhop_oe(f_in, f_mid)
+    pb.record()
+    torch.cuda.synchronize()
+    t_plain = pa.elapsed_time(pb) / args.steps
+    face = dwf.dwf_face_bytes(g.handle)
+    if rank == 0:
+        peak, peak_src = peaks()
+        mb = model_bytes_cb(w) + 4 * face + 4 * (sites // d[3]) * 24 * prec     # + write/read of 2 faces each way, 2 layers of in and out
+        achieved = mb / (t_oe * 1e-3) / 1e9
+        line = {
+            "metric": "Dhop GFlop/s (1320 flop/5D site)", "value": whole_job_gflops(world, sites, ms_step), "unit": "GFlop/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32" if prec == 4 else "f64", "data": "synthetic",
+            "config": {"workload": f"time-decomposed DWF even/odd Dhop (SURVEY.md 8(f3)): {world} slab(s) of {d[0]}x{d[1]}x{d[2]}x{d[3]} x Ls={Ls} "
+                                   f"fp{8 * prec} (global {gdims[0]}x{gdims[1]}x{gdims[2]}x{gdims[3]}, antiperiodic time), DhopOE then DhopEO",
+                       "name": args.workload, "dims": list(d), "Ls": Ls, "l2": "fields larger than L2; no flush",
+                       "parallelism": f"time slabs over {world} rank(s), half-spinor faces exchanged per half-Dhop" if world > 1 else
+                                      "single GPU (the rank is its own neighbour: face exchange = device copy)"},
+            "clocks": clocks, "gpu_launches": int(launches),
+            "kernels_ms": {"decomposed_dhop_oe": t_oe, "plain_periodic_dhop_oe": t_plain},
+            "halo": {"face_bytes": face, "sent_per_half_dhop": 2 * face, "overhead_vs_plain": t_oe / t_plain - 1.0},
+            "roofline": {"bound": "hbm", "kernel": g.kernel_info() + " + face_pack / face_apply (decomposed DhopOE)", "achieved": achieved,
+                         "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": mb, "traffic": None},
+        }
+        print(json.dumps(line), flush=True)
+    gp.close()
+    op.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def spawn_ranks(n: int, argv, check_devices: bool = True) -> int:
     """`python bench.py --gpus N` without a launcher: start N ranks of this script under
     torch.distributed.run on this node (one per GPU, rendezvous on 127.0.0.1) and return its exit
@@ -726,6 +827,8 @@ def main():
         run_gpu_schur(args, w)
     elif w.get("kind") == "mrhs":
         run_gpu_mrhs(args, w)
+    elif w.get("kind") == "slab":
+        run_gpu_slab(args, w)
     else:
         run_gpu(args, w)
 

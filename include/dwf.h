@@ -62,7 +62,9 @@ typedef struct dwf_geometry dwf_geometry;   /* opaque, library-owned */
 enum { DWF_OK = 0, DWF_ERR_INVALID_ARG = 1, DWF_ERR_BAD_GEOMETRY = 2, DWF_ERR_NO_GAUGE = 3,
        DWF_ERR_CUDA = 4, DWF_ERR_ALLOC = 5, DWF_ERR_UNSUPPORTED = 6 };
 enum { DWF_F32 = 4, DWF_F64 = 8 };                   /* precision = bytes per real            */
-enum { DWF_PERIODIC = 0, DWF_ANTIPERIODIC_T = 1 };   /* time = dims[3]                        */
+enum { DWF_PERIODIC = 0, DWF_ANTIPERIODIC_T = 1,     /* time = dims[3]                        */
+       DWF_OPEN_T = 2 };                             /* hops that would wrap in time contribute nothing: one time slab of a
+                                                        domain-decomposed lattice (dwf_face_pack_t / dwf_face_apply_t)     */
 enum { DWF_FULL = -1, DWF_EVEN = 0, DWF_ODD = 1 };   /* parity = (x0+x1+x2+x3) & 1            */
 
 /* Create a geometry: lattice extents dims[4] (each even and >= 2), fifth-dimension extent Ls >= 1,
@@ -131,6 +133,27 @@ DWF_API int dwf_dhop_eo_axpy(const dwf_geometry *g, const void *in_odd, const vo
  * per right-hand side.  Asynchronous.  Errors as dwf_dhop_oe; INVALID_ARG for nrhs < 1 or L3 Ls nrhs >= 2^31. */
 DWF_API int dwf_dhop_oe_mrhs(const dwf_geometry *g, const void *in_even, void *out_odd, int nrhs, int dagger, void *stream);
 DWF_API int dwf_dhop_eo_mrhs(const dwf_geometry *g, const void *in_odd, void *out_even, int nrhs, int dagger, void *stream);
+
+/* ---- Domain decomposition along time ("near perfect overlap of communication
+ * and computation", L250 "face assembly"; reading #26).  A rank owns a slab of dims[3] time layers and
+ * creates its geometry with DWF_OPEN_T; dwf_dhop_oe / _eo (and their _dag forms) then compute everything but the
+ * two face terms.  Per half-Dhop (in of parity q = 1 - p, out of parity p):
+ *   1. dwf_face_pack_t(g, in, q, dagger, send_down, send_up): projected half spinors (12 reals per face site and
+ *      slice, dwf_face_bytes(g) bytes per buffer) of the slab's first layer for the LOWER neighbour (send_down) and of
+ *      its last layer, already multiplied by U_t^dag, for the UPPER neighbour (send_up);
+ *   2. the exchange (outside this library: NCCL send / recv, a peer copy, or a plain copy when the rank is its own
+ *      neighbour), overlapped with 3. the bulk half-Dhop on `stream`;
+ *   4. dwf_face_apply_t(g, recv_lo, recv_hi, sign_lo, sign_hi, out, p, dagger): recv_lo = the lower neighbour's
+ *      send_up, recv_hi = the upper neighbour's send_down; adds sign_lo (1 + gamma_t) [recv_lo] to the first layer
+ *      and sign_hi (1 - gamma_t) U_t(x) [recv_hi] to the last layer of out (sign = -1 on the face that crosses a
+ *      global antiperiodic boundary, else +1).
+ * The assembled result equals the Dhop of the whole lattice.  All asynchronous on `stream`; device pointers,
+ * 16-byte aligned.  Errors: INVALID_ARG, NO_GAUGE, CUDA. */
+DWF_API size_t dwf_face_bytes(const dwf_geometry *g);
+DWF_API int dwf_face_pack_t(const dwf_geometry *g, const void *in, int parity_in, int dagger, void *send_down, void *send_up,
+                            void *stream);
+DWF_API int dwf_face_apply_t(const dwf_geometry *g, const void *recv_lo, const void *recv_hi, double sign_lo, double sign_hi,
+                             void *out, int parity_out, int dagger, void *stream);
 
 /* *result_host = sum over all reals of |field|^2, accumulated in fp64 in a fixed order
  * (deterministic).  parity = DWF_FULL for a full field, DWF_EVEN / DWF_ODD for a half field.

@@ -16,7 +16,7 @@ import numpy as np
 
 OK, ERR_INVALID_ARG, ERR_BAD_GEOMETRY, ERR_NO_GAUGE, ERR_CUDA, ERR_ALLOC, ERR_UNSUPPORTED = range(7)
 F32, F64 = 4, 8
-PERIODIC, ANTIPERIODIC_T = 0, 1
+PERIODIC, ANTIPERIODIC_T, OPEN_T = 0, 1, 2
 FULL, EVEN, ODD = -1, 0, 1
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -28,7 +28,7 @@ SYMBOLS = (
     "dwf_dhop_eo", "dwf_dhop_dag", "dwf_dhop_oe_dag", "dwf_dhop_eo_dag", "dwf_dhop_oe_axpy", "dwf_dhop_eo_axpy", "dwf_dhop_oe_norm2", "dwf_dhop_eo_norm2", "dwf_norm2", "dwf_inner_product", "dwf_field_bytes",
     "dwf_import_spinor", "dwf_export_spinor", "dwf_launch_count", "dwf_kernel_info", "dwf_set_option",
     "dwf_error_string", "dwf_last_error",
-    "dwf_dhop_oe_mrhs", "dwf_dhop_eo_mrhs", "dwf_host_wait",
+    "dwf_dhop_oe_mrhs", "dwf_dhop_eo_mrhs", "dwf_host_wait", "dwf_face_bytes", "dwf_face_pack_t", "dwf_face_apply_t",
     "dwf_mooee", "dwf_mooee_inv", "dwf_ddwf", "dwf_schur_work_bytes", "dwf_schur", "dwf_axpby", "dwf_cg_work_bytes", "dwf_cg_schur",
 )
 
@@ -72,6 +72,10 @@ def load(build_if_missing: bool = True):
     lib.dwf_import_spinor.argtypes = [vp, vp, ci, ci, vp, vp]
     lib.dwf_export_spinor.argtypes = [vp, vp, ci, vp, ci, vp]
     lib.dwf_host_wait.argtypes = [vp]
+    lib.dwf_face_bytes.argtypes = [vp]
+    lib.dwf_face_bytes.restype = cs
+    lib.dwf_face_pack_t.argtypes = [vp, vp, ci, ci, vp, vp, vp]
+    lib.dwf_face_apply_t.argtypes = [vp, vp, vp, ctypes.c_double, ctypes.c_double, vp, ci, ci, vp]
     lib.dwf_launch_count.argtypes = []
     lib.dwf_launch_count.restype = ctypes.c_ulonglong
     lib.dwf_kernel_info.argtypes = [vp, ctypes.c_char_p, cs]
@@ -326,6 +330,27 @@ def dwf_cg_schur(g: int, b, x, parity: int, M5: float, mass: float, tol: float, 
                                float(tol), int(max_iter), _work_ptr(work, dwf_cg_work_bytes(g)), ctypes.byref(it),
                                ctypes.byref(res), _stream(stream, g)), "dwf_cg_schur")
     return it.value, res.value
+
+
+def dwf_face_bytes(g: int) -> int:
+    return int(load().dwf_face_bytes(g))
+
+
+def _face_ptr(t, g) -> int:
+    if not getattr(t, "is_cuda", False) or not t.is_contiguous() or t.numel() * t.element_size() != dwf_face_bytes(g):
+        raise DwfError(ERR_INVALID_ARG, "binding", "face buffers must be contiguous CUDA tensors of dwf_face_bytes bytes")
+    return t.data_ptr()
+
+
+def dwf_face_pack_t(g: int, inp, parity_in: int, send_down, send_up, dagger: bool = False, stream=None) -> None:
+    _check(load().dwf_face_pack_t(g, _dev_ptr(inp, g, parity_in), int(parity_in), int(bool(dagger)), _face_ptr(send_down, g),
+                                  _face_ptr(send_up, g), _stream(stream, g)), "dwf_face_pack_t")
+
+
+def dwf_face_apply_t(g: int, recv_lo, recv_hi, sign_lo: float, sign_hi: float, out, parity_out: int, dagger: bool = False,
+                     stream=None) -> None:
+    _check(load().dwf_face_apply_t(g, _face_ptr(recv_lo, g), _face_ptr(recv_hi, g), float(sign_lo), float(sign_hi),
+                                   _dev_ptr(out, g, parity_out), int(parity_out), int(bool(dagger)), _stream(stream, g)), "dwf_face_apply_t")
 
 
 def dwf_host_wait(g: int) -> None:

@@ -282,7 +282,7 @@ int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, i
 {
     if (!dims || !out) { set_error("dwf_create_geometry: NULL argument"); return DWF_ERR_INVALID_ARG; }
     if (precision != DWF_F32 && precision != DWF_F64) { set_error("precision must be 4 or 8"); return DWF_ERR_UNSUPPORTED; }
-    if (bc_time != DWF_PERIODIC && bc_time != DWF_ANTIPERIODIC_T) { set_error("bad bc_time"); return DWF_ERR_INVALID_ARG; }
+    if (bc_time != DWF_PERIODIC && bc_time != DWF_ANTIPERIODIC_T && bc_time != DWF_OPEN_T) { set_error("bad bc_time"); return DWF_ERR_INVALID_ARG; }
     if (Ls < 1) { set_error("Ls must be >= 1"); return DWF_ERR_BAD_GEOMETRY; }
     long long V4 = 1;
     for (int d = 0; d < 4; d++) {
@@ -331,6 +331,8 @@ int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, i
     g->reduce_blocks = g->sm_count * 32;
     bool ok = cudaMalloc(&g->gauge[0], g->gauge_bytes) == cudaSuccess &&
               cudaMalloc(&g->gauge[1], g->gauge_bytes) == cudaSuccess &&
+              cudaMalloc(&g->tlink_top[0], (size_t)dims[1] * dims[2] * (dims[0] / 2) * 18 * (size_t)precision) == cudaSuccess &&
+              cudaMalloc(&g->tlink_top[1], (size_t)dims[1] * dims[2] * (dims[0] / 2) * 18 * (size_t)precision) == cudaSuccess &&
               cudaMalloc(&g->partials, sizeof(double) * 2 * (size_t)g->reduce_blocks) == cudaSuccess &&
               cudaMalloc(&g->result_dev, sizeof(double) * 2) == cudaSuccess &&
               cudaHostAlloc(&g->mailbox_host, sizeof(double) * 4, cudaHostAllocMapped) == cudaSuccess &&
@@ -354,6 +356,8 @@ int dwf_destroy_geometry(dwf_geometry *g)
     cudaFree(g->gauge[1]);
     cudaFree(g->gauge12[0]);
     cudaFree(g->gauge12[1]);
+    cudaFree(g->tlink_top[0]);
+    cudaFree(g->tlink_top[1]);
     cudaFree(g->partials);
     cudaFree(g->result_dev);
     cudaFreeHost(g->mailbox_host);
@@ -437,6 +441,7 @@ int dwf_load_gauge(dwf_geometry *g, const void *U, int src_is_device, void *stre
         src = tmp;
     }
     int rc = launch_pack_gauge(g, src, st);
+    if (!rc) rc = launch_pack_tlinks(g, src, st);
     if (!rc && g->opt_gauge12) {
         // the compressed copy (two thirds of the bytes) next to the full one: only the plain staged fp32 Dhop reads it
         const size_t b12 = g->gauge_bytes / 3 * 2;

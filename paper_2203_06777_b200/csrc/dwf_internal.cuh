@@ -76,6 +76,9 @@ struct dwf_geometry {
     // option "gauge12": rows 0, 1 of every link only (12 reals), [row][24 vectors][Lh]; fp32, used by the plain staged Dhop
     void *gauge12[2];
     int opt_gauge12;
+    // U_t of the last time layer, per parity of the site, complex[row2][9][h]: the links the face kernels of halo.cu need
+    // (in the packed sets the wrapping time links are sign-folded or, with DWF_OPEN_T, zero)
+    void *tlink_top[2];
     // direct kernel: CTA tile table (origins in rasterised launch order)
     dwf::Tiling tiling_cb;
     int4 *tiles_cb;
@@ -156,6 +159,8 @@ int fetch_reduction(const dwf_geometry *g, cudaStream_t st, int n, double *out);
 // pack.cu
 int launch_pack_gauge(const dwf_geometry *g, const void *U_canonical_dev, cudaStream_t st);
 int launch_compress_gauge12(const dwf_geometry *g, cudaStream_t st);      // gauge[p] -> gauge12[p]
+// halo.cu
+int launch_pack_tlinks(const dwf_geometry *g, const void *U_canonical_dev, cudaStream_t st);
 // row0, nrow_c: lattice lines (rows) covered, nrow_c < 0 = the whole field; canonical_dev points at the first site of the range
 int launch_import(const dwf_geometry *g, const void *canonical_dev, int parity, void *field,
                   cudaStream_t st, long long row0 = 0, long long nrow_c = -1);

@@ -16,7 +16,8 @@
 //         parity (cb index x>>1) the 8 links that site multiplies with:
 //            leg 2*mu   : U_mu(x)                       (forward hop,  psi(x+mu))
 //            leg 2*mu+1 : U_mu(x-mu)^dagger             (backward hop, psi(x-mu))
-//         each times -1 when the hop wraps around an antiperiodic time direction, stored planar
+//         each times -1 when the hop wraps around an antiperiodic time direction (times 0 with an open time
+//         boundary, DWF_OPEN_T: the slab operator of halo.cu), stored planar
 //         row by row as complex[row][f/2][h][f&1], f = leg*9 + a*3+b (the 72 link components of
 //         the Lh output sites of a row are one contiguous 576*Lh-byte block, in 128-bit pairs).
 //         Every canonical link appears exactly once in each parity set, so one half-Dhop reads
@@ -159,7 +160,7 @@ spinor_reorder_sites_kernel(const float *__restrict__ src, float *__restrict__ d
 template <typename T>
 __global__ void __launch_bounds__(256)
 gauge_pack_kernel(const T *__restrict__ U, T *__restrict__ set_even, T *__restrict__ set_odd,
-                  const Lattice lat, const int antiperiodic_t)
+                  const Lattice lat, const int bc_time)
 {
     // one thread per (lexicographic site x, leg)
     const long long n = lat.V4 * 8;
@@ -185,9 +186,9 @@ gauge_pack_kernel(const T *__restrict__ U, T *__restrict__ set_even, T *__restri
             int cm[4] = {c[0], c[1], c[2], c[3]};
             cm[mu] = (c[mu] == 0) ? lat.L[mu] - 1 : c[mu] - 1;
             src_site = cm[0] + (long long)lat.L[0] * (cm[1] + (long long)lat.L[1] * (cm[2] + (long long)lat.L[2] * cm[3]));
-            if (antiperiodic_t && mu == 3 && c[3] == 0) sign = -1;
+            if (bc_time && mu == 3 && c[3] == 0) sign = bc_time == DWF_OPEN_T ? 0 : -1;
         } else {
-            if (antiperiodic_t && mu == 3 && c[3] == lat.L[3] - 1) sign = -1;
+            if (bc_time && mu == 3 && c[3] == lat.L[3] - 1) sign = bc_time == DWF_OPEN_T ? 0 : -1;
         }
         const T *u = U + (src_site * 4 + mu) * 18;
         const long long row = cb / lat.Lh;
@@ -252,10 +253,10 @@ int launch_pack_gauge(const dwf_geometry *g, const void *U_dev, cudaStream_t st)
     const int grid = grid_for(g->lat.V4 * 8, g->sm_count);
     if (g->prec == DWF_F32)
         gauge_pack_kernel<float><<<grid, 256, 0, st>>>(static_cast<const float *>(U_dev), static_cast<float *>(g->gauge[0]),
-                                                      static_cast<float *>(g->gauge[1]), g->lat, g->bc_time == DWF_ANTIPERIODIC_T);
+                                                      static_cast<float *>(g->gauge[1]), g->lat, g->bc_time);
     else
         gauge_pack_kernel<double><<<grid, 256, 0, st>>>(static_cast<const double *>(U_dev), static_cast<double *>(g->gauge[0]),
-                                                       static_cast<double *>(g->gauge[1]), g->lat, g->bc_time == DWF_ANTIPERIODIC_T);
+                                                       static_cast<double *>(g->gauge[1]), g->lat, g->bc_time);
     count_launch();
     DWF_CUDA_CHECK(cudaGetLastError());
     return DWF_OK;
