@@ -49,7 +49,8 @@ struct Staged64Args {
     double *norm_partials;   // NORM kernels: one partial sum of |out|^2 per CTA (fixed order inside the CTA)
 };
 
-template <int LH, int B1, int B2, int B3> struct Staged64Cfg {
+// TM: the TMEM variant (tiles of 128 sites): link columns and the colour exchange live in tensor memory
+template <int LH, int B1, int B2, int B3, bool TM = false> struct Staged64Cfg {
     static constexpr int NROW_C = B1 * B2 * B3;
     static constexpr int T = LH * NROW_C;                        // output sites per tile
     static constexpr int TP = (T + 31) / 32 * 32;                // sites padded to whole warps: thread = colour * TP + site
@@ -64,15 +65,16 @@ template <int LH, int B1, int B2, int B3> struct Staged64Cfg {
     static constexpr int STAGE_BYTES = NROW_IN * ROWB;
     static constexpr int NSTAGE = 2;
     // exchange buffer: [parity of the step][destination colour][source slot][component j][site] complex
-    static constexpr int RED_BYTES = 2 * 3 * 2 * 4 * TP * 16;
+    static constexpr int RED_BYTES = TM ? 0 : 2 * 3 * 2 * 4 * TP * 16;
     // tail: full[2], empty[2][4 regions], exch[NGROUP][2] mbarriers, one fp64 slot per consumer warp (fused norm2)
-    static constexpr int TAIL_EXCH = 16 + 64, TAIL_NORM = TAIL_EXCH + 16 * NGROUP, TAIL = TAIL_NORM + 8 * NWARP_C;
+    static constexpr int TAIL_EXCH = 16 + 64, TAIL_NORM = TAIL_EXCH + 16 * NGROUP, TAIL_TMEM = TAIL_NORM + 8 * NWARP_C, TAIL = TAIL_TMEM + 8;
     static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + RED_BYTES + (TAIL + 15) / 16 * 16;
     static constexpr int PROD_REGS = 24;
     static constexpr int CONS_REGS_RAW = ((65536 - 128 * PROD_REGS) / NTC) / 8 * 8;
     static constexpr int CONS_REGS = CONS_REGS_RAW > 240 ? 240 : CONS_REGS_RAW;
     static_assert(ROWB % 128 == 0, "staged rows must keep TMA destinations 128-byte aligned");
     static_assert(SMEM_BYTES <= 232448, "tile too large for shared memory");
+    static_assert(!TM || NGROUP == 4, "the TMEM variant needs 128-site tiles: the three colour warps of a site group must share a lane quadrant");
 };
 
 __device__ __forceinline__ double2 ldg_d2_hint(const double2 *p, uint64_t policy)
@@ -85,6 +87,52 @@ __device__ __forceinline__ void stg_d2_hint(double2 *p, double2 v, uint64_t poli
 {
     asm volatile("st.global.L1::no_allocate.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(policy) : "memory");
 }
+
+// ---- tensor memory (TMEM) as thread-private storage -------------------------------------------------
+// tcgen05.ld / tcgen05.st with shape 32x32b: lane i of a warp reads / writes N consecutive 32-bit columns of TMEM
+// lane (32 * (warp % 4) + i).  Consumer warp w = colour * 4 + group sits in lane quadrant group (the CTA's first
+// four warps are the producer warpgroup), so the three colour threads of a site share ONE TMEM lane:
+//   columns [96 c, 96 c + 96)                        the link column of colour c: leg L at +12 L (3 complex = 12 words)
+//   columns [288 + 96 b + 32 c, +32), b = 0, 1       exchange buffer b written by colour c: block r = 1 at +0, r = 2 at +16
+// 480 of the 512 columns.  Measured (profiles/r02_tmem_microbench.md): >= 314 B/clk/SM with 12 warps, 2.5 x shared memory.
+__device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t (&r)[4])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_st4(uint32_t taddr, const uint32_t (&r)[4])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]) : "memory");
+}
+// one complex fp64 number = four columns
+__device__ __forceinline__ void tmem_st_c(uint32_t taddr, double2 v)
+{
+    uint32_t r[4] = {(uint32_t)__double2loint(v.x), (uint32_t)__double2hiint(v.x), (uint32_t)__double2loint(v.y), (uint32_t)__double2hiint(v.y)};
+    tmem_st4(taddr, r);
+}
+__device__ __forceinline__ double2 tmem_unpack(const uint32_t (&r)[4])
+{
+    return make_double2(__hiloint2double((int)r[1], (int)r[0]), __hiloint2double((int)r[3], (int)r[2]));
+}
+// tcgen05.ld is asynchronous: its destination registers are valid only after tcgen05.wait::ld.  The registers are
+// in/out operands of the wait, so that every later use depends on it -- without a memory clobber, which would keep
+// ptxas from moving the shared-memory loads of the next legs across it.
+__device__ __forceinline__ void tmem_wait_ld_regs3(uint32_t (&w)[3][4])
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+r"(w[0][0]), "+r"(w[0][1]), "+r"(w[0][2]), "+r"(w[0][3]), "+r"(w[1][0]), "+r"(w[1][1]), "+r"(w[1][2]), "+r"(w[1][3]),
+                   "+r"(w[2][0]), "+r"(w[2][1]), "+r"(w[2][2]), "+r"(w[2][3]));
+}
+__device__ __forceinline__ void tmem_wait_ld_regs(uint32_t (&a)[4][4], uint32_t (&b)[4][4])
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+r"(a[0][0]), "+r"(a[0][1]), "+r"(a[0][2]), "+r"(a[0][3]), "+r"(a[1][0]), "+r"(a[1][1]), "+r"(a[1][2]), "+r"(a[1][3]),
+                   "+r"(a[2][0]), "+r"(a[2][1]), "+r"(a[2][2]), "+r"(a[2][3]), "+r"(a[3][0]), "+r"(a[3][1]), "+r"(a[3][2]), "+r"(a[3][3]),
+                   "+r"(b[0][0]), "+r"(b[0][1]), "+r"(b[0][2]), "+r"(b[0][3]), "+r"(b[1][0]), "+r"(b[1][1]), "+r"(b[1][2]), "+r"(b[1][3]),
+                   "+r"(b[2][0]), "+r"(b[2][1]), "+r"(b[2][2]), "+r"(b[2][3]), "+r"(b[3][0]), "+r"(b[3][1]), "+r"(b[3][2]), "+r"(b[3][3]));
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tmem_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 
 // one leg for colour column c: acc += reconstruct( U[:, c] * project(psi)[c] ).  p0..p3 = colour c of the
 // four spin components of the neighbour; U[r] = U_{(c+r)%3, c}, r = 0..2 (the rows of the column ROTATED
@@ -161,12 +209,12 @@ __device__ __forceinline__ void leg64(double2 (&acc)[12], const double2 p0, cons
 // warps of a 32-site group drift by up to one step.  Two exchange buffers suffice: a buffer is overwritten
 // at step g+2, after this warp has seen all arrivals of step g+1, each of which follows that warp's reads
 // of step g.
-template <int LH, int B1, int B2, int B3, int MODE>
+template <int LH, int B1, int B2, int B3, int MODE, bool TM>
 __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned char *smem, const uint32_t full_base,
                                           const uint32_t empty_base, const uint32_t exch_base, const int site, const int c,
-                                          const int my_tiles, double &nsum)
+                                          const int my_tiles, double &nsum, const uint32_t tmem_base)
 {
-    using Cfg = Staged64Cfg<LH, B1, B2, B3>;
+    using Cfg = Staged64Cfg<LH, B1, B2, B3, TM>;
     constexpr bool DAG = (MODE & 1) != 0, AXPY = (MODE & 2) != 0, NORM = (MODE & 4) != 0;
     const bool active = site < Cfg::T;
     const int st = active ? site : 0;
@@ -206,7 +254,13 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
     const double2 *red_r = red + (size_t)((c * 2) * 4) * Cfg::TP + site;   // what the partners left for colour c
     constexpr int RED_BUF = 3 * 2 * 4 * Cfg::TP;                            // complex numbers per buffer
     const uint32_t my_exch = exch_base + 16 * (site >> 5);      // exch[group][2]
-    double2 U[24];              // column c of the 8 links, rows rotated: U[leg*3 + r] = U_leg[(c+r)%3][c]
+    // column c of the 8 links, rows rotated: U[leg*3 + r] = U_leg[(c+r)%3][c]; in registers, or (TM) in tensor memory
+    double2 U[TM ? 1 : 24];
+    // TM: this thread's TMEM lane is 32 * group + lane (group = site >> 5 = warp % 4); column ranges as above
+    const uint32_t tm_lane = tmem_base + ((uint32_t)((site >> 5) * 32) << 16);
+    const uint32_t tm_links = tm_lane + 96u * c;
+    const uint32_t tm_xw = tm_lane + 288u + 32u * c;                                   // where I publish (+ 96 buf)
+    const uint32_t tm_xr0 = tm_lane + 288u + 32u * c2, tm_xr1 = tm_lane + 288u + 32u * c1 + 16u;   // what is left for me
 
     // global row of this thread's site in the it-th tile, and the parity bit r of x0 = 2h + r
     auto tile_row = [&](int it, int &r) -> long long {
@@ -224,13 +278,27 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
     const int rot[3] = {c, c1, c2};
     auto load_links = [&](long long grow) {
         const double2 *gp = args.gauge + grow * (72 * LH) + 2 * h;
+        if constexpr (TM) {
+            double2 t[24];
 #pragma unroll
-        for (int leg = 0; leg < 8; leg++)
+            for (int leg = 0; leg < 8; leg++)
 #pragma unroll
-            for (int r = 0; r < 3; r++) {
-                const int f = leg * 9 + rot[r] * 3 + c;
-                U[leg * 3 + r] = ldg_d2_hint(gp + (f >> 1) * 2 * LH + (f & 1), pol_first);
-            }
+                for (int r = 0; r < 3; r++) {
+                    const int f = leg * 9 + rot[r] * 3 + c;
+                    t[leg * 3 + r] = ldg_d2_hint(gp + (f >> 1) * 2 * LH + (f & 1), pol_first);
+                }
+#pragma unroll
+            for (int k = 0; k < 24; k++) tmem_st_c(tm_links + 4 * k, t[k]);
+            tmem_wait_st();
+        } else {
+#pragma unroll
+            for (int leg = 0; leg < 8; leg++)
+#pragma unroll
+                for (int r = 0; r < 3; r++) {
+                    const int f = leg * 9 + rot[r] * 3 + c;
+                    U[leg * 3 + r] = ldg_d2_hint(gp + (f >> 1) * 2 * LH + (f & 1), pol_first);
+                }
+        }
     };
 
     // the pending step: the block of partial sums this thread owns, where it goes, its x (AXPY)
@@ -242,10 +310,23 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
         mbar_wait(my_exch + 8 * buf, (keep_g >> 1) & 1);
         if (active) {
             double2 a0[4], a1[4];
+            if constexpr (TM) {
+                tmem_fence_after();
+                uint32_t w0[4][4], w1[4][4];
 #pragma unroll
-            for (int j = 0; j < 4; j++) {
-                a0[j] = red_r[buf * RED_BUF + j * Cfg::TP];
-                a1[j] = red_r[buf * RED_BUF + (4 + j) * Cfg::TP];
+                for (int j = 0; j < 4; j++) {
+                    tmem_ld4(tm_xr0 + 96u * buf + 4 * j, w0[j]);
+                    tmem_ld4(tm_xr1 + 96u * buf + 4 * j, w1[j]);
+                }
+                tmem_wait_ld_regs(w0, w1);
+#pragma unroll
+                for (int j = 0; j < 4; j++) { a0[j] = tmem_unpack(w0[j]); a1[j] = tmem_unpack(w1[j]); }
+            } else {
+#pragma unroll
+                for (int j = 0; j < 4; j++) {
+                    a0[j] = red_r[buf * RED_BUF + j * Cfg::TP];
+                    a1[j] = red_r[buf * RED_BUF + (4 + j) * Cfg::TP];
+                }
             }
             double2 v[4];
 #pragma unroll
@@ -291,25 +372,41 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
                       q##L##_1 = *reinterpret_cast<const double2 *>(sb + off[L] + KSPIN),            \
                       q##L##_2 = *reinterpret_cast<const double2 *>(sb + off[L] + 2 * KSPIN),        \
                       q##L##_3 = *reinterpret_cast<const double2 *>(sb + off[L] + 3 * KSPIN);
-#define DWF_LEG64(L, MU, FWD, FIRST) leg64<MU, (FWD) != DAG, FIRST>(acc, q##L##_0, q##L##_1, q##L##_2, q##L##_3, U + 3 * (L));
+        // TM: the three link elements of leg L come out of tensor memory, requested two legs ahead: tcgen05.wait::ld
+        // waits for ALL loads in flight, so the request for leg NEXT goes out right after the wait of leg L, into the
+        // registers leg L has just been unpacked from, and lands during the arithmetic of leg L.
+#define DWF_TLOAD(L, W)                                                                             \
+        if constexpr (TM) { tmem_ld4(tm_links + 12 * (L), W[0]); tmem_ld4(tm_links + 12 * (L) + 4, W[1]); tmem_ld4(tm_links + 12 * (L) + 8, W[2]); }
+#define DWF_LEG64(L, MU, FWD, FIRST, W, NEXT)                                                       \
+        if constexpr (TM) {                                                                         \
+            tmem_wait_ld_regs3(W);                                                                  \
+            const double2 Ul[3] = {tmem_unpack(W[0]), tmem_unpack(W[1]), tmem_unpack(W[2])};        \
+            if constexpr ((NEXT) >= 0) { DWF_TLOAD((NEXT) < 0 ? 0 : (NEXT), W) }                    \
+            leg64<MU, (FWD) != DAG, FIRST>(acc, q##L##_0, q##L##_1, q##L##_2, q##L##_3, Ul);        \
+        } else {                                                                                    \
+            leg64<MU, (FWD) != DAG, FIRST>(acc, q##L##_0, q##L##_1, q##L##_2, q##L##_3, U + 3 * (L)); \
+        }
         // Legs in the order x3, x2, x1, x0.  The stage is handed back to the producer ONCE, after the last leg:
         // every lane's loads precede the warp barrier, lane 0's arrives (release) follow it and depend on the
         // data of the last legs' loads (tma.cuh: mbar_arrive_after8).  Releasing the face regions early, right
         // after the two legs that read them (as dhop_staged.cu does), was measured 4 % faster here but gave
         // wrong results in the last slice of a tile as soon as two regions were released early (r02 notes in
         // DESIGN.md): not understood, so not used.
+        uint32_t ua[3][4], ub[3][4];
+        DWF_TLOAD(6, ua)
+        DWF_TLOAD(7, ub)
         DWF_LOAD64(6) DWF_LOAD64(7)
-        DWF_LEG64(6, 3, true, true)
-        DWF_LEG64(7, 3, false, false)
+        DWF_LEG64(6, 3, true, true, ua, 4)
+        DWF_LEG64(7, 3, false, false, ub, 5)
         DWF_LOAD64(4) DWF_LOAD64(5)
-        DWF_LEG64(4, 2, true, false)
-        DWF_LEG64(5, 2, false, false)
+        DWF_LEG64(4, 2, true, false, ua, 2)
+        DWF_LEG64(5, 2, false, false, ub, 3)
         DWF_LOAD64(2) DWF_LOAD64(3)
-        DWF_LEG64(2, 1, true, false)
-        DWF_LEG64(3, 1, false, false)
+        DWF_LEG64(2, 1, true, false, ua, 0)
+        DWF_LEG64(3, 1, false, false, ub, 1)
         DWF_LOAD64(0) DWF_LOAD64(1)
-        DWF_LEG64(0, 0, true, false)
-        DWF_LEG64(1, 0, false, false)
+        DWF_LEG64(0, 0, true, false, ua, -1)
+        DWF_LEG64(1, 0, false, false, ub, -1)
         __syncwarp();
         if (lane == 0) {
             mbar_arrive(eb);
@@ -319,14 +416,25 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
         }
 #undef DWF_LOAD64
 #undef DWF_LEG64
+#undef DWF_TLOAD
 
         if (keep_g >= 0) finish();               // the previous step: its exchange has long completed
         // publish the blocks r = 1, 2 of this step
         const int buf = g & 1;
+        if constexpr (TM) {
 #pragma unroll
-        for (int j = 0; j < 4; j++) {
-            red_w1[buf * RED_BUF + j * Cfg::TP] = acc[3 * j + 1];
-            red_w2[buf * RED_BUF + j * Cfg::TP] = acc[3 * j + 2];
+            for (int j = 0; j < 4; j++) {
+                tmem_st_c(tm_xw + 96u * buf + 4 * j, acc[3 * j + 1]);
+                tmem_st_c(tm_xw + 96u * buf + 16 + 4 * j, acc[3 * j + 2]);
+            }
+            tmem_wait_st();
+            tmem_fence_before();
+        } else {
+#pragma unroll
+            for (int j = 0; j < 4; j++) {
+                red_w1[buf * RED_BUF + j * Cfg::TP] = acc[3 * j + 1];
+                red_w2[buf * RED_BUF + j * Cfg::TP] = acc[3 * j + 2];
+            }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(my_exch + 8 * buf);
@@ -359,13 +467,13 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
     if (keep_g >= 0) finish();
 }
 
-template <int LH, int B1, int B2, int B3, int MODE>
-__global__ void __launch_bounds__(Staged64Cfg<LH, B1, B2, B3>::NT, 1)
+template <int LH, int B1, int B2, int B3, int MODE, bool TM>
+__global__ void __launch_bounds__(Staged64Cfg<LH, B1, B2, B3, TM>::NT, 1)
 dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_x1,
                      const __grid_constant__ CUtensorMap map_x2, const __grid_constant__ CUtensorMap map_x3,
                      const Staged64Args args)
 {
-    using Cfg = Staged64Cfg<LH, B1, B2, B3>;
+    using Cfg = Staged64Cfg<LH, B1, B2, B3, TM>;
     extern __shared__ __align__(1024) unsigned char smem[];
     const uint32_t smem_base = smem_u32(smem);
     const uint32_t full_base = smem_base + Cfg::NSTAGE * Cfg::STAGE_BYTES + Cfg::RED_BYTES;   // full[2]
@@ -388,11 +496,26 @@ dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_con
         for (int i = 0; i < 2 * Cfg::NGROUP; i++) mbar_init(exch_base + 8 * i, 3);
         mbar_fence_init();
     }
+    // TM: warp 0 allocates all 512 columns of tensor memory (one CTA per SM) and leaves the base address in shared memory
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + Cfg::RED_BYTES + Cfg::TAIL_TMEM);
+    if constexpr (TM) {
+        if (tid < 32) {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(512) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        }
+        tmem_fence_before();
+    }
     __syncthreads();
+    uint32_t tmem_base = 0;
+    if constexpr (TM) {
+        tmem_fence_after();
+        tmem_base = *tmem_slot;
+    }
 
     if (tid < 128) {            // producer warpgroup: one thread issues the seven boxes of every step
         reg_dealloc<Cfg::PROD_REGS>();
-        if (tid != 0) return;
+        if (TM ? tid >= 32 : tid != 0) return;
+        if (tid == 0) {
         const int L1 = args.L1, L2 = args.L2, L3 = args.L3;
         const uint64_t pol_last = l2_policy(args.l2pol % 10);      // input boxes are re-read by neighbouring tiles
         for (int g = 0; g < nsteps; g++) {
@@ -424,6 +547,12 @@ dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_con
             mbar_arrive_expect_tx(bar, Cfg::NROW_C * Cfg::ROWB);
             tma_load_5d_hint(dst, &map_c, bar, 0, 0, o.x, o.y, c4, pol_last);
         }
+        }
+        if constexpr (TM) {     // warp 0 frees the tensor memory once every consumer warp is done with it
+            __syncwarp();
+            asm volatile("bar.sync 2, %0;" ::"n"((Cfg::NWARP_C + 1) * 32) : "memory");
+            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(512) : "memory");
+        }
         return;
     }
 
@@ -432,7 +561,7 @@ dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_con
     if (ctid >= 3 * Cfg::TP) return;
     const int c = ctid / Cfg::TP, site = ctid % Cfg::TP;         // colour-major: uniform per warp
     double nsum = 0.0;
-    consume64<LH, B1, B2, B3, MODE>(args, smem, full_base, empty_base, exch_base, site, c, my_tiles, nsum);
+    consume64<LH, B1, B2, B3, MODE, TM>(args, smem, full_base, empty_base, exch_base, site, c, my_tiles, nsum, tmem_base);
 
     if constexpr ((MODE & 4) != 0) {
         // lanes -> warp (xor butterfly), warps -> CTA in warp order: the same order in every run
@@ -448,6 +577,10 @@ dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_con
             args.norm_partials[blockIdx.x] = t;
         }
     }
+    if constexpr (TM) {
+        tmem_fence_before();
+        asm volatile("bar.sync 2, %0;" ::"n"((Cfg::NWARP_C + 1) * 32) : "memory");
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -457,6 +590,9 @@ dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_con
 // ---------------------------------------------------------------------------------------------
 #define DWF_STAGED64_VARIANTS(X) X(16, 2, 1, 2) X(16, 1, 1, 4) X(16, 1, 2, 2) X(16, 2, 2, 1) X(8, 4, 2, 1) X(8, 2, 2, 2) X(4, 4, 4, 1) X(4, 4, 2, 2) X(4, 2, 2, 2) X(4, 2, 2, 1) X(8, 2, 2, 1) X(16, 2, 1, 1) \
     X(12, 2, 1, 2) X(12, 2, 2, 1) X(12, 1, 2, 2) X(24, 2, 1, 1) X(24, 1, 1, 2) X(32, 2, 1, 1) X(32, 1, 1, 2) X(32, 1, 2, 1) X(20, 1, 1, 2) X(20, 2, 1, 1)
+
+// TMEM variants (128-site tiles), preferred when they fit the lattice
+#define DWF_STAGED64T_VARIANTS(X) X(16, 2, 2, 2) X(8, 4, 2, 2) X(8, 2, 4, 2) X(8, 2, 2, 4) X(4, 4, 4, 2) X(4, 4, 2, 4)
 
 const void *const *staged64_kernels_mode0();
 const void *const *staged64_kernels_mode1();
@@ -468,9 +604,11 @@ const void *const *staged64_kernels_mode4();
 #define DWF_CAT(a, b) DWF_CAT2(a, b)
 const void *const *DWF_CAT(staged64_kernels_mode, DWF_STAGED64_MODE)()
 {
-#define X(LH, B1, B2, B3) reinterpret_cast<const void *>(&dhop_staged64_kernel<LH, B1, B2, B3, DWF_STAGED64_MODE>),
-    static const void *const tab[] = {DWF_STAGED64_VARIANTS(X)};
+#define X(LH, B1, B2, B3) reinterpret_cast<const void *>(&dhop_staged64_kernel<LH, B1, B2, B3, DWF_STAGED64_MODE, true>),
+#define Y(LH, B1, B2, B3) reinterpret_cast<const void *>(&dhop_staged64_kernel<LH, B1, B2, B3, DWF_STAGED64_MODE, false>),
+    static const void *const tab[] = {DWF_STAGED64T_VARIANTS(X) DWF_STAGED64_VARIANTS(Y)};
 #undef X
+#undef Y
     return tab;
 }
 
@@ -479,7 +617,7 @@ const void *const *DWF_CAT(staged64_kernels_mode, DWF_STAGED64_MODE)()
 // host side
 // ---------------------------------------------------------------------------------------------
 struct Variant64 {
-    int lh, b1, b2, b3, smem, threads;
+    int lh, b1, b2, b3, smem, threads, tmem;
     const void *fn[5];       // MODE 0 plain, 1 dagger, 2 a x + b Dhop, 3 a x + b Dhop^dagger, 4 Dhop + norm2
 };
 
@@ -490,7 +628,12 @@ static const std::vector<Variant64> &variants64()
         const void *const *k0 = staged64_kernels_mode0(), *const *k1 = staged64_kernels_mode1(), *const *k2 = staged64_kernels_mode2(),
                           *const *k3 = staged64_kernels_mode3(), *const *k4 = staged64_kernels_mode4();
 #define X(LH, B1, B2, B3)                                                                             \
-        t.push_back({LH, B1, B2, B3, Staged64Cfg<LH, B1, B2, B3>::SMEM_BYTES, Staged64Cfg<LH, B1, B2, B3>::NT, \
+        t.push_back({LH, B1, B2, B3, Staged64Cfg<LH, B1, B2, B3, true>::SMEM_BYTES, Staged64Cfg<LH, B1, B2, B3, true>::NT, 1, \
+                     {k0[t.size()], k1[t.size()], k2[t.size()], k3[t.size()], k4[t.size()]}});
+        DWF_STAGED64T_VARIANTS(X)
+#undef X
+#define X(LH, B1, B2, B3)                                                                             \
+        t.push_back({LH, B1, B2, B3, Staged64Cfg<LH, B1, B2, B3>::SMEM_BYTES, Staged64Cfg<LH, B1, B2, B3>::NT, 0, \
                      {k0[t.size()], k1[t.size()], k2[t.size()], k3[t.size()], k4[t.size()]}});
         DWF_STAGED64_VARIANTS(X)
 #undef X
