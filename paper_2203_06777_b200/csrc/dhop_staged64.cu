@@ -103,6 +103,35 @@ __device__ __forceinline__ void tmem_st4(uint32_t taddr, const uint32_t (&r)[4])
 {
     asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]) : "memory");
 }
+// the 12 words of one leg's link column: columns [taddr, taddr + 12) as an x8 and an x4 load
+__device__ __forceinline__ void tmem_ld12(uint32_t taddr, uint32_t (&r)[3][4])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                 : "=r"(r[0][0]), "=r"(r[0][1]), "=r"(r[0][2]), "=r"(r[0][3]), "=r"(r[1][0]), "=r"(r[1][1]), "=r"(r[1][2]), "=r"(r[1][3]) : "r"(taddr));
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(r[2][0]), "=r"(r[2][1]), "=r"(r[2][2]), "=r"(r[2][3]) : "r"(taddr + 8));
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+                   "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]) : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
+                 ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]), "r"(r[10]),
+                   "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]),
+                   "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31]) : "memory");
+}
+__device__ __forceinline__ void tmem_pack(uint32_t *r, double2 v)
+{
+    r[0] = (uint32_t)__double2loint(v.x); r[1] = (uint32_t)__double2hiint(v.x);
+    r[2] = (uint32_t)__double2loint(v.y); r[3] = (uint32_t)__double2hiint(v.y);
+}
+__device__ __forceinline__ double2 tmem_unpack_p(const uint32_t *r)
+{
+    return make_double2(__hiloint2double((int)r[1], (int)r[0]), __hiloint2double((int)r[3], (int)r[2]));
+}
 // one complex fp64 number = four columns
 __device__ __forceinline__ void tmem_st_c(uint32_t taddr, double2 v)
 {
@@ -122,13 +151,12 @@ __device__ __forceinline__ void tmem_wait_ld_regs3(uint32_t (&w)[3][4])
                  : "+r"(w[0][0]), "+r"(w[0][1]), "+r"(w[0][2]), "+r"(w[0][3]), "+r"(w[1][0]), "+r"(w[1][1]), "+r"(w[1][2]), "+r"(w[1][3]),
                    "+r"(w[2][0]), "+r"(w[2][1]), "+r"(w[2][2]), "+r"(w[2][3]));
 }
-__device__ __forceinline__ void tmem_wait_ld_regs(uint32_t (&a)[4][4], uint32_t (&b)[4][4])
+__device__ __forceinline__ void tmem_wait_ld_regs(uint32_t (&a)[16], uint32_t (&b)[16])
 {
     asm volatile("tcgen05.wait::ld.sync.aligned;"
-                 : "+r"(a[0][0]), "+r"(a[0][1]), "+r"(a[0][2]), "+r"(a[0][3]), "+r"(a[1][0]), "+r"(a[1][1]), "+r"(a[1][2]), "+r"(a[1][3]),
-                   "+r"(a[2][0]), "+r"(a[2][1]), "+r"(a[2][2]), "+r"(a[2][3]), "+r"(a[3][0]), "+r"(a[3][1]), "+r"(a[3][2]), "+r"(a[3][3]),
-                   "+r"(b[0][0]), "+r"(b[0][1]), "+r"(b[0][2]), "+r"(b[0][3]), "+r"(b[1][0]), "+r"(b[1][1]), "+r"(b[1][2]), "+r"(b[1][3]),
-                   "+r"(b[2][0]), "+r"(b[2][1]), "+r"(b[2][2]), "+r"(b[2][3]), "+r"(b[3][0]), "+r"(b[3][1]), "+r"(b[3][2]), "+r"(b[3][3]));
+                 : "+r"(a[0]), "+r"(a[1]), "+r"(a[2]), "+r"(a[3]), "+r"(a[4]), "+r"(a[5]), "+r"(a[6]), "+r"(a[7]), "+r"(a[8]), "+r"(a[9]), "+r"(a[10]),
+                   "+r"(a[11]), "+r"(a[12]), "+r"(a[13]), "+r"(a[14]), "+r"(a[15]), "+r"(b[0]), "+r"(b[1]), "+r"(b[2]), "+r"(b[3]), "+r"(b[4]), "+r"(b[5]),
+                   "+r"(b[6]), "+r"(b[7]), "+r"(b[8]), "+r"(b[9]), "+r"(b[10]), "+r"(b[11]), "+r"(b[12]), "+r"(b[13]), "+r"(b[14]), "+r"(b[15]));
 }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -312,15 +340,12 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
             double2 a0[4], a1[4];
             if constexpr (TM) {
                 tmem_fence_after();
-                uint32_t w0[4][4], w1[4][4];
-#pragma unroll
-                for (int j = 0; j < 4; j++) {
-                    tmem_ld4(tm_xr0 + 96u * buf + 4 * j, w0[j]);
-                    tmem_ld4(tm_xr1 + 96u * buf + 4 * j, w1[j]);
-                }
+                uint32_t w0[16], w1[16];
+                tmem_ld16(tm_xr0 + 96u * buf, w0);
+                tmem_ld16(tm_xr1 + 96u * buf, w1);
                 tmem_wait_ld_regs(w0, w1);
 #pragma unroll
-                for (int j = 0; j < 4; j++) { a0[j] = tmem_unpack(w0[j]); a1[j] = tmem_unpack(w1[j]); }
+                for (int j = 0; j < 4; j++) { a0[j] = tmem_unpack_p(w0 + 4 * j); a1[j] = tmem_unpack_p(w1 + 4 * j); }
             } else {
 #pragma unroll
                 for (int j = 0; j < 4; j++) {
@@ -376,7 +401,7 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
         // waits for ALL loads in flight, so the request for leg NEXT goes out right after the wait of leg L, into the
         // registers leg L has just been unpacked from, and lands during the arithmetic of leg L.
 #define DWF_TLOAD(L, W)                                                                             \
-        if constexpr (TM) { tmem_ld4(tm_links + 12 * (L), W[0]); tmem_ld4(tm_links + 12 * (L) + 4, W[1]); tmem_ld4(tm_links + 12 * (L) + 8, W[2]); }
+        if constexpr (TM) { tmem_ld12(tm_links + 12 * (L), W); }
 #define DWF_LEG64(L, MU, FWD, FIRST, W, NEXT)                                                       \
         if constexpr (TM) {                                                                         \
             tmem_wait_ld_regs3(W);                                                                  \
@@ -422,11 +447,13 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
         // publish the blocks r = 1, 2 of this step
         const int buf = g & 1;
         if constexpr (TM) {
+            uint32_t w[32];
 #pragma unroll
             for (int j = 0; j < 4; j++) {
-                tmem_st_c(tm_xw + 96u * buf + 4 * j, acc[3 * j + 1]);
-                tmem_st_c(tm_xw + 96u * buf + 16 + 4 * j, acc[3 * j + 2]);
+                tmem_pack(w + 4 * j, acc[3 * j + 1]);
+                tmem_pack(w + 16 + 4 * j, acc[3 * j + 2]);
             }
+            tmem_st32(tm_xw + 96u * buf, w);
             tmem_wait_st();
             tmem_fence_before();
         } else {
