@@ -451,15 +451,17 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
                 U[2 * j + 1] = make_float2(q.z, q.w);                                               \
             }                                                                                       \
         }
-        // Hand region R of this stage back to the producer: every lane's shared-memory loads of the
-        // region precede the warp barrier, lane 0's arrive (release) follows it, and the producer
-        // issues the refilling TMA copy only after it has observed the arrivals of all consumer warps
-        // (acquire).  The barrier is also a compiler fence for memory operations; ptxas still issues the
-        // loads of the next leg right behind it, and against a release ordered only by a data dependence
-        // it costs nothing measurable (C4 fp32: 394-396 us vs 396-400 us, r02 batch 1).
+        // Hand region R of this stage back to the producer: every lane's shared-memory loads of the region precede
+        // the warp barrier in program order, lane 0's arrive (release) follows it, and the producer issues the
+        // refilling TMA copy only after it has observed the arrivals of all consumer warps (acquire).  In converged
+        // code __syncwarp() compiles to nothing and ptxas does not make SYNCS.ARRIVE wait for earlier LDS, so the
+        // arrive ALSO takes acc[0].x as an (unused) input: that value is derived from a word of every one of the twelve
+        // 128-bit loads of the two legs, and a warp-wide LDS delivers all lanes at once, so the arrive cannot issue
+        // while a load of the region is in flight (tma.cuh; the fp64 kernel showed stale reads without this).
+        // Cost: none measurable (r02).
 #define DWF_RELEASE(R)                                                                              \
         __syncwarp();                                                                               \
-        if ((ctid & 31) == 0) mbar_arrive(eb + 8 * (R));
+        if ((ctid & 31) == 0) mbar_arrive_after1(eb + 8 * (R), acc[0].x);
         // wait for the whole stage once (every mbarrier wait is a compiler barrier for memory
         // operations: a wait in front of each leg pair would expose the LDS latency four times per step)
         mbar_wait(fb, par);

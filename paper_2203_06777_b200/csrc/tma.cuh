@@ -45,6 +45,12 @@ __device__ __forceinline__ void mbar_arrive_after8(uint32_t bar, double a, doubl
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar), "d"(a), "d"(b), "d"(c), "d"(d), "d"(e), "d"(f), "d"(g),
                  "d"(h) : "memory");
 }
+// the same with one witness: a value that the arithmetic has derived from EVERY load of the region (the staged fp32
+// kernel passes an accumulator component, which depends on a word of each of the twelve 128-bit loads of a leg pair)
+__device__ __forceinline__ void mbar_arrive_after1(uint32_t bar, float witness)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar), "f"(witness) : "memory");
+}
 __device__ __forceinline__ void mbar_arrive_after12(uint32_t bar, float a, float b, float c, float d, float e, float f, float g,
                                                     float h, float i, float j, float k, float l)
 {
