@@ -228,7 +228,8 @@ def run_reference(args, w):
         "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": 1e3 * tot / len(times), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(w), "note": "CPU oracle on host cores: " + sample},
+        "config": {"workload": workload_name(w), "name": args.workload, "dims": list(d), "Ls": w["Ls"],
+                   "note": "CPU oracle on host cores: " + sample},
         "cpu_baseline": {"value": val, "unit": "GFlop/s", "cores": oracle.num_threads(), "kind": "oracle",
                          "sample": sample},
         "e2e": {"value": val, "unit": "GFlop/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
