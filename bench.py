@@ -279,7 +279,7 @@ def run_gpu(args, w):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+        raise SystemExit(f"bench.py: no CUDA device for rank {rank} of {world} (there is no CPU fallback; use --impl reference for the oracle)")
     torch.cuda.set_device(local_rank)
     dist = None
     if world > 1:

@@ -44,3 +44,17 @@ def test_single_rank_is_identity():
     import bench
     assert bench.max_over_ranks(3.0) == 3.0
     assert bench.whole_job_gflops(1, 8388608, 1.0) == pytest.approx(2 * 1320 * 8388608 / 1e-3 / 1e9)
+
+
+def test_gpus_flag_starts_that_many_ranks(tmp_path):
+    """`python bench.py --gpus 2` without a launcher starts two ranks under torch.distributed.run (127.0.0.1): on this
+    CPU box each rank gets as far as the first CUDA call and stops there with its rank and the world size in the message."""
+    import subprocess
+    code = ("import sys; sys.path.insert(0, %r); import bench; "
+            "sys.exit(bench.spawn_ranks(2, ['--gpus', '2', '--steps', '1', '--warmup', '3', '--no-cpu'], check_devices=False))" % ROOT)
+    env = dict(os.environ, CUDA_VISIBLE_DEVICES="")
+    env.pop("WORLD_SIZE", None)
+    r = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, env=env, timeout=600)
+    assert r.returncode != 0
+    out = r.stdout + r.stderr
+    assert "no CUDA device for rank 0 of 2" in out and "no CUDA device for rank 1 of 2" in out, out[-2000:]
