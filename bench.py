@@ -63,6 +63,8 @@ WORKLOADS = {
     "c4g12": dict(dims=(32, 32, 32, 32), Ls=16, prec=4, bc=0, gauge="near_unit", seed=1004, gauge12=1),
     # four right-hand sides sharing one gauge load, C4 shape
     "c4m4": dict(dims=(32, 32, 32, 32), Ls=16, prec=4, bc=0, gauge="near_unit", seed=1004, kind="mrhs", nrhs=4),
+    # the solver the paper's workload is: CG on the Schur normal equations, a fixed number of iterations on the C4 shape
+    "cg": dict(dims=(32, 32, 32, 32), Ls=16, prec=4, bc=1, gauge="near_unit", seed=1004, kind="cg"),
     "schurd": dict(dims=(32, 32, 32, 32), Ls=16, prec=8, bc=0, gauge="near_unit", seed=1004, kind="schur"),
 }
 
@@ -684,6 +686,76 @@ def run_gpu_mrhs(args, w):
         dist.destroy_process_group()
 
 
+def run_gpu_cg(args, w):
+    """--workload cg: dwf_cg_schur on the C4 shape, `steps` CG iterations per solve (tolerance 0, so every iteration runs).
+    One iteration = S p, S^dag (S p) (eight kernels of SURVEY.md 8(f2)), a fused x / r update with |r|^2, p = r + beta p, one
+    norm2, and two scalar round trips to the host.  Minimal-traffic model per iteration: two Schur applications plus ten
+    half-field passes of the vector algebra."""
+    import torch
+    import paper_2203_06777_b200 as dwf
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dwf.load()
+    d, Ls, prec = w["dims"], w["Ls"], w["prec"]
+    V4 = d[0] * d[1] * d[2] * d[3]
+    sites = (V4 // 2) * Ls
+    M5, mass = 1.8, 0.01
+    U, b = make_inputs(w)
+    g = dwf.Geometry(d, Ls, prec, w["bc"], device=local_rank)
+    g.load_gauge(U)
+    fb = g.import_spinor(b, dwf.EVEN)
+    x = g.new_field(dwf.EVEN)
+    work = g.new_work(dwf.dwf_cg_work_bytes(g.handle))
+    iters = max(2, args.steps)
+    g.cg_schur(fb, dwf.EVEN, M5, mass, 0.0, 2, x=x, work=work)              # warm-up
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    torch.cuda.synchronize()
+    sampler.start()
+    l0 = dwf.dwf_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    _, done, res = g.cg_schur(fb, dwf.EVEN, M5, mass, 0.0, iters, x=x, work=work)
+    e1.record()
+    torch.cuda.synchronize()
+    launches = dwf.dwf_launch_count() - l0
+    clocks = sampler.stop()
+    ms_total = max_over_ranks(e0.elapsed_time(e1), dist)
+    # the solve also applies S^dag once before and S once after the iterations: count them as one more iteration's matvecs
+    ms_iter = ms_total / (done + 1)
+    if rank == 0:
+        peak, peak_src = peaks()
+        half = b.nbytes
+        gauge = model_bytes_cb(w) - 2 * half
+        schur_bytes = (2 * half + gauge) + 2 * half + 2 * half + (3 * half + gauge)
+        iter_bytes = 2 * schur_bytes + 10 * half
+        line = {
+            "metric": "Dhop GFlop/s (1320 flop/5D site)", "value": world * 4 * FLOP_PER_SITE * sites / (ms_iter * 1e-3) / 1e9, "unit": "GFlop/s",
+            "n_gpus": world, "steps": int(done), "warmup": 2, "ms_per_step": ms_iter, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32" if prec == 4 else "f64", "data": "synthetic",
+            "config": {"workload": f"CG on the normal equations of the red-black Shamir DWF Schur complement, {d[0]}x{d[1]}x{d[2]}x{d[3]} x Ls={Ls} "
+                                   f"fp{8 * prec}, M5={M5}, m={mass}: {done} iterations (a step = one iteration: four half-Dhops counted in value)",
+                       "name": args.workload, "dims": list(d), "Ls": Ls, "l2": "fields larger than L2; no flush",
+                       "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "clocks": clocks, "gpu_launches": int(launches), "true_residual_after": res,
+            "roofline": {"bound": "hbm", "kernel": "one CG iteration (8 operator kernels + 3 vector kernels + 2 reductions)",
+                         "achieved": iter_bytes / (ms_iter * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                         "frac": iter_bytes / (ms_iter * 1e-3) / 1e9 / peak, "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": iter_bytes, "traffic": None},
+        }
+        print(json.dumps(line), flush=True)
+    g.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def run_gpu_slab(args, w):
     """--workload c4slab: SURVEY.md 8(f3).  Every rank owns one time slab of `dims` (the global lattice is `world`
     slabs long in time, antiperiodic), one step = DhopOE then DhopEO of the decomposed operator: face pack, face
@@ -828,6 +900,8 @@ def main():
         run_gpu_schur(args, w)
     elif w.get("kind") == "mrhs":
         run_gpu_mrhs(args, w)
+    elif w.get("kind") == "cg":
+        run_gpu_cg(args, w)
     elif w.get("kind") == "slab":
         run_gpu_slab(args, w)
     else:
