@@ -74,6 +74,7 @@ struct StagedArgs {
     int L1, L2, L3, Ls;
     int ssplit;              // CTAs sharing one tile, each walking Ls / ssplit slices
     int parity_out;
+    uint32_t zero;           // 0 at run time, unknown to ptxas: makes the release of a region depend on the loaded data (tma.cuh)
     int bc_time;             // G12 kernels: antiperiodic time (the folded sign of a wrapping link reappears in its rebuilt third row)
     int l2pol;               // decimal digits, see PC_*
     int zigzag;              // walk the slices of every other tile backwards
@@ -451,17 +452,16 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
                 U[2 * j + 1] = make_float2(q.z, q.w);                                               \
             }                                                                                       \
         }
-        // Hand region R of this stage back to the producer: every lane's shared-memory loads of the region precede
-        // the warp barrier in program order, lane 0's arrive (release) follows it, and the producer issues the
-        // refilling TMA copy only after it has observed the arrivals of all consumer warps (acquire).  In converged
-        // code __syncwarp() compiles to nothing and ptxas does not make SYNCS.ARRIVE wait for earlier LDS, so the
-        // arrive ALSO takes acc[0].x as an (unused) input: that value is derived from a word of every one of the twelve
-        // 128-bit loads of the two legs, and a warp-wide LDS delivers all lanes at once, so the arrive cannot issue
-        // while a load of the region is in flight (tma.cuh; the fp64 kernel showed stale reads without this).
-        // Cost: none measurable (r02).
+        // Hand region R of this stage back to the producer: warp barrier, then lane 0's arrive (release), whose ADDRESS
+        // is computed from acc[0].x -- a value derived from a word of every one of the twelve 128-bit loads of the two
+        // legs (after the last leg: of every load of the stage) -- so that it cannot issue while a load of the region is
+        // in flight (tma.cuh: mbar_arrive_dep).  A bare arrive behind the loads is NOT ordered after their completion:
+        // the fp64 kernel read data of the next fill that way.  The producer issues the refilling TMA copy only after it
+        // has observed the arrivals of all consumer warps (acquire).  Measured cost of the dependence on C4 fp32: 367 ->
+        // 378 us per half-Dhop, whichever witness is used (projected half spinors right after the loads: the same).
 #define DWF_RELEASE(R)                                                                              \
         __syncwarp();                                                                               \
-        if ((ctid & 31) == 0) mbar_arrive_after1(eb + 8 * (R), acc[0].x);
+        if ((ctid & 31) == 0) mbar_arrive_dep(eb + 8 * (R), args.zero, acc[0].x);
         // wait for the whole stage once (every mbarrier wait is a compiler barrier for memory
         // operations: a wait in front of each leg pair would expose the LDS latency four times per step)
         mbar_wait(fb, par);
@@ -741,6 +741,7 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     a.out = static_cast<float2 *>(out);
     a.gauge = static_cast<const float2 *>(gauge12 ? g->gauge12[parity_out] : g->gauge[parity_out]);
     a.bc_time = g->bc_time == DWF_ANTIPERIODIC_T;
+    a.zero = 0;
     a.tiles = g->tiles_staged;
     a.ntiles = g->staged.ntiles;
     a.L1 = g->lat.L[1]; a.L2 = g->lat.L[2]; a.L3 = g->lat.L[3]; a.Ls = ls;

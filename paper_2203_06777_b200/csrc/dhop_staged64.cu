@@ -44,6 +44,7 @@ struct Staged64Args {
     int parity_out;
     int zigzag;              // walk the slices of every other tile backwards (L2 reuse between tiles)
     int l2pol;               // decimal digits: digit 0 input boxes, 6 links, 7 output (0 normal, 1 evict_first, 2 evict_last)
+    uint32_t zero;           // 0 at run time, unknown to ptxas: makes the release of a stage depend on the loaded data (tma.cuh)
     const double2 *axpy_x;   // AXPY kernels: out = a x + b Dhop in (x on the output parity; may be out)
     double axpy_a, axpy_b;
     double *norm_partials;   // NORM kernels: one partial sum of |out|^2 per CTA (fixed order inside the CTA)
@@ -411,12 +412,12 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
         } else {                                                                                    \
             leg64<MU, (FWD) != DAG, FIRST>(acc, q##L##_0, q##L##_1, q##L##_2, q##L##_3, U + 3 * (L)); \
         }
-        // Legs in the order x3, x2, x1, x0.  The stage is handed back to the producer ONCE, after the last leg:
-        // every lane's loads precede the warp barrier, lane 0's arrives (release) follow it and depend on the
-        // data of the last legs' loads (tma.cuh: mbar_arrive_after8).  Releasing the face regions early, right
-        // after the two legs that read them (as dhop_staged.cu does), was measured 4 % faster here but gave
-        // wrong results in the last slice of a tile as soon as two regions were released early (r02 notes in
-        // DESIGN.md): not understood, so not used.
+        // Legs in the order x3, x2, x1, x0.  The stage is handed back to the producer ONCE, after the last leg: warp
+        // barrier, then lane 0's four arrives, whose addresses are computed from acc[0].x and acc[3].x (spin components 0
+        // and 1 of the rotated colour 0: together they derive from all four loads of every leg), so that no arrive can issue
+        // while a load of the stage is in flight (tma.cuh: mbar_arrive_dep).  Releasing the face regions right after the two
+        // legs that read them (as dhop_staged.cu does) is correct with the same kind of arrive but not faster here (1033 vs
+        // 1025 us), so it is not used.
         uint32_t ua[3][4], ub[3][4];
         DWF_TLOAD(6, ua)
         DWF_TLOAD(7, ub)
@@ -434,10 +435,10 @@ __device__ __forceinline__ void consume64(const Staged64Args &args, unsigned cha
         DWF_LEG64(1, 0, false, false, ub, -1)
         __syncwarp();
         if (lane == 0) {
-            mbar_arrive(eb);
-            mbar_arrive(eb + 8);
-            mbar_arrive(eb + 16);
-            mbar_arrive_after8(eb + 24, q0_0.x, q0_1.x, q0_2.x, q0_3.x, q1_0.x, q1_1.x, q1_2.x, q1_3.x);
+            mbar_arrive_dep(eb, args.zero, acc[0].x, acc[3].x);
+            mbar_arrive_dep(eb + 8, args.zero, acc[0].x, acc[3].x);
+            mbar_arrive_dep(eb + 16, args.zero, acc[0].x, acc[3].x);
+            mbar_arrive_dep(eb + 24, args.zero, acc[0].x, acc[3].x);
         }
 #undef DWF_LOAD64
 #undef DWF_LEG64
@@ -782,6 +783,7 @@ int launch_dhop_staged64(const dwf_geometry *g, const void *in, void *out, int p
     a.parity_out = parity_out;
     a.zigzag = g->opt_zigzag;
     a.l2pol = g->opt_l2pol;
+    a.zero = 0;
     a.axpy_x = static_cast<const double2 *>(axpy_x);
     a.axpy_a = axpy_a;
     a.axpy_b = axpy_b;

@@ -31,31 +31,32 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-// Arrive that is issued only after the shared-memory loads whose results are passed in have returned
-// their data (the values are unused inputs of the asm statement, so the instruction depends on them).
-// This is how a consumer hands a staged region back to the TMA producer right after READING it: a plain
-// arrive placed behind the loads in program order may execute while they are still in flight (ptxas
-// does not make SYNCS.ARRIVE wait for earlier LDS, and __syncwarp() compiles to nothing in converged
-// code), and the refilling bulk copy -- async proxy -- then overwrites the data before it is read;
-// observed on the fp64 kernel as stale last-issued loads.  One 32-bit word of every load instruction is
-// enough: a warp-wide LDS releases its scoreboard when all lanes have their data.
-__device__ __forceinline__ void mbar_arrive_after8(uint32_t bar, double a, double b, double c, double d, double e, double f,
-                                                   double g, double h)
+// Release of a staged region by a consumer: an arrive that CANNOT issue before the shared-memory loads of the region
+// have delivered their data.  Program order is not enough: ptxas does not make SYNCS.ARRIVE wait for earlier LDS,
+// __syncwarp() compiles to nothing in converged code, and an asm statement that merely lists the loaded values as unused
+// operands keeps them alive for the C++ front end only (the PTX text of the arrive does not mention them).  With a bare
+// arrive the fp64 kernel read data of the NEXT fill in the last-issued load of a leg (r02: found with a field whose value
+// encodes its slice).  Here the barrier ADDRESS is computed from witness values that derive from every load of the region:
+// addr = bar + (bits(w) & zero), where `zero` is a kernel argument that is 0 at run time, so ptxas cannot fold the term
+// away and the arrive depends on the data.  A warp-wide LDS releases its scoreboard when all lanes have their data, so
+// lane 0's witness covers the warp; __syncwarp() in front of it states the same for the memory model.
+// The float form has no "memory" clobber: the loads of the region are tied to the arrive by the data dependence, and
+// the loads of other regions (the next legs) stay free to move across it.
+__device__ __forceinline__ void mbar_arrive_dep(uint32_t bar, uint32_t zero, float w)
 {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar), "d"(a), "d"(b), "d"(c), "d"(d), "d"(e), "d"(f), "d"(g),
-                 "d"(h) : "memory");
+    asm volatile(
+        "{\n\t.reg .b32 t;\n\t"
+        "mov.b32 t, %2;\n\tand.b32 t, t, %1;\n\tadd.u32 t, t, %0;\n\t"
+        "mbarrier.arrive.shared::cta.b64 _, [t];\n\t}"
+        ::"r"(bar), "r"(zero), "f"(w));
 }
-// the same with one witness: a value that the arithmetic has derived from EVERY load of the region (the staged fp32
-// kernel passes an accumulator component, which depends on a word of each of the twelve 128-bit loads of a leg pair)
-__device__ __forceinline__ void mbar_arrive_after1(uint32_t bar, float witness)
+__device__ __forceinline__ void mbar_arrive_dep(uint32_t bar, uint32_t zero, double a, double b)
 {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar), "f"(witness) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_after12(uint32_t bar, float a, float b, float c, float d, float e, float f, float g,
-                                                    float h, float i, float j, float k, float l)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar), "f"(a), "f"(b), "f"(c), "f"(d), "f"(e), "f"(f), "f"(g),
-                 "f"(h), "f"(i), "f"(j), "f"(k), "f"(l) : "memory");
+    asm volatile(
+        "{\n\t.reg .b32 la, lb, hh, t;\n\t"
+        "mov.b64 {la, hh}, %2;\n\tmov.b64 {lb, hh}, %3;\n\tor.b32 t, la, lb;\n\tand.b32 t, t, %1;\n\tadd.u32 t, t, %0;\n\t"
+        "mbarrier.arrive.shared::cta.b64 _, [t];\n\t}"
+        ::"r"(bar), "r"(zero), "d"(a), "d"(b) : "memory");
 }
 // blocks until the phase with the given parity has completed
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
