@@ -17,6 +17,10 @@
 // Everything else follows dhop_staged.cu: a producer warpgroup (setmaxnreg) issues 5-D bulk tensor
 // copies (TMA) of the input slice -- rows box + 6 faces -- into a two-stage shared-memory ring with
 // full / empty mbarriers; consumers walk all Ls slices of a tile with their link columns in registers.
+// TMEM variant (template flag TM, tiles of 128 sites, preferred when the lattice fits): the link columns and the
+// exchanged partial sums live in tensor memory (tcgen05.alloc / st / ld, shape 32x32b, as thread-private storage:
+// "tensor memory as thread-private storage" below), which frees 96 registers and the shared-memory exchange buffer:
+// twelve consumer warps instead of six and a 4x instead of 5x halo.
 // Layouts (pack.cu): spinor complex[s][row][k][h], k = spin*3 + colour (one plane per component:
 // consecutive sites are consecutive 128-bit words); links
 // complex[row][f/2][h][f&1], f = leg*9 + a*3 + b.
