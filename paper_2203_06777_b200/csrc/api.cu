@@ -273,7 +273,8 @@ int dwf_kernel_info(const dwf_geometry *g, char *buf, size_t n)
     if (!g || !buf || n == 0) { set_error("dwf_kernel_info: bad argument"); return DWF_ERR_INVALID_ARG; }
     const bool s32 = g->staged.variant >= 0 && g->opt_kernel != 1, s64 = g->staged64.variant >= 0 && g->opt_kernel != 1;
     if (s32)      snprintf(buf, n, "dhop_staged_kernel<%d,%d,%d,%d>", g->lat.Lh, g->staged.b[0], g->staged.b[1], g->staged.b[2]);
-    else if (s64) snprintf(buf, n, "dhop_staged64_kernel<%d,%d,%d,%d>", g->lat.Lh, g->staged64.b[0], g->staged64.b[1], g->staged64.b[2]);
+    else if (s64) snprintf(buf, n, "dhop_staged64%s_kernel<%d,%d,%d,%d>", g->staged64.kind == 2 ? "s" : (g->staged64.kind == 1 ? "t" : ""), g->lat.Lh,
+                           g->staged64.b[0], g->staged64.b[1], g->staged64.b[2]);
     else          snprintf(buf, n, "dhop_direct_kernel<%s>", g->prec == DWF_F32 ? "float" : "double");
     return DWF_OK;
 }

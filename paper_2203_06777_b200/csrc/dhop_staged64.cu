@@ -615,6 +615,327 @@ dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_con
     }
 }
 
+// =============================================================================================
+// Site-per-thread TMEM variant ("S"): ONE thread per output site, as in the fp32 kernel, with all 8 links of the
+// site (72 complex = 288 words) parked in the thread's tensor-memory lane instead of in registers.  No colour split:
+// no repeated accumulation (840 instead of 1248 fp64 operations per site), no exchange, no exchange barriers.  A CTA is
+// the producer warpgroup plus FOUR consumer warps (128 sites, one warp per TMEM lane quadrant); the FP64 pipe has 64
+// lanes per SM, so four warps with the instruction-level parallelism of a whole SU(3) x half-spinor product each keep it
+// busy.  The links of leg L + 1 are requested from tensor memory right after leg L's have been unpacked and land
+// during leg L's arithmetic.  TMEM columns [36 L, 36 L + 36) of a lane: the 9 complex numbers U_ab (a*3 + b) of leg L.
+// =============================================================================================
+template <int LH, int B1, int B2, int B3> struct Staged64SCfg {
+    static constexpr int NROW_C = B1 * B2 * B3;
+    static constexpr int T = LH * NROW_C;                        // output sites per tile = consumer threads
+    static constexpr int NWARP_C = T / 32;
+    static constexpr int NT = 128 + T;
+    static constexpr int ROWB = 12 * LH * 16;
+    static constexpr int R_X1M = NROW_C, R_X1P = R_X1M + B2 * B3, R_X2M = R_X1P + B2 * B3,
+                         R_X2P = R_X2M + B1 * B3, R_X3M = R_X2P + B1 * B3, R_X3P = R_X3M + B1 * B2,
+                         NROW_IN = R_X3P + B1 * B2;
+    static constexpr int STAGE_BYTES = NROW_IN * ROWB;
+    static constexpr int NSTAGE = 2;
+    // tail: full[2] (16 B), empty[2] (16 B), TMEM base (8 B), one fp64 slot per consumer warp (fused norm2)
+    static constexpr int TAIL_TMEM = 32, TAIL_NORM = 40, TAIL = TAIL_NORM + 8 * NWARP_C;
+    static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + (TAIL + 15) / 16 * 16;
+    static_assert(T == 128, "one consumer warp per TMEM lane quadrant: 128 sites per tile");
+    static_assert(SMEM_BYTES <= 232448, "tile too large for shared memory");
+};
+
+// the 36 words of one link: an x32 and an x4 load
+__device__ __forceinline__ void tmem_ld36(uint32_t taddr, uint32_t (&r)[36])
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]), "=r"(r[10]),
+                   "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]),
+                   "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+                 : "r"(taddr));
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(r[32]), "=r"(r[33]), "=r"(r[34]), "=r"(r[35]) : "r"(taddr + 32));
+}
+__device__ __forceinline__ void tmem_wait_ld_regs36(uint32_t (&r)[36])
+{
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]), "+r"(r[8]), "+r"(r[9]), "+r"(r[10]),
+                   "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15]), "+r"(r[16]), "+r"(r[17]), "+r"(r[18]), "+r"(r[19]), "+r"(r[20]),
+                   "+r"(r[21]), "+r"(r[22]), "+r"(r[23]), "+r"(r[24]), "+r"(r[25]), "+r"(r[26]), "+r"(r[27]), "+r"(r[28]), "+r"(r[29]), "+r"(r[30]),
+                   "+r"(r[31]), "+r"(r[32]), "+r"(r[33]), "+r"(r[34]), "+r"(r[35]));
+}
+
+// one whole leg for one site: acc += reconstruct( U * project(psi) ), psi[spin][colour], U[a*3 + b], acc[spin*3 + colour]
+template <int MU, bool FWD, bool FIRST>
+__device__ __forceinline__ void leg64_site(double2 (&acc)[12], const double2 (&psi)[4][3], const double2 (&U)[9])
+{
+    double2 h[2][3];
+#pragma unroll
+    for (int c = 0; c < 3; c++) {
+        if constexpr (MU == 0) {
+            h[0][c] = FWD ? csubi(psi[0][c], psi[3][c]) : caddi(psi[0][c], psi[3][c]);
+            h[1][c] = FWD ? csubi(psi[1][c], psi[2][c]) : caddi(psi[1][c], psi[2][c]);
+        } else if constexpr (MU == 1) {
+            h[0][c] = FWD ? cadd(psi[0][c], psi[3][c]) : csub(psi[0][c], psi[3][c]);
+            h[1][c] = FWD ? csub(psi[1][c], psi[2][c]) : cadd(psi[1][c], psi[2][c]);
+        } else if constexpr (MU == 2) {
+            h[0][c] = FWD ? csubi(psi[0][c], psi[2][c]) : caddi(psi[0][c], psi[2][c]);
+            h[1][c] = FWD ? caddi(psi[1][c], psi[3][c]) : csubi(psi[1][c], psi[3][c]);
+        } else {
+            h[0][c] = FWD ? csub(psi[0][c], psi[2][c]) : cadd(psi[0][c], psi[2][c]);
+            h[1][c] = FWD ? csub(psi[1][c], psi[3][c]) : cadd(psi[1][c], psi[3][c]);
+        }
+    }
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+        const double2 x0 = cmac(cmac(cmul(U[3 * a], h[0][0]), U[3 * a + 1], h[0][1]), U[3 * a + 2], h[0][2]);
+        const double2 x1 = cmac(cmac(cmul(U[3 * a], h[1][0]), U[3 * a + 1], h[1][1]), U[3 * a + 2], h[1][2]);
+        if constexpr (FIRST) {
+            acc[0 + a] = x0;
+            acc[3 + a] = x1;
+            if constexpr (MU == 0) {
+                acc[6 + a] = FWD ? cmuli(x1) : cmulni(x1);
+                acc[9 + a] = FWD ? cmuli(x0) : cmulni(x0);
+            } else if constexpr (MU == 1) {
+                acc[6 + a] = FWD ? cneg(x1) : x1;
+                acc[9 + a] = FWD ? x0 : cneg(x0);
+            } else if constexpr (MU == 2) {
+                acc[6 + a] = FWD ? cmuli(x0) : cmulni(x0);
+                acc[9 + a] = FWD ? cmulni(x1) : cmuli(x1);
+            } else {
+                acc[6 + a] = FWD ? cneg(x0) : x0;
+                acc[9 + a] = FWD ? cneg(x1) : x1;
+            }
+        } else {
+            acc[0 + a] = cadd(acc[0 + a], x0);
+            acc[3 + a] = cadd(acc[3 + a], x1);
+            if constexpr (MU == 0) {
+                acc[6 + a] = FWD ? caddi(acc[6 + a], x1) : csubi(acc[6 + a], x1);
+                acc[9 + a] = FWD ? caddi(acc[9 + a], x0) : csubi(acc[9 + a], x0);
+            } else if constexpr (MU == 1) {
+                acc[6 + a] = FWD ? csub(acc[6 + a], x1) : cadd(acc[6 + a], x1);
+                acc[9 + a] = FWD ? cadd(acc[9 + a], x0) : csub(acc[9 + a], x0);
+            } else if constexpr (MU == 2) {
+                acc[6 + a] = FWD ? caddi(acc[6 + a], x0) : csubi(acc[6 + a], x0);
+                acc[9 + a] = FWD ? csubi(acc[9 + a], x1) : caddi(acc[9 + a], x1);
+            } else {
+                acc[6 + a] = FWD ? csub(acc[6 + a], x0) : cadd(acc[6 + a], x0);
+                acc[9 + a] = FWD ? csub(acc[9 + a], x1) : cadd(acc[9 + a], x1);
+            }
+        }
+    }
+}
+
+template <int LH, int B1, int B2, int B3, int MODE>
+__global__ void __launch_bounds__(Staged64SCfg<LH, B1, B2, B3>::NT, 1)
+dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_constant__ CUtensorMap map_x1,
+                      const __grid_constant__ CUtensorMap map_x2, const __grid_constant__ CUtensorMap map_x3,
+                      const Staged64Args args)
+{
+    using Cfg = Staged64SCfg<LH, B1, B2, B3>;
+    constexpr bool DAG = (MODE & 1) != 0, AXPY = (MODE & 2) != 0, NORM = (MODE & 4) != 0;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    const uint32_t smem_base = smem_u32(smem);
+    const uint32_t full_base = smem_base + Cfg::NSTAGE * Cfg::STAGE_BYTES;        // full[2]
+    const uint32_t empty_base = full_base + 16;                                   // empty[2]
+    uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + Cfg::TAIL_TMEM);
+    const int tid = threadIdx.x;
+    const int my_tiles = (args.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    const int nsteps = my_tiles * args.Ls;
+    if (nsteps <= 0) {
+        if (NORM && tid == 0) args.norm_partials[blockIdx.x] = 0.0;
+        return;
+    }
+    if (tid == 0) {
+        tma_prefetch_desc(&map_c);
+        tma_prefetch_desc(&map_x1);
+        tma_prefetch_desc(&map_x2);
+        tma_prefetch_desc(&map_x3);
+        for (int i = 0; i < 2; i++) {
+            mbar_init(full_base + 8 * i, 1);
+            mbar_init(empty_base + 8 * i, Cfg::NWARP_C);
+        }
+        mbar_fence_init();
+    }
+    if (tid < 32) {         // warp 0 allocates the tensor memory (one CTA per SM: all 512 columns)
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(512) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tmem_fence_before();
+    __syncthreads();
+    tmem_fence_after();
+    const uint32_t tmem_base = *tmem_slot;
+
+    if (tid < 128) {        // producer warpgroup: thread 0 issues the seven boxes of every step
+        if (tid >= 32) return;
+        if (tid == 0) {
+            const int L1 = args.L1, L2 = args.L2, L3 = args.L3;
+            const uint64_t pol_last = l2_policy(args.l2pol % 10);
+            for (int g = 0; g < nsteps; g++) {
+                const int it = g / args.Ls, i = g % args.Ls, stage = g & 1;
+                const int s = (args.zigzag && (it & 1)) ? args.Ls - 1 - i : i;
+                const int4 o = args.tiles[blockIdx.x + it * gridDim.x];
+                const uint32_t bar = full_base + 8 * stage;
+                const uint32_t dst = smem_base + stage * Cfg::STAGE_BYTES;
+                const int sb = s * L3;
+                const int x1m = o.x == 0 ? L1 - 1 : o.x - 1, x1p = o.x + B1 == L1 ? 0 : o.x + B1;
+                const int x2m = o.y == 0 ? L2 - 1 : o.y - 1, x2p = o.y + B2 == L2 ? 0 : o.y + B2;
+                const int x3m = o.z == 0 ? L3 - 1 : o.z - 1, x3p = o.z + B3 == L3 ? 0 : o.z + B3;
+                const int c4 = sb + o.z;
+                if (g >= 2) mbar_wait(empty_base + 8 * stage, ((g >> 1) - 1) & 1);
+                mbar_arrive_expect_tx(bar, Cfg::STAGE_BYTES);
+                tma_load_5d_hint(dst + Cfg::R_X3M * Cfg::ROWB, &map_x3, bar, 0, 0, o.x, o.y, sb + x3m, pol_last);
+                tma_load_5d_hint(dst + Cfg::R_X3P * Cfg::ROWB, &map_x3, bar, 0, 0, o.x, o.y, sb + x3p, pol_last);
+                tma_load_5d_hint(dst + Cfg::R_X2M * Cfg::ROWB, &map_x2, bar, 0, 0, o.x, x2m, c4, pol_last);
+                tma_load_5d_hint(dst + Cfg::R_X2P * Cfg::ROWB, &map_x2, bar, 0, 0, o.x, x2p, c4, pol_last);
+                tma_load_5d_hint(dst + Cfg::R_X1M * Cfg::ROWB, &map_x1, bar, 0, 0, x1m, o.y, c4, pol_last);
+                tma_load_5d_hint(dst + Cfg::R_X1P * Cfg::ROWB, &map_x1, bar, 0, 0, x1p, o.y, c4, pol_last);
+                tma_load_5d_hint(dst, &map_c, bar, 0, 0, o.x, o.y, c4, pol_last);
+            }
+        }
+        __syncwarp();       // warp 0 frees the tensor memory once every consumer warp is done with it
+        asm volatile("bar.sync 2, %0;" ::"n"((Cfg::NWARP_C + 1) * 32) : "memory");
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(512) : "memory");
+        return;
+    }
+
+    // =========================== consumers: one thread = one output site ===========================
+    const int site = tid - 128;
+    const int h = site % LH, row = site / LH;
+    const int i1 = row % B1, i2 = (row / B1) % B2, i3 = row / (B1 * B2);
+    const int lane = tid & 31;
+    const uint64_t pol_first = l2_policy(args.l2pol / 1000000 % 10), pol_out = l2_policy(args.l2pol / 10000000 % 10);
+    const int rc = row;
+    const int r1p = (i1 + 1 < B1) ? rc + 1 : Cfg::R_X1P + i2 + B2 * i3;
+    const int r1m = (i1 > 0) ? rc - 1 : Cfg::R_X1M + i2 + B2 * i3;
+    const int r2p = (i2 + 1 < B2) ? rc + B1 : Cfg::R_X2P + i1 + B1 * i3;
+    const int r2m = (i2 > 0) ? rc - B1 : Cfg::R_X2M + i1 + B1 * i3;
+    const int r3p = (i3 + 1 < B3) ? rc + B1 * B2 : Cfg::R_X3P + i1 + B1 * i2;
+    const int r3m = (i3 > 0) ? rc - B1 * B2 : Cfg::R_X3M + i1 + B1 * i2;
+    uint32_t off[8];            // byte offsets of (neighbour site, component 0) inside a stage; component k at + k * KB
+    constexpr uint32_t KB = LH * 16;
+    off[2] = r1p * Cfg::ROWB + h * 16;
+    off[3] = r1m * Cfg::ROWB + h * 16;
+    off[4] = r2p * Cfg::ROWB + h * 16;
+    off[5] = r2m * Cfg::ROWB + h * 16;
+    off[6] = r3p * Cfg::ROWB + h * 16;
+    off[7] = r3m * Cfg::ROWB + h * 16;
+    const long long nrow = (long long)args.L1 * args.L2 * args.L3;
+    // this thread's TMEM lane: consumer warp w (CTA warp 4 + w) sits in lane quadrant w
+    const uint32_t tm_links = tmem_base + ((uint32_t)((site >> 5) * 32) << 16);
+
+    auto tile_row = [&](int it, int &r) -> long long {
+        const int4 o = args.tiles[blockIdx.x + it * gridDim.x];
+        const int x1 = o.x + i1, x2 = o.y + i2, x3 = o.z + i3;
+        r = (x1 + x2 + x3 + args.parity_out) & 1;
+        return x1 + (long long)args.L1 * (x2 + (long long)args.L2 * x3);
+    };
+    auto set_x0_offsets = [&](int r) {
+        int hp = h + r;       if (hp == LH) hp = 0;
+        int hm = h - 1 + r;   if (hm < 0) hm = LH - 1;
+        off[0] = rc * Cfg::ROWB + hp * 16;
+        off[1] = rc * Cfg::ROWB + hm * 16;
+    };
+    // the 72 link elements of the site: global -> tensor memory, leg by leg (9 loads in flight)
+    auto load_links = [&](long long grow) {
+        const double2 *gp = args.gauge + grow * (72 * LH) + 2 * h;
+#pragma unroll
+        for (int leg = 0; leg < 8; leg++) {
+            double2 t[9];
+#pragma unroll
+            for (int k = 0; k < 9; k++) {
+                const int f = leg * 9 + k;
+                t[k] = ldg_d2_hint(gp + (f >> 1) * 2 * LH + (f & 1), pol_first);
+            }
+#pragma unroll
+            for (int k = 0; k < 9; k++) tmem_st_c(tm_links + 36 * leg + 4 * k, t[k]);
+        }
+        tmem_wait_st();
+    };
+
+    double nsum = 0.0;
+    int r_cur;
+    long long grow = tile_row(0, r_cur);
+    set_x0_offsets(r_cur);
+    load_links(grow);
+
+    int g = 0;
+    for (int it = 0; it < my_tiles; it++) {
+        const bool has_next = it + 1 < my_tiles;
+        int r_next = r_cur;
+        long long grow_next = grow;
+        if (has_next) grow_next = tile_row(it + 1, r_next);
+        for (int ss = 0; ss < args.Ls; ss++, g++) {
+            const int s = (args.zigzag && (it & 1)) ? args.Ls - 1 - ss : ss;
+            const int stage = g & 1;
+            double2 *o2 = args.out + grow * (12 * LH) + h + (long long)s * nrow * (12 * LH);
+            mbar_wait(full_base + 8 * stage, (g >> 1) & 1);
+            const unsigned char *sb = smem + stage * Cfg::STAGE_BYTES;
+            double2 acc[12];
+            uint32_t W[36];
+            tmem_ld36(tm_links + 36 * 6, W);
+            double2 xv[12];
+            // one leg: the neighbour spinor out of shared memory, the link out of tensor memory (requested one leg
+            // ahead: right after this leg's link has been unpacked, the next one's load goes into the same registers)
+#define DWF_LEG64S(L, MU, FWD, FIRST, NEXT)                                                         \
+            {                                                                                       \
+                double2 psi[4][3];                                                                  \
+                _Pragma("unroll") for (int k = 0; k < 12; k++)                                      \
+                    psi[k / 3][k % 3] = *reinterpret_cast<const double2 *>(sb + off[L] + k * KB);   \
+                tmem_wait_ld_regs36(W);                                                             \
+                double2 Ul[9];                                                                      \
+                _Pragma("unroll") for (int k = 0; k < 9; k++) Ul[k] = tmem_unpack_p(W + 4 * k);     \
+                if constexpr ((NEXT) >= 0) tmem_ld36(tm_links + 36 * ((NEXT) < 0 ? 0 : (NEXT)), W); \
+                leg64_site<MU, (FWD) != DAG, FIRST>(acc, psi, Ul);                                  \
+            }
+            DWF_LEG64S(6, 3, true, true, 7)
+            DWF_LEG64S(7, 3, false, false, 4)
+            DWF_LEG64S(4, 2, true, false, 5)
+            DWF_LEG64S(5, 2, false, false, 2)
+            DWF_LEG64S(2, 1, true, false, 3)
+            DWF_LEG64S(3, 1, false, false, 0)
+            DWF_LEG64S(0, 0, true, false, 1)
+            if constexpr (AXPY) {       // x of this site and slice, requested before the last leg
+                const double2 *xp = args.axpy_x + (o2 - args.out);
+#pragma unroll
+                for (int k = 0; k < 12; k++) xv[k] = __ldcs(xp + k * LH);
+            }
+            DWF_LEG64S(1, 0, false, false, -1)
+#undef DWF_LEG64S
+            // hand the stage back: every accumulator spin row derives from all loads of all legs (acc[0], acc[3]: spin
+            // components 0 and 1 of colour 0 use all three colours of all four spin components of every neighbour)
+            __syncwarp();
+            if (lane == 0) mbar_arrive_dep(empty_base + 8 * stage, args.zero, acc[0].x, acc[3].x);
+#pragma unroll
+            for (int k = 0; k < 12; k++) {
+                double2 v = acc[k];
+                if constexpr (AXPY) {
+                    v.x = fma(args.axpy_b, v.x, args.axpy_a * xv[k].x);
+                    v.y = fma(args.axpy_b, v.y, args.axpy_a * xv[k].y);
+                }
+                if constexpr (NORM) nsum = fma(v.x, v.x, fma(v.y, v.y, nsum));
+                stg_d2_hint(o2 + k * LH, v, pol_out);
+            }
+        }
+        grow = grow_next;
+        r_cur = r_next;
+        set_x0_offsets(r_cur);
+        if (has_next) load_links(grow);
+    }
+
+    if constexpr (NORM) {
+        double v = nsum;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        double *slots = reinterpret_cast<double *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + Cfg::TAIL_NORM);
+        if (lane == 0) slots[site >> 5] = v;
+        asm volatile("bar.sync 1, %0;" ::"n"(Cfg::NWARP_C * 32) : "memory");
+        if (site == 0) {
+            double t = 0.0;
+            for (int w = 0; w < Cfg::NWARP_C; w++) t += slots[w];
+            args.norm_partials[blockIdx.x] = t;
+        }
+    }
+    tmem_fence_before();
+    asm volatile("bar.sync 2, %0;" ::"n"((Cfg::NWARP_C + 1) * 32) : "memory");
+}
+
 // ---------------------------------------------------------------------------------------------
 // Kernel instances: this file is compiled once per MODE (-DDWF_STAGED64_MODE=0..4, build.py); each
 // translation unit exports the entry points of its MODE in the order of DWF_STAGED64_VARIANTS, the
@@ -638,9 +959,12 @@ const void *const *DWF_CAT(staged64_kernels_mode, DWF_STAGED64_MODE)()
 {
 #define X(LH, B1, B2, B3) reinterpret_cast<const void *>(&dhop_staged64_kernel<LH, B1, B2, B3, DWF_STAGED64_MODE, true>),
 #define Y(LH, B1, B2, B3) reinterpret_cast<const void *>(&dhop_staged64_kernel<LH, B1, B2, B3, DWF_STAGED64_MODE, false>),
-    static const void *const tab[] = {DWF_STAGED64T_VARIANTS(X) DWF_STAGED64_VARIANTS(Y)};
+#define Z(LH, B1, B2, B3) reinterpret_cast<const void *>(&dhop_staged64s_kernel<LH, B1, B2, B3, DWF_STAGED64_MODE>),
+    // order of preference: site-per-thread TMEM kernels, colour-split TMEM kernels, colour-split register kernels
+    static const void *const tab[] = {DWF_STAGED64T_VARIANTS(Z) DWF_STAGED64T_VARIANTS(X) DWF_STAGED64_VARIANTS(Y)};
 #undef X
 #undef Y
+#undef Z
     return tab;
 }
 
@@ -659,6 +983,11 @@ static const std::vector<Variant64> &variants64()
         std::vector<Variant64> t;
         const void *const *k0 = staged64_kernels_mode0(), *const *k1 = staged64_kernels_mode1(), *const *k2 = staged64_kernels_mode2(),
                           *const *k3 = staged64_kernels_mode3(), *const *k4 = staged64_kernels_mode4();
+#define X(LH, B1, B2, B3)                                                                             \
+        t.push_back({LH, B1, B2, B3, Staged64SCfg<LH, B1, B2, B3>::SMEM_BYTES, Staged64SCfg<LH, B1, B2, B3>::NT, 2, \
+                     {k0[t.size()], k1[t.size()], k2[t.size()], k3[t.size()], k4[t.size()]}});
+        DWF_STAGED64T_VARIANTS(X)
+#undef X
 #define X(LH, B1, B2, B3)                                                                             \
         t.push_back({LH, B1, B2, B3, Staged64Cfg<LH, B1, B2, B3, true>::SMEM_BYTES, Staged64Cfg<LH, B1, B2, B3, true>::NT, 1, \
                      {k0[t.size()], k1[t.size()], k2[t.size()], k3[t.size()], k4[t.size()]}});
@@ -685,6 +1014,7 @@ void plan_staged64(dwf_geometry *g)
         if (lat.L[1] % v[i].b1 || lat.L[2] % v[i].b2 || lat.L[3] % v[i].b3) continue;
         if (g->opt_variant > 0 && (int)i + 1 != g->opt_variant) continue;
         g->staged64.variant = (int)i;
+        g->staged64.kind = v[i].tmem;
         g->staged64.b[0] = v[i].b1; g->staged64.b[1] = v[i].b2; g->staged64.b[2] = v[i].b3;
         g->staged64.ntiles = (lat.L[1] / v[i].b1) * (lat.L[2] / v[i].b2) * (lat.L[3] / v[i].b3);
         // per-device opt-in to the large dynamic shared memory (the caller holds a DeviceGuard)

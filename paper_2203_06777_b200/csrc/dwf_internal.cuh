@@ -54,6 +54,7 @@ struct Tiling {
 // holds the Lh output sites of one parity of a lattice line along x0) and all Ls slices.
 struct StagedPlan {
     int variant;     // index into the table of compiled (Lh, B1, B2, B3) instances, -1: not usable
+    int kind;        // fp64 only: 0 colour split in registers, 1 colour split in tensor memory, 2 one thread per site, links in tensor memory
     int b[3];        // rows box
     int ntiles;
 };

@@ -371,7 +371,7 @@ def test_staged64_fp64_kernel(lib, dims, Ls, bc):
     with lib.Geometry(dims, Ls, 8, bc) as g:
         g.load_gauge(U)
         g.set_option("kernel", 2)
-        assert g.kernel_info().startswith("dhop_staged64_kernel")
+        assert g.kernel_info().startswith("dhop_staged64")
         fin, fx = g.import_spinor(half, lib.EVEN), g.import_spinor(xh, lib.ODD)
         want = oracle.dhop_cb(dims, Ls, bc, 1, U, half)
         a = g.dhop_oe_dag(fin).clone()
