@@ -624,6 +624,9 @@ dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_con
 // busy.  The links of leg L + 1 are requested from tensor memory right after leg L's have been unpacked and land
 // during leg L's arithmetic.  TMEM columns [36 L, 36 L + 36) of a lane: the 9 complex numbers U_ab (a*3 + b) of leg L.
 // =============================================================================================
+#ifndef DWF_S_LEGS
+#define DWF_S_LEGS 4            // legs of the link load in flight at a tile switch
+#endif
 template <int LH, int B1, int B2, int B3> struct Staged64SCfg {
     static constexpr int NROW_C = B1 * B2 * B3;
     static constexpr int T = LH * NROW_C;                        // output sites per tile = consumer threads
@@ -635,8 +638,10 @@ template <int LH, int B1, int B2, int B3> struct Staged64SCfg {
                          NROW_IN = R_X3P + B1 * B2;
     static constexpr int STAGE_BYTES = NROW_IN * ROWB;
     static constexpr int NSTAGE = 2;
-    // tail: full[2] (16 B), empty[2] (16 B), TMEM base (8 B), one fp64 slot per consumer warp (fused norm2)
-    static constexpr int TAIL_TMEM = 32, TAIL_NORM = 40, TAIL = TAIL_NORM + 8 * NWARP_C;
+    // regions of a stage, in the order the consumers finish with them: x3 faces, x2 faces, x1 faces, centre
+    static constexpr int NREG = 4;
+    // tail: full[2] (16 B), empty[2][4] (64 B), TMEM base (8 B), one fp64 slot per consumer warp (fused norm2)
+    static constexpr int TAIL_TMEM = 80, TAIL_NORM = 88, TAIL = TAIL_NORM + 8 * NWARP_C;
     static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + (TAIL + 15) / 16 * 16;
     static_assert(T == 128, "one consumer warp per TMEM lane quadrant: 128 sites per tile");
     static_assert(SMEM_BYTES <= 232448, "tile too large for shared memory");
@@ -733,7 +738,7 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
     extern __shared__ __align__(1024) unsigned char smem[];
     const uint32_t smem_base = smem_u32(smem);
     const uint32_t full_base = smem_base + Cfg::NSTAGE * Cfg::STAGE_BYTES;        // full[2]
-    const uint32_t empty_base = full_base + 16;                                   // empty[2]
+    const uint32_t empty_base = full_base + 16;                                   // empty[2][4]
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + Cfg::TAIL_TMEM);
     const int tid = threadIdx.x;
     const int my_tiles = (args.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
@@ -748,8 +753,8 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
         tma_prefetch_desc(&map_x2);
         tma_prefetch_desc(&map_x3);
         for (int i = 0; i < 2; i++) {
-            mbar_init(full_base + 8 * i, 1);
-            mbar_init(empty_base + 8 * i, Cfg::NWARP_C);
+            mbar_init(full_base + 8 * i, Cfg::NREG);           // one arrive.expect_tx per region
+            for (int r = 0; r < Cfg::NREG; r++) mbar_init(empty_base + 8 * (Cfg::NREG * i + r), Cfg::NWARP_C);
         }
         mbar_fence_init();
     }
@@ -778,14 +783,23 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
                 const int x2m = o.y == 0 ? L2 - 1 : o.y - 1, x2p = o.y + B2 == L2 ? 0 : o.y + B2;
                 const int x3m = o.z == 0 ? L3 - 1 : o.z - 1, x3p = o.z + B3 == L3 ? 0 : o.z + B3;
                 const int c4 = sb + o.z;
-                if (g >= 2) mbar_wait(empty_base + 8 * stage, ((g >> 1) - 1) & 1);
-                mbar_arrive_expect_tx(bar, Cfg::STAGE_BYTES);
+                // every region is refilled as soon as the four consumer warps have handed it back
+                const uint32_t eb = empty_base + 8 * Cfg::NREG * stage;
+                const uint32_t ph = ((g >> 1) - 1) & 1;
+                if (g >= 2) mbar_wait(eb, ph);
+                mbar_arrive_expect_tx(bar, 2 * B1 * B2 * Cfg::ROWB);
                 tma_load_5d_hint(dst + Cfg::R_X3M * Cfg::ROWB, &map_x3, bar, 0, 0, o.x, o.y, sb + x3m, pol_last);
                 tma_load_5d_hint(dst + Cfg::R_X3P * Cfg::ROWB, &map_x3, bar, 0, 0, o.x, o.y, sb + x3p, pol_last);
+                if (g >= 2) mbar_wait(eb + 8, ph);
+                mbar_arrive_expect_tx(bar, 2 * B1 * B3 * Cfg::ROWB);
                 tma_load_5d_hint(dst + Cfg::R_X2M * Cfg::ROWB, &map_x2, bar, 0, 0, o.x, x2m, c4, pol_last);
                 tma_load_5d_hint(dst + Cfg::R_X2P * Cfg::ROWB, &map_x2, bar, 0, 0, o.x, x2p, c4, pol_last);
+                if (g >= 2) mbar_wait(eb + 16, ph);
+                mbar_arrive_expect_tx(bar, 2 * B2 * B3 * Cfg::ROWB);
                 tma_load_5d_hint(dst + Cfg::R_X1M * Cfg::ROWB, &map_x1, bar, 0, 0, x1m, o.y, c4, pol_last);
                 tma_load_5d_hint(dst + Cfg::R_X1P * Cfg::ROWB, &map_x1, bar, 0, 0, x1p, o.y, c4, pol_last);
+                if (g >= 2) mbar_wait(eb + 24, ph);
+                mbar_arrive_expect_tx(bar, Cfg::NROW_C * Cfg::ROWB);
                 tma_load_5d_hint(dst, &map_c, bar, 0, 0, o.x, o.y, c4, pol_last);
             }
         }
@@ -832,19 +846,21 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
         off[0] = rc * Cfg::ROWB + hp * 16;
         off[1] = rc * Cfg::ROWB + hm * 16;
     };
-    // the 72 link elements of the site: global -> tensor memory, leg by leg (9 loads in flight)
+    // the 72 link elements of the site: global -> tensor memory, DWF_S_LEGS legs (9 loads each) in flight at a time;
+    // between tiles the accumulator and spinor registers are free
     auto load_links = [&](long long grow) {
         const double2 *gp = args.gauge + grow * (72 * LH) + 2 * h;
+        constexpr int NB = 9 * DWF_S_LEGS;
 #pragma unroll
-        for (int leg = 0; leg < 8; leg++) {
-            double2 t[9];
+        for (int b = 0; b < 72 / NB; b++) {
+            double2 t[NB];
 #pragma unroll
-            for (int k = 0; k < 9; k++) {
-                const int f = leg * 9 + k;
+            for (int k = 0; k < NB; k++) {
+                const int f = b * NB + k;
                 t[k] = ldg_d2_hint(gp + (f >> 1) * 2 * LH + (f & 1), pol_first);
             }
 #pragma unroll
-            for (int k = 0; k < 9; k++) tmem_st_c(tm_links + 36 * leg + 4 * k, t[k]);
+            for (int k = 0; k < NB; k++) tmem_st_c(tm_links + 4 * (b * NB + k), t[k]);
         }
         tmem_wait_st();
     };
@@ -884,12 +900,21 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
                 if constexpr ((NEXT) >= 0) tmem_ld36(tm_links + 36 * ((NEXT) < 0 ? 0 : (NEXT)), W); \
                 leg64_site<MU, (FWD) != DAG, FIRST>(acc, psi, Ul);                                  \
             }
+            // a region goes back to the producer as soon as this warp's loads from it have completed: the accumulator
+            // rows acc[0], acc[3] (spin 0 and 1, colour 0) derive from all twelve components of every neighbour read
+            // so far, and the arrive's address is computed from them (tma.cuh, mbar_arrive_dep)
+#define DWF_RELEASE64S(R)                                                                           \
+            __syncwarp();                                                                           \
+            if (lane == 0) mbar_arrive_dep(empty_base + 8 * (Cfg::NREG * stage + (R)), args.zero, acc[0].x, acc[3].x);
             DWF_LEG64S(6, 3, true, true, 7)
             DWF_LEG64S(7, 3, false, false, 4)
+            DWF_RELEASE64S(0)
             DWF_LEG64S(4, 2, true, false, 5)
             DWF_LEG64S(5, 2, false, false, 2)
+            DWF_RELEASE64S(1)
             DWF_LEG64S(2, 1, true, false, 3)
             DWF_LEG64S(3, 1, false, false, 0)
+            DWF_RELEASE64S(2)
             DWF_LEG64S(0, 0, true, false, 1)
             if constexpr (AXPY) {       // x of this site and slice, requested before the last leg
                 const double2 *xp = args.axpy_x + (o2 - args.out);
@@ -898,10 +923,8 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
             }
             DWF_LEG64S(1, 0, false, false, -1)
 #undef DWF_LEG64S
-            // hand the stage back: every accumulator spin row derives from all loads of all legs (acc[0], acc[3]: spin
-            // components 0 and 1 of colour 0 use all three colours of all four spin components of every neighbour)
-            __syncwarp();
-            if (lane == 0) mbar_arrive_dep(empty_base + 8 * stage, args.zero, acc[0].x, acc[3].x);
+            DWF_RELEASE64S(3)
+#undef DWF_RELEASE64S
 #pragma unroll
             for (int k = 0; k < 12; k++) {
                 double2 v = acc[k];
