@@ -88,6 +88,12 @@ __device__ __forceinline__ double2 ldg_d2_hint(const double2 *p, uint64_t policy
     asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(policy));
     return v;
 }
+// two consecutive complex numbers (32 bytes, 32-byte aligned) in one 256-bit load
+__device__ __forceinline__ void ldg_d4_hint(const double2 *p, uint64_t policy, double2 &a, double2 &b)
+{
+    asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.f64 {%0, %1, %2, %3}, [%4], %5;"
+                 : "=d"(a.x), "=d"(a.y), "=d"(b.x), "=d"(b.y) : "l"(p), "l"(policy));
+}
 __device__ __forceinline__ void stg_d2_hint(double2 *p, double2 v, uint64_t policy)
 {
     asm volatile("st.global.L1::no_allocate.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(policy) : "memory");
@@ -846,19 +852,18 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
         off[0] = rc * Cfg::ROWB + hp * 16;
         off[1] = rc * Cfg::ROWB + hm * 16;
     };
-    // the 72 link elements of the site: global -> tensor memory, DWF_S_LEGS legs (9 loads each) in flight at a time;
-    // between tiles the accumulator and spinor registers are free
+    // the 72 link elements of the site: global -> tensor memory, DWF_S_LEGS legs in flight at a time (between tiles the
+    // accumulator and spinor registers are free).  Elements 2j and 2j + 1 of a site are adjacent in memory (pack.cu):
+    // one 256-bit load per pair, a warp reads whole 512-byte runs.
     auto load_links = [&](long long grow) {
         const double2 *gp = args.gauge + grow * (72 * LH) + 2 * h;
         constexpr int NB = 9 * DWF_S_LEGS;
+        static_assert(NB % 2 == 0 && 72 % NB == 0, "DWF_S_LEGS: 2, 4 or 8");
 #pragma unroll
         for (int b = 0; b < 72 / NB; b++) {
             double2 t[NB];
 #pragma unroll
-            for (int k = 0; k < NB; k++) {
-                const int f = b * NB + k;
-                t[k] = ldg_d2_hint(gp + (f >> 1) * 2 * LH + (f & 1), pol_first);
-            }
+            for (int k = 0; k < NB; k += 2) ldg_d4_hint(gp + (b * NB + k) * LH, pol_first, t[k], t[k + 1]);
 #pragma unroll
             for (int k = 0; k < NB; k++) tmem_st_c(tm_links + 4 * (b * NB + k), t[k]);
         }
