@@ -630,14 +630,16 @@ dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_con
 // busy.  The links of leg L + 1 are requested from tensor memory right after leg L's have been unpacked and land
 // during leg L's arithmetic.  TMEM columns [36 L, 36 L + 36) of a lane: the 9 complex numbers U_ab (a*3 + b) of leg L.
 // =============================================================================================
-#ifndef DWF_S_LEGS
-#define DWF_S_LEGS 4            // legs of the link load in flight at a tile switch
-#endif
 template <int LH, int B1, int B2, int B3> struct Staged64SCfg {
     static constexpr int NROW_C = B1 * B2 * B3;
     static constexpr int T = LH * NROW_C;                        // output sites per tile = consumer threads
     static constexpr int NWARP_C = T / 32;
-    static constexpr int NT = 128 + T;
+    // warpgroup 0: link loaders (one thread per site), warpgroup 1: consumers (one thread per site),
+    // warpgroup 2: its first warp issues the bulk tensor loads
+    static constexpr int NT = 384;
+    // register split (setmaxnreg): the loaders keep the 168 of the launch, the producer warpgroup gives up what the
+    // consumers take
+    static constexpr int CONS_REGS = 256, PROD_REGS = 40;
     static constexpr int ROWB = 12 * LH * 16;
     static constexpr int R_X1M = NROW_C, R_X1P = R_X1M + B2 * B3, R_X2M = R_X1P + B2 * B3,
                          R_X2P = R_X2M + B1 * B3, R_X3M = R_X2P + B1 * B3, R_X3P = R_X3M + B1 * B2,
@@ -646,8 +648,13 @@ template <int LH, int B1, int B2, int B3> struct Staged64SCfg {
     static constexpr int NSTAGE = 2;
     // regions of a stage, in the order the consumers finish with them: x3 faces, x2 faces, x1 faces, centre
     static constexpr int NREG = 4;
-    // tail: full[2] (16 B), empty[2][4] (64 B), TMEM base (8 B), one fp64 slot per consumer warp (fused norm2)
-    static constexpr int TAIL_TMEM = 80, TAIL_NORM = 88, TAIL = TAIL_NORM + 8 * NWARP_C;
+    // tensor memory: 14 slots of 36 columns (one link each).  Tile number t of a CTA keeps the link of the leg at
+    // position p of the leg order (6 7 4 5 2 3 0 1) in slot (8 t + p) mod 14: the first six links of the next tile go
+    // into the six slots this tile does not use, the last two into the slots of this tile's first two legs.
+    static constexpr int NSLOT = 14;
+    // tail: full[2] (16 B), empty[2][4] (64 B), four link barriers per lane quadrant (128 B: ready, early, free, done),
+    // TMEM base (8 B), one fp64 slot per consumer warp (fused norm2)
+    static constexpr int TAIL_LINK = 80, TAIL_TMEM = 208, TAIL_NORM = 216, TAIL = TAIL_NORM + 8 * NWARP_C;
     static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + (TAIL + 15) / 16 * 16;
     static_assert(T == 128, "one consumer warp per TMEM lane quadrant: 128 sites per tile");
     static_assert(SMEM_BYTES <= 232448, "tile too large for shared memory");
@@ -745,6 +752,7 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
     const uint32_t smem_base = smem_u32(smem);
     const uint32_t full_base = smem_base + Cfg::NSTAGE * Cfg::STAGE_BYTES;        // full[2]
     const uint32_t empty_base = full_base + 16;                                   // empty[2][4]
+    const uint32_t link_base = full_base + Cfg::TAIL_LINK;                        // [quadrant][ready, early, free, done]
     uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + Cfg::TAIL_TMEM);
     const int tid = threadIdx.x;
     const int my_tiles = (args.ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
@@ -754,17 +762,14 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
         return;
     }
     if (tid == 0) {
-        tma_prefetch_desc(&map_c);
-        tma_prefetch_desc(&map_x1);
-        tma_prefetch_desc(&map_x2);
-        tma_prefetch_desc(&map_x3);
         for (int i = 0; i < 2; i++) {
             mbar_init(full_base + 8 * i, Cfg::NREG);           // one arrive.expect_tx per region
             for (int r = 0; r < Cfg::NREG; r++) mbar_init(empty_base + 8 * (Cfg::NREG * i + r), Cfg::NWARP_C);
         }
+        for (int i = 0; i < 16; i++) mbar_init(link_base + 8 * i, 1);
         mbar_fence_init();
     }
-    if (tid < 32) {         // warp 0 allocates the tensor memory (one CTA per SM: all 512 columns)
+    if (tid >= 256 && tid < 288) {      // the producer warp allocates the tensor memory (one CTA per SM: all 512 columns)
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "n"(512) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
@@ -773,9 +778,14 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
     tmem_fence_after();
     const uint32_t tmem_base = *tmem_slot;
 
-    if (tid < 128) {        // producer warpgroup: thread 0 issues the seven boxes of every step
-        if (tid >= 32) return;
-        if (tid == 0) {
+    if (tid >= 256) {       // ===================== producer: one thread issues the seven boxes of every step =====
+        reg_dealloc<Cfg::PROD_REGS>();
+        if (tid >= 288) return;
+        if (tid == 256) {
+            tma_prefetch_desc(&map_c);
+            tma_prefetch_desc(&map_x1);
+            tma_prefetch_desc(&map_x2);
+            tma_prefetch_desc(&map_x3);
             const int L1 = args.L1, L2 = args.L2, L3 = args.L3;
             const uint64_t pol_last = l2_policy(args.l2pol % 10);
             for (int g = 0; g < nsteps; g++) {
@@ -809,18 +819,87 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
                 tma_load_5d_hint(dst, &map_c, bar, 0, 0, o.x, o.y, c4, pol_last);
             }
         }
-        __syncwarp();       // warp 0 frees the tensor memory once every consumer warp is done with it
-        asm volatile("bar.sync 2, %0;" ::"n"((Cfg::NWARP_C + 1) * 32) : "memory");
+        __syncwarp();       // this warp frees the tensor memory once the loaders and the consumers are done with it
+        asm volatile("bar.sync 2, %0;" ::"n"(288) : "memory");
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(512) : "memory");
         return;
     }
 
-    // =========================== consumers: one thread = one output site ===========================
-    const int site = tid - 128;
+    // loaders and consumers: thread <-> site of the tile, warp <-> TMEM lane quadrant
+    const int site = tid & 127;
     const int h = site % LH, row = site / LH;
     const int i1 = row % B1, i2 = (row / B1) % B2, i3 = row / (B1 * B2);
-    const int lane = tid & 31;
-    const uint64_t pol_first = l2_policy(args.l2pol / 1000000 % 10), pol_out = l2_policy(args.l2pol / 10000000 % 10);
+    const int lane = tid & 31, quad = site >> 5;
+    const uint32_t tm_links = tmem_base + ((uint32_t)(quad * 32) << 16);
+    const uint32_t bar_ready = link_base + 32 * quad, bar_early = bar_ready + 8, bar_free = bar_ready + 16, bar_done = bar_ready + 24;
+    auto tile_row = [&](int it, int &r) -> long long {
+        const int4 o = args.tiles[blockIdx.x + it * gridDim.x];
+        const int x1 = o.x + i1, x2 = o.y + i2, x3 = o.z + i3;
+        r = (x1 + x2 + x3 + args.parity_out) & 1;
+        return x1 + (long long)args.L1 * (x2 + (long long)args.L2 * x3);
+    };
+    // TMEM column of the link at position p (0..7) of the leg order for the tile whose slot base is b8 = (8 t) mod 14
+    auto slot_col = [&](int b8, int p) -> uint32_t {
+        int sl = b8 + p;
+        if (sl >= Cfg::NSLOT) sl -= Cfg::NSLOT;
+        return 36u * (uint32_t)sl;
+    };
+
+    if (tid < 128) {        // ===================== link loaders: global -> tensor memory, one tile ahead ============
+        const uint64_t pol_first = l2_policy(args.l2pol / 1000000 % 10);
+        int b8 = 0;
+        for (int n = 0; n < my_tiles; n++) {
+            int r_unused;
+            const long long grow = tile_row(n, r_unused);
+            const double2 *gp = args.gauge + grow * (72 * LH) + 2 * h;
+            // position p of the leg order holds leg (6 - 2 (p / 2)) + (p & 1): elements [9 leg, 9 leg + 9) of the site.
+            // Elements 2j and 2j + 1 are adjacent in memory (pack.cu): 256-bit loads, whole 512-byte runs per warp.
+            // Two batches of 18 elements (72 registers each) are in flight at a time.
+            double2 ta[18], tb[18];
+#pragma unroll
+            for (int k = 0; k < 18; k += 2) ldg_d4_hint(gp + (54 + k) * LH, pol_first, ta[k], ta[k + 1]);      // legs 6, 7
+#pragma unroll
+            for (int k = 0; k < 18; k += 2) ldg_d4_hint(gp + (36 + k) * LH, pol_first, tb[k], tb[k + 1]);      // legs 4, 5
+            // the slots of positions 0..5 were last read by tile n - 2 (n >= 2)
+            if (n >= 2) {
+                mbar_wait(bar_done, (n - 2) & 1);
+                tmem_fence_after();
+            }
+#pragma unroll
+            for (int k = 0; k < 18; k++) tmem_st_c(tm_links + slot_col(b8, 0 + k / 9) + 4 * (k % 9), ta[k]);
+#pragma unroll
+            for (int k = 0; k < 18; k += 2) ldg_d4_hint(gp + (18 + k) * LH, pol_first, ta[k], ta[k + 1]);      // legs 2, 3
+#pragma unroll
+            for (int k = 0; k < 18; k++) tmem_st_c(tm_links + slot_col(b8, 2 + k / 9) + 4 * (k % 9), tb[k]);
+#pragma unroll
+            for (int k = 0; k < 18; k += 2) ldg_d4_hint(gp + k * LH, pol_first, tb[k], tb[k + 1]);             // legs 0, 1
+#pragma unroll
+            for (int k = 0; k < 18; k++) tmem_st_c(tm_links + slot_col(b8, 4 + k / 9) + 4 * (k % 9), ta[k]);
+            tmem_wait_st();
+            tmem_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_early);
+            // the slots of positions 6, 7 are those of the first two legs of tile n - 1: free once its last slice has
+            // taken them into registers
+            if (n >= 1) {
+                mbar_wait(bar_free, (n - 1) & 1);
+                tmem_fence_after();
+            }
+#pragma unroll
+            for (int k = 0; k < 18; k++) tmem_st_c(tm_links + slot_col(b8, 6 + k / 9) + 4 * (k % 9), tb[k]);
+            tmem_wait_st();
+            tmem_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_ready);
+            b8 = (b8 + 8) % Cfg::NSLOT;
+        }
+        asm volatile("bar.sync 2, %0;" ::"n"(288) : "memory");
+        return;
+    }
+
+    // =========================== consumers: one thread = one output site ===========================
+    reg_alloc<Cfg::CONS_REGS>();
+    const uint64_t pol_out = l2_policy(args.l2pol / 10000000 % 10);
     const int rc = row;
     const int r1p = (i1 + 1 < B1) ? rc + 1 : Cfg::R_X1P + i2 + B2 * i3;
     const int r1m = (i1 > 0) ? rc - 1 : Cfg::R_X1M + i2 + B2 * i3;
@@ -837,64 +916,39 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
     off[6] = r3p * Cfg::ROWB + h * 16;
     off[7] = r3m * Cfg::ROWB + h * 16;
     const long long nrow = (long long)args.L1 * args.L2 * args.L3;
-    // this thread's TMEM lane: consumer warp w (CTA warp 4 + w) sits in lane quadrant w
-    const uint32_t tm_links = tmem_base + ((uint32_t)((site >> 5) * 32) << 16);
-
-    auto tile_row = [&](int it, int &r) -> long long {
-        const int4 o = args.tiles[blockIdx.x + it * gridDim.x];
-        const int x1 = o.x + i1, x2 = o.y + i2, x3 = o.z + i3;
-        r = (x1 + x2 + x3 + args.parity_out) & 1;
-        return x1 + (long long)args.L1 * (x2 + (long long)args.L2 * x3);
-    };
     auto set_x0_offsets = [&](int r) {
         int hp = h + r;       if (hp == LH) hp = 0;
         int hm = h - 1 + r;   if (hm < 0) hm = LH - 1;
         off[0] = rc * Cfg::ROWB + hp * 16;
         off[1] = rc * Cfg::ROWB + hm * 16;
     };
-    // the 72 link elements of the site: global -> tensor memory, DWF_S_LEGS legs in flight at a time (between tiles the
-    // accumulator and spinor registers are free).  Elements 2j and 2j + 1 of a site are adjacent in memory (pack.cu):
-    // one 256-bit load per pair, a warp reads whole 512-byte runs.
-    auto load_links = [&](long long grow) {
-        const double2 *gp = args.gauge + grow * (72 * LH) + 2 * h;
-        constexpr int NB = 9 * DWF_S_LEGS;
-        static_assert(NB % 2 == 0 && 72 % NB == 0, "DWF_S_LEGS: 2, 4 or 8");
-#pragma unroll
-        for (int b = 0; b < 72 / NB; b++) {
-            double2 t[NB];
-#pragma unroll
-            for (int k = 0; k < NB; k += 2) ldg_d4_hint(gp + (b * NB + k) * LH, pol_first, t[k], t[k + 1]);
-#pragma unroll
-            for (int k = 0; k < NB; k++) tmem_st_c(tm_links + 4 * (b * NB + k), t[k]);
-        }
-        tmem_wait_st();
-    };
 
     double nsum = 0.0;
-    int r_cur;
-    long long grow = tile_row(0, r_cur);
-    set_x0_offsets(r_cur);
-    load_links(grow);
-
-    int g = 0;
+    int g = 0, b8 = 0;
     for (int it = 0; it < my_tiles; it++) {
         const bool has_next = it + 1 < my_tiles;
-        int r_next = r_cur;
-        long long grow_next = grow;
-        if (has_next) grow_next = tile_row(it + 1, r_next);
+        int r_cur;
+        const long long grow = tile_row(it, r_cur);
+        set_x0_offsets(r_cur);
+        const uint32_t tm_tile = tm_links + 36u * (uint32_t)b8;
+        // TMEM address of the link at position p of this tile (slots wrap at 14)
+#define DWF_LINK_AT(p) (tm_tile + ((b8 + (p)) >= Cfg::NSLOT ? (uint32_t)(36 * (p)) - 36u * Cfg::NSLOT : (uint32_t)(36 * (p))))
+        mbar_wait(bar_ready, it & 1);           // the loader warp of this lane quadrant has written all eight links
+        tmem_fence_after();
         for (int ss = 0; ss < args.Ls; ss++, g++) {
             const int s = (args.zigzag && (it & 1)) ? args.Ls - 1 - ss : ss;
             const int stage = g & 1;
+            const bool hand_over = has_next && ss == args.Ls - 1;
             double2 *o2 = args.out + grow * (12 * LH) + h + (long long)s * nrow * (12 * LH);
             mbar_wait(full_base + 8 * stage, (g >> 1) & 1);
             const unsigned char *sb = smem + stage * Cfg::STAGE_BYTES;
             double2 acc[12];
             uint32_t W[36];
-            tmem_ld36(tm_links + 36 * 6, W);
+            tmem_ld36(DWF_LINK_AT(0), W);
             double2 xv[12];
             // one leg: the neighbour spinor out of shared memory, the link out of tensor memory (requested one leg
             // ahead: right after this leg's link has been unpacked, the next one's load goes into the same registers)
-#define DWF_LEG64S(L, MU, FWD, FIRST, NEXT)                                                         \
+#define DWF_LEG64S(L, MU, FWD, FIRST, NEXTP)                                                        \
             {                                                                                       \
                 double2 psi[4][3];                                                                  \
                 _Pragma("unroll") for (int k = 0; k < 12; k++)                                      \
@@ -902,7 +956,7 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
                 tmem_wait_ld_regs36(W);                                                             \
                 double2 Ul[9];                                                                      \
                 _Pragma("unroll") for (int k = 0; k < 9; k++) Ul[k] = tmem_unpack_p(W + 4 * k);     \
-                if constexpr ((NEXT) >= 0) tmem_ld36(tm_links + 36 * ((NEXT) < 0 ? 0 : (NEXT)), W); \
+                if constexpr ((NEXTP) >= 0) tmem_ld36(DWF_LINK_AT((NEXTP) < 0 ? 0 : (NEXTP)), W);   \
                 leg64_site<MU, (FWD) != DAG, FIRST>(acc, psi, Ul);                                  \
             }
             // a region goes back to the producer as soon as this warp's loads from it have completed: the accumulator
@@ -911,16 +965,25 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
 #define DWF_RELEASE64S(R)                                                                           \
             __syncwarp();                                                                           \
             if (lane == 0) mbar_arrive_dep(empty_base + 8 * (Cfg::NREG * stage + (R)), args.zero, acc[0].x, acc[3].x);
-            DWF_LEG64S(6, 3, true, true, 7)
-            DWF_LEG64S(7, 3, false, false, 4)
+            DWF_LEG64S(6, 3, true, true, 1)
+            DWF_LEG64S(7, 3, false, false, 2)
             DWF_RELEASE64S(0)
-            DWF_LEG64S(4, 2, true, false, 5)
-            DWF_LEG64S(5, 2, false, false, 2)
+            if (hand_over) {
+                // last slice of the tile: the links of its first two legs are in registers (tcgen05.wait::ld inside the
+                // leg), their slots go to the loader for the next tile's last two links.  The wait on `early` keeps
+                // this warp at most one phase ahead of the loader on `free` and `done`.
+                mbar_wait(bar_early, (it + 1) & 1);
+                tmem_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_free);
+            }
+            DWF_LEG64S(4, 2, true, false, 3)
+            DWF_LEG64S(5, 2, false, false, 4)
             DWF_RELEASE64S(1)
-            DWF_LEG64S(2, 1, true, false, 3)
-            DWF_LEG64S(3, 1, false, false, 0)
+            DWF_LEG64S(2, 1, true, false, 5)
+            DWF_LEG64S(3, 1, false, false, 6)
             DWF_RELEASE64S(2)
-            DWF_LEG64S(0, 0, true, false, 1)
+            DWF_LEG64S(0, 0, true, false, 7)
             if constexpr (AXPY) {       // x of this site and slice, requested before the last leg
                 const double2 *xp = args.axpy_x + (o2 - args.out);
 #pragma unroll
@@ -930,6 +993,11 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
 #undef DWF_LEG64S
             DWF_RELEASE64S(3)
 #undef DWF_RELEASE64S
+            if (ss == args.Ls - 1) {    // every link of this tile has been read for the last time
+                tmem_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_done);
+            }
 #pragma unroll
             for (int k = 0; k < 12; k++) {
                 double2 v = acc[k];
@@ -941,10 +1009,8 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
                 stg_d2_hint(o2 + k * LH, v, pol_out);
             }
         }
-        grow = grow_next;
-        r_cur = r_next;
-        set_x0_offsets(r_cur);
-        if (has_next) load_links(grow);
+#undef DWF_LINK_AT
+        b8 = (b8 + 8) % Cfg::NSLOT;
     }
 
     if constexpr (NORM) {
@@ -952,7 +1018,7 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
         double *slots = reinterpret_cast<double *>(smem + Cfg::NSTAGE * Cfg::STAGE_BYTES + Cfg::TAIL_NORM);
-        if (lane == 0) slots[site >> 5] = v;
+        if (lane == 0) slots[quad] = v;
         asm volatile("bar.sync 1, %0;" ::"n"(Cfg::NWARP_C * 32) : "memory");
         if (site == 0) {
             double t = 0.0;
@@ -961,7 +1027,7 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
         }
     }
     tmem_fence_before();
-    asm volatile("bar.sync 2, %0;" ::"n"((Cfg::NWARP_C + 1) * 32) : "memory");
+    asm volatile("bar.sync 2, %0;" ::"n"(288) : "memory");
 }
 
 // ---------------------------------------------------------------------------------------------
