@@ -1,5 +1,7 @@
-// dhop_staged64.cu -- the fp64 TMA-staged Dhop kernel for sm_100a: link-stationary with the links of
-// a site split by COLOUR COLUMN over three threads.
+// dhop_staged64.cu -- the fp64 TMA-staged Dhop kernels for sm_100a.  Three kernels, in the order of preference of
+// the host tables: the site-per-thread kernel with the links in tensor memory (dhop_staged64s_kernel, second half of
+// this file; 128-site tiles), and the two colour-split kernels described first: links of a site split by COLOUR COLUMN
+// over three threads, kept in tensor memory (128-site tiles) or in registers (64-site tiles, every row length).
 //
 //   Dhop psi(x,s) = sum_mu [ (1-gamma_mu) U_mu(x) psi(x+mu,s) + (1+gamma_mu) U_mu^dag(x-mu) psi(x-mu,s) ]
 //
@@ -624,11 +626,16 @@ dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_con
 // =============================================================================================
 // Site-per-thread TMEM variant ("S"): ONE thread per output site, as in the fp32 kernel, with all 8 links of the
 // site (72 complex = 288 words) parked in the thread's tensor-memory lane instead of in registers.  No colour split:
-// no repeated accumulation (840 instead of 1248 fp64 operations per site), no exchange, no exchange barriers.  A CTA is
-// the producer warpgroup plus FOUR consumer warps (128 sites, one warp per TMEM lane quadrant); the FP64 pipe has 64
-// lanes per SM, so four warps with the instruction-level parallelism of a whole SU(3) x half-spinor product each keep it
-// busy.  The links of leg L + 1 are requested from tensor memory right after leg L's have been unpacked and land
-// during leg L's arithmetic.  TMEM columns [36 L, 36 L + 36) of a lane: the 9 complex numbers U_ab (a*3 + b) of leg L.
+// no repeated accumulation (840 instead of 1248 fp64 operations per site), no exchange, no exchange barriers.
+// Three warpgroups per CTA:
+//   warps 0-3   link loaders: thread <-> site of the tile; write the NEXT tile's links into tensor memory while the
+//               consumers compute (global -> registers -> tcgen05.st)
+//   warps 4-7   consumers: 128 sites, one warp per TMEM lane quadrant (and per scheduler).  The link of leg L + 1 is
+//               requested from tensor memory right after leg L's has been unpacked and lands during leg L's arithmetic
+//   warp 8      producer: one thread issues the bulk tensor loads, region by region (warps 9-11 exit)
+// Loader warp q and consumer warp q address the same 32 TMEM lanes (tcgen05.ld / .st reach lane quadrant warp % 4).
+// A lane's 512 columns are 14 link slots of 36 columns (9 complex numbers U_ab at a*3 + b); the slot assignment and the
+// four mbarriers per quadrant that hand slots back and forth are described at Staged64SCfg::NSLOT and in the kernel.
 // =============================================================================================
 template <int LH, int B1, int B2, int B3> struct Staged64SCfg {
     static constexpr int NROW_C = B1 * B2 * B3;
