@@ -409,6 +409,10 @@ int dwf_set_option(dwf_geometry *g, const char *key, long long value)
     } else if (!strcmp(key, "async_host")) {
         g->opt_async_host = v != 0;
         return DWF_OK;
+    } else if (!strcmp(key, "max_ctas")) {
+        if (v < 0) { set_error("max_ctas must be >= 0"); return DWF_ERR_INVALID_ARG; }
+        g->opt_max_ctas = (int)v;
+        return DWF_OK;
     } else if (!strcmp(key, "kernel")) {
         if (v < 0 || v > 2) { set_error("kernel must be 0 (auto), 1 (direct) or 2 (staged)"); return DWF_ERR_INVALID_ARG; }
         g->opt_kernel = v;

@@ -758,7 +758,8 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     while (ssplit > 1 && (ls % ssplit || slots % ssplit)) ssplit--;
     a.ssplit = ssplit;
     const void *fn = v.fn[mode];
-    const int ngroup_max = slots / ssplit;
+    int ngroup_max = slots / ssplit;
+    if (g->opt_max_ctas > 0 && ngroup_max * ssplit > g->opt_max_ctas) ngroup_max = g->opt_max_ctas / ssplit > 0 ? g->opt_max_ctas / ssplit : 1;
     const int ngroup = g->staged.ntiles < ngroup_max ? g->staged.ntiles : ngroup_max;
     void *params[] = {&mc, &m1, &m2, &m3, &m1l, &m2l, &mxc, &a};
     DWF_CUDA_CHECK(cudaLaunchKernel(fn, dim3((unsigned)(ngroup * ssplit)), dim3((unsigned)v.threads), params,

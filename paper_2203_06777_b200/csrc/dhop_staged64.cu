@@ -1224,7 +1224,8 @@ int launch_dhop_staged64(const dwf_geometry *g, const void *in, void *out, int p
     a.axpy_b = axpy_b;
     a.norm_partials = norm_partials;
     const void *fn = v.fn[norm_partials ? 4 : (dagger ? 1 : 0) + (axpy_x ? 2 : 0)];
-    const int grid = g->staged64.ntiles < g->sm_count ? g->staged64.ntiles : g->sm_count;
+    const int grid_max = (g->opt_max_ctas > 0 && g->opt_max_ctas < g->sm_count) ? g->opt_max_ctas : g->sm_count;
+    const int grid = g->staged64.ntiles < grid_max ? g->staged64.ntiles : grid_max;
     void *params[] = {&mc, &m1, &m2, &m3, &a};
     DWF_CUDA_CHECK(cudaLaunchKernel(fn, dim3((unsigned)grid), dim3((unsigned)v.threads), params, (size_t)v.smem, st));
     if (norm_blocks) *norm_blocks = grid;

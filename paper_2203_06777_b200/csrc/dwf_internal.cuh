@@ -118,6 +118,7 @@ struct dwf_geometry {
         size_t export_bytes;
     } xfer;
     int opt_async_host;     // 1: host imports / exports return without synchronising (dwf_host_wait)
+    int opt_max_ctas;       // > 0: cap on the grid of the staged kernels (more tiles per CTA; tests of the tile switch)
     // tunables (dwf_set_option)
     int opt_tile[4];        // requested log2 tile extents (cb: dim 0 in pairs)
     int opt_cpc;

@@ -391,3 +391,46 @@ def test_staged64_fp64_kernel(lib, dims, Ls, bc):
         assert torch.equal(g.dhop_oe(fin), plain)
         g.set_option("kernel", 1)                                 # direct kernel: another summation order
         assert rel_err(g.export_spinor(g.dhop_oe_dag(fin), lib.ODD), g.export_spinor(a, lib.ODD)) <= TOL[8]
+
+
+@pytest.mark.parametrize("prec,dims,Ls,bc,max_ctas", [
+    (8, (32, 8, 8, 8), 3, 1, 5),        # staged64s <16,2,2,2>: 64 tiles on 5 CTAs = 12-13 tiles each: the 14-slot link ring wraps
+    (8, (32, 8, 8, 8), 1, 0, 3),        # Ls = 1: every slice is a tile's first and last one (all four link barriers per slice)
+    (8, (32, 8, 8, 8), 2, 1, 64),       # one tile per CTA: no hand-over at all
+    (8, (32, 8, 8, 8), 2, 0, 63),       # CTA 0 walks two tiles, all others one
+    (8, (16, 8, 8, 8), 4, 1, 2),        # staged64s <8,4,2,2>: 16 tiles on 2 CTAs
+    (8, (8, 8, 8, 8), 5, 1, 1),         # staged64s <4,4,4,2>: all 16 tiles on ONE CTA
+    (8, (24, 8, 6, 8), 3, 1, 4),        # colour-split 64-site kernel (Lh = 12), many tiles per CTA
+    (4, (32, 8, 8, 8), 3, 1, 3),        # fp32 staged <16,4,2,2>: 32 tiles on 3 CTAs (link refill in the last slice)
+    (4, (32, 8, 8, 8), 1, 0, 2),
+])
+def test_staged_many_tiles_per_cta(lib, prec, dims, Ls, bc, max_ctas):
+    """Tile switches on small lattices: the option "max_ctas" caps the grid of the staged kernels, so that a CTA walks
+    many tiles -- every phase of the loader / consumer link hand-over of the fp64 site-per-thread kernel (slot ring of
+    14 wraps after 7 tiles), the link refill of the fp32 kernel, odd and even tile counts per CTA.  Plain, dagger, fused
+    norm2 and fused a x + b Dhop against the oracle; the result does not depend on the grid (bit-identical)."""
+    import torch
+    U = gen.gauge_random(dims, 91, prec=prec)
+    half = gen.spinor_gaussian(gen.volume(dims) // 2, Ls, 91, prec=prec)
+    xh = gen.spinor_gaussian(gen.volume(dims) // 2, Ls, 91, gen.STREAM_SPINOR2, prec)
+    with lib.Geometry(dims, Ls, prec, bc) as g:
+        g.load_gauge(U)
+        g.set_option("kernel", 2)
+        fin, fx = g.import_spinor(half, lib.EVEN), g.import_spinor(xh, lib.ODD)
+        full_grid = g.dhop_oe(fin).clone()
+        full_grid_eo = g.dhop_eo(fx).clone()
+        g.set_option("max_ctas", max_ctas)
+        want = oracle.dhop_cb(dims, Ls, bc, 1, U, half)
+        out = g.dhop_oe(fin)
+        assert rel_err(g.export_spinor(out, lib.ODD), want) <= TOL[prec]
+        assert torch.equal(out, full_grid)
+        assert torch.equal(g.dhop_eo(fx), full_grid_eo)
+        want_d = oracle.dhop_cb(dims, Ls, bc, 1, U, half, dagger=True)
+        assert rel_err(g.export_spinor(g.dhop_oe_dag(fin), lib.ODD), want_d) <= TOL[prec]
+        fused, n = g.dhop_oe_norm2(fin)
+        assert torch.equal(fused, full_grid)
+        assert abs(n - oracle.norm2(g.export_spinor(fused, lib.ODD))) <= 1e-12 * n
+        ax = g.dhop_oe_axpy(fin, fx, -0.25, 2.0)
+        assert rel_err(g.export_spinor(ax, lib.ODD), -0.25 * xh.astype(np.float64) + 2.0 * want) <= TOL[prec]
+        with pytest.raises(lib.DwfError):
+            g.set_option("max_ctas", -1)
