@@ -52,6 +52,7 @@ WORKLOADS = {
     "c4d": dict(dims=(32, 32, 32, 32), Ls=16, prec=8, bc=0, gauge="near_unit", seed=1004),
     # the paper's threshold volume per GPU ("24^4 and above") with the C4 recipe
     "c24": dict(dims=(24, 24, 24, 24), Ls=16, prec=4, bc=0, gauge="near_unit", seed=1004),
+    "c24d": dict(dims=(24, 24, 24, 24), Ls=16, prec=8, bc=0, gauge="near_unit", seed=1004),
     "c64": dict(dims=(64, 16, 16, 32), Ls=16, prec=4, bc=0, gauge="near_unit", seed=1004),
     "c5": dict(dims=(48, 48, 48, 96), Ls=12, prec=4, bc=1, gauge="random", seed=1005),
     "tiny": dict(dims=(8, 8, 8, 8), Ls=8, prec=4, bc=1, gauge="random", seed=1002),

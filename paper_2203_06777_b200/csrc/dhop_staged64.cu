@@ -639,8 +639,9 @@ dhop_staged64_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_con
 // =============================================================================================
 template <int LH, int B1, int B2, int B3> struct Staged64SCfg {
     static constexpr int NROW_C = B1 * B2 * B3;
-    static constexpr int T = LH * NROW_C;                        // output sites per tile = consumer threads
-    static constexpr int NWARP_C = T / 32;
+    static constexpr int T = LH * NROW_C;                        // output sites per tile (<= 128: one per TMEM lane)
+    static constexpr int NWARP_C = 4;                            // consumer warps of the CTA
+    static constexpr int NWARP_ACT = (T + 31) / 32;              // ... that own sites (row lengths that do not divide 128)
     // warpgroup 0: link loaders (one thread per site), warpgroup 1: consumers (one thread per site),
     // warpgroup 2: its first warp issues the bulk tensor loads
     static constexpr int NT = 384;
@@ -663,7 +664,7 @@ template <int LH, int B1, int B2, int B3> struct Staged64SCfg {
     // TMEM base (8 B), one fp64 slot per consumer warp (fused norm2)
     static constexpr int TAIL_LINK = 80, TAIL_TMEM = 208, TAIL_NORM = 216, TAIL = TAIL_NORM + 8 * NWARP_C;
     static constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + (TAIL + 15) / 16 * 16;
-    static_assert(T == 128, "one consumer warp per TMEM lane quadrant: 128 sites per tile");
+    static_assert(T <= 128 && T > 64, "one site per TMEM lane, one consumer warp per lane quadrant: 65..128 sites per tile");
     static_assert(SMEM_BYTES <= 232448, "tile too large for shared memory");
 };
 
@@ -771,7 +772,7 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
     if (tid == 0) {
         for (int i = 0; i < 2; i++) {
             mbar_init(full_base + 8 * i, Cfg::NREG);           // one arrive.expect_tx per region
-            for (int r = 0; r < Cfg::NREG; r++) mbar_init(empty_base + 8 * (Cfg::NREG * i + r), Cfg::NWARP_C);
+            for (int r = 0; r < Cfg::NREG; r++) mbar_init(empty_base + 8 * (Cfg::NREG * i + r), Cfg::NWARP_ACT);
         }
         for (int i = 0; i < 16; i++) mbar_init(link_base + 8 * i, 1);
         mbar_fence_init();
@@ -832,11 +833,15 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
         return;
     }
 
-    // loaders and consumers: thread <-> site of the tile, warp <-> TMEM lane quadrant
-    const int site = tid & 127;
+    // loaders and consumers: thread <-> site of the tile, warp <-> TMEM lane quadrant.  Tiles of fewer than 128 sites
+    // (row lengths 12, 20, 24, 28): a warp without sites idles; the lanes without a site in the last active warp run
+    // along on the tile's last site (the warp-wide tcgen05 instructions need every lane) and do not store.
+    const int site_raw = tid & 127;
+    const bool warp_act = (site_raw & ~31) < Cfg::T, lane_act = site_raw < Cfg::T;
+    const int site = lane_act ? site_raw : Cfg::T - 1;
     const int h = site % LH, row = site / LH;
     const int i1 = row % B1, i2 = (row / B1) % B2, i3 = row / (B1 * B2);
-    const int lane = tid & 31, quad = site >> 5;
+    const int lane = tid & 31, quad = site_raw >> 5;
     const uint32_t tm_links = tmem_base + ((uint32_t)(quad * 32) << 16);
     const uint32_t bar_ready = link_base + 32 * quad, bar_early = bar_ready + 8, bar_free = bar_ready + 16, bar_done = bar_ready + 24;
     auto tile_row = [&](int it, int &r) -> long long {
@@ -855,7 +860,7 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
     if (tid < 128) {        // ===================== link loaders: global -> tensor memory, one tile ahead ============
         const uint64_t pol_first = l2_policy(args.l2pol / 1000000 % 10);
         int b8 = 0;
-        for (int n = 0; n < my_tiles; n++) {
+        for (int n = 0; warp_act && n < my_tiles; n++) {
             int r_unused;
             const long long grow = tile_row(n, r_unused);
             const double2 *gp = args.gauge + grow * (72 * LH) + 2 * h;
@@ -932,7 +937,7 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
 
     double nsum = 0.0;
     int g = 0, b8 = 0;
-    for (int it = 0; it < my_tiles; it++) {
+    for (int it = 0; warp_act && it < my_tiles; it++) {
         const bool has_next = it + 1 < my_tiles;
         int r_cur;
         const long long grow = tile_row(it, r_cur);
@@ -994,7 +999,7 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
             if constexpr (AXPY) {       // x of this site and slice, requested before the last leg
                 const double2 *xp = args.axpy_x + (o2 - args.out);
 #pragma unroll
-                for (int k = 0; k < 12; k++) xv[k] = __ldcs(xp + k * LH);
+                for (int k = 0; k < 12; k++) xv[k] = lane_act ? __ldcs(xp + k * LH) : make_double2(0.0, 0.0);
             }
             DWF_LEG64S(1, 0, false, false, -1)
 #undef DWF_LEG64S
@@ -1012,8 +1017,10 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
                     v.x = fma(args.axpy_b, v.x, args.axpy_a * xv[k].x);
                     v.y = fma(args.axpy_b, v.y, args.axpy_a * xv[k].y);
                 }
-                if constexpr (NORM) nsum = fma(v.x, v.x, fma(v.y, v.y, nsum));
-                stg_d2_hint(o2 + k * LH, v, pol_out);
+                if (lane_act) {
+                    if constexpr (NORM) nsum = fma(v.x, v.x, fma(v.y, v.y, nsum));
+                    stg_d2_hint(o2 + k * LH, v, pol_out);
+                }
             }
         }
 #undef DWF_LINK_AT
@@ -1047,6 +1054,9 @@ dhop_staged64s_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_co
 
 // TMEM variants (128-site tiles), preferred when they fit the lattice
 #define DWF_STAGED64T_VARIANTS(X) X(16, 2, 2, 2) X(8, 4, 2, 2) X(8, 2, 4, 2) X(8, 2, 2, 4) X(4, 4, 4, 2) X(4, 4, 2, 4)
+// site-per-thread TMEM variants: the 128-site shapes plus 96 .. 120-site tiles for the row lengths that do not divide 128
+#define DWF_STAGED64S_VARIANTS(X) DWF_STAGED64T_VARIANTS(X) X(12, 2, 2, 2) X(24, 2, 2, 1) X(24, 1, 2, 2) X(24, 2, 1, 2) \
+    X(20, 3, 2, 1) X(20, 1, 2, 3) X(28, 2, 2, 1) X(28, 1, 2, 2)
 
 const void *const *staged64_kernels_mode0();
 const void *const *staged64_kernels_mode1();
@@ -1062,7 +1072,7 @@ const void *const *DWF_CAT(staged64_kernels_mode, DWF_STAGED64_MODE)()
 #define Y(LH, B1, B2, B3) reinterpret_cast<const void *>(&dhop_staged64_kernel<LH, B1, B2, B3, DWF_STAGED64_MODE, false>),
 #define Z(LH, B1, B2, B3) reinterpret_cast<const void *>(&dhop_staged64s_kernel<LH, B1, B2, B3, DWF_STAGED64_MODE>),
     // order of preference: site-per-thread TMEM kernels, colour-split TMEM kernels, colour-split register kernels
-    static const void *const tab[] = {DWF_STAGED64T_VARIANTS(Z) DWF_STAGED64T_VARIANTS(X) DWF_STAGED64_VARIANTS(Y)};
+    static const void *const tab[] = {DWF_STAGED64S_VARIANTS(Z) DWF_STAGED64T_VARIANTS(X) DWF_STAGED64_VARIANTS(Y)};
 #undef X
 #undef Y
 #undef Z
@@ -1087,7 +1097,7 @@ static const std::vector<Variant64> &variants64()
 #define X(LH, B1, B2, B3)                                                                             \
         t.push_back({LH, B1, B2, B3, Staged64SCfg<LH, B1, B2, B3>::SMEM_BYTES, Staged64SCfg<LH, B1, B2, B3>::NT, 2, \
                      {k0[t.size()], k1[t.size()], k2[t.size()], k3[t.size()], k4[t.size()]}});
-        DWF_STAGED64T_VARIANTS(X)
+        DWF_STAGED64S_VARIANTS(X)
 #undef X
 #define X(LH, B1, B2, B3)                                                                             \
         t.push_back({LH, B1, B2, B3, Staged64Cfg<LH, B1, B2, B3, true>::SMEM_BYTES, Staged64Cfg<LH, B1, B2, B3, true>::NT, 1, \

@@ -357,11 +357,11 @@ def test_dhop_calls_can_be_captured_in_a_cuda_graph(lib):
 
 
 @pytest.mark.parametrize("dims,Ls,bc", [((32, 8, 8, 8), 3, 1), ((16, 8, 4, 6), 5, 0), ((8, 8, 8, 8), 8, 1), ((32, 6, 4, 10), 2, 0),
-                                        ((24, 8, 6, 8), 4, 1), ((48, 4, 6, 4), 3, 0), ((64, 4, 4, 6), 3, 1), ((40, 6, 4, 4), 5, 1)])
+                                        ((24, 8, 6, 8), 4, 1), ((48, 4, 6, 4), 3, 0), ((64, 4, 4, 6), 3, 1), ((40, 6, 4, 4), 5, 1),
+                                        ((56, 4, 4, 6), 2, 1), ((40, 8, 8, 6), 2, 0)])
 def test_staged64_fp64_kernel(lib, dims, Ls, bc):
-    """The fp64 staged kernel (csrc/dhop_staged64.cu: three threads per site, one colour column of the
-    links each, partial sums exchanged through shared memory one step late), forced with kernel=2:
-    several tiles per CTA (tile switch with link refill), Lh = 4 .. 32, plain, dagger, fused norm2 and
+    """The fp64 staged kernels (csrc/dhop_staged64.cu: site-per-thread with the links in tensor memory for
+    Lh = 4 .. 28, tiles of 96 .. 128 sites; colour-split for Lh = 32), forced with kernel=2: plain, dagger, fused norm2 and
     fused a x + b Dhop against the oracle at the fp64 bar; bit-identical from run to run and under zigzag."""
     import torch
     check_cb_against_oracle(lib, dims, Ls, 8, bc, 48)
@@ -400,7 +400,9 @@ def test_staged64_fp64_kernel(lib, dims, Ls, bc):
     (8, (32, 8, 8, 8), 2, 0, 63),       # CTA 0 walks two tiles, all others one
     (8, (16, 8, 8, 8), 4, 1, 2),        # staged64s <8,4,2,2>: 16 tiles on 2 CTAs
     (8, (8, 8, 8, 8), 5, 1, 1),         # staged64s <4,4,4,2>: all 16 tiles on ONE CTA
-    (8, (24, 8, 6, 8), 3, 1, 4),        # colour-split 64-site kernel (Lh = 12), many tiles per CTA
+    (8, (24, 8, 6, 8), 3, 1, 4),        # staged64s <12,2,2,2>: 96-site tiles, the fourth consumer / loader warp idles
+    (8, (40, 6, 4, 4), 2, 1, 3),        # staged64s <20,3,2,1>: 120-site tiles, eight lanes of the last warp own no site
+    (8, (56, 4, 4, 6), 2, 0, 5),        # staged64s <28,2,2,1>: 112-site tiles
     (4, (32, 8, 8, 8), 3, 1, 3),        # fp32 staged <16,4,2,2>: 32 tiles on 3 CTAs (link refill in the last slice)
     (4, (32, 8, 8, 8), 1, 0, 2),
 ])
