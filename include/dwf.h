@@ -161,6 +161,26 @@ DWF_API int dwf_face_apply_t(const dwf_geometry *g, const void *recv_lo, const v
 DWF_API int dwf_norm2(const dwf_geometry *g, const void *field, int parity, double *result_host,
               void *stream);
 
+/* norm2 WITHOUT any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it): no geometry is needed, and the per-CTA partial sums live in a file-scope __device__
+ * array of the library (512.25 KB, held by every GPU that loads the library until the process exits) instead of the
+ * scratch a geometry allocates.  *result_dev = sum over the n_reals reals at x_dev of x^2, accumulated in fp64 in a
+ * fixed order (deterministic; it differs from dwf_norm2 of the same buffer only in summation order, relative
+ * difference <= 1e-12).  x_dev: device pointer on cuda_device, 16-byte aligned, n_reals values of `precision`
+ * (DWF_F32 / DWF_F64), any buffer (a field in device layout, or anything else); result_dev: device pointer to ONE
+ * double, 8-byte aligned, owned by the caller, written asynchronously on `stream` (the call does not synchronise
+ * and copies nothing to the host).  The call issues one memset of the arrival counter and one kernel on `stream`
+ * and calls no cudaMalloc / cudaFree or allocating routine; the first call on a device looks the array's address
+ * up (cudaGetSymbolAddress), so make one call outside a capture first.
+ * LIMIT: n_reals * precision <= DWF_NORM2_STATIC_MAX_BYTES (2 GiB: 2^29 fp32 or 2^28 fp64 values; a C4 half
+ * field is 0.8 / 1.6 GB); larger buffers are rejected with INVALID_ARG and a message naming the limit.
+ * SHARING: every call on a device uses the same array.  Calls that may overlap on the GPU (different streams,
+ * parallel graph branches, several host threads) race on it: the caller serialises them.
+ * Errors: INVALID_ARG (NULL, alignment, size, device ordinal), UNSUPPORTED (precision), CUDA. */
+#define DWF_NORM2_STATIC_MAX_BYTES ((size_t)1 << 31)
+DWF_API int dwf_norm2_static(const void *x_dev, size_t n_reals, int precision, int cuda_device, double *result_dev,
+                             void *stream);
+
 /* DhopOE / DhopEO fused with the norm2 of their result (SURVEY.md 8(a) rows a6 + a7 in one pass):
  * out = D in and *result_host = sum |out|^2, fp64 accumulation in a fixed order (deterministic
  * for a given geometry and option set; it differs from dwf_norm2(out) only in summation order,

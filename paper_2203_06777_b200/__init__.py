@@ -30,6 +30,7 @@ SYMBOLS = (
     "dwf_error_string", "dwf_last_error",
     "dwf_dhop_oe_mrhs", "dwf_dhop_eo_mrhs", "dwf_host_wait", "dwf_face_bytes", "dwf_face_pack_t", "dwf_face_apply_t",
     "dwf_mooee", "dwf_mooee_inv", "dwf_ddwf", "dwf_schur_work_bytes", "dwf_schur", "dwf_axpby", "dwf_cg_work_bytes", "dwf_cg_schur",
+    "dwf_norm2_static",
 )
 
 
@@ -62,6 +63,7 @@ def load(build_if_missing: bool = True):
     for f in (lib.dwf_dhop_oe_mrhs, lib.dwf_dhop_eo_mrhs):
         f.argtypes = [vp, vp, vp, ci, ci, vp]
     lib.dwf_norm2.argtypes = [vp, vp, ci, ctypes.POINTER(ctypes.c_double), vp]
+    lib.dwf_norm2_static.argtypes = [vp, ctypes.c_size_t, ci, ci, vp, vp]
     for f in (lib.dwf_dhop_oe_axpy, lib.dwf_dhop_eo_axpy):
         f.argtypes = [vp, vp, vp, ctypes.c_double, ctypes.c_double, vp, vp]
     for f in (lib.dwf_dhop_oe_norm2, lib.dwf_dhop_eo_norm2):
@@ -259,6 +261,24 @@ def dwf_norm2(g: int, field, parity: int = FULL, stream=None) -> float:
     r = ctypes.c_double()
     _check(load().dwf_norm2(g, _dev_ptr(field, g, parity), int(parity), ctypes.byref(r), _stream(stream, g)), "dwf_norm2")
     return r.value
+
+
+NORM2_STATIC_MAX_BYTES = 1 << 31
+
+
+def dwf_norm2_static(x, result, n_reals: int | None = None, stream=None) -> None:
+    """result[0] = sum x^2 without any allocation (include/dwf.h).  x: CUDA tensor (float32 / float64, contiguous),
+    result: CUDA float64 tensor of one element on the same device; asynchronous on `stream` (None = torch's current
+    stream on x's device).  n_reals: number of leading elements to sum (default: all)."""
+    import torch
+    if not (x.is_cuda and result.is_cuda and x.device == result.device and x.is_contiguous()):
+        raise DwfError(ERR_INVALID_ARG, "binding", "x and result must be contiguous CUDA tensors on one device")
+    if x.dtype not in (torch.float32, torch.float64) or result.dtype != torch.float64 or result.numel() < 1:
+        raise DwfError(ERR_INVALID_ARG, "binding", "x must be float32 / float64, result float64 with one element")
+    n = x.numel() if n_reals is None else int(n_reals)
+    dev = x.device.index if x.device.index is not None else torch.cuda.current_device()
+    st = int(torch.cuda.current_stream(dev).cuda_stream) if stream is None else _stream(stream)
+    _check(load().dwf_norm2_static(x.data_ptr(), n, x.element_size(), dev, result.data_ptr(), st), "dwf_norm2_static")
 
 
 def dwf_inner_product(g: int, a, b, parity: int = FULL, stream=None) -> complex:
