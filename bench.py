@@ -386,6 +386,41 @@ def run_gpu(args, w):
         us_graph = 1e3 * ga.elapsed_time(gb) / (5 * 2 * reps)
         graph_line = {"us_per_half_dhop": us_graph, "frac": model_bytes_cb(w) / (us_graph * 1e-6) / 1e9 / peaks()[0],
                       "note": f"{reps} DhopOE + DhopEO pairs captured in one CUDA graph, replayed 5 times"}
+        # the full-field operator dwf_dhop (fp32 staged geometries: ONE launch over both parities), event-timed with the
+        # host in the loop and replayed from a graph; two half fields of traffic per launch
+        ff_in, ff_out = g.new_field(dwf.FULL), g.new_field(dwf.FULL)
+        ff_in.normal_()
+        n_l0 = dwf.dwf_launch_count()
+        g.dhop(ff_in, ff_out)
+        launches_full = dwf.dwf_launch_count() - n_l0
+        torch.cuda.synchronize()
+        ga.record()
+        for _ in range(2 * reps):
+            g.dhop(ff_in, ff_out)
+        gb.record()
+        torch.cuda.synchronize()
+        us_full = 1e3 * ga.elapsed_time(gb) / (2 * reps)
+        graph2 = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(side):
+            torch.cuda.synchronize()
+            with torch.cuda.graph(graph2, stream=side):
+                for _ in range(reps):
+                    g.dhop(ff_in, ff_out)
+        graph2.replay()
+        torch.cuda.synchronize()
+        ga.record()
+        for _ in range(5):
+            graph2.replay()
+        gb.record()
+        torch.cuda.synchronize()
+        us_full_graph = 1e3 * ga.elapsed_time(gb) / (5 * reps)
+        mb_full = 2 * model_bytes_cb(w)
+        graph_line["full_dhop"] = {"launches_per_dhop": launches_full, "us_per_dhop": us_full, "us_per_dhop_graph": us_full_graph,
+                                   "frac": mb_full / (us_full * 1e-6) / 1e9 / peaks()[0],
+                                   "frac_graph": mb_full / (us_full_graph * 1e-6) / 1e9 / peaks()[0],
+                                   "note": "dwf_dhop on a full field; fields of this size stay partly resident in the 126 MB L2 "
+                                           "between launches, so the HBM model is an upper bound on the DRAM traffic (SURVEY.md 8(d))"}
+        del ff_in, ff_out
 
     # ---- e2e: the same step through the C ABI with HOST buffers ----
     host_in = torch.empty(psi_e.shape, dtype=torch.from_numpy(psi_e).dtype, pin_memory=True)

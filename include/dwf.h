@@ -293,6 +293,8 @@ DWF_API int dwf_kernel_info(const dwf_geometry *g, char *buf, size_t n);
  *                    Dhop calls return NO_GAUGE.  UNSUPPORTED on fp64 geometries.
  *   "async_host"     1: dwf_import_spinor / dwf_export_spinor with host arrays return without synchronising
  *                    (pipelined steps; dwf_host_wait before touching the host arrays)
+ *   "full_launch"    1 (default): dwf_dhop on an fp32 geometry with a staged variant is ONE launch whose tile table spans
+ *                    both parities; 0: two half-field launches (same bits)
  *   "max_ctas"       > 0: cap on the number of CTAs of the staged kernels (0: one per SM, or two for small tiles).  Fewer
  *                    CTAs walk more tiles each: used by the tests of the tile switch on small lattices.
  *   "raster", "tile0".."tile3", "cpc"   direct kernel: CTA launch order, log2 tile extents, slices per CTA */

@@ -95,7 +95,10 @@ int rebuild_tilings(dwf_geometry *g)
     if (g->tiles_staged) { cudaFree(g->tiles_staged); g->tiles_staged = nullptr; }
     plan_staged(g);
     if (g->staged.variant >= 0) {
-        std::vector<int4> st((size_t)g->staged.ntiles);
+        // [0, ntiles): the tiles of a half-field launch; [ntiles, 3 ntiles): the table of the full-field launch, every
+        // tile twice with its output parity in .w (odd sites first, as two half launches would run)
+        const size_t nt = (size_t)g->staged.ntiles;
+        std::vector<int4> st(3 * nt);
         int raster = g->opt_raster_staged;
         if (raster < 0) {
             // auto: x1 fastest, x3 slowest, direction 2 split until a macro block has at most 96 tile
@@ -105,6 +108,10 @@ int rebuild_tilings(dwf_geometry *g)
             while (raster < 9 && n1 * (n2 >> raster) > 96 && (n2 % (2 << raster)) == 0) raster++;
         }
         build_staged_tile_table(g, raster, st.data());
+        for (size_t i = 0; i < nt; i++) {
+            st[nt + i] = st[i];     st[nt + i].w = DWF_ODD;
+            st[2 * nt + i] = st[i]; st[2 * nt + i].w = DWF_EVEN;
+        }
         DWF_CUDA_CHECK(cudaMalloc(&g->tiles_staged, st.size() * sizeof(int4)));
         DWF_CUDA_CHECK(cudaMemcpy(g->tiles_staged, st.data(), st.size() * sizeof(int4), cudaMemcpyHostToDevice));
     }
@@ -327,6 +334,7 @@ int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, i
     g->opt_ssplit = 1;
     g->opt_zigzag = 1;
     g->opt_layered = 1;
+    g->opt_full_launch = 1;
 
     g->gauge_bytes = (size_t)8 * 18 * (size_t)g->lat.Vh * (size_t)precision;
     g->reduce_blocks = g->sm_count * 32;
@@ -408,6 +416,9 @@ int dwf_set_option(dwf_geometry *g, const char *key, long long value)
         return DWF_OK;
     } else if (!strcmp(key, "async_host")) {
         g->opt_async_host = v != 0;
+        return DWF_OK;
+    } else if (!strcmp(key, "full_launch")) {
+        g->opt_full_launch = v != 0;
         return DWF_OK;
     } else if (!strcmp(key, "max_ctas")) {
         if (v < 0) { set_error("max_ctas must be >= 0"); return DWF_ERR_INVALID_ARG; }
@@ -514,6 +525,11 @@ static int dhop_common(const dwf_geometry *g, const void *in, void *out, int par
     if (parity_out != DWF_FULL) return half_dhop(g, in, out, parity_out, st, dagger);
     // a full field is its even half field followed by its odd half field:
     // (Dhop psi)_odd = DhopOE psi_even, (Dhop psi)_even = DhopEO psi_odd
+    // fp32 geometries with a staged variant: ONE launch whose tile table spans both parities
+    if (!dagger && g->staged.variant >= 0 && g->opt_kernel != 1 && g->opt_full_launch && !(g->opt_gauge12 && g->gauge12[0])) {
+        wait_for_exports(g, st, out, dwf_field_bytes(g, DWF_FULL));
+        return launch_dhop_staged(g, in, out, DWF_FULL, st, nullptr, nullptr, false, nullptr, 0.f, 0.f, 1, false, true);
+    }
     const size_t half = dwf_field_bytes(g, DWF_EVEN);
     const char *ie = static_cast<const char *>(in), *io = ie + half;
     char *oe = static_cast<char *>(out), *oo = oe + half;

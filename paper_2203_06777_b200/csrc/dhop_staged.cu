@@ -81,6 +81,11 @@ struct StagedArgs {
     int layered;             // one TMA box per x3 layer (per-layer L2 policies) instead of one per region
     float axpy_a, axpy_b;    // AXPY kernels: out = a x + b Dhop in
     double *norm_partials;   // NORM kernels: one partial sum of |out|^2 per CTA (fixed order inside the CTA)
+    // FULL kernels (one launch for both parities of a full field): tile t of the table carries its output parity in
+    // .w; `gauge` / `gauge_odd` are the link sets of the even / odd output sites, `out` is the full output field
+    // (even half, then odd half, `half_vecs` 128-bit vectors each); the tensor maps cover the full input field
+    const float2 *gauge_odd;
+    long long half_vecs;
 };
 
 template <int LH, int B1, int B2, int B3> struct StagedCfg {
@@ -218,7 +223,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
                    const __grid_constant__ CUtensorMap map_xc, const StagedArgs args)
 {
     using Cfg = StagedCfg<LH, B1, B2, B3>;
-    constexpr bool NORM = MODE == 1, DAG = MODE == 2 || MODE == 4, AXPY = MODE == 3 || MODE == 4, G12 = MODE == 5;
+    constexpr bool NORM = MODE == 1, DAG = MODE == 2 || MODE == 4, AXPY = MODE == 3 || MODE == 4, G12 = MODE == 5, FULL = MODE == 6;
     // MODE 3 stages the rows box of the field x as well (read in the epilogue): NROW_C more rows per stage
     constexpr int STAGE = Cfg::STAGE_BYTES + (AXPY ? Cfg::NROW_C * Cfg::ROWB : 0);
     extern __shared__ __align__(1024) unsigned char smem[];
@@ -277,7 +282,8 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             const int it = g / nsl, i = g % nsl;
             const int s = s_first + ((args.zigzag && (it & 1)) ? nsl - 1 - i : i);
             const int4 o = tile_origin(it);
-            const int sb = s * L3;                 // x3 and s share tensor dimension 4: coordinate s*L3 + x3
+            int sb = s * L3;                       // x3 and s share tensor dimension 4: coordinate s*L3 + x3
+            if constexpr (FULL) sb += (1 - o.w) * args.Ls * L3;    // input half field of the opposite parity: Ls * L3 further on
             Boxes b;
             b.o1 = o.x; b.o2 = o.y; b.c4 = sb + o.z;
             b.x1m = o.x == 0 ? L1 - 1 : o.x - 1; b.x1p = o.x + B1 == L1 ? 0 : o.x + B1;
@@ -371,8 +377,17 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     auto tile_row = [&](int it, int &r) -> long long {
         const int4 o = tile_origin(it);
         const int x1 = o.x + i1, x2 = o.y + i2, x3 = o.z + i3;
-        r = (x1 + x2 + x3 + args.parity_out) & 1;
+        r = (x1 + x2 + x3 + (FULL ? o.w : args.parity_out)) & 1;
         return x1 + (long long)args.L1 * (x2 + (long long)args.L2 * x3);
+    };
+    // link set and output half field of the it-th tile (FULL: by the tile's parity)
+    auto tile_gauge = [&](int it) -> const float4 * {
+        if constexpr (FULL) return reinterpret_cast<const float4 *>(tile_origin(it).w ? args.gauge_odd : args.gauge);
+        else return reinterpret_cast<const float4 *>(args.gauge);
+    };
+    auto tile_out = [&](int it) -> float4 * {
+        if constexpr (FULL) return reinterpret_cast<float4 *>(args.out) + (tile_origin(it).w ? args.half_vecs : 0LL);
+        else return reinterpret_cast<float4 *>(args.out);
     };
     auto set_x0_offsets = [&](int r) {
         int hp = h + r;       if (hp == LH) hp = 0;
@@ -386,7 +401,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     int r_cur;
     long long grow = tile_row(0, r_cur);
     set_x0_offsets(r_cur);
-    float4 *optr = reinterpret_cast<float4 *>(args.out) + grow * (6 * LH) + h + (long long)s_first * slice_vecs;
+    float4 *optr = tile_out(0) + grow * (6 * LH) + h + (long long)s_first * slice_vecs;
     // G12: vector 3L + v of a site holds the complex numbers 2v, 2v+1 of rows 0, 1 of leg L (row-major), i.e. U[9L + 2v], U[9L + 2v + 1]
     constexpr int GV = G12 ? 24 : 36;                // 128-bit link vectors per site
     // row 2 of every link from rows 0, 1: r2 = sgn conj(r0 x r1); sgn = -1 for a time link whose hop wraps around an
@@ -407,7 +422,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         }
     };
     if (active) {
-        const float4 *gp = reinterpret_cast<const float4 *>(args.gauge) + grow * (GV * LH) + h;
+        const float4 *gp = tile_gauge(0) + grow * (GV * LH) + h;
         if constexpr (G12) {
 #pragma unroll
             for (int j = 0; j < 24; j++) {
@@ -505,7 +520,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         int r_next = r_cur;
         long long grow_next = grow;
         if (has_next) grow_next = tile_row(it + 1, r_next);
-        const float4 *gnext = reinterpret_cast<const float4 *>(args.gauge) + grow_next * (GV * LH) + h;
+        const float4 *gnext = tile_gauge(has_next ? it + 1 : it) + grow_next * (GV * LH) + h;
         for (int s = 0; s < nsl; s++, g++) {
             const bool fetch = has_next && s == nsl - 1;     // refill the links during the last slice
             const int stage = g & 1;
@@ -520,7 +535,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         grow = grow_next;
         r_cur = r_next;
         set_x0_offsets(r_cur);
-        optr = reinterpret_cast<float4 *>(args.out) + grow * (6 * LH) + h + (long long)s_first * slice_vecs;
+        optr = tile_out(has_next ? it + 1 : it) + grow * (6 * LH) + h + (long long)s_first * slice_vecs;
     }
 
     if constexpr (NORM) {
@@ -559,6 +574,7 @@ const void *const *staged_kernels_mode2();
 const void *const *staged_kernels_mode3();
 const void *const *staged_kernels_mode4();
 const void *const *staged_kernels_mode5();
+const void *const *staged_kernels_mode6();
 
 #define DWF_CAT2(a, b) a##b
 #define DWF_CAT(a, b) DWF_CAT2(a, b)
@@ -577,7 +593,8 @@ const void *const *DWF_CAT(staged_kernels_mode, DWF_STAGED_MODE)()
 struct Variant {
     int lh, b1, b2, b3;
     int smem, threads, ctas_per_sm;
-    const void *fn[6];       // MODE 0 (Dhop), 1 (Dhop + norm2), 2 (Dhop^dagger), 3 (a x + b Dhop), 4 (a x + b Dhop^dagger), 5 (Dhop, 12-real links)
+    const void *fn[7];       // MODE 0 (Dhop), 1 (Dhop + norm2), 2 (Dhop^dagger), 3 (a x + b Dhop), 4 (a x + b Dhop^dagger), 5 (Dhop, 12-real links),
+                             // 6 (Dhop of a full field, both parities in one launch)
     int smem_axpy;           // MODEs 3, 4 stage the rows box of x as well
 };
 
@@ -586,10 +603,11 @@ static const std::vector<Variant> &variants()
     static const std::vector<Variant> v = [] {
         std::vector<Variant> t;
         const void *const *k0 = staged_kernels_mode0(), *const *k1 = staged_kernels_mode1(), *const *k2 = staged_kernels_mode2(),
-                          *const *k3 = staged_kernels_mode3(), *const *k4 = staged_kernels_mode4(), *const *k5 = staged_kernels_mode5();
+                          *const *k3 = staged_kernels_mode3(), *const *k4 = staged_kernels_mode4(), *const *k5 = staged_kernels_mode5(),
+                          *const *k6 = staged_kernels_mode6();
 #define X(LH, B1, B2, B3)                                                                            \
         t.push_back({LH, B1, B2, B3, StagedCfg<LH, B1, B2, B3>::SMEM_BYTES, StagedCfg<LH, B1, B2, B3>::NT,  \
-                     StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM, {k0[t.size()], k1[t.size()], k2[t.size()], k3[t.size()], k4[t.size()], k5[t.size()]},    \
+                     StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM, {k0[t.size()], k1[t.size()], k2[t.size()], k3[t.size()], k4[t.size()], k5[t.size()], k6[t.size()]},    \
                      StagedCfg<LH, B1, B2, B3>::SMEM_BYTES + 2 * StagedCfg<LH, B1, B2, B3>::NROW_C * StagedCfg<LH, B1, B2, B3>::ROWB});
         DWF_STAGED_VARIANTS(X)
 #undef X
@@ -615,7 +633,7 @@ void plan_staged(dwf_geometry *g)
         g->staged.ntiles = (lat.L[1] / v[i].b1) * (lat.L[2] / v[i].b2) * (lat.L[3] / v[i].b3);
         // Opt in to the large dynamic shared memory here, on the geometry's device (the attribute is per
         // device; the caller holds a DeviceGuard), for every kernel MODE of the chosen tile shape.
-        for (int mode = 0; mode < 6; mode++) {
+        for (int mode = 0; mode < 7; mode++) {
             const int smem = (mode == 3 || mode == 4) ? v[i].smem_axpy : v[i].smem;
             if (smem > SMEM_LIMIT) continue;
             if (cudaFuncSetAttribute(v[i].fn[mode], cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) {
@@ -711,7 +729,7 @@ bool staged_supports_axpy(const dwf_geometry *g)
 
 int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st,
                        double *norm_partials, int *norm_blocks, bool dagger, const void *axpy_x, float axpy_a,
-                       float axpy_b, int nrhs, bool gauge12)
+                       float axpy_b, int nrhs, bool gauge12, bool full)
 {
     // nrhs > 1: `in`, `out` (and x) hold nrhs fields one after the other.  Dhop is diagonal
     // in s, so they are ONE field of nrhs * Ls slices to this kernel: the links of a tile stay in registers
@@ -723,14 +741,17 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     }
     const Variant &v = variants()[(size_t)g->staged.variant];
     if (gauge12 && (norm_partials || dagger || axpy_x)) { set_error("12-real links: plain Dhop only"); return DWF_ERR_UNSUPPORTED; }
-    const int mode = gauge12 ? 5 : norm_partials ? 1 : (axpy_x ? (dagger ? 4 : 3) : (dagger ? 2 : 0));
+    // full (VERDICT r01 task 8): `in` / `out` are FULL fields (even half, then odd half), one launch whose
+    // tile table lists every tile twice, once per output parity; the tensor maps cover both input halves (2 Ls slices)
+    if (full && (norm_partials || dagger || axpy_x || gauge12 || nrhs != 1)) { set_error("full-field launch: plain Dhop only"); return DWF_ERR_UNSUPPORTED; }
+    const int mode = full ? 6 : gauge12 ? 5 : norm_partials ? 1 : (axpy_x ? (dagger ? 4 : 3) : (dagger ? 2 : 0));
     const int smem = (mode == 3 || mode == 4) ? v.smem_axpy : v.smem;
     if (smem > SMEM_LIMIT) { set_error("tile too large for the fused axpy"); return DWF_ERR_UNSUPPORTED; }
     // The cache hands out pointers into its slots and the second lookup may evict the slot of the
     // first, so the maps are copied before it (they are passed to the kernel by value anyway).
     MapSet *ms = nullptr;
     int rc;
-    if ((rc = get_maps(g, v, in, ls, &ms))) return rc;
+    if ((rc = get_maps(g, v, in, full ? 2 * ls : ls, &ms))) return rc;
     CUtensorMap mc = ms->m[0], m1 = ms->m[1], m2 = ms->m[2], m3 = ms->m[3], m1l = ms->m[4], m2l = ms->m[5];
     CUtensorMap mxc = mc;
     if (axpy_x) {
@@ -744,6 +765,15 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     a.zero = 0;
     a.tiles = g->tiles_staged;
     a.ntiles = g->staged.ntiles;
+    a.gauge_odd = nullptr;
+    a.half_vecs = 0;
+    if (full) {             // the second part of the table: all tiles with .w = 1 (odd output sites), then all with .w = 0
+        a.tiles = g->tiles_staged + g->staged.ntiles;
+        a.ntiles = 2 * g->staged.ntiles;
+        a.gauge = static_cast<const float2 *>(g->gauge[0]);
+        a.gauge_odd = static_cast<const float2 *>(g->gauge[1]);
+        a.half_vecs = (long long)(dwf_field_bytes(g, DWF_EVEN) / 16);
+    }
     a.L1 = g->lat.L[1]; a.L2 = g->lat.L[2]; a.L3 = g->lat.L[3]; a.Ls = ls;
     a.parity_out = parity_out;
     a.l2pol = g->opt_l2pol;
@@ -760,7 +790,7 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     const void *fn = v.fn[mode];
     int ngroup_max = slots / ssplit;
     if (g->opt_max_ctas > 0 && ngroup_max * ssplit > g->opt_max_ctas) ngroup_max = g->opt_max_ctas / ssplit > 0 ? g->opt_max_ctas / ssplit : 1;
-    const int ngroup = g->staged.ntiles < ngroup_max ? g->staged.ntiles : ngroup_max;
+    const int ngroup = a.ntiles < ngroup_max ? a.ntiles : ngroup_max;
     void *params[] = {&mc, &m1, &m2, &m3, &m1l, &m2l, &mxc, &a};
     DWF_CUDA_CHECK(cudaLaunchKernel(fn, dim3((unsigned)(ngroup * ssplit)), dim3((unsigned)v.threads), params,
                                     (size_t)smem, st));

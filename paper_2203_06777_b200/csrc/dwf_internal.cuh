@@ -118,6 +118,7 @@ struct dwf_geometry {
         size_t export_bytes;
     } xfer;
     int opt_async_host;     // 1: host imports / exports return without synchronising (dwf_host_wait)
+    int opt_full_launch;    // 1: dwf_dhop of a full fp32 field is one launch over both parities (0: two half launches)
     int opt_max_ctas;       // > 0: cap on the grid of the staged kernels (more tiles per CTA; tests of the tile switch)
     // tunables (dwf_set_option)
     int opt_tile[4];        // requested log2 tile extents (cb: dim 0 in pairs)
@@ -179,7 +180,8 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
                        double *norm_partials = nullptr, int *norm_blocks = nullptr, bool dagger = false,
                        const void *axpy_x = nullptr, float axpy_a = 0.f, float axpy_b = 0.f,     // axpy_x: out = a x + b Dhop in
                        int nrhs = 1,                                                            // nrhs fields one after the other
-                       bool gauge12 = false);                                                   // 12-real links (plain Dhop only)
+                       bool gauge12 = false,
+                       bool full = false);                                                      // in / out are full fields: one launch for both parities                                                   // 12-real links (plain Dhop only)
 bool staged_supports_axpy(const dwf_geometry *g);
 // pack.cu: out = a x + b out, elementwise over nreal reals (the unfused path of dwf_dhop_*_axpy)
 int launch_axpby(const dwf_geometry *g, const void *x, void *out, double a, double b, size_t nreal, cudaStream_t st);

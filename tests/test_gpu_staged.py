@@ -436,3 +436,32 @@ def test_staged_many_tiles_per_cta(lib, prec, dims, Ls, bc, max_ctas):
         assert rel_err(g.export_spinor(ax, lib.ODD), -0.25 * xh.astype(np.float64) + 2.0 * want) <= TOL[prec]
         with pytest.raises(lib.DwfError):
             g.set_option("max_ctas", -1)
+
+
+@pytest.mark.parametrize("dims,Ls,bc,max_ctas", [((32, 8, 8, 8), 3, 1, 0), ((16, 8, 8, 8), 4, 0, 0), ((32, 8, 8, 8), 2, 1, 3),
+                                                 ((24, 8, 6, 8), 2, 1, 5), ((8, 8, 8, 8), 5, 1, 1)])
+def test_full_field_dhop_is_one_launch(lib, dims, Ls, bc, max_ctas):
+    """dwf_dhop on an fp32 geometry with a staged variant: ONE launch whose tile table spans both parities (VERDICT r01
+    task 8).  Against the oracle on every element, bit-identical to the two half-field launches (option full_launch = 0),
+    also when few CTAs walk tiles of both parities one after the other (max_ctas: the tile switch changes the link set,
+    the input half and the output half)."""
+    import torch
+    U = gen.gauge_random(dims, 95, prec=4)
+    psi = gen.spinor_gaussian(gen.volume(dims), Ls, 95, prec=4)
+    with lib.Geometry(dims, Ls, 4, bc) as g:
+        g.load_gauge(U)
+        g.set_option("kernel", 2)
+        if max_ctas:
+            g.set_option("max_ctas", max_ctas)
+        fin = g.import_spinor(psi, lib.FULL)
+        n0 = lib.dwf_launch_count()
+        out = g.dhop(fin).clone()
+        assert lib.dwf_launch_count() - n0 == 1
+        assert rel_err(g.export_spinor(out, lib.FULL), oracle.dhop(dims, Ls, bc, U, psi)) <= TOL[4]
+        g.set_option("full_launch", 0)
+        n0 = lib.dwf_launch_count()
+        two = g.dhop(fin)
+        assert lib.dwf_launch_count() - n0 == 2
+        assert torch.equal(two, out)
+        g.set_option("full_launch", 1)
+        assert torch.equal(g.dhop(fin), out)
