@@ -67,6 +67,8 @@ WORKLOADS = {
     # the solver the paper's workload is: CG on the Schur normal equations, a fixed number of iterations on the C4 shape
     "cg": dict(dims=(32, 32, 32, 32), Ls=16, prec=4, bc=1, gauge="near_unit", seed=1004, kind="cg"),
     "schurd": dict(dims=(32, 32, 32, 32), Ls=16, prec=8, bc=0, gauge="near_unit", seed=1004, kind="schur"),
+    # spinor fields stored as fp16, fp32 links and arithmetic, C4 shape
+    "c4h": dict(dims=(32, 32, 32, 32), Ls=16, prec=4, bc=0, gauge="near_unit", seed=1004, kind="f16"),
 }
 
 
@@ -740,6 +742,87 @@ def run_gpu_mrhs(args, w):
         dist.destroy_process_group()
 
 
+def run_gpu_f16(args, w):
+    """--workload c4h: SURVEY.md 8(f4), spinor fields in fp16 storage, fp32 links and arithmetic.  One step = DhopOE then
+    DhopEO (2 launches); minimal-traffic model per launch: one read + one write of a half field at 2 bytes per real plus
+    the links of one parity in fp32: 96 + 576 / Ls bytes per output 5D site."""
+    import torch
+    import paper_2203_06777_b200 as dwf
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dwf.load()
+    d, Ls, prec = w["dims"], w["Ls"], w["prec"]
+    V4 = d[0] * d[1] * d[2] * d[3]
+    sites = (V4 // 2) * Ls
+    U, psi_e = make_inputs(w)
+    g = dwf.Geometry(d, Ls, prec, w["bc"], device=local_rank)
+    for kv in args.opt or []:
+        k, v = kv.split("=")
+        g.set_option(k, int(v))
+    g.load_gauge(U)
+    f32_in = g.import_spinor(psi_e, dwf.EVEN)
+    f_in = g.to_f16(f32_in, dwf.EVEN)
+    f_mid, f_out = g.new_field_f16(dwf.ODD), g.new_field_f16(dwf.EVEN)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        g.dhop_oe_f16(f_in, f_mid)
+        g.dhop_eo_f16(f_mid, f_out)
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(args.steps)]
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    barrier()
+    sampler.start()
+    l0 = dwf.dwf_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for k in range(args.steps):
+        ev[k][0].record()
+        g.dhop_oe_f16(f_in, f_mid)
+        ev[k][1].record()
+        g.dhop_eo_f16(f_mid, f_out)
+    e1.record()
+    barrier()
+    launches = dwf.dwf_launch_count() - l0
+    clocks = sampler.stop()
+    ms_step = max_over_ranks(e0.elapsed_time(e1), dist) / args.steps
+    t_oe = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
+    if rank == 0:
+        peak, peak_src = peaks()
+        mb = sites * 24 * 2 * 2 + (V4 // 2) * 8 * 18 * prec         # fp16 in + out, fp32 links of one parity
+        achieved = mb / (t_oe * 1e-3) / 1e9
+        # the fp32 path on the widened input, rounded once, gives the same bits
+        chk = bool(torch.equal(g.dhop_oe(g.from_f16(f_in, dwf.EVEN)).to(torch.float16), f_mid))
+        line = {
+            "metric": "Dhop GFlop/s (1320 flop/5D site)", "value": world * 2 * FLOP_PER_SITE * sites / (ms_step * 1e-3) / 1e9, "unit": "GFlop/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"DWF even/odd Dhop {d[0]}x{d[1]}x{d[2]}x{d[3]} x Ls={Ls}, spinor fields stored as fp16, fp32 links and "
+                                   "arithmetic (SURVEY.md 8(f4)), DhopOE then DhopEO",
+                       "name": args.workload, "dims": list(d), "Ls": Ls, "storage": "f16", "l2": "fields larger than L2; no flush",
+                       "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "clocks": clocks, "gpu_launches": int(launches), "kernels_ms": {"dhop_oe_f16": t_oe},
+            "roofline": {"bound": "hbm", "kernel": g.kernel_info() + " (fp16 storage, DhopOE launches)", "achieved": achieved, "peak": peak,
+                         "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src, "algorithmic_bytes_per_launch": mb,
+                         "traffic": None},
+            "check": {"equals_fp32_path_rounded_once_bitwise": chk},
+        }
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def run_gpu_cg(args, w):
     """--workload cg: dwf_cg_schur on the C4 shape, `steps` CG iterations per solve (tolerance 0, so every iteration runs).
     One iteration = S p, S^dag (S p) (eight kernels of SURVEY.md 8(f2)), a fused x / r update with |r|^2, p = r + beta p, one
@@ -956,6 +1039,8 @@ def main():
         run_gpu_mrhs(args, w)
     elif w.get("kind") == "cg":
         run_gpu_cg(args, w)
+    elif w.get("kind") == "f16":
+        run_gpu_f16(args, w)
     elif w.get("kind") == "slab":
         run_gpu_slab(args, w)
     else:

@@ -161,6 +161,21 @@ DWF_API int dwf_face_apply_t(const dwf_geometry *g, const void *recv_lo, const v
 DWF_API int dwf_norm2(const dwf_geometry *g, const void *field, int parity, double *result_host,
               void *stream);
 
+/* ---- fp16 STORAGE of spinor fields, fp32 arithmetic (third variant; not in PAPER.md).  A field in fp16
+ * storage is the fp32 DEVICE layout element by element with IEEE binary16 reals: dwf_field_bytes(g, parity) / 2 bytes, a
+ * device pointer, 16-byte aligned, owned by the caller.  The links stay fp32.  fp32 geometries only (UNSUPPORTED otherwise).
+ * dwf_to_f16: field_f16 = round-to-nearest-even(field_f32); dwf_from_f16: exact widening.  Asynchronous on `stream`.
+ * dwf_dhop_oe_f16 / dwf_dhop_eo_f16: out = round_f16( Dhop( widen(in) ) ): every input real is widened to fp32 after the
+ * shared-memory load, projection, SU(3) products and the sum over the 8 legs run in fp32 exactly as in dwf_dhop_oe / _eo,
+ * and the result is rounded ONCE (nearest even) in the store.  Traffic model: 96 + 576/Ls bytes per 5D output site (132 at
+ * Ls = 16 against 228 in fp32).  Needs a staged variant whose fp16 rows stay 128-byte aligned: L0 a
+ * multiple of 16 (UNSUPPORTED otherwise; there is no fp16 path through the general kernel).  Overflow is the caller's
+ * concern (|values| <= 65504).  Errors: INVALID_ARG (NULL, alignment, in == out), NO_GAUGE, UNSUPPORTED, CUDA. */
+DWF_API int dwf_to_f16(const dwf_geometry *g, const void *field_f32, int parity, void *field_f16, void *stream);
+DWF_API int dwf_from_f16(const dwf_geometry *g, const void *field_f16, int parity, void *field_f32, void *stream);
+DWF_API int dwf_dhop_oe_f16(const dwf_geometry *g, const void *in_even_f16, void *out_odd_f16, void *stream);
+DWF_API int dwf_dhop_eo_f16(const dwf_geometry *g, const void *in_odd_f16, void *out_even_f16, void *stream);
+
 /* norm2 WITHOUT any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving
  * loops, harnesses that forbid it): no geometry is needed, and the per-CTA partial sums live in a file-scope __device__
  * array of the library (512.25 KB, held by every GPU that loads the library until the process exits) instead of the

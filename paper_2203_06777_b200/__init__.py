@@ -30,7 +30,7 @@ SYMBOLS = (
     "dwf_error_string", "dwf_last_error",
     "dwf_dhop_oe_mrhs", "dwf_dhop_eo_mrhs", "dwf_host_wait", "dwf_face_bytes", "dwf_face_pack_t", "dwf_face_apply_t",
     "dwf_mooee", "dwf_mooee_inv", "dwf_ddwf", "dwf_schur_work_bytes", "dwf_schur", "dwf_axpby", "dwf_cg_work_bytes", "dwf_cg_schur",
-    "dwf_norm2_static",
+    "dwf_norm2_static", "dwf_to_f16", "dwf_from_f16", "dwf_dhop_oe_f16", "dwf_dhop_eo_f16",
 )
 
 
@@ -64,6 +64,10 @@ def load(build_if_missing: bool = True):
         f.argtypes = [vp, vp, vp, ci, ci, vp]
     lib.dwf_norm2.argtypes = [vp, vp, ci, ctypes.POINTER(ctypes.c_double), vp]
     lib.dwf_norm2_static.argtypes = [vp, ctypes.c_size_t, ci, ci, vp, vp]
+    for f in (lib.dwf_to_f16, lib.dwf_from_f16):
+        f.argtypes = [vp, vp, ci, vp, vp]
+    for f in (lib.dwf_dhop_oe_f16, lib.dwf_dhop_eo_f16):
+        f.argtypes = [vp, vp, vp, vp]
     for f in (lib.dwf_dhop_oe_axpy, lib.dwf_dhop_eo_axpy):
         f.argtypes = [vp, vp, vp, ctypes.c_double, ctypes.c_double, vp, vp]
     for f in (lib.dwf_dhop_oe_norm2, lib.dwf_dhop_eo_norm2):
@@ -261,6 +265,34 @@ def dwf_norm2(g: int, field, parity: int = FULL, stream=None) -> float:
     r = ctypes.c_double()
     _check(load().dwf_norm2(g, _dev_ptr(field, g, parity), int(parity), ctypes.byref(r), _stream(stream, g)), "dwf_norm2")
     return r.value
+
+
+def _f16_ptr(t, g: int, parity: int) -> int:
+    """Address of a device field in fp16 storage (include/dwf.h): a float16 tensor with as many reals as the fp32 field."""
+    import torch
+    if not getattr(t, "is_cuda", False) or not t.is_contiguous() or t.dtype != torch.float16:
+        raise DwfError(ERR_INVALID_ARG, "binding", "fp16-stored fields must be contiguous float16 CUDA tensors")
+    if g in _geom_info:
+        prec, dev, _ = _geom_info[g]
+        if t.numel() * prec != dwf_field_bytes(g, parity) or t.device.index != dev:
+            raise DwfError(ERR_INVALID_ARG, "binding", "fp16-stored field does not match the geometry (size, parity or device)")
+    return t.data_ptr()
+
+
+def dwf_to_f16(g: int, field_f32, parity: int, field_f16, stream=None) -> None:
+    _check(load().dwf_to_f16(g, _dev_ptr(field_f32, g, parity), int(parity), _f16_ptr(field_f16, g, parity), _stream(stream, g)), "dwf_to_f16")
+
+
+def dwf_from_f16(g: int, field_f16, parity: int, field_f32, stream=None) -> None:
+    _check(load().dwf_from_f16(g, _f16_ptr(field_f16, g, parity), int(parity), _dev_ptr(field_f32, g, parity), _stream(stream, g)), "dwf_from_f16")
+
+
+def dwf_dhop_oe_f16(g: int, in_even_f16, out_odd_f16, stream=None) -> None:
+    _check(load().dwf_dhop_oe_f16(g, _f16_ptr(in_even_f16, g, EVEN), _f16_ptr(out_odd_f16, g, ODD), _stream(stream, g)), "dwf_dhop_oe_f16")
+
+
+def dwf_dhop_eo_f16(g: int, in_odd_f16, out_even_f16, stream=None) -> None:
+    _check(load().dwf_dhop_eo_f16(g, _f16_ptr(in_odd_f16, g, ODD), _f16_ptr(out_even_f16, g, EVEN), _stream(stream, g)), "dwf_dhop_eo_f16")
 
 
 NORM2_STATIC_MAX_BYTES = 1 << 31
@@ -475,6 +507,31 @@ class Geometry:
     def dhop_oe(self, in_even, out=None, stream=None):
         out = self.new_field(ODD) if out is None else out
         dwf_dhop_oe(self.handle, in_even, out, stream)
+        return out
+
+    # fp16 storage: float16 tensors in the fp32 device layout
+    def new_field_f16(self, parity: int = FULL):
+        n = dwf_field_bytes(self.handle, parity) // self.precision
+        return self._torch.empty(n, dtype=self._torch.float16, device=f"cuda:{self.device}")
+
+    def to_f16(self, field, parity: int, out=None, stream=None):
+        out = self.new_field_f16(parity) if out is None else out
+        dwf_to_f16(self.handle, field, parity, out, stream)
+        return out
+
+    def from_f16(self, field_f16, parity: int, out=None, stream=None):
+        out = self.new_field(parity) if out is None else out
+        dwf_from_f16(self.handle, field_f16, parity, out, stream)
+        return out
+
+    def dhop_oe_f16(self, in_even_f16, out=None, stream=None):
+        out = self.new_field_f16(ODD) if out is None else out
+        dwf_dhop_oe_f16(self.handle, in_even_f16, out, stream)
+        return out
+
+    def dhop_eo_f16(self, in_odd_f16, out=None, stream=None):
+        out = self.new_field_f16(EVEN) if out is None else out
+        dwf_dhop_eo_f16(self.handle, in_odd_f16, out, stream)
         return out
 
     def dhop_eo(self, in_odd, out=None, stream=None):

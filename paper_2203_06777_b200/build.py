@@ -30,7 +30,8 @@ SOURCES = [*[("dhop_staged64.cu", f"dhop_staged64_m{m}.o", [f"-DDWF_STAGED64_MOD
            ("dhop_staged.cu", "dhop_staged_m4.o", ["-DDWF_STAGED_MODE=4"]),
            ("dhop_staged.cu", "dhop_staged_m5.o", ["-DDWF_STAGED_MODE=5"]),
            ("dhop_staged.cu", "dhop_staged_m6.o", ["-DDWF_STAGED_MODE=6"]),
-           ("dwf5d.cu", "dwf5d.o", []), ("halo.cu", "halo.o", []), ("norm2_static.cu", "norm2_static.o", [])]
+           ("dhop_staged.cu", "dhop_staged_m7.o", ["-DDWF_STAGED_MODE=7"]),
+           ("dwf5d.cu", "dwf5d.o", []), ("halo.cu", "halo.o", []), ("norm2_static.cu", "norm2_static.o", []), ("half.cu", "half.o", [])]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden",

@@ -32,6 +32,7 @@
 // 128-bit vector, so every LDS / LDG / STG is 128 bits wide.
 // Shared-memory image of one slice: [row of the staged region][k/2][Lh][k&1],
 // regions in the order centre, x1-, x1+, x2-, x2+, x3-, x3+; inside a region x3 layer slowest.
+#include <cuda_fp16.h>
 #include <type_traits>
 #include <vector>
 
@@ -133,15 +134,24 @@ __device__ __forceinline__ float2 neg(float2 a) { return make_float2(-a.x, -a.y)
 // one leg: acc += reconstruct( U * project(psi) ), psi read from shared memory.
 // acc[4a + t]: t = 0 (re of out spins 0,1), 1 (im of 0,1), 2 (re of 2,3), 3 (im of 2,3), colour a:
 // exactly the slot order of the stored field, so the store needs no shuffling.
-template <int LH, int MU, bool FWD, bool FIRST>
-__device__ __forceinline__ void staged_leg(float2 (&acc)[12], const float4 *__restrict__ nb, const float2 *__restrict__ U)
+// HALF (fp16 storage): a slot pair is four halves (8 bytes); widened to fp32 right after the load, all
+// arithmetic in fp32 as in the fp32 kernel.
+template <int LH, int MU, bool FWD, bool FIRST, bool HALF = false>
+__device__ __forceinline__ void staged_leg(float2 (&acc)[12], const typename std::conditional<HALF, uint2, float4>::type *__restrict__ nb,
+                                           const float2 *__restrict__ U)
 {
     float2 q[12];
 #pragma unroll
-    for (int j = 0; j < 6; j++) {      // LDS.128: slots 2j and 2j+1 of the neighbour site
-        const float4 v = nb[j * LH];
-        q[2 * j] = make_float2(v.x, v.y);
-        q[2 * j + 1] = make_float2(v.z, v.w);
+    for (int j = 0; j < 6; j++) {      // LDS.128 (LDS.64): slots 2j and 2j+1 of the neighbour site
+        if constexpr (HALF) {
+            const uint2 v = nb[j * LH];
+            q[2 * j] = __half22float2(*reinterpret_cast<const __half2 *>(&v.x));
+            q[2 * j + 1] = __half22float2(*reinterpret_cast<const __half2 *>(&v.y));
+        } else {
+            const float4 v = nb[j * LH];
+            q[2 * j] = make_float2(v.x, v.y);
+            q[2 * j + 1] = make_float2(v.z, v.w);
+        }
     }
     // projection (1 -/+ gamma_mu) psi -> upper two spin components, table in SURVEY.md section 8(c)
     float2 P[3], Q[3];
@@ -223,9 +233,12 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
                    const __grid_constant__ CUtensorMap map_xc, const StagedArgs args)
 {
     using Cfg = StagedCfg<LH, B1, B2, B3>;
-    constexpr bool NORM = MODE == 1, DAG = MODE == 2 || MODE == 4, AXPY = MODE == 3 || MODE == 4, G12 = MODE == 5, FULL = MODE == 6;
+    constexpr bool NORM = MODE == 1, DAG = MODE == 2 || MODE == 4, AXPY = MODE == 3 || MODE == 4, G12 = MODE == 5, FULL = MODE == 6, HALF = MODE == 7;
+    // HALF: fields stored as fp16 (same slot order, 8 instead of 16 bytes per slot pair): rows, stages and the output vectors are half as long
+    constexpr int ROWB = HALF ? Cfg::ROWB / 2 : Cfg::ROWB;
+    using VecT = typename std::conditional<HALF, uint2, float4>::type;      // one slot pair of a site in a field
     // MODE 3 stages the rows box of the field x as well (read in the epilogue): NROW_C more rows per stage
-    constexpr int STAGE = Cfg::STAGE_BYTES + (AXPY ? Cfg::NROW_C * Cfg::ROWB : 0);
+    constexpr int STAGE = (HALF ? Cfg::STAGE_BYTES / 2 : Cfg::STAGE_BYTES) + (AXPY ? Cfg::NROW_C * Cfg::ROWB : 0);
     extern __shared__ __align__(1024) unsigned char smem[];
     const uint32_t smem_base = smem_u32(smem);
     const uint32_t full_base = smem_base + Cfg::NSTAGE * STAGE;      // full[stage][region]: TMA data has landed
@@ -299,43 +312,43 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             const uint32_t epar = ((g >> 1) - 1) & 1;
             // regions in the order the consumers release them (x3 faces, x2 faces, x1 faces, centre)
             if (g >= 2) mbar_wait(eb, epar);
-            mbar_arrive_expect_tx(fb, 2 * B1 * B2 * Cfg::ROWB);
-            tma_load_5d_hint(dst + Cfg::R_X3M * Cfg::ROWB, &map_x3, fb, 0, 0, b.o1, b.o2, b.c3m, pol[PC_X3M]);
-            tma_load_5d_hint(dst + Cfg::R_X3P * Cfg::ROWB, &map_x3, fb, 0, 0, b.o1, b.o2, b.c3p, pol[PC_X3P]);
+            mbar_arrive_expect_tx(fb, 2 * B1 * B2 * ROWB);
+            tma_load_5d_hint(dst + Cfg::R_X3M * ROWB, &map_x3, fb, 0, 0, b.o1, b.o2, b.c3m, pol[PC_X3M]);
+            tma_load_5d_hint(dst + Cfg::R_X3P * ROWB, &map_x3, fb, 0, 0, b.o1, b.o2, b.c3p, pol[PC_X3P]);
             if (g >= 2) mbar_wait(eb + 8, epar);
-            mbar_arrive_expect_tx(fb, 2 * B1 * B3 * Cfg::ROWB);
+            mbar_arrive_expect_tx(fb, 2 * B1 * B3 * ROWB);
             if (args.layered) {
 #pragma unroll
                 for (int j = 0; j < B3; j++) {
                     const uint64_t pf = pol[j == B3 - 1 ? PC_X12_TOP : PC_X12];
-                    tma_load_5d_hint(dst + (Cfg::R_X2M + j * B1) * Cfg::ROWB, &map_x2l, fb, 0, 0, b.o1, b.x2m, b.c4 + j, pf);
-                    tma_load_5d_hint(dst + (Cfg::R_X2P + j * B1) * Cfg::ROWB, &map_x2l, fb, 0, 0, b.o1, b.x2p, b.c4 + j, pf);
+                    tma_load_5d_hint(dst + (Cfg::R_X2M + j * B1) * ROWB, &map_x2l, fb, 0, 0, b.o1, b.x2m, b.c4 + j, pf);
+                    tma_load_5d_hint(dst + (Cfg::R_X2P + j * B1) * ROWB, &map_x2l, fb, 0, 0, b.o1, b.x2p, b.c4 + j, pf);
                 }
             } else {
-                tma_load_5d_hint(dst + Cfg::R_X2M * Cfg::ROWB, &map_x2, fb, 0, 0, b.o1, b.x2m, b.c4, pol[PC_X12]);
-                tma_load_5d_hint(dst + Cfg::R_X2P * Cfg::ROWB, &map_x2, fb, 0, 0, b.o1, b.x2p, b.c4, pol[PC_X12]);
+                tma_load_5d_hint(dst + Cfg::R_X2M * ROWB, &map_x2, fb, 0, 0, b.o1, b.x2m, b.c4, pol[PC_X12]);
+                tma_load_5d_hint(dst + Cfg::R_X2P * ROWB, &map_x2, fb, 0, 0, b.o1, b.x2p, b.c4, pol[PC_X12]);
             }
             if (g >= 2) mbar_wait(eb + 16, epar);
-            mbar_arrive_expect_tx(fb, 2 * B2 * B3 * Cfg::ROWB);
+            mbar_arrive_expect_tx(fb, 2 * B2 * B3 * ROWB);
             if (args.layered) {
 #pragma unroll
                 for (int j = 0; j < B3; j++) {
                     const uint64_t pf = pol[j == B3 - 1 ? PC_X12_TOP : PC_X12];
-                    tma_load_5d_hint(dst + (Cfg::R_X1M + j * B2) * Cfg::ROWB, &map_x1l, fb, 0, 0, b.x1m, b.o2, b.c4 + j, pf);
-                    tma_load_5d_hint(dst + (Cfg::R_X1P + j * B2) * Cfg::ROWB, &map_x1l, fb, 0, 0, b.x1p, b.o2, b.c4 + j, pf);
+                    tma_load_5d_hint(dst + (Cfg::R_X1M + j * B2) * ROWB, &map_x1l, fb, 0, 0, b.x1m, b.o2, b.c4 + j, pf);
+                    tma_load_5d_hint(dst + (Cfg::R_X1P + j * B2) * ROWB, &map_x1l, fb, 0, 0, b.x1p, b.o2, b.c4 + j, pf);
                 }
             } else {
-                tma_load_5d_hint(dst + Cfg::R_X1M * Cfg::ROWB, &map_x1, fb, 0, 0, b.x1m, b.o2, b.c4, pol[PC_X12]);
-                tma_load_5d_hint(dst + Cfg::R_X1P * Cfg::ROWB, &map_x1, fb, 0, 0, b.x1p, b.o2, b.c4, pol[PC_X12]);
+                tma_load_5d_hint(dst + Cfg::R_X1M * ROWB, &map_x1, fb, 0, 0, b.x1m, b.o2, b.c4, pol[PC_X12]);
+                tma_load_5d_hint(dst + Cfg::R_X1P * ROWB, &map_x1, fb, 0, 0, b.x1p, b.o2, b.c4, pol[PC_X12]);
             }
             if (g >= 2) mbar_wait(eb + 24, epar);
-            mbar_arrive_expect_tx(fb, (AXPY ? 2 : 1) * Cfg::NROW_C * Cfg::ROWB);
+            mbar_arrive_expect_tx(fb, (AXPY ? 2 : 1) * Cfg::NROW_C * ROWB);
             if constexpr (AXPY)         // rows box of x for this slice, behind the input rows of the stage
                 tma_load_5d_hint(dst + Cfg::STAGE_BYTES, &map_xc, fb, 0, 0, b.o1, b.o2, b.c4, pol[PC_X3M]);
             if (args.layered) {
 #pragma unroll
                 for (int j = 0; j < B3; j++)
-                    tma_load_5d_hint(dst + (j * B1 * B2) * Cfg::ROWB, &map_x3, fb, 0, 0, b.o1, b.o2, b.c4 + j,
+                    tma_load_5d_hint(dst + (j * B1 * B2) * ROWB, &map_x3, fb, 0, 0, b.o1, b.o2, b.c4 + j,
                                      pol[j == B3 - 1 ? PC_CENTRE_TOP : PC_CENTRE]);
             } else {
                 tma_load_5d_hint(dst, &map_c, fb, 0, 0, b.o1, b.o2, b.c4, pol[PC_CENTRE]);
@@ -365,7 +378,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     // Offsets of the 8 neighbour spinors inside a stage, in 16-byte units, two per register.  They
     // are made opaque to the compiler (empty asm) so that it keeps the four registers instead of
     // recomputing every offset from the thread index at the head of every leg.
-    constexpr uint32_t ROWV = Cfg::ROWB / 16;
+    constexpr uint32_t ROWV = Cfg::ROWB / 16;          // HALF: the same numbers in 8-byte units
     uint32_t offp[4];
     offp[1] = (r1p * ROWV + h) | ((r1m * ROWV + h) << 16);
     offp[2] = (r2p * ROWV + h) | ((r2m * ROWV + h) << 16);
@@ -385,9 +398,9 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
         if constexpr (FULL) return reinterpret_cast<const float4 *>(tile_origin(it).w ? args.gauge_odd : args.gauge);
         else return reinterpret_cast<const float4 *>(args.gauge);
     };
-    auto tile_out = [&](int it) -> float4 * {
-        if constexpr (FULL) return reinterpret_cast<float4 *>(args.out) + (tile_origin(it).w ? args.half_vecs : 0LL);
-        else return reinterpret_cast<float4 *>(args.out);
+    auto tile_out = [&](int it) -> VecT * {
+        if constexpr (FULL) return reinterpret_cast<VecT *>(args.out) + (tile_origin(it).w ? args.half_vecs : 0LL);
+        else return reinterpret_cast<VecT *>(args.out);
     };
     auto set_x0_offsets = [&](int r) {
         int hp = h + r;       if (hp == LH) hp = 0;
@@ -401,7 +414,7 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     int r_cur;
     long long grow = tile_row(0, r_cur);
     set_x0_offsets(r_cur);
-    float4 *optr = tile_out(0) + grow * (6 * LH) + h + (long long)s_first * slice_vecs;
+    VecT *optr = tile_out(0) + grow * (6 * LH) + h + (long long)s_first * slice_vecs;
     // G12: vector 3L + v of a site holds the complex numbers 2v, 2v+1 of rows 0, 1 of leg L (row-major), i.e. U[9L + 2v], U[9L + 2v + 1]
     constexpr int GV = G12 ? 24 : 36;                // 128-bit link vectors per site
     // row 2 of every link from rows 0, 1: r2 = sgn conj(r0 x r1); sgn = -1 for a time link whose hop wraps around an
@@ -447,13 +460,13 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
     // Leg order x3, x2, x1, x0: the face regions are handed back to the producer as soon as the
     // two legs reading them are done, so that their refill has almost two steps to land.
     double nsum = 0.0;          // NORM: this thread's share of |out|^2
-    auto step = [&](auto fetch_tag, int stage, uint32_t par, float4 *o, const float4 *gnext) {
+    auto step = [&](auto fetch_tag, int stage, uint32_t par, VecT *o, const float4 *gnext) {
         constexpr bool FETCH = decltype(fetch_tag)::value;
         const unsigned char *sb = smem + stage * STAGE;
         const uint32_t fb = full_base + 32 * stage, eb = empty_base + 32 * stage;
         float2 acc[12];
 #define DWF_LEG(L, MU, FWD, FIRST)                                                                  \
-        staged_leg<LH, MU, (FWD) != DAG, FIRST>(acc, reinterpret_cast<const float4 *>(sb) + (((L) & 1) ? offp[(L) >> 1] >> 16 : offp[(L) >> 1] & 0xffffu), U + 9 * (L)); \
+        staged_leg<LH, MU, (FWD) != DAG, FIRST, HALF>(acc, reinterpret_cast<const VecT *>(sb) + (((L) & 1) ? offp[(L) >> 1] >> 16 : offp[(L) >> 1] & 0xffffu), U + 9 * (L)); \
         if constexpr (FETCH && G12) {   /* rows 0, 1 of this leg; row 2 is rebuilt at the tile switch */ \
             _Pragma("unroll") for (int v = 0; v < 3; v++) {                                         \
                 const float4 q = ldg128_hint(gnext + (3 * (L) + v) * LH, pol_g);                    \
@@ -510,8 +523,14 @@ dhop_staged_kernel(const __grid_constant__ CUtensorMap map_c, const __grid_const
             for (int k = 0; k < 12; k++) nsum += (double)acc[k].x * acc[k].x + (double)acc[k].y * acc[k].y;
         }
 #pragma unroll
-        for (int j = 0; j < 6; j++)
-            stg128_hint(o + j * LH, make_float4(acc[2 * j].x, acc[2 * j].y, acc[2 * j + 1].x, acc[2 * j + 1].y), pol_o);
+        for (int j = 0; j < 6; j++) {
+            if constexpr (HALF) {       // round to nearest even, four halves per store
+                const __half2 lo = __floats2half2_rn(acc[2 * j].x, acc[2 * j].y), hi = __floats2half2_rn(acc[2 * j + 1].x, acc[2 * j + 1].y);
+                stg64_hint(o + j * LH, make_uint2(*reinterpret_cast<const uint32_t *>(&lo), *reinterpret_cast<const uint32_t *>(&hi)), pol_o);
+            } else {
+                stg128_hint(o + j * LH, make_float4(acc[2 * j].x, acc[2 * j].y, acc[2 * j + 1].x, acc[2 * j + 1].y), pol_o);
+            }
+        }
     };
 
     int g = 0;
@@ -575,6 +594,7 @@ const void *const *staged_kernels_mode3();
 const void *const *staged_kernels_mode4();
 const void *const *staged_kernels_mode5();
 const void *const *staged_kernels_mode6();
+const void *const *staged_kernels_mode7();
 
 #define DWF_CAT2(a, b) a##b
 #define DWF_CAT(a, b) DWF_CAT2(a, b)
@@ -593,8 +613,8 @@ const void *const *DWF_CAT(staged_kernels_mode, DWF_STAGED_MODE)()
 struct Variant {
     int lh, b1, b2, b3;
     int smem, threads, ctas_per_sm;
-    const void *fn[7];       // MODE 0 (Dhop), 1 (Dhop + norm2), 2 (Dhop^dagger), 3 (a x + b Dhop), 4 (a x + b Dhop^dagger), 5 (Dhop, 12-real links),
-                             // 6 (Dhop of a full field, both parities in one launch)
+    const void *fn[8];       // MODE 0 (Dhop), 1 (Dhop + norm2), 2 (Dhop^dagger), 3 (a x + b Dhop), 4 (a x + b Dhop^dagger), 5 (Dhop, 12-real links),
+                             // 6 (Dhop of a full field, both parities in one launch), 7 (Dhop on fp16-stored fields)
     int smem_axpy;           // MODEs 3, 4 stage the rows box of x as well
 };
 
@@ -604,10 +624,10 @@ static const std::vector<Variant> &variants()
         std::vector<Variant> t;
         const void *const *k0 = staged_kernels_mode0(), *const *k1 = staged_kernels_mode1(), *const *k2 = staged_kernels_mode2(),
                           *const *k3 = staged_kernels_mode3(), *const *k4 = staged_kernels_mode4(), *const *k5 = staged_kernels_mode5(),
-                          *const *k6 = staged_kernels_mode6();
+                          *const *k6 = staged_kernels_mode6(), *const *k7 = staged_kernels_mode7();
 #define X(LH, B1, B2, B3)                                                                            \
         t.push_back({LH, B1, B2, B3, StagedCfg<LH, B1, B2, B3>::SMEM_BYTES, StagedCfg<LH, B1, B2, B3>::NT,  \
-                     StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM, {k0[t.size()], k1[t.size()], k2[t.size()], k3[t.size()], k4[t.size()], k5[t.size()], k6[t.size()]},    \
+                     StagedCfg<LH, B1, B2, B3>::CTAS_PER_SM, {k0[t.size()], k1[t.size()], k2[t.size()], k3[t.size()], k4[t.size()], k5[t.size()], k6[t.size()], k7[t.size()]},    \
                      StagedCfg<LH, B1, B2, B3>::SMEM_BYTES + 2 * StagedCfg<LH, B1, B2, B3>::NROW_C * StagedCfg<LH, B1, B2, B3>::ROWB});
         DWF_STAGED_VARIANTS(X)
 #undef X
@@ -633,7 +653,7 @@ void plan_staged(dwf_geometry *g)
         g->staged.ntiles = (lat.L[1] / v[i].b1) * (lat.L[2] / v[i].b2) * (lat.L[3] / v[i].b3);
         // Opt in to the large dynamic shared memory here, on the geometry's device (the attribute is per
         // device; the caller holds a DeviceGuard), for every kernel MODE of the chosen tile shape.
-        for (int mode = 0; mode < 7; mode++) {
+        for (int mode = 0; mode < 8; mode++) {
             const int smem = (mode == 3 || mode == 4) ? v[i].smem_axpy : v[i].smem;
             if (smem > SMEM_LIMIT) continue;
             if (cudaFuncSetAttribute(v[i].fn[mode], cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess) {
@@ -677,16 +697,16 @@ void build_staged_tile_table(const dwf_geometry *g, int raster, int4 *tab)
 
 // tensor map of a half field complex[s][x3][x2][x1][k/2][h][k&1] seen as 5-D fp32 tensor
 // (4*Lh, 6, L1, L2, L3*Ls): x3 and s share the slowest dimension (the s stride is L3 x3-strides)
-static int encode_map(CUtensorMap *m, const void *base, const Lattice &lat, int Ls, int b1, int b2, int b3)
+static int encode_map(CUtensorMap *m, const void *base, const Lattice &lat, int Ls, int b1, int b2, int b3, bool half = false)
 {
     PFN_tensorMapEncodeTiled enc = get_tensor_map_encoder();
     const cuuint64_t dims[5] = {(cuuint64_t)4 * lat.Lh, 6, (cuuint64_t)lat.L[1], (cuuint64_t)lat.L[2],
                                 (cuuint64_t)lat.L[3] * Ls};
-    const cuuint64_t krow = (cuuint64_t)lat.Lh * 16, row = 6 * krow;
+    const cuuint64_t krow = (cuuint64_t)lat.Lh * (half ? 8 : 16), row = 6 * krow;
     const cuuint64_t strides[4] = {krow, row, row * lat.L[1], row * lat.L[1] * lat.L[2]};
     const cuuint32_t box[5] = {(cuuint32_t)4 * lat.Lh, 6, (cuuint32_t)b1, (cuuint32_t)b2, (cuuint32_t)b3};
     const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
-    CUresult rc = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, const_cast<void *>(base), dims, strides, box, estr,
+    CUresult rc = enc(m, half ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, const_cast<void *>(base), dims, strides, box, estr,
                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (rc != CUDA_SUCCESS) {
@@ -699,27 +719,32 @@ static int encode_map(CUtensorMap *m, const void *base, const Lattice &lat, int 
 // The six tensor maps of a field depend on its pointer and the tile shape only.  A solver applies the
 // operator to the same few buffers over and over, so the encoded maps are kept in a small
 // per-thread cache (keyed by geometry id, variant, pointer and slice count): no driver calls on a hit.
-struct MapSet { unsigned long long gid; int variant, ls; const void *ptr; CUtensorMap m[6]; };
+struct MapSet { unsigned long long gid; int variant, ls, half; const void *ptr; CUtensorMap m[6]; };
 
-static int get_maps(const dwf_geometry *g, const Variant &v, const void *ptr, int ls, MapSet **out)
+static int get_maps(const dwf_geometry *g, const Variant &v, const void *ptr, int ls, MapSet **out, bool half = false)
 {
     static thread_local MapSet cache[8];
     static thread_local unsigned next_slot = 0;
     for (MapSet &c : cache)
-        if (c.ptr == ptr && c.gid == g->uid && c.variant == g->staged.variant && c.ls == ls) { *out = &c; return DWF_OK; }
+        if (c.ptr == ptr && c.gid == g->uid && c.variant == g->staged.variant && c.ls == ls && c.half == (int)half) { *out = &c; return DWF_OK; }
     MapSet t;
-    t.gid = g->uid; t.variant = g->staged.variant; t.ptr = ptr; t.ls = ls;
+    t.gid = g->uid; t.variant = g->staged.variant; t.ptr = ptr; t.ls = ls; t.half = (int)half;
     int rc;
-    if ((rc = encode_map(&t.m[0], ptr, g->lat, ls, v.b1, v.b2, v.b3))) return rc;
-    if ((rc = encode_map(&t.m[1], ptr, g->lat, ls, 1, v.b2, v.b3))) return rc;
-    if ((rc = encode_map(&t.m[2], ptr, g->lat, ls, v.b1, 1, v.b3))) return rc;
-    if ((rc = encode_map(&t.m[3], ptr, g->lat, ls, v.b1, v.b2, 1))) return rc;
-    if ((rc = encode_map(&t.m[4], ptr, g->lat, ls, 1, v.b2, 1))) return rc;
-    if ((rc = encode_map(&t.m[5], ptr, g->lat, ls, v.b1, 1, 1))) return rc;
+    if ((rc = encode_map(&t.m[0], ptr, g->lat, ls, v.b1, v.b2, v.b3, half))) return rc;
+    if ((rc = encode_map(&t.m[1], ptr, g->lat, ls, 1, v.b2, v.b3, half))) return rc;
+    if ((rc = encode_map(&t.m[2], ptr, g->lat, ls, v.b1, 1, v.b3, half))) return rc;
+    if ((rc = encode_map(&t.m[3], ptr, g->lat, ls, v.b1, v.b2, 1, half))) return rc;
+    if ((rc = encode_map(&t.m[4], ptr, g->lat, ls, 1, v.b2, 1, half))) return rc;
+    if ((rc = encode_map(&t.m[5], ptr, g->lat, ls, v.b1, 1, 1, half))) return rc;
     MapSet *ms = &cache[next_slot++ % 8];
     *ms = t;
     *out = ms;
     return DWF_OK;
+}
+
+bool staged_supports_half(const dwf_geometry *g)
+{
+    return g->staged.variant >= 0 && (variants()[(size_t)g->staged.variant].lh * 48) % 128 == 0;
 }
 
 bool staged_supports_axpy(const dwf_geometry *g)
@@ -729,7 +754,7 @@ bool staged_supports_axpy(const dwf_geometry *g)
 
 int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st,
                        double *norm_partials, int *norm_blocks, bool dagger, const void *axpy_x, float axpy_a,
-                       float axpy_b, int nrhs, bool gauge12, bool full)
+                       float axpy_b, int nrhs, bool gauge12, bool full, bool half)
 {
     // nrhs > 1: `in`, `out` (and x) hold nrhs fields one after the other.  Dhop is diagonal
     // in s, so they are ONE field of nrhs * Ls slices to this kernel: the links of a tile stay in registers
@@ -744,14 +769,18 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
     // full (VERDICT r01 task 8): `in` / `out` are FULL fields (even half, then odd half), one launch whose
     // tile table lists every tile twice, once per output parity; the tensor maps cover both input halves (2 Ls slices)
     if (full && (norm_partials || dagger || axpy_x || gauge12 || nrhs != 1)) { set_error("full-field launch: plain Dhop only"); return DWF_ERR_UNSUPPORTED; }
-    const int mode = full ? 6 : gauge12 ? 5 : norm_partials ? 1 : (axpy_x ? (dagger ? 4 : 3) : (dagger ? 2 : 0));
+    // half: `in` / `out` are half fields stored as fp16 (device layout, 2 bytes per real); the rows must keep the
+    // TMA destinations 128-byte aligned (Lh a multiple of 8)
+    if (half && (norm_partials || dagger || axpy_x || gauge12 || full || nrhs != 1)) { set_error("fp16 storage: plain half-field Dhop only"); return DWF_ERR_UNSUPPORTED; }
+    if (half && (v.lh * 48) % 128 != 0) { set_error("fp16 storage needs L0 to be a multiple of 16 (rows of the staged tile 128-byte aligned)"); return DWF_ERR_UNSUPPORTED; }
+    const int mode = half ? 7 : full ? 6 : gauge12 ? 5 : norm_partials ? 1 : (axpy_x ? (dagger ? 4 : 3) : (dagger ? 2 : 0));
     const int smem = (mode == 3 || mode == 4) ? v.smem_axpy : v.smem;
     if (smem > SMEM_LIMIT) { set_error("tile too large for the fused axpy"); return DWF_ERR_UNSUPPORTED; }
     // The cache hands out pointers into its slots and the second lookup may evict the slot of the
     // first, so the maps are copied before it (they are passed to the kernel by value anyway).
     MapSet *ms = nullptr;
     int rc;
-    if ((rc = get_maps(g, v, in, full ? 2 * ls : ls, &ms))) return rc;
+    if ((rc = get_maps(g, v, in, full ? 2 * ls : ls, &ms, half))) return rc;
     CUtensorMap mc = ms->m[0], m1 = ms->m[1], m2 = ms->m[2], m3 = ms->m[3], m1l = ms->m[4], m2l = ms->m[5];
     CUtensorMap mxc = mc;
     if (axpy_x) {

@@ -180,9 +180,11 @@ int launch_dhop_staged(const dwf_geometry *g, const void *in, void *out, int par
                        double *norm_partials = nullptr, int *norm_blocks = nullptr, bool dagger = false,
                        const void *axpy_x = nullptr, float axpy_a = 0.f, float axpy_b = 0.f,     // axpy_x: out = a x + b Dhop in
                        int nrhs = 1,                                                            // nrhs fields one after the other
-                       bool gauge12 = false,
-                       bool full = false);                                                      // in / out are full fields: one launch for both parities                                                   // 12-real links (plain Dhop only)
+                       bool gauge12 = false,                                                    // 12-real links (plain Dhop only)
+                       bool full = false,                                                       // in / out are full fields: one launch for both parities
+                       bool half = false);                                                      // in / out are fp16-stored half fields
 bool staged_supports_axpy(const dwf_geometry *g);
+bool staged_supports_half(const dwf_geometry *g);       // a staged variant whose fp16 rows stay 128-byte aligned
 // pack.cu: out = a x + b out, elementwise over nreal reals (the unfused path of dwf_dhop_*_axpy)
 int launch_axpby(const dwf_geometry *g, const void *x, void *out, double a, double b, size_t nreal, cudaStream_t st);
 // dhop_staged64.cu (TMA-staged fp64 kernel, links split by colour column over three threads)

@@ -116,6 +116,11 @@ __device__ __forceinline__ void stg128_hint(float4 *p, float4 v, uint64_t policy
     asm volatile("st.global.L1::no_allocate.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p), "f"(v.x),
                  "f"(v.y), "f"(v.z), "f"(v.w), "l"(policy) : "memory");
 }
+__device__ __forceinline__ void stg64_hint(uint2 *p, uint2 v, uint64_t policy)
+{
+    asm volatile("st.global.L1::no_allocate.L2::cache_hint.v2.b32 [%0], {%1, %2}, %3;" ::"l"(p), "r"(v.x), "r"(v.y),
+                 "l"(policy) : "memory");
+}
 __device__ __forceinline__ void stg_hint(float2 *p, float2 v, uint64_t policy)
 {
     asm volatile("st.global.L1::no_allocate.L2::cache_hint.v2.f32 [%0], {%1, %2}, %3;" ::"l"(p), "f"(v.x), "f"(v.y),
