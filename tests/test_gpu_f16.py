@@ -43,12 +43,14 @@ def test_conversion_is_round_to_nearest_even_and_exact_back(lib):
         assert np.array_equal(back, _quantise(psi))                         # numpy's round-to-nearest-even, through the layout permutation
 
 
-@pytest.mark.parametrize("dims,Ls,bc,max_ctas", [((32, 8, 8, 8), 3, 1, 0),     # <16,4,2,2>, the C4 tile
-                                                 ((32, 8, 8, 8), 2, 0, 3),     # many tiles per CTA: link refill, zigzag
-                                                 ((16, 8, 8, 8), 4, 1, 0),     # <8,4,4,2>
-                                                 ((48, 4, 6, 4), 2, 1, 0),     # Lh = 24
-                                                 ((64, 4, 4, 6), 2, 0, 0)])    # Lh = 32
-def test_dhop_f16_against_oracle(lib, dims, Ls, bc, max_ctas):
+@pytest.mark.parametrize("dims,Ls,bc,max_ctas,opts", [((32, 8, 8, 8), 3, 1, 0, {}),     # <16,4,2,2>, the C4 tile
+                                                      ((32, 8, 8, 8), 2, 0, 3, {}),     # many tiles per CTA: link refill, zigzag
+                                                      ((16, 8, 8, 8), 4, 1, 0, {}),     # <8,4,4,2>
+                                                      ((48, 4, 6, 4), 2, 1, 0, {}),     # Lh = 24
+                                                      ((64, 4, 4, 6), 2, 0, 0, {}),     # Lh = 32
+                                                      ((32, 8, 8, 8), 4, 1, 6, {"ssplit": 2}),
+                                                      ((32, 8, 8, 8), 1, 1, 2, {"layered": 0, "zigzag": 0})])
+def test_dhop_f16_against_oracle(lib, dims, Ls, bc, max_ctas, opts):
     import torch
     U = gen.gauge_random(dims, 402, prec=4)
     he = _quantise(gen.spinor_gaussian(gen.volume(dims) // 2, Ls, 402, prec=4))
@@ -57,6 +59,8 @@ def test_dhop_f16_against_oracle(lib, dims, Ls, bc, max_ctas):
         g.load_gauge(U)
         if max_ctas:
             g.set_option("max_ctas", max_ctas)
+        for k, v in opts.items():
+            g.set_option(k, v)
         fe = g.to_f16(g.import_spinor(he, lib.EVEN), lib.EVEN)
         fo = g.to_f16(g.import_spinor(ho, lib.ODD), lib.ODD)
         out_o = g.dhop_oe_f16(fe)

@@ -438,9 +438,10 @@ def test_staged_many_tiles_per_cta(lib, prec, dims, Ls, bc, max_ctas):
             g.set_option("max_ctas", -1)
 
 
-@pytest.mark.parametrize("dims,Ls,bc,max_ctas", [((32, 8, 8, 8), 3, 1, 0), ((16, 8, 8, 8), 4, 0, 0), ((32, 8, 8, 8), 2, 1, 3),
-                                                 ((24, 8, 6, 8), 2, 1, 5), ((8, 8, 8, 8), 5, 1, 1)])
-def test_full_field_dhop_is_one_launch(lib, dims, Ls, bc, max_ctas):
+@pytest.mark.parametrize("dims,Ls,bc,max_ctas,opts", [((32, 8, 8, 8), 3, 1, 0, {}), ((16, 8, 8, 8), 4, 0, 0, {}), ((32, 8, 8, 8), 2, 1, 3, {}),
+                                                      ((24, 8, 6, 8), 2, 1, 5, {}), ((8, 8, 8, 8), 5, 1, 1, {}),
+                                                      ((32, 8, 8, 8), 4, 1, 6, {"ssplit": 2}), ((32, 8, 8, 8), 3, 0, 0, {"zigzag": 0, "layered": 0})])
+def test_full_field_dhop_is_one_launch(lib, dims, Ls, bc, max_ctas, opts):
     """dwf_dhop on an fp32 geometry with a staged variant: ONE launch whose tile table spans both parities (VERDICT r01
     task 8).  Against the oracle on every element, bit-identical to the two half-field launches (option full_launch = 0),
     also when few CTAs walk tiles of both parities one after the other (max_ctas: the tile switch changes the link set,
@@ -453,6 +454,8 @@ def test_full_field_dhop_is_one_launch(lib, dims, Ls, bc, max_ctas):
         g.set_option("kernel", 2)
         if max_ctas:
             g.set_option("max_ctas", max_ctas)
+        for k, v in opts.items():
+            g.set_option(k, v)
         fin = g.import_spinor(psi, lib.FULL)
         n0 = lib.dwf_launch_count()
         out = g.dhop(fin).clone()
