@@ -264,11 +264,11 @@ def test_c4_stress_many_launches_bit_identical(lib, prec):
         f_e = g.import_spinor(psi_e, lib.EVEN)
         ref = g.dhop_oe(f_e).clone()
         out = g.new_field(lib.ODD)
-        variations = [{}, {"ssplit": 2}, {"zigzag": 0}, {"ssplit": 4, "zigzag": 0}, {"raster_staged": 0}] if prec == 4 else [{}, {"raster_staged": 0}]
+        variations = [{}, {"ssplit": 2}, {"zigzag": 0}, {"ssplit": 4, "zigzag": 0}, {"raster_staged": 0}] if prec == 4 else [{}, {"raster_staged": 0}, {"zigzag": 0}, {"max_ctas": 101}]
         n = 0
-        for rep in range(45 if prec == 4 else 100):
+        for rep in range(45 if prec == 4 else 60):
             for opts in variations:
-                for k, v in {"ssplit": 1, "zigzag": 1, "raster_staged": -1, **opts}.items():
+                for k, v in {"ssplit": 1, "zigzag": 1, "raster_staged": -1, "max_ctas": 0, **opts}.items():
                     g.set_option(k, v)
                 out.zero_()
                 g.dhop_oe(f_e, out)
