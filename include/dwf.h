@@ -205,6 +205,17 @@ DWF_API int dwf_norm2_static(const void *x_dev, size_t n_reals, int precision, i
 DWF_API int dwf_dhop_oe_norm2(const dwf_geometry *g, const void *in_even, void *out_odd, double *result_host, void *stream);
 DWF_API int dwf_dhop_eo_norm2(const dwf_geometry *g, const void *in_odd, void *out_even, double *result_host, void *stream);
 
+/* The same two calls WITHOUT the wait: the kernels are enqueued on `stream`, *ticket names the reduction, and the call
+ * returns at once; dwf_reduction_wait(g, ticket, &value, stream) later waits for that reduction (same `stream`) and
+ * returns its value -- so that a caller can enqueue the next step's kernels before it reads this step's norm and the GPU
+ * never idles on the host (`bench.py` does).  The library keeps the results of the last 8 reductions of a geometry
+ * (every dwf_norm2, dwf_inner_product, dwf_dhop_*_norm2[_async] and every reduction inside dwf_cg_schur counts): waiting
+ * for an older ticket is INVALID_ARG.  The serialisation rule of the geometry's scratch (above) applies unchanged: all of
+ * these calls on one geometry go to ONE stream, one host thread at a time. */
+DWF_API int dwf_dhop_oe_norm2_async(const dwf_geometry *g, const void *in_even, void *out_odd, unsigned long long *ticket, void *stream);
+DWF_API int dwf_dhop_eo_norm2_async(const dwf_geometry *g, const void *in_odd, void *out_even, unsigned long long *ticket, void *stream);
+DWF_API int dwf_reduction_wait(const dwf_geometry *g, unsigned long long ticket, double *result_host, void *stream);
+
 /* result_host[0..1] = (re, im) of sum conj(a) b.  Same rules as dwf_norm2. */
 DWF_API int dwf_inner_product(const dwf_geometry *g, const void *a, const void *b, int parity,
                       double result_host[2], void *stream);

@@ -30,6 +30,7 @@ SYMBOLS = (
     "dwf_error_string", "dwf_last_error",
     "dwf_dhop_oe_mrhs", "dwf_dhop_eo_mrhs", "dwf_host_wait", "dwf_face_bytes", "dwf_face_pack_t", "dwf_face_apply_t",
     "dwf_mooee", "dwf_mooee_inv", "dwf_ddwf", "dwf_schur_work_bytes", "dwf_schur", "dwf_axpby", "dwf_cg_work_bytes", "dwf_cg_schur",
+    "dwf_dhop_oe_norm2_async", "dwf_dhop_eo_norm2_async", "dwf_reduction_wait",
     "dwf_norm2_static", "dwf_to_f16", "dwf_from_f16", "dwf_dhop_oe_f16", "dwf_dhop_eo_f16",
 )
 
@@ -64,6 +65,9 @@ def load(build_if_missing: bool = True):
         f.argtypes = [vp, vp, vp, ci, ci, vp]
     lib.dwf_norm2.argtypes = [vp, vp, ci, ctypes.POINTER(ctypes.c_double), vp]
     lib.dwf_norm2_static.argtypes = [vp, ctypes.c_size_t, ci, ci, vp, vp]
+    for f in (lib.dwf_dhop_oe_norm2_async, lib.dwf_dhop_eo_norm2_async):
+        f.argtypes = [vp, vp, vp, ctypes.POINTER(ctypes.c_ulonglong), vp]
+    lib.dwf_reduction_wait.argtypes = [vp, ctypes.c_ulonglong, ctypes.POINTER(ctypes.c_double), vp]
     for f in (lib.dwf_to_f16, lib.dwf_from_f16):
         f.argtypes = [vp, vp, ci, vp, vp]
     for f in (lib.dwf_dhop_oe_f16, lib.dwf_dhop_eo_f16):
@@ -264,6 +268,27 @@ def dwf_dhop_eo_norm2(g: int, in_odd, out_even, stream=None) -> float:
 def dwf_norm2(g: int, field, parity: int = FULL, stream=None) -> float:
     r = ctypes.c_double()
     _check(load().dwf_norm2(g, _dev_ptr(field, g, parity), int(parity), ctypes.byref(r), _stream(stream, g)), "dwf_norm2")
+    return r.value
+
+
+def dwf_dhop_oe_norm2_async(g: int, in_even, out_odd, stream=None) -> int:
+    """Enqueues DhopOE + norm2 and returns the ticket of the reduction (dwf_reduction_wait collects the value)."""
+    t = ctypes.c_ulonglong()
+    _check(load().dwf_dhop_oe_norm2_async(g, _dev_ptr(in_even, g, EVEN), _dev_ptr(out_odd, g, ODD), ctypes.byref(t), _stream(stream, g)),
+           "dwf_dhop_oe_norm2_async")
+    return int(t.value)
+
+
+def dwf_dhop_eo_norm2_async(g: int, in_odd, out_even, stream=None) -> int:
+    t = ctypes.c_ulonglong()
+    _check(load().dwf_dhop_eo_norm2_async(g, _dev_ptr(in_odd, g, ODD), _dev_ptr(out_even, g, EVEN), ctypes.byref(t), _stream(stream, g)),
+           "dwf_dhop_eo_norm2_async")
+    return int(t.value)
+
+
+def dwf_reduction_wait(g: int, ticket: int, stream=None) -> float:
+    r = ctypes.c_double()
+    _check(load().dwf_reduction_wait(g, int(ticket), ctypes.byref(r), _stream(stream, g)), "dwf_reduction_wait")
     return r.value
 
 
@@ -508,6 +533,18 @@ class Geometry:
         out = self.new_field(ODD) if out is None else out
         dwf_dhop_oe(self.handle, in_even, out, stream)
         return out
+
+    def dhop_oe_norm2_async(self, in_even, out=None, stream=None):
+        """(out, ticket): enqueued, not waited for; reduction_wait(ticket) returns the norm2"""
+        out = self.new_field(ODD) if out is None else out
+        return out, dwf_dhop_oe_norm2_async(self.handle, in_even, out, stream)
+
+    def dhop_eo_norm2_async(self, in_odd, out=None, stream=None):
+        out = self.new_field(EVEN) if out is None else out
+        return out, dwf_dhop_eo_norm2_async(self.handle, in_odd, out, stream)
+
+    def reduction_wait(self, ticket: int, stream=None) -> float:
+        return dwf_reduction_wait(self.handle, ticket, stream)
 
     # fp16 storage (SURVEY.md 8(f4)): float16 tensors in the fp32 device layout
     def new_field_f16(self, parity: int = FULL):

@@ -344,9 +344,9 @@ int dwf_create_geometry(const int dims[4], int Ls, int precision, int bc_time, i
               cudaMalloc(&g->tlink_top[1], (size_t)dims[1] * dims[2] * (dims[0] / 2) * 18 * (size_t)precision) == cudaSuccess &&
               cudaMalloc(&g->partials, sizeof(double) * 2 * (size_t)g->reduce_blocks) == cudaSuccess &&
               cudaMalloc(&g->result_dev, sizeof(double) * 2) == cudaSuccess &&
-              cudaHostAlloc(&g->mailbox_host, sizeof(double) * 4, cudaHostAllocMapped) == cudaSuccess &&
+              cudaHostAlloc(&g->mailbox_host, sizeof(double) * 4 * MAILBOX_SLOTS, cudaHostAllocMapped) == cudaSuccess &&
               cudaHostGetDevicePointer(&g->mailbox_dev, g->mailbox_host, 0) == cudaSuccess;
-    if (ok) memset(g->mailbox_host, 0, sizeof(double) * 4);
+    if (ok) memset(g->mailbox_host, 0, sizeof(double) * 4 * MAILBOX_SLOTS);
     if (!ok || rebuild_tilings(g) != DWF_OK) {
         cudaGetLastError();
         if (ok == false) set_error("device allocation failed (gauge %zu bytes x 2)", g->gauge_bytes);
@@ -591,10 +591,15 @@ int dwf_dhop_eo_mrhs(const dwf_geometry *g, const void *in_odd, void *out_even, 
 // word instead of paying a device-to-host copy plus a stream synchronise; cudaStreamQuery is
 // consulted now and then so that a failed launch surfaces as an error instead of a hang.  When the
 // sequence number is visible every earlier operation of the stream has completed (in-order stream).
-int dwf::fetch_reduction(const dwf_geometry *g, cudaStream_t st, int n, double *out)
+int dwf::fetch_reduction(const dwf_geometry *g, cudaStream_t st, int n, double *out, unsigned long long ticket)
 {
-    const unsigned long long want = g->mailbox_seq;
-    volatile unsigned long long *seq = reinterpret_cast<volatile unsigned long long *>(g->mailbox_host + 2);
+    const unsigned long long want = ticket ? ticket : g->mailbox_seq;
+    if (want == 0 || want > g->mailbox_seq || g->mailbox_seq - want >= MAILBOX_SLOTS) {
+        set_error("reduction %llu is not pending (last issued %llu, at most %llu results are kept)", want, g->mailbox_seq, MAILBOX_SLOTS);
+        return DWF_ERR_INVALID_ARG;
+    }
+    const double *slot = g->mailbox_host + 4 * (want % MAILBOX_SLOTS);
+    volatile unsigned long long *seq = reinterpret_cast<volatile unsigned long long *>(const_cast<double *>(slot) + 2);
     for (unsigned long long spins = 1; *seq != want; spins++) {
         if ((spins & 0x3fff) == 0) {
             cudaError_t e = cudaStreamQuery(st);
@@ -610,7 +615,7 @@ int dwf::fetch_reduction(const dwf_geometry *g, cudaStream_t st, int n, double *
             return DWF_ERR_CUDA;
         }
     }
-    for (int i = 0; i < n; i++) out[i] = const_cast<const volatile double *>(g->mailbox_host)[i];
+    for (int i = 0; i < n; i++) out[i] = const_cast<const volatile double *>(slot)[i];
     return DWF_OK;
 }
 
@@ -619,9 +624,9 @@ extern "C" {
 // out = D in on half fields and *result_host = norm2(out): the reduction runs in the epilogue of the
 // Dhop kernel (staged path) or as a second pass over `out` (direct path)
 static int dhop_norm2_common(const dwf_geometry *g, const void *in, void *out, int parity_out, double *result_host,
-                             void *stream, const char *who)
+                             void *stream, const char *who, unsigned long long *ticket = nullptr)
 {
-    if (!g || !in || !out || !result_host) { set_error("%s: NULL argument", who); return DWF_ERR_INVALID_ARG; }
+    if (!g || !in || !out || (!result_host && !ticket)) { set_error("%s: NULL argument", who); return DWF_ERR_INVALID_ARG; }
     if (in == out) { set_error("%s: in-place application is not defined (in == out)", who); return DWF_ERR_INVALID_ARG; }
     if (!aligned16(in) || !aligned16(out)) { set_error("%s: field pointers must be 16-byte aligned", who); return DWF_ERR_INVALID_ARG; }
     if (!g->gauge_loaded) { set_error("%s: call dwf_load_gauge first", who); return DWF_ERR_NO_GAUGE; }
@@ -650,7 +655,23 @@ static int dhop_norm2_common(const dwf_geometry *g, const void *in, void *out, i
         rc = launch_norm2(g, out, dwf_field_bytes(g, parity_out) / (size_t)g->prec, st);
     }
     if (rc) return rc;
+    if (ticket) { *ticket = g->mailbox_seq; return DWF_OK; }       // asynchronous form: the caller collects the value later
     return fetch_reduction(g, st, 1, result_host);
+}
+
+int dwf_dhop_oe_norm2_async(const dwf_geometry *g, const void *in_even, void *out_odd, unsigned long long *ticket, void *stream)
+{
+    return dhop_norm2_common(g, in_even, out_odd, DWF_ODD, nullptr, stream, "dwf_dhop_oe_norm2_async", ticket);
+}
+int dwf_dhop_eo_norm2_async(const dwf_geometry *g, const void *in_odd, void *out_even, unsigned long long *ticket, void *stream)
+{
+    return dhop_norm2_common(g, in_odd, out_even, DWF_EVEN, nullptr, stream, "dwf_dhop_eo_norm2_async", ticket);
+}
+int dwf_reduction_wait(const dwf_geometry *g, unsigned long long ticket, double *result_host, void *stream)
+{
+    if (!g || !result_host || !ticket) { set_error("dwf_reduction_wait: bad argument"); return DWF_ERR_INVALID_ARG; }
+    DeviceGuard guard(g->device);
+    return fetch_reduction(g, static_cast<cudaStream_t>(stream), 1, result_host, ticket);
 }
 
 int dwf_dhop_oe_norm2(const dwf_geometry *g, const void *in_even, void *out_odd, double *result_host, void *stream)

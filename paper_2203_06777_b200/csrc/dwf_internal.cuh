@@ -92,7 +92,7 @@ struct dwf_geometry {
     // reductions
     double *partials;       // [2 * max_blocks]
     double *result_dev;     // [2]
-    double *mailbox_host;   // mapped pinned host memory: [0..1] values, [2] sequence number of the reduction that wrote them
+    double *mailbox_host;   // mapped pinned host memory, MAILBOX_SLOTS slots of four words: [0..1] values, [2] sequence number of the reduction that wrote them
     double *mailbox_dev;    // the same words as the device sees them
     unsigned long long mailbox_seq;   // last sequence number handed to a reduction
     int reduce_blocks;
@@ -138,6 +138,7 @@ namespace dwf {
 int rebuild_tilings(dwf_geometry *g);
 
 // api.cu helpers used by the other translation units
+constexpr unsigned long long MAILBOX_SLOTS = 8;
 struct DeviceGuard {
     int prev = -1;
     bool ok = true;
@@ -157,7 +158,7 @@ bool aligned16(const void *p);
 int half_dhop(const dwf_geometry *g, const void *in, void *out, int parity_out, cudaStream_t st, bool dagger = false,
               const void *axpy_x = nullptr, double a = 0.0, double b = 0.0, int nrhs = 1);
 // waits for the reduction last enqueued on st and returns its n values (through the mapped mailbox)
-int fetch_reduction(const dwf_geometry *g, cudaStream_t st, int n, double *out);
+int fetch_reduction(const dwf_geometry *g, cudaStream_t st, int n, double *out, unsigned long long seq = 0);     // seq 0: the reduction enqueued last
 
 // pack.cu
 int launch_pack_gauge(const dwf_geometry *g, const void *U_canonical_dev, cudaStream_t st);

@@ -104,6 +104,12 @@ static unsigned long long next_seq(const dwf_geometry *g)
 {
     return ++const_cast<dwf_geometry *>(g)->mailbox_seq;
 }
+// the mailbox is a ring of MAILBOX_SLOTS slots of four words: reduction number q writes slot q % MAILBOX_SLOTS, so that a
+// caller may leave up to MAILBOX_SLOTS - 1 results unread while it enqueues more work (dwf_dhop_*_norm2_async)
+static double *mailbox_slot(const dwf_geometry *g, unsigned long long seq)
+{
+    return g->mailbox_dev + 4 * (seq % MAILBOX_SLOTS);
+}
 
 int launch_norm2(const dwf_geometry *g, const void *field, size_t nreal, cudaStream_t st)
 {
@@ -112,7 +118,7 @@ int launch_norm2(const dwf_geometry *g, const void *field, size_t nreal, cudaStr
         norm2_partial_kernel<float><<<nb, 256, 0, st>>>(static_cast<const float *>(field), nreal, g->partials);
     else
         norm2_partial_kernel<double><<<nb, 256, 0, st>>>(static_cast<const double *>(field), nreal, g->partials);
-    final_sum_kernel<1><<<1, 256, 0, st>>>(g->partials, nb, g->result_dev, g->mailbox_dev, next_seq(g));
+    { const unsigned long long q = next_seq(g); final_sum_kernel<1><<<1, 256, 0, st>>>(g->partials, nb, g->result_dev, mailbox_slot(g, q), q); }
     count_launch(2);
     DWF_CUDA_CHECK(cudaGetLastError());
     return DWF_OK;
@@ -120,7 +126,7 @@ int launch_norm2(const dwf_geometry *g, const void *field, size_t nreal, cudaStr
 
 int launch_final_sum(const dwf_geometry *g, int nblocks, cudaStream_t st)
 {
-    final_sum_kernel<1><<<1, 256, 0, st>>>(g->partials, nblocks, g->result_dev, g->mailbox_dev, next_seq(g));
+    { const unsigned long long q = next_seq(g); final_sum_kernel<1><<<1, 256, 0, st>>>(g->partials, nblocks, g->result_dev, mailbox_slot(g, q), q); }
     count_launch();
     DWF_CUDA_CHECK(cudaGetLastError());
     return DWF_OK;
@@ -133,7 +139,7 @@ int launch_inner(const dwf_geometry *g, const void *a, const void *b, size_t nco
         inner_partial_kernel<float><<<nb, 256, 0, st>>>(static_cast<const float *>(a), static_cast<const float *>(b), ncomplex, g->partials);
     else
         inner_partial_kernel<double><<<nb, 256, 0, st>>>(static_cast<const double *>(a), static_cast<const double *>(b), ncomplex, g->partials);
-    final_sum_kernel<2><<<1, 256, 0, st>>>(g->partials, nb, g->result_dev, g->mailbox_dev, next_seq(g));
+    { const unsigned long long q = next_seq(g); final_sum_kernel<2><<<1, 256, 0, st>>>(g->partials, nb, g->result_dev, mailbox_slot(g, q), q); }
     count_launch(2);
     DWF_CUDA_CHECK(cudaGetLastError());
     return DWF_OK;

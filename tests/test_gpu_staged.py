@@ -468,3 +468,34 @@ def test_full_field_dhop_is_one_launch(lib, dims, Ls, bc, max_ctas, opts):
         assert torch.equal(two, out)
         g.set_option("full_launch", 1)
         assert torch.equal(g.dhop(fin), out)
+
+
+@pytest.mark.parametrize("prec,dims,Ls", [(4, (32, 8, 8, 8), 4), (8, (32, 8, 8, 8), 3), (4, (12, 6, 4, 6), 3)])
+def test_norm2_async_tickets(lib, prec, dims, Ls):
+    """dwf_dhop_*_norm2_async + dwf_reduction_wait: several steps enqueued before any value is read; every ticket returns the
+    value of its own step (the same bits as the waiting call), out of order as well; a ticket older than the ring of kept
+    results is refused."""
+    import torch
+    U = gen.gauge_random(dims, 97, prec=prec)
+    with lib.Geometry(dims, Ls, prec, 1) as g:
+        g.load_gauge(U)
+        fields = [g.import_spinor(gen.spinor_gaussian(gen.volume(dims) // 2, Ls, 100 + i, prec=prec), lib.EVEN) for i in range(5)]
+        want = [g.dhop_oe_norm2(f)[1] for f in fields]
+        ref_out = g.dhop_oe(fields[3]).clone()
+        outs, tickets = [], []
+        for f in fields:                                    # five steps in flight
+            o, t = g.dhop_oe_norm2_async(f)
+            outs.append(o)
+            tickets.append(t)
+        assert tickets == list(range(tickets[0], tickets[0] + 5))
+        for i in (4, 0, 2, 1, 3):
+            assert g.reduction_wait(tickets[i]) == want[i]
+        assert torch.equal(outs[3], ref_out)
+        assert g.norm2(fields[0], lib.EVEN) > 0.0           # the waiting calls still work in between
+        for f in fields * 2:
+            _, t_last = g.dhop_eo_norm2_async(g.dhop_oe(f))
+        with pytest.raises(lib.DwfError):
+            g.reduction_wait(tickets[0])                    # more than 8 reductions ago
+        with pytest.raises(lib.DwfError):
+            g.reduction_wait(t_last + 1)                    # never issued
+        assert g.reduction_wait(t_last) > 0.0
