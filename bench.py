@@ -8,7 +8,8 @@ Workload at N=1: BASELINE.json configs[3] ("C4"): 32^4 x Ls=16, complex fp32, ne
 (eps=0.2), Gaussian spinor on the even checkerboard.  One STEP = one red-black matvec as the
 config states it, plus the reduction of the hot path's last row:
     chi_o = DhopOE psi_e ;  phi_e = DhopEO chi_o ;  n = norm2(phi_e) -> host (8 bytes)
-(the last two through dwf_dhop_eo_norm2: the reduction runs in the epilogue of the DhopEO kernel)
+(the last two through dwf_dhop_eo_norm2_async: the reduction runs in the epilogue of the DhopEO kernel; the host reads the
+value of step k with dwf_reduction_wait while step k + 1 runs, all K values inside the timed region)
 `value` counts 2 x 1320 x (V4/2 x Ls) flop per step (the norm2 flops are not counted).
 Inputs are resident in HBM before the timed region; fields are far larger than L2 (805 MB per
 half field, 604 MB of links), so no L2 flush is needed between iterations.
