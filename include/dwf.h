@@ -74,10 +74,10 @@ enum { DWF_FULL = -1, DWF_EVEN = 0, DWF_ODD = 1 };   /* parity = (x0+x1+x2+x3) &
  * limited to 2^31 - 1 complex numbers, i.e. V4 * Ls * 12 < 2^31 -- C5 has 1.5e9 -- and V4 to 2^30 sites),
  * UNSUPPORTED (precision), CUDA / ALLOC.
  *
- * CONCURRENCY.  dwf_dhop, dwf_dhop_oe/eo, their _dag, _axpy and _mrhs forms, dwf_mooee, dwf_mooee_inv, dwf_ddwf,
- * dwf_schur and dwf_axpby only read the geometry: they may be called concurrently on different streams.
- * Calls that use the geometry's scratch -- dwf_norm2, dwf_inner_product, dwf_dhop_oe_norm2 / _eo_norm2,
- * dwf_cg_schur (reduction partials and the result mailbox), dwf_import_spinor / dwf_export_spinor with HOST
+ * CONCURRENCY.  dwf_dhop, dwf_dhop_oe/eo, their _dag, _axpy, _mrhs and _f16 forms, dwf_to_f16 / dwf_from_f16, dwf_mooee,
+ * dwf_mooee_inv, dwf_ddwf, dwf_schur and dwf_axpby only read the geometry: they may be called concurrently on different streams.
+ * Calls that use the geometry's scratch -- dwf_norm2, dwf_inner_product, dwf_dhop_oe_norm2 / _eo_norm2 and their _async
+ * forms, dwf_reduction_wait, dwf_cg_schur (reduction partials and the result mailbox), dwf_import_spinor / dwf_export_spinor with HOST
  * arrays and dwf_host_wait (the transfer ring) -- must be serialised by the caller per geometry (one at a
  * time; they may overlap with the read-only calls).  dwf_load_gauge, dwf_set_option and dwf_destroy_geometry
  * must not race with anything on the same geometry. */
