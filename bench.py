@@ -823,7 +823,7 @@ def run_gpu_f16(args, w):
             "clocks": clocks, "gpu_launches": int(launches), "kernels_ms": {"dhop_oe_f16": t_oe},
             "roofline": {"bound": "hbm", "kernel": g.kernel_info() + " (fp16 storage, DhopOE launches)", "achieved": achieved, "peak": peak,
                          "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src, "algorithmic_bytes_per_launch": mb,
-                         "traffic": None},
+                         "traffic": ncu_traffic(args.workload, g.kernel_info())[0]},
             "check": {"equals_fp32_path_rounded_once_bitwise": chk},
         }
         print(json.dumps(line), flush=True)
