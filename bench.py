@@ -1024,8 +1024,8 @@ def spawn_ranks(n: int, argv, check_devices: bool = True) -> int:
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)        # a burst of ~15 ms; the regime over seconds is roofline.frac_sustained
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="dwf", choices=["dwf", "reference"])
     ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
